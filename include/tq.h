@@ -1,0 +1,184 @@
+/*
+ * tq.h — C ABI of the B200-native TurboESM hot path (arxiv/paper_2603_26110).
+ *
+ * Two operations, defined by the paper and by BASELINE.json:north_star:
+ *
+ *  (a) KV quantize-and-pack  [PAPER.md:111-116 prefill pipeline steps 1,3,4; §3.3 Eq. 5; §3.4 Eq. 6;
+ *      §4.2 packing snippet PAPER.md:203-213]: per vector, RoPE (keys only, Eq. 1-2) -> rotate by the
+ *      per-(layer, head) orthogonal PI (Eq. 4) -> store the norm -> code every coordinate of the unit
+ *      vector against an 8-point Lloyd-Max LUT (separate K and V tables) -> pack at
+ *      3 bits per coordinate -> residual r = u - lut[code], store sign(S r) (1 bit per row of S) and |r|.
+ *  (b) fused decode attention  [PAPER.md:118-124 decode pipeline, Algorithm 1 PAPER.md:223-237]: rotate
+ *      the query once (q'' = PI_K RoPE(q), z = S q''), stream the packed cache, per cached token
+ *      logit = n * ( <q'', lut_K[codes]> + sqrt(pi/2)/m * |r| * <z, sigma> ) / sqrt(d), online softmax,
+ *      accumulate p * n_v * lut_V[codes_v]; out = PI_V^T (o / l).  No fp16 K or V tensor is ever formed.
+ *
+ * Conventions
+ *  - Every call returns a tq_status.  Argument validation is synchronous on the host; kernels are
+ *    launched asynchronously on the given CUDA stream; nothing here calls cudaDeviceSynchronize and
+ *    nothing here allocates or frees device memory: the caller owns every buffer.
+ *  - "HOST" / "DEVICE" beside a pointer says where it must live.  Device pointers must be 16-byte aligned.
+ *  - There is no CPU fallback: with no usable CUDA device every device entry point returns TQ_ERR_CUDA.
+ *  - Matrices are row-major.  y = PI x means y[i] = sum_k PI[i*d + k] * x[k].
+ *
+ * Canonical packed format (what the paper fixes; the oracle emits exactly this; PAPER.md:203-213,
+ * tightened to 3 bit/coordinate per BASELINE.json:north_star):
+ *   codes : per vector 3d/8 bytes; bit (3i + b) of the LSB-first bit stream = bit b of code_i
+ *           (each 8-code group = 3 bytes = the low 24 bits of the paper's INT32 container);
+ *   signs : per key vector m/8 bytes; bit j of the LSB-first stream = [ (S r)_j >= 0 ];
+ *   norm  : IEEE binary16 bits of |PI x'| (round-to-nearest-even, clamped to 65504);
+ *   rnorm : IEEE binary16 bits of |r| (keys only), r taken on the unit vector.
+ *
+ * Device cache format (opaque to callers; tq_cache_export_canonical / tq_cache_import_canonical convert):
+ *   tokens are grouped in tiles of TQ_TILE_TOKENS = 32 and every (layer, batch, head) owns one contiguous
+ *   stream of ceil(max_seq/32) tiles.  Inside a tile every per-token word string is stored "chunk-major"
+ *   ([16-byte chunk][token]) so that a warp with lane = token reads it with coalesced 128-bit loads:
+ *     K codes : P = d/2 six-bit fields (code_{2g} | code_{2g+1} << 3); the token in tile slot t stores pair
+ *               group g at field position (g - t) mod P  (the rotation makes the decode kernel's
+ *               shared-memory table reads bank-conflict free);
+ *     K signs : m/4 nibbles; nibble group n (coordinates 4n..4n+3, bit b = coordinate 4n+b) is stored at
+ *               nibble position (n - t) mod (m/4);
+ *     V codes : P six-bit fields, pair group g at position g (no rotation);
+ *     norms   : three 64-byte arrays of binary16: |k|, |r_k|, |v|.
+ *   Bytes per cached token-head: 62 (d = 64), 118 (d = 128) — the same as the canonical format.
+ */
+#ifndef TQ_H_
+#define TQ_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define TQ_TILE_TOKENS 32
+
+typedef enum {
+  TQ_OK = 0,
+  TQ_ERR_INVALID_ARG = 1, /* NULL / misaligned pointer, negative size, layer out of range, ...          */
+  TQ_ERR_UNSUPPORTED = 2, /* head_dim not in {64,128}, qjl_dim != head_dim, v_qjl != 0                    */
+  TQ_ERR_CAPACITY = 3,    /* host-visible: start_pos + n_tokens > max_seq; workspace / buffer too small   */
+  TQ_ERR_CUDA = 4         /* a CUDA runtime call or launch failed (or no device)                         */
+} tq_status;
+
+typedef enum { TQ_F16 = 0, TQ_F32 = 1 } tq_dtype;
+
+/* Plain data, caller-filled, passed by pointer, never retained. */
+typedef struct {
+  int32_t n_layers;    /* L                                                                             */
+  int32_t batch;       /* B                                                                             */
+  int32_t n_heads;     /* H                                                                             */
+  int32_t head_dim;    /* d: 64 or 128                                                                  */
+  int32_t qjl_dim;     /* m: must equal head_dim                                                        */
+  int32_t max_seq;     /* cache capacity in tokens per (layer, batch, head)                             */
+  float rope_base;     /* theta_g = rope_base^(-2g/d); 10000 in BASELINE.json:configs[0]                */
+  int32_t rope_layout; /* 0 = interleaved pairs (2g, 2g+1) [PAPER.md:102, Eq. 2]; 1 = half-split (g, g+d/2) */
+  int32_t v_qjl;       /* 0 = K-only residual sketch (reading D3); 1 is TQ_ERR_UNSUPPORTED     */
+} tq_shape;
+
+/* Calibration arrays.  HOST pointers for tq_calibrate_host, DEVICE pointers for every other call.     */
+typedef struct {
+  float *pi_k;    /* [L][H][d][d]  PI_K, orthogonal, y = PI x                                           */
+  float *pi_v;    /* [L][H][d][d]  PI_V                                                                 */
+  float *lut_k;   /* [L][H][8]     ascending Lloyd-Max centroids for unit-norm rotated keys             */
+  float *lut_v;   /* [L][H][8]     same for values                                                      */
+  float *S;       /* [m][d]        QJL sketch matrix, shared by all layers and heads                    */
+  float *rope_cs; /* [max_seq][d/2][2]  (cos, sin)(p * theta_g), evaluated in fp64 and rounded to fp32  */
+} tq_params;
+
+/* Packed cache: one caller-allocated DEVICE buffer of tq_cache_bytes() bytes, zero-filled by the caller
+ * before first use.  It holds a header (seq_len[L][B], append arrival counters, a sticky status word)
+ * followed by the token tiles.                                                                        */
+typedef struct {
+  void *data; /* DEVICE, 256-byte aligned */
+} tq_cache;
+
+/* ---- sizes (pure host arithmetic; return 0 on an invalid shape) ---------------------------------- */
+size_t tq_cache_bytes(const tq_shape *shape);
+size_t tq_cache_bytes_per_token_head(const tq_shape *shape); /* 62 or 118                               */
+/* Byte offset inside tq_cache.data of int32 seq_len[L][B] (tokens currently cached) and of the
+ * int32 sticky status word (0, or TQ_ERR_CAPACITY once an append was refused on the device).          */
+size_t tq_cache_seq_len_offset(const tq_shape *shape);
+size_t tq_cache_status_offset(const tq_shape *shape);
+/* Workspace for tq_decode_attn over n_layers_call layers: rotated queries, split-K partials, arrival
+ * counters.  Must be zero-filled once by the caller; every call leaves it reusable.                    */
+size_t tq_decode_workspace_bytes(const tq_shape *shape, int32_t n_layers_call);
+/* Canonical plane sizes in bytes for n_tokens tokens of every (layer?, batch, head) of ONE layer:
+ * plane 0 k_codes, 1 k_signs, 2 k_norm, 3 k_rnorm, 4 v_codes, 5 v_norm.                                */
+size_t tq_canonical_plane_bytes(const tq_shape *shape, int32_t plane, int32_t n_tokens);
+
+/* ---- host-side calibration (not hot) [PAPER.md:128-143 §3.2; 145-164 §3.3; north_star] ------------
+ * Fills out_host (all HOST arrays, caller-allocated with the sizes given in tq_params).
+ *  mode 0: PI = V^T from the SVD of the uncentred sample matrix X (n_samples x d) per (layer, head)
+ *          [PAPER.md:132-137]; LUTs by Lloyd-Max (1-D k-means) on the pooled coordinates of the
+ *          normalised rotated samples.
+ *  mode 1: PI = Q of the QR factorisation of a seeded Gaussian d x d matrix (columns sign-fixed so that
+ *          diag(R) > 0) [BASELINE.json:configs[0]]; LUTs = Lloyd-Max fixed point for N(0, 1/d) [configs[0]].
+ *          k_samples / v_samples may be NULL.
+ * S: seeded i.i.d. N(0,1).  rope_cs: fp64 evaluation rounded to fp32.
+ * k_samples: [L][H][n_samples][d] post-RoPE keys; v_samples: same shape, values.                        */
+int tq_calibrate_host(const tq_shape *shape, int32_t mode, const float *k_samples, const float *v_samples,
+                      int64_t n_samples, uint64_t seed, tq_params *out_host);
+
+/* ---- (a) quantize-and-pack, prefill form [PAPER.md:111-116; §3.3; §3.4; §4.2] ----------------------
+ * k, v: DEVICE, [B][H][n_tokens][d] contiguous, dtype dt, pre-RoPE keys and values of layer `layer`.
+ * Token i of the call is cached at index start_pos + i and its RoPE position is that index.
+ * Sets seq_len[layer][b] = start_pos + n_tokens for every b.  n_tokens == 0 only sets seq_len.
+ * TQ_ERR_CAPACITY if start_pos + n_tokens > max_seq.                                                    */
+int tq_quantize_pack(const tq_shape *shape, const tq_params *dev, tq_cache *cache, int32_t layer,
+                     const void *k, const void *v, tq_dtype dt, int32_t n_tokens, int32_t start_pos,
+                     void *cuda_stream);
+
+/* ---- (a) quantize-and-pack, per appended token [BASELINE.json:configs[2]] --------------------------
+ * k, v: DEVICE, [B][H][d].  For every b the token is cached at index seq_len[layer][b] (read on the
+ * device), RoPE position = that index; afterwards seq_len[layer][b] += 1 on the device.  A batch entry
+ * whose cache is full is left unchanged and the cache's sticky status word is set to TQ_ERR_CAPACITY.    */
+int tq_append(const tq_shape *shape, const tq_params *dev, tq_cache *cache, int32_t layer, const void *k,
+              const void *v, tq_dtype dt, void *cuda_stream);
+
+/* ---- (b) fused decode attention [PAPER.md:118-124; Algorithm 1, 223-237; north_star] ---------------
+ * Layers layer_begin .. layer_begin + n_layers_call - 1 in one call (1 for a real model).
+ * q: DEVICE [n_layers_call][B][H][d], pre-RoPE queries, dtype dt.  q_pos: DEVICE int32
+ * [n_layers_call][B] RoPE positions of the queries, or NULL for seq_len - 1 (the query is the newest
+ * cached token).  out: DEVICE [n_layers_call][B][H][d], dtype dt.  Attends, without a mask, to all
+ * seq_len[layer][b] cached tokens; an empty cache gives out = 0.  t_hint: upper bound on seq_len used
+ * only to size the split-K grid (0 = max_seq).  workspace: see tq_decode_workspace_bytes.               */
+int tq_decode_attn(const tq_shape *shape, const tq_params *dev, const tq_cache *cache, int32_t layer_begin,
+                   int32_t n_layers_call, const void *q, const int32_t *q_pos, tq_dtype dt, void *out,
+                   int32_t t_hint, void *workspace, size_t workspace_bytes, void *cuda_stream);
+
+/* ---- format conversion (tests, interchange; not hot) -----------------------------------------------
+ * Canonical planes are DEVICE arrays for ONE layer, index [b][h][t] with t < n_tokens:
+ * k_codes/v_codes 3d/8 bytes per entry, k_signs m/8 bytes, norms uint16.  Export reads tokens
+ * 0 .. n_tokens-1 of `layer`; import writes them and sets seq_len[layer][b] = n_tokens.                  */
+typedef struct {
+  uint8_t *k_codes, *k_signs;
+  uint16_t *k_norm, *k_rnorm;
+  uint8_t *v_codes;
+  uint16_t *v_norm;
+} tq_canonical;
+
+int tq_cache_export_canonical(const tq_shape *shape, const tq_cache *cache, int32_t layer, int32_t n_tokens,
+                              tq_canonical *out_dev, void *cuda_stream);
+int tq_cache_import_canonical(const tq_shape *shape, tq_cache *cache, int32_t layer, int32_t n_tokens,
+                              const tq_canonical *in_dev, void *cuda_stream);
+
+/* ---- host-buffer convenience (the end-to-end path bench.py times as "e2e") -------------------------
+ * One decode step for one layer with HOST q/k/v/out ([B][H][d], dtype dt): copies k, v, q to the device
+ * staging buffers, runs tq_append + tq_decode_attn, copies out back and synchronises the stream.
+ * staging: DEVICE buffer of tq_step_staging_bytes() bytes.                                              */
+size_t tq_step_staging_bytes(const tq_shape *shape, tq_dtype dt);
+int tq_decode_step_host(const tq_shape *shape, const tq_params *dev, tq_cache *cache, int32_t layer,
+                        const void *q_host, const void *k_host, const void *v_host, tq_dtype dt,
+                        void *out_host, int32_t t_hint, void *staging, void *workspace,
+                        size_t workspace_bytes, void *cuda_stream);
+
+const char *tq_status_string(int status);
+/* Number of kernels the library launched since load (bench.py's gpu_launches).                          */
+int64_t tq_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TQ_H_ */
