@@ -1,0 +1,303 @@
+// tq_api.cu — the extern "C" boundary declared in include/tq.h: host-side validation, size arithmetic,
+// launch configuration.  No torch types, no allocation, no hidden synchronisation (except the explicit
+// host-buffer convenience call tq_decode_step_host, which must synchronise to hand back host data).
+#include <atomic>
+#include <cstdlib>
+#include <cstring>
+
+#include "tq_common.cuh"
+
+namespace tq {
+
+static std::atomic<long long> g_launches{0};
+void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
+
+
+constexpr int kMaxSplits = 64;
+
+static int num_sms() {
+  static int cached = -1;
+  if (cached < 0) {
+    int dev = 0, n = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return -1;
+    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return -1;
+    cached = n;
+  }
+  return cached;
+}
+
+static int check_shape(const tq_shape* s, CacheGeom* g) {
+  if (!s) return TQ_ERR_INVALID_ARG;
+  if (s->n_layers <= 0 || s->batch <= 0 || s->n_heads <= 0 || s->max_seq <= 0 || !(s->rope_base > 0.f))
+    return TQ_ERR_INVALID_ARG;
+  if (s->rope_layout != 0 && s->rope_layout != 1) return TQ_ERR_INVALID_ARG;
+  if ((s->head_dim != 64 && s->head_dim != 128) || s->qjl_dim != s->head_dim || s->v_qjl != 0) return TQ_ERR_UNSUPPORTED;
+  if (!make_geom(s, g)) return TQ_ERR_INVALID_ARG;
+  return TQ_OK;
+}
+
+static bool aligned16(const void* p) { return p && ((uintptr_t)p & 15u) == 0; }
+
+static int check_params(const tq_params* p) {
+  if (!p) return TQ_ERR_INVALID_ARG;
+  if (!aligned16(p->pi_k) || !aligned16(p->pi_v) || !aligned16(p->lut_k) || !aligned16(p->lut_v) || !aligned16(p->S) ||
+      !aligned16(p->rope_cs))
+    return TQ_ERR_INVALID_ARG;
+  return TQ_OK;
+}
+
+struct WorkspaceGeom {
+  size_t off_counters, off_qrot, off_partials, total;
+};
+static WorkspaceGeom workspace_geom(const CacheGeom& g, int n_layers_call) {
+  WorkspaceGeom w;
+  size_t units = (size_t)n_layers_call * g.B * g.H;
+  w.off_counters = 0;
+  w.off_qrot = (units * 4 + 255) / 256 * 256;
+  w.off_partials = w.off_qrot + (units * 2 * g.D * 4 + 255) / 256 * 256;
+  w.total = w.off_partials + units * kMaxSplits * (size_t)(g.D + 2) * 4;
+  return w;
+}
+
+}  // namespace tq
+
+using namespace tq;
+
+extern "C" {
+
+size_t tq_cache_bytes(const tq_shape* shape) {
+  CacheGeom g;
+  return check_shape(shape, &g) == TQ_OK ? g.total_bytes : 0;
+}
+size_t tq_cache_bytes_per_token_head(const tq_shape* shape) {
+  CacheGeom g;
+  return check_shape(shape, &g) == TQ_OK ? g.tile_bytes / kTile : 0;
+}
+size_t tq_cache_seq_len_offset(const tq_shape* shape) {
+  CacheGeom g;
+  return check_shape(shape, &g) == TQ_OK ? g.off_seq_len : 0;
+}
+size_t tq_cache_status_offset(const tq_shape* shape) {
+  CacheGeom g;
+  return check_shape(shape, &g) == TQ_OK ? g.off_status : 0;
+}
+size_t tq_decode_workspace_bytes(const tq_shape* shape, int32_t n_layers_call) {
+  CacheGeom g;
+  if (check_shape(shape, &g) != TQ_OK || n_layers_call <= 0 || n_layers_call > g.L) return 0;
+  return workspace_geom(g, n_layers_call).total;
+}
+size_t tq_canonical_plane_bytes(const tq_shape* shape, int32_t plane, int32_t n_tokens) {
+  CacheGeom g;
+  if (check_shape(shape, &g) != TQ_OK || n_tokens < 0) return 0;
+  size_t e = (size_t)g.B * g.H * n_tokens;
+  switch (plane) {
+    case 0:
+    case 4:
+      return e * (3 * g.D / 8);
+    case 1:
+      return e * (g.D / 8);
+    case 2:
+    case 3:
+    case 5:
+      return e * 2;
+    default:
+      return 0;
+  }
+}
+
+int tq_quantize_pack(const tq_shape* shape, const tq_params* dev, tq_cache* cache, int32_t layer, const void* k,
+                     const void* v, tq_dtype dt, int32_t n_tokens, int32_t start_pos, void* cuda_stream) {
+  CacheGeom g;
+  int rc = check_shape(shape, &g);
+  if (rc != TQ_OK) return rc;
+  if ((rc = check_params(dev)) != TQ_OK) return rc;
+  if (!cache || !cache->data || ((uintptr_t)cache->data & 255u)) return TQ_ERR_INVALID_ARG;
+  if (layer < 0 || layer >= g.L || n_tokens < 0 || start_pos < 0) return TQ_ERR_INVALID_ARG;
+  if (dt != TQ_F16 && dt != TQ_F32) return TQ_ERR_INVALID_ARG;
+  if (n_tokens > 0 && (!aligned16(k) || !aligned16(v))) return TQ_ERR_INVALID_ARG;
+  if ((long long)start_pos + n_tokens > g.max_seq) return TQ_ERR_CAPACITY;
+  int sms = num_sms();
+  if (sms <= 0) return TQ_ERR_CUDA;
+  QuantArgs a;
+  a.cv = make_view(g, cache->data);
+  a.k = k;
+  a.v = v;
+  a.pi_k = dev->pi_k + (size_t)layer * g.H * g.D * g.D;
+  a.pi_v = dev->pi_v + (size_t)layer * g.H * g.D * g.D;
+  a.lut_k = dev->lut_k + (size_t)layer * g.H * 8;
+  a.lut_v = dev->lut_v + (size_t)layer * g.H * 8;
+  a.S = dev->S;
+  a.rope_cs = dev->rope_cs;
+  a.layer = layer;
+  a.n_tokens = n_tokens;
+  a.start_pos = start_pos;
+  a.rope_layout = shape->rope_layout;
+  a.tiles_per_cta = 1;
+  return launch_quantize_pack(a, g.D, dt, sms, (cudaStream_t)cuda_stream) == cudaSuccess ? TQ_OK : TQ_ERR_CUDA;
+}
+
+int tq_append(const tq_shape* shape, const tq_params* dev, tq_cache* cache, int32_t layer, const void* k, const void* v,
+              tq_dtype dt, void* cuda_stream) {
+  CacheGeom g;
+  int rc = check_shape(shape, &g);
+  if (rc != TQ_OK) return rc;
+  if ((rc = check_params(dev)) != TQ_OK) return rc;
+  if (!cache || !cache->data || ((uintptr_t)cache->data & 255u)) return TQ_ERR_INVALID_ARG;
+  if (layer < 0 || layer >= g.L || !aligned16(k) || !aligned16(v)) return TQ_ERR_INVALID_ARG;
+  if (dt != TQ_F16 && dt != TQ_F32) return TQ_ERR_INVALID_ARG;
+  if (num_sms() <= 0) return TQ_ERR_CUDA;
+  QuantArgs a;
+  a.cv = make_view(g, cache->data);
+  a.k = k;
+  a.v = v;
+  a.pi_k = dev->pi_k + (size_t)layer * g.H * g.D * g.D;
+  a.pi_v = dev->pi_v + (size_t)layer * g.H * g.D * g.D;
+  a.lut_k = dev->lut_k + (size_t)layer * g.H * 8;
+  a.lut_v = dev->lut_v + (size_t)layer * g.H * 8;
+  a.S = dev->S;
+  a.rope_cs = dev->rope_cs;
+  a.layer = layer;
+  a.n_tokens = 1;
+  a.start_pos = 0;
+  a.rope_layout = shape->rope_layout;
+  a.tiles_per_cta = 1;
+  return launch_append(a, g.D, dt, (cudaStream_t)cuda_stream) == cudaSuccess ? TQ_OK : TQ_ERR_CUDA;
+}
+
+int tq_decode_attn(const tq_shape* shape, const tq_params* dev, const tq_cache* cache, int32_t layer_begin,
+                   int32_t n_layers_call, const void* q, const int32_t* q_pos, tq_dtype dt, void* out, int32_t t_hint,
+                   void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  CacheGeom g;
+  int rc = check_shape(shape, &g);
+  if (rc != TQ_OK) return rc;
+  if ((rc = check_params(dev)) != TQ_OK) return rc;
+  if (!cache || !cache->data || ((uintptr_t)cache->data & 255u)) return TQ_ERR_INVALID_ARG;
+  if (layer_begin < 0 || n_layers_call <= 0 || layer_begin + n_layers_call > g.L) return TQ_ERR_INVALID_ARG;
+  if (!aligned16(q) || !aligned16(out) || !workspace || ((uintptr_t)workspace & 255u)) return TQ_ERR_INVALID_ARG;
+  if (dt != TQ_F16 && dt != TQ_F32) return TQ_ERR_INVALID_ARG;
+  if (t_hint < 0) return TQ_ERR_INVALID_ARG;
+  WorkspaceGeom w = workspace_geom(g, n_layers_call);
+  if (workspace_bytes < w.total) return TQ_ERR_CAPACITY;
+  int sms = num_sms();
+  if (sms <= 0) return TQ_ERR_CUDA;
+  int th = (t_hint == 0 || t_hint > g.max_seq) ? g.max_seq : t_hint;
+  int ntiles = (th + kTile - 1) / kTile;
+  long units = (long)n_layers_call * g.B * g.H;
+  // split-K: enough CTAs for ~3 waves of 4 resident CTAs per SM, at least 4 tiles (one per warp) per CTA
+  long target = 12L * sms;
+  long nsplit = (target + units - 1) / units;
+  long cap = ntiles / 4 > 0 ? ntiles / 4 : 1;
+  if (nsplit > cap) nsplit = cap;
+  if (nsplit > kMaxSplits) nsplit = kMaxSplits;
+  if (nsplit < 1) nsplit = 1;
+  if (const char* e = getenv("TQ_DECODE_NSPLIT")) {  // tuning knob for profiling runs
+    long v = atol(e);
+    if (v >= 1 && v <= kMaxSplits) nsplit = v;
+  }
+  DecodeArgs a;
+  a.cv = make_view(g, cache->data);
+  a.pi_k = dev->pi_k;
+  a.pi_v = dev->pi_v;
+  a.lut_k = dev->lut_k;
+  a.lut_v = dev->lut_v;
+  a.S = dev->S;
+  a.rope_cs = dev->rope_cs;
+  a.q = q;
+  a.out = out;
+  a.q_pos = q_pos;
+  unsigned char* ws = (unsigned char*)workspace;
+  a.counters = (int*)(ws + w.off_counters);
+  a.qrot = (float*)(ws + w.off_qrot);
+  a.partials = (float*)(ws + w.off_partials);
+  a.layer_begin = layer_begin;
+  a.n_layers_call = n_layers_call;
+  a.nsplit = (int)nsplit;
+  a.rope_layout = shape->rope_layout;
+  a.dt = (int)dt;
+  return launch_decode(a, g.D, (cudaStream_t)cuda_stream) == cudaSuccess ? TQ_OK : TQ_ERR_CUDA;
+}
+
+int tq_cache_export_canonical(const tq_shape* shape, const tq_cache* cache, int32_t layer, int32_t n_tokens,
+                              tq_canonical* out_dev, void* cuda_stream) {
+  CacheGeom g;
+  int rc = check_shape(shape, &g);
+  if (rc != TQ_OK) return rc;
+  if (!cache || !cache->data || !out_dev || layer < 0 || layer >= g.L || n_tokens < 0) return TQ_ERR_INVALID_ARG;
+  if (n_tokens > g.max_seq) return TQ_ERR_CAPACITY;
+  if (n_tokens > 0 && (!out_dev->k_codes || !out_dev->k_signs || !out_dev->k_norm || !out_dev->k_rnorm ||
+                       !out_dev->v_codes || !out_dev->v_norm))
+    return TQ_ERR_INVALID_ARG;
+  if (num_sms() <= 0) return TQ_ERR_CUDA;
+  return launch_export(g, make_view(g, cache->data), layer, n_tokens, *out_dev, (cudaStream_t)cuda_stream) == cudaSuccess
+             ? TQ_OK
+             : TQ_ERR_CUDA;
+}
+
+int tq_cache_import_canonical(const tq_shape* shape, tq_cache* cache, int32_t layer, int32_t n_tokens,
+                              const tq_canonical* in_dev, void* cuda_stream) {
+  CacheGeom g;
+  int rc = check_shape(shape, &g);
+  if (rc != TQ_OK) return rc;
+  if (!cache || !cache->data || !in_dev || layer < 0 || layer >= g.L || n_tokens < 0) return TQ_ERR_INVALID_ARG;
+  if (n_tokens > g.max_seq) return TQ_ERR_CAPACITY;
+  if (n_tokens > 0 && (!in_dev->k_codes || !in_dev->k_signs || !in_dev->k_norm || !in_dev->k_rnorm || !in_dev->v_codes ||
+                       !in_dev->v_norm))
+    return TQ_ERR_INVALID_ARG;
+  if (num_sms() <= 0) return TQ_ERR_CUDA;
+  return launch_import(g, make_view(g, cache->data), layer, n_tokens, *in_dev, (cudaStream_t)cuda_stream) == cudaSuccess
+             ? TQ_OK
+             : TQ_ERR_CUDA;
+}
+
+size_t tq_step_staging_bytes(const tq_shape* shape, tq_dtype dt) {
+  CacheGeom g;
+  if (check_shape(shape, &g) != TQ_OK) return 0;
+  size_t vec = ((size_t)g.B * g.H * g.D * (dt == TQ_F16 ? 2 : 4) + 255) / 256 * 256;
+  return 4 * vec;
+}
+
+int tq_decode_step_host(const tq_shape* shape, const tq_params* dev, tq_cache* cache, int32_t layer, const void* q_host,
+                        const void* k_host, const void* v_host, tq_dtype dt, void* out_host, int32_t t_hint,
+                        void* staging, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  CacheGeom g;
+  int rc = check_shape(shape, &g);
+  if (rc != TQ_OK) return rc;
+  if (!q_host || !k_host || !v_host || !out_host || !staging || ((uintptr_t)staging & 255u)) return TQ_ERR_INVALID_ARG;
+  if (dt != TQ_F16 && dt != TQ_F32) return TQ_ERR_INVALID_ARG;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  size_t bytes = (size_t)g.B * g.H * g.D * (dt == TQ_F16 ? 2 : 4);
+  size_t vec = (bytes + 255) / 256 * 256;
+  unsigned char* s = (unsigned char*)staging;
+  void *dq = s, *dk = s + vec, *dv = s + 2 * vec, *dout = s + 3 * vec;
+  if (cudaMemcpyAsync(dk, k_host, bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return TQ_ERR_CUDA;
+  if (cudaMemcpyAsync(dv, v_host, bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return TQ_ERR_CUDA;
+  if (cudaMemcpyAsync(dq, q_host, bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return TQ_ERR_CUDA;
+  if ((rc = tq_append(shape, dev, cache, layer, dk, dv, dt, cuda_stream)) != TQ_OK) return rc;
+  if ((rc = tq_decode_attn(shape, dev, cache, layer, 1, dq, nullptr, dt, dout, t_hint, workspace, workspace_bytes,
+                           cuda_stream)) != TQ_OK)
+    return rc;
+  if (cudaMemcpyAsync(out_host, dout, bytes, cudaMemcpyDeviceToHost, st) != cudaSuccess) return TQ_ERR_CUDA;
+  if (cudaStreamSynchronize(st) != cudaSuccess) return TQ_ERR_CUDA;
+  return TQ_OK;
+}
+
+const char* tq_status_string(int status) {
+  switch (status) {
+    case TQ_OK:
+      return "TQ_OK";
+    case TQ_ERR_INVALID_ARG:
+      return "TQ_ERR_INVALID_ARG";
+    case TQ_ERR_UNSUPPORTED:
+      return "TQ_ERR_UNSUPPORTED";
+    case TQ_ERR_CAPACITY:
+      return "TQ_ERR_CAPACITY";
+    case TQ_ERR_CUDA:
+      return "TQ_ERR_CUDA";
+    default:
+      return "TQ_ERR_UNKNOWN";
+  }
+}
+
+int64_t tq_launch_count(void) { return (int64_t)tq::g_launches.load(); }
+
+}  // extern "C"

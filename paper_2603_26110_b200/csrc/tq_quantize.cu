@@ -1,0 +1,438 @@
+// tq_quantize.cu — KV quantize-and-pack kernels (prefill tiles and single-token append), sm_100a.
+//
+// Per vector (PAPER.md:111-116 prefill steps 1,3,4; §3.3 Eq. 5; §3.4 Eq. 6 in the sign(S r) form of
+// BASELINE.json:north_star): RoPE (keys) -> y = PI x' -> n = |y|, u = y / n -> code_i = #{k: u_i > t_k}
+// -> r = u - lut[code], |r|, bits_j = [(S r)_j >= 0] -> device tile layout (include/tq.h).
+//
+// Prefill kernel: one CTA owns a run of 32-token tiles of one (batch, head).  PI_K, S and PI_V stay
+// resident in shared memory (transposed, [k][i]) for the whole run; each tile is a
+// (32 tokens x D) x (D x D) fp32 register-tiled GEMM (4 outputs x 4 tokens per thread) on the CUDA cores,
+// followed by warp-shuffle norm reductions and a conflict-free word assembly.  All arithmetic is fp32
+// with IEEE division and square root so that codes agree with the fp64 oracle except inside the 1e-5
+// band around a threshold.
+#include "tq_common.cuh"
+
+namespace tq {
+
+
+__device__ __forceinline__ int swz(int k) { return ((k >> 1) * 4) & 31; }
+
+// acc[ii][tk] += sum_k Mt[k][4 ti + ii] * xs[k][4 tt + tk]
+template <int D>
+__device__ __forceinline__ void gemm_tile(const float* __restrict__ Mt, const float* __restrict__ xs, int ti, int tt,
+                                          float (&acc)[4][4]) {
+#pragma unroll
+  for (int ii = 0; ii < 4; ++ii)
+#pragma unroll
+    for (int tk = 0; tk < 4; ++tk) acc[ii][tk] = 0.f;
+#pragma unroll 4
+  for (int k = 0; k < D; ++k) {
+    float4 m = *reinterpret_cast<const float4*>(Mt + k * D + 4 * ti);
+    float4 x = *reinterpret_cast<const float4*>(xs + k * kTile + ((4 * tt) ^ swz(k)));
+    const float mm[4] = {m.x, m.y, m.z, m.w};
+    const float xx[4] = {x.x, x.y, x.z, x.w};
+#pragma unroll
+    for (int ii = 0; ii < 4; ++ii)
+#pragma unroll
+      for (int tk = 0; tk < 4; ++tk) acc[ii][tk] = fmaf(mm[ii], xx[tk], acc[ii][tk]);
+  }
+}
+
+// sum over the D/4 "ti" lanes that share a token group (16 lanes for D = 64, 32 for D = 128)
+template <int D>
+__device__ __forceinline__ float ti_sum(float v) {
+#pragma unroll
+  for (int o = D / 8; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
+// transposed load of a row-major [i][k] matrix into shared [k][i]
+template <int D>
+__device__ __forceinline__ void load_matrix_t(float* Mt, const float* __restrict__ M, int tid, int nthreads) {
+  for (int idx = tid; idx < D * D; idx += nthreads) {
+    int i = idx % D, k = idx / D;
+    Mt[k * D + i] = M[i * D + k];
+  }
+}
+
+__device__ __forceinline__ int code_of(float u, const float (&thr)[7]) {
+  int c = 0;
+#pragma unroll
+  for (int q = 0; q < 7; ++q) c += (u > thr[q]) ? 1 : 0;
+  return c;
+}
+
+// Load one tile of 32 tokens into xs[k][tok] (swizzled), applying RoPE when kIsKey.
+template <int D, typename T, bool kIsKey>
+__device__ __forceinline__ void load_tile(float* xs, const T* __restrict__ src /* [n_tokens][D] of this (b,h) */,
+                                          const float* __restrict__ rope_cs, int tile, int start_pos, int n_tokens,
+                                          int rope_layout, int tid, int nthreads) {
+  constexpr int HP = D / 2;
+  for (int idx = tid; idx < kTile * HP; idx += nthreads) {
+    int g = idx % HP, slot = idx / HP;
+    int pos = tile * kTile + slot;
+    int i = pos - start_pos;
+    int a = rope_layout == 0 ? 2 * g : g;
+    int b = rope_layout == 0 ? 2 * g + 1 : g + HP;
+    float xa = 0.f, xb = 0.f;
+    if (i >= 0 && i < n_tokens) {
+      xa = load_as_float<T>(src + (size_t)i * D + a);
+      xb = load_as_float<T>(src + (size_t)i * D + b);
+      if (kIsKey) {
+        float2 cs = *reinterpret_cast<const float2*>(rope_cs + ((size_t)pos * HP + g) * 2);
+        float ya = xa * cs.x - xb * cs.y;
+        float yb = xa * cs.y + xb * cs.x;
+        xa = ya;
+        xb = yb;
+      }
+    }
+    xs[a * kTile + (slot ^ swz(a))] = xa;
+    xs[b * kTile + (slot ^ swz(b))] = xb;
+  }
+}
+
+template <int D, typename T>
+__global__ void __launch_bounds__(2 * D) quantize_pack_kernel(QuantArgs a) {
+  using Lo = Layout<D>;
+  constexpr int NT = 2 * D;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  float* Mk = reinterpret_cast<float*>(smem_raw);  // [D][D] PI_K^T
+  float* Ms = Mk + D * D;                           // S^T
+  float* Mv = Ms + D * D;                           // PI_V^T
+  float* xs = Mv + D * D;                           // [D][32]
+  unsigned char* cbK = reinterpret_cast<unsigned char*>(xs + D * kTile);  // [32][D] K codes
+  unsigned char* cbV = cbK + kTile * D;                                    // [32][D] V codes
+  unsigned char* bbK = cbV + kTile * D;                                    // [32][D] sign bits
+  float* lutK = reinterpret_cast<float*>(bbK + kTile * D);                 // [8]
+  float* lutV = lutK + 8;
+  unsigned short* nK = reinterpret_cast<unsigned short*>(lutV + 8);  // [32]
+  unsigned short* rK = nK + kTile;
+  unsigned short* nV = rK + kTile;
+
+  const int tid = threadIdx.x;
+  const int ti = tid % (D / 4), tt = tid / (D / 4);
+  const int bh = blockIdx.y;
+  const int b = bh / a.cv.H, h = bh % a.cv.H;
+  const int first_tile = a.start_pos / kTile;
+  const int last_tile = (a.start_pos + a.n_tokens - 1) / kTile;
+  const int tile0 = first_tile + blockIdx.x * a.tiles_per_cta;
+  if (tile0 > last_tile) return;
+  const int tile1 = min(last_tile, tile0 + a.tiles_per_cta - 1);
+
+  if (blockIdx.x == 0 && h == 0 && tid == 0) a.cv.seq_len[a.layer * a.cv.B + b] = a.start_pos + a.n_tokens;
+
+  load_matrix_t<D>(Mk, a.pi_k + (size_t)h * D * D, tid, NT);
+  load_matrix_t<D>(Ms, a.S, tid, NT);
+  load_matrix_t<D>(Mv, a.pi_v + (size_t)h * D * D, tid, NT);
+  if (tid < 8) lutK[tid] = a.lut_k[h * 8 + tid];
+  if (tid >= 32 && tid < 40) lutV[tid - 32] = a.lut_v[h * 8 + tid - 32];
+  __syncthreads();
+  float thrK[7], thrV[7];
+#pragma unroll
+  for (int q = 0; q < 7; ++q) {
+    thrK[q] = 0.5f * (lutK[q] + lutK[q + 1]);
+    thrV[q] = 0.5f * (lutV[q] + lutV[q + 1]);
+  }
+
+  const T* ksrc = reinterpret_cast<const T*>(a.k) + (size_t)bh * a.n_tokens * D;
+  const T* vsrc = reinterpret_cast<const T*>(a.v) + (size_t)bh * a.n_tokens * D;
+  const size_t unit = (size_t)a.layer * a.cv.B * a.cv.H + bh;
+  unsigned char* stream = a.cv.tiles + unit * a.cv.stream_bytes;
+
+  for (int tile = tile0; tile <= tile1; ++tile) {
+    float acc[4][4];
+    // ------------------------------------------------------------------ keys
+    load_tile<D, T, true>(xs, ksrc, a.rope_cs, tile, a.start_pos, a.n_tokens, a.rope_layout, tid, NT);
+    __syncthreads();
+    gemm_tile<D>(Mk, xs, ti, tt, acc);
+    __syncthreads();  // xs is about to be overwritten with the residuals
+#pragma unroll
+    for (int tk = 0; tk < 4; ++tk) {
+      float n2 = 0.f;
+#pragma unroll
+      for (int ii = 0; ii < 4; ++ii) n2 = fmaf(acc[ii][tk], acc[ii][tk], n2);
+      n2 = ti_sum<D>(n2);
+      float n = sqrtf(n2);
+      float g2 = 0.f;
+      const int slot = 4 * tt + tk;
+#pragma unroll
+      for (int ii = 0; ii < 4; ++ii) {
+        float u = n > 0.f ? acc[ii][tk] / n : 0.f;
+        int c = code_of(u, thrK);
+        float r = u - lutK[c];
+        g2 = fmaf(r, r, g2);
+        const int i = 4 * ti + ii;
+        cbK[slot * D + i] = (unsigned char)c;
+        xs[i * kTile + (slot ^ swz(i))] = r;
+      }
+      g2 = ti_sum<D>(g2);
+      if (ti == 0) {
+        nK[slot] = f32_to_f16_bits_clamped(n);
+        rK[slot] = f32_to_f16_bits_clamped(sqrtf(g2));
+      }
+    }
+    __syncthreads();
+    gemm_tile<D>(Ms, xs, ti, tt, acc);
+#pragma unroll
+    for (int tk = 0; tk < 4; ++tk)
+#pragma unroll
+      for (int ii = 0; ii < 4; ++ii) bbK[(4 * tt + tk) * D + 4 * ti + ii] = acc[ii][tk] >= 0.f ? 1 : 0;
+    __syncthreads();
+    // ------------------------------------------------------------------ values
+    load_tile<D, T, false>(xs, vsrc, a.rope_cs, tile, a.start_pos, a.n_tokens, a.rope_layout, tid, NT);
+    __syncthreads();
+    gemm_tile<D>(Mv, xs, ti, tt, acc);
+#pragma unroll
+    for (int tk = 0; tk < 4; ++tk) {
+      float n2 = 0.f;
+#pragma unroll
+      for (int ii = 0; ii < 4; ++ii) n2 = fmaf(acc[ii][tk], acc[ii][tk], n2);
+      n2 = ti_sum<D>(n2);
+      float n = sqrtf(n2);
+      const int slot = 4 * tt + tk;
+#pragma unroll
+      for (int ii = 0; ii < 4; ++ii) {
+        float u = n > 0.f ? acc[ii][tk] / n : 0.f;
+        cbV[slot * D + 4 * ti + ii] = (unsigned char)code_of(u, thrV);
+      }
+      if (ti == 0) nV[slot] = f32_to_f16_bits_clamped(n);
+    }
+    __syncthreads();
+    // ------------------------------------------------------------------ assemble and store the tile
+    unsigned char* tp = stream + (size_t)tile * Lo::kTileBytes;
+    // K and V code words: 32 slots x KCW words each
+    for (int idx = tid; idx < 2 * kTile * Lo::KCW; idx += NT) {
+      const int isV = idx / (kTile * Lo::KCW);
+      const int rem = idx % (kTile * Lo::KCW);
+      const int w = rem / kTile, slot = rem % kTile;  // lanes vary slot -> coalesced chunk-major stores
+      const int pos = tile * kTile + slot;
+      if (pos < a.start_pos || pos >= a.start_pos + a.n_tokens) continue;
+      const unsigned char* cb = (isV ? cbV : cbK) + slot * D;
+      unsigned long long word = 0;
+      const int k_lo = (32 * w) / 6, k_hi = (32 * w + 31) / 6;
+      for (int kf = k_lo; kf <= k_hi; ++kf) {
+        const int g = isV ? kf : (kf + slot) % Lo::P;
+        unsigned long long f = cb[2 * g] | ((unsigned)cb[2 * g + 1] << 3);
+        const int sh = 6 * kf - 32 * w;  // may be negative for the field straddling in from the previous word
+        word |= sh >= 0 ? (f << sh) : (f >> (-sh));
+      }
+      *reinterpret_cast<unsigned*>(tp + (isV ? Lo::kOffVC : Lo::kOffKC) + word_offset(Lo::KCW, w, slot)) =
+          (unsigned)word;
+    }
+    for (int idx = tid; idx < kTile * Lo::KSW; idx += NT) {
+      const int w = idx / kTile, slot = idx % kTile;
+      const int pos = tile * kTile + slot;
+      if (pos < a.start_pos || pos >= a.start_pos + a.n_tokens) continue;
+      const unsigned char* bb = bbK + slot * D;
+      unsigned word = 0;
+      for (int kn = 0; kn < 8; ++kn) {
+        const int n = (8 * w + kn + slot) % Lo::NG;
+        unsigned nib = bb[4 * n] | (bb[4 * n + 1] << 1) | (bb[4 * n + 2] << 2) | (bb[4 * n + 3] << 3);
+        word |= nib << (4 * kn);
+      }
+      *reinterpret_cast<unsigned*>(tp + Lo::kOffKS + word_offset(Lo::KSW, w, slot)) = word;
+    }
+    if (tid < kTile) {
+      const int pos = tile * kTile + tid;
+      if (pos >= a.start_pos && pos < a.start_pos + a.n_tokens) {
+        reinterpret_cast<unsigned short*>(tp + Lo::kOffKN)[tid] = nK[tid];
+        reinterpret_cast<unsigned short*>(tp + Lo::kOffKR)[tid] = rK[tid];
+        reinterpret_cast<unsigned short*>(tp + Lo::kOffVN)[tid] = nV[tid];
+      }
+    }
+    __syncthreads();
+  }
+}
+
+// ---- single-token append --------------------------------------------------------------------------------
+// One CTA (128 threads) per (batch, head).  Matrices are read straight from global/L2 (each row by one
+// warp, coalesced along k); the token lands at index seq_len[layer][b], which the last-arriving head of
+// batch entry b then increments (BASELINE.json:configs[2]).
+template <int D>
+__device__ __forceinline__ void matvec_rows(const float* __restrict__ M, const float* xsm, float* ysm, int warp,
+                                            int lane, int nwarps) {
+  for (int i = warp; i < D; i += nwarps) {
+    float p = 0.f;
+#pragma unroll
+    for (int k = lane; k < D; k += 32) p = fmaf(M[(size_t)i * D + k], xsm[k], p);
+    p = warp_sum(p);
+    if (lane == 0) ysm[i] = p;
+  }
+}
+
+__device__ __forceinline__ float block_sum_128(float v, float* red, int warp, int lane) {
+  v = warp_sum(v);
+  __syncthreads();
+  if (lane == 0) red[warp] = v;
+  __syncthreads();
+  return red[0] + red[1] + red[2] + red[3];
+}
+
+template <int D, typename T>
+__global__ void __launch_bounds__(128) append_kernel(QuantArgs a) {
+  using Lo = Layout<D>;
+  __shared__ float x[D], y[D], r[D], sr[D];
+  __shared__ unsigned char cK[D], cV[D], bK[D];
+  __shared__ float red[4];
+  __shared__ float lutK[8], lutV[8];
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int bh = blockIdx.x;
+  const int b = bh / a.cv.H, h = bh % a.cv.H;
+  const int lb = a.layer * a.cv.B + b;
+  const int pos = a.cv.seq_len[lb];
+  const bool full = pos >= a.cv.max_seq;
+  constexpr int HP = D / 2;
+  if (tid < 8) lutK[tid] = a.lut_k[h * 8 + tid];
+  if (tid >= 32 && tid < 40) lutV[tid - 32] = a.lut_v[h * 8 + tid - 32];
+  if (!full) {
+    const T* kp = reinterpret_cast<const T*>(a.k) + (size_t)bh * D;
+    const T* vp = reinterpret_cast<const T*>(a.v) + (size_t)bh * D;
+    // ---- key: RoPE, PI_K, norm, codes, residual, S, bits
+    for (int g = tid; g < HP; g += 128) {
+      int ia = a.rope_layout == 0 ? 2 * g : g, ib = a.rope_layout == 0 ? 2 * g + 1 : g + HP;
+      float xa = load_as_float<T>(kp + ia), xb = load_as_float<T>(kp + ib);
+      float2 cs = *reinterpret_cast<const float2*>(a.rope_cs + ((size_t)pos * HP + g) * 2);
+      x[ia] = xa * cs.x - xb * cs.y;
+      x[ib] = xa * cs.y + xb * cs.x;
+    }
+    __syncthreads();
+    matvec_rows<D>(a.pi_k + (size_t)h * D * D, x, y, warp, lane, 4);
+    __syncthreads();
+    float thr[7];
+#pragma unroll
+    for (int q = 0; q < 7; ++q) thr[q] = 0.5f * (lutK[q] + lutK[q + 1]);
+    float part = 0.f;
+    for (int i = tid; i < D; i += 128) part = fmaf(y[i], y[i], part);
+    float n = sqrtf(block_sum_128(part, red, warp, lane));
+    part = 0.f;
+    for (int i = tid; i < D; i += 128) {
+      float u = n > 0.f ? y[i] / n : 0.f;
+      int c = code_of(u, thr);
+      float rr = u - lutK[c];
+      cK[i] = (unsigned char)c;
+      r[i] = rr;
+      part = fmaf(rr, rr, part);
+    }
+    float gnorm = sqrtf(block_sum_128(part, red, warp, lane));
+    __syncthreads();
+    matvec_rows<D>(a.S, r, sr, warp, lane, 4);
+    __syncthreads();
+    for (int j = tid; j < D; j += 128) bK[j] = sr[j] >= 0.f ? 1 : 0;
+    // ---- value: PI_V, norm, codes
+    for (int i = tid; i < D; i += 128) x[i] = load_as_float<T>(vp + i);
+    __syncthreads();
+    matvec_rows<D>(a.pi_v + (size_t)h * D * D, x, y, warp, lane, 4);
+    __syncthreads();
+#pragma unroll
+    for (int q = 0; q < 7; ++q) thr[q] = 0.5f * (lutV[q] + lutV[q + 1]);
+    part = 0.f;
+    for (int i = tid; i < D; i += 128) part = fmaf(y[i], y[i], part);
+    float nv = sqrtf(block_sum_128(part, red, warp, lane));
+    for (int i = tid; i < D; i += 128) {
+      float u = nv > 0.f ? y[i] / nv : 0.f;
+      cV[i] = (unsigned char)code_of(u, thr);
+    }
+    __syncthreads();
+    // ---- assemble this token's words
+    const size_t unit = (size_t)a.layer * a.cv.B * a.cv.H + bh;
+    unsigned char* tp = a.cv.tiles + unit * a.cv.stream_bytes + (size_t)(pos / kTile) * Lo::kTileBytes;
+    const int slot = pos % kTile;
+    for (int idx = tid; idx < 2 * Lo::KCW; idx += 128) {
+      const int isV = idx / Lo::KCW, w = idx % Lo::KCW;
+      const unsigned char* cb = isV ? cV : cK;
+      unsigned long long word = 0;
+      const int k_lo = (32 * w) / 6, k_hi = (32 * w + 31) / 6;
+      for (int kf = k_lo; kf <= k_hi; ++kf) {
+        const int g = isV ? kf : (kf + slot) % Lo::P;
+        unsigned long long f = cb[2 * g] | ((unsigned)cb[2 * g + 1] << 3);
+        const int sh = 6 * kf - 32 * w;
+        word |= sh >= 0 ? (f << sh) : (f >> (-sh));
+      }
+      *reinterpret_cast<unsigned*>(tp + (isV ? Lo::kOffVC : Lo::kOffKC) + word_offset(Lo::KCW, w, slot)) =
+          (unsigned)word;
+    }
+    if (tid >= 64 && tid < 64 + Lo::KSW) {
+      const int w = tid - 64;
+      unsigned word = 0;
+      for (int kn = 0; kn < 8; ++kn) {
+        const int ng = (8 * w + kn + slot) % Lo::NG;
+        unsigned nib = bK[4 * ng] | (bK[4 * ng + 1] << 1) | (bK[4 * ng + 2] << 2) | (bK[4 * ng + 3] << 3);
+        word |= nib << (4 * kn);
+      }
+      *reinterpret_cast<unsigned*>(tp + Lo::kOffKS + word_offset(Lo::KSW, w, slot)) = word;
+    }
+    if (tid == 96) {
+      reinterpret_cast<unsigned short*>(tp + Lo::kOffKN)[slot] = f32_to_f16_bits_clamped(n);
+      reinterpret_cast<unsigned short*>(tp + Lo::kOffKR)[slot] = f32_to_f16_bits_clamped(gnorm);
+      reinterpret_cast<unsigned short*>(tp + Lo::kOffVN)[slot] = f32_to_f16_bits_clamped(nv);
+    }
+  }
+  // ---- arrival: the last head of batch entry b publishes the new length
+  __syncthreads();
+  if (tid == 0) {
+    __threadfence();
+    int old = atomicAdd(&a.cv.arrive[lb], 1);
+    if (old == a.cv.H - 1) {
+      a.cv.arrive[lb] = 0;
+      if (full)
+        atomicExch(a.cv.status, (int)TQ_ERR_CAPACITY);
+      else
+        a.cv.seq_len[lb] = pos + 1;
+      __threadfence();
+    }
+  }
+}
+
+__global__ void set_seq_len_kernel(CacheView cv, int layer, int value) {
+  int b = blockIdx.x * blockDim.x + threadIdx.x;
+  if (b < cv.B) cv.seq_len[layer * cv.B + b] = value;
+}
+
+// ---- launchers --------------------------------------------------------------------------------------------
+template <int D>
+static size_t quant_smem_bytes() {
+  return (size_t)(3 * D * D + D * kTile) * 4 + 3 * kTile * D + 16 * 4 + 3 * kTile * 2;
+}
+
+template <int D, typename T>
+static cudaError_t launch_quant_t(const QuantArgs& a, int num_sms, cudaStream_t st) {
+  const int first_tile = a.start_pos / kTile, last_tile = (a.start_pos + a.n_tokens - 1) / kTile;
+  const int ntiles = last_tile - first_tile + 1;
+  const int BH = a.cv.B * a.cv.H;
+  QuantArgs b = a;
+  long want = 4L * num_sms;  // aim for >= ~4 CTAs per SM worth of work items
+  int tpc = (int)(((long)ntiles * BH + want - 1) / want);
+  b.tiles_per_cta = tpc < 1 ? 1 : (tpc > 16 ? 16 : tpc);
+  dim3 grid((ntiles + b.tiles_per_cta - 1) / b.tiles_per_cta, BH);
+  size_t smem = quant_smem_bytes<D>();
+  cudaError_t e = cudaFuncSetAttribute(quantize_pack_kernel<D, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
+  quantize_pack_kernel<D, T><<<grid, 2 * D, smem, st>>>(b);
+  count_launch();
+  return cudaGetLastError();
+}
+
+cudaError_t launch_quantize_pack(const QuantArgs& a, int D, tq_dtype dt, int num_sms, cudaStream_t st) {
+  if (a.n_tokens == 0) {
+    set_seq_len_kernel<<<(a.cv.B + 127) / 128, 128, 0, st>>>(a.cv, a.layer, a.start_pos);
+    count_launch();
+    return cudaGetLastError();
+  }
+  if (D == 64) return dt == TQ_F16 ? launch_quant_t<64, __half>(a, num_sms, st) : launch_quant_t<64, float>(a, num_sms, st);
+  return dt == TQ_F16 ? launch_quant_t<128, __half>(a, num_sms, st) : launch_quant_t<128, float>(a, num_sms, st);
+}
+
+cudaError_t launch_append(const QuantArgs& a, int D, tq_dtype dt, cudaStream_t st) {
+  const int BH = a.cv.B * a.cv.H;
+  if (D == 64) {
+    if (dt == TQ_F16) append_kernel<64, __half><<<BH, 128, 0, st>>>(a);
+    else append_kernel<64, float><<<BH, 128, 0, st>>>(a);
+  } else {
+    if (dt == TQ_F16) append_kernel<128, __half><<<BH, 128, 0, st>>>(a);
+    else append_kernel<128, float><<<BH, 128, 0, st>>>(a);
+  }
+  count_launch();
+  return cudaGetLastError();
+}
+
+}  // namespace tq

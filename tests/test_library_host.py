@@ -1,0 +1,163 @@
+"""Host-side checks of the C-ABI library that need no GPU: it loads, exports every symbol include/tq.h
+declares, its size arithmetic matches the documented format, argument validation is synchronous, device
+entry points fail loudly (never fall back) without a device, and tq_calibrate_host meets the invariants
+the paper fixes (checked against the oracle / numpy, never bitwise — DESIGN.md D9)."""
+import ctypes as C
+import math
+import os
+import re
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def tq():
+    from paper_2603_26110_b200 import build
+
+    build.build()
+    from paper_2603_26110_b200 import binding
+
+    binding.lib()
+    return binding
+
+
+def test_exports_every_declared_symbol(tq):
+    hdr = open(os.path.join(ROOT, "include", "tq.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = sorted(set(re.findall(r"\b(tq_[a-z0-9_]+)\s*\(", hdr)))
+    assert len(declared) >= 14
+    for name in declared:
+        assert hasattr(tq.lib(), name), name
+    assert sorted(declared) == sorted(tq.EXPORTS)
+
+
+def test_no_torch_or_python_symbols_in_abi(tq):
+    import subprocess
+
+    out = subprocess.run(["nm", "-D", "--defined-only", tq.LIB_PATH], capture_output=True, text=True).stdout
+    names = [l.split()[-1] for l in out.splitlines() if " T " in l]
+    assert all(n in names for n in tq.EXPORTS)
+    assert not any("torch" in n.lower() or "Py" in n[:2] for n in names)
+
+
+def test_size_arithmetic(tq):
+    s = tq.make_shape(33, 1, 20, 64, 1024)
+    assert tq.tq_cache_bytes_per_token_head(s) == 62  # 24 + 8 + 2 + 2 (K) + 24 + 2 (V)
+    units, tiles = 33 * 20, 1024 // 32
+    assert tq.tq_cache_bytes(s) == 512 + units * tiles * 1984  # header (2*33*4 + 4 -> 512) + tiles
+    s128 = tq.make_shape(1, 8, 40, 128, 4096)
+    assert tq.tq_cache_bytes_per_token_head(s128) == 118
+    assert tq.tq_canonical_plane_bytes(s, 0, 10) == 20 * 10 * 24
+    assert tq.tq_canonical_plane_bytes(s, 1, 10) == 20 * 10 * 8
+    assert tq.tq_canonical_plane_bytes(s, 5, 10) == 20 * 10 * 2
+    assert tq.tq_decode_workspace_bytes(s, 33) > 0 and tq.tq_decode_workspace_bytes(s, 34) == 0
+    # capacity is rounded up to whole tiles
+    s2 = tq.make_shape(1, 1, 1, 64, 33)
+    assert tq.tq_cache_bytes(s2) == 256 + 2 * 1984
+    # invalid shapes give 0
+    assert tq.tq_cache_bytes(tq.make_shape(1, 1, 1, 96, 64)) == 0
+    assert tq.tq_cache_bytes(tq.make_shape(0, 1, 1, 64, 64)) == 0
+    assert tq.tq_cache_bytes(tq.make_shape(1, 1, 1, 64, 64, qjl_dim=32)) == 0
+    assert tq.tq_cache_bytes(tq.make_shape(1, 1, 1, 64, 64, v_qjl=1)) == 0
+
+
+def test_validation_is_synchronous_and_there_is_no_fallback(tq):
+    s = tq.make_shape(1, 1, 1, 64, 64)
+    L = tq.lib()
+    null = C.c_void_p(None)
+    p = tq.TqParams(*[C.c_void_p(0x1000)] * 6)
+    c = tq.TqCache(C.c_void_p(0x10000))
+    # NULL / misaligned / out-of-range arguments are rejected before anything touches the device
+    assert L.tq_quantize_pack(C.byref(s), None, C.byref(c), 0, null, null, 0, 1, 0, null) == tq.TQ_ERR_INVALID_ARG
+    assert L.tq_quantize_pack(C.byref(s), C.byref(p), C.byref(c), 3, C.c_void_p(0x2000), C.c_void_p(0x2000), 0, 1, 0, null) == tq.TQ_ERR_INVALID_ARG
+    assert L.tq_quantize_pack(C.byref(s), C.byref(p), C.byref(c), 0, C.c_void_p(0x2004), C.c_void_p(0x2000), 0, 1, 0, null) == tq.TQ_ERR_INVALID_ARG
+    assert L.tq_quantize_pack(C.byref(s), C.byref(p), C.byref(c), 0, C.c_void_p(0x2000), C.c_void_p(0x2000), 0, 60, 10, null) == tq.TQ_ERR_CAPACITY
+    bad = tq.make_shape(1, 1, 1, 80, 64)
+    assert L.tq_append(C.byref(bad), C.byref(p), C.byref(c), 0, C.c_void_p(0x2000), C.c_void_p(0x2000), 0, null) == tq.TQ_ERR_UNSUPPORTED
+    assert L.tq_decode_attn(C.byref(s), C.byref(p), C.byref(c), 0, 2, C.c_void_p(0x2000), null, 0, C.c_void_p(0x3000), 0,
+                            C.c_void_p(0x4000), C.c_size_t(1 << 30), null) == tq.TQ_ERR_INVALID_ARG
+    assert L.tq_decode_attn(C.byref(s), C.byref(p), C.byref(c), 0, 1, C.c_void_p(0x2000), null, 0, C.c_void_p(0x3000), 0,
+                            C.c_void_p(0x4000), C.c_size_t(16), null) == tq.TQ_ERR_CAPACITY
+    assert tq.status_string(3) == "TQ_ERR_CAPACITY" and tq.status_string(0) == "TQ_OK"
+    import torch
+
+    if not torch.cuda.is_available():
+        # valid arguments but no device: the call must fail loudly, not compute on the CPU
+        rc = L.tq_append(C.byref(s), C.byref(p), C.byref(c), 0, C.c_void_p(0x2000), C.c_void_p(0x2000), 0, null)
+        assert rc == tq.TQ_ERR_CUDA
+
+
+def test_missing_extension_fails_loudly(tq, monkeypatch):
+    monkeypatch.setattr(tq, "_lib", None)
+    monkeypatch.setattr(tq, "LIB_PATH", "/nonexistent/libtq.so")
+    with pytest.raises(RuntimeError, match="no CPU fallback"):
+        tq.lib()
+
+
+# ------------------------------------------------------------------------------- tq_calibrate_host
+def test_calibrate_mode1_qr_gaussian(tq, oracle):
+    s = tq.make_shape(2, 1, 3, 64, 128)
+    out = tq.tq_calibrate_host(s, 1, seed=7)
+    for name in ("pi_k", "pi_v"):
+        for l in range(2):
+            for h in range(3):
+                P = out[name][l, h].astype(np.float64)
+                assert np.abs(P.T @ P - np.eye(64)).max() < 1e-6  # north_star pin
+    assert not np.allclose(out["pi_k"][0, 0], out["pi_k"][0, 1]) and not np.allclose(out["pi_k"][0, 0], out["pi_v"][0, 0])
+    # LUT = Lloyd-Max fixed point for N(0, 1/64): compare with the oracle's (pinned to Max 1960)
+    c, _, _ = oracle.lloyd_max_gauss(1 / 8, 8)
+    assert np.allclose(out["lut_k"][1, 2], c, atol=1e-7) and np.array_equal(out["lut_k"], out["lut_v"])
+    # S ~ N(0,1) i.i.d.
+    S = out["S"]
+    assert abs(S.mean()) < 0.06 and abs(S.std() - 1) < 0.05 and abs(np.mean(S ** 4) - 3) < 0.5
+    # RoPE table = (cos, sin)(p * base^(-2g/d)) to fp32 rounding
+    p, g = 97, 5
+    th = 10000.0 ** (-2.0 * g / 64)
+    assert abs(out["rope_cs"][p, g, 0] - math.cos(p * th)) < 1e-7 and abs(out["rope_cs"][p, g, 1] - math.sin(p * th)) < 1e-7
+    # seeded: same seed same result, different seed different rotation
+    again = tq.tq_calibrate_host(s, 1, seed=7)
+    other = tq.tq_calibrate_host(s, 1, seed=8)
+    assert np.array_equal(again["pi_k"], out["pi_k"]) and not np.array_equal(other["pi_k"], out["pi_k"])
+    # d = 128
+    s128 = tq.make_shape(1, 1, 1, 128, 8)
+    o128 = tq.tq_calibrate_host(s128, 1, seed=1)
+    P = o128["pi_k"][0, 0].astype(np.float64)
+    assert np.abs(P.T @ P - np.eye(128)).max() < 1e-6
+    assert np.allclose(o128["lut_k"][0, 0], oracle.lloyd_max_gauss(1 / math.sqrt(128), 8)[0], atol=1e-7)
+
+
+def test_calibrate_mode0_svd_and_kmeans(tq, oracle):
+    rng = np.random.default_rng(3)
+    d, n = 64, 3000
+    s = tq.make_shape(1, 1, 2, d, 32)
+    # anisotropic keys with two outlier channels; values with a different spectrum
+    A = rng.standard_normal((2, d, d)) * np.linspace(3.0, 0.2, d)[None, None, :]
+    ks = np.einsum("hnd,hde->hne", rng.standard_normal((2, n, d)), A)[None].astype(np.float32)
+    vs = (rng.standard_normal((1, 2, n, d)) * np.linspace(0.5, 1.5, d)).astype(np.float32)
+    out = tq.tq_calibrate_host(s, 0, ks, vs, seed=1)
+    for h in range(2):
+        P = out["pi_k"][0, h].astype(np.float64)
+        assert np.abs(P @ P.T - np.eye(d)).max() < 1e-5
+        X = ks[0, h].astype(np.float64)
+        # PI = V^T: rows are right singular vectors, i.e. PI X^T X PI^T is diagonal with descending entries
+        G = P @ (X.T @ X) @ P.T
+        offdiag = G - np.diag(np.diag(G))
+        assert np.abs(offdiag).max() < 1e-4 * np.diag(G).max()
+        assert np.all(np.diff(np.diag(G)) <= 1e-6 * np.diag(G).max())
+        # same subspaces as the oracle's numpy SVD, up to sign
+        Vt = oracle.svd_rotation(X)
+        assert np.allclose(np.abs(np.sum(Vt[:8] * P[:8], axis=1)), 1.0, atol=1e-4)
+        # LUT: k-means fixed point on the pooled unit-norm rotated coordinates, ascending
+        Y = X @ P.T
+        U = (Y / np.linalg.norm(Y, axis=1, keepdims=True)).ravel()
+        lut = out["lut_k"][0, h].astype(np.float64)
+        assert np.all(np.diff(lut) > 0)
+        nearest = np.abs(U[:, None] - lut[None, :]).argmin(axis=1)
+        means = np.array([U[nearest == k].mean() for k in range(8)])
+        assert np.allclose(means, lut, atol=2e-4)
+        co, _ = oracle.lloyd_max_samples(U, 8, iters=300)
+        assert np.allclose(co, lut, atol=5e-3)
+    assert not np.allclose(out["lut_k"][0, 0], out["lut_v"][0, 0], atol=1e-3)  # dual LUTs differ
