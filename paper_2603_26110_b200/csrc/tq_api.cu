@@ -13,7 +13,8 @@ static std::atomic<long long> g_launches{0};
 void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
 
 
-constexpr int kMaxSplits = 64;
+constexpr int kMaxSplits = 64;        // = kMaxSegments in tq_decode.cu
+constexpr int kMaxPlanEntries = 1024;  // = kMaxPlanEntries in tq_decode.cu
 
 static int num_sms() {
   static int cached = -1;
@@ -180,41 +181,44 @@ int tq_decode_attn(const tq_shape* shape, const tq_params* dev, const tq_cache* 
   if (workspace_bytes < w.total) return TQ_ERR_CAPACITY;
   int sms = num_sms();
   if (sms <= 0) return TQ_ERR_CUDA;
-  int th = (t_hint == 0 || t_hint > g.max_seq) ? g.max_seq : t_hint;
-  int ntiles = (th + kTile - 1) / kTile;
-  long units = (long)n_layers_call * g.B * g.H;
-  // split-K: enough CTAs for ~3 waves of 4 resident CTAs per SM, at least 4 tiles (one per warp) per CTA
-  long target = 12L * sms;
-  long nsplit = (target + units - 1) / units;
-  long cap = ntiles / 4 > 0 ? ntiles / 4 : 1;
-  if (nsplit > cap) nsplit = cap;
-  if (nsplit > kMaxSplits) nsplit = kMaxSplits;
-  if (nsplit < 1) nsplit = 1;
-  if (const char* e = getenv("TQ_DECODE_NSPLIT")) {  // tuning knob for profiling runs
+  if (g.B > kMaxPlanEntries) return TQ_ERR_UNSUPPORTED;
+  const int th = (t_hint == 0 || t_hint > g.max_seq) ? g.max_seq : t_hint;
+  const int ntiles = (th + kTile - 1) / kTile;
+  // stream-K: one persistent CTA per resident slot; a unit may be cut into at most kMaxSplits segments
+  const int min_q = (ntiles + kMaxSplits - 3) / (kMaxSplits - 2);
+  int grid_override = 0;
+  if (const char* e = getenv("TQ_DECODE_NSPLIT")) {  // profiling / test knob: number of CTAs of the streaming kernel
     long v = atol(e);
-    if (v >= 1 && v <= kMaxSplits) nsplit = v;
+    if (v >= 1 && v <= 65535) grid_override = (int)v;
   }
-  DecodeArgs a;
-  a.cv = make_view(g, cache->data);
-  a.pi_k = dev->pi_k;
-  a.pi_v = dev->pi_v;
-  a.lut_k = dev->lut_k;
-  a.lut_v = dev->lut_v;
-  a.S = dev->S;
-  a.rope_cs = dev->rope_cs;
-  a.q = q;
-  a.out = out;
-  a.q_pos = q_pos;
+  const size_t esz = dt == TQ_F16 ? 2 : 4;
   unsigned char* ws = (unsigned char*)workspace;
-  a.counters = (int*)(ws + w.off_counters);
-  a.qrot = (float*)(ws + w.off_qrot);
-  a.partials = (float*)(ws + w.off_partials);
-  a.layer_begin = layer_begin;
-  a.n_layers_call = n_layers_call;
-  a.nsplit = (int)nsplit;
-  a.rope_layout = shape->rope_layout;
-  a.dt = (int)dt;
-  return launch_decode(a, g.D, (cudaStream_t)cuda_stream) == cudaSuccess ? TQ_OK : TQ_ERR_CUDA;
+  const int layers_per_launch = kMaxPlanEntries / g.B;
+  for (int l0 = 0; l0 < n_layers_call; l0 += layers_per_launch) {
+    const int nl = n_layers_call - l0 < layers_per_launch ? n_layers_call - l0 : layers_per_launch;
+    const size_t u0 = (size_t)l0 * g.B * g.H;  // first unit of this launch inside the call
+    DecodeArgs a;
+    a.cv = make_view(g, cache->data);
+    a.pi_k = dev->pi_k;
+    a.pi_v = dev->pi_v;
+    a.lut_k = dev->lut_k;
+    a.lut_v = dev->lut_v;
+    a.S = dev->S;
+    a.rope_cs = dev->rope_cs;
+    a.q = (const unsigned char*)q + u0 * g.D * esz;
+    a.out = (unsigned char*)out + u0 * g.D * esz;
+    a.q_pos = q_pos ? q_pos + (size_t)l0 * g.B : nullptr;
+    a.counters = (int*)(ws + w.off_counters) + u0;
+    a.qrot = (float*)(ws + w.off_qrot) + u0 * 2 * g.D;
+    a.partials = (float*)(ws + w.off_partials) + u0 * kMaxSplits * (g.D + 2);
+    a.layer_begin = layer_begin + l0;
+    a.n_layers_call = nl;
+    a.nsplit = grid_override;
+    a.rope_layout = shape->rope_layout;
+    a.dt = (int)dt;
+    if (launch_decode(a, g.D, sms, min_q, (cudaStream_t)cuda_stream) != cudaSuccess) return TQ_ERR_CUDA;
+  }
+  return TQ_OK;
 }
 
 int tq_cache_export_canonical(const tq_shape* shape, const tq_cache* cache, int32_t layer, int32_t n_tokens,

@@ -123,14 +123,14 @@ struct DecodeArgs {
   void* out;             // [Lc][B][H][D]
   const int32_t* q_pos;  // [Lc][B] or nullptr
   float* qrot;           // workspace [units_call][2 D]: q'' then z
-  float* partials;       // workspace [units_call][nsplit][D + 2]
+  float* partials;       // workspace [units_call][64][D + 2]
   int* counters;         // workspace [units_call]
-  int layer_begin, n_layers_call, nsplit, rope_layout, dt;
+  int layer_begin, n_layers_call, nsplit /* 0, or a CTA-count override */, rope_layout, dt;
 };
 
 cudaError_t launch_quantize_pack(const QuantArgs& a, int D, tq_dtype dt, int num_sms, cudaStream_t st);
 cudaError_t launch_append(const QuantArgs& a, int D, tq_dtype dt, cudaStream_t st);
-cudaError_t launch_decode(const DecodeArgs& a, int D, cudaStream_t st);
+cudaError_t launch_decode(const DecodeArgs& a, int D, int num_sms, int min_q, cudaStream_t st);
 cudaError_t launch_export(const CacheGeom& g, const CacheView& cv, int layer, int n_tokens, const tq_canonical& out,
                           cudaStream_t st);
 cudaError_t launch_import(const CacheGeom& g, const CacheView& cv, int layer, int n_tokens, const tq_canonical& in,
@@ -168,5 +168,42 @@ template <>
 __device__ __forceinline__ float load_as_float<__half>(const __half* p) {
   return __half2float(*p);
 }
+
+// y[i] = sum_k M[i][k] x[k] for the rows owned by this warp, all loads of a batch of RB rows issued before
+// the first reduction so that the L2 latency is paid once per batch, not once per row.
+template <int D, int NWARPS>
+__device__ __forceinline__ void matvec_rows_ilp(const float* __restrict__ M, const float* xsm, float* ysm, int warp,
+                                                int lane) {
+  constexpr int ROWS = D / NWARPS;  // rows per warp
+  constexpr int RB = ROWS < 8 ? ROWS : 8;
+  constexpr int KP = D / 32;  // elements per lane per row
+  float xr[KP];
+#pragma unroll
+  for (int j = 0; j < KP; ++j) xr[j] = xsm[lane + 32 * j];
+#pragma unroll
+  for (int r0 = 0; r0 < ROWS; r0 += RB) {
+    float m[RB][KP];
+#pragma unroll
+    for (int r = 0; r < RB; ++r)
+#pragma unroll
+      for (int j = 0; j < KP; ++j) m[r][j] = __ldg(M + (size_t)(warp * ROWS + r0 + r) * D + lane + 32 * j);
+    float p[RB];
+#pragma unroll
+    for (int r = 0; r < RB; ++r) {
+      p[r] = 0.f;
+#pragma unroll
+      for (int j = 0; j < KP; ++j) p[r] = fmaf(m[r][j], xr[j], p[r]);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1)
+#pragma unroll
+      for (int r = 0; r < RB; ++r) p[r] += __shfl_xor_sync(0xffffffffu, p[r], o);
+    if (lane == 0) {
+#pragma unroll
+      for (int r = 0; r < RB; ++r) ysm[warp * ROWS + r0 + r] = p[r];
+    }
+  }
+}
+
 
 }  // namespace tq

@@ -26,18 +26,27 @@ namespace tq {
 
 // ------------------------------------------------------------------------------------------ query prep
 template <int D, typename T>
-__global__ void __launch_bounds__(128) decode_prep_kernel(DecodeArgs a) {
+__global__ void __launch_bounds__(256) decode_prep_kernel(DecodeArgs a) {
   __shared__ float x[D], y[D];
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int uc = blockIdx.x;
   const int BH = a.cv.B * a.cv.H;
   const int lc = uc / BH, bh = uc % BH, b = bh / a.cv.H, h = bh % a.cv.H;
   const int layer = a.layer_begin + lc;
-  int pos = a.q_pos ? a.q_pos[lc * a.cv.B + b] : a.cv.seq_len[layer * a.cv.B + b] - 1;
+  const int Tlen = a.cv.seq_len[layer * a.cv.B + b];
+  int pos = a.q_pos ? a.q_pos[lc * a.cv.B + b] : Tlen - 1;
   pos = max(0, min(pos, a.cv.max_seq - 1));
   constexpr int HP = D / 2;
+  if (Tlen <= 0) {  // empty cache: the main kernel has no tile for this unit, the output is defined as 0
+    T* outp = reinterpret_cast<T*>(a.out) + (size_t)uc * D;
+    for (int i = tid; i < D; i += 256) {
+      if constexpr (sizeof(T) == 2) outp[i] = __float2half_rn(0.f);
+      else outp[i] = 0.f;
+    }
+    return;
+  }
   const T* qp = reinterpret_cast<const T*>(a.q) + (size_t)uc * D;
-  for (int g = tid; g < HP; g += 128) {
+  for (int g = tid; g < HP; g += 256) {
     int ia = a.rope_layout == 0 ? 2 * g : g, ib = a.rope_layout == 0 ? 2 * g + 1 : g + HP;
     float xa = load_as_float<T>(qp + ia), xb = load_as_float<T>(qp + ib);
     float2 cs = *reinterpret_cast<const float2*>(a.rope_cs + ((size_t)pos * HP + g) * 2);
@@ -45,24 +54,13 @@ __global__ void __launch_bounds__(128) decode_prep_kernel(DecodeArgs a) {
     x[ib] = xa * cs.y + xb * cs.x;
   }
   __syncthreads();
-  const float* Pk = a.pi_k + ((size_t)layer * a.cv.H + h) * D * D;
-  for (int i = warp; i < D; i += 4) {
-    float p = 0.f;
-#pragma unroll
-    for (int k = lane; k < D; k += 32) p = fmaf(Pk[(size_t)i * D + k], x[k], p);
-    p = warp_sum(p);
-    if (lane == 0) y[i] = p;
-  }
+  matvec_rows_ilp<D, 8>(a.pi_k + ((size_t)layer * a.cv.H + h) * D * D, x, y, warp, lane);
   __syncthreads();
   float* dst = a.qrot + (size_t)uc * 2 * D;
-  for (int i = tid; i < D; i += 128) dst[i] = y[i];
-  for (int j = warp; j < D; j += 4) {
-    float p = 0.f;
-#pragma unroll
-    for (int k = lane; k < D; k += 32) p = fmaf(a.S[(size_t)j * D + k], y[k], p);
-    p = warp_sum(p);
-    if (lane == 0) dst[D + j] = p;
-  }
+  for (int i = tid; i < D; i += 256) dst[i] = y[i];
+  matvec_rows_ilp<D, 8>(a.S, y, x, warp, lane);
+  __syncthreads();
+  for (int i = tid; i < D; i += 256) dst[D + i] = x[i];
 }
 
 // ------------------------------------------------------------------------------------------ smem helpers
@@ -93,49 +91,118 @@ __device__ __forceinline__ unsigned field_at(const unsigned (&w)[NW]) {
   return v & mask;
 }
 
+// Shared-memory map in ABSOLUTE shared-window addresses (the OR-addressing needs the K/V tables aligned to
+// their own size, the sign table to 4 KB).  Dynamic shared memory starts right after the 1 KB the driver
+// reserves, so everything is placed at fixed absolute addresses and the kernel traps if the window starts
+// later than kAbsWbuf.
 template <int D>
 struct DecodeCfg {
   using Lo = Layout<D>;
-  static constexpr int NCK = D == 64 ? 64 : 128;        // columns of the K table (>= P + 31)
-  static constexpr int LSK = D == 64 ? 8 : 9;           // log2(NCK * 4)
+  static constexpr int NCK = D;                          // columns of the K table = 2 P (>= P + 31)
+  static constexpr int LSK = D == 64 ? 8 : 9;            // log2(NCK * 4)
   static constexpr int kKtabBytes = 64 * NCK * 4;        // 16 KB | 32 KB
   static constexpr int kVtabBytes = 64 * 32 * 8;         // 16 KB
   static constexpr int kStabBytes = 16 * 64 * 4;         // 4 KB
-  static constexpr int kAlign = kKtabBytes;              // base alignment that makes the OR-addressing valid
-  static constexpr int kRedFloats = 4 * (D + 2) + D + 4;  // per-warp (m, l, o'), merged o, flags
-  static constexpr int kSmemBytes = kAlign + kKtabBytes + kVtabBytes + kStabBytes + kRedFloats * 4;
+  static constexpr unsigned kAbsWbuf = 2048;             // 8 warps x 32 softmax weights, then the arrival flag
+  static constexpr unsigned kAbsStab = 4096;
+  static constexpr unsigned kAbsScratch = 8192;          // plan prefix, per-warp partials, merged o (8 KB)
+  static constexpr unsigned kAbsKtab = kKtabBytes;       // 16384 | 32768
+  static constexpr unsigned kAbsVtab = kAbsKtab + kKtabBytes;
+  static constexpr unsigned kAbsEnd = kAbsVtab + kVtabBytes;
+  static constexpr int kSmemBytes = kAbsEnd;             // requested dynamic bytes (window start <= 4 KB)
+  static constexpr int kCtasPerSm = D == 64 ? 3 : 2;
 };
 
+// ---- packed fp32x2 arithmetic (sm_100: FFMA2 / FADD2 / FMUL2 issue two fp32 operations per slot) ----------
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pack2(float lo, float hi) {
+  f32x2 r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+  return r;
+}
+__device__ __forceinline__ void unpack2(f32x2 v, float& lo, float& hi) {
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) {
+  f32x2 r;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+  return r;
+}
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) {
+  f32x2 r;
+  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+  return r;
+}
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) {
+  f32x2 r;
+  asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+  return r;
+}
+__device__ __forceinline__ f32x2 lds_b64(unsigned addr) {
+  f32x2 v;
+  asm("ld.shared.b64 %0, [%1];" : "=l"(v) : "r"(addr));
+  return v;
+}
+
+// <q'', lut_K[codes]>: P table reads, summed two at a time
 template <int D, int... K>
 __device__ __forceinline__ float k_score(const unsigned (&kw)[Layout<D>::KCW], unsigned kbase,
                                          std::integer_sequence<int, K...>) {
-  float acc[4] = {0.f, 0.f, 0.f, 0.f};
-  ((acc[K & 3] += lds_f32<4 * K>(field_at<DecodeCfg<D>::LSK, 6 * K, 6>(kw) | kbase)), ...);
-  return (acc[0] + acc[1]) + (acc[2] + acc[3]);
+  f32x2 acc[2] = {0ull, 0ull};
+  ((acc[K & 1] = add2(acc[K & 1],
+                      pack2(lds_f32<8 * K>(field_at<DecodeCfg<D>::LSK, 12 * K, 6>(kw) | kbase),
+                            lds_f32<8 * K + 4>(field_at<DecodeCfg<D>::LSK, 12 * K + 6, 6>(kw) | kbase)))),
+   ...);
+  float a, b;
+  unpack2(add2(acc[0], acc[1]), a, b);
+  return a + b;
 }
 
+// <z, sigma>: d/4 nibble-table reads
 template <int D, int... K>
 __device__ __forceinline__ float s_score(const unsigned (&sw)[Layout<D>::KSW], unsigned sbase,
                                          std::integer_sequence<int, K...>) {
-  float acc[4] = {0.f, 0.f, 0.f, 0.f};
-  ((acc[K & 3] += lds_f32<4 * K>(field_at<8, 4 * K, 4>(sw) | sbase)), ...);
-  return (acc[0] + acc[1]) + (acc[2] + acc[3]);
+  f32x2 acc[2] = {0ull, 0ull};
+  ((acc[K & 1] = add2(acc[K & 1], pack2(lds_f32<8 * K>(field_at<8, 8 * K, 4>(sw) | sbase),
+                                        lds_f32<8 * K + 4>(field_at<8, 8 * K + 4, 4>(sw) | sbase)))),
+   ...);
+  float a, b;
+  unpack2(add2(acc[0], acc[1]), a, b);
+  return a + b;
 }
 
-template <int D, int... K>
-__device__ __forceinline__ void v_accum(const unsigned (&vw)[Layout<D>::KCW], unsigned vbase, float w, float (&o)[D],
-                                        std::integer_sequence<int, K...>) {
+// V accumulate, lane = coordinate pair: for token J of the tile, o2[part] += w_J * (lut_V[c0], lut_V[c1])
+template <int D, int J>
+__device__ __forceinline__ void v_token(const unsigned (&vw)[Layout<D>::KCW], unsigned vbase, float w,
+                                        f32x2 (&o2)[Layout<D>::P / kTile]) {
+  const f32x2 w2 = pack2(w, w);
+#pragma unroll
+  for (int part = 0; part < Layout<D>::P / kTile; ++part) {
+    unsigned f = part == 0 ? field_at<8, 6 * J, 6>(vw) : field_at<8, 192 * (Layout<D>::P / kTile - 1) + 6 * J, 6>(vw);
+    o2[part] = fma2(lds_b64(f | vbase), w2, o2[part]);
+  }
+}
+template <int D, int... J>
+__device__ __forceinline__ void v_accum(const unsigned (&vw)[Layout<D>::KCW], unsigned vbase, unsigned wbuf,
+                                        f32x2 (&o2)[Layout<D>::P / kTile], std::integer_sequence<int, J...>) {
+  // w of tokens 4J .. 4J+3 arrive with one broadcast 128-bit read
   (([&] {
-     float2 lv = lds_f32x2(field_at<8, 6 * K, 6>(vw) | vbase);
-     o[2 * K] = fmaf(w, lv.x, o[2 * K]);
-     o[2 * K + 1] = fmaf(w, lv.y, o[2 * K + 1]);
+     float4 w4;
+     asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4+%5];"
+                  : "=f"(w4.x), "=f"(w4.y), "=f"(w4.z), "=f"(w4.w)
+                  : "r"(wbuf), "n"(16 * J));
+     v_token<D, 4 * J>(vw, vbase, w4.x, o2);
+     v_token<D, 4 * J + 1>(vw, vbase, w4.y, o2);
+     v_token<D, 4 * J + 2>(vw, vbase, w4.z, o2);
+     v_token<D, 4 * J + 3>(vw, vbase, w4.w, o2);
    }()),
    ...);
 }
 
-// one token's packed words, as loaded by the lane that owns it
+// What one lane loads per tile: its own token's K code / sign strings and norms (lane = token), and the V
+// code string of its coordinate pair(s) for all 32 tokens (lane = pair).
 template <int D>
-struct TokenWords {
+struct TileWords {
   unsigned kw[Layout<D>::KCW];
   unsigned sw[Layout<D>::KSW];
   unsigned vw[Layout<D>::KCW];
@@ -160,7 +227,7 @@ __device__ __forceinline__ void load_words(unsigned (&dst)[W], const unsigned ch
 }
 
 template <int D>
-__device__ __forceinline__ void load_token(TokenWords<D>& t, const unsigned char* tp, int lane) {
+__device__ __forceinline__ void load_tile_words(TileWords<D>& t, const unsigned char* tp, int lane) {
   using Lo = Layout<D>;
   load_words<Lo::KCW>(t.kw, tp + Lo::kOffKC, lane);
   load_words<Lo::KSW>(t.sw, tp + Lo::kOffKS, lane);
@@ -170,205 +237,318 @@ __device__ __forceinline__ void load_token(TokenWords<D>& t, const unsigned char
   t.vn = __ldg(reinterpret_cast<const unsigned short*>(tp + Lo::kOffVN) + lane);
 }
 
-// Sum o[0..N) over the 32 lanes; afterwards lane holds elements [ (N/32) * lane, (N/32) * (lane+1) ) in o[0..N/32).
-template <int N>
-__device__ __forceinline__ void lanes_transpose_sum(float (&o)[N], int lane) {
-  static_assert(N % 32 == 0, "");
+constexpr int kMaxSegments = 64;       // split-K partial slots per unit (tq_api.cu sizes the workspace)
+constexpr int kDecodeThreads = 256;
+constexpr int kDecodeWarps = kDecodeThreads / 32;
+
+// ---- table construction (per unit; pre-scaled so that logits come out in log2 units) ---------------------
+template <int D>
+__device__ __forceinline__ void build_k_tables(float* Ktab, float* Stab, const float* qr, const float* __restrict__ lk,
+                                               int tid) {
+  using Lo = Layout<D>;
+  using Cfg = DecodeCfg<D>;
+  const float sc_k = 1.4426950408889634f * rsqrtf((float)D);
+  const float sc_s = sc_k * 1.2533141373155003f / (float)D;  // log2(e)/sqrt(d) * sqrt(pi/2)/m, m = D
+  {  // Ktab[e][c] = (q''_{2g} lut[e & 7] + q''_{2g+1} lut[e >> 3]) * sc_k,  g = c mod P, both copies c = g, g + P
+    constexpr int EG = kDecodeThreads / Lo::P;  // entry groups: 8 (D = 64) | 4 (D = 128)
+    constexpr int EPT = 64 / EG;                // entries per thread: 8 | 16
+    const int g = tid % Lo::P, eq = tid / Lo::P;
+    const float q0 = __ldcg(qr + 2 * g) * sc_k, q1 = __ldcg(qr + 2 * g + 1) * sc_k;
+    float a0[8], a1[EPT / 8];
 #pragma unroll
-  for (int stage = 0; stage < 5; ++stage) {
-    const int off = 16 >> stage;
-    const int half = N >> (stage + 1);  // elements kept after this stage
-    const bool upper = (lane & off) != 0;
+    for (int c = 0; c < 8; ++c) a0[c] = q0 * __ldg(lk + c);
 #pragma unroll
-    for (int i = 0; i < N / 2; ++i) {
-      if (i < half) {
-        float send = upper ? o[i] : o[i + half];
-        float keep = upper ? o[i + half] : o[i];
-        o[i] = keep + __shfl_xor_sync(0xffffffffu, send, off);
-      }
+    for (int jj = 0; jj < EPT / 8; ++jj) a1[jj] = q1 * __ldg(lk + eq * (EPT / 8) + jj);
+    float* dst = Ktab + (size_t)(eq * EPT) * Cfg::NCK + g;
+#pragma unroll
+    for (int j = 0; j < EPT; ++j) {
+      const float v = a0[j & 7] + a1[j >> 3];
+      dst[j * Cfg::NCK] = v;
+      dst[j * Cfg::NCK + Lo::P] = v;
+    }
+  }
+  if (tid < 128) {  // Stab[e][c] = sum_b (bit b of e ? +z : -z)[4n + b] * sc_s,  n = c mod NG, all 64 / NG copies
+    constexpr int TG = 128 / Lo::NG;  // thread groups: 8 | 4
+    constexpr int EPT = 16 / TG;      // entries per thread: 2 | 4
+    const int n = tid % Lo::NG, eq = tid / Lo::NG;
+    float z[4];
+#pragma unroll
+    for (int b = 0; b < 4; ++b) z[b] = __ldcg(qr + D + 4 * n + b) * sc_s;
+#pragma unroll
+    for (int j = 0; j < EPT; ++j) {
+      const int e = eq * EPT + j;
+      float v = 0.f;
+#pragma unroll
+      for (int b = 0; b < 4; ++b) v += ((e >> b) & 1) ? z[b] : -z[b];
+#pragma unroll
+      for (int cp = 0; cp < 64 / Lo::NG; ++cp) Stab[e * 64 + n + cp * Lo::NG] = v;
     }
   }
 }
 
-constexpr float kLazyThreshold = 16.0f;  // log2 units: rescale only when the running max grows by > 2^16
+__device__ __forceinline__ void build_v_table(float2* Vtab, const float* __restrict__ lv, int tid) {
+  const int lane = tid & 31, eq = tid >> 5;  // 8 warps: entries 8 eq .. 8 eq + 7, i.e. hi code = eq
+  const float hi = __ldg(lv + eq);
+#pragma unroll
+  for (int j = 0; j < 8; ++j) Vtab[(eq * 8 + j) * 32 + lane] = make_float2(__ldg(lv + j), hi);
+}
 
+// ---- the streaming kernel ------------------------------------------------------------------------------------
+// Persistent, stream-K: the flat sequence of all 32-token tiles of the launch (unit-major) is cut into
+// gridDim.x equal contiguous ranges, so every CTA streams the same number of bytes regardless of how the
+// tiles fall on units.  A CTA walks its range unit by unit ("segments"); a unit covered by one CTA is finished
+// in place, a unit covered by several is merged by whichever CTA finishes it last.
 template <int D, typename TIO>
-__global__ void __launch_bounds__(128) decode_main_kernel(DecodeArgs a) {
+__global__ void __launch_bounds__(kDecodeThreads, DecodeCfg<D>::kCtasPerSm) decode_main_kernel(DecodeArgs a, int min_q) {
   using Lo = Layout<D>;
   using Cfg = DecodeCfg<D>;
+  constexpr int NW = kDecodeWarps;
+  constexpr int VP = Lo::P / kTile;  // coordinate pairs per lane: 1 | 2
   extern __shared__ unsigned char smem_raw[];
   const unsigned raw = (unsigned)__cvta_generic_to_shared(smem_raw);
-  const unsigned ktab = (raw + Cfg::kAlign - 1) & ~(unsigned)(Cfg::kAlign - 1);
-  const unsigned vtab = ktab + Cfg::kKtabBytes;
-  const unsigned stab = vtab + Cfg::kVtabBytes;
-  unsigned char* gen = smem_raw + (ktab - raw);  // generic pointer to the aligned region
-  float* Ktab = reinterpret_cast<float*>(gen);
-  float2* Vtab = reinterpret_cast<float2*>(gen + Cfg::kKtabBytes);
-  float* Stab = reinterpret_cast<float*>(gen + Cfg::kKtabBytes + Cfg::kVtabBytes);
-  float* red = reinterpret_cast<float*>(gen + Cfg::kKtabBytes + Cfg::kVtabBytes + Cfg::kStabBytes);
-  float* omerged = red + 4 * (D + 2);  // [D] + flags
-  int* flag = reinterpret_cast<int*>(omerged + D);
+  if (raw > Cfg::kAbsWbuf) __trap();  // the fixed shared-memory map does not fit: fail loudly
+  unsigned char* abs0 = smem_raw - raw;  // generic pointer to absolute shared address 0 of this CTA's window
+  float* Stab = reinterpret_cast<float*>(abs0 + Cfg::kAbsStab);
+  int* plan = reinterpret_cast<int*>(abs0 + Cfg::kAbsScratch);            // [E + 1] exclusive prefix of tiles
+  float* red = reinterpret_cast<float*>(abs0 + Cfg::kAbsScratch + 4608);  // NW x (D + 2)
+  float* omerged = red + NW * (D + 2);                                     // [D] + [3 D] partial matvecs
+  float* wbuf_f = reinterpret_cast<float*>(abs0 + Cfg::kAbsWbuf);         // NW x 32 softmax weights
+  int* flag = reinterpret_cast<int*>(wbuf_f + NW * 32);
+  float* Ktab = reinterpret_cast<float*>(abs0 + Cfg::kAbsKtab);
+  float2* Vtab = reinterpret_cast<float2*>(abs0 + Cfg::kAbsVtab);
+  const unsigned ktab = Cfg::kAbsKtab, vtab = Cfg::kAbsVtab, stab = Cfg::kAbsStab;
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int uc = blockIdx.x / a.nsplit, split = blockIdx.x % a.nsplit;
-  const int BH = a.cv.B * a.cv.H;
-  const int lc = uc / BH, bh = uc % BH, b = bh / a.cv.H, h = bh % a.cv.H;
-  const int layer = a.layer_begin + lc;
-  const int T = a.cv.seq_len[layer * a.cv.B + b];
-  const int ntiles = (T + kTile - 1) / kTile;
-  const int tps = (ntiles + a.nsplit - 1) / a.nsplit;
-  const int tile_begin = split * tps;
-  const int tile_end = min(ntiles, tile_begin + tps);
+  const int B = a.cv.B, H = a.cv.H;
+  const int E = a.n_layers_call * B;  // plan entries (layer-in-call, batch); seq_len is contiguous over them
+  const int32_t* seq = a.cv.seq_len + a.layer_begin * B;
 
-  // ---- tables (pre-scaled so that the logit comes out in log2 units)
+  // ---- plan: exclusive prefix sum of tiles per entry
   {
-    const float* qr = a.qrot + (size_t)uc * 2 * D;
-    const float* lk = a.lut_k + ((size_t)layer * a.cv.H + h) * 8;
-    const float* lv = a.lut_v + ((size_t)layer * a.cv.H + h) * 8;
-    const float sc_k = 1.4426950408889634f * rsqrtf((float)D);
-    const float sc_s = sc_k * 1.2533141373155003f / (float)D;  // sqrt(pi/2) / m, m = D
-    for (int idx = tid; idx < 64 * Cfg::NCK; idx += 128) {
-      const int e = idx / Cfg::NCK, c = idx % Cfg::NCK, g = c % Lo::P;
-      Ktab[idx] = fmaf(qr[2 * g], lk[e & 7], qr[2 * g + 1] * lk[e >> 3]) * sc_k;
-    }
-    for (int idx = tid; idx < 16 * 64; idx += 128) {
-      const int e = idx / 64, c = idx % 64, n = c % Lo::NG;
-      float s = 0.f;
+    const int CH = (E + kDecodeThreads - 1) / kDecodeThreads;
+    int local = 0;
+    for (int e = tid * CH; e < min(E, (tid + 1) * CH); ++e) local += (seq[e] + kTile - 1) / kTile;
+    int incl = local;
 #pragma unroll
-      for (int bb = 0; bb < 4; ++bb) s += ((e >> bb) & 1) ? qr[D + 4 * n + bb] : -qr[D + 4 * n + bb];
-      Stab[idx] = s * sc_s;
+    for (int o = 1; o < 32; o <<= 1) {
+      int v = __shfl_up_sync(0xffffffffu, incl, o);
+      if (lane >= o) incl += v;
     }
-    for (int idx = tid; idx < 64 * 32; idx += 128) {
-      const int e = idx / 32;
-      Vtab[idx] = make_float2(lv[e & 7], lv[e >> 3]);
+    int* wtot = reinterpret_cast<int*>(red);
+    if (lane == 31) wtot[warp] = incl;
+    __syncthreads();
+    int base = 0;
+    for (int w = 0; w < warp; ++w) base += wtot[w];
+    int run = base + incl - local;
+    for (int e = tid * CH; e < min(E, (tid + 1) * CH); ++e) {
+      plan[e] = run;
+      run += (seq[e] + kTile - 1) / kTile;
     }
+    if (tid == kDecodeThreads - 1) plan[E] = base + incl;
+    __syncthreads();
   }
-  __syncthreads();
+  const int total = plan[E] * H;  // tiles of the whole launch (< 2^31: checked on the host)
+  int Q = (total + (int)gridDim.x - 1) / (int)gridDim.x;
+  if (Q < min_q) Q = min_q;
+  int f = (int)blockIdx.x * Q;
+  const int fend = min(total, f + Q);
+  if (f >= fend) return;
 
   const unsigned kbase = ktab + lane * 4, sbase = stab + lane * 4, vbase = vtab + lane * 8;
-  const size_t unit = (size_t)layer * BH + bh;
-  const unsigned char* stream = a.cv.tiles + unit * a.cv.stream_bytes;
+  const unsigned wbuf = (unsigned)__cvta_generic_to_shared(wbuf_f + warp * 32);
+  int vtab_owner = -1;  // (layer, head) the V table currently holds
 
-  float o[D];
-#pragma unroll
-  for (int i = 0; i < D; ++i) o[i] = 0.f;
-  float m = -INFINITY, l = 0.f;
+  // ---- locate the unit that owns flat tile f (binary search once; afterwards units are walked in order)
+  int e;
+  {
+    int lo = 0, hi = E;  // invariant: H * plan[lo] <= f < H * plan[hi]
+    while (hi - lo > 1) {
+      const int mid = (lo + hi) >> 1;
+      if (plan[mid] * H <= f) lo = mid;
+      else hi = mid;
+    }
+    e = lo;
+  }
+  int nt = plan[e + 1] - plan[e];
+  int h = (f - plan[e] * H) / nt;
+  int tile0 = (f - plan[e] * H) % nt;
 
-  TokenWords<D> cur, nxt;
-  int tile = tile_begin + warp;
-  if (tile < tile_end) load_token<D>(cur, stream + (size_t)tile * Lo::kTileBytes, lane);
-  for (; tile < tile_end; tile += 4) {
-    const bool has_next = tile + 4 < tile_end;
-    if (has_next) load_token<D>(nxt, stream + (size_t)(tile + 4) * Lo::kTileBytes, lane);
-    const bool valid = tile * kTile + lane < T;
-    const float sa = k_score<D>(cur.kw, kbase, std::make_integer_sequence<int, Lo::P>{});
-    const float sb = s_score<D>(cur.sw, sbase, std::make_integer_sequence<int, Lo::NG>{});
-    float s2 = f16_bits_to_f32(cur.kn) * fmaf(f16_bits_to_f32(cur.kr), sb, sa);
-    s2 = valid ? s2 : -INFINITY;
-    const float tmax = warp_max(s2);  // finite: slot 0 of every processed tile is valid
-    if (tmax > m + kLazyThreshold) {  // warp-uniform; also taken on the first tile (m = -inf)
-      const float f = exp2f(m - tmax);  // 0 on the first tile
-      l *= f;
-#pragma unroll
-      for (int i = 0; i < D; ++i) o[i] *= f;
-      m = tmax;
-    }
-    const float p = exp2f(s2 - m);  // invalid lanes: exp2(-inf) = 0
-    l += p;
-    const float w = valid ? p * f16_bits_to_f32(cur.vn) : 0.f;
-    v_accum<D>(cur.vw, vbase, w, o, std::make_integer_sequence<int, Lo::P>{});
-    if (has_next) cur = nxt;
-  }
+  while (true) {
+    const int tile1 = min(nt, tile0 + (fend - f));  // exclusive
+    const int lc = e / B, b = e - lc * B;
+    const int layer = a.layer_begin + lc;
+    const int uc = e * H + h;
+    const int T = seq[e];
+    const int ustart = plan[e] * H + h * nt;
+    const int cfirst = ustart / Q, clast = (ustart + nt - 1) / Q;
+    const int nseg = clast - cfirst + 1, slot = (int)blockIdx.x - cfirst;
 
-  // ---- per-warp reduction over lanes, then over the CTA's warps
-  lanes_transpose_sum<D>(o, lane);
-  l = warp_sum(l);
-  float* wr = red + warp * (D + 2);
-  if (lane == 0) {
-    wr[0] = m;
-    wr[1] = l;
-  }
-#pragma unroll
-  for (int i = 0; i < D / 32; ++i) wr[2 + (D / 32) * lane + i] = o[i];
-  __syncthreads();
-  float M = fmaxf(fmaxf(red[0], red[D + 2]), fmaxf(red[2 * (D + 2)], red[3 * (D + 2)]));
-  float Lsum = 0.f, oi = 0.f;
-  if (tid < D) {
-#pragma unroll
-    for (int w = 0; w < 4; ++w) {
-      const float mw = red[w * (D + 2)];
-      const float f = mw == -INFINITY ? 0.f : exp2f(mw - M);
-      Lsum = fmaf(red[w * (D + 2) + 1], f, Lsum);
-      oi = fmaf(red[w * (D + 2) + 2 + tid], f, oi);
-    }
-  }
-  TIO* outp = reinterpret_cast<TIO*>(a.out) + (size_t)uc * D;
-  const float* Pv = a.pi_v + ((size_t)layer * a.cv.H + h) * D * D;
-  if (a.nsplit > 1) {
-    float* part = a.partials + ((size_t)uc * a.nsplit + split) * (D + 2);
-    if (tid < D) part[2 + tid] = oi;
-    if (tid == 0) {
-      part[0] = M;
-      part[1] = Lsum;
-    }
-    __threadfence();
-    __syncthreads();
-    if (tid == 0) {
-      int old = atomicAdd(&a.counters[uc], 1);
-      *flag = (old == a.nsplit - 1);
-      if (old == a.nsplit - 1) a.counters[uc] = 0;
+    // ---- tables of this unit
+    __syncthreads();  // every warp is done with the previous unit's tables and scratch
+    build_k_tables<D>(Ktab, Stab, a.qrot + (size_t)uc * 2 * D, a.lut_k + ((size_t)layer * H + h) * 8, tid);
+    if (vtab_owner != layer * H + h) {
+      build_v_table(Vtab, a.lut_v + ((size_t)layer * H + h) * 8, tid);
+      vtab_owner = layer * H + h;
     }
     __syncthreads();
-    if (!*flag) return;
-    __threadfence();
-    const float* pp = a.partials + (size_t)uc * a.nsplit * (D + 2);
-    M = -INFINITY;
-    for (int s = 0; s < a.nsplit; ++s) M = fmaxf(M, __ldcg(pp + s * (D + 2)));
-    Lsum = 0.f;
-    oi = 0.f;
+
+    const unsigned char* stream = a.cv.tiles + ((size_t)layer * B * H + (size_t)b * H + h) * a.cv.stream_bytes;
+    f32x2 o2[VP];
+#pragma unroll
+    for (int i = 0; i < VP; ++i) o2[i] = 0ull;
+    float m = -INFINITY, l = 0.f;
+
+    TileWords<D> cur, nxt;
+    int tile = tile0 + warp;
+    if (tile < tile1) load_tile_words<D>(cur, stream + (size_t)tile * Lo::kTileBytes, lane);
+    for (; tile < tile1; tile += NW) {
+      const bool has_next = tile + NW < tile1;
+      if (has_next) load_tile_words<D>(nxt, stream + (size_t)(tile + NW) * Lo::kTileBytes, lane);
+      if (tile + 2 * NW < tile1 && lane < (Lo::kTileBytes + 127) / 128)  // pull the tile after next into L2
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(stream + (size_t)(tile + 2 * NW) * Lo::kTileBytes + lane * 128));
+      const bool valid = tile * kTile + lane < T;
+      const float sa = k_score<D>(cur.kw, kbase, std::make_integer_sequence<int, Lo::P / 2>{});
+      const float sb = s_score<D>(cur.sw, sbase, std::make_integer_sequence<int, Lo::NG / 2>{});
+      float s2 = f16_bits_to_f32(cur.kn) * fmaf(f16_bits_to_f32(cur.kr), sb, sa);
+      s2 = valid ? s2 : -INFINITY;
+      const float mnew = fmaxf(m, warp_max(s2));  // finite: slot 0 of every processed tile is valid
+      const float fsc = exp2f(m - mnew);          // 0 on a warp's first tile (m = -inf)
+      m = mnew;
+      const float p = exp2f(s2 - m);              // invalid lanes: exp2(-inf) = 0
+      l = fmaf(l, fsc, p);
+      const f32x2 fsc2 = pack2(fsc, fsc);
+#pragma unroll
+      for (int i = 0; i < VP; ++i) o2[i] = mul2(o2[i], fsc2);
+      // hand the softmax weights from lane = token to lane = coordinate pair through shared memory
+      __syncwarp();
+      asm volatile("st.shared.f32 [%0], %1;" ::"r"(wbuf + lane * 4), "f"(valid ? p * f16_bits_to_f32(cur.vn) : 0.f));
+      __syncwarp();
+      v_accum<D>(cur.vw, vbase, wbuf, o2, std::make_integer_sequence<int, kTile / 4>{});
+      if (has_next) cur = nxt;
+    }
+
+    // ---- reduce over the CTA's warps (lanes already own distinct coordinates)
+    l = warp_sum(l);
+    float* wr = red + warp * (D + 2);
+    if (lane == 0) {
+      wr[0] = m;
+      wr[1] = l;
+    }
+#pragma unroll
+    for (int i = 0; i < VP; ++i) {
+      float x0, x1;
+      unpack2(o2[i], x0, x1);
+      wr[2 + 2 * (lane + kTile * i)] = x0;
+      wr[2 + 2 * (lane + kTile * i) + 1] = x1;
+    }
+    __syncthreads();
+    float M = -INFINITY;
+#pragma unroll
+    for (int w = 0; w < NW; ++w) M = fmaxf(M, red[w * (D + 2)]);
+    float Lsum = 0.f, oi = 0.f;
     if (tid < D) {
-      for (int s = 0; s < a.nsplit; ++s) {
-        const float ms = __ldcg(pp + s * (D + 2));
-        const float f = ms == -INFINITY ? 0.f : exp2f(ms - M);
-        Lsum = fmaf(__ldcg(pp + s * (D + 2) + 1), f, Lsum);
-        oi = fmaf(__ldcg(pp + s * (D + 2) + 2 + tid), f, oi);
+#pragma unroll
+      for (int w = 0; w < NW; ++w) {
+        const float mw = red[w * (D + 2)];
+        const float fw = mw == -INFINITY ? 0.f : exp2f(mw - M);
+        Lsum = fmaf(red[w * (D + 2) + 1], fw, Lsum);
+        oi = fmaf(red[w * (D + 2) + 2 + tid], fw, oi);
       }
     }
-  }
-  // ---- finalise: out = PI_V^T (o' / l); an empty cache gives 0
-  if (tid < D) omerged[tid] = Lsum > 0.f ? oi / Lsum : 0.f;
-  __syncthreads();
-  if (tid < D) {
-    float r = 0.f;
-#pragma unroll 8
-    for (int k = 0; k < D; ++k) r = fmaf(Pv[(size_t)k * D + tid], omerged[k], r);
-    if constexpr (sizeof(TIO) == 2)
-      outp[tid] = __float2half_rn(r);
-    else
-      outp[tid] = r;
+    bool finish = true;
+    if (nseg > 1) {
+      float* part = a.partials + ((size_t)uc * kMaxSegments + slot) * (D + 2);
+      if (tid < D) part[2 + tid] = oi;
+      if (tid == 0) {
+        part[0] = M;
+        part[1] = Lsum;
+      }
+      __threadfence();
+      __syncthreads();
+      if (tid == 0) {
+        const int old = atomicAdd(&a.counters[uc], 1);
+        *flag = (old == nseg - 1);
+        if (old == nseg - 1) a.counters[uc] = 0;
+      }
+      __syncthreads();
+      finish = *flag != 0;
+      if (finish) {
+        __threadfence();
+        const float* pp = a.partials + (size_t)uc * kMaxSegments * (D + 2);
+        M = -INFINITY;
+        for (int s = 0; s < nseg; ++s) M = fmaxf(M, __ldcg(pp + s * (D + 2)));
+        Lsum = 0.f;
+        oi = 0.f;
+        if (tid < D) {
+          for (int s = 0; s < nseg; ++s) {
+            const float ms = __ldcg(pp + s * (D + 2));
+            const float fs = ms == -INFINITY ? 0.f : exp2f(ms - M);
+            Lsum = fmaf(__ldcg(pp + s * (D + 2) + 1), fs, Lsum);
+            oi = fmaf(__ldcg(pp + s * (D + 2) + 2 + tid), fs, oi);
+          }
+        }
+      }
+    }
+    if (finish) {  // out = PI_V^T (o' / l): the k range is split over the 256 / D thread groups
+      if (tid < D) omerged[tid] = Lsum > 0.f ? oi / Lsum : 0.f;
+      __syncthreads();
+      constexpr int PARTS = kDecodeThreads / D;  // 4 | 2
+      constexpr int KP = D / PARTS;              // 16 | 64
+      const int i = tid % D, part = tid / D;
+      const float* Pv = a.pi_v + ((size_t)layer * H + h) * D * D + (size_t)part * KP * D + i;
+      float r = 0.f;
+#pragma unroll 16
+      for (int k = 0; k < KP; ++k) r = fmaf(__ldg(Pv + (size_t)k * D), omerged[part * KP + k], r);
+      if (part > 0) omerged[part * D + i] = r;
+      __syncthreads();
+      if (part == 0) {
+#pragma unroll
+        for (int pp = 1; pp < PARTS; ++pp) r += omerged[pp * D + i];
+        TIO* outp = reinterpret_cast<TIO*>(a.out) + (size_t)uc * D;
+        if constexpr (sizeof(TIO) == 2) outp[i] = __float2half_rn(r);
+        else outp[i] = r;
+      }
+    }
+    // ---- next unit of this CTA's range
+    f += tile1 - tile0;
+    if (f >= fend) break;
+    tile0 = 0;
+    if (++h == H) {
+      h = 0;
+      do { ++e; } while (plan[e + 1] == plan[e]);  // skip empty caches; f < fend <= total guarantees a hit
+      nt = plan[e + 1] - plan[e];
+    }
   }
 }
 
 // ------------------------------------------------------------------------------------------ launchers
 template <int D, typename T>
-static cudaError_t launch_decode_t(const DecodeArgs& a, cudaStream_t st) {
+static cudaError_t launch_decode_t(const DecodeArgs& a, int num_sms, int min_q, cudaStream_t st) {
   const int units = a.n_layers_call * a.cv.B * a.cv.H;
-  decode_prep_kernel<D, T><<<units, 128, 0, st>>>(a);
+  decode_prep_kernel<D, T><<<units, 256, 0, st>>>(a);
   count_launch();
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;
   constexpr int smem = DecodeCfg<D>::kSmemBytes;
-  e = cudaFuncSetAttribute(decode_main_kernel<D, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-  if (e != cudaSuccess) return e;
-  decode_main_kernel<D, T><<<units * a.nsplit, 128, smem, st>>>(a);
+  static bool attr_set = false;
+  if (!attr_set) {
+    e = cudaFuncSetAttribute(decode_main_kernel<D, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e != cudaSuccess) return e;
+    attr_set = true;
+  }
+  int grid = num_sms * DecodeCfg<D>::kCtasPerSm;
+  if (a.nsplit > 0) grid = a.nsplit;  // profiling / test override: number of CTAs
+  decode_main_kernel<D, T><<<grid, kDecodeThreads, smem, st>>>(a, min_q);
   count_launch();
   return cudaGetLastError();
 }
 
-cudaError_t launch_decode(const DecodeArgs& a, int D, cudaStream_t st) {
+cudaError_t launch_decode(const DecodeArgs& a, int D, int num_sms, int min_q, cudaStream_t st) {
   if (D == 64)
-    return a.dt == TQ_F16 ? launch_decode_t<64, __half>(a, st) : launch_decode_t<64, float>(a, st);
-  return a.dt == TQ_F16 ? launch_decode_t<128, __half>(a, st) : launch_decode_t<128, float>(a, st);
+    return a.dt == TQ_F16 ? launch_decode_t<64, __half>(a, num_sms, min_q, st)
+                          : launch_decode_t<64, float>(a, num_sms, min_q, st);
+  return a.dt == TQ_F16 ? launch_decode_t<128, __half>(a, num_sms, min_q, st)
+                        : launch_decode_t<128, float>(a, num_sms, min_q, st);
 }
 
 }  // namespace tq

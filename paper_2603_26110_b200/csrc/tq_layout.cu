@@ -69,11 +69,15 @@ __global__ void export_kernel(CacheView cv, int layer, int n_tokens, tq_canonica
     }
     ks[byte] = (unsigned char)v;
   }
-  // V codes: pair group g at position g
-  load_section<D>(tile + Lo::kOffVC, Lo::KCW, slot, words);
-  words[Lo::KCW] = 0;
+  // V codes: lane g of the tile owns pair groups g (+32 for d = 128); token slot j sits at bits [6j, 6j+6)
   for (int g = 0; g < Lo::P; ++g) {
-    unsigned f = get_bits(words, 6 * g, 6);
+    const int lane = g % kTile, part = g / kTile;
+    const int bit = 192 * part + 6 * slot;
+    const unsigned char* sec = tile + Lo::kOffVC;
+    unsigned w0 = *(const unsigned*)(sec + word_offset(Lo::KCW, bit >> 5, lane));
+    unsigned w1 = ((bit & 31) > 26) ? *(const unsigned*)(sec + word_offset(Lo::KCW, (bit >> 5) + 1, lane)) : 0u;
+    unsigned long long v = w0 | ((unsigned long long)w1 << 32);
+    unsigned f = (unsigned)(v >> (bit & 31)) & 63u;
     codes[2 * g] = f & 7;
     codes[2 * g + 1] = f >> 3;
   }
@@ -124,17 +128,46 @@ __global__ void import_kernel(CacheView cv, int layer, int n_tokens, tq_canonica
     or_bits(words, 4 * k, 4, nib);
   }
   store_section<D>(tile + Lo::kOffKS, Lo::KSW, slot, words);
-  const unsigned char* vc = in.v_codes + (size_t)idx * (3 * D / 8);
-  for (int grp = 0; grp < D / 8; ++grp) {
-    unsigned p = vc[3 * grp] | ((unsigned)vc[3 * grp + 1] << 8) | ((unsigned)vc[3 * grp + 2] << 16);
-    for (int i = 0; i < 8; ++i) codes[8 * grp + i] = (p >> (3 * i)) & 7;
-  }
-  for (int w = 0; w <= Lo::KCW; ++w) words[w] = 0;
-  for (int g = 0; g < Lo::P; ++g) or_bits(words, 6 * g, 6, codes[2 * g] | ((unsigned)codes[2 * g + 1] << 3));
-  store_section<D>(tile + Lo::kOffVC, Lo::KCW, slot, words);
+  // V code words are shared by the 32 tokens of a tile: import_v_kernel (second pass) writes them.
   ((unsigned short*)(tile + Lo::kOffKN))[slot] = in.k_norm[idx];
   ((unsigned short*)(tile + Lo::kOffKR))[slot] = in.k_rnorm[idx];
   ((unsigned short*)(tile + Lo::kOffVN))[slot] = in.v_norm[idx];
+}
+
+// V code words of one tile hold all 32 tokens: one thread per (b, h, tile, lane) assembles its words from the
+// canonical planes (tokens beyond n_tokens keep whatever the tile held).
+template <int D>
+__global__ void import_v_kernel(CacheView cv, int layer, int n_tokens, tq_canonical in) {
+  using Lo = Layout<D>;
+  const int ntile = (n_tokens + kTile - 1) / kTile;
+  long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  long total = (long)cv.B * cv.H * ntile * kTile;
+  if (idx >= total) return;
+  const int lane = (int)(idx % kTile);
+  const int tl = (int)((idx / kTile) % ntile);
+  const long bh = idx / ((long)kTile * ntile);
+  size_t unit = (size_t)layer * cv.B * cv.H + bh;
+  unsigned char* sec = cv.tiles + unit * cv.stream_bytes + (size_t)tl * Lo::kTileBytes + Lo::kOffVC;
+  unsigned words[Lo::KCW + 1];
+  unsigned keep[Lo::KCW + 1];
+  for (int w = 0; w <= Lo::KCW; ++w) words[w] = 0, keep[w] = 0;
+  for (int part = 0; part < Lo::P / kTile; ++part) {
+    const int g = lane + kTile * part;
+    for (int j = 0; j < kTile; ++j) {
+      const int t = tl * kTile + j;
+      if (t >= n_tokens) continue;
+      const unsigned char* vc = in.v_codes + ((size_t)bh * n_tokens + t) * (3 * D / 8);
+      const int cbit = 6 * g;  // codes 2g, 2g+1 are 6 consecutive bits of the canonical stream
+      unsigned v = vc[cbit >> 3] | ((unsigned)vc[(cbit >> 3) + 1 < 3 * D / 8 ? (cbit >> 3) + 1 : (cbit >> 3)] << 8);
+      unsigned f = (v >> (cbit & 7)) & 63u;
+      or_bits(words, 192 * part + 6 * j, 6, f);
+      or_bits(keep, 192 * part + 6 * j, 6, 63u);
+    }
+  }
+  for (int w = 0; w < Lo::KCW; ++w) {
+    unsigned* p = (unsigned*)(sec + word_offset(Lo::KCW, w, lane));
+    *p = (*p & ~keep[w]) | words[w];
+  }
 }
 
 cudaError_t launch_export(const CacheGeom& g, const CacheView& cv, int layer, int n_tokens, const tq_canonical& out,
@@ -160,6 +193,15 @@ cudaError_t launch_import(const CacheGeom& g, const CacheView& cv, int layer, in
   else
     import_kernel<128><<<blocks, 128, 0, st>>>(cv, layer, n_tokens, in);
   count_launch();
+  if (total > 0) {
+    long vt = (long)g.B * g.H * ((n_tokens + kTile - 1) / kTile) * kTile;
+    int vb = (int)((vt + 127) / 128);
+    if (g.D == 64)
+      import_v_kernel<64><<<vb, 128, 0, st>>>(cv, layer, n_tokens, in);
+    else
+      import_v_kernel<128><<<vb, 128, 0, st>>>(cv, layer, n_tokens, in);
+    count_launch();
+  }
   return cudaGetLastError();
 }
 

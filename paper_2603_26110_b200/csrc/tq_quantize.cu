@@ -200,24 +200,42 @@ __global__ void __launch_bounds__(2 * D) quantize_pack_kernel(QuantArgs a) {
     __syncthreads();
     // ------------------------------------------------------------------ assemble and store the tile
     unsigned char* tp = stream + (size_t)tile * Lo::kTileBytes;
-    // K and V code words: 32 slots x KCW words each
-    for (int idx = tid; idx < 2 * kTile * Lo::KCW; idx += NT) {
-      const int isV = idx / (kTile * Lo::KCW);
-      const int rem = idx % (kTile * Lo::KCW);
-      const int w = rem / kTile, slot = rem % kTile;  // lanes vary slot -> coalesced chunk-major stores
+    // K code words: 32 slots x KCW words, field g of slot t at position (g - t) mod P
+    for (int idx = tid; idx < kTile * Lo::KCW; idx += NT) {
+      const int w = idx / kTile, slot = idx % kTile;  // lanes vary slot -> coalesced chunk-major stores
       const int pos = tile * kTile + slot;
       if (pos < a.start_pos || pos >= a.start_pos + a.n_tokens) continue;
-      const unsigned char* cb = (isV ? cbV : cbK) + slot * D;
+      const unsigned char* cb = cbK + slot * D;
       unsigned long long word = 0;
       const int k_lo = (32 * w) / 6, k_hi = (32 * w + 31) / 6;
       for (int kf = k_lo; kf <= k_hi; ++kf) {
-        const int g = isV ? kf : (kf + slot) % Lo::P;
+        const int g = (kf + slot) % Lo::P;
         unsigned long long f = cb[2 * g] | ((unsigned)cb[2 * g + 1] << 3);
         const int sh = 6 * kf - 32 * w;  // may be negative for the field straddling in from the previous word
         word |= sh >= 0 ? (f << sh) : (f >> (-sh));
       }
-      *reinterpret_cast<unsigned*>(tp + (isV ? Lo::kOffVC : Lo::kOffKC) + word_offset(Lo::KCW, w, slot)) =
-          (unsigned)word;
+      *reinterpret_cast<unsigned*>(tp + Lo::kOffKC + word_offset(Lo::KCW, w, slot)) = (unsigned)word;
+    }
+    // V code words: lane g owns pair groups g (+32): token slot j at bits [6j, 6j+6) of its string; tokens of
+    // the tile that are outside this call keep their bits (read-modify-write under a mask)
+    for (int idx = tid; idx < kTile * Lo::KCW; idx += NT) {
+      const int w = idx / kTile, lane = idx % kTile;
+      const int part = (32 * w) / 192, sb = 32 * w - 192 * part;
+      const int g = lane + kTile * part;
+      unsigned long long word = 0, mask = 0;
+      const int j_lo = sb / 6, j_hi = (sb + 31) / 6;
+      for (int j = j_lo; j <= j_hi && j < kTile; ++j) {
+        const int pos = tile * kTile + j;
+        if (pos < a.start_pos || pos >= a.start_pos + a.n_tokens) continue;
+        unsigned long long f = cbV[j * D + 2 * g] | ((unsigned)cbV[j * D + 2 * g + 1] << 3);
+        const int sh = 6 * j - sb;
+        word |= sh >= 0 ? (f << sh) : (f >> (-sh));
+        mask |= sh >= 0 ? (63ull << sh) : (63ull >> (-sh));
+      }
+      unsigned* p = reinterpret_cast<unsigned*>(tp + Lo::kOffVC + word_offset(Lo::KCW, w, lane));
+      const unsigned m32 = (unsigned)mask;
+      if (m32 == 0xffffffffu) *p = (unsigned)word;
+      else if (m32) *p = (*p & ~m32) | ((unsigned)word & m32);
     }
     for (int idx = tid; idx < kTile * Lo::KSW; idx += NT) {
       const int w = idx / kTile, slot = idx % kTile;
@@ -245,35 +263,15 @@ __global__ void __launch_bounds__(2 * D) quantize_pack_kernel(QuantArgs a) {
 }
 
 // ---- single-token append --------------------------------------------------------------------------------
-// One CTA (128 threads) per (batch, head).  Matrices are read straight from global/L2 (each row by one
-// warp, coalesced along k); the token lands at index seq_len[layer][b], which the last-arriving head of
-// batch entry b then increments (BASELINE.json:configs[2]).
-template <int D>
-__device__ __forceinline__ void matvec_rows(const float* __restrict__ M, const float* xsm, float* ysm, int warp,
-                                            int lane, int nwarps) {
-  for (int i = warp; i < D; i += nwarps) {
-    float p = 0.f;
-#pragma unroll
-    for (int k = lane; k < D; k += 32) p = fmaf(M[(size_t)i * D + k], xsm[k], p);
-    p = warp_sum(p);
-    if (lane == 0) ysm[i] = p;
-  }
-}
-
-__device__ __forceinline__ float block_sum_128(float v, float* red, int warp, int lane) {
-  v = warp_sum(v);
-  __syncthreads();
-  if (lane == 0) red[warp] = v;
-  __syncthreads();
-  return red[0] + red[1] + red[2] + red[3];
-}
-
+// One CTA (256 threads) per (batch, head).  Matrix rows are read straight from global/L2, a batch of rows
+// per warp with all loads in flight at once (matvec_rows_ilp); the token lands at index seq_len[layer][b],
+// which the last-arriving head of batch entry b then increments (BASELINE.json:configs[2]).
 template <int D, typename T>
-__global__ void __launch_bounds__(128) append_kernel(QuantArgs a) {
+__global__ void __launch_bounds__(256) append_kernel(QuantArgs a) {
   using Lo = Layout<D>;
-  __shared__ float x[D], y[D], r[D], sr[D];
+  __shared__ float xk[D], xv[D], yk[D], yv[D], r[D], sr[D];
   __shared__ unsigned char cK[D], cV[D], bK[D];
-  __shared__ float red[4];
+  __shared__ float nrm[4];
   __shared__ float lutK[8], lutV[8];
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int bh = blockIdx.x;
@@ -287,72 +285,75 @@ __global__ void __launch_bounds__(128) append_kernel(QuantArgs a) {
   if (!full) {
     const T* kp = reinterpret_cast<const T*>(a.k) + (size_t)bh * D;
     const T* vp = reinterpret_cast<const T*>(a.v) + (size_t)bh * D;
-    // ---- key: RoPE, PI_K, norm, codes, residual, S, bits
-    for (int g = tid; g < HP; g += 128) {
+    if (tid < HP) {
+      const int g = tid;
       int ia = a.rope_layout == 0 ? 2 * g : g, ib = a.rope_layout == 0 ? 2 * g + 1 : g + HP;
       float xa = load_as_float<T>(kp + ia), xb = load_as_float<T>(kp + ib);
       float2 cs = *reinterpret_cast<const float2*>(a.rope_cs + ((size_t)pos * HP + g) * 2);
-      x[ia] = xa * cs.x - xb * cs.y;
-      x[ib] = xa * cs.y + xb * cs.x;
+      xk[ia] = xa * cs.x - xb * cs.y;
+      xk[ib] = xa * cs.y + xb * cs.x;
+    } else if (tid >= 128 && tid < 128 + D) {
+      xv[tid - 128] = load_as_float<T>(vp + tid - 128);
     }
     __syncthreads();
-    matvec_rows<D>(a.pi_k + (size_t)h * D * D, x, y, warp, lane, 4);
+    matvec_rows_ilp<D, 8>(a.pi_k + (size_t)h * D * D, xk, yk, warp, lane);
+    matvec_rows_ilp<D, 8>(a.pi_v + (size_t)h * D * D, xv, yv, warp, lane);
     __syncthreads();
-    float thr[7];
+    if (warp < 2) {  // warp 0: |y_k|, warp 1: |y_v|
+      const float* y = warp == 0 ? yk : yv;
+      float p = 0.f;
 #pragma unroll
-    for (int q = 0; q < 7; ++q) thr[q] = 0.5f * (lutK[q] + lutK[q + 1]);
-    float part = 0.f;
-    for (int i = tid; i < D; i += 128) part = fmaf(y[i], y[i], part);
-    float n = sqrtf(block_sum_128(part, red, warp, lane));
-    part = 0.f;
-    for (int i = tid; i < D; i += 128) {
-      float u = n > 0.f ? y[i] / n : 0.f;
-      int c = code_of(u, thr);
-      float rr = u - lutK[c];
-      cK[i] = (unsigned char)c;
-      r[i] = rr;
-      part = fmaf(rr, rr, part);
+      for (int i = lane; i < D; i += 32) p = fmaf(y[i], y[i], p);
+      p = warp_sum(p);
+      if (lane == 0) nrm[warp] = sqrtf(p);
     }
-    float gnorm = sqrtf(block_sum_128(part, red, warp, lane));
     __syncthreads();
-    matvec_rows<D>(a.S, r, sr, warp, lane, 4);
-    __syncthreads();
-    for (int j = tid; j < D; j += 128) bK[j] = sr[j] >= 0.f ? 1 : 0;
-    // ---- value: PI_V, norm, codes
-    for (int i = tid; i < D; i += 128) x[i] = load_as_float<T>(vp + i);
-    __syncthreads();
-    matvec_rows<D>(a.pi_v + (size_t)h * D * D, x, y, warp, lane, 4);
-    __syncthreads();
+    const float n = nrm[0], nv = nrm[1];
+    if (tid < D) {
+      float thr[7];
 #pragma unroll
-    for (int q = 0; q < 7; ++q) thr[q] = 0.5f * (lutV[q] + lutV[q + 1]);
-    part = 0.f;
-    for (int i = tid; i < D; i += 128) part = fmaf(y[i], y[i], part);
-    float nv = sqrtf(block_sum_128(part, red, warp, lane));
-    for (int i = tid; i < D; i += 128) {
-      float u = nv > 0.f ? y[i] / nv : 0.f;
+      for (int q = 0; q < 7; ++q) thr[q] = 0.5f * (lutK[q] + lutK[q + 1]);
+      const float u = n > 0.f ? yk[tid] / n : 0.f;
+      const int c = code_of(u, thr);
+      cK[tid] = (unsigned char)c;
+      r[tid] = u - lutK[c];
+    } else if (tid >= 128 && tid < 128 + D) {
+      const int i = tid - 128;
+      float thr[7];
+#pragma unroll
+      for (int q = 0; q < 7; ++q) thr[q] = 0.5f * (lutV[q] + lutV[q + 1]);
+      const float u = nv > 0.f ? yv[i] / nv : 0.f;
       cV[i] = (unsigned char)code_of(u, thr);
     }
+    __syncthreads();
+    if (warp == 0) {
+      float p = 0.f;
+#pragma unroll
+      for (int i = lane; i < D; i += 32) p = fmaf(r[i], r[i], p);
+      p = warp_sum(p);
+      if (lane == 0) nrm[2] = sqrtf(p);
+    }
+    matvec_rows_ilp<D, 8>(a.S, r, sr, warp, lane);
+    __syncthreads();
+    if (tid < D) bK[tid] = sr[tid] >= 0.f ? 1 : 0;
     __syncthreads();
     // ---- assemble this token's words
     const size_t unit = (size_t)a.layer * a.cv.B * a.cv.H + bh;
     unsigned char* tp = a.cv.tiles + unit * a.cv.stream_bytes + (size_t)(pos / kTile) * Lo::kTileBytes;
     const int slot = pos % kTile;
-    for (int idx = tid; idx < 2 * Lo::KCW; idx += 128) {
-      const int isV = idx / Lo::KCW, w = idx % Lo::KCW;
-      const unsigned char* cb = isV ? cV : cK;
+    if (tid < Lo::KCW) {
+      const int w = tid;
       unsigned long long word = 0;
       const int k_lo = (32 * w) / 6, k_hi = (32 * w + 31) / 6;
       for (int kf = k_lo; kf <= k_hi; ++kf) {
-        const int g = isV ? kf : (kf + slot) % Lo::P;
-        unsigned long long f = cb[2 * g] | ((unsigned)cb[2 * g + 1] << 3);
+        const int g = (kf + slot) % Lo::P;
+        unsigned long long f = cK[2 * g] | ((unsigned)cK[2 * g + 1] << 3);
         const int sh = 6 * kf - 32 * w;
         word |= sh >= 0 ? (f << sh) : (f >> (-sh));
       }
-      *reinterpret_cast<unsigned*>(tp + (isV ? Lo::kOffVC : Lo::kOffKC) + word_offset(Lo::KCW, w, slot)) =
-          (unsigned)word;
-    }
-    if (tid >= 64 && tid < 64 + Lo::KSW) {
-      const int w = tid - 64;
+      *reinterpret_cast<unsigned*>(tp + Lo::kOffKC + word_offset(Lo::KCW, w, slot)) = (unsigned)word;
+    } else if (tid >= 32 && tid < 32 + Lo::KSW) {
+      const int w = tid - 32;
       unsigned word = 0;
       for (int kn = 0; kn < 8; ++kn) {
         const int ng = (8 * w + kn + slot) % Lo::NG;
@@ -360,10 +361,20 @@ __global__ void __launch_bounds__(128) append_kernel(QuantArgs a) {
         word |= nib << (4 * kn);
       }
       *reinterpret_cast<unsigned*>(tp + Lo::kOffKS + word_offset(Lo::KSW, w, slot)) = word;
-    }
-    if (tid == 96) {
+    } else if (tid >= 64 && tid < 64 + Lo::P) {
+      // V: pair group g lives in lane (g mod 32)'s string at bits [192 part + 6 slot, +6): read-modify-write
+      const int g = tid - 64, vl = g % kTile, part = g / kTile;
+      const unsigned f = cV[2 * g] | ((unsigned)cV[2 * g + 1] << 3);
+      const int bit = 192 * part + 6 * slot, s = bit & 31;
+      unsigned* p0 = reinterpret_cast<unsigned*>(tp + Lo::kOffVC + word_offset(Lo::KCW, bit >> 5, vl));
+      *p0 = (*p0 & ~(63u << s)) | (f << s);
+      if (s > 26) {
+        unsigned* p1 = reinterpret_cast<unsigned*>(tp + Lo::kOffVC + word_offset(Lo::KCW, (bit >> 5) + 1, vl));
+        *p1 = (*p1 & ~(63u >> (32 - s))) | (f >> (32 - s));
+      }
+    } else if (tid == 192) {
       reinterpret_cast<unsigned short*>(tp + Lo::kOffKN)[slot] = f32_to_f16_bits_clamped(n);
-      reinterpret_cast<unsigned short*>(tp + Lo::kOffKR)[slot] = f32_to_f16_bits_clamped(gnorm);
+      reinterpret_cast<unsigned short*>(tp + Lo::kOffKR)[slot] = f32_to_f16_bits_clamped(nrm[2]);
       reinterpret_cast<unsigned short*>(tp + Lo::kOffVN)[slot] = f32_to_f16_bits_clamped(nv);
     }
   }
@@ -425,11 +436,11 @@ cudaError_t launch_quantize_pack(const QuantArgs& a, int D, tq_dtype dt, int num
 cudaError_t launch_append(const QuantArgs& a, int D, tq_dtype dt, cudaStream_t st) {
   const int BH = a.cv.B * a.cv.H;
   if (D == 64) {
-    if (dt == TQ_F16) append_kernel<64, __half><<<BH, 128, 0, st>>>(a);
-    else append_kernel<64, float><<<BH, 128, 0, st>>>(a);
+    if (dt == TQ_F16) append_kernel<64, __half><<<BH, 256, 0, st>>>(a);
+    else append_kernel<64, float><<<BH, 256, 0, st>>>(a);
   } else {
-    if (dt == TQ_F16) append_kernel<128, __half><<<BH, 128, 0, st>>>(a);
-    else append_kernel<128, float><<<BH, 128, 0, st>>>(a);
+    if (dt == TQ_F16) append_kernel<128, __half><<<BH, 256, 0, st>>>(a);
+    else append_kernel<128, float><<<BH, 256, 0, st>>>(a);
   }
   count_launch();
   return cudaGetLastError();
