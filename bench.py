@@ -260,10 +260,9 @@ def run_ours(args, w: W.Workload):
         cache.seq_len.fill_(T0)
 
     def one_step():
-        for layer in range(L):
-            tq.tq_append(shape, params, cache, layer, kn[layer], vn[layer], stream)
-            tq.tq_decode_attn(shape, params, cache, layer, 1, qs[layer:layer + 1], outs[layer:layer + 1], ws, None,
-                              max_seq, stream)
+        for layer in range(L):  # tq_decode_step == tq_append followed by tq_decode_attn, two launches per layer
+            tq.tq_decode_step(shape, params, cache, layer, qs[layer], kn[layer], vn[layer], outs[layer], ws, max_seq,
+                              stream)
 
     # ---- capture one model decode step as a CUDA graph (seq_len lives on the device, so it replays)
     with torch.cuda.stream(stream):
@@ -312,25 +311,24 @@ def run_ours(args, w: W.Workload):
     clocks = sampler.stop() if rank == 0 else None
     assert int(cache.status.item()) == 0, "an append was refused during the timed region"
 
-    # ---- live per-launch duration of the decode call (prep + fused kernel) and of append, CUDA events on `stream`
+    # ---- live duration of the decode call (query prep + streaming kernel) measured with CUDA events on
+    #      `stream`: 20 back-to-back tq_decode_attn launches over rotating layers between one event pair
     with torch.cuda.stream(stream):
         reset_len()
-        dec_ms, app_ms = [], []
-        for it in range(3):
-            for layer in range(L):
-                e0, e1, e2 = ev(), ev(), ev()
-                e0.record(stream)
-                tq.tq_append(shape, params, cache, layer, kn[layer], vn[layer], stream)
-                e1.record(stream)
+        dec_ms = []
+        reps = 20
+        for it in range(4):
+            e0, e1 = ev(), ev()
+            e0.record(stream)
+            for r in range(reps):
+                layer = (it * reps + r) % L
                 tq.tq_decode_attn(shape, params, cache, layer, 1, qs[layer:layer + 1], outs[layer:layer + 1], ws, None,
                                   max_seq, stream)
-                e2.record(stream)
-                e2.synchronize()
-                if it > 0:
-                    app_ms.append(e0.elapsed_time(e1))
-                    dec_ms.append(e1.elapsed_time(e2))
-    t_live = T0 + 2.5
-    dec_bytes = B * H * t_live * 62
+            e1.record(stream)
+            e1.synchronize()
+            if it > 0:
+                dec_ms.append(e0.elapsed_time(e1) / reps)
+    dec_bytes = B * H * T0 * 62
     dec_s = statistics.mean(dec_ms) * 1e-3
 
     # ---- end to end through the host-buffer call: pinned q/k/v in, out back, every layer of every step
@@ -383,7 +381,7 @@ def run_ours(args, w: W.Workload):
             "cuda_graph": True, "bytes_per_token_head": 62,
             "us_per_layer_step": 1e3 * ms_max / args.steps / L,
             "packed_gbs_whole_step": value / world * 62 / 1e9,
-            "decode_call_us_live": dec_s * 1e6, "append_call_us_live": statistics.mean(app_ms) * 1e3,
+            "decode_call_us_live": dec_s * 1e6,
             "quantize_pack_gbs": quant_gbs, "quantize_pack_ms_per_layer": statistics.median(q_ms),
             "parallelism": f"dp{world} (independent batches, no collective)",
         },

@@ -38,7 +38,10 @@
  *               shared-memory table reads bank-conflict free);
  *     K signs : m/4 nibbles; nibble group n (coordinates 4n..4n+3, bit b = coordinate 4n+b) is stored at
  *               nibble position (n - t) mod (m/4);
- *     V codes : P six-bit fields, pair group g at position g (no rotation);
+ *     V codes : stored per coordinate pair, not per token: "lane" g (< 32) of the tile owns the string of
+ *               pair group g (and g + 32 for d = 128, appended after it); inside it token slot j of the tile
+ *               sits at bits [6j, 6j + 6).  The decode kernel accumulates V with lane = coordinate pair, so
+ *               it needs two fp32 accumulators per lane instead of d;
  *     norms   : three 64-byte arrays of binary16: |k|, |r_k|, |v|.
  *   Bytes per cached token-head: 62 (d = 64), 118 (d = 128) — the same as the canonical format.
  */
@@ -148,6 +151,15 @@ int tq_decode_attn(const tq_shape *shape, const tq_params *dev, const tq_cache *
                    int32_t n_layers_call, const void *q, const int32_t *q_pos, tq_dtype dt, void *out,
                    int32_t t_hint, void *workspace, size_t workspace_bytes, void *cuda_stream);
 
+/* ---- one decode step of one layer, fused: tq_append(k, v) followed by tq_decode_attn(q) with the query at
+ * the newly appended position, in two kernel launches instead of three (the append and the query
+ * preparation share one kernel and the rows of PI_K and S).  q, k, v, out: DEVICE [B][H][d], dtype dt.
+ * Result and cache state are identical to calling the two entry points one after the other
+ * (BASELINE.json:configs[2] "each step appending one quantized token per head via tq_append").            */
+int tq_decode_step(const tq_shape *shape, const tq_params *dev, tq_cache *cache, int32_t layer, const void *q,
+                   const void *k, const void *v, tq_dtype dt, void *out, int32_t t_hint, void *workspace,
+                   size_t workspace_bytes, void *cuda_stream);
+
 /* ---- format conversion (tests, interchange; not hot) -----------------------------------------------
  * Canonical planes are DEVICE arrays for ONE layer, index [b][h][t] with t < n_tokens:
  * k_codes/v_codes 3d/8 bytes per entry, k_signs m/8 bytes, norms uint16.  Export reads tokens
@@ -166,7 +178,7 @@ int tq_cache_import_canonical(const tq_shape *shape, tq_cache *cache, int32_t la
 
 /* ---- host-buffer convenience (the end-to-end path bench.py times as "e2e") -------------------------
  * One decode step for one layer with HOST q/k/v/out ([B][H][d], dtype dt): copies k, v, q to the device
- * staging buffers, runs tq_append + tq_decode_attn, copies out back and synchronises the stream.
+ * staging buffers, runs tq_decode_step, copies out back and synchronises the stream.
  * staging: DEVICE buffer of tq_step_staging_bytes() bytes.                                              */
 size_t tq_step_staging_bytes(const tq_shape *shape, tq_dtype dt);
 int tq_decode_step_host(const tq_shape *shape, const tq_params *dev, tq_cache *cache, int32_t layer,

@@ -21,7 +21,7 @@ TILE_TOKENS = 32
 EXPORTS = [
     "tq_cache_bytes", "tq_cache_bytes_per_token_head", "tq_cache_seq_len_offset", "tq_cache_status_offset",
     "tq_decode_workspace_bytes", "tq_canonical_plane_bytes", "tq_calibrate_host", "tq_quantize_pack", "tq_append",
-    "tq_decode_attn", "tq_cache_export_canonical", "tq_cache_import_canonical", "tq_step_staging_bytes",
+    "tq_decode_attn", "tq_decode_step", "tq_cache_export_canonical", "tq_cache_import_canonical", "tq_step_staging_bytes",
     "tq_decode_step_host", "tq_status_string", "tq_launch_count",
 ]
 
@@ -226,6 +226,15 @@ def tq_decode_attn(shape, params: Params, cache: Cache, layer_begin: int, n_laye
                               C.c_int32(n_layers_call), _ptr(q), _ptr(q_pos), C.c_int(_dtype_code(q)), _ptr(out),
                               C.c_int32(t_hint), _ptr(workspace.data), C.c_size_t(workspace.bytes), _stream_ptr(stream))
     _check(rc, "tq_decode_attn")
+
+
+def tq_decode_step(shape, params: Params, cache: Cache, layer: int, q, k, v, out, workspace: Workspace, t_hint: int = 0,
+                   stream=None):
+    """q, k, v, out: device tensors [B,H,d]: append (k, v), then attend with q at the new position."""
+    rc = lib().tq_decode_step(C.byref(shape), C.byref(params.c), C.byref(cache.c), C.c_int32(layer), _ptr(q), _ptr(k),
+                              _ptr(v), C.c_int(_dtype_code(q)), _ptr(out), C.c_int32(t_hint), _ptr(workspace.data),
+                              C.c_size_t(workspace.bytes), _stream_ptr(stream))
+    _check(rc, "tq_decode_step")
 
 
 def _canon_struct(planes: dict) -> TqCanonical:

@@ -14,7 +14,7 @@ void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
 
 
 constexpr int kMaxSplits = 64;        // = kMaxSegments in tq_decode.cu
-constexpr int kMaxPlanEntries = 1024;  // = kMaxPlanEntries in tq_decode.cu
+constexpr int kMaxPlanEntries = 256;   // = kMaxPlanEntries in tq_decode.cu
 
 static int num_sms() {
   static int cached = -1;
@@ -137,63 +137,41 @@ int tq_quantize_pack(const tq_shape* shape, const tq_params* dev, tq_cache* cach
   return launch_quantize_pack(a, g.D, dt, sms, (cudaStream_t)cuda_stream) == cudaSuccess ? TQ_OK : TQ_ERR_CUDA;
 }
 
-int tq_append(const tq_shape* shape, const tq_params* dev, tq_cache* cache, int32_t layer, const void* k, const void* v,
-              tq_dtype dt, void* cuda_stream) {
-  CacheGeom g;
-  int rc = check_shape(shape, &g);
-  if (rc != TQ_OK) return rc;
-  if ((rc = check_params(dev)) != TQ_OK) return rc;
-  if (!cache || !cache->data || ((uintptr_t)cache->data & 255u)) return TQ_ERR_INVALID_ARG;
-  if (layer < 0 || layer >= g.L || !aligned16(k) || !aligned16(v)) return TQ_ERR_INVALID_ARG;
-  if (dt != TQ_F16 && dt != TQ_F32) return TQ_ERR_INVALID_ARG;
-  if (num_sms() <= 0) return TQ_ERR_CUDA;
-  QuantArgs a;
-  a.cv = make_view(g, cache->data);
-  a.k = k;
-  a.v = v;
-  a.pi_k = dev->pi_k + (size_t)layer * g.H * g.D * g.D;
-  a.pi_v = dev->pi_v + (size_t)layer * g.H * g.D * g.D;
-  a.lut_k = dev->lut_k + (size_t)layer * g.H * 8;
-  a.lut_v = dev->lut_v + (size_t)layer * g.H * 8;
-  a.S = dev->S;
-  a.rope_cs = dev->rope_cs;
-  a.layer = layer;
-  a.n_tokens = 1;
-  a.start_pos = 0;
-  a.rope_layout = shape->rope_layout;
-  a.tiles_per_cta = 1;
-  return launch_append(a, g.D, dt, (cudaStream_t)cuda_stream) == cudaSuccess ? TQ_OK : TQ_ERR_CUDA;
-}
-
-int tq_decode_attn(const tq_shape* shape, const tq_params* dev, const tq_cache* cache, int32_t layer_begin,
-                   int32_t n_layers_call, const void* q, const int32_t* q_pos, tq_dtype dt, void* out, int32_t t_hint,
-                   void* workspace, size_t workspace_bytes, void* cuda_stream) {
+// Shared body of tq_append / tq_decode_attn / tq_decode_step: validation, then per launch chunk
+// [prep kernel (append and/or query prep)] + [streaming decode kernel].
+static int run_decode(const tq_shape* shape, const tq_params* dev, const tq_cache* cache, int32_t layer_begin,
+                      int32_t n_layers_call, const void* q, const void* k, const void* v, const int32_t* q_pos,
+                      tq_dtype dt, void* out, int32_t t_hint, void* workspace, size_t workspace_bytes, bool do_append,
+                      bool do_query, void* cuda_stream) {
   CacheGeom g;
   int rc = check_shape(shape, &g);
   if (rc != TQ_OK) return rc;
   if ((rc = check_params(dev)) != TQ_OK) return rc;
   if (!cache || !cache->data || ((uintptr_t)cache->data & 255u)) return TQ_ERR_INVALID_ARG;
   if (layer_begin < 0 || n_layers_call <= 0 || layer_begin + n_layers_call > g.L) return TQ_ERR_INVALID_ARG;
-  if (!aligned16(q) || !aligned16(out) || !workspace || ((uintptr_t)workspace & 255u)) return TQ_ERR_INVALID_ARG;
   if (dt != TQ_F16 && dt != TQ_F32) return TQ_ERR_INVALID_ARG;
-  if (t_hint < 0) return TQ_ERR_INVALID_ARG;
+  if (do_append && (!aligned16(k) || !aligned16(v))) return TQ_ERR_INVALID_ARG;
   WorkspaceGeom w = workspace_geom(g, n_layers_call);
-  if (workspace_bytes < w.total) return TQ_ERR_CAPACITY;
-  int sms = num_sms();
+  if (do_query) {
+    if (!aligned16(q) || !aligned16(out) || !workspace || ((uintptr_t)workspace & 255u)) return TQ_ERR_INVALID_ARG;
+    if (t_hint < 0) return TQ_ERR_INVALID_ARG;
+    if (workspace_bytes < w.total) return TQ_ERR_CAPACITY;
+    if (g.B > kMaxPlanEntries) return TQ_ERR_UNSUPPORTED;
+  }
+  const int sms = num_sms();
   if (sms <= 0) return TQ_ERR_CUDA;
-  if (g.B > kMaxPlanEntries) return TQ_ERR_UNSUPPORTED;
   const int th = (t_hint == 0 || t_hint > g.max_seq) ? g.max_seq : t_hint;
   const int ntiles = (th + kTile - 1) / kTile;
   // stream-K: one persistent CTA per resident slot; a unit may be cut into at most kMaxSplits segments
   const int min_q = (ntiles + kMaxSplits - 3) / (kMaxSplits - 2);
   int grid_override = 0;
   if (const char* e = getenv("TQ_DECODE_NSPLIT")) {  // profiling / test knob: number of CTAs of the streaming kernel
-    long v = atol(e);
-    if (v >= 1 && v <= 65535) grid_override = (int)v;
+    long vv = atol(e);
+    if (vv >= 1 && vv <= 65535) grid_override = (int)vv;
   }
   const size_t esz = dt == TQ_F16 ? 2 : 4;
   unsigned char* ws = (unsigned char*)workspace;
-  const int layers_per_launch = kMaxPlanEntries / g.B;
+  const int layers_per_launch = do_query ? (kMaxPlanEntries / g.B > 0 ? kMaxPlanEntries / g.B : 1) : n_layers_call;
   for (int l0 = 0; l0 < n_layers_call; l0 += layers_per_launch) {
     const int nl = n_layers_call - l0 < layers_per_launch ? n_layers_call - l0 : layers_per_launch;
     const size_t u0 = (size_t)l0 * g.B * g.H;  // first unit of this launch inside the call
@@ -205,20 +183,43 @@ int tq_decode_attn(const tq_shape* shape, const tq_params* dev, const tq_cache* 
     a.lut_v = dev->lut_v;
     a.S = dev->S;
     a.rope_cs = dev->rope_cs;
-    a.q = (const unsigned char*)q + u0 * g.D * esz;
-    a.out = (unsigned char*)out + u0 * g.D * esz;
+    a.q = q ? (const unsigned char*)q + u0 * g.D * esz : nullptr;
+    a.out = out ? (unsigned char*)out + u0 * g.D * esz : nullptr;
     a.q_pos = q_pos ? q_pos + (size_t)l0 * g.B : nullptr;
-    a.counters = (int*)(ws + w.off_counters) + u0;
-    a.qrot = (float*)(ws + w.off_qrot) + u0 * 2 * g.D;
-    a.partials = (float*)(ws + w.off_partials) + u0 * kMaxSplits * (g.D + 2);
+    a.counters = ws ? (int*)(ws + w.off_counters) + u0 : nullptr;
+    a.qrot = ws ? (float*)(ws + w.off_qrot) + u0 * 2 * g.D : nullptr;
+    a.partials = ws ? (float*)(ws + w.off_partials) + u0 * kMaxSplits * (g.D + 2) : nullptr;
     a.layer_begin = layer_begin + l0;
     a.n_layers_call = nl;
     a.nsplit = grid_override;
     a.rope_layout = shape->rope_layout;
     a.dt = (int)dt;
-    if (launch_decode(a, g.D, sms, min_q, (cudaStream_t)cuda_stream) != cudaSuccess) return TQ_ERR_CUDA;
+    const void* kc = k ? (const unsigned char*)k + u0 * g.D * esz : nullptr;
+    const void* vc = v ? (const unsigned char*)v + u0 * g.D * esz : nullptr;
+    if (launch_prep(a, kc, vc, g.D, do_append, do_query, (cudaStream_t)cuda_stream) != cudaSuccess) return TQ_ERR_CUDA;
+    if (do_query && launch_decode(a, g.D, sms, min_q, (cudaStream_t)cuda_stream) != cudaSuccess) return TQ_ERR_CUDA;
   }
   return TQ_OK;
+}
+
+int tq_append(const tq_shape* shape, const tq_params* dev, tq_cache* cache, int32_t layer, const void* k, const void* v,
+              tq_dtype dt, void* cuda_stream) {
+  return run_decode(shape, dev, cache, layer, 1, nullptr, k, v, nullptr, dt, nullptr, 0, nullptr, 0, true, false,
+                    cuda_stream);
+}
+
+int tq_decode_attn(const tq_shape* shape, const tq_params* dev, const tq_cache* cache, int32_t layer_begin,
+                   int32_t n_layers_call, const void* q, const int32_t* q_pos, tq_dtype dt, void* out, int32_t t_hint,
+                   void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  return run_decode(shape, dev, cache, layer_begin, n_layers_call, q, nullptr, nullptr, q_pos, dt, out, t_hint, workspace,
+                    workspace_bytes, false, true, cuda_stream);
+}
+
+int tq_decode_step(const tq_shape* shape, const tq_params* dev, tq_cache* cache, int32_t layer, const void* q,
+                   const void* k, const void* v, tq_dtype dt, void* out, int32_t t_hint, void* workspace,
+                   size_t workspace_bytes, void* cuda_stream) {
+  return run_decode(shape, dev, cache, layer, 1, q, k, v, nullptr, dt, out, t_hint, workspace, workspace_bytes, true,
+                    true, cuda_stream);
 }
 
 int tq_cache_export_canonical(const tq_shape* shape, const tq_cache* cache, int32_t layer, int32_t n_tokens,
@@ -276,8 +277,7 @@ int tq_decode_step_host(const tq_shape* shape, const tq_params* dev, tq_cache* c
   if (cudaMemcpyAsync(dk, k_host, bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return TQ_ERR_CUDA;
   if (cudaMemcpyAsync(dv, v_host, bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return TQ_ERR_CUDA;
   if (cudaMemcpyAsync(dq, q_host, bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return TQ_ERR_CUDA;
-  if ((rc = tq_append(shape, dev, cache, layer, dk, dv, dt, cuda_stream)) != TQ_OK) return rc;
-  if ((rc = tq_decode_attn(shape, dev, cache, layer, 1, dq, nullptr, dt, dout, t_hint, workspace, workspace_bytes,
+  if ((rc = tq_decode_step(shape, dev, cache, layer, dq, dk, dv, dt, dout, t_hint, workspace, workspace_bytes,
                            cuda_stream)) != TQ_OK)
     return rc;
   if (cudaMemcpyAsync(out_host, dout, bytes, cudaMemcpyDeviceToHost, st) != cudaSuccess) return TQ_ERR_CUDA;

@@ -129,7 +129,8 @@ struct DecodeArgs {
 };
 
 cudaError_t launch_quantize_pack(const QuantArgs& a, int D, tq_dtype dt, int num_sms, cudaStream_t st);
-cudaError_t launch_append(const QuantArgs& a, int D, tq_dtype dt, cudaStream_t st);
+cudaError_t launch_prep(const DecodeArgs& d, const void* k, const void* v, int D, bool do_append, bool do_query,
+                        cudaStream_t st);
 cudaError_t launch_decode(const DecodeArgs& a, int D, int num_sms, int min_q, cudaStream_t st);
 cudaError_t launch_export(const CacheGeom& g, const CacheView& cv, int layer, int n_tokens, const tq_canonical& out,
                           cudaStream_t st);

@@ -24,45 +24,6 @@
 namespace tq {
 
 
-// ------------------------------------------------------------------------------------------ query prep
-template <int D, typename T>
-__global__ void __launch_bounds__(256) decode_prep_kernel(DecodeArgs a) {
-  __shared__ float x[D], y[D];
-  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int uc = blockIdx.x;
-  const int BH = a.cv.B * a.cv.H;
-  const int lc = uc / BH, bh = uc % BH, b = bh / a.cv.H, h = bh % a.cv.H;
-  const int layer = a.layer_begin + lc;
-  const int Tlen = a.cv.seq_len[layer * a.cv.B + b];
-  int pos = a.q_pos ? a.q_pos[lc * a.cv.B + b] : Tlen - 1;
-  pos = max(0, min(pos, a.cv.max_seq - 1));
-  constexpr int HP = D / 2;
-  if (Tlen <= 0) {  // empty cache: the main kernel has no tile for this unit, the output is defined as 0
-    T* outp = reinterpret_cast<T*>(a.out) + (size_t)uc * D;
-    for (int i = tid; i < D; i += 256) {
-      if constexpr (sizeof(T) == 2) outp[i] = __float2half_rn(0.f);
-      else outp[i] = 0.f;
-    }
-    return;
-  }
-  const T* qp = reinterpret_cast<const T*>(a.q) + (size_t)uc * D;
-  for (int g = tid; g < HP; g += 256) {
-    int ia = a.rope_layout == 0 ? 2 * g : g, ib = a.rope_layout == 0 ? 2 * g + 1 : g + HP;
-    float xa = load_as_float<T>(qp + ia), xb = load_as_float<T>(qp + ib);
-    float2 cs = *reinterpret_cast<const float2*>(a.rope_cs + ((size_t)pos * HP + g) * 2);
-    x[ia] = xa * cs.x - xb * cs.y;
-    x[ib] = xa * cs.y + xb * cs.x;
-  }
-  __syncthreads();
-  matvec_rows_ilp<D, 8>(a.pi_k + ((size_t)layer * a.cv.H + h) * D * D, x, y, warp, lane);
-  __syncthreads();
-  float* dst = a.qrot + (size_t)uc * 2 * D;
-  for (int i = tid; i < D; i += 256) dst[i] = y[i];
-  matvec_rows_ilp<D, 8>(a.S, y, x, warp, lane);
-  __syncthreads();
-  for (int i = tid; i < D; i += 256) dst[D + i] = x[i];
-}
-
 // ------------------------------------------------------------------------------------------ smem helpers
 template <int IMM>
 __device__ __forceinline__ float lds_f32(unsigned addr) {
@@ -91,6 +52,11 @@ __device__ __forceinline__ unsigned field_at(const unsigned (&w)[NW]) {
   return v & mask;
 }
 
+constexpr int kMaxPlanEntries = 256;  // (layers in one launch) x batch
+constexpr int kMaxSegments = 64;      // split-K partial slots per unit (tq_api.cu sizes the workspace)
+constexpr int kDecodeThreads = 128;
+constexpr int kDecodeWarps = kDecodeThreads / 32;
+
 // Shared-memory map in ABSOLUTE shared-window addresses (the OR-addressing needs the K/V tables aligned to
 // their own size, the sign table to 4 KB).  Dynamic shared memory starts right after the 1 KB the driver
 // reserves, so everything is placed at fixed absolute addresses and the kernel traps if the window starts
@@ -101,16 +67,18 @@ struct DecodeCfg {
   static constexpr int NCK = D;                          // columns of the K table = 2 P (>= P + 31)
   static constexpr int LSK = D == 64 ? 8 : 9;            // log2(NCK * 4)
   static constexpr int kKtabBytes = 64 * NCK * 4;        // 16 KB | 32 KB
-  static constexpr int kVtabBytes = 64 * 32 * 8;         // 16 KB
+  static constexpr int kVtabBytes = 64 * 16 * 8;         // 8 KB: [entry][lane mod 16] float2 (64-bit reads are
+                                                         // served one half-warp at a time)
   static constexpr int kStabBytes = 16 * 64 * 4;         // 4 KB
-  static constexpr unsigned kAbsWbuf = 2048;             // 8 warps x 32 softmax weights, then the arrival flag
+  static constexpr unsigned kAbsWbuf = 2048;             // 4 warps x 32 softmax weights, then the arrival flag
   static constexpr unsigned kAbsStab = 4096;
-  static constexpr unsigned kAbsScratch = 8192;          // plan prefix, per-warp partials, merged o (8 KB)
-  static constexpr unsigned kAbsKtab = kKtabBytes;       // 16384 | 32768
-  static constexpr unsigned kAbsVtab = kAbsKtab + kKtabBytes;
-  static constexpr unsigned kAbsEnd = kAbsVtab + kVtabBytes;
-  static constexpr int kSmemBytes = kAbsEnd;             // requested dynamic bytes (window start <= 4 KB)
-  static constexpr int kCtasPerSm = D == 64 ? 3 : 2;
+  static constexpr unsigned kAbsVtab = 8192;
+  static constexpr unsigned kAbsKtab = D == 64 ? 16384 : 32768;
+  static constexpr unsigned kAbsScratch = D == 64 ? 32768 : 16384;  // plan prefix, per-warp partials, merged o
+  static constexpr int kScratchBytes = (kMaxPlanEntries + 1) * 4 + 12 + 4 * (D + 2) * 4 + 2 * D * 4;
+  static constexpr unsigned kAbsEnd = D == 64 ? kAbsScratch + kScratchBytes : kAbsKtab + kKtabBytes;
+  static constexpr int kSmemBytes = kAbsEnd;             // requested dynamic bytes (window start <= 2 KB)
+  static constexpr int kCtasPerSm = D == 64 ? 6 : 3;
 };
 
 // ---- packed fp32x2 arithmetic (sm_100: FFMA2 / FADD2 / FMUL2 issue two fp32 operations per slot) ----------
@@ -145,27 +113,31 @@ __device__ __forceinline__ f32x2 lds_b64(unsigned addr) {
 }
 
 // <q'', lut_K[codes]>: P table reads, summed two at a time
+template <int D, int K>
+__device__ __forceinline__ f32x2 k_pair(const unsigned (&kw)[Layout<D>::KCW], unsigned kbase) {
+  return pack2(lds_f32<8 * K>(field_at<DecodeCfg<D>::LSK, 12 * K, 6>(kw) | kbase),
+               lds_f32<8 * K + 4>(field_at<DecodeCfg<D>::LSK, 12 * K + 6, 6>(kw) | kbase));
+}
 template <int D, int... K>
 __device__ __forceinline__ float k_score(const unsigned (&kw)[Layout<D>::KCW], unsigned kbase,
                                          std::integer_sequence<int, K...>) {
-  f32x2 acc[2] = {0ull, 0ull};
-  ((acc[K & 1] = add2(acc[K & 1],
-                      pack2(lds_f32<8 * K>(field_at<DecodeCfg<D>::LSK, 12 * K, 6>(kw) | kbase),
-                            lds_f32<8 * K + 4>(field_at<DecodeCfg<D>::LSK, 12 * K + 6, 6>(kw) | kbase)))),
-   ...);
+  f32x2 acc[2] = {k_pair<D, 0>(kw, kbase), k_pair<D, 1>(kw, kbase)};
+  ((acc[K & 1] = add2(acc[K & 1], k_pair<D, K + 2>(kw, kbase))), ...);
   float a, b;
   unpack2(add2(acc[0], acc[1]), a, b);
   return a + b;
 }
 
 // <z, sigma>: d/4 nibble-table reads
+template <int D, int K>
+__device__ __forceinline__ f32x2 s_pair(const unsigned (&sw)[Layout<D>::KSW], unsigned sbase) {
+  return pack2(lds_f32<8 * K>(field_at<8, 8 * K, 4>(sw) | sbase), lds_f32<8 * K + 4>(field_at<8, 8 * K + 4, 4>(sw) | sbase));
+}
 template <int D, int... K>
 __device__ __forceinline__ float s_score(const unsigned (&sw)[Layout<D>::KSW], unsigned sbase,
                                          std::integer_sequence<int, K...>) {
-  f32x2 acc[2] = {0ull, 0ull};
-  ((acc[K & 1] = add2(acc[K & 1], pack2(lds_f32<8 * K>(field_at<8, 8 * K, 4>(sw) | sbase),
-                                        lds_f32<8 * K + 4>(field_at<8, 8 * K + 4, 4>(sw) | sbase)))),
-   ...);
+  f32x2 acc[2] = {s_pair<D, 0>(sw, sbase), s_pair<D, 1>(sw, sbase)};
+  ((acc[K & 1] = add2(acc[K & 1], s_pair<D, K + 2>(sw, sbase))), ...);
   float a, b;
   unpack2(add2(acc[0], acc[1]), a, b);
   return a + b;
@@ -174,17 +146,17 @@ __device__ __forceinline__ float s_score(const unsigned (&sw)[Layout<D>::KSW], u
 // V accumulate, lane = coordinate pair: for token J of the tile, o2[part] += w_J * (lut_V[c0], lut_V[c1])
 template <int D, int J>
 __device__ __forceinline__ void v_token(const unsigned (&vw)[Layout<D>::KCW], unsigned vbase, float w,
-                                        f32x2 (&o2)[Layout<D>::P / kTile]) {
+                                        f32x2 (&o2)[2 * (Layout<D>::P / kTile)]) {
   const f32x2 w2 = pack2(w, w);
 #pragma unroll
   for (int part = 0; part < Layout<D>::P / kTile; ++part) {
-    unsigned f = part == 0 ? field_at<8, 6 * J, 6>(vw) : field_at<8, 192 * (Layout<D>::P / kTile - 1) + 6 * J, 6>(vw);
-    o2[part] = fma2(lds_b64(f | vbase), w2, o2[part]);
+    unsigned f = part == 0 ? field_at<7, 6 * J, 6>(vw) : field_at<7, 192 * (Layout<D>::P / kTile - 1) + 6 * J, 6>(vw);
+    o2[2 * part + (J & 1)] = fma2(lds_b64(f | vbase), w2, o2[2 * part + (J & 1)]);
   }
 }
 template <int D, int... J>
 __device__ __forceinline__ void v_accum(const unsigned (&vw)[Layout<D>::KCW], unsigned vbase, unsigned wbuf,
-                                        f32x2 (&o2)[Layout<D>::P / kTile], std::integer_sequence<int, J...>) {
+                                        f32x2 (&o2)[2 * (Layout<D>::P / kTile)], std::integer_sequence<int, J...>) {
   // w of tokens 4J .. 4J+3 arrive with one broadcast 128-bit read
   (([&] {
      float4 w4;
@@ -237,11 +209,9 @@ __device__ __forceinline__ void load_tile_words(TileWords<D>& t, const unsigned 
   t.vn = __ldg(reinterpret_cast<const unsigned short*>(tp + Lo::kOffVN) + lane);
 }
 
-constexpr int kMaxSegments = 64;       // split-K partial slots per unit (tq_api.cu sizes the workspace)
-constexpr int kDecodeThreads = 256;
-constexpr int kDecodeWarps = kDecodeThreads / 32;
 
 // ---- table construction (per unit; pre-scaled so that logits come out in log2 units) ---------------------
+// Every thread owns four consecutive table columns and writes them with 128-bit stores.
 template <int D>
 __device__ __forceinline__ void build_k_tables(float* Ktab, float* Stab, const float* qr, const float* __restrict__ lk,
                                                int tid) {
@@ -249,48 +219,57 @@ __device__ __forceinline__ void build_k_tables(float* Ktab, float* Stab, const f
   using Cfg = DecodeCfg<D>;
   const float sc_k = 1.4426950408889634f * rsqrtf((float)D);
   const float sc_s = sc_k * 1.2533141373155003f / (float)D;  // log2(e)/sqrt(d) * sqrt(pi/2)/m, m = D
-  {  // Ktab[e][c] = (q''_{2g} lut[e & 7] + q''_{2g+1} lut[e >> 3]) * sc_k,  g = c mod P, both copies c = g, g + P
-    constexpr int EG = kDecodeThreads / Lo::P;  // entry groups: 8 (D = 64) | 4 (D = 128)
-    constexpr int EPT = 64 / EG;                // entries per thread: 8 | 16
-    const int g = tid % Lo::P, eq = tid / Lo::P;
-    const float q0 = __ldcg(qr + 2 * g) * sc_k, q1 = __ldcg(qr + 2 * g + 1) * sc_k;
-    float a0[8], a1[EPT / 8];
+  const float4 l0 = __ldg(reinterpret_cast<const float4*>(lk)), l1 = __ldg(reinterpret_cast<const float4*>(lk) + 1);
+  const float lut[8] = {l0.x, l0.y, l0.z, l0.w, l1.x, l1.y, l1.z, l1.w};
+  {  // Ktab[8 hi + lo][c] = (q''_{2g} lut[lo] + q''_{2g+1} lut[hi]) * sc_k,  g = c mod P
+    constexpr int NQ = Cfg::NCK / 4;            // column quads: 16 | 32
+    constexpr int HPT = 8 / (kDecodeThreads / NQ);  // hi codes per thread: 1 | 2
+    const int cq = tid % NQ, eg = tid / NQ;
+    const int g0 = (4 * cq) % Lo::P;
+    const float4 qa = __ldcg(reinterpret_cast<const float4*>(qr + 2 * g0));
+    const float4 qb = __ldcg(reinterpret_cast<const float4*>(qr + 2 * g0) + 1);
+    const float q0[4] = {qa.x * sc_k, qa.z * sc_k, qb.x * sc_k, qb.z * sc_k};  // q''_{2g}
+    const float q1[4] = {qa.y * sc_k, qa.w * sc_k, qb.y * sc_k, qb.w * sc_k};  // q''_{2g+1}
 #pragma unroll
-    for (int c = 0; c < 8; ++c) a0[c] = q0 * __ldg(lk + c);
+    for (int hh = 0; hh < HPT; ++hh) {
+      const int hi = eg * HPT + hh;
+      float lh = lut[0];
 #pragma unroll
-    for (int jj = 0; jj < EPT / 8; ++jj) a1[jj] = q1 * __ldg(lk + eq * (EPT / 8) + jj);
-    float* dst = Ktab + (size_t)(eq * EPT) * Cfg::NCK + g;
+      for (int c = 1; c < 8; ++c) lh = (hi == c) ? lut[c] : lh;
+      const float b0 = q1[0] * lh, b1 = q1[1] * lh, b2 = q1[2] * lh, b3 = q1[3] * lh;
+      float* dst = Ktab + (size_t)(hi * 8) * Cfg::NCK + 4 * cq;
 #pragma unroll
-    for (int j = 0; j < EPT; ++j) {
-      const float v = a0[j & 7] + a1[j >> 3];
-      dst[j * Cfg::NCK] = v;
-      dst[j * Cfg::NCK + Lo::P] = v;
+      for (int lo = 0; lo < 8; ++lo)
+        *reinterpret_cast<float4*>(dst + lo * Cfg::NCK) =
+            make_float4(fmaf(q0[0], lut[lo], b0), fmaf(q0[1], lut[lo], b1), fmaf(q0[2], lut[lo], b2), fmaf(q0[3], lut[lo], b3));
     }
   }
-  if (tid < 128) {  // Stab[e][c] = sum_b (bit b of e ? +z : -z)[4n + b] * sc_s,  n = c mod NG, all 64 / NG copies
-    constexpr int TG = 128 / Lo::NG;  // thread groups: 8 | 4
-    constexpr int EPT = 16 / TG;      // entries per thread: 2 | 4
-    const int n = tid % Lo::NG, eq = tid / Lo::NG;
-    float z[4];
+  {  // Stab[e][c] = sum_b (bit b of e ? +z : -z)[4n + b] * sc_s,  n = c mod NG; 16 column quads x 8 entry pairs
+    const int cq = tid % 16, eg = tid / 16;
+    const int n0 = (4 * cq) % Lo::NG;
+    float4 zz[4];
 #pragma unroll
-    for (int b = 0; b < 4; ++b) z[b] = __ldcg(qr + D + 4 * n + b) * sc_s;
+    for (int i = 0; i < 4; ++i) {
+      zz[i] = __ldcg(reinterpret_cast<const float4*>(qr + D + 4 * (n0 + i)));
+      zz[i].x *= sc_s, zz[i].y *= sc_s, zz[i].z *= sc_s, zz[i].w *= sc_s;
+    }
 #pragma unroll
-    for (int j = 0; j < EPT; ++j) {
-      const int e = eq * EPT + j;
-      float v = 0.f;
+    for (int j = 0; j < 2; ++j) {
+      const int e = 2 * eg + j;
+      const float s0 = (e & 1) ? 1.f : -1.f, s1 = (e & 2) ? 1.f : -1.f, s2 = (e & 4) ? 1.f : -1.f, s3 = (e & 8) ? 1.f : -1.f;
+      float v[4];
 #pragma unroll
-      for (int b = 0; b < 4; ++b) v += ((e >> b) & 1) ? z[b] : -z[b];
-#pragma unroll
-      for (int cp = 0; cp < 64 / Lo::NG; ++cp) Stab[e * 64 + n + cp * Lo::NG] = v;
+      for (int i = 0; i < 4; ++i) v[i] = fmaf(s0, zz[i].x, fmaf(s1, zz[i].y, fmaf(s2, zz[i].z, s3 * zz[i].w)));
+      *reinterpret_cast<float4*>(Stab + e * 64 + 4 * cq) = make_float4(v[0], v[1], v[2], v[3]);
     }
   }
 }
 
 __device__ __forceinline__ void build_v_table(float2* Vtab, const float* __restrict__ lv, int tid) {
-  const int lane = tid & 31, eq = tid >> 5;  // 8 warps: entries 8 eq .. 8 eq + 7, i.e. hi code = eq
+  const int col = tid & 15, eq = tid >> 4;  // 128 threads: hi code = eq, entries 8 eq .. 8 eq + 7
   const float hi = __ldg(lv + eq);
 #pragma unroll
-  for (int j = 0; j < 8; ++j) Vtab[(eq * 8 + j) * 32 + lane] = make_float2(__ldg(lv + j), hi);
+  for (int j = 0; j < 8; ++j) Vtab[(eq * 8 + j) * 16 + col] = make_float2(__ldg(lv + j), hi);
 }
 
 // ---- the streaming kernel ------------------------------------------------------------------------------------
@@ -310,8 +289,8 @@ __global__ void __launch_bounds__(kDecodeThreads, DecodeCfg<D>::kCtasPerSm) deco
   unsigned char* abs0 = smem_raw - raw;  // generic pointer to absolute shared address 0 of this CTA's window
   float* Stab = reinterpret_cast<float*>(abs0 + Cfg::kAbsStab);
   int* plan = reinterpret_cast<int*>(abs0 + Cfg::kAbsScratch);            // [E + 1] exclusive prefix of tiles
-  float* red = reinterpret_cast<float*>(abs0 + Cfg::kAbsScratch + 4608);  // NW x (D + 2)
-  float* omerged = red + NW * (D + 2);                                     // [D] + [3 D] partial matvecs
+  float* red = reinterpret_cast<float*>(abs0 + Cfg::kAbsScratch + (kMaxPlanEntries + 1) * 4 + 12);  // NW x (D + 2)
+  float* omerged = red + NW * (D + 2);                                     // [D] + [D] partial matvec
   float* wbuf_f = reinterpret_cast<float*>(abs0 + Cfg::kAbsWbuf);         // NW x 32 softmax weights
   int* flag = reinterpret_cast<int*>(wbuf_f + NW * 32);
   float* Ktab = reinterpret_cast<float*>(abs0 + Cfg::kAbsKtab);
@@ -354,7 +333,9 @@ __global__ void __launch_bounds__(kDecodeThreads, DecodeCfg<D>::kCtasPerSm) deco
   const int fend = min(total, f + Q);
   if (f >= fend) return;
 
-  const unsigned kbase = ktab + lane * 4, sbase = stab + lane * 4, vbase = vtab + lane * 8;
+  // table base | lane column, kept opaque so that the compiler ORs it in with a single LOP3 per lookup
+  unsigned kbase = ktab + lane * 4, sbase = stab + lane * 4, vbase = vtab + (lane & 15) * 8;
+  asm volatile("" : "+r"(kbase), "+r"(sbase), "+r"(vbase));
   const unsigned wbuf = (unsigned)__cvta_generic_to_shared(wbuf_f + warp * 32);
   int vtab_owner = -1;  // (layer, head) the V table currently holds
 
@@ -383,6 +364,16 @@ __global__ void __launch_bounds__(kDecodeThreads, DecodeCfg<D>::kCtasPerSm) deco
     const int cfirst = ustart / Q, clast = (ustart + nt - 1) / Q;
     const int nseg = clast - cfirst + 1, slot = (int)blockIdx.x - cfirst;
 
+    // ---- start the memory system on this segment before anything else: one bulk L2 prefetch of all its
+    //      bytes, and this warp's first tile into registers
+    const unsigned char* stream = a.cv.tiles + ((size_t)layer * B * H + (size_t)b * H + h) * a.cv.stream_bytes;
+    if (tid == 0)
+      asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(stream + (size_t)tile0 * Lo::kTileBytes),
+                   "r"((tile1 - tile0) * Lo::kTileBytes)
+                   : "memory");
+    TileWords<D> bufA, bufB;  // register double buffer, ping-pong (no copies)
+    if (tile0 + warp < tile1) load_tile_words<D>(bufA, stream + (size_t)(tile0 + warp) * Lo::kTileBytes, lane);
+
     // ---- tables of this unit
     __syncthreads();  // every warp is done with the previous unit's tables and scratch
     build_k_tables<D>(Ktab, Stab, a.qrot + (size_t)uc * 2 * D, a.lut_k + ((size_t)layer * H + h) * 8, tid);
@@ -392,24 +383,17 @@ __global__ void __launch_bounds__(kDecodeThreads, DecodeCfg<D>::kCtasPerSm) deco
     }
     __syncthreads();
 
-    const unsigned char* stream = a.cv.tiles + ((size_t)layer * B * H + (size_t)b * H + h) * a.cv.stream_bytes;
-    f32x2 o2[VP];
+    f32x2 o2[2 * VP];  // [pair][even / odd tokens]
 #pragma unroll
-    for (int i = 0; i < VP; ++i) o2[i] = 0ull;
+    for (int i = 0; i < 2 * VP; ++i) o2[i] = 0ull;
     float m = -INFINITY, l = 0.f;
 
-    TileWords<D> cur, nxt;
-    int tile = tile0 + warp;
-    if (tile < tile1) load_tile_words<D>(cur, stream + (size_t)tile * Lo::kTileBytes, lane);
-    for (; tile < tile1; tile += NW) {
-      const bool has_next = tile + NW < tile1;
-      if (has_next) load_tile_words<D>(nxt, stream + (size_t)(tile + NW) * Lo::kTileBytes, lane);
-      if (tile + 2 * NW < tile1 && lane < (Lo::kTileBytes + 127) / 128)  // pull the tile after next into L2
-        asm volatile("prefetch.global.L2 [%0];" ::"l"(stream + (size_t)(tile + 2 * NW) * Lo::kTileBytes + lane * 128));
+    // one 32-token tile: scores (lane = token) -> online softmax -> V accumulate (lane = coordinate pair)
+    auto process = [&](const TileWords<D>& tw, int tile) {
       const bool valid = tile * kTile + lane < T;
-      const float sa = k_score<D>(cur.kw, kbase, std::make_integer_sequence<int, Lo::P / 2>{});
-      const float sb = s_score<D>(cur.sw, sbase, std::make_integer_sequence<int, Lo::NG / 2>{});
-      float s2 = f16_bits_to_f32(cur.kn) * fmaf(f16_bits_to_f32(cur.kr), sb, sa);
+      const float sa = k_score<D>(tw.kw, kbase, std::make_integer_sequence<int, Lo::P / 2 - 2>{});
+      const float sb = s_score<D>(tw.sw, sbase, std::make_integer_sequence<int, Lo::NG / 2 - 2>{});
+      float s2 = f16_bits_to_f32(tw.kn) * fmaf(f16_bits_to_f32(tw.kr), sb, sa);
       s2 = valid ? s2 : -INFINITY;
       const float mnew = fmaxf(m, warp_max(s2));  // finite: slot 0 of every processed tile is valid
       const float fsc = exp2f(m - mnew);          // 0 on a warp's first tile (m = -inf)
@@ -418,13 +402,25 @@ __global__ void __launch_bounds__(kDecodeThreads, DecodeCfg<D>::kCtasPerSm) deco
       l = fmaf(l, fsc, p);
       const f32x2 fsc2 = pack2(fsc, fsc);
 #pragma unroll
-      for (int i = 0; i < VP; ++i) o2[i] = mul2(o2[i], fsc2);
+      for (int i = 0; i < 2 * VP; ++i) o2[i] = mul2(o2[i], fsc2);
       // hand the softmax weights from lane = token to lane = coordinate pair through shared memory
       __syncwarp();
-      asm volatile("st.shared.f32 [%0], %1;" ::"r"(wbuf + lane * 4), "f"(valid ? p * f16_bits_to_f32(cur.vn) : 0.f));
+      asm volatile("st.shared.f32 [%0], %1;" ::"r"(wbuf + lane * 4), "f"(valid ? p * f16_bits_to_f32(tw.vn) : 0.f));
       __syncwarp();
-      v_accum<D>(cur.vw, vbase, wbuf, o2, std::make_integer_sequence<int, kTile / 4>{});
-      if (has_next) cur = nxt;
+      v_accum<D>(tw.vw, vbase, wbuf, o2, std::make_integer_sequence<int, kTile / 4>{});
+    };
+    auto fetch = [&](TileWords<D>& tw, int tile) {
+      if (tile < tile1) load_tile_words<D>(tw, stream + (size_t)tile * Lo::kTileBytes, lane);
+    };
+    int tile = tile0 + warp;
+    while (tile < tile1) {
+      fetch(bufB, tile + NW);
+      process(bufA, tile);
+      tile += NW;
+      if (tile >= tile1) break;
+      fetch(bufA, tile + NW);
+      process(bufB, tile);
+      tile += NW;
     }
 
     // ---- reduce over the CTA's warps (lanes already own distinct coordinates)
@@ -437,7 +433,7 @@ __global__ void __launch_bounds__(kDecodeThreads, DecodeCfg<D>::kCtasPerSm) deco
 #pragma unroll
     for (int i = 0; i < VP; ++i) {
       float x0, x1;
-      unpack2(o2[i], x0, x1);
+      unpack2(add2(o2[2 * i], o2[2 * i + 1]), x0, x1);
       wr[2 + 2 * (lane + kTile * i)] = x0;
       wr[2 + 2 * (lane + kTile * i) + 1] = x1;
     }
@@ -463,17 +459,17 @@ __global__ void __launch_bounds__(kDecodeThreads, DecodeCfg<D>::kCtasPerSm) deco
         part[0] = M;
         part[1] = Lsum;
       }
-      __threadfence();
       __syncthreads();
-      if (tid == 0) {
+      if (tid == 0) {  // release: the barrier orders the CTA's partial stores before this fence (cumulativity)
+        __threadfence();
         const int old = atomicAdd(&a.counters[uc], 1);
         *flag = (old == nseg - 1);
         if (old == nseg - 1) a.counters[uc] = 0;
+        __threadfence();  // acquire side for the CTA that merges
       }
       __syncthreads();
       finish = *flag != 0;
       if (finish) {
-        __threadfence();
         const float* pp = a.partials + (size_t)uc * kMaxSegments * (D + 2);
         M = -INFINITY;
         for (int s = 0; s < nseg; ++s) M = fmaxf(M, __ldcg(pp + s * (D + 2)));
@@ -492,14 +488,14 @@ __global__ void __launch_bounds__(kDecodeThreads, DecodeCfg<D>::kCtasPerSm) deco
     if (finish) {  // out = PI_V^T (o' / l): the k range is split over the 256 / D thread groups
       if (tid < D) omerged[tid] = Lsum > 0.f ? oi / Lsum : 0.f;
       __syncthreads();
-      constexpr int PARTS = kDecodeThreads / D;  // 4 | 2
-      constexpr int KP = D / PARTS;              // 16 | 64
+      constexpr int PARTS = kDecodeThreads / D;  // 2 | 1
+      constexpr int KP = D / PARTS;              // 32 | 128
       const int i = tid % D, part = tid / D;
       const float* Pv = a.pi_v + ((size_t)layer * H + h) * D * D + (size_t)part * KP * D + i;
       float r = 0.f;
-#pragma unroll 16
+#pragma unroll 32
       for (int k = 0; k < KP; ++k) r = fmaf(__ldg(Pv + (size_t)k * D), omerged[part * KP + k], r);
-      if (part > 0) omerged[part * D + i] = r;
+      if (PARTS > 1 && part > 0) omerged[part * D + i] = r;
       __syncthreads();
       if (part == 0) {
 #pragma unroll
@@ -524,11 +520,7 @@ __global__ void __launch_bounds__(kDecodeThreads, DecodeCfg<D>::kCtasPerSm) deco
 // ------------------------------------------------------------------------------------------ launchers
 template <int D, typename T>
 static cudaError_t launch_decode_t(const DecodeArgs& a, int num_sms, int min_q, cudaStream_t st) {
-  const int units = a.n_layers_call * a.cv.B * a.cv.H;
-  decode_prep_kernel<D, T><<<units, 256, 0, st>>>(a);
-  count_launch();
-  cudaError_t e = cudaGetLastError();
-  if (e != cudaSuccess) return e;
+  cudaError_t e;
   constexpr int smem = DecodeCfg<D>::kSmemBytes;
   static bool attr_set = false;
   if (!attr_set) {

@@ -262,138 +262,6 @@ __global__ void __launch_bounds__(2 * D) quantize_pack_kernel(QuantArgs a) {
   }
 }
 
-// ---- single-token append --------------------------------------------------------------------------------
-// One CTA (256 threads) per (batch, head).  Matrix rows are read straight from global/L2, a batch of rows
-// per warp with all loads in flight at once (matvec_rows_ilp); the token lands at index seq_len[layer][b],
-// which the last-arriving head of batch entry b then increments (BASELINE.json:configs[2]).
-template <int D, typename T>
-__global__ void __launch_bounds__(256) append_kernel(QuantArgs a) {
-  using Lo = Layout<D>;
-  __shared__ float xk[D], xv[D], yk[D], yv[D], r[D], sr[D];
-  __shared__ unsigned char cK[D], cV[D], bK[D];
-  __shared__ float nrm[4];
-  __shared__ float lutK[8], lutV[8];
-  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int bh = blockIdx.x;
-  const int b = bh / a.cv.H, h = bh % a.cv.H;
-  const int lb = a.layer * a.cv.B + b;
-  const int pos = a.cv.seq_len[lb];
-  const bool full = pos >= a.cv.max_seq;
-  constexpr int HP = D / 2;
-  if (tid < 8) lutK[tid] = a.lut_k[h * 8 + tid];
-  if (tid >= 32 && tid < 40) lutV[tid - 32] = a.lut_v[h * 8 + tid - 32];
-  if (!full) {
-    const T* kp = reinterpret_cast<const T*>(a.k) + (size_t)bh * D;
-    const T* vp = reinterpret_cast<const T*>(a.v) + (size_t)bh * D;
-    if (tid < HP) {
-      const int g = tid;
-      int ia = a.rope_layout == 0 ? 2 * g : g, ib = a.rope_layout == 0 ? 2 * g + 1 : g + HP;
-      float xa = load_as_float<T>(kp + ia), xb = load_as_float<T>(kp + ib);
-      float2 cs = *reinterpret_cast<const float2*>(a.rope_cs + ((size_t)pos * HP + g) * 2);
-      xk[ia] = xa * cs.x - xb * cs.y;
-      xk[ib] = xa * cs.y + xb * cs.x;
-    } else if (tid >= 128 && tid < 128 + D) {
-      xv[tid - 128] = load_as_float<T>(vp + tid - 128);
-    }
-    __syncthreads();
-    matvec_rows_ilp<D, 8>(a.pi_k + (size_t)h * D * D, xk, yk, warp, lane);
-    matvec_rows_ilp<D, 8>(a.pi_v + (size_t)h * D * D, xv, yv, warp, lane);
-    __syncthreads();
-    if (warp < 2) {  // warp 0: |y_k|, warp 1: |y_v|
-      const float* y = warp == 0 ? yk : yv;
-      float p = 0.f;
-#pragma unroll
-      for (int i = lane; i < D; i += 32) p = fmaf(y[i], y[i], p);
-      p = warp_sum(p);
-      if (lane == 0) nrm[warp] = sqrtf(p);
-    }
-    __syncthreads();
-    const float n = nrm[0], nv = nrm[1];
-    if (tid < D) {
-      float thr[7];
-#pragma unroll
-      for (int q = 0; q < 7; ++q) thr[q] = 0.5f * (lutK[q] + lutK[q + 1]);
-      const float u = n > 0.f ? yk[tid] / n : 0.f;
-      const int c = code_of(u, thr);
-      cK[tid] = (unsigned char)c;
-      r[tid] = u - lutK[c];
-    } else if (tid >= 128 && tid < 128 + D) {
-      const int i = tid - 128;
-      float thr[7];
-#pragma unroll
-      for (int q = 0; q < 7; ++q) thr[q] = 0.5f * (lutV[q] + lutV[q + 1]);
-      const float u = nv > 0.f ? yv[i] / nv : 0.f;
-      cV[i] = (unsigned char)code_of(u, thr);
-    }
-    __syncthreads();
-    if (warp == 0) {
-      float p = 0.f;
-#pragma unroll
-      for (int i = lane; i < D; i += 32) p = fmaf(r[i], r[i], p);
-      p = warp_sum(p);
-      if (lane == 0) nrm[2] = sqrtf(p);
-    }
-    matvec_rows_ilp<D, 8>(a.S, r, sr, warp, lane);
-    __syncthreads();
-    if (tid < D) bK[tid] = sr[tid] >= 0.f ? 1 : 0;
-    __syncthreads();
-    // ---- assemble this token's words
-    const size_t unit = (size_t)a.layer * a.cv.B * a.cv.H + bh;
-    unsigned char* tp = a.cv.tiles + unit * a.cv.stream_bytes + (size_t)(pos / kTile) * Lo::kTileBytes;
-    const int slot = pos % kTile;
-    if (tid < Lo::KCW) {
-      const int w = tid;
-      unsigned long long word = 0;
-      const int k_lo = (32 * w) / 6, k_hi = (32 * w + 31) / 6;
-      for (int kf = k_lo; kf <= k_hi; ++kf) {
-        const int g = (kf + slot) % Lo::P;
-        unsigned long long f = cK[2 * g] | ((unsigned)cK[2 * g + 1] << 3);
-        const int sh = 6 * kf - 32 * w;
-        word |= sh >= 0 ? (f << sh) : (f >> (-sh));
-      }
-      *reinterpret_cast<unsigned*>(tp + Lo::kOffKC + word_offset(Lo::KCW, w, slot)) = (unsigned)word;
-    } else if (tid >= 32 && tid < 32 + Lo::KSW) {
-      const int w = tid - 32;
-      unsigned word = 0;
-      for (int kn = 0; kn < 8; ++kn) {
-        const int ng = (8 * w + kn + slot) % Lo::NG;
-        unsigned nib = bK[4 * ng] | (bK[4 * ng + 1] << 1) | (bK[4 * ng + 2] << 2) | (bK[4 * ng + 3] << 3);
-        word |= nib << (4 * kn);
-      }
-      *reinterpret_cast<unsigned*>(tp + Lo::kOffKS + word_offset(Lo::KSW, w, slot)) = word;
-    } else if (tid >= 64 && tid < 64 + Lo::P) {
-      // V: pair group g lives in lane (g mod 32)'s string at bits [192 part + 6 slot, +6): read-modify-write
-      const int g = tid - 64, vl = g % kTile, part = g / kTile;
-      const unsigned f = cV[2 * g] | ((unsigned)cV[2 * g + 1] << 3);
-      const int bit = 192 * part + 6 * slot, s = bit & 31;
-      unsigned* p0 = reinterpret_cast<unsigned*>(tp + Lo::kOffVC + word_offset(Lo::KCW, bit >> 5, vl));
-      *p0 = (*p0 & ~(63u << s)) | (f << s);
-      if (s > 26) {
-        unsigned* p1 = reinterpret_cast<unsigned*>(tp + Lo::kOffVC + word_offset(Lo::KCW, (bit >> 5) + 1, vl));
-        *p1 = (*p1 & ~(63u >> (32 - s))) | (f >> (32 - s));
-      }
-    } else if (tid == 192) {
-      reinterpret_cast<unsigned short*>(tp + Lo::kOffKN)[slot] = f32_to_f16_bits_clamped(n);
-      reinterpret_cast<unsigned short*>(tp + Lo::kOffKR)[slot] = f32_to_f16_bits_clamped(nrm[2]);
-      reinterpret_cast<unsigned short*>(tp + Lo::kOffVN)[slot] = f32_to_f16_bits_clamped(nv);
-    }
-  }
-  // ---- arrival: the last head of batch entry b publishes the new length
-  __syncthreads();
-  if (tid == 0) {
-    __threadfence();
-    int old = atomicAdd(&a.cv.arrive[lb], 1);
-    if (old == a.cv.H - 1) {
-      a.cv.arrive[lb] = 0;
-      if (full)
-        atomicExch(a.cv.status, (int)TQ_ERR_CAPACITY);
-      else
-        a.cv.seq_len[lb] = pos + 1;
-      __threadfence();
-    }
-  }
-}
-
 __global__ void set_seq_len_kernel(CacheView cv, int layer, int value) {
   int b = blockIdx.x * blockDim.x + threadIdx.x;
   if (b < cv.B) cv.seq_len[layer * cv.B + b] = value;
@@ -431,19 +299,6 @@ cudaError_t launch_quantize_pack(const QuantArgs& a, int D, tq_dtype dt, int num
   }
   if (D == 64) return dt == TQ_F16 ? launch_quant_t<64, __half>(a, num_sms, st) : launch_quant_t<64, float>(a, num_sms, st);
   return dt == TQ_F16 ? launch_quant_t<128, __half>(a, num_sms, st) : launch_quant_t<128, float>(a, num_sms, st);
-}
-
-cudaError_t launch_append(const QuantArgs& a, int D, tq_dtype dt, cudaStream_t st) {
-  const int BH = a.cv.B * a.cv.H;
-  if (D == 64) {
-    if (dt == TQ_F16) append_kernel<64, __half><<<BH, 256, 0, st>>>(a);
-    else append_kernel<64, float><<<BH, 256, 0, st>>>(a);
-  } else {
-    if (dt == TQ_F16) append_kernel<128, __half><<<BH, 256, 0, st>>>(a);
-    else append_kernel<128, float><<<BH, 256, 0, st>>>(a);
-  }
-  count_launch();
-  return cudaGetLastError();
 }
 
 }  // namespace tq

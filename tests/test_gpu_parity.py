@@ -323,6 +323,36 @@ def test_prefill_append_decode_end_to_end_and_host_step(tq, oracle):
         assert np.all(np.abs(got - want) <= ulp + TL.OUT_MAX_ABS), step
 
 
+def test_fused_decode_step_equals_append_then_decode(tq, oracle):
+    """tq_decode_step must leave the same cache bytes and give the same output as tq_append + tq_decode_attn."""
+    import torch
+
+    w = W.CONFIGS["cfg2_650m_batch32"].scaled(batch=3, n_heads=4, seq=70)
+    outs, caches = [], []
+    for fused in (False, True):
+        c = Case(tq, oracle, w, max_seq=96)
+        k, v = W.layer_activations(w, 0)
+        tq.tq_quantize_pack(c.shape, c.params, c.cache, 0, c.dev(k), c.dev(v))
+        c.cache.seq_len[0, 2] = 40  # ragged
+        ws = tq.Workspace(c.shape, 1)
+        res = []
+        for step in range(3):
+            q, kn, vn = (c.dev(x) for x in W.step_tokens(w, 0, step))
+            out = torch.empty_like(q)
+            if fused:
+                tq.tq_decode_step(c.shape, c.params, c.cache, 0, q, kn, vn, out, ws)
+            else:
+                tq.tq_append(c.shape, c.params, c.cache, 0, kn, vn)
+                tq.tq_decode_attn(c.shape, c.params, c.cache, 0, 1, q[None], out[None], ws)
+            res.append(out.cpu().numpy())
+        torch.cuda.synchronize()
+        outs.append(np.stack(res))
+        caches.append(c.cache.data.cpu().numpy().copy())
+        assert c.cache.seq_len.cpu().numpy().tolist() == [[73, 73, 43]]
+    assert np.array_equal(outs[0], outs[1])
+    assert np.array_equal(caches[0], caches[1])
+
+
 def test_full_size_cfg2_sampled_units(tq, oracle):
     """BASELINE.json:configs[2] at full size in bench.py's launch configuration (batch 32 x 20 heads x 1024
     tokens, fp16): the GPU quantises and decodes everything; the oracle re-computes a sample of batch entries."""
