@@ -101,15 +101,18 @@ def torch_activations(w: W.Workload, layer: int, shape, device, gen):
     import torch
 
     ch = W.outlier_channels(w)[layer]
+    scale = np.ones((w.n_heads, w.head_dim), np.float32)
+    for h in range(w.n_heads):
+        scale[h, ch[h]] = w.outlier_scale
+    # [H, d] -> broadcast over [B, H, (T,) d]
+    scale = torch.from_numpy(scale).to(device).view((1, w.n_heads) + (1,) * (len(shape) - 3) + (w.head_dim,))
     out = []
     for _ in range(2):
         x = torch.randn(shape, device=device, generator=gen)
         if w.dist == "student_t4":
             chi = torch.randn((4,) + tuple(shape), device=device, generator=gen).square_().sum(0)
             x = x / torch.sqrt(chi / 4.0)
-        for h in range(w.n_heads):
-            for c in ch[h]:
-                x[:, h, ..., int(c)] *= w.outlier_scale
+        x = x * scale
         out.append(x.to(torch.float16 if w.dtype == "f16" else torch.float32).contiguous())
     return out
 
