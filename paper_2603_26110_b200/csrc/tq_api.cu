@@ -13,8 +13,27 @@ static std::atomic<long long> g_launches{0};
 void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
 
 
-constexpr int kMaxSplits = 64;        // = kMaxSegments in tq_decode.cu
-constexpr int kMaxPlanEntries = 256;   // = kMaxPlanEntries in tq_decode.cu
+constexpr int kMaxSplits = 64;  // = kMaxSegments in tq_decode.cu
+
+// Splits per unit for the streaming decode kernel.  Model: CTAs land round-robin on the SMs and the CTAs of an
+// SM share it, so the launch takes (max CTAs on one SM) x (tiles per CTA + a fixed per-CTA cost for the table
+// build, the cross-warp reduction and the split-K hand-off, in tile units).
+static int choose_nsplit(int units, int ntiles, int sms) {
+  const double kFixedTiles = 3.0;
+  int best = 1;
+  double best_t = 1e300;
+  for (int ns = 1; ns <= kMaxSplits && (ns == 1 || ntiles / ns >= 4); ++ns) {
+    const long ctas = (long)units * ns;
+    const long per_sm = (ctas + sms - 1) / sms;
+    const int per = (ntiles + ns - 1) / ns;
+    const double t = (double)per_sm * (per + kFixedTiles + (ns > 1 ? 1.0 : 0.0));
+    if (t < best_t * 0.97) {  // prefer fewer splits unless the gain is real
+      best_t = t;
+      best = ns;
+    }
+  }
+  return best;
+}
 
 static int num_sms() {
   static int cached = -1;
@@ -156,22 +175,19 @@ static int run_decode(const tq_shape* shape, const tq_params* dev, const tq_cach
     if (!aligned16(q) || !aligned16(out) || !workspace || ((uintptr_t)workspace & 255u)) return TQ_ERR_INVALID_ARG;
     if (t_hint < 0) return TQ_ERR_INVALID_ARG;
     if (workspace_bytes < w.total) return TQ_ERR_CAPACITY;
-    if (g.B > kMaxPlanEntries) return TQ_ERR_UNSUPPORTED;
   }
   const int sms = num_sms();
   if (sms <= 0) return TQ_ERR_CUDA;
   const int th = (t_hint == 0 || t_hint > g.max_seq) ? g.max_seq : t_hint;
   const int ntiles = (th + kTile - 1) / kTile;
-  // stream-K: one persistent CTA per resident slot; a unit may be cut into at most kMaxSplits segments
-  const int min_q = (ntiles + kMaxSplits - 3) / (kMaxSplits - 2);
-  int grid_override = 0;
-  if (const char* e = getenv("TQ_DECODE_NSPLIT")) {  // profiling / test knob: number of CTAs of the streaming kernel
+  int nsplit = choose_nsplit(n_layers_call * g.B * g.H, ntiles, sms);
+  if (const char* e = getenv("TQ_DECODE_NSPLIT")) {  // profiling / test knob: CTAs per unit of the streaming kernel
     long vv = atol(e);
-    if (vv >= 1 && vv <= 65535) grid_override = (int)vv;
+    if (vv >= 1 && vv <= kMaxSplits) nsplit = (int)vv;
   }
   const size_t esz = dt == TQ_F16 ? 2 : 4;
   unsigned char* ws = (unsigned char*)workspace;
-  const int layers_per_launch = do_query ? (kMaxPlanEntries / g.B > 0 ? kMaxPlanEntries / g.B : 1) : n_layers_call;
+  const int layers_per_launch = n_layers_call;
   for (int l0 = 0; l0 < n_layers_call; l0 += layers_per_launch) {
     const int nl = n_layers_call - l0 < layers_per_launch ? n_layers_call - l0 : layers_per_launch;
     const size_t u0 = (size_t)l0 * g.B * g.H;  // first unit of this launch inside the call
@@ -191,13 +207,15 @@ static int run_decode(const tq_shape* shape, const tq_params* dev, const tq_cach
     a.partials = ws ? (float*)(ws + w.off_partials) + u0 * kMaxSplits * (g.D + 2) : nullptr;
     a.layer_begin = layer_begin + l0;
     a.n_layers_call = nl;
-    a.nsplit = grid_override;
+    a.nsplit = nsplit;
+    a.per = (ntiles + nsplit - 1) / nsplit;
+    a.zero = 0;
     a.rope_layout = shape->rope_layout;
     a.dt = (int)dt;
     const void* kc = k ? (const unsigned char*)k + u0 * g.D * esz : nullptr;
     const void* vc = v ? (const unsigned char*)v + u0 * g.D * esz : nullptr;
     if (launch_prep(a, kc, vc, g.D, do_append, do_query, (cudaStream_t)cuda_stream) != cudaSuccess) return TQ_ERR_CUDA;
-    if (do_query && launch_decode(a, g.D, sms, min_q, (cudaStream_t)cuda_stream) != cudaSuccess) return TQ_ERR_CUDA;
+    if (do_query && launch_decode(a, g.D, (cudaStream_t)cuda_stream) != cudaSuccess) return TQ_ERR_CUDA;
   }
   return TQ_OK;
 }

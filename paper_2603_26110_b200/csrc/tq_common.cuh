@@ -122,16 +122,18 @@ struct DecodeArgs {
   const void* q;         // [Lc][B][H][D]
   void* out;             // [Lc][B][H][D]
   const int32_t* q_pos;  // [Lc][B] or nullptr
-  float* qrot;           // workspace [units_call][2 D]: q'' then z
+  float* qrot;           // workspace [units_call][2 D]: q'' then z, pre-scaled (tq_prep.cu)
   float* partials;       // workspace [units_call][64][D + 2]
   int* counters;         // workspace [units_call]
-  int layer_begin, n_layers_call, nsplit /* 0, or a CTA-count override */, rope_layout, dt;
+  int layer_begin, n_layers_call, nsplit /* CTAs per unit, >= 1 */, per /* tiles per split planned from t_hint */, rope_layout, dt;
+  int zero;  // always 0 (see tq_decode.cu: keeps table base registers opaque to ptxas)
 };
 
 cudaError_t launch_quantize_pack(const QuantArgs& a, int D, tq_dtype dt, int num_sms, cudaStream_t st);
 cudaError_t launch_prep(const DecodeArgs& d, const void* k, const void* v, int D, bool do_append, bool do_query,
                         cudaStream_t st);
-cudaError_t launch_decode(const DecodeArgs& a, int D, int num_sms, int min_q, cudaStream_t st);
+cudaError_t launch_decode(const DecodeArgs& a, int D, cudaStream_t st);
+int decode_ctas_per_sm(int D);
 cudaError_t launch_export(const CacheGeom& g, const CacheView& cv, int layer, int n_tokens, const tq_canonical& out,
                           cudaStream_t st);
 cudaError_t launch_import(const CacheGeom& g, const CacheView& cv, int layer, int n_tokens, const tq_canonical& in,

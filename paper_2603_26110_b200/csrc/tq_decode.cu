@@ -15,8 +15,11 @@
 //   * <z, sigma> becomes d/4 reads of a 16-entry nibble table with the same rotation;
 //   * V is dequantised two coordinates per 64-bit table read ([field][lane] float2, conflict free) and
 //     accumulated into d fp32 registers per lane; lanes are summed once per warp at the end.
-// Split-K over the sequence: grid = units x nsplit CTAs; the last CTA to finish a unit merges the partial
-// (m, l, o') triples and applies PI_V^T.
+// Split-K over the sequence: grid = units x nsplit CTAs (nsplit chosen on the host from t_hint so that the SMs
+// carry equal work); a unit covered by one CTA is finished in place, otherwise the last CTA to arrive merges
+// the partial (m, l, o') triples.  Either way the finishing CTA applies PI_V^T.
+// Tokens whose softmax weight underflows to exactly 0 in fp32 add nothing to o': their V lookups are skipped
+// (a warp-uniform test on a ballot of the weights), which changes no bit of the result.
 #include <utility>
 
 #include "tq_common.cuh"
@@ -52,10 +55,16 @@ __device__ __forceinline__ unsigned field_at(const unsigned (&w)[NW]) {
   return v & mask;
 }
 
-constexpr int kMaxPlanEntries = 256;  // (layers in one launch) x batch
 constexpr int kMaxSegments = 64;      // split-K partial slots per unit (tq_api.cu sizes the workspace)
-constexpr int kDecodeThreads = 128;
+#ifndef TQ_DECODE_CTAS64
+#define TQ_DECODE_CTAS64 5
+#endif
+#ifndef TQ_DECODE_THREADS
+#define TQ_DECODE_THREADS 128
+#endif
+constexpr int kDecodeThreads = TQ_DECODE_THREADS;  // warps of one CTA share the tables of one unit
 constexpr int kDecodeWarps = kDecodeThreads / 32;
+constexpr int kBuildThreads = 128;  // threads that build the tables and apply PI_V^T
 
 // Shared-memory map in ABSOLUTE shared-window addresses (the OR-addressing needs the K/V tables aligned to
 // their own size, the sign table to 4 KB).  Dynamic shared memory starts right after the 1 KB the driver
@@ -74,11 +83,11 @@ struct DecodeCfg {
   static constexpr unsigned kAbsStab = 4096;
   static constexpr unsigned kAbsVtab = 8192;
   static constexpr unsigned kAbsKtab = D == 64 ? 16384 : 32768;
-  static constexpr unsigned kAbsScratch = D == 64 ? 32768 : 16384;  // plan prefix, per-warp partials, merged o
-  static constexpr int kScratchBytes = (kMaxPlanEntries + 1) * 4 + 12 + 4 * (D + 2) * 4 + 2 * D * 4;
+  static constexpr unsigned kAbsScratch = D == 64 ? 32768 : 16384;  // per-warp partials, merged o
+  static constexpr int kScratchBytes = 16 + 8 * (D + 2) * 4 + 2 * D * 4;  // up to 8 warps
   static constexpr unsigned kAbsEnd = D == 64 ? kAbsScratch + kScratchBytes : kAbsKtab + kKtabBytes;
   static constexpr int kSmemBytes = kAbsEnd;             // requested dynamic bytes (window start <= 2 KB)
-  static constexpr int kCtasPerSm = D == 64 ? 6 : 3;
+  static constexpr int kCtasPerSm = D == 64 ? TQ_DECODE_CTAS64 : 3;
 };
 
 // ---- packed fp32x2 arithmetic (sm_100: FFMA2 / FADD2 / FMUL2 issue two fp32 operations per slot) ----------
@@ -156,17 +165,20 @@ __device__ __forceinline__ void v_token(const unsigned (&vw)[Layout<D>::KCW], un
 }
 template <int D, int... J>
 __device__ __forceinline__ void v_accum(const unsigned (&vw)[Layout<D>::KCW], unsigned vbase, unsigned wbuf,
+                                        unsigned nz /* ballot: token slots with a non-zero weight */,
                                         f32x2 (&o2)[2 * (Layout<D>::P / kTile)], std::integer_sequence<int, J...>) {
-  // w of tokens 4J .. 4J+3 arrive with one broadcast 128-bit read
+  // w of tokens 4J .. 4J+3 arrive with one broadcast 128-bit read; groups whose weights are all 0 are skipped
   (([&] {
-     float4 w4;
-     asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4+%5];"
-                  : "=f"(w4.x), "=f"(w4.y), "=f"(w4.z), "=f"(w4.w)
-                  : "r"(wbuf), "n"(16 * J));
-     v_token<D, 4 * J>(vw, vbase, w4.x, o2);
-     v_token<D, 4 * J + 1>(vw, vbase, w4.y, o2);
-     v_token<D, 4 * J + 2>(vw, vbase, w4.z, o2);
-     v_token<D, 4 * J + 3>(vw, vbase, w4.w, o2);
+     if (nz & (0xfu << (4 * J))) {
+       float4 w4;
+       asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4+%5];"
+                    : "=f"(w4.x), "=f"(w4.y), "=f"(w4.z), "=f"(w4.w)
+                    : "r"(wbuf), "n"(16 * J));
+       v_token<D, 4 * J>(vw, vbase, w4.x, o2);
+       v_token<D, 4 * J + 1>(vw, vbase, w4.y, o2);
+       v_token<D, 4 * J + 2>(vw, vbase, w4.z, o2);
+       v_token<D, 4 * J + 3>(vw, vbase, w4.w, o2);
+     }
    }()),
    ...);
 }
@@ -209,27 +221,45 @@ __device__ __forceinline__ void load_tile_words(TileWords<D>& t, const unsigned 
   t.vn = __ldg(reinterpret_cast<const unsigned short*>(tp + Lo::kOffVN) + lane);
 }
 
-
-// ---- table construction (per unit; pre-scaled so that logits come out in log2 units) ---------------------
+// ---- table construction (per CTA; the prep kernel stores q'' and z pre-scaled so that logits come out in
+//      log2 units: q'' * log2(e)/sqrt(d), z * log2(e)/sqrt(d) * sqrt(pi/2)/m) ------------------------------------
 // Every thread owns four consecutive table columns and writes them with 128-bit stores.
 template <int D>
-__device__ __forceinline__ void build_k_tables(float* Ktab, float* Stab, const float* qr, const float* __restrict__ lk,
-                                               int tid) {
+struct TableInputs {  // everything a thread needs from global memory, requested before anything is used
+  float4 qa[1], qb[1];
+  float4 zz[4];
+  float4 lk0, lk1, lv0, lv1;
+};
+
+template <int D>
+__device__ __forceinline__ void load_table_inputs(TableInputs<D>& t, const float* qr, const float* __restrict__ lk,
+                                                  const float* __restrict__ lv, int tid) {
   using Lo = Layout<D>;
   using Cfg = DecodeCfg<D>;
-  const float sc_k = 1.4426950408889634f * rsqrtf((float)D);
-  const float sc_s = sc_k * 1.2533141373155003f / (float)D;  // log2(e)/sqrt(d) * sqrt(pi/2)/m, m = D
-  const float4 l0 = __ldg(reinterpret_cast<const float4*>(lk)), l1 = __ldg(reinterpret_cast<const float4*>(lk) + 1);
-  const float lut[8] = {l0.x, l0.y, l0.z, l0.w, l1.x, l1.y, l1.z, l1.w};
-  {  // Ktab[8 hi + lo][c] = (q''_{2g} lut[lo] + q''_{2g+1} lut[hi]) * sc_k,  g = c mod P
-    constexpr int NQ = Cfg::NCK / 4;            // column quads: 16 | 32
-    constexpr int HPT = 8 / (kDecodeThreads / NQ);  // hi codes per thread: 1 | 2
+  constexpr int NQ = Cfg::NCK / 4;
+  const int g0 = (4 * (tid % NQ)) % Lo::P;
+  t.qa[0] = __ldcg(reinterpret_cast<const float4*>(qr + 2 * g0));
+  t.qb[0] = __ldcg(reinterpret_cast<const float4*>(qr + 2 * g0) + 1);
+  const int n0 = (4 * (tid % 16)) % Lo::NG;
+#pragma unroll
+  for (int i = 0; i < 4; ++i) t.zz[i] = __ldcg(reinterpret_cast<const float4*>(qr + D + 4 * (n0 + i)));
+  t.lk0 = __ldg(reinterpret_cast<const float4*>(lk));
+  t.lk1 = __ldg(reinterpret_cast<const float4*>(lk) + 1);
+  t.lv0 = __ldg(reinterpret_cast<const float4*>(lv));
+  t.lv1 = __ldg(reinterpret_cast<const float4*>(lv) + 1);
+}
+
+template <int D>
+__device__ __forceinline__ void build_tables(float* Ktab, float* Stab, float2* Vtab, const TableInputs<D>& t, int tid) {
+  using Lo = Layout<D>;
+  using Cfg = DecodeCfg<D>;
+  const float lut[8] = {t.lk0.x, t.lk0.y, t.lk0.z, t.lk0.w, t.lk1.x, t.lk1.y, t.lk1.z, t.lk1.w};
+  {  // Ktab[8 hi + lo][c] = q''_{2g} lut[lo] + q''_{2g+1} lut[hi],  g = c mod P
+    constexpr int NQ = Cfg::NCK / 4;                // column quads: 16 | 32
+    constexpr int HPT = 8 / (kBuildThreads / NQ);  // hi codes per thread: 1 | 2
     const int cq = tid % NQ, eg = tid / NQ;
-    const int g0 = (4 * cq) % Lo::P;
-    const float4 qa = __ldcg(reinterpret_cast<const float4*>(qr + 2 * g0));
-    const float4 qb = __ldcg(reinterpret_cast<const float4*>(qr + 2 * g0) + 1);
-    const float q0[4] = {qa.x * sc_k, qa.z * sc_k, qb.x * sc_k, qb.z * sc_k};  // q''_{2g}
-    const float q1[4] = {qa.y * sc_k, qa.w * sc_k, qb.y * sc_k, qb.w * sc_k};  // q''_{2g+1}
+    const float q0[4] = {t.qa[0].x, t.qa[0].z, t.qb[0].x, t.qb[0].z};  // q''_{2g}
+    const float q1[4] = {t.qa[0].y, t.qa[0].w, t.qb[0].y, t.qb[0].w};  // q''_{2g+1}
 #pragma unroll
     for (int hh = 0; hh < HPT; ++hh) {
       const int hi = eg * HPT + hh;
@@ -244,41 +274,46 @@ __device__ __forceinline__ void build_k_tables(float* Ktab, float* Stab, const f
             make_float4(fmaf(q0[0], lut[lo], b0), fmaf(q0[1], lut[lo], b1), fmaf(q0[2], lut[lo], b2), fmaf(q0[3], lut[lo], b3));
     }
   }
-  {  // Stab[e][c] = sum_b (bit b of e ? +z : -z)[4n + b] * sc_s,  n = c mod NG; 16 column quads x 8 entry pairs
+  {  // Stab[e][c] = sum_b (bit b of e ? +z : -z)[4n + b],  n = c mod NG; 16 column quads x 8 entry pairs
     const int cq = tid % 16, eg = tid / 16;
-    const int n0 = (4 * cq) % Lo::NG;
-    float4 zz[4];
-#pragma unroll
-    for (int i = 0; i < 4; ++i) {
-      zz[i] = __ldcg(reinterpret_cast<const float4*>(qr + D + 4 * (n0 + i)));
-      zz[i].x *= sc_s, zz[i].y *= sc_s, zz[i].z *= sc_s, zz[i].w *= sc_s;
-    }
 #pragma unroll
     for (int j = 0; j < 2; ++j) {
       const int e = 2 * eg + j;
       const float s0 = (e & 1) ? 1.f : -1.f, s1 = (e & 2) ? 1.f : -1.f, s2 = (e & 4) ? 1.f : -1.f, s3 = (e & 8) ? 1.f : -1.f;
       float v[4];
 #pragma unroll
-      for (int i = 0; i < 4; ++i) v[i] = fmaf(s0, zz[i].x, fmaf(s1, zz[i].y, fmaf(s2, zz[i].z, s3 * zz[i].w)));
+      for (int i = 0; i < 4; ++i) v[i] = fmaf(s0, t.zz[i].x, fmaf(s1, t.zz[i].y, fmaf(s2, t.zz[i].z, s3 * t.zz[i].w)));
       *reinterpret_cast<float4*>(Stab + e * 64 + 4 * cq) = make_float4(v[0], v[1], v[2], v[3]);
     }
   }
+  {  // Vtab[8 hi + lo][col] = (lut_V[lo], lut_V[hi]); 128 threads: hi = tid / 16, col = tid % 16
+    const float lv[8] = {t.lv0.x, t.lv0.y, t.lv0.z, t.lv0.w, t.lv1.x, t.lv1.y, t.lv1.z, t.lv1.w};
+    const int col = tid & 15, eq = tid >> 4;
+    float hi = lv[0];
+#pragma unroll
+    for (int c = 1; c < 8; ++c) hi = (eq == c) ? lv[c] : hi;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) Vtab[(eq * 8 + j) * 16 + col] = make_float2(lv[j], hi);
+  }
 }
 
-__device__ __forceinline__ void build_v_table(float2* Vtab, const float* __restrict__ lv, int tid) {
-  const int col = tid & 15, eq = tid >> 4;  // 128 threads: hi code = eq, entries 8 eq .. 8 eq + 7
-  const float hi = __ldg(lv + eq);
-#pragma unroll
-  for (int j = 0; j < 8; ++j) Vtab[(eq * 8 + j) * 16 + col] = make_float2(__ldg(lv + j), hi);
+__device__ __forceinline__ float ex2_ftz(float x) {
+  float y;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+__device__ __forceinline__ float warp_max_f32(float x) {  // sm_100a: one CREDUX instead of five shuffles
+  float y;
+  asm volatile("redux.sync.max.f32 %0, %1, 0xffffffff;" : "=f"(y) : "f"(x));
+  return y;
 }
 
 // ---- the streaming kernel ------------------------------------------------------------------------------------
-// Persistent, stream-K: the flat sequence of all 32-token tiles of the launch (unit-major) is cut into
-// gridDim.x equal contiguous ranges, so every CTA streams the same number of bytes regardless of how the
-// tiles fall on units.  A CTA walks its range unit by unit ("segments"); a unit covered by one CTA is finished
-// in place, a unit covered by several is merged by whichever CTA finishes it last.
+// grid = units x nsplit.  CTA (unit uc, split sp) streams tiles [sp * per, (sp + 1) * per) of its unit, where
+// per = ceil(ceil(T / 32) / nsplit) is derived on the device from seq_len, so a shorter cache simply leaves the
+// trailing splits empty.  The four warps take tiles round-robin with a register double buffer.
 template <int D, typename TIO>
-__global__ void __launch_bounds__(kDecodeThreads, DecodeCfg<D>::kCtasPerSm) decode_main_kernel(DecodeArgs a, int min_q) {
+__global__ void __launch_bounds__(kDecodeThreads, DecodeCfg<D>::kCtasPerSm) decode_main_kernel(DecodeArgs a) {
   using Lo = Layout<D>;
   using Cfg = DecodeCfg<D>;
   constexpr int NW = kDecodeWarps;
@@ -288,10 +323,9 @@ __global__ void __launch_bounds__(kDecodeThreads, DecodeCfg<D>::kCtasPerSm) deco
   if (raw > Cfg::kAbsWbuf) __trap();  // the fixed shared-memory map does not fit: fail loudly
   unsigned char* abs0 = smem_raw - raw;  // generic pointer to absolute shared address 0 of this CTA's window
   float* Stab = reinterpret_cast<float*>(abs0 + Cfg::kAbsStab);
-  int* plan = reinterpret_cast<int*>(abs0 + Cfg::kAbsScratch);            // [E + 1] exclusive prefix of tiles
-  float* red = reinterpret_cast<float*>(abs0 + Cfg::kAbsScratch + (kMaxPlanEntries + 1) * 4 + 12);  // NW x (D + 2)
-  float* omerged = red + NW * (D + 2);                                     // [D] + [D] partial matvec
-  float* wbuf_f = reinterpret_cast<float*>(abs0 + Cfg::kAbsWbuf);         // NW x 32 softmax weights
+  float* red = reinterpret_cast<float*>(abs0 + Cfg::kAbsScratch + 16);  // NW x (D + 2)
+  float* omerged = red + NW * (D + 2);                                   // [D] + [D] partial matvec
+  float* wbuf_f = reinterpret_cast<float*>(abs0 + Cfg::kAbsWbuf);       // NW x 32 softmax weights
   int* flag = reinterpret_cast<int*>(wbuf_f + NW * 32);
   float* Ktab = reinterpret_cast<float*>(abs0 + Cfg::kAbsKtab);
   float2* Vtab = reinterpret_cast<float2*>(abs0 + Cfg::kAbsVtab);
@@ -299,227 +333,182 @@ __global__ void __launch_bounds__(kDecodeThreads, DecodeCfg<D>::kCtasPerSm) deco
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int B = a.cv.B, H = a.cv.H;
-  const int E = a.n_layers_call * B;  // plan entries (layer-in-call, batch); seq_len is contiguous over them
-  const int32_t* seq = a.cv.seq_len + a.layer_begin * B;
-
-  // ---- plan: exclusive prefix sum of tiles per entry
-  {
-    const int CH = (E + kDecodeThreads - 1) / kDecodeThreads;
-    int local = 0;
-    for (int e = tid * CH; e < min(E, (tid + 1) * CH); ++e) local += (seq[e] + kTile - 1) / kTile;
-    int incl = local;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-      int v = __shfl_up_sync(0xffffffffu, incl, o);
-      if (lane >= o) incl += v;
-    }
-    int* wtot = reinterpret_cast<int*>(red);
-    if (lane == 31) wtot[warp] = incl;
-    __syncthreads();
-    int base = 0;
-    for (int w = 0; w < warp; ++w) base += wtot[w];
-    int run = base + incl - local;
-    for (int e = tid * CH; e < min(E, (tid + 1) * CH); ++e) {
-      plan[e] = run;
-      run += (seq[e] + kTile - 1) / kTile;
-    }
-    if (tid == kDecodeThreads - 1) plan[E] = base + incl;
-    __syncthreads();
-  }
-  const int total = plan[E] * H;  // tiles of the whole launch (< 2^31: checked on the host)
-  int Q = (total + (int)gridDim.x - 1) / (int)gridDim.x;
-  if (Q < min_q) Q = min_q;
-  int f = (int)blockIdx.x * Q;
-  const int fend = min(total, f + Q);
-  if (f >= fend) return;
-
-  // table base | lane column, kept opaque so that the compiler ORs it in with a single LOP3 per lookup
-  unsigned kbase = ktab + lane * 4, sbase = stab + lane * 4, vbase = vtab + (lane & 15) * 8;
-  asm volatile("" : "+r"(kbase), "+r"(sbase), "+r"(vbase));
-  const unsigned wbuf = (unsigned)__cvta_generic_to_shared(wbuf_f + warp * 32);
-  int vtab_owner = -1;  // (layer, head) the V table currently holds
-
-  // ---- locate the unit that owns flat tile f (binary search once; afterwards units are walked in order)
-  int e;
-  {
-    int lo = 0, hi = E;  // invariant: H * plan[lo] <= f < H * plan[hi]
-    while (hi - lo > 1) {
-      const int mid = (lo + hi) >> 1;
-      if (plan[mid] * H <= f) lo = mid;
-      else hi = mid;
-    }
-    e = lo;
-  }
-  int nt = plan[e + 1] - plan[e];
-  int h = (f - plan[e] * H) / nt;
-  int tile0 = (f - plan[e] * H) % nt;
-
-  while (true) {
-    const int tile1 = min(nt, tile0 + (fend - f));  // exclusive
-    const int lc = e / B, b = e - lc * B;
-    const int layer = a.layer_begin + lc;
-    const int uc = e * H + h;
-    const int T = seq[e];
-    const int ustart = plan[e] * H + h * nt;
-    const int cfirst = ustart / Q, clast = (ustart + nt - 1) / Q;
-    const int nseg = clast - cfirst + 1, slot = (int)blockIdx.x - cfirst;
-
-    // ---- start the memory system on this segment before anything else: one bulk L2 prefetch of all its
-    //      bytes, and this warp's first tile into registers
-    const unsigned char* stream = a.cv.tiles + ((size_t)layer * B * H + (size_t)b * H + h) * a.cv.stream_bytes;
-    if (tid == 0)
-      asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(stream + (size_t)tile0 * Lo::kTileBytes),
-                   "r"((tile1 - tile0) * Lo::kTileBytes)
+  const int nsplit = a.nsplit;
+  const int uc = (int)blockIdx.x / nsplit, sp = (int)blockIdx.x - uc * nsplit;
+  const int e = uc / H, h = uc - e * H;  // e = (layer-in-call, batch); seq_len is contiguous over e
+  const int lc = e / B, b = e - lc * B;
+  const int layer = a.layer_begin + lc;
+  // ---- every global request the prologue depends on goes out first and together: the cache length, the table
+  //      inputs, then (speculatively, from the host's split plan) this warp's first tile and the L2 prefetches of
+  //      its next ones, so that the small loads never queue behind the bulk ones
+  const size_t lh = (size_t)layer * H + h;
+  int T;
+  asm volatile("ld.global.b32 %0, [%1];" : "=r"(T) : "l"(a.cv.seq_len + a.layer_begin * B + e));
+  TableInputs<D> tin;
+  if (tid < kBuildThreads) load_table_inputs<D>(tin, a.qrot + (size_t)uc * 2 * D, a.lut_k + lh * 8, a.lut_v + lh * 8, tid);
+  const int per = a.per;  // tiles per split planned from t_hint; the last split also takes whatever lies beyond
+  const int tile0 = sp * per;
+  const int cap1 = sp == nsplit - 1 ? a.cv.tiles_cap : min(a.cv.tiles_cap, tile0 + per);  // static bound of this split
+  const unsigned char* stream = a.cv.tiles + (((size_t)layer * B + b) * H + h) * a.cv.stream_bytes;
+  TileWords<D> bufA, bufB;  // register double buffer, ping-pong (no copies)
+  if (tile0 + warp < cap1) load_tile_words<D>(bufA, stream + (size_t)(tile0 + warp) * Lo::kTileBytes, lane);
+  auto prefetch_tile = [&](int t, int bound) {  // one bulk L2 prefetch per tile, issued by one lane
+    if (t < bound && lane == 0)
+      asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(stream + (size_t)t * Lo::kTileBytes),
+                   "r"(Lo::kTileBytes)
                    : "memory");
-    TileWords<D> bufA, bufB;  // register double buffer, ping-pong (no copies)
-    if (tile0 + warp < tile1) load_tile_words<D>(bufA, stream + (size_t)(tile0 + warp) * Lo::kTileBytes, lane);
-
-    // ---- tables of this unit
-    __syncthreads();  // every warp is done with the previous unit's tables and scratch
-    build_k_tables<D>(Ktab, Stab, a.qrot + (size_t)uc * 2 * D, a.lut_k + ((size_t)layer * H + h) * 8, tid);
-    if (vtab_owner != layer * H + h) {
-      build_v_table(Vtab, a.lut_v + ((size_t)layer * H + h) * 8, tid);
-      vtab_owner = layer * H + h;
-    }
-    __syncthreads();
-
-    f32x2 o2[2 * VP];  // [pair][even / odd tokens]
+  };
+  constexpr int kPrefetchAhead = 3;  // rounds of NW tiles
 #pragma unroll
-    for (int i = 0; i < 2 * VP; ++i) o2[i] = 0ull;
-    float m = -INFINITY, l = 0.f;
-
-    // one 32-token tile: scores (lane = token) -> online softmax -> V accumulate (lane = coordinate pair)
-    auto process = [&](const TileWords<D>& tw, int tile) {
-      const bool valid = tile * kTile + lane < T;
-      const float sa = k_score<D>(tw.kw, kbase, std::make_integer_sequence<int, Lo::P / 2 - 2>{});
-      const float sb = s_score<D>(tw.sw, sbase, std::make_integer_sequence<int, Lo::NG / 2 - 2>{});
-      float s2 = f16_bits_to_f32(tw.kn) * fmaf(f16_bits_to_f32(tw.kr), sb, sa);
-      s2 = valid ? s2 : -INFINITY;
-      const float mnew = fmaxf(m, warp_max(s2));  // finite: slot 0 of every processed tile is valid
-      const float fsc = exp2f(m - mnew);          // 0 on a warp's first tile (m = -inf)
-      m = mnew;
-      const float p = exp2f(s2 - m);              // invalid lanes: exp2(-inf) = 0
-      l = fmaf(l, fsc, p);
-      const f32x2 fsc2 = pack2(fsc, fsc);
+  for (int i = 1; i < kPrefetchAhead; ++i) prefetch_tile(tile0 + warp + i * NW, cap1);
+  const float* Pv = a.pi_v + lh * D * D;
 #pragma unroll
-      for (int i = 0; i < 2 * VP; ++i) o2[i] = mul2(o2[i], fsc2);
+  for (int i = 0; i < D * D * 4 / 128 / kBuildThreads; ++i)
+    if (tid < kBuildThreads) asm volatile("prefetch.global.L2 [%0];" ::"l"(Pv + (size_t)(i * kBuildThreads + tid) * 32));
+  const int nt = (T + kTile - 1) / kTile;
+  if (tile0 >= nt) return;  // empty cache (the prep kernel wrote out = 0) or a trailing split with nothing to do
+  const int tile1 = min(nt, cap1);
+  const int nseg = min(nsplit, (nt + per - 1) / per);  // splits of this unit that have work
+  if (tid < kBuildThreads) build_tables<D>(Ktab, Stab, Vtab, tin, tid);
+  __syncthreads();
+
+  // table base | lane column as ONE register.  ptxas sees through an empty asm and would split the constant base
+  // from the lane term again (an extra LOP3 per lookup); XOR with a kernel argument that is always 0 keeps it whole,
+  // so every lookup address is a single LOP3: (field & mask) | base.
+  const unsigned kbase = (ktab + lane * 4) ^ (unsigned)a.zero, sbase = (stab + lane * 4) ^ (unsigned)a.zero,
+                 vbase = (vtab + (lane & 15) * 8) ^ (unsigned)a.zero;
+  const unsigned wbuf = (unsigned)__cvta_generic_to_shared(wbuf_f + warp * 32);
+
+  f32x2 o2[2 * VP];  // [pair][even / odd tokens]
+#pragma unroll
+  for (int i = 0; i < 2 * VP; ++i) o2[i] = 0ull;
+  float m = -INFINITY, l = 0.f;
+
+  // one 32-token tile: scores (lane = token) -> online softmax -> V accumulate (lane = coordinate pair)
+  auto process = [&](const TileWords<D>& tw, int tile) {
+    const bool valid = tile * kTile + lane < T;
+    const float sa = k_score<D>(tw.kw, kbase, std::make_integer_sequence<int, Lo::P / 2 - 2>{});
+    const float sb = s_score<D>(tw.sw, sbase, std::make_integer_sequence<int, Lo::NG / 2 - 2>{});
+    float s2 = f16_bits_to_f32(tw.kn) * fmaf(f16_bits_to_f32(tw.kr), sb, sa);
+    s2 = valid ? s2 : -INFINITY;
+    const float mnew = fmaxf(m, warp_max_f32(s2));  // finite: slot 0 of every processed tile is valid
+    const float fsc = ex2_ftz(m - mnew);            // 0 on a warp's first tile (m = -inf)
+    m = mnew;
+    const float p = ex2_ftz(s2 - m);                // invalid lanes: exp2(-inf) = 0
+    l = fmaf(l, fsc, p);
+    const f32x2 fsc2 = pack2(fsc, fsc);
+#pragma unroll
+    for (int i = 0; i < 2 * VP; ++i) o2[i] = mul2(o2[i], fsc2);
+    const float wv = valid ? p * f16_bits_to_f32(tw.vn) : 0.f;
+    const unsigned nz = __ballot_sync(0xffffffffu, wv != 0.f);
+    if (nz) {
       // hand the softmax weights from lane = token to lane = coordinate pair through shared memory
       __syncwarp();
-      asm volatile("st.shared.f32 [%0], %1;" ::"r"(wbuf + lane * 4), "f"(valid ? p * f16_bits_to_f32(tw.vn) : 0.f));
+      asm volatile("st.shared.f32 [%0], %1;" ::"r"(wbuf + lane * 4), "f"(wv));
       __syncwarp();
-      v_accum<D>(tw.vw, vbase, wbuf, o2, std::make_integer_sequence<int, kTile / 4>{});
-    };
-    auto fetch = [&](TileWords<D>& tw, int tile) {
-      if (tile < tile1) load_tile_words<D>(tw, stream + (size_t)tile * Lo::kTileBytes, lane);
-    };
-    int tile = tile0 + warp;
-    while (tile < tile1) {
-      fetch(bufB, tile + NW);
-      process(bufA, tile);
-      tile += NW;
-      if (tile >= tile1) break;
-      fetch(bufA, tile + NW);
-      process(bufB, tile);
-      tile += NW;
+      v_accum<D>(tw.vw, vbase, wbuf, nz, o2, std::make_integer_sequence<int, kTile / 4>{});
     }
+  };
+  auto fetch = [&](TileWords<D>& tw, int tile) {
+    prefetch_tile(tile + (kPrefetchAhead - 1) * NW, tile1);
+    if (tile < tile1) load_tile_words<D>(tw, stream + (size_t)tile * Lo::kTileBytes, lane);
+  };
+  int tile = tile0 + warp;
+  while (tile < tile1) {
+    fetch(bufB, tile + NW);
+    process(bufA, tile);
+    tile += NW;
+    if (tile >= tile1) break;
+    fetch(bufA, tile + NW);
+    process(bufB, tile);
+    tile += NW;
+  }
 
-    // ---- reduce over the CTA's warps (lanes already own distinct coordinates)
-    l = warp_sum(l);
-    float* wr = red + warp * (D + 2);
-    if (lane == 0) {
-      wr[0] = m;
-      wr[1] = l;
-    }
+  // ---- reduce over the CTA's warps (lanes already own distinct coordinates)
+  l = warp_sum(l);
+  float* wr = red + warp * (D + 2);
+  if (lane == 0) {
+    wr[0] = m;
+    wr[1] = l;
+  }
 #pragma unroll
-    for (int i = 0; i < VP; ++i) {
-      float x0, x1;
-      unpack2(add2(o2[2 * i], o2[2 * i + 1]), x0, x1);
-      wr[2 + 2 * (lane + kTile * i)] = x0;
-      wr[2 + 2 * (lane + kTile * i) + 1] = x1;
+  for (int i = 0; i < VP; ++i) {
+    float x0, x1;
+    unpack2(add2(o2[2 * i], o2[2 * i + 1]), x0, x1);
+    wr[2 + 2 * (lane + kTile * i)] = x0;
+    wr[2 + 2 * (lane + kTile * i) + 1] = x1;
+  }
+  __syncthreads();
+  float M = -INFINITY;
+#pragma unroll
+  for (int w = 0; w < NW; ++w) M = fmaxf(M, red[w * (D + 2)]);
+  float Lsum = 0.f, oi = 0.f;
+  if (tid < D) {
+#pragma unroll
+    for (int w = 0; w < NW; ++w) {
+      const float mw = red[w * (D + 2)];
+      const float fw = mw == -INFINITY ? 0.f : ex2_ftz(mw - M);
+      Lsum = fmaf(red[w * (D + 2) + 1], fw, Lsum);
+      oi = fmaf(red[w * (D + 2) + 2 + tid], fw, oi);
+    }
+  }
+  if (nseg > 1) {
+    float* part = a.partials + ((size_t)uc * kMaxSegments + sp) * (D + 2);
+    if (tid < D) part[2 + tid] = oi;
+    if (tid == 0) {
+      part[0] = M;
+      part[1] = Lsum;
     }
     __syncthreads();
-    float M = -INFINITY;
-#pragma unroll
-    for (int w = 0; w < NW; ++w) M = fmaxf(M, red[w * (D + 2)]);
-    float Lsum = 0.f, oi = 0.f;
+    if (tid == 0) {  // release: the barrier orders the CTA's partial stores before this fence (cumulativity)
+      __threadfence();
+      const int old = atomicAdd(&a.counters[uc], 1);
+      *flag = (old == nseg - 1);
+      if (old == nseg - 1) a.counters[uc] = 0;
+      __threadfence();  // acquire side for the CTA that merges
+    }
+    __syncthreads();
+    if (*flag == 0) return;
+    const float* pp = a.partials + (size_t)uc * kMaxSegments * (D + 2);
+    M = -INFINITY;
+    for (int s = 0; s < nseg; ++s) M = fmaxf(M, __ldcg(pp + s * (D + 2)));
+    Lsum = 0.f;
+    oi = 0.f;
     if (tid < D) {
-#pragma unroll
-      for (int w = 0; w < NW; ++w) {
-        const float mw = red[w * (D + 2)];
-        const float fw = mw == -INFINITY ? 0.f : exp2f(mw - M);
-        Lsum = fmaf(red[w * (D + 2) + 1], fw, Lsum);
-        oi = fmaf(red[w * (D + 2) + 2 + tid], fw, oi);
+      for (int s = 0; s < nseg; ++s) {
+        const float ms = __ldcg(pp + s * (D + 2));
+        const float fs = ms == -INFINITY ? 0.f : ex2_ftz(ms - M);
+        Lsum = fmaf(__ldcg(pp + s * (D + 2) + 1), fs, Lsum);
+        oi = fmaf(__ldcg(pp + s * (D + 2) + 2 + tid), fs, oi);
       }
     }
-    bool finish = true;
-    if (nseg > 1) {
-      float* part = a.partials + ((size_t)uc * kMaxSegments + slot) * (D + 2);
-      if (tid < D) part[2 + tid] = oi;
-      if (tid == 0) {
-        part[0] = M;
-        part[1] = Lsum;
-      }
-      __syncthreads();
-      if (tid == 0) {  // release: the barrier orders the CTA's partial stores before this fence (cumulativity)
-        __threadfence();
-        const int old = atomicAdd(&a.counters[uc], 1);
-        *flag = (old == nseg - 1);
-        if (old == nseg - 1) a.counters[uc] = 0;
-        __threadfence();  // acquire side for the CTA that merges
-      }
-      __syncthreads();
-      finish = *flag != 0;
-      if (finish) {
-        const float* pp = a.partials + (size_t)uc * kMaxSegments * (D + 2);
-        M = -INFINITY;
-        for (int s = 0; s < nseg; ++s) M = fmaxf(M, __ldcg(pp + s * (D + 2)));
-        Lsum = 0.f;
-        oi = 0.f;
-        if (tid < D) {
-          for (int s = 0; s < nseg; ++s) {
-            const float ms = __ldcg(pp + s * (D + 2));
-            const float fs = ms == -INFINITY ? 0.f : exp2f(ms - M);
-            Lsum = fmaf(__ldcg(pp + s * (D + 2) + 1), fs, Lsum);
-            oi = fmaf(__ldcg(pp + s * (D + 2) + 2 + tid), fs, oi);
-          }
-        }
-      }
-    }
-    if (finish) {  // out = PI_V^T (o' / l): the k range is split over the 256 / D thread groups
-      if (tid < D) omerged[tid] = Lsum > 0.f ? oi / Lsum : 0.f;
-      __syncthreads();
-      constexpr int PARTS = kDecodeThreads / D;  // 2 | 1
-      constexpr int KP = D / PARTS;              // 32 | 128
-      const int i = tid % D, part = tid / D;
-      const float* Pv = a.pi_v + ((size_t)layer * H + h) * D * D + (size_t)part * KP * D + i;
-      float r = 0.f;
+  }
+  // ---- out = PI_V^T (o' / l): the k range is split over the 128 / D thread groups
+  if (tid < D) omerged[tid] = Lsum > 0.f ? oi / Lsum : 0.f;
+  __syncthreads();
+  constexpr int PARTS = kBuildThreads / D;  // 2 | 1
+  constexpr int KP = D / PARTS;             // 32 | 128
+  const int i = tid % D, part = (tid / D) % PARTS;
+  float r = 0.f;
+  if (tid < kBuildThreads) {
+    const float* Pvp = Pv + (size_t)part * KP * D + i;
 #pragma unroll 32
-      for (int k = 0; k < KP; ++k) r = fmaf(__ldg(Pv + (size_t)k * D), omerged[part * KP + k], r);
-      if (PARTS > 1 && part > 0) omerged[part * D + i] = r;
-      __syncthreads();
-      if (part == 0) {
+    for (int k = 0; k < KP; ++k) r = fmaf(__ldg(Pvp + (size_t)k * D), omerged[part * KP + k], r);
+  }
+  if (PARTS > 1 && tid < kBuildThreads && part > 0) omerged[part * D + i] = r;
+  __syncthreads();
+  if (tid < D) {
 #pragma unroll
-        for (int pp = 1; pp < PARTS; ++pp) r += omerged[pp * D + i];
-        TIO* outp = reinterpret_cast<TIO*>(a.out) + (size_t)uc * D;
-        if constexpr (sizeof(TIO) == 2) outp[i] = __float2half_rn(r);
-        else outp[i] = r;
-      }
-    }
-    // ---- next unit of this CTA's range
-    f += tile1 - tile0;
-    if (f >= fend) break;
-    tile0 = 0;
-    if (++h == H) {
-      h = 0;
-      do { ++e; } while (plan[e + 1] == plan[e]);  // skip empty caches; f < fend <= total guarantees a hit
-      nt = plan[e + 1] - plan[e];
-    }
+    for (int pp = 1; pp < PARTS; ++pp) r += omerged[pp * D + i];
+    TIO* outp = reinterpret_cast<TIO*>(a.out) + (size_t)uc * D;
+    if constexpr (sizeof(TIO) == 2) outp[i] = __float2half_rn(r);
+    else outp[i] = r;
   }
 }
 
 // ------------------------------------------------------------------------------------------ launchers
 template <int D, typename T>
-static cudaError_t launch_decode_t(const DecodeArgs& a, int num_sms, int min_q, cudaStream_t st) {
+static cudaError_t launch_decode_t(const DecodeArgs& a, cudaStream_t st) {
   cudaError_t e;
   constexpr int smem = DecodeCfg<D>::kSmemBytes;
   static bool attr_set = false;
@@ -528,19 +517,17 @@ static cudaError_t launch_decode_t(const DecodeArgs& a, int num_sms, int min_q, 
     if (e != cudaSuccess) return e;
     attr_set = true;
   }
-  int grid = num_sms * DecodeCfg<D>::kCtasPerSm;
-  if (a.nsplit > 0) grid = a.nsplit;  // profiling / test override: number of CTAs
-  decode_main_kernel<D, T><<<grid, kDecodeThreads, smem, st>>>(a, min_q);
+  const int units = a.n_layers_call * a.cv.B * a.cv.H;
+  decode_main_kernel<D, T><<<units * a.nsplit, kDecodeThreads, smem, st>>>(a);
   count_launch();
   return cudaGetLastError();
 }
 
-cudaError_t launch_decode(const DecodeArgs& a, int D, int num_sms, int min_q, cudaStream_t st) {
-  if (D == 64)
-    return a.dt == TQ_F16 ? launch_decode_t<64, __half>(a, num_sms, min_q, st)
-                          : launch_decode_t<64, float>(a, num_sms, min_q, st);
-  return a.dt == TQ_F16 ? launch_decode_t<128, __half>(a, num_sms, min_q, st)
-                        : launch_decode_t<128, float>(a, num_sms, min_q, st);
+int decode_ctas_per_sm(int D) { return D == 64 ? DecodeCfg<64>::kCtasPerSm : DecodeCfg<128>::kCtasPerSm; }
+
+cudaError_t launch_decode(const DecodeArgs& a, int D, cudaStream_t st) {
+  if (D == 64) return a.dt == TQ_F16 ? launch_decode_t<64, __half>(a, st) : launch_decode_t<64, float>(a, st);
+  return a.dt == TQ_F16 ? launch_decode_t<128, __half>(a, st) : launch_decode_t<128, float>(a, st);
 }
 
 }  // namespace tq

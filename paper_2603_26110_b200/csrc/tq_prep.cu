@@ -70,6 +70,9 @@ __global__ void __launch_bounds__(4 * D) prep_kernel(PrepArgs a) {
   using Lo = Layout<D>;
   constexpr int NT = 4 * D;  // 8 rows per warp
   constexpr int HP = D / 2;
+  constexpr float kInvSqrtD = D == 64 ? 0.125f : 0.08838834764831845f;
+  constexpr float kScaleK = 1.4426950408889634f * kInvSqrtD;             // log2(e) / sqrt(d)
+  constexpr float kScaleS = kScaleK * 1.2533141373155003f / (float)D;  // ... * sqrt(pi/2) / m, m = D
   __shared__ float xk[D], xq[D], xv[D], yk[D], yq[D], yv[D], r[D], sr[D], zq[D];
   __shared__ unsigned char cK[D], cV[D], bK[D];
   __shared__ float nrm[4];
@@ -125,7 +128,7 @@ __global__ void __launch_bounds__(4 * D) prep_kernel(PrepArgs a) {
   __syncthreads();
   if (kQuery) {
     float* dst = a.qrot + (size_t)uc * 2 * D;
-    if (tid < D) dst[tid] = yq[tid];
+    if (tid < D) dst[tid] = yq[tid] * kScaleK;  // logits in log2 units
     if (len1 <= 0 && tid < D) {  // empty cache: no tile for this unit in the streaming kernel, out = 0
       T* outp = reinterpret_cast<T*>(a.out) + (size_t)uc * D;
       if constexpr (sizeof(T) == 2) outp[tid] = __float2half_rn(0.f);
@@ -166,7 +169,8 @@ __global__ void __launch_bounds__(4 * D) prep_kernel(PrepArgs a) {
   if (kAppend) Ms.apply(r, sr, warp, lane);
   if (kQuery) Ms.apply(yq, zq, warp, lane);
   __syncthreads();
-  if (kQuery && tid < D) a.qrot[(size_t)uc * 2 * D + D + tid] = zq[tid];
+  if (kQuery && tid < D)  // log2(e)/sqrt(d) * sqrt(pi/2)/m, m = D
+    a.qrot[(size_t)uc * 2 * D + D + tid] = zq[tid] * kScaleS;
   if (kAppend) {
     if (tid < D) bK[tid] = sr[tid] >= 0.f ? 1 : 0;
     __syncthreads();
