@@ -1,16 +1,19 @@
-// tq_prep.cu — the small per-(batch, head) kernel in front of the streaming decode kernel.
+// tq_prep.cu — the small kernel in front of the streaming decode kernel.
 //
-// One CTA per (layer-in-call, batch, head) does, depending on the template flags,
-//   kAppend : quantize-and-pack ONE new token (PAPER.md:111-116 per vector; BASELINE.json:configs[2]):
-//             RoPE(k) -> PI_K -> norm, codes, residual -> S r -> bits;  PI_V v -> norm, codes; the words are
-//             written into the tile slot seq_len[layer][b] and the last head of the batch entry bumps seq_len;
+// One CTA per (layer-in-call, head, group of BG batch entries) does, depending on the template flags,
+//   kAppend : quantize-and-pack ONE new token per batch entry (PAPER.md:111-116 per vector;
+//             BASELINE.json:configs[2]): RoPE(k) -> PI_K -> norm, codes, residual -> S r -> bits;
+//             PI_V v -> norm, codes; the words are written into the tile slot seq_len[layer][b] and the last head of
+//             the batch entry to arrive bumps seq_len;
 //   kQuery  : query preparation for the fused decode kernel (Eq. 4 moves PI to the query; north_star):
-//             q'' = PI_K RoPE(q), z = S q''  -> workspace.
-// tq_append = <true,false>, tq_decode_attn = <false,true>, tq_decode_step = <true,true>; in the fused form the
-// rows of PI_K and S are fetched once and used for both the key and the query.
+//             q'' = PI_K RoPE(q), z = S q''  -> workspace, pre-scaled so that logits come out in log2 units.
+// tq_append = <true,false>, tq_decode_attn = <false,true>, tq_decode_step = <true,true>.
 //
-// These are latency-bound 3-stage chains (load -> mat-vec -> mat-vec); every matrix row a warp needs is
-// requested before the first barrier so that the L2 latency is paid once, not once per stage.
+// The work is tiny (five d x d mat-vecs per unit) and the kernel is bound by latency and by re-reading the three
+// d x d fp32 matrices of a head: so a CTA keeps them in REGISTERS — three thread groups (PI_K, S, PI_V), TPR = d/64
+// threads per matrix row, 64 row elements per thread — fetches them once and applies them to all BG batch entries
+// of its head at once (vectors are read from shared memory as broadcast float4).  Four barriers per CTA:
+//   inputs + RoPE | PI_K k, PI_K q, PI_V v and their norms | codes, residual, its norm | S r, S q'' | words out.
 #include "tq_common.cuh"
 
 namespace tq {
@@ -22,39 +25,6 @@ __device__ __forceinline__ int code_of7(float u, const float* lut) {
   return c;
 }
 
-// rows [8 warp, 8 warp + 8) of a row-major D x D matrix, lane holds elements lane + 32 j of each row
-template <int D>
-struct RowRegs {
-  float m[8][D / 32];
-  __device__ __forceinline__ void load(const float* __restrict__ M, int warp, int lane) {
-#pragma unroll
-    for (int r = 0; r < 8; ++r)
-#pragma unroll
-      for (int j = 0; j < D / 32; ++j) m[r][j] = __ldg(M + (size_t)(warp * 8 + r) * D + lane + 32 * j);
-  }
-  // y[8 warp + r] = <row r, x>
-  __device__ __forceinline__ void apply(const float* xsm, float* ysm, int warp, int lane) const {
-    float xr[D / 32];
-#pragma unroll
-    for (int j = 0; j < D / 32; ++j) xr[j] = xsm[lane + 32 * j];
-    float p[8];
-#pragma unroll
-    for (int r = 0; r < 8; ++r) {
-      p[r] = 0.f;
-#pragma unroll
-      for (int j = 0; j < D / 32; ++j) p[r] = fmaf(m[r][j], xr[j], p[r]);
-    }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1)
-#pragma unroll
-      for (int r = 0; r < 8; ++r) p[r] += __shfl_xor_sync(0xffffffffu, p[r], o);
-    if (lane == 0) {
-#pragma unroll
-      for (int r = 0; r < 8; ++r) ysm[warp * 8 + r] = p[r];
-    }
-  }
-};
-
 struct PrepArgs {
   CacheView cv;
   const float *pi_k, *pi_v, *lut_k, *lut_v, *S, *rope_cs;  // full [L][H]... arrays
@@ -65,177 +35,306 @@ struct PrepArgs {
   int layer_begin, rope_layout;
 };
 
+template <int D>
+struct PrepCfg {
+  static constexpr int TPR = D / 64;          // threads per matrix row (64 row elements each)
+  static constexpr int GT = D * TPR;          // threads per group: 64 | 256
+  static constexpr int BG = D == 64 ? 4 : 2;  // batch entries per CTA
+};
+
+// 64 consecutive elements of one matrix row, in registers
+struct RowRegs64 {
+  float4 m[16];
+  __device__ __forceinline__ void load(const float* __restrict__ p) {
+#pragma unroll
+    for (int c = 0; c < 16; ++c) m[c] = __ldg(reinterpret_cast<const float4*>(p) + c);
+  }
+  // acc[e] += <row part, x[e] part>, x in shared memory (every lane of a row group reads the same address)
+  template <int BG>
+  __device__ __forceinline__ void dot(const float* xs /* [BG][stride] */, int stride, float (&acc)[BG]) const {
+#pragma unroll
+    for (int c = 0; c < 16; ++c) {
+#pragma unroll
+      for (int e = 0; e < BG; ++e) {
+        const float4 x = *reinterpret_cast<const float4*>(xs + e * stride + 4 * c);
+        acc[e] = fmaf(m[c].x, x.x, fmaf(m[c].y, x.y, fmaf(m[c].z, x.z, fmaf(m[c].w, x.w, acc[e]))));
+      }
+    }
+  }
+};
+
 template <int D, typename T, bool kAppend, bool kQuery>
-__global__ void __launch_bounds__(4 * D) prep_kernel(PrepArgs a) {
+__global__ void __launch_bounds__((kAppend ? 3 : 2) * PrepCfg<D>::GT) prep_kernel(PrepArgs a, int nbg) {
   using Lo = Layout<D>;
-  constexpr int NT = 4 * D;  // 8 rows per warp
+  using Cfg = PrepCfg<D>;
+  constexpr int TPR = Cfg::TPR, GT = Cfg::GT, BG = Cfg::BG;
+  constexpr int NT = (kAppend ? 3 : 2) * GT;
+  constexpr int WG = GT / 32;  // warps per group
   constexpr int HP = D / 2;
   constexpr float kInvSqrtD = D == 64 ? 0.125f : 0.08838834764831845f;
   constexpr float kScaleK = 1.4426950408889634f * kInvSqrtD;             // log2(e) / sqrt(d)
   constexpr float kScaleS = kScaleK * 1.2533141373155003f / (float)D;  // ... * sqrt(pi/2) / m, m = D
-  __shared__ float xk[D], xq[D], xv[D], yk[D], yq[D], yv[D], r[D], sr[D], zq[D];
-  __shared__ unsigned char cK[D], cV[D], bK[D];
-  __shared__ float nrm[4];
+  __shared__ __align__(16) float xk[BG][D], xq[BG][D], xv[BG][D], yq[BG][D], rr[BG][D];
+  __shared__ unsigned char cK[BG][D], cV[BG][D], bitb[BG][D];
+  __shared__ float redk[BG][WG], redv[BG][WG], redr[BG][WG];
   __shared__ float lutK[8], lutV[8];
-  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int uc = blockIdx.x;
-  const int B = a.cv.B, H = a.cv.H;
-  const int lc = uc / (B * H), bh = uc % (B * H), b = bh / H, h = bh % H;
-  const int layer = a.layer_begin + lc;
-  const int lb = layer * B + b;
-  const int len0 = a.cv.seq_len[lb];
-  const bool full = kAppend && len0 >= a.cv.max_seq;
-  const int len1 = (kAppend && !full) ? len0 + 1 : len0;  // length the decode kernel will see
-  // RoPE positions: the appended key sits at index len0; the query defaults to the newest cached token
-  int qpos = a.q_pos ? a.q_pos[lc * B + b] : len1 - 1;
-  qpos = max(0, min(qpos, a.cv.max_seq - 1));
-  const int kpos = min(len0, a.cv.max_seq - 1);
+  __shared__ int s_len0[BG], s_full[BG];
 
-  // ---- every global load that does not depend on a result, up front
-  RowRegs<D> Mk, Mv, Ms;
+  const int tid = threadIdx.x, lane = tid & 31;
+  const int grp = tid / GT, gt = tid % GT, row = gt / TPR, part = gt % TPR, wg = gt >> 5;
+  const int B = a.cv.B, H = a.cv.H;
+  const int bgi = (int)blockIdx.x % nbg, lh_c = (int)blockIdx.x / nbg;  // (layer-in-call, head), batch group
+  const int lc = lh_c / H, h = lh_c % H;
+  const int layer = a.layer_begin + lc;
+  const int b0 = bgi * BG, nb = min(BG, B - b0);
   const size_t lh = (size_t)layer * H + h;
-  Mk.load(a.pi_k + lh * D * D, warp, lane);
-  if (kAppend) Mv.load(a.pi_v + lh * D * D, warp, lane);
-  Ms.load(a.S, warp, lane);
+
+  // ---- the cache lengths first: the RoPE positions and the target tile slot hang off them
+  int len_e[BG];
+#pragma unroll
+  for (int e = 0; e < BG; ++e) len_e[e] = e < nb ? __ldcg(a.cv.seq_len + layer * B + b0 + e) : 0;
+  // ---- matrix rows into registers: the only loads that miss L2 after the first CTA of a head
+  RowRegs64 rowreg;
+  {
+    const float* M = grp == 0 ? a.pi_k + lh * D * D : grp == 1 ? a.S : a.pi_v + lh * D * D;
+    rowreg.load(M + (size_t)row * D + part * 64);
+  }
+  // ---- stage-4 work item of this thread (one word of one token), and an early read of the V word it will modify
+  constexpr int ITEMS = Lo::KCW + Lo::KSW + Lo::P + 1;
+  static_assert(!kAppend || BG * ITEMS <= NT, "one output item per thread");
+  const int it_e = tid / ITEMS, it = tid % ITEMS;
+  int it_len = len_e[0];
+#pragma unroll
+  for (int j = 1; j < BG; ++j) it_len = it_e == j ? len_e[j] : it_len;
+  const bool it_on = kAppend && it_e < nb && it_len < a.cv.max_seq;
+  unsigned char* it_tp = a.cv.tiles + (((size_t)layer * B + b0 + min(it_e, nb - 1)) * H + h) * a.cv.stream_bytes +
+                         (size_t)(min(it_len, a.cv.max_seq - 1) / kTile) * Lo::kTileBytes;
+  const int it_slot = it_len % kTile;
+  unsigned vold0 = 0, vold1 = 0;
+  unsigned *vp0 = nullptr, *vp1 = nullptr;
+  if (it_on && it >= Lo::KCW + Lo::KSW && it < Lo::KCW + Lo::KSW + Lo::P) {
+    const int g = it - Lo::KCW - Lo::KSW, vl = g % kTile, vp = g / kTile;
+    const int bit = 192 * vp + 6 * it_slot;
+    vp0 = reinterpret_cast<unsigned*>(it_tp + Lo::kOffVC + word_offset(Lo::KCW, bit >> 5, vl));
+    vold0 = __ldcg(vp0);
+    if ((bit & 31) > 26) {
+      vp1 = reinterpret_cast<unsigned*>(it_tp + Lo::kOffVC + word_offset(Lo::KCW, (bit >> 5) + 1, vl));
+      vold1 = __ldcg(vp1);
+    }
+  }
   if (tid < 8) lutK[tid] = a.lut_k[lh * 8 + tid];
   if (tid >= 32 && tid < 40) lutV[tid - 32] = a.lut_v[lh * 8 + tid - 32];
-  if (tid < HP) {
-    const int g = tid;
+
+  // ---- inputs of the BG batch entries of this head, RoPE applied to k and q (positions read on the device)
+  for (int idx = tid; idx < BG * HP; idx += NT) {
+    const int e = idx / HP, g = idx % HP;
     const int ia = a.rope_layout == 0 ? 2 * g : g, ib = a.rope_layout == 0 ? 2 * g + 1 : g + HP;
-    if (kAppend) {
-      const T* kp = reinterpret_cast<const T*>(a.k) + (size_t)uc * D;
-      const float xa = load_as_float<T>(kp + ia), xb = load_as_float<T>(kp + ib);
-      const float2 cs = *reinterpret_cast<const float2*>(a.rope_cs + ((size_t)kpos * HP + g) * 2);
-      xk[ia] = xa * cs.x - xb * cs.y;
-      xk[ib] = xa * cs.y + xb * cs.x;
+    float ka = 0.f, kb = 0.f, qa = 0.f, qb = 0.f;
+    if (e < nb) {
+      const int b = b0 + e;
+      int len0 = len_e[0];
+#pragma unroll
+      for (int j = 1; j < BG; ++j) len0 = e == j ? len_e[j] : len0;
+      const bool full = kAppend && len0 >= a.cv.max_seq;
+      const int len1 = (kAppend && !full) ? len0 + 1 : len0;  // length the decode kernel will see
+      const size_t uc = ((size_t)lc * B + b) * H + h;
+      if (g == 0) {
+        s_len0[e] = len0;
+        s_full[e] = full;
+      }
+      if (kAppend) {  // the appended key sits at index len0
+        const int kpos = min(len0, a.cv.max_seq - 1);
+        const T* kp = reinterpret_cast<const T*>(a.k) + uc * D;
+        const float xa = load_as_float<T>(kp + ia), xb = load_as_float<T>(kp + ib);
+        const float2 cs = *reinterpret_cast<const float2*>(a.rope_cs + ((size_t)kpos * HP + g) * 2);
+        ka = xa * cs.x - xb * cs.y;
+        kb = xa * cs.y + xb * cs.x;
+      }
+      if (kQuery) {  // the query defaults to the newest cached token
+        int qpos = a.q_pos ? a.q_pos[lc * B + b] : len1 - 1;
+        qpos = max(0, min(qpos, a.cv.max_seq - 1));
+        const T* qp = reinterpret_cast<const T*>(a.q) + uc * D;
+        const float xa = load_as_float<T>(qp + ia), xb = load_as_float<T>(qp + ib);
+        const float2 cs = *reinterpret_cast<const float2*>(a.rope_cs + ((size_t)qpos * HP + g) * 2);
+        qa = xa * cs.x - xb * cs.y;
+        qb = xa * cs.y + xb * cs.x;
+        if (len1 <= 0) {  // empty cache: no tile for this unit in the streaming kernel, out = 0
+          T* outp = reinterpret_cast<T*>(a.out) + uc * D;
+          if constexpr (sizeof(T) == 2) outp[ia] = outp[ib] = __float2half_rn(0.f);
+          else outp[ia] = outp[ib] = 0.f;
+        }
+      }
     }
-    if (kQuery) {
-      const T* qp = reinterpret_cast<const T*>(a.q) + (size_t)uc * D;
-      const float xa = load_as_float<T>(qp + ia), xb = load_as_float<T>(qp + ib);
-      const float2 cs = *reinterpret_cast<const float2*>(a.rope_cs + ((size_t)qpos * HP + g) * 2);
-      xq[ia] = xa * cs.x - xb * cs.y;
-      xq[ib] = xa * cs.y + xb * cs.x;
+    if (kAppend) xk[e][ia] = ka, xk[e][ib] = kb;
+    if (kQuery) xq[e][ia] = qa, xq[e][ib] = qb;
+  }
+  if (kAppend) {
+    for (int idx = tid; idx < BG * D; idx += NT) {
+      const int e = idx / D, i = idx % D;
+      xv[e][i] = e < nb ? load_as_float<T>(reinterpret_cast<const T*>(a.v) + (((size_t)lc * B + b0 + e) * H + h) * D + i) : 0.f;
     }
-  } else if (kAppend && tid >= NT / 2 && tid < NT / 2 + D) {
-    xv[tid - NT / 2] = load_as_float<T>(reinterpret_cast<const T*>(a.v) + (size_t)uc * D + tid - NT / 2);
   }
   __syncthreads();
 
-  // ---- stage 1: rotations
-  if (kAppend) Mk.apply(xk, yk, warp, lane);
-  if (kQuery) Mk.apply(xq, yq, warp, lane);
-  if (kAppend) Mv.apply(xv, yv, warp, lane);
-  __syncthreads();
-  if (kQuery) {
-    float* dst = a.qrot + (size_t)uc * 2 * D;
-    if (tid < D) dst[tid] = yq[tid] * kScaleK;  // logits in log2 units
-    if (len1 <= 0 && tid < D) {  // empty cache: no tile for this unit in the streaming kernel, out = 0
-      T* outp = reinterpret_cast<T*>(a.out) + (size_t)uc * D;
-      if constexpr (sizeof(T) == 2) outp[tid] = __float2half_rn(0.f);
-      else outp[tid] = 0.f;
-    }
-  }
-  if (kAppend) {
-    if (warp < 2) {  // warp 0: |y_k|, warp 1: |y_v|
-      const float* y = warp == 0 ? yk : yv;
-      float p = 0.f;
+  // ---- stage 1: rotations (groups 0 and 2) and the norms of the rotated key / value
+  float yk[BG], yv[BG];
+  if (grp == 0) {
+    float aq[BG];
 #pragma unroll
-      for (int i = lane; i < D; i += 32) p = fmaf(y[i], y[i], p);
-      p = warp_sum(p);
-      if (lane == 0) nrm[warp] = sqrtf(p);
-    }
-    __syncthreads();
-    const float n = nrm[0], nv = nrm[1];
-    if (tid < D) {
-      const float u = n > 0.f ? yk[tid] / n : 0.f;
-      const int c = code_of7(u, lutK);
-      cK[tid] = (unsigned char)c;
-      r[tid] = u - lutK[c];
-    } else if (tid >= NT / 2 && tid < NT / 2 + D) {
-      const int i = tid - NT / 2;
-      const float u = nv > 0.f ? yv[i] / nv : 0.f;
-      cV[i] = (unsigned char)code_of7(u, lutV);
-    }
-    __syncthreads();
-    if (warp == 0) {
-      float p = 0.f;
+    for (int e = 0; e < BG; ++e) yk[e] = 0.f, aq[e] = 0.f;
+    if (kAppend) rowreg.dot<BG>(&xk[0][part * 64], D, yk);
+    if (kQuery) rowreg.dot<BG>(&xq[0][part * 64], D, aq);
 #pragma unroll
-      for (int i = lane; i < D; i += 32) p = fmaf(r[i], r[i], p);
-      p = warp_sum(p);
-      if (lane == 0) nrm[2] = sqrtf(p);
-    }
-  }
-  // ---- stage 2: sketch of the residual / of the rotated query
-  if (kAppend) Ms.apply(r, sr, warp, lane);
-  if (kQuery) Ms.apply(yq, zq, warp, lane);
-  __syncthreads();
-  if (kQuery && tid < D)  // log2(e)/sqrt(d) * sqrt(pi/2)/m, m = D
-    a.qrot[(size_t)uc * 2 * D + D + tid] = zq[tid] * kScaleS;
-  if (kAppend) {
-    if (tid < D) bK[tid] = sr[tid] >= 0.f ? 1 : 0;
-    __syncthreads();
-    if (!full) {  // ---- assemble this token's words (device layout, include/tq.h)
-      const int pos = len0;
-      const size_t unit = (size_t)layer * B * H + bh;
-      unsigned char* tp = a.cv.tiles + unit * a.cv.stream_bytes + (size_t)(pos / kTile) * Lo::kTileBytes;
-      const int slot = pos % kTile;
-      if (tid < Lo::KCW) {
-        const int w = tid;
-        unsigned long long word = 0;
-        const int k_lo = (32 * w) / 6, k_hi = (32 * w + 31) / 6;
-        for (int kf = k_lo; kf <= k_hi; ++kf) {
-          const int g = (kf + slot) % Lo::P;
-          unsigned long long f = cK[2 * g] | ((unsigned)cK[2 * g + 1] << 3);
-          const int sh = 6 * kf - 32 * w;
-          word |= sh >= 0 ? (f << sh) : (f >> (-sh));
-        }
-        *reinterpret_cast<unsigned*>(tp + Lo::kOffKC + word_offset(Lo::KCW, w, slot)) = (unsigned)word;
-      } else if (tid >= 32 && tid < 32 + Lo::KSW) {
-        const int w = tid - 32;
-        unsigned word = 0;
-        for (int kn = 0; kn < 8; ++kn) {
-          const int ng = (8 * w + kn + slot) % Lo::NG;
-          unsigned nib = bK[4 * ng] | (bK[4 * ng + 1] << 1) | (bK[4 * ng + 2] << 2) | (bK[4 * ng + 3] << 3);
-          word |= nib << (4 * kn);
-        }
-        *reinterpret_cast<unsigned*>(tp + Lo::kOffKS + word_offset(Lo::KSW, w, slot)) = word;
-      } else if (tid >= 64 && tid < 64 + Lo::P) {
-        // V: pair group g lives in lane (g mod 32)'s string at bits [192 part + 6 slot, +6): read-modify-write
-        const int g = tid - 64, vl = g % kTile, part = g / kTile;
-        const unsigned f = cV[2 * g] | ((unsigned)cV[2 * g + 1] << 3);
-        const int bit = 192 * part + 6 * slot, s = bit & 31;
-        unsigned* p0 = reinterpret_cast<unsigned*>(tp + Lo::kOffVC + word_offset(Lo::KCW, bit >> 5, vl));
-        *p0 = (*p0 & ~(63u << s)) | (f << s);
-        if (s > 26) {
-          unsigned* p1 = reinterpret_cast<unsigned*>(tp + Lo::kOffVC + word_offset(Lo::KCW, (bit >> 5) + 1, vl));
-          *p1 = (*p1 & ~(63u >> (32 - s))) | (f >> (32 - s));
-        }
-      } else if (tid == 192) {
-        reinterpret_cast<unsigned short*>(tp + Lo::kOffKN)[slot] = f32_to_f16_bits_clamped(nrm[0]);
-        reinterpret_cast<unsigned short*>(tp + Lo::kOffKR)[slot] = f32_to_f16_bits_clamped(nrm[2]);
-        reinterpret_cast<unsigned short*>(tp + Lo::kOffVN)[slot] = f32_to_f16_bits_clamped(nrm[1]);
+    for (int e = 0; e < BG; ++e) {
+      if (TPR == 2) {
+        yk[e] += __shfl_xor_sync(0xffffffffu, yk[e], 1);
+        aq[e] += __shfl_xor_sync(0xffffffffu, aq[e], 1);
+      }
+      if (kAppend) {
+        const float ss = warp_sum(part == 0 ? yk[e] * yk[e] : 0.f);
+        if (lane == 0) redk[e][wg] = ss;
+      }
+      if (kQuery && part == 0) {
+        yq[e][row] = aq[e];
+        if (e < nb) a.qrot[(((size_t)lc * B + b0 + e) * H + h) * 2 * D + row] = aq[e] * kScaleK;
       }
     }
-    // ---- arrival: the last head of batch entry b publishes the new length
+  } else if (kAppend && grp == 2) {
+#pragma unroll
+    for (int e = 0; e < BG; ++e) yv[e] = 0.f;
+    rowreg.dot<BG>(&xv[0][part * 64], D, yv);
+#pragma unroll
+    for (int e = 0; e < BG; ++e) {
+      if (TPR == 2) yv[e] += __shfl_xor_sync(0xffffffffu, yv[e], 1);
+      const float ss = warp_sum(part == 0 ? yv[e] * yv[e] : 0.f);
+      if (lane == 0) redv[e][wg] = ss;
+    }
+  }
+  __syncthreads();
+
+  // ---- stage 2 (append): unit vectors, codes, residual and its norm
+  if (kAppend) {
+    if (grp == 0 && part == 0) {
+#pragma unroll
+      for (int e = 0; e < BG; ++e) {
+        float n2 = 0.f;
+#pragma unroll
+        for (int w = 0; w < WG; ++w) n2 += redk[e][w];
+        const float n = sqrtf(n2);
+        const float u = n > 0.f ? yk[e] / n : 0.f;
+        const int c = code_of7(u, lutK);
+        const float r = u - lutK[c];
+        cK[e][row] = (unsigned char)c;
+        rr[e][row] = r;
+        yk[e] = r * r;
+      }
+    }
+    if (grp == 0) {  // whole warps: the shuffles need every lane
+#pragma unroll
+      for (int e = 0; e < BG; ++e) {
+        const float ss = warp_sum(part == 0 ? yk[e] : 0.f);
+        if (lane == 0) redr[e][wg] = ss;
+      }
+    } else if (grp == 2 && part == 0) {
+#pragma unroll
+      for (int e = 0; e < BG; ++e) {
+        float n2 = 0.f;
+#pragma unroll
+        for (int w = 0; w < WG; ++w) n2 += redv[e][w];
+        const float n = sqrtf(n2);
+        const float u = n > 0.f ? yv[e] / n : 0.f;
+        cV[e][row] = (unsigned char)code_of7(u, lutV);
+      }
+    }
     __syncthreads();
-    if (tid == 0) {
+  }
+
+  // ---- stage 3: sketch of the residual (bits) and of the rotated query (z)
+  if (grp == 1) {
+    float sr[BG], zq[BG];
+#pragma unroll
+    for (int e = 0; e < BG; ++e) sr[e] = 0.f, zq[e] = 0.f;
+    if (kAppend) rowreg.dot<BG>(&rr[0][part * 64], D, sr);
+    if (kQuery) rowreg.dot<BG>(&yq[0][part * 64], D, zq);
+#pragma unroll
+    for (int e = 0; e < BG; ++e) {
+      if (TPR == 2) {
+        sr[e] += __shfl_xor_sync(0xffffffffu, sr[e], 1);
+        zq[e] += __shfl_xor_sync(0xffffffffu, zq[e], 1);
+      }
+      if (part == 0) {
+        if (kAppend) bitb[e][row] = sr[e] >= 0.f ? 1 : 0;
+        if (kQuery && e < nb) a.qrot[(((size_t)lc * B + b0 + e) * H + h) * 2 * D + D + row] = zq[e] * kScaleS;
+      }
+    }
+  }
+  if (!kAppend) return;
+  __syncthreads();
+
+  // ---- stage 4 (append): every thread assembles one word of one token in the device layout (include/tq.h)
+  if (it_on) {
+    const int e = it_e, slot = it_slot;
+    unsigned char* tp = it_tp;
+    if (it < Lo::KCW) {
+      const int w = it;
+      unsigned long long word = 0;
+      const int k_lo = (32 * w) / 6, k_hi = (32 * w + 31) / 6;
+      for (int kf = k_lo; kf <= k_hi; ++kf) {
+        const int g = (kf + slot) % Lo::P;
+        unsigned long long f = cK[e][2 * g] | ((unsigned)cK[e][2 * g + 1] << 3);
+        const int sh = 6 * kf - 32 * w;  // negative for the field straddling in from the previous word
+        word |= sh >= 0 ? (f << sh) : (f >> (-sh));
+      }
+      *reinterpret_cast<unsigned*>(tp + Lo::kOffKC + word_offset(Lo::KCW, w, slot)) = (unsigned)word;
+    } else if (it < Lo::KCW + Lo::KSW) {
+      const int w = it - Lo::KCW;
+      unsigned word = 0;
+      for (int kn = 0; kn < 8; ++kn) {
+        const int ng = (8 * w + kn + slot) % Lo::NG;
+        const unsigned char* bb = &bitb[e][4 * ng];
+        word |= (unsigned)(bb[0] | (bb[1] << 1) | (bb[2] << 2) | (bb[3] << 3)) << (4 * kn);
+      }
+      *reinterpret_cast<unsigned*>(tp + Lo::kOffKS + word_offset(Lo::KSW, w, slot)) = word;
+    } else if (it < Lo::KCW + Lo::KSW + Lo::P) {
+      // V: pair group g lives in lane (g mod 32)'s string at bits [192 part + 6 slot, +6): modify the word read at
+      // the top (nobody else writes this token slot's bits, and the other slots' bits are not written by this launch)
+      const int g = it - Lo::KCW - Lo::KSW;
+      const unsigned f = cV[e][2 * g] | ((unsigned)cV[e][2 * g + 1] << 3);
+      const int s = (192 * (g / kTile) + 6 * slot) & 31;
+      *vp0 = (vold0 & ~(63u << s)) | (f << s);
+      if (s > 26) *vp1 = (vold1 & ~(63u >> (32 - s))) | (f >> (32 - s));
+    } else {
+      float nk = 0.f, nr = 0.f, nv = 0.f;
+#pragma unroll
+      for (int w = 0; w < WG; ++w) nk += redk[e][w], nr += redr[e][w], nv += redv[e][w];
+      reinterpret_cast<unsigned short*>(tp + Lo::kOffKN)[slot] = f32_to_f16_bits_clamped(sqrtf(nk));
+      reinterpret_cast<unsigned short*>(tp + Lo::kOffKR)[slot] = f32_to_f16_bits_clamped(sqrtf(nr));
+      reinterpret_cast<unsigned short*>(tp + Lo::kOffVN)[slot] = f32_to_f16_bits_clamped(sqrtf(nv));
+    }
+  }
+  // ---- arrival: the last head of a batch entry publishes the new length
+  __syncthreads();
+  if (tid < nb) {
+    const int lb = layer * B + b0 + tid;
+    __threadfence();
+    const int old = atomicAdd(&a.cv.arrive[lb], 1);
+    if (old == H - 1) {
+      a.cv.arrive[lb] = 0;
+      if (s_full[tid]) atomicExch(a.cv.status, (int)TQ_ERR_CAPACITY);
+      else a.cv.seq_len[lb] = s_len0[tid] + 1;
       __threadfence();
-      const int old = atomicAdd(&a.cv.arrive[lb], 1);
-      if (old == H - 1) {
-        a.cv.arrive[lb] = 0;
-        if (full) atomicExch(a.cv.status, (int)TQ_ERR_CAPACITY);
-        else a.cv.seq_len[lb] = len0 + 1;
-        __threadfence();
-      }
     }
   }
 }
 
 template <int D, typename T>
-static cudaError_t launch_prep_t(const PrepArgs& a, int units, bool do_append, bool do_query, cudaStream_t st) {
-  if (do_append && do_query) prep_kernel<D, T, true, true><<<units, 4 * D, 0, st>>>(a);
-  else if (do_append) prep_kernel<D, T, true, false><<<units, 4 * D, 0, st>>>(a);
-  else prep_kernel<D, T, false, true><<<units, 4 * D, 0, st>>>(a);
+static cudaError_t launch_prep_t(const PrepArgs& a, int lh_count, int B, bool do_append, bool do_query, cudaStream_t st) {
+  using Cfg = PrepCfg<D>;
+  const int nbg = (B + Cfg::BG - 1) / Cfg::BG;
+  const int grid = lh_count * nbg;
+  if (do_append && do_query) prep_kernel<D, T, true, true><<<grid, 3 * Cfg::GT, 0, st>>>(a, nbg);
+  else if (do_append) prep_kernel<D, T, true, false><<<grid, 3 * Cfg::GT, 0, st>>>(a, nbg);
+  else prep_kernel<D, T, false, true><<<grid, 2 * Cfg::GT, 0, st>>>(a, nbg);
   count_launch();
   return cudaGetLastError();
 }
@@ -258,12 +357,12 @@ cudaError_t launch_prep(const DecodeArgs& d, const void* k, const void* v, int D
   a.qrot = d.qrot;
   a.layer_begin = d.layer_begin;
   a.rope_layout = d.rope_layout;
-  const int units = d.n_layers_call * d.cv.B * d.cv.H;
+  const int lh_count = d.n_layers_call * d.cv.H;
   if (D == 64)
-    return d.dt == TQ_F16 ? launch_prep_t<64, __half>(a, units, do_append, do_query, st)
-                          : launch_prep_t<64, float>(a, units, do_append, do_query, st);
-  return d.dt == TQ_F16 ? launch_prep_t<128, __half>(a, units, do_append, do_query, st)
-                        : launch_prep_t<128, float>(a, units, do_append, do_query, st);
+    return d.dt == TQ_F16 ? launch_prep_t<64, __half>(a, lh_count, d.cv.B, do_append, do_query, st)
+                          : launch_prep_t<64, float>(a, lh_count, d.cv.B, do_append, do_query, st);
+  return d.dt == TQ_F16 ? launch_prep_t<128, __half>(a, lh_count, d.cv.B, do_append, do_query, st)
+                        : launch_prep_t<128, float>(a, lh_count, d.cv.B, do_append, do_query, st);
 }
 
 }  // namespace tq
