@@ -10,6 +10,8 @@
 // followed by warp-shuffle norm reductions and a conflict-free word assembly.  All arithmetic is fp32
 // with IEEE division and square root so that codes agree with the fp64 oracle except inside the 1e-5
 // band around a threshold.
+#include <cstdlib>
+
 #include "tq_common.cuh"
 
 namespace tq {
@@ -297,7 +299,16 @@ cudaError_t launch_quantize_pack(const QuantArgs& a, int D, tq_dtype dt, int num
     count_launch();
     return cudaGetLastError();
   }
-  if (D == 64) return dt == TQ_F16 ? launch_quant_t<64, __half>(a, num_sms, st) : launch_quant_t<64, float>(a, num_sms, st);
+  if (D == 64) {
+    // head_dim 64 runs on the tensor cores (tq_quantize_tc.cu); TQ_QUANTIZE_IMPL=fp32 selects the CUDA-core kernel below
+    // (kept as the d = 128 path and as a cross-check)
+    static const bool force_fp32 = [] {
+      const char* e = getenv("TQ_QUANTIZE_IMPL");
+      return e && e[0] == 'f';
+    }();
+    if (!force_fp32) return launch_quantize_pack_tc(a, dt, num_sms, st);
+    return dt == TQ_F16 ? launch_quant_t<64, __half>(a, num_sms, st) : launch_quant_t<64, float>(a, num_sms, st);
+  }
   return dt == TQ_F16 ? launch_quant_t<128, __half>(a, num_sms, st) : launch_quant_t<128, float>(a, num_sms, st);
 }
 

@@ -73,7 +73,9 @@ def compare_quantize(can_oracle, gpu: dict, d: int, what: str = ""):
             dd = dd[mask]
         assert dd.max(initial=0) <= 1, (what, name, dd.max())
         rep[f"{name}_ulp_mismatch_frac"] = float((dd > 0).mean()) if dd.size else 0.0
-        assert rep[f"{name}_ulp_mismatch_frac"] <= 2e-3, (what, name, rep[f"{name}_ulp_mismatch_frac"])
+        # ... which happens to a fraction ~ (relative error of the fp32 norm) / (binary16 spacing 2^-11) of the entries;
+        # a single such entry is always allowed (small cases have only a few hundred norms)
+        assert rep[f"{name}_ulp_mismatch_frac"] <= max(2e-3, 1.0 / max(1, dd.size)), (what, name, rep[f"{name}_ulp_mismatch_frac"])
     del rep["k_vec_equal"], rep["v_vec_equal"]
     return rep
 
