@@ -36,6 +36,7 @@ from paper_2603_26110_b200 import workloads as W
 METRIC = "fused 3-bit decode-attn cached tokens/s"
 UNIT = "cached token-heads/s"
 FALLBACK_HBM_GBS = 6650.0  # B200_PROFILING.md fallback
+NCU_DRAM_BYTES_PER_LAUNCH = 42.63e6  # decode_main_kernel, one ncu --set full capture (profiles/r01_decode_main_full.md)
 
 
 def measured_peaks():
@@ -359,6 +360,24 @@ def run_ours(args, w: W.Workload):
     dec_bytes = B * H * T0 * 62
     dec_s = statistics.mean(dec_ms) * 1e-3
 
+    # ---- the dominant kernel alone (decode_main_kernel): the library records a CUDA event pair on `stream` directly
+    #      around that launch (tq_profile_decode_events), in a stream that is kept busy with calls over all L layer caches
+    with torch.cuda.stream(stream):
+        k0, k1 = ev(), ev()
+        k0.record(stream), k1.record(stream)  # create the handles
+        stream.synchronize()
+        tq.tq_profile_decode_events(k0, k1)
+        main_ms = []
+        for it in range(12):  # each round: L back-to-back calls, the events end up around the LAST streaming launch
+            for layer in range(L):
+                tq.tq_decode_attn(shape, params, cache, layer, 1, qs[layer:layer + 1], outs[layer:layer + 1], ws, None,
+                                  max_seq, stream)
+            k1.synchronize()
+            if it > 1:
+                main_ms.append(k0.elapsed_time(k1))
+        tq.tq_profile_decode_events(None, None)
+    main_s = statistics.mean(main_ms) * 1e-3
+
     # ---- end to end through the host-buffer call: pinned q/k/v in, out back, every layer of every step
     e2e_steps = max(3, min(args.steps, 20))
     staging = torch.zeros(tq.tq_step_staging_bytes(shape, dt_code) + 256, dtype=torch.uint8, device=dev)
@@ -392,7 +411,7 @@ def run_ours(args, w: W.Workload):
             dist.destroy_process_group()
         return
     peak, peak_src = measured_peaks()
-    achieved = dec_bytes / dec_s / 1e9
+    achieved = dec_bytes / main_s / 1e9
     value = whole_job_value(tok_heads, world, ms_max)
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
@@ -406,7 +425,8 @@ def run_ours(args, w: W.Workload):
             "cuda_graph": True, "bytes_per_token_head": 62,
             "us_per_layer_step": 1e3 * ms_max / args.steps / L,
             "packed_gbs_whole_step": value / world * 62 / 1e9,
-            "decode_call_us_live": dec_s * 1e6,
+            "decode_call_us_live": dec_s * 1e6, "decode_call_packed_gbs": dec_bytes / dec_s / 1e9,
+            "decode_main_kernel_us_live": main_s * 1e6,
             "quantize_pack_gbs": quant_gbs, "quantize_pack_ms_per_layer": statistics.median(q_ms),
             "parallelism": f"dp{world} (independent batches, no collective)",
         },
@@ -415,7 +435,8 @@ def run_ours(args, w: W.Workload):
                 "d2h_bytes_per_step": L * vec_bytes, "steps": e2e_steps},
         "gpu_launches": int(launches_per_step * args.steps),
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": None, "kernel": "tq_decode_attn call (decode_prep_kernel + decode_main_kernel)",
+                     "traffic": NCU_DRAM_BYTES_PER_LAUNCH, "kernel": "decode_main_kernel<64, __half>",
+                     "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum per launch, profiles/r01_decode_main_full.md",
                      "peak_source": peak_src, "bytes_per_launch": dec_bytes},
     }
     if world == 1 and not args.no_cpu_baseline:

@@ -129,11 +129,15 @@ __device__ __forceinline__ void pow2_scale(float amax, float& s, float& inv_s) {
   inv_s = __uint_as_float(E << 23);
 }
 
+// code = #{k : u > thr[k]} for ascending thresholds, as a three-step binary search (3 compares + 4 selects instead of
+// 7 compares + 7 adds); identical result, ties included (u > t is evaluated on the same thresholds)
 __device__ __forceinline__ int code_of(float u, const float (&thr)[7]) {
-  int c = 0;
-#pragma unroll
-  for (int q = 0; q < 7; ++q) c += (u > thr[q]) ? 1 : 0;
-  return c;
+  const bool b2 = u > thr[3];
+  const float tm = b2 ? thr[5] : thr[1];
+  const bool b1 = u > tm;
+  const float tl = b2 ? (b1 ? thr[6] : thr[4]) : (b1 ? thr[2] : thr[0]);
+  const bool b0 = u > tl;
+  return (b2 ? 4 : 0) + (b1 ? 2 : 0) + (b0 ? 1 : 0);
 }
 
 template <typename T>
