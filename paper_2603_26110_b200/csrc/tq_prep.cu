@@ -49,6 +49,10 @@ struct RowRegs64 {
 #pragma unroll
     for (int c = 0; c < 16; ++c) m[c] = __ldg(reinterpret_cast<const float4*>(p) + c);
   }
+  __device__ __forceinline__ void load_shared(const float* p) {  // 16-byte aligned, conflict-free for a 68-float row pitch
+#pragma unroll
+    for (int c = 0; c < 16; ++c) m[c] = *(reinterpret_cast<const float4*>(p) + c);
+  }
   // acc[e] += <row part, x[e] part>, x in shared memory (every lane of a row group reads the same address)
   template <int BG>
   __device__ __forceinline__ void dot(const float* xs /* [BG][stride] */, int stride, float (&acc)[BG]) const {
@@ -93,9 +97,23 @@ __global__ void __launch_bounds__((kAppend ? 3 : 2) * PrepCfg<D>::GT) prep_kerne
   int len_e[BG];
 #pragma unroll
   for (int e = 0; e < BG; ++e) len_e[e] = e < nb ? __ldcg(a.cv.seq_len + layer * B + b0 + e) : 0;
-  // ---- matrix rows into registers: the only loads that miss L2 after the first CTA of a head
+  // ---- matrix rows into registers.  d = 64: the CTA copies its (up to) three 16 KB matrices with fully coalesced
+  //      16-byte cp.async into shared memory (row pitch 68 floats: a thread-per-row read is then conflict free) and
+  //      every thread picks up its row from there; d = 128: straight from global memory (three 64 KB matrices do not fit)
+  constexpr bool kStageRows = D == 64;
+  constexpr int kPitch = 68;
+  extern __shared__ __align__(16) float msm[];  // [groups][D][kPitch] when kStageRows
   RowRegs64 rowreg;
-  {
+  if (kStageRows) {
+    constexpr int NG_ = kAppend ? 3 : 2;
+    for (int idx = tid; idx < NG_ * D * (D / 4); idx += NT) {
+      const int gsel = idx / (D * (D / 4)), rem = idx % (D * (D / 4)), r = rem / (D / 4), c4 = rem % (D / 4);
+      const float* M = gsel == 0 ? a.pi_k + lh * D * D : gsel == 1 ? a.S : a.pi_v + lh * D * D;
+      const unsigned dst = (unsigned)__cvta_generic_to_shared(msm + ((size_t)gsel * D + r) * kPitch + 4 * c4);
+      asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(M + (size_t)r * D + 4 * c4) : "memory");
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+  } else {
     const float* M = grp == 0 ? a.pi_k + lh * D * D : grp == 1 ? a.S : a.pi_v + lh * D * D;
     rowreg.load(M + (size_t)row * D + part * 64);
   }
@@ -174,7 +192,9 @@ __global__ void __launch_bounds__((kAppend ? 3 : 2) * PrepCfg<D>::GT) prep_kerne
       xv[e][i] = e < nb ? load_as_float<T>(reinterpret_cast<const T*>(a.v) + (((size_t)lc * B + b0 + e) * H + h) * D + i) : 0.f;
     }
   }
+  if (kStageRows) asm volatile("cp.async.wait_group 0;" ::: "memory");
   __syncthreads();
+  if (kStageRows) rowreg.load_shared(msm + ((size_t)grp * D + row) * kPitch);
 
   // ---- stage 1: rotations (groups 0 and 2) and the norms of the rotated key / value
   float yk[BG], yv[BG];
@@ -332,9 +352,18 @@ static cudaError_t launch_prep_t(const PrepArgs& a, int lh_count, int B, bool do
   using Cfg = PrepCfg<D>;
   const int nbg = (B + Cfg::BG - 1) / Cfg::BG;
   const int grid = lh_count * nbg;
-  if (do_append && do_query) prep_kernel<D, T, true, true><<<grid, 3 * Cfg::GT, 0, st>>>(a, nbg);
-  else if (do_append) prep_kernel<D, T, true, false><<<grid, 3 * Cfg::GT, 0, st>>>(a, nbg);
-  else prep_kernel<D, T, false, true><<<grid, 2 * Cfg::GT, 0, st>>>(a, nbg);
+  const size_t sm3 = D == 64 ? (size_t)3 * D * 68 * 4 : 0, sm2 = D == 64 ? (size_t)2 * D * 68 * 4 : 0;
+  static bool attr_set = false;
+  if (!attr_set && D == 64) {
+    cudaError_t e1 = cudaFuncSetAttribute(prep_kernel<D, T, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm3);
+    cudaError_t e2 = cudaFuncSetAttribute(prep_kernel<D, T, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm3);
+    if (e1 != cudaSuccess) return e1;
+    if (e2 != cudaSuccess) return e2;
+    attr_set = true;
+  }
+  if (do_append && do_query) prep_kernel<D, T, true, true><<<grid, 3 * Cfg::GT, sm3, st>>>(a, nbg);
+  else if (do_append) prep_kernel<D, T, true, false><<<grid, 3 * Cfg::GT, sm3, st>>>(a, nbg);
+  else prep_kernel<D, T, false, true><<<grid, 2 * Cfg::GT, sm2, st>>>(a, nbg);
   count_launch();
   return cudaGetLastError();
 }
