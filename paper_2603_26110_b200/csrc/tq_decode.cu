@@ -122,34 +122,35 @@ __device__ __forceinline__ f32x2 lds_b64(unsigned addr) {
 }
 
 // <q'', lut_K[codes]>: P table reads, summed two at a time
-template <int D, int K>
-__device__ __forceinline__ f32x2 k_pair(const unsigned (&kw)[Layout<D>::KCW], unsigned kbase) {
-  return pack2(lds_f32<8 * K>(field_at<DecodeCfg<D>::LSK, 12 * K, 6>(kw) | kbase),
-               lds_f32<8 * K + 4>(field_at<DecodeCfg<D>::LSK, 12 * K + 6, 6>(kw) | kbase));
+// pairwise (tree) sum of N packed pairs, then of the two halves: short dependency chains for the scheduler
+template <int N>
+__device__ __forceinline__ float tree_sum(f32x2 (&v)[N]) {
+#pragma unroll
+  for (int n = N / 2; n >= 1; n >>= 1)
+#pragma unroll
+    for (int i = 0; i < n; ++i) v[i] = add2(v[i], v[i + n]);
+  float a, b;
+  unpack2(v[0], a, b);
+  return a + b;
 }
 template <int D, int... K>
 __device__ __forceinline__ float k_score(const unsigned (&kw)[Layout<D>::KCW], unsigned kbase,
                                          std::integer_sequence<int, K...>) {
-  f32x2 acc[2] = {k_pair<D, 0>(kw, kbase), k_pair<D, 1>(kw, kbase)};
-  ((acc[K & 1] = add2(acc[K & 1], k_pair<D, K + 2>(kw, kbase))), ...);
-  float a, b;
-  unpack2(add2(acc[0], acc[1]), a, b);
-  return a + b;
+  // all table addresses first, then all reads, then the sum: three wide phases instead of 32 short chains
+  const unsigned a0[sizeof...(K)] = {(field_at<DecodeCfg<D>::LSK, 12 * K, 6>(kw) | kbase)...};
+  const unsigned a1[sizeof...(K)] = {(field_at<DecodeCfg<D>::LSK, 12 * K + 6, 6>(kw) | kbase)...};
+  f32x2 v[sizeof...(K)] = {pack2(lds_f32<8 * K>(a0[K]), lds_f32<8 * K + 4>(a1[K]))...};
+  return tree_sum(v);
 }
 
 // <z, sigma>: d/4 nibble-table reads
-template <int D, int K>
-__device__ __forceinline__ f32x2 s_pair(const unsigned (&sw)[Layout<D>::KSW], unsigned sbase) {
-  return pack2(lds_f32<8 * K>(field_at<8, 8 * K, 4>(sw) | sbase), lds_f32<8 * K + 4>(field_at<8, 8 * K + 4, 4>(sw) | sbase));
-}
 template <int D, int... K>
 __device__ __forceinline__ float s_score(const unsigned (&sw)[Layout<D>::KSW], unsigned sbase,
                                          std::integer_sequence<int, K...>) {
-  f32x2 acc[2] = {s_pair<D, 0>(sw, sbase), s_pair<D, 1>(sw, sbase)};
-  ((acc[K & 1] = add2(acc[K & 1], s_pair<D, K + 2>(sw, sbase))), ...);
-  float a, b;
-  unpack2(add2(acc[0], acc[1]), a, b);
-  return a + b;
+  const unsigned a0[sizeof...(K)] = {(field_at<8, 8 * K, 4>(sw) | sbase)...};
+  const unsigned a1[sizeof...(K)] = {(field_at<8, 8 * K + 4, 4>(sw) | sbase)...};
+  f32x2 v[sizeof...(K)] = {pack2(lds_f32<8 * K>(a0[K]), lds_f32<8 * K + 4>(a1[K]))...};
+  return tree_sum(v);
 }
 
 // V accumulate, lane = coordinate pair: for token J of the tile, o2[part] += w_J * (lut_V[c0], lut_V[c1])
@@ -387,8 +388,8 @@ __global__ void __launch_bounds__(kDecodeThreads, DecodeCfg<D>::kCtasPerSm) deco
   // one 32-token tile: scores (lane = token) -> online softmax -> V accumulate (lane = coordinate pair)
   auto process = [&](const TileWords<D>& tw, int tile) {
     const bool valid = tile * kTile + lane < T;
-    const float sa = k_score<D>(tw.kw, kbase, std::make_integer_sequence<int, Lo::P / 2 - 2>{});
-    const float sb = s_score<D>(tw.sw, sbase, std::make_integer_sequence<int, Lo::NG / 2 - 2>{});
+    const float sa = k_score<D>(tw.kw, kbase, std::make_integer_sequence<int, Lo::P / 2>{});
+    const float sb = s_score<D>(tw.sw, sbase, std::make_integer_sequence<int, Lo::NG / 2>{});
     float s2 = f16_bits_to_f32(tw.kn) * fmaf(f16_bits_to_f32(tw.kr), sb, sa);
     s2 = valid ? s2 : -INFINITY;
     const float mnew = fmaxf(m, warp_max_f32(s2));  // finite: slot 0 of every processed tile is valid
