@@ -23,7 +23,7 @@ constexpr int kD = 64;
 constexpr int kBlk = 128;             // tokens per block = UMMA M = threads per CTA
 constexpr int kOpBytes = kBlk * kD * 2;  // one fp16 A operand: 16 KB
 constexpr int kMatBytes = kD * kD * 2;   // one fp16 B operand: 8 KB
-constexpr int kTmemCols = 256;        // D_K [0,64), D_V [64,128), D_S [128,192)
+constexpr int kTmemCols = 128;        // key CTAs: D_K [0,64), D_S [64,128); value CTAs: D_V [0,64)
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -96,11 +96,12 @@ __device__ __forceinline__ void tmem_ld64(uint32_t taddr, float (&v)[64]) {
 __device__ __forceinline__ void split8(const float* x, uint4& hi, uint4& lo) {
   unsigned h[4], l[4];
 #pragma unroll
-  for (int j = 0; j < 4; ++j) {
-    const __half h0 = __float2half_rn(x[2 * j]), h1 = __float2half_rn(x[2 * j + 1]);
-    const __half l0 = __float2half_rn(x[2 * j] - __half2float(h0)), l1 = __float2half_rn(x[2 * j + 1] - __half2float(h1));
-    h[j] = (unsigned)__half_as_ushort(h0) | ((unsigned)__half_as_ushort(h1) << 16);
-    l[j] = (unsigned)__half_as_ushort(l0) | ((unsigned)__half_as_ushort(l1) << 16);
+  for (int j = 0; j < 4; ++j) {  // packed conversions: one cvt per pair each way
+    const __half2 h2 = __floats2half2_rn(x[2 * j], x[2 * j + 1]);
+    const float2 hf = __half22float2(h2);
+    const __half2 l2 = __floats2half2_rn(x[2 * j] - hf.x, x[2 * j + 1] - hf.y);
+    h[j] = *reinterpret_cast<const unsigned*>(&h2);
+    l[j] = *reinterpret_cast<const unsigned*>(&l2);
   }
   hi = make_uint4(h[0], h[1], h[2], h[3]);
   lo = make_uint4(l[0], l[1], l[2], l[3]);
@@ -185,15 +186,19 @@ __device__ __forceinline__ float stage_split(const float (&x)[64], unsigned char
   return inv_s;
 }
 
-template <typename T>
-__global__ void __launch_bounds__(kBlk) quantize_pack_tc_kernel(QuantArgs a, int blocks_per_cta) {
+// Shared memory of one CTA (keys and values run as separate CTAs, blockIdx.z, so that three of them fit an SM):
+//   B operands 4 x 8 KB (keys: PI_K hi/lo, S hi/lo; values: PI_V hi/lo) | A operands 2 x 16 KB (hi, lo) | staging, LUT,
+//   barriers
+constexpr int kOffA = 4 * kMatBytes, kOffMisc = kOffA + 2 * kOpBytes;
+constexpr int kSmemBytes = kOffMisc + kBlk * 32 + kBlk * 7 * 4 + 8 * 4 + 3 * 8 + 16;
+
+template <typename T, bool kKey>
+__device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int blocks_per_cta, unsigned char* smem) {
   using Lo = Layout<kD>;
   constexpr bool kF16 = sizeof(T) == 2;
-  constexpr int kOffA = 6 * kMatBytes, kOffAV = kOffA + 2 * kOpBytes, kOffMisc = kOffAV + (kF16 ? 1 : 2) * kOpBytes;
-  extern __shared__ __align__(1024) unsigned char smem[];
   unsigned char *Bk_hi = smem, *Bk_lo = smem + kMatBytes, *Bs_hi = smem + 2 * kMatBytes, *Bs_lo = smem + 3 * kMatBytes,
-                *Bv_hi = smem + 4 * kMatBytes, *Bv_lo = smem + 5 * kMatBytes;
-  unsigned char *A_hi = smem + kOffA, *A_lo = A_hi + kOpBytes, *AV_hi = smem + kOffAV, *AV_lo = AV_hi + kOpBytes;
+                *Bv_hi = smem, *Bv_lo = smem + kMatBytes;
+  unsigned char *A_hi = smem + kOffA, *A_lo = A_hi + kOpBytes, *AV_hi = A_hi, *AV_lo = A_lo;
   unsigned char* cbV = smem + kOffMisc;                                  // [128 tokens][32 pair fields]
   unsigned* crot = reinterpret_cast<unsigned*>(cbV + kBlk * 32);          // [128][7] K code words, rotation staging
   float* lutK = reinterpret_cast<float*>(crot + kBlk * 7);                // [8]
@@ -206,7 +211,7 @@ __global__ void __launch_bounds__(kBlk) quantize_pack_tc_kernel(QuantArgs a, int
   const int blk0 = first_blk + (int)blockIdx.x * blocks_per_cta;
   if (blk0 > last_blk) return;
   const int blk1 = min(last_blk, blk0 + blocks_per_cta - 1);
-  if (blockIdx.x == 0 && h == 0 && tid == 0) a.cv.seq_len[a.layer * a.cv.B + b] = a.start_pos + a.n_tokens;
+  if (kKey && blockIdx.x == 0 && h == 0 && tid == 0) a.cv.seq_len[a.layer * a.cv.B + b] = a.start_pos + a.n_tokens;
 
   // ---- one-time setup: tensor memory, barriers, the three B operands of this head, LUTs
   if (warp == 0) {
@@ -220,9 +225,12 @@ __global__ void __launch_bounds__(kBlk) quantize_pack_tc_kernel(QuantArgs a, int
     mbar_init(smem_u32(mbar + 2), 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  stage_matrix(Bk_hi, Bk_lo, a.pi_k + (size_t)h * kD * kD, 16.f, tid);
-  stage_matrix(Bs_hi, Bs_lo, a.S, 1.f, tid);
-  stage_matrix(Bv_hi, Bv_lo, a.pi_v + (size_t)h * kD * kD, 16.f, tid);
+  if constexpr (kKey) {
+    stage_matrix(Bk_hi, Bk_lo, a.pi_k + (size_t)h * kD * kD, 16.f, tid);
+    stage_matrix(Bs_hi, Bs_lo, a.S, 1.f, tid);
+  } else {
+    stage_matrix(Bv_hi, Bv_lo, a.pi_v + (size_t)h * kD * kD, 16.f, tid);
+  }
   float thrK[7], thrV[7], lutVr[8];
   {
     float lk[8];
@@ -261,7 +269,7 @@ __global__ void __launch_bounds__(kBlk) quantize_pack_tc_kernel(QuantArgs a, int
 
     // ---- stage the A operands: RoPE'd, scaled, split keys; values (exact fp16 operands when the input is fp16)
     float inv_sk = 1.f, inv_sv = 1.f;
-    {
+    if constexpr (kKey) {
       float x[64];
       if (valid) load_vec64<T>(ksrc + (size_t)i * kD, x);
       else {
@@ -283,8 +291,7 @@ __global__ void __launch_bounds__(kBlk) quantize_pack_tc_kernel(QuantArgs a, int
         }
       }
       inv_sk = stage_split(x, A_hi, A_lo, tid);
-    }
-    if (kF16) {
+    } else if (kF16) {
 #pragma unroll
       for (int kj = 0; kj < 8; ++kj) {
         const uint4 v = valid ? __ldg(reinterpret_cast<const uint4*>(vsrc + (size_t)i * kD) + kj) : make_uint4(0, 0, 0, 0);
@@ -304,14 +311,18 @@ __global__ void __launch_bounds__(kBlk) quantize_pack_tc_kernel(QuantArgs a, int
     __syncthreads();
     if (tid == 0) {
       tc_fence_after();
-      gemm(0, aK_hi, bK_hi, true), gemm(0, aK_lo, bK_hi, false), gemm(0, aK_hi, bK_lo, false);
-      umma_commit(smem_u32(mbar + 0));
-      gemm(64, aV_hi, bV_hi, true), gemm(64, aV_hi, bV_lo, false);
-      if (!kF16) gemm(64, aV_lo, bV_hi, false);
-      umma_commit(smem_u32(mbar + 1));
+      if constexpr (kKey) {
+        gemm(0, aK_hi, bK_hi, true), gemm(0, aK_lo, bK_hi, false), gemm(0, aK_hi, bK_lo, false);
+        umma_commit(smem_u32(mbar + 0));
+      } else {
+        gemm(0, aV_hi, bV_hi, true), gemm(0, aV_hi, bV_lo, false);
+        if (!kF16) gemm(0, aV_lo, bV_hi, false);
+        umma_commit(smem_u32(mbar + 1));
+      }
     }
 
     // ---- keys: thread = token.  y = D_K / (16 s): norm, unit vector, codes, residual, its norm
+    if constexpr (kKey) {
     mbar_wait(smem_u32(mbar + 0), parity);
     tc_fence_after();
     {
@@ -368,16 +379,18 @@ __global__ void __launch_bounds__(kBlk) quantize_pack_tc_kernel(QuantArgs a, int
     __syncthreads();
     if (tid == 0) {
       tc_fence_after();
-      gemm(128, aK_hi, bS_hi, true), gemm(128, aK_lo, bS_hi, false), gemm(128, aK_hi, bS_lo, false);
+      gemm(64, aK_hi, bS_hi, true), gemm(64, aK_lo, bS_hi, false), gemm(64, aK_hi, bS_lo, false);
       umma_commit(smem_u32(mbar + 2));
     }
+    }  // kKey
 
     // ---- values: norm, codes; the cache stores V codes per coordinate pair across the 32 tokens of a tile
+    if constexpr (!kKey) {
     mbar_wait(smem_u32(mbar + 1), parity);
     tc_fence_after();
     {
       float y[64];
-      tmem_ld64(t_lane + 64, y);
+      tmem_ld64(t_lane + 0, y);
       float n2 = 0.f;
 #pragma unroll
       for (int j = 0; j < 64; ++j) n2 = fmaf(y[j], y[j], n2);
@@ -424,12 +437,15 @@ __global__ void __launch_bounds__(kBlk) quantize_pack_tc_kernel(QuantArgs a, int
       }
     }
 
+    }  // !kKey
+
     // ---- residual sketch: bit j = [(S r)_j >= 0]; nibble group n sits at nibble position (n - t) mod 16
+    if constexpr (kKey) {
     mbar_wait(smem_u32(mbar + 2), parity);
     tc_fence_after();
     {
       float y[64];
-      tmem_ld64(t_lane + 128, y);
+      tmem_ld64(t_lane + 64, y);
       unsigned long long bits = 0ull;
 #pragma unroll
       for (int j = 0; j < 64; ++j) bits |= (unsigned long long)(y[j] >= 0.f ? 1u : 0u) << j;
@@ -437,6 +453,7 @@ __global__ void __launch_bounds__(kBlk) quantize_pack_tc_kernel(QuantArgs a, int
       const unsigned long long rot = rs ? ((bits >> rs) | (bits << (64 - rs))) : bits;
       if (valid) *reinterpret_cast<uint2*>(tp + Lo::kOffKS + slot * 8) = make_uint2((unsigned)rot, (unsigned)(rot >> 32));
     }
+    }  // kKey
     tc_fence_before();  // the next block's MMAs overwrite the accumulators every thread has just read
   }
   __syncthreads();
@@ -447,16 +464,22 @@ __global__ void __launch_bounds__(kBlk) quantize_pack_tc_kernel(QuantArgs a, int
 }
 
 template <typename T>
+__global__ void __launch_bounds__(kBlk) quantize_pack_tc_kernel(QuantArgs a, int blocks_per_cta) {
+  extern __shared__ __align__(1024) unsigned char smem_dyn[];
+  if (blockIdx.z == 0) quantize_pack_tc_body<T, true>(a, blocks_per_cta, smem_dyn);
+  else quantize_pack_tc_body<T, false>(a, blocks_per_cta, smem_dyn);
+}
+
+template <typename T>
 cudaError_t launch_quant_tc_t(const QuantArgs& a, int num_sms, cudaStream_t st) {
-  constexpr bool kF16 = sizeof(T) == 2;
-  const size_t smem = 6 * kMatBytes + (kF16 ? 3 : 4) * kOpBytes + kBlk * 32 + kBlk * 7 * 4 + 8 * 4 + 3 * 8 + 16;
+  const size_t smem = kSmemBytes;
   const int first_blk = a.start_pos / kBlk, last_blk = (a.start_pos + a.n_tokens - 1) / kBlk;
   const int nblk = last_blk - first_blk + 1;
   const int BH = a.cv.B * a.cv.H;
-  const long want = 8L * num_sms;  // CTAs: enough to balance the SMs, few enough to amortise staging the matrices
+  const long want = 6L * num_sms;  // per operand (keys / values)  // CTAs: enough to balance the SMs, few enough to amortise staging the matrices
   int bpc = (int)(((long)nblk * BH + want - 1) / want);
   bpc = bpc < 1 ? 1 : (bpc > 16 ? 16 : bpc);
-  dim3 grid((nblk + bpc - 1) / bpc, BH);
+  dim3 grid((nblk + bpc - 1) / bpc, BH, 2);  // z: keys | values
   cudaError_t e = cudaFuncSetAttribute(quantize_pack_tc_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
   quantize_pack_tc_kernel<T><<<grid, kBlk, smem, st>>>(a, bpc);
