@@ -189,12 +189,11 @@ int tq_decode_step_host(const tq_shape *shape, const tq_params *dev, tq_cache *c
 const char *tq_status_string(int status);
 /* Number of kernels the library launched since load (bench.py's gpu_launches).                          */
 int64_t tq_launch_count(void);
-/* Measurement hook (bench.py's roofline leg): while two cudaEvent_t handles are set, every tq_decode_attn /
- * tq_decode_step records them on the call's stream directly before and after the launch of the streaming
- * fused-attention kernel (not the small query-preparation launch in front of it), so that the caller can
- * read that kernel's own duration with cudaEventElapsedTime.  Pass NULL, NULL to switch it off.  Process-wide
- * state; not for use during stream capture.                                                              */
-void tq_profile_decode_events(void *cuda_event_begin, void *cuda_event_end);
+/* Measurement hook (bench.py's roofline leg): while on, tq_decode_attn launches ONLY the streaming
+ * fused-attention kernel and re-uses the rotated queries its previous ordinary call left in the workspace
+ * (same queries, same layers), so that a run of such calls times that kernel alone.  Process-wide state;
+ * results are only meaningful directly after an ordinary call with the same arguments.                   */
+void tq_profile_decode_main_only(int on);
 
 #ifdef __cplusplus
 }

@@ -22,7 +22,7 @@ EXPORTS = [
     "tq_cache_bytes", "tq_cache_bytes_per_token_head", "tq_cache_seq_len_offset", "tq_cache_status_offset",
     "tq_decode_workspace_bytes", "tq_canonical_plane_bytes", "tq_calibrate_host", "tq_quantize_pack", "tq_append",
     "tq_decode_attn", "tq_decode_step", "tq_cache_export_canonical", "tq_cache_import_canonical", "tq_step_staging_bytes",
-    "tq_decode_step_host", "tq_status_string", "tq_launch_count", "tq_profile_decode_events",
+    "tq_decode_step_host", "tq_status_string", "tq_launch_count", "tq_profile_decode_main_only",
 ]
 
 
@@ -140,11 +140,9 @@ def tq_launch_count() -> int:
     return int(lib().tq_launch_count())
 
 
-def tq_profile_decode_events(begin=None, end=None):
-    """begin, end: torch.cuda.Event(enable_timing=True) that have been recorded once (so their handles exist), or
-    None to switch the hook off."""
-    lib().tq_profile_decode_events(C.c_void_p(begin.cuda_event if begin is not None else None),
-                                   C.c_void_p(end.cuda_event if end is not None else None))
+def tq_profile_decode_main_only(on: bool):
+    """Measurement hook: tq_decode_attn launches only the streaming kernel (queries from the previous ordinary call)."""
+    lib().tq_profile_decode_main_only(C.c_int(1 if on else 0))
 
 
 # ---- calibration (host) -------------------------------------------------------------------------------

@@ -10,7 +10,7 @@
 namespace tq {
 
 static std::atomic<long long> g_launches{0};
-static cudaEvent_t g_ev_begin = nullptr, g_ev_end = nullptr;  // tq_profile_decode_events
+static int g_profile_skip_prep = 0;  // tq_profile_decode_main_only
 void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
 
 
@@ -215,12 +215,10 @@ static int run_decode(const tq_shape* shape, const tq_params* dev, const tq_cach
     a.dt = (int)dt;
     const void* kc = k ? (const unsigned char*)k + u0 * g.D * esz : nullptr;
     const void* vc = v ? (const unsigned char*)v + u0 * g.D * esz : nullptr;
-    if (launch_prep(a, kc, vc, g.D, do_append, do_query, (cudaStream_t)cuda_stream) != cudaSuccess) return TQ_ERR_CUDA;
-    if (do_query) {
-      if (g_ev_begin && cudaEventRecord(g_ev_begin, (cudaStream_t)cuda_stream) != cudaSuccess) return TQ_ERR_CUDA;
-      if (launch_decode(a, g.D, (cudaStream_t)cuda_stream) != cudaSuccess) return TQ_ERR_CUDA;
-      if (g_ev_end && cudaEventRecord(g_ev_end, (cudaStream_t)cuda_stream) != cudaSuccess) return TQ_ERR_CUDA;
-    }
+    if (!(g_profile_skip_prep && do_query && !do_append) &&
+        launch_prep(a, kc, vc, g.D, do_append, do_query, (cudaStream_t)cuda_stream) != cudaSuccess)
+      return TQ_ERR_CUDA;
+    if (do_query && launch_decode(a, g.D, (cudaStream_t)cuda_stream) != cudaSuccess) return TQ_ERR_CUDA;
   }
   return TQ_OK;
 }
@@ -327,9 +325,6 @@ const char* tq_status_string(int status) {
 
 int64_t tq_launch_count(void) { return (int64_t)tq::g_launches.load(); }
 
-void tq_profile_decode_events(void* cuda_event_begin, void* cuda_event_end) {
-  tq::g_ev_begin = (cudaEvent_t)cuda_event_begin;
-  tq::g_ev_end = (cudaEvent_t)cuda_event_end;
-}
+void tq_profile_decode_main_only(int on) { tq::g_profile_skip_prep = on != 0; }
 
 }  // extern "C"
