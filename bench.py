@@ -36,7 +36,7 @@ from paper_2603_26110_b200 import workloads as W
 METRIC = "fused 3-bit decode-attn cached tokens/s"
 UNIT = "cached token-heads/s"
 FALLBACK_HBM_GBS = 6650.0  # B200_PROFILING.md fallback
-NCU_DRAM_BYTES_PER_LAUNCH = 42.63e6  # decode_main_kernel, one ncu --set full capture (profiles/r01_decode_main_full.md)
+NCU_DRAM_BYTES_PER_LAUNCH = 42.63e6  # decode_main_kernel, one ncu --set full capture (profiles/r01b_decode_main_full.md)
 
 
 def measured_peaks():
@@ -449,7 +449,7 @@ def run_ours(args, w: W.Workload):
         "gpu_launches": int(launches_per_step * args.steps),
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "traffic": NCU_DRAM_BYTES_PER_LAUNCH, "kernel": "decode_main_kernel<64, __half>",
-                     "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum per launch, profiles/r01_decode_main_full.md",
+                     "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum per launch, profiles/r01b_decode_main_full.md",
                      "peak_source": peak_src, "bytes_per_launch": dec_bytes},
     }
     if world == 1 and not args.no_cpu_baseline:
