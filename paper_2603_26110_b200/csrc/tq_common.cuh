@@ -130,7 +130,7 @@ struct DecodeArgs {
 };
 
 cudaError_t launch_quantize_pack(const QuantArgs& a, int D, tq_dtype dt, int num_sms, cudaStream_t st);
-cudaError_t launch_quantize_pack_tc(const QuantArgs& a, tq_dtype dt, int num_sms, cudaStream_t st);  // d = 64, tcgen05
+cudaError_t launch_quantize_pack_tc(const QuantArgs& a, int D, tq_dtype dt, int num_sms, cudaStream_t st);  // tcgen05
 cudaError_t launch_prep(const DecodeArgs& d, const void* k, const void* v, int D, bool do_append, bool do_query,
                         cudaStream_t st);
 cudaError_t launch_decode(const DecodeArgs& a, int D, cudaStream_t st);
