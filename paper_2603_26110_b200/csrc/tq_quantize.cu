@@ -301,10 +301,8 @@ cudaError_t launch_quantize_pack(const QuantArgs& a, int D, tq_dtype dt, int num
   }
   // the tensor-core kernel (tq_quantize_tc.cu) is the product path; TQ_QUANTIZE_IMPL=fp32 selects the CUDA-core kernel
   // of this file (kept as a cross-check)
-  static const bool force_fp32 = [] {
-    const char* e = getenv("TQ_QUANTIZE_IMPL");
-    return e && e[0] == 'f';
-  }();
+  const char* impl = getenv("TQ_QUANTIZE_IMPL");  // read per call: a test switches it in-process
+  const bool force_fp32 = impl && impl[0] == 'f';
   if (!force_fp32) return launch_quantize_pack_tc(a, D, dt, num_sms, st);
   if (D == 64) return dt == TQ_F16 ? launch_quant_t<64, __half>(a, num_sms, st) : launch_quant_t<64, float>(a, num_sms, st);
   return dt == TQ_F16 ? launch_quant_t<128, __half>(a, num_sms, st) : launch_quant_t<128, float>(a, num_sms, st);

@@ -379,3 +379,50 @@ def test_full_size_cfg2_sampled_units(tq, oracle):
     assert np.all(np.abs(got[sample].astype(np.float64) - want) <= ulp + TL.OUT_MAX_ABS)
     # property at any size: every output is finite and |out| <= max_j |v~_j| (a convex combination)
     assert np.all(np.isfinite(got.astype(np.float64)))
+
+
+# ---------------------------------------------------------------------------------------------- cross-checks
+@pytest.mark.gpu
+@pytest.mark.parametrize("name,kw", [("cfg2_650m_batch32", dict(batch=3, n_heads=4, seq=300)),
+                                     ("cfg4_15b_heads", dict(batch=2, n_heads=3, seq=200))])
+def test_tensor_core_quantize_agrees_with_cuda_core_kernel(tq, oracle, monkeypatch, name, kw):
+    """The tcgen05 kernel (two-term fp16 split operands) and the fp32 CUDA-core kernel are two roundings of the same
+    fp64 definition: they may only differ where the oracle marks a coordinate within 1e-5 of a threshold."""
+    w = W.CONFIGS[name].scaled(**kw)
+    k, v = W.layer_activations(w, 0)
+    planes = {}
+    for impl in ("tc", "fp32"):
+        monkeypatch.setenv("TQ_QUANTIZE_IMPL", impl)
+        c = Case(tq, oracle, w)
+        tq.tq_quantize_pack(c.shape, c.params, c.cache, 0, c.dev(k), c.dev(v))
+        planes[impl] = c.gpu_export(0, w.seq)
+        can = c.oracle_quantize(0, k, v)
+    d = w.head_dim
+    for key, near in (("k_codes", can.near_k), ("v_codes", can.near_v)):
+        a = TL.unpack_codes_np(planes["tc"][key], d)
+        b = TL.unpack_codes_np(planes["fp32"][key], d)
+        assert not np.any((a != b) & (near == 0)), key
+    for key in ("k_norm", "v_norm"):
+        dd = np.abs(planes["tc"][key].view(np.uint16).astype(int) - planes["fp32"][key].view(np.uint16).astype(int))
+        assert dd.max() <= 1 and (dd > 0).mean() <= 5e-3, key
+
+
+@pytest.mark.gpu
+def test_main_only_measurement_hook_reproduces_the_call(tq, oracle):
+    """bench.py times decode_main_kernel alone through tq_profile_decode_main_only: the hooked call must produce the
+    same output as the ordinary call it follows (it re-uses that call's rotated queries)."""
+    w = W.CONFIGS["cfg2_650m_batch32"].scaled(batch=2, n_heads=3, seq=130)
+    c = Case(tq, oracle, w)
+    k, v = W.layer_activations(w, 0)
+    tq.tq_quantize_pack(c.shape, c.params, c.cache, 0, c.dev(k), c.dev(v))
+    qd = c.dev(W.queries(w, 0)[None])
+    ws = tq.Workspace(c.shape, 1)
+    full, hooked = c.torch.full_like(qd, float("nan")), c.torch.full_like(qd, float("nan"))
+    tq.tq_decode_attn(c.shape, c.params, c.cache, 0, 1, qd, full, ws)
+    tq.tq_profile_decode_main_only(True)
+    try:
+        tq.tq_decode_attn(c.shape, c.params, c.cache, 0, 1, qd, hooked, ws)
+    finally:
+        tq.tq_profile_decode_main_only(False)
+    c.torch.cuda.synchronize()
+    assert c.torch.isfinite(full).all() and c.torch.equal(full, hooked)
