@@ -9,7 +9,7 @@ decode step appends one quantised token per head (tq_append) and runs the fused 
 
 value     : cached token-heads attended per second (L*B*H*T per step / step time), inputs resident in HBM,
             the 33-layer step replayed as one CUDA graph.
-e2e       : same metric through tq_decode_step_host with pinned HOST q/k/v/out buffers (copies inside).
+e2e       : same metric through tq_decode_model_step_host with pinned HOST q/k/v/out buffers (copies inside).
 roofline  : fused decode kernel, algorithmic packed bytes (62 B per cached token-head) / its average launch
             duration measured live with CUDA events, against MEASURED_PEAKS.json hbm_gbs.
 cpu_baseline : the CPU oracle (oracle/, as it stands) timed on this box's host cores on a bounded sample.
@@ -393,15 +393,13 @@ def run_ours(args, w: W.Workload):
 
     # ---- end to end through the host-buffer call: pinned q/k/v in, out back, every layer of every step
     e2e_steps = max(3, min(args.steps, 20))
-    staging = torch.zeros(tq.tq_step_staging_bytes(shape, dt_code) + 256, dtype=torch.uint8, device=dev)
+    staging = torch.zeros(tq.tq_model_step_staging_bytes(shape, dt_code, L) + 256, dtype=torch.uint8, device=dev)
     staging = staging[(-staging.data_ptr()) % 256:]
     qh, kh, vh = qs.cpu().pin_memory(), kn.cpu().pin_memory(), vn.cpu().pin_memory()
     oh = torch.empty_like(qh).pin_memory()
 
-    def e2e_step():
-        for layer in range(L):
-            tq.tq_decode_step_host(shape, params, cache, layer, qh[layer], kh[layer], vh[layer], oh[layer], staging, ws,
-                                   max_seq, stream)
+    def e2e_step():  # one model decode step: pinned q/k/v of all L layers in, L x (append + decode), outputs back, sync
+        tq.tq_decode_model_step_host(shape, params, cache, 0, L, qh, kh, vh, oh, staging, ws, max_seq, stream)
 
     with torch.cuda.stream(stream):
         reset_len()

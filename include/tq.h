@@ -186,6 +186,16 @@ int tq_decode_step_host(const tq_shape *shape, const tq_params *dev, tq_cache *c
                         void *out_host, int32_t t_hint, void *staging, void *workspace,
                         size_t workspace_bytes, void *cuda_stream);
 
+/* One decode step of n_layers_call consecutive layers with HOST buffers (the end-to-end path bench.py times as
+ * "e2e"): q/k/v/out are HOST [n_layers_call][B][H][d]; three host-to-device copies, tq_decode_step per layer,
+ * one device-to-host copy, one stream synchronisation.  staging: DEVICE, tq_model_step_staging_bytes() bytes,
+ * 256-byte aligned.  Per-layer results are identical to tq_decode_step_host called layer by layer.             */
+size_t tq_model_step_staging_bytes(const tq_shape *shape, tq_dtype dt, int32_t n_layers_call);
+int tq_decode_model_step_host(const tq_shape *shape, const tq_params *dev, tq_cache *cache, int32_t layer_begin,
+                              int32_t n_layers_call, const void *q_host, const void *k_host, const void *v_host,
+                              tq_dtype dt, void *out_host, int32_t t_hint, void *staging, void *workspace,
+                              size_t workspace_bytes, void *cuda_stream);
+
 const char *tq_status_string(int status);
 /* Number of kernels the library launched since load (bench.py's gpu_launches).                          */
 int64_t tq_launch_count(void);

@@ -22,7 +22,7 @@ EXPORTS = [
     "tq_cache_bytes", "tq_cache_bytes_per_token_head", "tq_cache_seq_len_offset", "tq_cache_status_offset",
     "tq_decode_workspace_bytes", "tq_canonical_plane_bytes", "tq_calibrate_host", "tq_quantize_pack", "tq_append",
     "tq_decode_attn", "tq_decode_step", "tq_cache_export_canonical", "tq_cache_import_canonical", "tq_step_staging_bytes",
-    "tq_decode_step_host", "tq_status_string", "tq_launch_count", "tq_profile_decode_main_only",
+    "tq_decode_step_host", "tq_model_step_staging_bytes", "tq_decode_model_step_host", "tq_status_string", "tq_launch_count", "tq_profile_decode_main_only",
 ]
 
 
@@ -64,7 +64,7 @@ def lib():
         l = C.CDLL(LIB_PATH)
         for n in ("tq_cache_bytes", "tq_cache_bytes_per_token_head", "tq_cache_seq_len_offset",
                   "tq_cache_status_offset", "tq_decode_workspace_bytes", "tq_canonical_plane_bytes",
-                  "tq_step_staging_bytes"):
+                  "tq_step_staging_bytes", "tq_model_step_staging_bytes"):
             getattr(l, n).restype = C.c_size_t
         l.tq_status_string.restype = C.c_char_p
         l.tq_launch_count.restype = C.c_int64
@@ -282,3 +282,17 @@ def tq_decode_step_host(shape, params: Params, cache: Cache, layer: int, q_host,
                                    C.c_int32(t_hint), _ptr(staging), _ptr(workspace.data), C.c_size_t(workspace.bytes),
                                    _stream_ptr(stream))
     _check(rc, "tq_decode_step_host")
+
+
+def tq_model_step_staging_bytes(shape: TqShape, dt: int, n_layers_call: int) -> int:
+    return int(lib().tq_model_step_staging_bytes(C.byref(shape), C.c_int(dt), C.c_int32(n_layers_call)))
+
+
+def tq_decode_model_step_host(shape, params: Params, cache: Cache, layer_begin: int, n_layers_call: int, q_host, k_host,
+                              v_host, out_host, staging, workspace: Workspace, t_hint: int = 0, stream=None):
+    """Host (pinned) tensors q/k/v/out [Lc,B,H,d]: three copies in, a decode step per layer, one copy out, one sync."""
+    rc = lib().tq_decode_model_step_host(C.byref(shape), C.byref(params.c), C.byref(cache.c), C.c_int32(layer_begin),
+                                         C.c_int32(n_layers_call), _ptr(q_host), _ptr(k_host), _ptr(v_host),
+                                         C.c_int(_dtype_code(q_host)), _ptr(out_host), C.c_int32(t_hint), _ptr(staging),
+                                         _ptr(workspace.data), C.c_size_t(workspace.bytes), _stream_ptr(stream))
+    _check(rc, "tq_decode_model_step_host")

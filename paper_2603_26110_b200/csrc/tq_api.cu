@@ -306,6 +306,43 @@ int tq_decode_step_host(const tq_shape* shape, const tq_params* dev, tq_cache* c
   return TQ_OK;
 }
 
+size_t tq_model_step_staging_bytes(const tq_shape* shape, tq_dtype dt, int32_t n_layers_call) {
+  CacheGeom g;
+  if (check_shape(shape, &g) != TQ_OK || n_layers_call <= 0 || n_layers_call > g.L) return 0;
+  size_t vec = ((size_t)n_layers_call * g.B * g.H * g.D * (dt == TQ_F16 ? 2 : 4) + 255) / 256 * 256;
+  return 4 * vec;
+}
+
+int tq_decode_model_step_host(const tq_shape* shape, const tq_params* dev, tq_cache* cache, int32_t layer_begin,
+                              int32_t n_layers_call, const void* q_host, const void* k_host, const void* v_host,
+                              tq_dtype dt, void* out_host, int32_t t_hint, void* staging, void* workspace,
+                              size_t workspace_bytes, void* cuda_stream) {
+  CacheGeom g;
+  int rc = check_shape(shape, &g);
+  if (rc != TQ_OK) return rc;
+  if (!q_host || !k_host || !v_host || !out_host || !staging || ((uintptr_t)staging & 255u)) return TQ_ERR_INVALID_ARG;
+  if (dt != TQ_F16 && dt != TQ_F32) return TQ_ERR_INVALID_ARG;
+  if (layer_begin < 0 || n_layers_call <= 0 || layer_begin + n_layers_call > g.L) return TQ_ERR_INVALID_ARG;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const size_t per_layer = (size_t)g.B * g.H * g.D * (dt == TQ_F16 ? 2 : 4);
+  const size_t bytes = per_layer * n_layers_call;
+  const size_t vec = (bytes + 255) / 256 * 256;
+  unsigned char* s = (unsigned char*)staging;
+  unsigned char *dq = s, *dk = s + vec, *dv = s + 2 * vec, *dout = s + 3 * vec;
+  if (cudaMemcpyAsync(dk, k_host, bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return TQ_ERR_CUDA;
+  if (cudaMemcpyAsync(dv, v_host, bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return TQ_ERR_CUDA;
+  if (cudaMemcpyAsync(dq, q_host, bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return TQ_ERR_CUDA;
+  for (int l = 0; l < n_layers_call; ++l) {
+    const size_t off = per_layer * l;
+    if ((rc = tq_decode_step(shape, dev, cache, layer_begin + l, dq + off, dk + off, dv + off, dt, dout + off, t_hint,
+                             workspace, workspace_bytes, cuda_stream)) != TQ_OK)
+      return rc;
+  }
+  if (cudaMemcpyAsync(out_host, dout, bytes, cudaMemcpyDeviceToHost, st) != cudaSuccess) return TQ_ERR_CUDA;
+  if (cudaStreamSynchronize(st) != cudaSuccess) return TQ_ERR_CUDA;
+  return TQ_OK;
+}
+
 const char* tq_status_string(int status) {
   switch (status) {
     case TQ_OK:

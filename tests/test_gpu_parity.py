@@ -426,3 +426,37 @@ def test_main_only_measurement_hook_reproduces_the_call(tq, oracle):
         tq.tq_profile_decode_main_only(False)
     c.torch.cuda.synchronize()
     assert c.torch.isfinite(full).all() and c.torch.equal(full, hooked)
+
+
+@pytest.mark.gpu
+def test_model_step_host_equals_per_layer_host_steps(tq, oracle):
+    """tq_decode_model_step_host (all layers, one pair of copies and one sync) == tq_decode_step_host layer by layer."""
+    import torch
+
+    w = W.CONFIGS["cfg1_650m_step"].scaled(n_layers=3, batch=2, n_heads=4, seq=70)
+    outs = []
+    for mode in ("per_layer", "model"):
+        c = Case(tq, oracle, w, max_seq=w.seq + 8)
+        for layer in range(w.n_layers):
+            k, v = W.layer_activations(w, layer)
+            tq.tq_quantize_pack(c.shape, c.params, c.cache, layer, c.dev(k), c.dev(v))
+        toks = [W.step_tokens(w, layer, 0) for layer in range(w.n_layers)]
+        q = torch.from_numpy(np.stack([t[0] for t in toks])).pin_memory()
+        kn = torch.from_numpy(np.stack([t[1] for t in toks])).pin_memory()
+        vn = torch.from_numpy(np.stack([t[2] for t in toks])).pin_memory()
+        out = torch.empty_like(q).pin_memory()
+        ws = tq.Workspace(c.shape, 1)
+        dt = tq.TQ_F16 if w.dtype == "f16" else tq.TQ_F32
+        if mode == "per_layer":
+            st = torch.zeros(tq.tq_step_staging_bytes(c.shape, dt) + 256, dtype=torch.uint8, device="cuda")
+            st = st[(-st.data_ptr()) % 256:]
+            for layer in range(w.n_layers):
+                tq.tq_decode_step_host(c.shape, c.params, c.cache, layer, q[layer], kn[layer], vn[layer], out[layer], st, ws,
+                                       w.seq + 8)
+        else:
+            st = torch.zeros(tq.tq_model_step_staging_bytes(c.shape, dt, w.n_layers) + 256, dtype=torch.uint8, device="cuda")
+            st = st[(-st.data_ptr()) % 256:]
+            tq.tq_decode_model_step_host(c.shape, c.params, c.cache, 0, w.n_layers, q, kn, vn, out, st, ws, w.seq + 8)
+        assert torch.all(c.cache.seq_len == w.seq + 1)
+        outs.append(out.clone())
+    assert torch.isfinite(outs[0].float()).all() and torch.equal(outs[0], outs[1])
