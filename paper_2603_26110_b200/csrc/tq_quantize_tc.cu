@@ -529,7 +529,7 @@ cudaError_t launch_quant_tc_t(const QuantArgs& a, int num_sms, cudaStream_t st) 
   const int first_blk = a.start_pos / kBlk, last_blk = (a.start_pos + a.n_tokens - 1) / kBlk;
   const int nblk = last_blk - first_blk + 1;
   const int BH = a.cv.B * a.cv.H;
-  const long want = 6L * num_sms;  // CTAs per operand: enough to balance the SMs, few enough to amortise the matrices
+  const long want = 4L * num_sms;  // CTAs per operand: enough to balance the SMs, few enough to amortise the matrices
   int bpc = (int)(((long)nblk * BH + want - 1) / want);
   bpc = bpc < 1 ? 1 : (bpc > 16 ? 16 : bpc);
   dim3 grid((nblk + bpc - 1) / bpc, BH, 2);  // z: keys | values
