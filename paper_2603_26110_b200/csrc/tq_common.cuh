@@ -143,6 +143,13 @@ cudaError_t launch_import(const CacheGeom& g, const CacheView& cv, int layer, in
 // ---- launch bookkeeping ---------------------------------------------------------------------------------
 void count_launch(int n = 1);
 
+// Programmatic dependent launch: the streaming decode kernel is launched with programmatic stream serialization, so
+// its CTAs may be scheduled while the prep kernel in front of it is still running; it must call pdl_wait() before it
+// reads anything an earlier kernel may have written (only L2 prefetch hints and constants come before that).  The
+// prep kernel calls pdl_trigger() to let that happen.  Both are no-ops for ordinary launches.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;"); }
+
 // ---- small device helpers -------------------------------------------------------------------------------
 __device__ __forceinline__ float warp_sum(float v) {
 #pragma unroll

@@ -339,10 +339,24 @@ __global__ void __launch_bounds__(kDecodeThreads, DecodeCfg<D>::kCtasPerSm) deco
   const int e = uc / H, h = uc - e * H;  // e = (layer-in-call, batch); seq_len is contiguous over e
   const int lc = e / B, b = e - lc * B;
   const int layer = a.layer_begin + lc;
-  // ---- every global request the prologue depends on goes out first and together: the cache length, the table
-  //      inputs, then (speculatively, from the host's split plan) this warp's first tile and the L2 prefetches of
-  //      its next ones, so that the small loads never queue behind the bulk ones
   const size_t lh = (size_t)layer * H + h;
+  {  // before the PDL wait: hints only.  The cache stream of this CTA starts towards L2 while the prep kernel in front
+     // of this launch is still running (it rewrites at most one tile per unit, and L2 stays coherent); PI_V too.
+    const int per0 = a.per, t0 = sp * per0;
+    const int c1 = sp == nsplit - 1 ? a.cv.tiles_cap : min(a.cv.tiles_cap, t0 + per0);
+    const unsigned char* st0 = a.cv.tiles + (((size_t)layer * B + b) * H + h) * a.cv.stream_bytes;
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+      const int t = t0 + warp + i * NW;
+      if (t < c1 && lane == 0)
+        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(st0 + (size_t)t * Lo::kTileBytes), "r"(Lo::kTileBytes)
+                     : "memory");
+    }
+  }
+  pdl_wait();
+  // ---- every global request the prologue depends on goes out first and together: the cache length, the table
+  //      inputs, then (speculatively, from the host's split plan) this warp's first tile, so that the small loads
+  //      never queue behind the bulk ones
   int T;
   asm volatile("ld.global.b32 %0, [%1];" : "=r"(T) : "l"(a.cv.seq_len + a.layer_begin * B + e));
   TableInputs<D> tin;
@@ -360,8 +374,6 @@ __global__ void __launch_bounds__(kDecodeThreads, DecodeCfg<D>::kCtasPerSm) deco
                    : "memory");
   };
   constexpr int kPrefetchAhead = 3;  // rounds of NW tiles
-#pragma unroll
-  for (int i = 1; i < kPrefetchAhead; ++i) prefetch_tile(tile0 + warp + i * NW, cap1);
   const float* Pv = a.pi_v + lh * D * D;
 #pragma unroll
   for (int i = 0; i < D * D * 4 / 128 / kBuildThreads; ++i)
@@ -519,9 +531,19 @@ static cudaError_t launch_decode_t(const DecodeArgs& a, cudaStream_t st) {
     attr_set = true;
   }
   const int units = a.n_layers_call * a.cv.B * a.cv.H;
-  decode_main_kernel<D, T><<<units * a.nsplit, kDecodeThreads, smem, st>>>(a);
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(units * a.nsplit);
+  cfg.blockDim = dim3(kDecodeThreads);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = a.nsplit == 1 ? 1 : 0;  // measured: early scheduling helps one-CTA-per-unit launches, hurts split ones
+  e = cudaLaunchKernelEx(&cfg, decode_main_kernel<D, T>, a);
   count_launch();
-  return cudaGetLastError();
+  return e != cudaSuccess ? e : cudaGetLastError();
 }
 
 int decode_ctas_per_sm(int D) { return D == 64 ? DecodeCfg<64>::kCtasPerSm : DecodeCfg<128>::kCtasPerSm; }

@@ -93,6 +93,7 @@ __global__ void __launch_bounds__((kAppend ? 3 : 2) * PrepCfg<D>::GT) prep_kerne
   const int b0 = bgi * BG, nb = min(BG, B - b0);
   const size_t lh = (size_t)layer * H + h;
 
+  pdl_trigger();  // the streaming kernel behind this one may start its L2 prefetches
   // ---- the cache lengths first: the RoPE positions and the target tile slot hang off them
   int len_e[BG];
 #pragma unroll
