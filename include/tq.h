@@ -187,14 +187,26 @@ int tq_decode_step_host(const tq_shape *shape, const tq_params *dev, tq_cache *c
                         size_t workspace_bytes, void *cuda_stream);
 
 /* One decode step of n_layers_call consecutive layers with HOST buffers (the end-to-end path bench.py times as
- * "e2e"): q/k/v/out are HOST [n_layers_call][B][H][d]; three host-to-device copies, tq_decode_step per layer,
- * one device-to-host copy, one stream synchronisation.  staging: DEVICE, tq_model_step_staging_bytes() bytes,
+ * "e2e"): q/k/v/out are HOST [n_layers_call][B][H][d]; three host-to-device copies, tq_decode_model_step,
+ * one device-to-host copy, one stream synchronisation.  workspace: for n_layers_call layers.  staging: DEVICE, tq_model_step_staging_bytes() bytes,
  * 256-byte aligned.  Per-layer results are identical to tq_decode_step_host called layer by layer.             */
 size_t tq_model_step_staging_bytes(const tq_shape *shape, tq_dtype dt, int32_t n_layers_call);
 int tq_decode_model_step_host(const tq_shape *shape, const tq_params *dev, tq_cache *cache, int32_t layer_begin,
                               int32_t n_layers_call, const void *q_host, const void *k_host, const void *v_host,
                               tq_dtype dt, void *out_host, int32_t t_hint, void *staging, void *workspace,
                               size_t workspace_bytes, void *cuda_stream);
+
+/* ---- one decode step of a run of layers, DEVICE buffers [BASELINE.json:configs[2]; configs[1] for the shape] --------
+ * q, k, v, out: DEVICE [n_layers_call][B][H][d], dtype dt.  Result and cache state are identical to tq_decode_step
+ * called layer by layer (layers are independent: "each (layer, head)").  What differs is the launch
+ * plan: ONE kernel appends the new token and prepares the query operands of every layer, then one streaming kernel
+ * per layer cache is launched as a programmatic-dependent-launch chain in which only the first waits for the prep
+ * kernel; the others run ahead, so that the ramp and the tail of consecutive layers overlap.  The caller must have
+ * every layer's q/k/v ready before the call (a model that produces layer l+1's inputs from layer l's output uses
+ * tq_decode_step).  workspace: tq_decode_workspace_bytes(shape, n_layers_call), zero-filled once.                  */
+int tq_decode_model_step(const tq_shape *shape, const tq_params *dev, tq_cache *cache, int32_t layer_begin,
+                         int32_t n_layers_call, const void *q, const void *k, const void *v, tq_dtype dt, void *out,
+                         int32_t t_hint, void *workspace, size_t workspace_bytes, void *cuda_stream);
 
 const char *tq_status_string(int status);
 /* Number of kernels the library launched since load (bench.py's gpu_launches).                          */
@@ -204,6 +216,10 @@ int64_t tq_launch_count(void);
  * (same queries, same layers), so that a run of such calls times that kernel alone.  Process-wide state;
  * results are only meaningful directly after an ordinary call with the same arguments.                   */
 void tq_profile_decode_main_only(int on);
+/* Test / sweep knobs (process-wide, not part of the product path; both default to 0 = the library's own choice):
+ * CTAs per unit of the streaming decode kernel; 1 = route tq_quantize_pack to the fp32 CUDA-core cross-check kernel. */
+void tq_debug_set_decode_nsplit(int nsplit);
+void tq_debug_set_quantize_impl(int fp32_cuda_cores);
 
 #ifdef __cplusplus
 }

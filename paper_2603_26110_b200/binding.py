@@ -22,7 +22,8 @@ EXPORTS = [
     "tq_cache_bytes", "tq_cache_bytes_per_token_head", "tq_cache_seq_len_offset", "tq_cache_status_offset",
     "tq_decode_workspace_bytes", "tq_canonical_plane_bytes", "tq_calibrate_host", "tq_quantize_pack", "tq_append",
     "tq_decode_attn", "tq_decode_step", "tq_cache_export_canonical", "tq_cache_import_canonical", "tq_step_staging_bytes",
-    "tq_decode_step_host", "tq_model_step_staging_bytes", "tq_decode_model_step_host", "tq_status_string", "tq_launch_count", "tq_profile_decode_main_only",
+    "tq_decode_step_host", "tq_model_step_staging_bytes", "tq_decode_model_step_host", "tq_decode_model_step", "tq_status_string", "tq_launch_count", "tq_profile_decode_main_only",
+    "tq_debug_set_decode_nsplit", "tq_debug_set_quantize_impl",
 ]
 
 
@@ -240,6 +241,25 @@ def tq_decode_step(shape, params: Params, cache: Cache, layer: int, q, k, v, out
                               _ptr(v), C.c_int(_dtype_code(q)), _ptr(out), C.c_int32(t_hint), _ptr(workspace.data),
                               C.c_size_t(workspace.bytes), _stream_ptr(stream))
     _check(rc, "tq_decode_step")
+
+
+def tq_decode_model_step(shape, params: Params, cache: Cache, layer_begin: int, n_layers_call: int, q, k, v, out,
+                         workspace: Workspace, t_hint: int = 0, stream=None):
+    """q, k, v, out: device tensors [Lc,B,H,d]: one decode step of Lc consecutive layers (workspace for Lc layers)."""
+    rc = lib().tq_decode_model_step(C.byref(shape), C.byref(params.c), C.byref(cache.c), C.c_int32(layer_begin),
+                                    C.c_int32(n_layers_call), _ptr(q), _ptr(k), _ptr(v), C.c_int(_dtype_code(q)), _ptr(out),
+                                    C.c_int32(t_hint), _ptr(workspace.data), C.c_size_t(workspace.bytes), _stream_ptr(stream))
+    _check(rc, "tq_decode_model_step")
+
+
+def tq_debug_set_decode_nsplit(nsplit: int):
+    """Test / sweep knob: CTAs per unit of the streaming decode kernel (0 = the library's own plan)."""
+    lib().tq_debug_set_decode_nsplit(C.c_int(nsplit))
+
+
+def tq_debug_set_quantize_impl(fp32_cuda_cores: bool):
+    """Test knob: route tq_quantize_pack to the fp32 CUDA-core kernel (cross-check of the tensor-core kernel)."""
+    lib().tq_debug_set_quantize_impl(C.c_int(1 if fp32_cuda_cores else 0))
 
 
 def _canon_struct(planes: dict) -> TqCanonical:

@@ -2,7 +2,6 @@
 // launch configuration.  No torch types, no allocation, no hidden synchronisation (except the explicit
 // host-buffer convenience call tq_decode_step_host, which must synchronise to hand back host data).
 #include <atomic>
-#include <cstdlib>
 #include <cstring>
 
 #include "tq_common.cuh"
@@ -36,15 +35,23 @@ static int choose_nsplit(int units, int ntiles, int sms) {
   return best;
 }
 
+// split factor of a launch: the plan above, or the value set with tq_debug_set_decode_nsplit (tests, sweeps)
+static std::atomic<int> g_debug_nsplit{0};
+static int pick_nsplit(int units, int ntiles, int sms) {
+  const int forced = g_debug_nsplit.load(std::memory_order_relaxed);
+  return forced >= 1 && forced <= kMaxSplits ? forced : choose_nsplit(units, ntiles, sms);
+}
+
+// SM count of the CURRENT device (a process may drive several): cached per device ordinal
 static int num_sms() {
-  static int cached = -1;
-  if (cached < 0) {
-    int dev = 0, n = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess) return -1;
-    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return -1;
-    cached = n;
-  }
-  return cached;
+  constexpr int kMaxDev = 64;
+  static std::atomic<int> cached[kMaxDev];  // zero-initialised: 0 = not queried yet
+  int dev = 0, n = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return -1;
+  if (dev >= 0 && dev < kMaxDev && (n = cached[dev].load(std::memory_order_relaxed)) > 0) return n;
+  if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) return -1;
+  if (dev >= 0 && dev < kMaxDev) cached[dev].store(n, std::memory_order_relaxed);
+  return n;
 }
 
 static int check_shape(const tq_shape* s, CacheGeom* g) {
@@ -68,14 +75,17 @@ static int check_params(const tq_params* p) {
 }
 
 struct WorkspaceGeom {
-  size_t off_counters, off_qrot, off_partials, total;
+  size_t off_counters, off_frags, off_tabs, off_partials, total;
+  size_t frag_words;
 };
 static WorkspaceGeom workspace_geom(const CacheGeom& g, int n_layers_call) {
   WorkspaceGeom w;
   size_t units = (size_t)n_layers_call * g.B * g.H;
   w.off_counters = 0;
-  w.off_qrot = (units * 4 + 255) / 256 * 256;
-  w.off_partials = w.off_qrot + (units * 2 * g.D * 4 + 255) / 256 * 256;
+  w.frag_words = g.D == 64 ? FragLayout<64>::kWords : FragLayout<128>::kWords;
+  w.off_frags = (units * 4 + 255) / 256 * 256;
+  w.off_tabs = w.off_frags + (units * w.frag_words * 4 + 255) / 256 * 256;
+  w.off_partials = w.off_tabs + ((size_t)n_layers_call * g.H * kTabWords * 4 + 255) / 256 * 256;
   w.total = w.off_partials + units * kMaxSplits * (size_t)(g.D + 2) * 4;
   return w;
 }
@@ -181,11 +191,7 @@ static int run_decode(const tq_shape* shape, const tq_params* dev, const tq_cach
   if (sms <= 0) return TQ_ERR_CUDA;
   const int th = (t_hint == 0 || t_hint > g.max_seq) ? g.max_seq : t_hint;
   const int ntiles = (th + kTile - 1) / kTile;
-  int nsplit = choose_nsplit(n_layers_call * g.B * g.H, ntiles, sms);
-  if (const char* e = getenv("TQ_DECODE_NSPLIT")) {  // profiling / test knob: CTAs per unit of the streaming kernel
-    long vv = atol(e);
-    if (vv >= 1 && vv <= kMaxSplits) nsplit = (int)vv;
-  }
+  const int nsplit = pick_nsplit(n_layers_call * g.B * g.H, ntiles, sms);
   const size_t esz = dt == TQ_F16 ? 2 : 4;
   unsigned char* ws = (unsigned char*)workspace;
   const int layers_per_launch = n_layers_call;
@@ -204,13 +210,14 @@ static int run_decode(const tq_shape* shape, const tq_params* dev, const tq_cach
     a.out = out ? (unsigned char*)out + u0 * g.D * esz : nullptr;
     a.q_pos = q_pos ? q_pos + (size_t)l0 * g.B : nullptr;
     a.counters = ws ? (int*)(ws + w.off_counters) + u0 : nullptr;
-    a.qrot = ws ? (float*)(ws + w.off_qrot) + u0 * 2 * g.D : nullptr;
+    a.frags = ws ? (unsigned*)(ws + w.off_frags) + u0 * w.frag_words : nullptr;
+    a.tabs = ws ? (unsigned*)(ws + w.off_tabs) + (size_t)l0 * g.H * kTabWords : nullptr;
     a.partials = ws ? (float*)(ws + w.off_partials) + u0 * kMaxSplits * (g.D + 2) : nullptr;
     a.layer_begin = layer_begin + l0;
     a.n_layers_call = nl;
     a.nsplit = nsplit;
     a.per = (ntiles + nsplit - 1) / nsplit;
-    a.zero = 0;
+    a.chain_mode = 0;
     a.rope_layout = shape->rope_layout;
     a.dt = (int)dt;
     const void* kc = k ? (const unsigned char*)k + u0 * g.D * esz : nullptr;
@@ -275,6 +282,60 @@ int tq_cache_import_canonical(const tq_shape* shape, tq_cache* cache, int32_t la
              : TQ_ERR_CUDA;
 }
 
+int tq_decode_model_step(const tq_shape* shape, const tq_params* dev, tq_cache* cache, int32_t layer_begin,
+                         int32_t n_layers_call, const void* q, const void* k, const void* v, tq_dtype dt, void* out,
+                         int32_t t_hint, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  CacheGeom g;
+  int rc = check_shape(shape, &g);
+  if (rc != TQ_OK) return rc;
+  if ((rc = check_params(dev)) != TQ_OK) return rc;
+  if (!cache || !cache->data || ((uintptr_t)cache->data & 255u)) return TQ_ERR_INVALID_ARG;
+  if (layer_begin < 0 || n_layers_call <= 0 || layer_begin + n_layers_call > g.L) return TQ_ERR_INVALID_ARG;
+  if (dt != TQ_F16 && dt != TQ_F32) return TQ_ERR_INVALID_ARG;
+  if (!aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(out) || !workspace || ((uintptr_t)workspace & 255u))
+    return TQ_ERR_INVALID_ARG;
+  if (t_hint < 0) return TQ_ERR_INVALID_ARG;
+  WorkspaceGeom w = workspace_geom(g, n_layers_call);
+  if (workspace_bytes < w.total) return TQ_ERR_CAPACITY;
+  const int sms = num_sms();
+  if (sms <= 0) return TQ_ERR_CUDA;
+  const int th = (t_hint == 0 || t_hint > g.max_seq) ? g.max_seq : t_hint;
+  const int ntiles = (th + kTile - 1) / kTile;
+  const int nsplit = pick_nsplit(g.B * g.H, ntiles, sms);
+  const size_t esz = dt == TQ_F16 ? 2 : 4;
+  unsigned char* ws = (unsigned char*)workspace;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  DecodeArgs a;
+  a.cv = make_view(g, cache->data);
+  a.pi_k = dev->pi_k, a.pi_v = dev->pi_v, a.lut_k = dev->lut_k, a.lut_v = dev->lut_v, a.S = dev->S, a.rope_cs = dev->rope_cs;
+  a.q = q, a.out = out, a.q_pos = nullptr;
+  a.counters = (int*)(ws + w.off_counters);
+  a.frags = (unsigned*)(ws + w.off_frags);
+  a.tabs = (unsigned*)(ws + w.off_tabs);
+  a.partials = (float*)(ws + w.off_partials);
+  a.layer_begin = layer_begin, a.n_layers_call = n_layers_call;
+  a.nsplit = nsplit, a.per = (ntiles + nsplit - 1) / nsplit;
+  a.chain_mode = 0, a.rope_layout = shape->rope_layout, a.dt = (int)dt;
+  // one prep launch for every layer of the step (append + query operands), then one streaming launch per layer cache:
+  // the first waits for the prep kernel, the others run ahead of one another (DecodeArgs::chain_mode)
+  if (!g_profile_skip_prep && launch_prep(a, k, v, g.D, true, true, st) != cudaSuccess) return TQ_ERR_CUDA;
+  const size_t units = (size_t)g.B * g.H;
+  for (int l = 0; l < n_layers_call; ++l) {
+    DecodeArgs b = a;
+    const size_t u0 = (size_t)l * units;
+    b.q = (const unsigned char*)q + u0 * g.D * esz;
+    b.out = (unsigned char*)out + u0 * g.D * esz;
+    b.counters = a.counters + u0;
+    b.frags = a.frags + u0 * w.frag_words;
+    b.tabs = a.tabs + (size_t)l * g.H * kTabWords;
+    b.partials = a.partials + u0 * kMaxSplits * (g.D + 2);
+    b.layer_begin = layer_begin + l, b.n_layers_call = 1;
+    b.chain_mode = l == 0 ? 0 : 1;
+    if (launch_decode(b, g.D, st) != cudaSuccess) return TQ_ERR_CUDA;
+  }
+  return TQ_OK;
+}
+
 size_t tq_step_staging_bytes(const tq_shape* shape, tq_dtype dt) {
   CacheGeom g;
   if (check_shape(shape, &g) != TQ_OK) return 0;
@@ -332,12 +393,9 @@ int tq_decode_model_step_host(const tq_shape* shape, const tq_params* dev, tq_ca
   if (cudaMemcpyAsync(dk, k_host, bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return TQ_ERR_CUDA;
   if (cudaMemcpyAsync(dv, v_host, bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return TQ_ERR_CUDA;
   if (cudaMemcpyAsync(dq, q_host, bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return TQ_ERR_CUDA;
-  for (int l = 0; l < n_layers_call; ++l) {
-    const size_t off = per_layer * l;
-    if ((rc = tq_decode_step(shape, dev, cache, layer_begin + l, dq + off, dk + off, dv + off, dt, dout + off, t_hint,
-                             workspace, workspace_bytes, cuda_stream)) != TQ_OK)
-      return rc;
-  }
+  if ((rc = tq_decode_model_step(shape, dev, cache, layer_begin, n_layers_call, dq, dk, dv, dt, dout, t_hint, workspace,
+                                 workspace_bytes, cuda_stream)) != TQ_OK)
+    return rc;
   if (cudaMemcpyAsync(out_host, dout, bytes, cudaMemcpyDeviceToHost, st) != cudaSuccess) return TQ_ERR_CUDA;
   if (cudaStreamSynchronize(st) != cudaSuccess) return TQ_ERR_CUDA;
   return TQ_OK;
@@ -363,5 +421,9 @@ const char* tq_status_string(int status) {
 int64_t tq_launch_count(void) { return (int64_t)tq::g_launches.load(); }
 
 void tq_profile_decode_main_only(int on) { tq::g_profile_skip_prep = on != 0; }
+
+void tq_debug_set_quantize_impl(int fp32_cuda_cores) { tq::debug_set_quantize_fp32(fp32_cuda_cores); }
+
+void tq_debug_set_decode_nsplit(int nsplit) { tq::g_debug_nsplit.store(nsplit, std::memory_order_relaxed); }
 
 }  // extern "C"

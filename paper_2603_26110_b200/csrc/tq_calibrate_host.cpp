@@ -138,6 +138,21 @@ double phi(double x) { return std::exp(-0.5 * x * x) * 0.3989422804014326779; }
 double Phi(double x) { return 0.5 * std::erfc(-x * 0.7071067811865475244); }
 
 // Lloyd-Max fixed point for N(0, sigma^2), 8 levels (Eq. 5): alternate midpoints / conditional means.
+// Centroids are rounded to the nearest binary16-representable value (reading D15): the
+// fused decode kernel then dequantises with exact fp16 tables (one 32-bit shared-memory read per code pair).  The
+// change is 2^-12 relative, far below the quantiser's own error; every kernel also accepts LUTs that are not
+// representable (two-term tables), so this is a calibration choice, not a format restriction.
+float round_to_binary16(double x) {
+  if (x == 0.0 || !std::isfinite(x)) return (float)x;
+  int e;
+  const double m = std::frexp(std::fabs(x), &e);  // |x| = m 2^e, m in [0.5, 1)
+  if (e > 16) return (float)(x < 0 ? -65504.0 : 65504.0);
+  const int qe = (e < -13 ? -24 : e - 11);        // spacing 2^qe: 11 significant bits, subnormals below 2^-14
+  const double q = std::ldexp(std::nearbyint(std::ldexp(std::fabs(x), -qe)), qe);
+  (void)m;
+  return (float)(x < 0 ? -q : q);
+}
+
 void lloyd_max_gauss8(double sigma, float* lut8) {
   double c[8], t[9];
   for (int k = 0; k < 8; ++k) c[k] = -2.1 + 0.6 * k;
@@ -153,7 +168,7 @@ void lloyd_max_gauss8(double sigma, float* lut8) {
     }
     if (delta < 1e-15) break;
   }
-  for (int k = 0; k < 8; ++k) lut8[k] = (float)(sigma * c[k]);
+  for (int k = 0; k < 8; ++k) lut8[k] = round_to_binary16(sigma * c[k]);
 }
 
 // Lloyd-Max on samples (1-D k-means), samples sorted ascending.
@@ -179,7 +194,7 @@ void lloyd_max_samples8(std::vector<double>& s, float* lut8) {
       }
     if (delta < 1e-12) break;
   }
-  for (int k = 0; k < 8; ++k) lut8[k] = (float)c[k];
+  for (int k = 0; k < 8; ++k) lut8[k] = round_to_binary16(c[k]);
 }
 
 void pooled_unit_coords(const float* X, int64_t n, int d, const float* pi, std::vector<double>& pool) {

@@ -13,32 +13,91 @@ namespace tq {
 constexpr int kTile = TQ_TILE_TOKENS;  // tokens per tile == lanes per warp
 
 // ---- per-head-dim tile layout ------------------------------------------------------------------------
-// A "section" is a per-token string of W 32-bit words stored chunk-major: 16-byte chunks [c][token], then
-// (if W % 4 == 2) one 8-byte chunk [token].
+// The fused decode kernel runs its three contractions (<q'', lut_K[codes]>, <z, sigma>, sum_j w_j lut_V[codes_j]) as
+// warp-level mma.sync.m16n8k16 with fp16 operands built in registers, so a tile of 32 tokens is stored in exactly the
+// order of the m16n8k16 A-fragment: lane = 4 g + t (g = lane / 4 = fragment row, t = lane % 4 = fragment column group).
+//   K codes : lane (g, t) owns, for the four token slots s = g + 8 r (r = 0..3), the six-bit pair fields
+//             (code_{2p} | code_{2p+1} << 3) of the pairs p = t + 4 j (j < J = d/8); field (r, j) sits at bit
+//             6 (J r + j) of the lane's string of KCW = 3d/32 words;
+//   K signs : lane (g, t) owns sketch rows [t d/4, (t+1) d/4) of the same four slots, as 16-bit pieces u < d/64;
+//             the pieces of slots g + 16 mt ("A") and g + 8 + 16 mt ("B") are byte-interleaved in word (mt, u):
+//             bytes [A bits 0..7 | B bits 0..7 | A bits 8..15 | B bits 8..15], so that (word >> 8 ab) & (0x00010001 << p)
+//             is an fp16x2 register holding two sign bits as the (subnormal) values 2^(p-24);
+//   V codes : lane (g, t) owns coordinates i = g + 8 c (c < C = d/8) of the token pairs pp = t + 4 j (j < 4); field
+//             (j, c) = code_i(token 2pp) | code_i(token 2pp+1) << 3 sits at bit 6 (C j + c);
+//   norms   : lane (g, t) owns token slot g + 8 t: one u32 (|k| | |r_k| << 16, binary16 bits) and one u16 (|v|).
+// A "section" is a per-lane string of W 32-bit words stored chunk-major: 16-byte chunks [c][lane], then (if
+// W % 4 == 2) one 8-byte chunk [lane].  62 (d = 64) / 118 (d = 128) bytes per token, as the canonical format.
 template <int D>
 struct Layout {
   static_assert(D == 64 || D == 128, "head_dim must be 64 or 128");
-  static constexpr int P = D / 2;            // six-bit pair fields per code string
-  static constexpr int NG = D / 4;           // sign nibble groups
-  static constexpr int KCW = 3 * D / 32;     // words per K (or V) code string: 6 | 12
-  static constexpr int KSW = D / 32;         // words per sign string: 2 | 4
+  static constexpr int P = D / 2;            // coordinate pairs per vector
+  static constexpr int J = D / 8;            // K pair fields per (lane, token slot)
+  static constexpr int C = D / 8;            // V coordinates per lane
+  static constexpr int U = D / 64;           // 16-bit sign pieces per (lane, token slot)
+  static constexpr int KCW = 3 * D / 32;     // words per lane of the K (or V) code section: 6 | 12
+  static constexpr int KSW = D / 32;         // words per lane of the sign section: 2 | 4
   static constexpr int kCodeBytes = KCW * 4 * kTile;
   static constexpr int kSignBytes = KSW * 4 * kTile;
   static constexpr int kOffKC = 0;
   static constexpr int kOffKS = kOffKC + kCodeBytes;
   static constexpr int kOffVC = kOffKS + kSignBytes;
-  static constexpr int kOffKN = kOffVC + kCodeBytes;  // binary16 |k|   [32]
-  static constexpr int kOffKR = kOffKN + 2 * kTile;   // binary16 |r_k| [32]
-  static constexpr int kOffVN = kOffKR + 2 * kTile;   // binary16 |v|   [32]
+  static constexpr int kOffNK = kOffVC + kCodeBytes;  // u32 per lane: binary16 |k| | binary16 |r_k| << 16
+  static constexpr int kOffVN = kOffNK + 4 * kTile;   // u16 per lane: binary16 |v|
   static constexpr int kTileBytes = kOffVN + 2 * kTile;  // 1984 | 3776
   static constexpr int kBytesPerToken = kTileBytes / kTile;
 };
 
-// byte offset (inside its section) of word w of the token in slot t, section of W words per token
-__host__ __device__ constexpr int word_offset(int W, int w, int t) {
-  return (w < (W / 4) * 4) ? ((w / 4) * 16 * kTile + t * 16 + (w % 4) * 4)
-                           : ((W / 4) * 16 * kTile + t * 8 + (w - (W / 4) * 4) * 4);
+// byte offset (inside its section) of word w of lane l, section of W words per lane
+__host__ __device__ constexpr int word_offset(int W, int w, int l) {
+  return (w < (W / 4) * 4) ? ((w / 4) * 16 * kTile + l * 16 + (w % 4) * 4)
+                           : ((W / 4) * 16 * kTile + l * 8 + (w - (W / 4) * 4) * 4);
 }
+
+// lane that owns token slot s for the norms and the softmax, and its inverse
+__host__ __device__ constexpr int slot_lane(int s) { return 4 * (s & 7) + (s >> 3); }
+__host__ __device__ constexpr int lane_slot(int l) { return (l >> 2) + 8 * (l & 3); }
+
+struct BitPos {
+  int lane, bit;  // bit offset inside the lane's word string of that section
+};
+// six-bit K pair field of (slot s, pair p)
+template <int D>
+__host__ __device__ constexpr BitPos k_field_pos(int s, int p) {
+  return BitPos{4 * (s & 7) + (p & 3), 6 * (Layout<D>::J * (s >> 3) + (p >> 2))};
+}
+// sign bit of (slot s, sketch row rho)
+template <int D>
+__host__ __device__ constexpr BitPos sign_bit_pos(int s, int rho) {
+  const int t = rho / (D / 4), i = rho % (D / 4), u = i >> 4, ib = i & 15;
+  const int word = (s >> 4) * Layout<D>::U + u, byte = (ib >> 3) * 2 + ((s >> 3) & 1);
+  return BitPos{4 * (s & 7) + t, 32 * word + 8 * byte + (ib & 7)};
+}
+// three-bit V code of (slot s, coordinate i)
+template <int D>
+__host__ __device__ constexpr BitPos v_code_pos(int s, int i) {
+  const int pp = s >> 1;
+  return BitPos{4 * (i & 7) + (pp & 3), 6 * (Layout<D>::C * (pp >> 2) + (i >> 3)) + 3 * (s & 1)};
+}
+
+// ---- per-unit operands of the fused decode kernel (written by the prep kernel into the workspace) -------------------
+// The decode kernel feeds q'' and z to mma.sync.m16n8k16 as B fragments in fp16, split hi + lo (column n of B holds
+// the hi part for even n and the lo part for odd n).  A lane (g, t) needs the pattern x = g & 1, t:
+//   words [0, 2 KS)    bq[ks][reg] : q''_s (16 ks + 2 t + 8 reg), (.. + 1)           q''_s = q'' log2(e)/sqrt(d) 2^eq
+//   words [2 KS, 4 KS) bz[ks][reg] : z_s (rho), z_s (rho + 8), rho = t d/4 + 16 (ks / 4) + 2 (ks % 4) + reg,
+//                                    scaled by 2^(ez - 2 (ks % 4) - reg)             z_s = z log2(e)/sqrt(d) sqrt(pi/2)/m
+// followed by four floats: kscale = 2^-eq, sscale = 2^(25 - ez), zsum = sum_rho z_s(rho), 0.
+template <int D>
+struct FragLayout {
+  static constexpr int KS = D / 16;
+  static constexpr int kWordsPerPat = 4 * KS;               // 16 | 32
+  static constexpr int kScalOff = 8 * kWordsPerPat;         // in words
+  static constexpr int kWords = kScalOff + 4;
+  static constexpr int kBytes = kWords * 4;                 // 528 | 1040
+};
+// Dequantisation tables of one (layer, head), also written by the prep kernel: [K hi | K lo | V hi | V lo][64] fp16
+// pairs (entry c0 | c1 << 3 -> (lut[c0], lut[c1]), lo = lut - hi), then one word: 1 if every lo is zero.
+constexpr int kTabWords = 4 * 64 + 4;
 
 // ---- cache header -------------------------------------------------------------------------------------
 struct CacheGeom {
@@ -122,11 +181,16 @@ struct DecodeArgs {
   const void* q;         // [Lc][B][H][D]
   void* out;             // [Lc][B][H][D]
   const int32_t* q_pos;  // [Lc][B] or nullptr
-  float* qrot;           // workspace [units_call][2 D]: q'' then z, pre-scaled (tq_prep.cu)
+  unsigned* frags;       // workspace [units_call][FragLayout<D>::kWords] (tq_prep.cu)
+  unsigned* tabs;        // workspace [layers_call * H][kTabWords]
   float* partials;       // workspace [units_call][64][D + 2]
   int* counters;         // workspace [units_call]
   int layer_begin, n_layers_call, nsplit /* CTAs per unit, >= 1 */, per /* tiles per split planned from t_hint */, rope_layout, dt;
-  int zero;  // always 0 (see tq_decode.cu: keeps table base registers opaque to ptxas)
+  // 0: wait for the kernel in front of this launch before touching memory (any stream order is safe);
+  // 1: run ahead — this launch is one of a chain of streaming kernels over DIFFERENT layers whose common producer (the
+  //    multi-layer prep kernel) was already awaited by the first of the chain: nothing is awaited at the start, and the
+  //    CTAs wait for the kernel in front only before they exit, so that the chain still completes in order.
+  int chain_mode;
 };
 
 cudaError_t launch_quantize_pack(const QuantArgs& a, int D, tq_dtype dt, int num_sms, cudaStream_t st);
@@ -139,6 +203,8 @@ cudaError_t launch_export(const CacheGeom& g, const CacheView& cv, int layer, in
                           cudaStream_t st);
 cudaError_t launch_import(const CacheGeom& g, const CacheView& cv, int layer, int n_tokens, const tq_canonical& in,
                           cudaStream_t st);
+
+void debug_set_quantize_fp32(int on);
 
 // ---- launch bookkeeping ---------------------------------------------------------------------------------
 void count_launch(int n = 1);

@@ -1,6 +1,4 @@
-// tq_decode.cu — fused decode attention over the packed 3-bit cache (sm_100a, CUDA cores by design:
-// a one-query GEMV over a packed stream is bound by HBM bandwidth and by instruction issue, not by
-// tensor throughput — DESIGN.md "Decode kernel").
+// tq_decode.cu — fused decode attention over the packed 3-bit cache (sm_100a).
 //
 // Algorithm 1 of the paper re-associated as BASELINE.json:north_star asks: the query is
 // rotated once (q'' = PI_K RoPE(q), z = S q''; Eq. 4 moves PI from every key to the query), then the cache
@@ -8,36 +6,115 @@
 //   logit_j = n_j ( <q'', lut_K[codes_j]> + sqrt(pi/2)/m * g_j * <z, sigma_j> ) / sqrt(d)
 //   online softmax (running max m, sum l), o' += p_j * nv_j * lut_V[codesV_j];   out = PI_V^T (o' / l).
 //
-// Mapping: lane = token.  Each lane owns one token of a 32-token tile and walks its 6-bit code-pair fields.
-//   * <q'', lut_K[.]> becomes P = d/2 table reads: Ktab[field][col] = q''_{2g} lut[c0] + q''_{2g+1} lut[c1],
-//     col = (lane + k) so that the 32 lanes always hit 32 different banks (the cache stores field g at
-//     position (g - lane) mod P for exactly this reason);
-//   * <z, sigma> becomes d/4 reads of a 16-entry nibble table with the same rotation;
-//   * V is dequantised two coordinates per 64-bit table read ([field][lane] float2, conflict free) and
-//     accumulated into d fp32 registers per lane; lanes are summed once per warp at the end.
-// Split-K over the sequence: grid = units x nsplit CTAs (nsplit chosen on the host from t_hint so that the SMs
-// carry equal work); a unit covered by one CTA is finished in place, otherwise the last CTA to arrive merges
-// the partial (m, l, o') triples.  Either way the finishing CTA applies PI_V^T.
-// Tokens whose softmax weight underflows to exactly 0 in fp32 add nothing to o': their V lookups are skipped
-// (a warp-uniform test on a ballot of the weights), which changes no bit of the result.
+// Why warp-level tensor-core MMAs (DESIGN.md §5.1 has the counters): the round-1 kernel did these three
+// contractions with per-unit shared-memory tables of partial dot products and CUDA-core adds; ncu showed it bound by
+// the shared-memory pipe (LSU 49 %) and the integer ALU (46 %) at 36 % of the HBM roofline — 70 % of the roofline
+// would have needed more than 95 % of both.  Here a lookup only DEQUANTISES (a 64-entry table of fp16 pairs
+// (lut[c0], lut[c1]) that does not depend on the query), and the multiply-accumulate runs on mma.sync.m16n8k16
+// (fp16 x fp16 -> fp32), which is otherwise idle:
+//   * K scores : A = dequantised key codes (16 tokens x 16 coordinates per MMA), B = q'' split hi + lo in fp16 in
+//                the columns of B (both products exact in the fp32 accumulator);
+//   * sign term: A = the stored sign bits themselves: (word & (0x00010001 << p)) is an fp16x2 register whose halves
+//                are 0 or the subnormal 2^(p-24) (mma.sync multiplies fp16 subnormals exactly); B = z scaled by
+//                2^(E-p), so the accumulator holds 2^(E-24) sum_j bit_j z_j and <z, sigma> = 2 sum - sum(z);
+//   * V        : A = dequantised value codes (16 coordinates x 16 tokens), B = the softmax weights split hi + lo.
+// The tile layout (tq_common.cuh) stores every word in A-fragment order, so a lookup is SHF + LOP3 + LDS and needs no
+// cross-lane traffic; the table column is the lane, so no lookup ever has a bank conflict.
+// The fp16 tables are exact when the LUT entries are binary16-representable (tq_calibrate_host emits such LUTs:
+// DESIGN.md reading D15); any other fp32 LUT takes the two-term path (hi + lo tables, twice the MMAs).
+//
+// Staging: every warp owns a ring of kStages tile slots in shared memory filled by cp.async.bulk (1-D TMA copy,
+// mbarrier complete_tx); lane 0 re-arms a slot as soon as the warp has consumed it.
+// Split-K over the sequence: grid = units x nsplit CTAs; a unit covered by one CTA is finished in place, otherwise the
+// last CTA to arrive merges the partial (m, l, o') triples.  Either way the finishing CTA applies PI_V^T.
 #include <utility>
 
 #include "tq_common.cuh"
 
 namespace tq {
 
+constexpr int kMaxSegments = 64;      // split-K partial slots per unit (tq_api.cu sizes the workspace)
+#ifndef TQ_DECODE_CTAS64
+#define TQ_DECODE_CTAS64 5
+#endif
+#ifndef TQ_DECODE_STAGES
+#define TQ_DECODE_STAGES 3
+#endif
+constexpr int kDecodeThreads = 128;   // warps of one CTA share the dequantisation tables of one head
+constexpr int kDecodeWarps = kDecodeThreads / 32;
+constexpr int kStages = TQ_DECODE_STAGES;  // tile slots per warp
 
-// ------------------------------------------------------------------------------------------ smem helpers
-template <int IMM>
-__device__ __forceinline__ float lds_f32(unsigned addr) {
-  float v;
-  asm("ld.shared.f32 %0, [%1+%2];" : "=f"(v) : "r"(addr), "n"(IMM));
+// Shared-memory map in ABSOLUTE shared-window addresses: the table and ring bases are immediates of the ld.shared
+// instructions, so a lookup address is one LOP3 ((field & mask) | lane * 4).  Dynamic shared memory starts right after
+// the 1 KB the driver reserves; the kernel traps if the window starts later than kAbsMisc.
+template <int D>
+struct DecodeCfg {
+  using Lo = Layout<D>;
+  static constexpr unsigned kAbsMisc = 1024;   // mbarriers [warps][kStages], weights [warps][2][32] halves, flag
+  static constexpr unsigned kAbsBar = kAbsMisc;
+  static constexpr unsigned kAbsWbuf = kAbsMisc + 128;
+  static constexpr unsigned kAbsFlag = kAbsWbuf + kDecodeWarps * 128;
+  static constexpr unsigned kAbsRed = 2048;    // per-warp (m, l, o'[D]) then the merged o [2 D]
+  static constexpr int kRedBytes = kDecodeWarps * (D + 2) * 4 + 2 * D * 4;
+  static constexpr unsigned kAbsRing = (kAbsRed + kRedBytes + 127) / 128 * 128;
+  static constexpr int kRingBytes = kDecodeWarps * kStages * Lo::kTileBytes;
+  static constexpr unsigned kAbsTab = (kAbsRing + kRingBytes + 255) / 256 * 256;  // K table then V table
+  // bytes per table: [64 entries][32 lanes] fp16 pairs, or [64][16] (hi pair, lo pair) for LUTs that are not
+  // binary16-representable (64-bit reads are served one half-warp at a time, so 16 columns are conflict free)
+  static constexpr int kTabBytes = 64 * 32 * 4;
+  static constexpr int kSmemBytes = kAbsTab + 2 * kTabBytes;  // requested dynamic bytes (window start <= 1 KB)
+  static constexpr int kCtasPerSm = D == 64 ? TQ_DECODE_CTAS64 : 2;
+};
+
+// ---- small PTX helpers --------------------------------------------------------------------------------------------
+template <unsigned BASE>
+__device__ __forceinline__ unsigned lds_u32(unsigned addr) {
+  unsigned v;  // not volatile: the tables are constant once built, the scheduler may hoist and interleave lookups
+  asm("ld.shared.u32 %0, [%1+%2];" : "=r"(v) : "r"(addr), "n"(BASE));
   return v;
 }
-__device__ __forceinline__ float2 lds_f32x2(unsigned addr) {
-  float2 v;
-  asm("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(addr));
+template <unsigned BASE>
+__device__ __forceinline__ uint2 lds_u32x2(unsigned addr) {
+  uint2 v;
+  asm("ld.shared.v2.u32 {%0, %1}, [%2+%3];" : "=r"(v.x), "=r"(v.y) : "r"(addr), "n"(BASE));
   return v;
+}
+__device__ __forceinline__ uint4 lds_u32x4(unsigned addr) {
+  uint4 v;
+  asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr) : "memory");
+  return v;
+}
+__device__ __forceinline__ uint2 lds_u32x2_dyn(unsigned addr) {
+  uint2 v;
+  asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(addr) : "memory");
+  return v;
+}
+__device__ __forceinline__ void mma16816(float (&d)[4], unsigned a0, unsigned a1, unsigned a2, unsigned a3, unsigned b0,
+                                         unsigned b1) {
+  asm("mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+      : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
+      : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
+}
+__device__ __forceinline__ void mbar_init(unsigned bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
+  asm volatile(
+      "{\n\t.reg .pred P1;\n\t"
+      "WAIT_%=:\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n\t"
+      "@P1 bra DONE_%=;\n\t"
+      "bra WAIT_%=;\n\t"
+      "DONE_%=:\n\t}" ::"r"(bar),
+      "r"(parity)
+      : "memory");
+}
+// one 1-D TMA copy of `bytes` (multiple of 16) global -> shared, completion counted on the mbarrier
+__device__ __forceinline__ void tma_load_tile(unsigned dst, const void* src, unsigned bytes, unsigned bar) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+               "l"(src), "r"(bytes), "r"(bar)
+               : "memory");
 }
 
 // bits [BIT, BIT+NB) of the little-endian word string w, moved to bit position LS and masked
@@ -47,255 +124,12 @@ __device__ __forceinline__ unsigned field_at(const unsigned (&w)[NW]) {
   constexpr unsigned mask = ((1u << NB) - 1u) << LS;
   unsigned v;
   if constexpr (s + NB > 32)
-    v = __funnelshift_r(w[wi], w[(wi + 1) % NW], s - LS);
+    v = __funnelshift_r(w[wi], w[(wi + 1) % NW], (s - LS) & 31);
   else if constexpr (s >= LS)
     v = w[wi] >> (s - LS);
   else
     v = w[wi] << (LS - s);
   return v & mask;
-}
-
-constexpr int kMaxSegments = 64;      // split-K partial slots per unit (tq_api.cu sizes the workspace)
-#ifndef TQ_DECODE_CTAS64
-#define TQ_DECODE_CTAS64 5
-#endif
-#ifndef TQ_DECODE_THREADS
-#define TQ_DECODE_THREADS 128
-#endif
-constexpr int kDecodeThreads = TQ_DECODE_THREADS;  // warps of one CTA share the tables of one unit
-constexpr int kDecodeWarps = kDecodeThreads / 32;
-constexpr int kBuildThreads = 128;  // threads that build the tables and apply PI_V^T
-
-// Shared-memory map in ABSOLUTE shared-window addresses (the OR-addressing needs the K/V tables aligned to
-// their own size, the sign table to 4 KB).  Dynamic shared memory starts right after the 1 KB the driver
-// reserves, so everything is placed at fixed absolute addresses and the kernel traps if the window starts
-// later than kAbsWbuf.
-template <int D>
-struct DecodeCfg {
-  using Lo = Layout<D>;
-  static constexpr int NCK = D;                          // columns of the K table = 2 P (>= P + 31)
-  static constexpr int LSK = D == 64 ? 8 : 9;            // log2(NCK * 4)
-  static constexpr int kKtabBytes = 64 * NCK * 4;        // 16 KB | 32 KB
-  static constexpr int kVtabBytes = 64 * 16 * 8;         // 8 KB: [entry][lane mod 16] float2 (64-bit reads are
-                                                         // served one half-warp at a time)
-  static constexpr int kStabBytes = 16 * 64 * 4;         // 4 KB
-  static constexpr unsigned kAbsWbuf = 2048;             // 4 warps x 32 softmax weights, then the arrival flag
-  static constexpr unsigned kAbsStab = 4096;
-  static constexpr unsigned kAbsVtab = 8192;
-  static constexpr unsigned kAbsKtab = D == 64 ? 16384 : 32768;
-  static constexpr unsigned kAbsScratch = D == 64 ? 32768 : 16384;  // per-warp partials, merged o
-  static constexpr int kScratchBytes = 16 + 8 * (D + 2) * 4 + 2 * D * 4;  // up to 8 warps
-  static constexpr unsigned kAbsEnd = D == 64 ? kAbsScratch + kScratchBytes : kAbsKtab + kKtabBytes;
-  static constexpr int kSmemBytes = kAbsEnd;             // requested dynamic bytes (window start <= 2 KB)
-  static constexpr int kCtasPerSm = D == 64 ? TQ_DECODE_CTAS64 : 3;
-};
-
-// ---- packed fp32x2 arithmetic (sm_100: FFMA2 / FADD2 / FMUL2 issue two fp32 operations per slot) ----------
-typedef unsigned long long f32x2;
-__device__ __forceinline__ f32x2 pack2(float lo, float hi) {
-  f32x2 r;
-  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
-  return r;
-}
-__device__ __forceinline__ void unpack2(f32x2 v, float& lo, float& hi) {
-  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
-}
-__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) {
-  f32x2 r;
-  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
-  return r;
-}
-__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) {
-  f32x2 r;
-  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
-  return r;
-}
-__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) {
-  f32x2 r;
-  asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
-  return r;
-}
-__device__ __forceinline__ f32x2 lds_b64(unsigned addr) {
-  f32x2 v;
-  asm("ld.shared.b64 %0, [%1];" : "=l"(v) : "r"(addr));
-  return v;
-}
-
-// <q'', lut_K[codes]>: P table reads, summed two at a time
-// pairwise (tree) sum of N packed pairs, then of the two halves: short dependency chains for the scheduler
-template <int N>
-__device__ __forceinline__ float tree_sum(f32x2 (&v)[N]) {
-#pragma unroll
-  for (int n = N / 2; n >= 1; n >>= 1)
-#pragma unroll
-    for (int i = 0; i < n; ++i) v[i] = add2(v[i], v[i + n]);
-  float a, b;
-  unpack2(v[0], a, b);
-  return a + b;
-}
-template <int D, int... K>
-__device__ __forceinline__ float k_score(const unsigned (&kw)[Layout<D>::KCW], unsigned kbase,
-                                         std::integer_sequence<int, K...>) {
-  // all table addresses first, then all reads, then the sum: three wide phases instead of 32 short chains
-  const unsigned a0[sizeof...(K)] = {(field_at<DecodeCfg<D>::LSK, 12 * K, 6>(kw) | kbase)...};
-  const unsigned a1[sizeof...(K)] = {(field_at<DecodeCfg<D>::LSK, 12 * K + 6, 6>(kw) | kbase)...};
-  f32x2 v[sizeof...(K)] = {pack2(lds_f32<8 * K>(a0[K]), lds_f32<8 * K + 4>(a1[K]))...};
-  return tree_sum(v);
-}
-
-// <z, sigma>: d/4 nibble-table reads
-template <int D, int... K>
-__device__ __forceinline__ float s_score(const unsigned (&sw)[Layout<D>::KSW], unsigned sbase,
-                                         std::integer_sequence<int, K...>) {
-  const unsigned a0[sizeof...(K)] = {(field_at<8, 8 * K, 4>(sw) | sbase)...};
-  const unsigned a1[sizeof...(K)] = {(field_at<8, 8 * K + 4, 4>(sw) | sbase)...};
-  f32x2 v[sizeof...(K)] = {pack2(lds_f32<8 * K>(a0[K]), lds_f32<8 * K + 4>(a1[K]))...};
-  return tree_sum(v);
-}
-
-// V accumulate, lane = coordinate pair: for token J of the tile, o2[part] += w_J * (lut_V[c0], lut_V[c1])
-template <int D, int J>
-__device__ __forceinline__ void v_token(const unsigned (&vw)[Layout<D>::KCW], unsigned vbase, float w,
-                                        f32x2 (&o2)[2 * (Layout<D>::P / kTile)]) {
-  const f32x2 w2 = pack2(w, w);
-#pragma unroll
-  for (int part = 0; part < Layout<D>::P / kTile; ++part) {
-    unsigned f = part == 0 ? field_at<7, 6 * J, 6>(vw) : field_at<7, 192 * (Layout<D>::P / kTile - 1) + 6 * J, 6>(vw);
-    o2[2 * part + (J & 1)] = fma2(lds_b64(f | vbase), w2, o2[2 * part + (J & 1)]);
-  }
-}
-template <int D, int... J>
-__device__ __forceinline__ void v_accum(const unsigned (&vw)[Layout<D>::KCW], unsigned vbase, unsigned wbuf,
-                                        unsigned nz /* ballot: token slots with a non-zero weight */,
-                                        f32x2 (&o2)[2 * (Layout<D>::P / kTile)], std::integer_sequence<int, J...>) {
-  // w of tokens 4J .. 4J+3 arrive with one broadcast 128-bit read; groups whose weights are all 0 are skipped
-  (([&] {
-     if (nz & (0xfu << (4 * J))) {
-       float4 w4;
-       asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4+%5];"
-                    : "=f"(w4.x), "=f"(w4.y), "=f"(w4.z), "=f"(w4.w)
-                    : "r"(wbuf), "n"(16 * J));
-       v_token<D, 4 * J>(vw, vbase, w4.x, o2);
-       v_token<D, 4 * J + 1>(vw, vbase, w4.y, o2);
-       v_token<D, 4 * J + 2>(vw, vbase, w4.z, o2);
-       v_token<D, 4 * J + 3>(vw, vbase, w4.w, o2);
-     }
-   }()),
-   ...);
-}
-
-// What one lane loads per tile: its own token's K code / sign strings and norms (lane = token), and the V
-// code string of its coordinate pair(s) for all 32 tokens (lane = pair).
-template <int D>
-struct TileWords {
-  unsigned kw[Layout<D>::KCW];
-  unsigned sw[Layout<D>::KSW];
-  unsigned vw[Layout<D>::KCW];
-  unsigned short kn, kr, vn;
-};
-
-template <int W>
-__device__ __forceinline__ void load_words(unsigned (&dst)[W], const unsigned char* sec, int lane) {
-#pragma unroll
-  for (int c = 0; c < W / 4; ++c) {
-    uint4 v = __ldg(reinterpret_cast<const uint4*>(sec + c * 16 * kTile + lane * 16));
-    dst[4 * c] = v.x;
-    dst[4 * c + 1] = v.y;
-    dst[4 * c + 2] = v.z;
-    dst[4 * c + 3] = v.w;
-  }
-  if constexpr (W % 4 == 2) {
-    uint2 v = __ldg(reinterpret_cast<const uint2*>(sec + (W / 4) * 16 * kTile + lane * 8));
-    dst[W - 2] = v.x;
-    dst[W - 1] = v.y;
-  }
-}
-
-template <int D>
-__device__ __forceinline__ void load_tile_words(TileWords<D>& t, const unsigned char* tp, int lane) {
-  using Lo = Layout<D>;
-  load_words<Lo::KCW>(t.kw, tp + Lo::kOffKC, lane);
-  load_words<Lo::KSW>(t.sw, tp + Lo::kOffKS, lane);
-  load_words<Lo::KCW>(t.vw, tp + Lo::kOffVC, lane);
-  t.kn = __ldg(reinterpret_cast<const unsigned short*>(tp + Lo::kOffKN) + lane);
-  t.kr = __ldg(reinterpret_cast<const unsigned short*>(tp + Lo::kOffKR) + lane);
-  t.vn = __ldg(reinterpret_cast<const unsigned short*>(tp + Lo::kOffVN) + lane);
-}
-
-// ---- table construction (per CTA; the prep kernel stores q'' and z pre-scaled so that logits come out in
-//      log2 units: q'' * log2(e)/sqrt(d), z * log2(e)/sqrt(d) * sqrt(pi/2)/m) ------------------------------------
-// Every thread owns four consecutive table columns and writes them with 128-bit stores.
-template <int D>
-struct TableInputs {  // everything a thread needs from global memory, requested before anything is used
-  float4 qa[1], qb[1];
-  float4 zz[4];
-  float4 lk0, lk1, lv0, lv1;
-};
-
-template <int D>
-__device__ __forceinline__ void load_table_inputs(TableInputs<D>& t, const float* qr, const float* __restrict__ lk,
-                                                  const float* __restrict__ lv, int tid) {
-  using Lo = Layout<D>;
-  using Cfg = DecodeCfg<D>;
-  constexpr int NQ = Cfg::NCK / 4;
-  const int g0 = (4 * (tid % NQ)) % Lo::P;
-  t.qa[0] = __ldcg(reinterpret_cast<const float4*>(qr + 2 * g0));
-  t.qb[0] = __ldcg(reinterpret_cast<const float4*>(qr + 2 * g0) + 1);
-  const int n0 = (4 * (tid % 16)) % Lo::NG;
-#pragma unroll
-  for (int i = 0; i < 4; ++i) t.zz[i] = __ldcg(reinterpret_cast<const float4*>(qr + D + 4 * (n0 + i)));
-  t.lk0 = __ldg(reinterpret_cast<const float4*>(lk));
-  t.lk1 = __ldg(reinterpret_cast<const float4*>(lk) + 1);
-  t.lv0 = __ldg(reinterpret_cast<const float4*>(lv));
-  t.lv1 = __ldg(reinterpret_cast<const float4*>(lv) + 1);
-}
-
-template <int D>
-__device__ __forceinline__ void build_tables(float* Ktab, float* Stab, float2* Vtab, const TableInputs<D>& t, int tid) {
-  using Lo = Layout<D>;
-  using Cfg = DecodeCfg<D>;
-  const float lut[8] = {t.lk0.x, t.lk0.y, t.lk0.z, t.lk0.w, t.lk1.x, t.lk1.y, t.lk1.z, t.lk1.w};
-  {  // Ktab[8 hi + lo][c] = q''_{2g} lut[lo] + q''_{2g+1} lut[hi],  g = c mod P
-    constexpr int NQ = Cfg::NCK / 4;                // column quads: 16 | 32
-    constexpr int HPT = 8 / (kBuildThreads / NQ);  // hi codes per thread: 1 | 2
-    const int cq = tid % NQ, eg = tid / NQ;
-    const float q0[4] = {t.qa[0].x, t.qa[0].z, t.qb[0].x, t.qb[0].z};  // q''_{2g}
-    const float q1[4] = {t.qa[0].y, t.qa[0].w, t.qb[0].y, t.qb[0].w};  // q''_{2g+1}
-#pragma unroll
-    for (int hh = 0; hh < HPT; ++hh) {
-      const int hi = eg * HPT + hh;
-      float lh = lut[0];
-#pragma unroll
-      for (int c = 1; c < 8; ++c) lh = (hi == c) ? lut[c] : lh;
-      const float b0 = q1[0] * lh, b1 = q1[1] * lh, b2 = q1[2] * lh, b3 = q1[3] * lh;
-      float* dst = Ktab + (size_t)(hi * 8) * Cfg::NCK + 4 * cq;
-#pragma unroll
-      for (int lo = 0; lo < 8; ++lo)
-        *reinterpret_cast<float4*>(dst + lo * Cfg::NCK) =
-            make_float4(fmaf(q0[0], lut[lo], b0), fmaf(q0[1], lut[lo], b1), fmaf(q0[2], lut[lo], b2), fmaf(q0[3], lut[lo], b3));
-    }
-  }
-  {  // Stab[e][c] = sum_b (bit b of e ? +z : -z)[4n + b],  n = c mod NG; 16 column quads x 8 entry pairs
-    const int cq = tid % 16, eg = tid / 16;
-#pragma unroll
-    for (int j = 0; j < 2; ++j) {
-      const int e = 2 * eg + j;
-      const float s0 = (e & 1) ? 1.f : -1.f, s1 = (e & 2) ? 1.f : -1.f, s2 = (e & 4) ? 1.f : -1.f, s3 = (e & 8) ? 1.f : -1.f;
-      float v[4];
-#pragma unroll
-      for (int i = 0; i < 4; ++i) v[i] = fmaf(s0, t.zz[i].x, fmaf(s1, t.zz[i].y, fmaf(s2, t.zz[i].z, s3 * t.zz[i].w)));
-      *reinterpret_cast<float4*>(Stab + e * 64 + 4 * cq) = make_float4(v[0], v[1], v[2], v[3]);
-    }
-  }
-  {  // Vtab[8 hi + lo][col] = (lut_V[lo], lut_V[hi]); 128 threads: hi = tid / 16, col = tid % 16
-    const float lv[8] = {t.lv0.x, t.lv0.y, t.lv0.z, t.lv0.w, t.lv1.x, t.lv1.y, t.lv1.z, t.lv1.w};
-    const int col = tid & 15, eq = tid >> 4;
-    float hi = lv[0];
-#pragma unroll
-    for (int c = 1; c < 8; ++c) hi = (eq == c) ? lv[c] : hi;
-#pragma unroll
-    for (int j = 0; j < 8; ++j) Vtab[(eq * 8 + j) * 16 + col] = make_float2(lv[j], hi);
-  }
 }
 
 __device__ __forceinline__ float ex2_ftz(float x) {
@@ -308,29 +142,260 @@ __device__ __forceinline__ float warp_max_f32(float x) {  // sm_100a: one CREDUX
   asm volatile("redux.sync.max.f32 %0, %1, 0xffffffff;" : "=f"(y) : "f"(x));
   return y;
 }
+__device__ __forceinline__ unsigned pack_h2(__half lo, __half hi) {
+  return (unsigned)__half_as_ushort(lo) | ((unsigned)__half_as_ushort(hi) << 16);
+}
+// x = hi + lo in binary16 (two-term split; exact to 2^-22 |x| while |x| stays in the normal range)
+__device__ __forceinline__ void split_h(float x, __half& hi, __half& lo) {
+  hi = __float2half_rn(x);
+  lo = __float2half_rn(x - __half2float(hi));
+}
+__device__ __forceinline__ bool f16_exact(float x) { return __half2float(__float2half_rn(x)) == x; }
+// 2^e as a float, e in [-126, 127]
+__device__ __forceinline__ float pow2i(int e) { return __uint_as_float((unsigned)(e + 127) << 23); }
+// exponent e with 2^e <= |x| < 2^(e+1) (0 for zero / denormal / non-finite input)
+__device__ __forceinline__ int exponent_of(float x) {
+  const int E = (int)((__float_as_uint(x) >> 23) & 0xffu);
+  return (E == 0 || E == 255) ? 0 : E - 127;
+}
+
+// ---- the per-unit B operands ------------------------------------------------------------------------------------------
+// The prep kernel leaves q'' log2(e)/sqrt(d) and z log2(e)/sqrt(d) sqrt(pi/2)/m as fp32 in the workspace.  Every lane
+// builds the B fragments it feeds to the MMAs: column n of B holds the hi part for even n and the lo part for odd n, so a
+// lane's accumulator pair (columns 2t, 2t+1) sums to the full product for every t: no cross-lane traffic afterwards.
+template <int D>
+struct UnitFrags {
+  unsigned bq[D / 16][2];  // K scores: k-step ks, registers b0 (coordinates 16 ks + 2t, +1), b1 (+8, +9)
+  unsigned bz[D / 16][2];  // sign term
+  float kscale;            // accumulator -> <q'', lut> in log2 units
+  float sscale, zsum;      // accumulator -> 2 sum_j bit_j z_j ; sum_j z_j
+};
+
+// this lane's pattern (g & 1, t) of the unit's fragment block (tq_common.cuh FragLayout), four 128-bit loads per 16 words
+template <int D>
+__device__ __forceinline__ void load_frags(UnitFrags<D>& f, const unsigned* fb, int lane) {
+  using FL = FragLayout<D>;
+  constexpr int KS = D / 16;
+  const uint4* src = reinterpret_cast<const uint4*>(fb + (((lane >> 2) & 1) * 4 + (lane & 3)) * FL::kWordsPerPat);
+  unsigned w[4 * KS];
+#pragma unroll
+  for (int i = 0; i < KS; ++i) {
+    const uint4 v = __ldcg(src + i);
+    w[4 * i] = v.x, w[4 * i + 1] = v.y, w[4 * i + 2] = v.z, w[4 * i + 3] = v.w;
+  }
+  const float4 sc = __ldcg(reinterpret_cast<const float4*>(fb + FL::kScalOff));
+#pragma unroll
+  for (int ks = 0; ks < KS; ++ks) {
+    f.bq[ks][0] = w[2 * ks], f.bq[ks][1] = w[2 * ks + 1];
+    f.bz[ks][0] = w[2 * KS + 2 * ks], f.bz[ks][1] = w[2 * KS + 2 * ks + 1];
+  }
+  f.kscale = sc.x, f.sscale = sc.y, f.zsum = sc.z;
+}
+
+// ---- one 32-token tile ------------------------------------------------------------------------------------------------
+// kFast: the LUT entries are binary16-representable, the tables hold fp16 pairs (one 32-bit read per field);
+// otherwise they hold (hi pair, lo pair) and every field costs one 64-bit read and two MMAs.
+template <int D, bool kFast>
+struct TileMath {
+  using Lo = Layout<D>;
+  using Cfg = DecodeCfg<D>;
+  static constexpr int KS = D / 16;       // k-steps of the K / sign contractions
+  static constexpr int MV = D / 16;       // m-tiles (16 coordinates each) of the V contraction
+  static constexpr int LS = 7;            // log2 of the table row pitch (32 lanes x 4 bytes | 16 x 8 bytes)
+  static constexpr unsigned kAbsKtab = Cfg::kAbsTab;
+  static constexpr unsigned kAbsVtab = Cfg::kAbsTab + Cfg::kTabBytes;
+
+  // scores of this lane's four token slots: kacc[mt] / sacc[mt] = {row g: hi, lo; row g+8: hi, lo} of m-tile mt
+  template <int... KSI>
+  static __device__ __forceinline__ void scores(const unsigned (&kw)[Lo::KCW], const unsigned (&sw)[Lo::KSW],
+                                                const UnitFrags<D>& f, unsigned lane_off, float (&kacc)[2][4],
+                                                float (&sacc)[2][4], std::integer_sequence<int, KSI...>) {
+    (([&] {
+       constexpr int ks = KSI;
+#pragma unroll
+       for (int mt = 0; mt < 2; ++mt) {
+         // K: fields (r = 2 mt | 2 mt + 1, j = 2 ks | 2 ks + 1) at bit 6 (J r + j)
+         const unsigned x0 = fieldk<2 * 0 + 0, ks>(kw, mt) | lane_off, x1 = fieldk<1, ks>(kw, mt) | lane_off;
+         const unsigned x2 = fieldk<2, ks>(kw, mt) | lane_off, x3 = fieldk<3, ks>(kw, mt) | lane_off;
+         if constexpr (kFast) {
+           mma16816(kacc[mt], lds_u32<kAbsKtab>(x0), lds_u32<kAbsKtab>(x1), lds_u32<kAbsKtab>(x2), lds_u32<kAbsKtab>(x3),
+                    f.bq[ks][0], f.bq[ks][1]);
+         } else {
+           const uint2 a0 = lds_u32x2<kAbsKtab>(x0), a1 = lds_u32x2<kAbsKtab>(x1), a2 = lds_u32x2<kAbsKtab>(x2),
+                       a3 = lds_u32x2<kAbsKtab>(x3);
+           mma16816(kacc[mt], a0.x, a1.x, a2.x, a3.x, f.bq[ks][0], f.bq[ks][1]);
+           mma16816(kacc[mt], a0.y, a1.y, a2.y, a3.y, f.bq[ks][0], f.bq[ks][1]);
+         }
+         // signs: word (mt, u), rows {p0, p0 + 8} and {p0 + 1, p0 + 9} of piece u as fp16 subnormals
+         constexpr int u = ks >> 2, p0 = 2 * (ks & 3);
+         const unsigned w = sw[mt * Lo::U + u], wb = w >> 8;
+         mma16816(sacc[mt], w & (0x00010001u << p0), wb & (0x00010001u << p0), w & (0x00010001u << (p0 + 1)),
+                  wb & (0x00010001u << (p0 + 1)), f.bz[ks][0], f.bz[ks][1]);
+       }
+     }()),
+     ...);
+  }
+  // A register index q (0..3) of (mt, ks): r = 2 mt + (q & 1), j = 2 ks + (q >> 1)
+  template <int Q, int KSI>
+  static __device__ __forceinline__ unsigned fieldk(const unsigned (&kw)[Lo::KCW], int mt) {
+    constexpr int j = 2 * KSI + (Q >> 1);
+    return mt == 0 ? field_at<LS, 6 * (Lo::J * (Q & 1) + j), 6>(kw) : field_at<LS, 6 * (Lo::J * (2 + (Q & 1)) + j), 6>(kw);
+  }
+
+  // V accumulate for the 16 tokens of k-step KSV: o[mt] += A(16 coordinates x 16 tokens) w
+  template <int KSV, int... MTI>
+  static __device__ __forceinline__ void values(const unsigned (&vw)[Lo::KCW], unsigned lane_off, unsigned b0, unsigned b1,
+                                                float (&o)[MV][4], std::integer_sequence<int, MTI...>) {
+    (([&] {
+       constexpr int mt = MTI;
+       // fields (j = 2 ksv | 2 ksv + 1, c = 2 mt | 2 mt + 1) at bit 6 (C j + c)
+       const unsigned x0 = field_at<LS, 6 * (Lo::C * (2 * KSV) + 2 * mt), 6>(vw) | lane_off;
+       const unsigned x1 = field_at<LS, 6 * (Lo::C * (2 * KSV) + 2 * mt + 1), 6>(vw) | lane_off;
+       const unsigned x2 = field_at<LS, 6 * (Lo::C * (2 * KSV + 1) + 2 * mt), 6>(vw) | lane_off;
+       const unsigned x3 = field_at<LS, 6 * (Lo::C * (2 * KSV + 1) + 2 * mt + 1), 6>(vw) | lane_off;
+       if constexpr (kFast) {
+         mma16816(o[mt], lds_u32<kAbsVtab>(x0), lds_u32<kAbsVtab>(x1), lds_u32<kAbsVtab>(x2), lds_u32<kAbsVtab>(x3), b0, b1);
+       } else {
+         const uint2 a0 = lds_u32x2<kAbsVtab>(x0), a1 = lds_u32x2<kAbsVtab>(x1), a2 = lds_u32x2<kAbsVtab>(x2),
+                     a3 = lds_u32x2<kAbsVtab>(x3);
+         mma16816(o[mt], a0.x, a1.x, a2.x, a3.x, b0, b1);
+         mma16816(o[mt], a0.y, a1.y, a2.y, a3.y, b0, b1);
+       }
+     }()),
+     ...);
+  }
+};
+
+// words of a section of W words per lane, from the tile image in shared memory
+template <int W>
+__device__ __forceinline__ void lds_words(unsigned (&dst)[W], unsigned sec, int lane) {
+#pragma unroll
+  for (int c = 0; c < W / 4; ++c) {
+    const uint4 v = lds_u32x4(sec + c * 16 * kTile + lane * 16);
+    dst[4 * c] = v.x, dst[4 * c + 1] = v.y, dst[4 * c + 2] = v.z, dst[4 * c + 3] = v.w;
+  }
+  if constexpr (W % 4 == 2) {
+    const uint2 v = lds_u32x2_dyn(sec + (W / 4) * 16 * kTile + lane * 8);
+    dst[W - 2] = v.x, dst[W - 1] = v.y;
+  }
+}
+
+// ---- the streaming loop of one warp -----------------------------------------------------------------------------------
+template <int D, bool kFast>
+__device__ __forceinline__ void stream_tiles(const unsigned char* stream, int tile_first, int tile1, int T, int warp, int lane,
+                                             const UnitFrags<D>& f, float& m_out, float& l_out, float (&o)[D / 16][4]) {
+  using Lo = Layout<D>;
+  using Cfg = DecodeCfg<D>;
+  using TM = TileMath<D, kFast>;
+  constexpr int NW = kDecodeWarps;
+  const int t = lane & 3;
+  const unsigned lane_off = kFast ? (unsigned)lane << 2 : (unsigned)(lane & 15) << 3;  // table column of this lane
+  const unsigned ring = Cfg::kAbsRing + warp * kStages * Lo::kTileBytes;
+  const unsigned bar0 = Cfg::kAbsBar + warp * kStages * 8;
+  const unsigned wbuf = Cfg::kAbsWbuf + warp * 128;  // [hi | lo][32 slots] binary16
+  const int my_slot = lane_slot(lane);
+  float m = -INFINITY, l = 0.f;
+
+  // ring state: slot image and barrier of the tile at hand, phase parity of this round over the ring, and the global
+  // address of the tile kStages rounds ahead
+  unsigned img = ring, bar = bar0, parity = 0;
+  int st = 0;
+  const unsigned char* src_next = stream + (size_t)(tile_first + kStages * NW) * Lo::kTileBytes;
+  for (int tile = tile_first; tile < tile1; tile += NW) {
+    mbar_wait(bar, parity);
+
+    // ---- scores (tensor cores): lane (g, t) ends up with the K and sign sums of slots g + 8 r
+    unsigned kw[Lo::KCW], sw[Lo::KSW];
+    lds_words<Lo::KCW>(kw, img + Lo::kOffKC, lane);
+    lds_words<Lo::KSW>(sw, img + Lo::kOffKS, lane);
+    float kacc[2][4], sacc[2][4];
+#pragma unroll
+    for (int i = 0; i < 2; ++i)
+#pragma unroll
+      for (int j = 0; j < 4; ++j) kacc[i][j] = 0.f, sacc[i][j] = 0.f;
+    TM::scores(kw, sw, f, lane_off, kacc, sacc, std::make_integer_sequence<int, D / 16>{});
+    // this lane's own slot g + 8 t: m-tile t >> 1, row half t & 1
+    const float k01 = t & 2 ? kacc[1][0] + kacc[1][1] : kacc[0][0] + kacc[0][1];
+    const float k23 = t & 2 ? kacc[1][2] + kacc[1][3] : kacc[0][2] + kacc[0][3];
+    const float s01 = t & 2 ? sacc[1][0] + sacc[1][1] : sacc[0][0] + sacc[0][1];
+    const float s23 = t & 2 ? sacc[1][2] + sacc[1][3] : sacc[0][2] + sacc[0][3];
+    const float kval = (t & 1 ? k23 : k01) * f.kscale;
+    const float sval = fmaf(t & 1 ? s23 : s01, f.sscale, -f.zsum);
+
+    // ---- online softmax, lane = token slot
+    unsigned nk;
+    unsigned short nv;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(nk) : "r"(img + Lo::kOffNK + lane * 4) : "memory");
+    asm volatile("ld.shared.u16 %0, [%1];" : "=h"(nv) : "r"(img + Lo::kOffVN + lane * 2) : "memory");
+    const bool valid = tile * kTile + my_slot < T;
+    float s2 = f16_bits_to_f32((unsigned short)(nk & 0xffffu)) * fmaf(f16_bits_to_f32((unsigned short)(nk >> 16)), sval, kval);
+    s2 = valid ? s2 : -INFINITY;
+    const float mnew = fmaxf(m, warp_max_f32(s2));  // finite: slot 0 of every processed tile is valid
+    const float fsc = ex2_ftz(m - mnew);            // 0 on a warp's first tile (m = -inf)
+    const float p = ex2_ftz(s2 - mnew);             // invalid lanes: exp2(-inf) = 0
+    l = fmaf(l, fsc, p);
+    if (mnew != m) {  // warp-uniform
+#pragma unroll
+      for (int i = 0; i < D / 16; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) o[i][j] *= fsc;
+    }
+    m = mnew;
+    const float wv = valid ? p * f16_bits_to_f32(nv) : 0.f;
+    const unsigned nz = __ballot_sync(0xffffffffu, wv != 0.f);
+    if (nz) {
+      // hand the weights from lane = slot to the B-fragment order (tokens 2t, 2t+1, 2t+8, 2t+9 of each k-step) through
+      // shared memory, split hi + lo: lanes with even g feed the hi column, odd g the lo column
+      __half wh, wl;
+      split_h(wv, wh, wl);
+      __syncwarp();
+      asm volatile("st.shared.u16 [%0], %1;" ::"r"(wbuf + my_slot * 2), "h"(__half_as_ushort(wh)) : "memory");
+      asm volatile("st.shared.u16 [%0], %1;" ::"r"(wbuf + 64 + my_slot * 2), "h"(__half_as_ushort(wl)) : "memory");
+      __syncwarp();
+      unsigned vw[Lo::KCW];
+      lds_words<Lo::KCW>(vw, img + Lo::kOffVC, lane);
+      const unsigned wsrc = wbuf + ((lane >> 2) & 1) * 64 + t * 4;
+      // slots 16 ks .. 16 ks + 15 belong to the lanes with (t >> 1) == ks
+      if (nz & 0x33333333u) {
+        unsigned b0, b1;
+        asm volatile("ld.shared.u32 %0, [%1];" : "=r"(b0) : "r"(wsrc) : "memory");
+        asm volatile("ld.shared.u32 %0, [%1+16];" : "=r"(b1) : "r"(wsrc) : "memory");
+        TM::template values<0>(vw, lane_off, b0, b1, o, std::make_integer_sequence<int, D / 16>{});
+      }
+      if (nz & 0xccccccccu) {
+        unsigned b0, b1;
+        asm volatile("ld.shared.u32 %0, [%1+32];" : "=r"(b0) : "r"(wsrc) : "memory");
+        asm volatile("ld.shared.u32 %0, [%1+48];" : "=r"(b1) : "r"(wsrc) : "memory");
+        TM::template values<1>(vw, lane_off, b0, b1, o, std::make_integer_sequence<int, D / 16>{});
+      }
+    }
+    // ---- the slot is consumed (every word of the image has been used): refill it with the tile kStages rounds ahead
+    __syncwarp();
+    if (lane == 0 && tile + kStages * NW < tile1) tma_load_tile(img, src_next, Lo::kTileBytes, bar);
+    src_next += NW * Lo::kTileBytes;
+    img += Lo::kTileBytes, bar += 8;
+    if (++st == kStages) st = 0, img = ring, bar = bar0, parity ^= 1u;
+  }
+  m_out = m;
+  l_out = l;
+}
 
 // ---- the streaming kernel ------------------------------------------------------------------------------------
-// grid = units x nsplit.  CTA (unit uc, split sp) streams tiles [sp * per, (sp + 1) * per) of its unit, where
-// per = ceil(ceil(T / 32) / nsplit) is derived on the device from seq_len, so a shorter cache simply leaves the
-// trailing splits empty.  The four warps take tiles round-robin with a register double buffer.
+// grid = units x nsplit.  CTA (unit uc, split sp) streams tiles [sp * per, (sp + 1) * per) of its unit, per = tiles per
+// split planned on the host from t_hint (the last split also takes whatever lies beyond); a shorter cache simply
+// leaves the trailing splits empty.  The four warps take tiles round-robin.
 template <int D, typename TIO>
 __global__ void __launch_bounds__(kDecodeThreads, DecodeCfg<D>::kCtasPerSm) decode_main_kernel(DecodeArgs a) {
   using Lo = Layout<D>;
   using Cfg = DecodeCfg<D>;
   constexpr int NW = kDecodeWarps;
-  constexpr int VP = Lo::P / kTile;  // coordinate pairs per lane: 1 | 2
   extern __shared__ unsigned char smem_raw[];
   const unsigned raw = (unsigned)__cvta_generic_to_shared(smem_raw);
-  if (raw > Cfg::kAbsWbuf) __trap();  // the fixed shared-memory map does not fit: fail loudly
+  if (raw > Cfg::kAbsMisc) __trap();  // the fixed shared-memory map does not fit: fail loudly
   unsigned char* abs0 = smem_raw - raw;  // generic pointer to absolute shared address 0 of this CTA's window
-  float* Stab = reinterpret_cast<float*>(abs0 + Cfg::kAbsStab);
-  float* red = reinterpret_cast<float*>(abs0 + Cfg::kAbsScratch + 16);  // NW x (D + 2)
-  float* omerged = red + NW * (D + 2);                                   // [D] + [D] partial matvec
-  float* wbuf_f = reinterpret_cast<float*>(abs0 + Cfg::kAbsWbuf);       // NW x 32 softmax weights
-  int* flag = reinterpret_cast<int*>(wbuf_f + NW * 32);
-  float* Ktab = reinterpret_cast<float*>(abs0 + Cfg::kAbsKtab);
-  float2* Vtab = reinterpret_cast<float2*>(abs0 + Cfg::kAbsVtab);
-  const unsigned ktab = Cfg::kAbsKtab, vtab = Cfg::kAbsVtab, stab = Cfg::kAbsStab;
+  float* red = reinterpret_cast<float*>(abs0 + Cfg::kAbsRed);  // NW x (D + 2)
+  float* omerged = red + NW * (D + 2);                          // [D] + [D] partial matvec
+  int* flag = reinterpret_cast<int*>(abs0 + Cfg::kAbsFlag);
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int B = a.cv.B, H = a.cv.H;
@@ -340,116 +405,120 @@ __global__ void __launch_bounds__(kDecodeThreads, DecodeCfg<D>::kCtasPerSm) deco
   const int lc = e / B, b = e - lc * B;
   const int layer = a.layer_begin + lc;
   const size_t lh = (size_t)layer * H + h;
-  {  // before the PDL wait: hints only.  The cache stream of this CTA starts towards L2 while the prep kernel in front
-     // of this launch is still running (it rewrites at most one tile per unit, and L2 stays coherent); PI_V too.
-    const int per0 = a.per, t0 = sp * per0;
-    const int c1 = sp == nsplit - 1 ? a.cv.tiles_cap : min(a.cv.tiles_cap, t0 + per0);
-    const unsigned char* st0 = a.cv.tiles + (((size_t)layer * B + b) * H + h) * a.cv.stream_bytes;
-#pragma unroll
-    for (int i = 0; i < 3; ++i) {
-      const int t = t0 + warp + i * NW;
-      if (t < c1 && lane == 0)
-        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(st0 + (size_t)t * Lo::kTileBytes), "r"(Lo::kTileBytes)
-                     : "memory");
-    }
-  }
-  pdl_wait();
-  // ---- every global request the prologue depends on goes out first and together: the cache length, the table
-  //      inputs, then (speculatively, from the host's split plan) this warp's first tile, so that the small loads
-  //      never queue behind the bulk ones
-  int T;
-  asm volatile("ld.global.b32 %0, [%1];" : "=r"(T) : "l"(a.cv.seq_len + a.layer_begin * B + e));
-  TableInputs<D> tin;
-  if (tid < kBuildThreads) load_table_inputs<D>(tin, a.qrot + (size_t)uc * 2 * D, a.lut_k + lh * 8, a.lut_v + lh * 8, tid);
-  const int per = a.per;  // tiles per split planned from t_hint; the last split also takes whatever lies beyond
-  const int tile0 = sp * per;
+  const int per = a.per, tile0 = sp * per;
   const int cap1 = sp == nsplit - 1 ? a.cv.tiles_cap : min(a.cv.tiles_cap, tile0 + per);  // static bound of this split
   const unsigned char* stream = a.cv.tiles + (((size_t)layer * B + b) * H + h) * a.cv.stream_bytes;
-  TileWords<D> bufA, bufB;  // register double buffer, ping-pong (no copies)
-  if (tile0 + warp < cap1) load_tile_words<D>(bufA, stream + (size_t)(tile0 + warp) * Lo::kTileBytes, lane);
-  auto prefetch_tile = [&](int t, int bound) {  // one bulk L2 prefetch per tile, issued by one lane
-    if (t < bound && lane == 0)
-      asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(stream + (size_t)t * Lo::kTileBytes),
-                   "r"(Lo::kTileBytes)
+
+  // ---- before the PDL wait: only constants and hints.  The cache stream of this CTA starts towards L2 while the
+  //      kernel in front of this launch is still running (L2 stays coherent with whatever it still writes); the
+  //      dequantisation tables depend on the LUTs alone.
+#pragma unroll
+  for (int i = 0; i < kStages; ++i) {
+    const int tl = tile0 + warp + i * NW;
+    if (tl < cap1 && lane == 0)
+      asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(stream + (size_t)tl * Lo::kTileBytes), "r"(Lo::kTileBytes)
                    : "memory");
-  };
-  constexpr int kPrefetchAhead = 3;  // rounds of NW tiles
+  }
+  if (lane == 0) {
+#pragma unroll
+    for (int i = 0; i < kStages; ++i) mbar_init(Cfg::kAbsBar + (warp * kStages + i) * 8, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
   const float* Pv = a.pi_v + lh * D * D;
 #pragma unroll
-  for (int i = 0; i < D * D * 4 / 128 / kBuildThreads; ++i)
-    if (tid < kBuildThreads) asm volatile("prefetch.global.L2 [%0];" ::"l"(Pv + (size_t)(i * kBuildThreads + tid) * 32));
+  for (int i = 0; i < D * D * 4 / 128 / kDecodeThreads; ++i)
+    asm volatile("prefetch.global.L2 [%0];" ::"l"(Pv + (size_t)(i * kDecodeThreads + tid) * 32));
+
+  if (a.chain_mode == 0) pdl_wait();
+  pdl_trigger();  // the launch behind this one may be scheduled: it either waits for this grid or belongs to the same chain
+  // ---- the first kStages tiles of this warp go on their way at once (their addresses follow from the host's split
+  //      plan alone); the cache length and the unit's B operands are fetched while they fly
+  int issued = 0;
+#pragma unroll
+  for (int i = 0; i < kStages; ++i) issued += (tile0 + warp + i * NW < cap1) ? 1 : 0;
+  if (lane == 0) {
+#pragma unroll
+    for (int i = 0; i < kStages; ++i) {
+      const int tl = tile0 + warp + i * NW;
+      if (tl < cap1)
+        tma_load_tile(Cfg::kAbsRing + (warp * kStages + i) * Lo::kTileBytes, stream + (size_t)tl * Lo::kTileBytes, Lo::kTileBytes,
+                      Cfg::kAbsBar + (warp * kStages + i) * 8);
+    }
+  }
+  int T;
+  asm volatile("ld.global.cg.b32 %0, [%1];" : "=r"(T) : "l"(a.cv.seq_len + a.layer_begin * B + e) : "memory");
+  // dequantisation tables of this head (prep kernel): warp w expands entries 16 w .. 16 w + 15 over the lane columns
+  const unsigned* tb = a.tabs + ((size_t)lc * H + h) * kTabWords;
+  const bool fast = __ldcg(tb + 256) != 0u;
+  {
+    unsigned kt[16], vt[16];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const uint4 k4 = __ldcg(reinterpret_cast<const uint4*>(tb + warp * 16) + i);
+      const uint4 v4 = __ldcg(reinterpret_cast<const uint4*>(tb + 128 + warp * 16) + i);
+      kt[4 * i] = k4.x, kt[4 * i + 1] = k4.y, kt[4 * i + 2] = k4.z, kt[4 * i + 3] = k4.w;
+      vt[4 * i] = v4.x, vt[4 * i + 1] = v4.y, vt[4 * i + 2] = v4.z, vt[4 * i + 3] = v4.w;
+    }
+    if (fast) {  // [64][32 lanes] fp16 pairs
+      unsigned* kd = reinterpret_cast<unsigned*>(abs0 + Cfg::kAbsTab) + warp * 16 * 32 + lane;
+      unsigned* vd = reinterpret_cast<unsigned*>(abs0 + Cfg::kAbsTab + Cfg::kTabBytes) + warp * 16 * 32 + lane;
+#pragma unroll
+      for (int i = 0; i < 16; ++i) kd[i * 32] = kt[i], vd[i * 32] = vt[i];
+    } else {  // [64][16] (hi pair, lo pair)
+      uint2* kd = reinterpret_cast<uint2*>(abs0 + Cfg::kAbsTab) + warp * 16 * 16 + (lane & 15);
+      uint2* vd = reinterpret_cast<uint2*>(abs0 + Cfg::kAbsTab + Cfg::kTabBytes) + warp * 16 * 16 + (lane & 15);
+#pragma unroll
+      for (int i = 0; i < 4; ++i) {
+        const uint4 k4 = __ldcg(reinterpret_cast<const uint4*>(tb + 64 + warp * 16) + i);
+        const uint4 v4 = __ldcg(reinterpret_cast<const uint4*>(tb + 192 + warp * 16) + i);
+        kd[(4 * i) * 16] = make_uint2(kt[4 * i], k4.x), kd[(4 * i + 1) * 16] = make_uint2(kt[4 * i + 1], k4.y);
+        kd[(4 * i + 2) * 16] = make_uint2(kt[4 * i + 2], k4.z), kd[(4 * i + 3) * 16] = make_uint2(kt[4 * i + 3], k4.w);
+        vd[(4 * i) * 16] = make_uint2(vt[4 * i], v4.x), vd[(4 * i + 1) * 16] = make_uint2(vt[4 * i + 1], v4.y);
+        vd[(4 * i + 2) * 16] = make_uint2(vt[4 * i + 2], v4.z), vd[(4 * i + 3) * 16] = make_uint2(vt[4 * i + 3], v4.w);
+      }
+    }
+  }
+  UnitFrags<D> fr;
+  load_frags<D>(fr, a.frags + (size_t)uc * FragLayout<D>::kWords, lane);
   const int nt = (T + kTile - 1) / kTile;
-  if (tile0 >= nt) return;  // empty cache (the prep kernel wrote out = 0) or a trailing split with nothing to do
   const int tile1 = min(nt, cap1);
   const int nseg = min(nsplit, (nt + per - 1) / per);  // splits of this unit that have work
-  if (tid < kBuildThreads) build_tables<D>(Ktab, Stab, Vtab, tin, tid);
-  __syncthreads();
-
-  // table base | lane column as ONE register.  ptxas sees through an empty asm and would split the constant base
-  // from the lane term again (an extra LOP3 per lookup); XOR with a kernel argument that is always 0 keeps it whole,
-  // so every lookup address is a single LOP3: (field & mask) | base.
-  const unsigned kbase = (ktab + lane * 4) ^ (unsigned)a.zero, sbase = (stab + lane * 4) ^ (unsigned)a.zero,
-                 vbase = (vtab + (lane & 15) * 8) ^ (unsigned)a.zero;
-  const unsigned wbuf = (unsigned)__cvta_generic_to_shared(wbuf_f + warp * 32);
-
-  f32x2 o2[2 * VP];  // [pair][even / odd tokens]
-#pragma unroll
-  for (int i = 0; i < 2 * VP; ++i) o2[i] = 0ull;
-  float m = -INFINITY, l = 0.f;
-
-  // one 32-token tile: scores (lane = token) -> online softmax -> V accumulate (lane = coordinate pair)
-  auto process = [&](const TileWords<D>& tw, int tile) {
-    const bool valid = tile * kTile + lane < T;
-    const float sa = k_score<D>(tw.kw, kbase, std::make_integer_sequence<int, Lo::P / 2>{});
-    const float sb = s_score<D>(tw.sw, sbase, std::make_integer_sequence<int, Lo::NG / 2>{});
-    float s2 = f16_bits_to_f32(tw.kn) * fmaf(f16_bits_to_f32(tw.kr), sb, sa);
-    s2 = valid ? s2 : -INFINITY;
-    const float mnew = fmaxf(m, warp_max_f32(s2));  // finite: slot 0 of every processed tile is valid
-    const float fsc = ex2_ftz(m - mnew);            // 0 on a warp's first tile (m = -inf)
-    m = mnew;
-    const float p = ex2_ftz(s2 - m);                // invalid lanes: exp2(-inf) = 0
-    l = fmaf(l, fsc, p);
-    const f32x2 fsc2 = pack2(fsc, fsc);
-#pragma unroll
-    for (int i = 0; i < 2 * VP; ++i) o2[i] = mul2(o2[i], fsc2);
-    const float wv = valid ? p * f16_bits_to_f32(tw.vn) : 0.f;
-    const unsigned nz = __ballot_sync(0xffffffffu, wv != 0.f);
-    if (nz) {
-      // hand the softmax weights from lane = token to lane = coordinate pair through shared memory
-      __syncwarp();
-      asm volatile("st.shared.f32 [%0], %1;" ::"r"(wbuf + lane * 4), "f"(wv));
-      __syncwarp();
-      v_accum<D>(tw.vw, vbase, wbuf, nz, o2, std::make_integer_sequence<int, kTile / 4>{});
-    }
-  };
-  auto fetch = [&](TileWords<D>& tw, int tile) {
-    prefetch_tile(tile + (kPrefetchAhead - 1) * NW, tile1);
-    if (tile < tile1) load_tile_words<D>(tw, stream + (size_t)tile * Lo::kTileBytes, lane);
-  };
-  int tile = tile0 + warp;
-  while (tile < tile1) {
-    fetch(bufB, tile + NW);
-    process(bufA, tile);
-    tile += NW;
-    if (tile >= tile1) break;
-    fetch(bufA, tile + NW);
-    process(bufB, tile);
-    tile += NW;
+  // every copy that was started must land before this CTA may leave (its shared memory is recycled): the streaming loop
+  // consumes the tiles below tile1, the rest is drained here
+  {
+    const int mine = tile0 + warp < tile1 ? (tile1 - tile0 - warp + NW - 1) / NW : 0;  // tiles this warp will stream
+    for (int i = mine; i < issued; ++i) mbar_wait(Cfg::kAbsBar + (warp * kStages + i) * 8, 0u);
   }
+  if (tile0 >= nt) {  // empty cache (the prep kernel wrote out = 0) or a trailing split with nothing to do
+    if (a.chain_mode != 0) pdl_wait();
+    return;
+  }
+  __syncthreads();  // tables
 
-  // ---- reduce over the CTA's warps (lanes already own distinct coordinates)
+  float o[D / 16][4];
+#pragma unroll
+  for (int i = 0; i < D / 16; ++i)
+#pragma unroll
+    for (int j = 0; j < 4; ++j) o[i][j] = 0.f;
+  float m, l;
+  if (fast) stream_tiles<D, true>(stream, tile0 + warp, tile1, T, warp, lane, fr, m, l, o);
+  else stream_tiles<D, false>(stream, tile0 + warp, tile1, T, warp, lane, fr, m, l, o);
+
+  // ---- reduce over the CTA's warps.  o[mt] = {coordinate 16 mt + g: hi, lo; coordinate 16 mt + g + 8: hi, lo}, the same
+  //      in all four lanes of a quad
   l = warp_sum(l);
   float* wr = red + warp * (D + 2);
   if (lane == 0) {
     wr[0] = m;
     wr[1] = l;
   }
+  if ((lane & 3) == 0) {
+    const int g = lane >> 2;
 #pragma unroll
-  for (int i = 0; i < VP; ++i) {
-    float x0, x1;
-    unpack2(add2(o2[2 * i], o2[2 * i + 1]), x0, x1);
-    wr[2 + 2 * (lane + kTile * i)] = x0;
-    wr[2 + 2 * (lane + kTile * i) + 1] = x1;
+    for (int mt = 0; mt < D / 16; ++mt) {
+      wr[2 + 16 * mt + g] = o[mt][0] + o[mt][1];
+      wr[2 + 16 * mt + g + 8] = o[mt][2] + o[mt][3];
+    }
   }
   __syncthreads();
   float M = -INFINITY;
@@ -481,7 +550,10 @@ __global__ void __launch_bounds__(kDecodeThreads, DecodeCfg<D>::kCtasPerSm) deco
       __threadfence();  // acquire side for the CTA that merges
     }
     __syncthreads();
-    if (*flag == 0) return;
+    if (*flag == 0) {
+      if (a.chain_mode != 0) pdl_wait();
+      return;
+    }
     const float* pp = a.partials + (size_t)uc * kMaxSegments * (D + 2);
     M = -INFINITY;
     for (int s = 0; s < nseg; ++s) M = fmaxf(M, __ldcg(pp + s * (D + 2)));
@@ -496,19 +568,33 @@ __global__ void __launch_bounds__(kDecodeThreads, DecodeCfg<D>::kCtasPerSm) deco
       }
     }
   }
-  // ---- out = PI_V^T (o' / l): the k range is split over the 128 / D thread groups
+  // ---- out = PI_V^T (o' / l): the k range is split over the 128 / D thread groups; every load is issued before the
+  //      first multiply (one L2 round trip), four independent chains per thread
   if (tid < D) omerged[tid] = Lsum > 0.f ? oi / Lsum : 0.f;
   __syncthreads();
-  constexpr int PARTS = kBuildThreads / D;  // 2 | 1
-  constexpr int KP = D / PARTS;             // 32 | 128
+  constexpr int PARTS = kDecodeThreads / D;  // 2 | 1
+  constexpr int KP = D / PARTS;              // 32 | 128
   const int i = tid % D, part = (tid / D) % PARTS;
   float r = 0.f;
-  if (tid < kBuildThreads) {
+  {
     const float* Pvp = Pv + (size_t)part * KP * D + i;
-#pragma unroll 32
-    for (int k = 0; k < KP; ++k) r = fmaf(__ldg(Pvp + (size_t)k * D), omerged[part * KP + k], r);
+#pragma unroll
+    for (int k0 = 0; k0 < KP; k0 += 32) {
+      float pv[32];
+#pragma unroll
+      for (int k = 0; k < 32; ++k) pv[k] = __ldg(Pvp + (size_t)(k0 + k) * D);
+      float r0 = 0.f, r1 = 0.f, r2 = 0.f, r3 = 0.f;
+#pragma unroll
+      for (int k = 0; k < 32; k += 4) {
+        r0 = fmaf(pv[k], omerged[part * KP + k0 + k], r0);
+        r1 = fmaf(pv[k + 1], omerged[part * KP + k0 + k + 1], r1);
+        r2 = fmaf(pv[k + 2], omerged[part * KP + k0 + k + 2], r2);
+        r3 = fmaf(pv[k + 3], omerged[part * KP + k0 + k + 3], r3);
+      }
+      r += (r0 + r1) + (r2 + r3);
+    }
   }
-  if (PARTS > 1 && tid < kBuildThreads && part > 0) omerged[part * D + i] = r;
+  if (PARTS > 1 && part > 0) omerged[part * D + i] = r;
   __syncthreads();
   if (tid < D) {
 #pragma unroll
@@ -517,19 +603,16 @@ __global__ void __launch_bounds__(kDecodeThreads, DecodeCfg<D>::kCtasPerSm) deco
     if constexpr (sizeof(TIO) == 2) outp[i] = __float2half_rn(r);
     else outp[i] = r;
   }
+  if (a.chain_mode != 0) pdl_wait();  // complete in launch order (see DecodeArgs::chain_mode)
 }
 
 // ------------------------------------------------------------------------------------------ launchers
 template <int D, typename T>
 static cudaError_t launch_decode_t(const DecodeArgs& a, cudaStream_t st) {
-  cudaError_t e;
   constexpr int smem = DecodeCfg<D>::kSmemBytes;
-  static bool attr_set = false;
-  if (!attr_set) {
-    e = cudaFuncSetAttribute(decode_main_kernel<D, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    if (e != cudaSuccess) return e;
-    attr_set = true;
-  }
+  // per launch: the attribute is per device and a process may drive several
+  cudaError_t e = cudaFuncSetAttribute(decode_main_kernel<D, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+  if (e != cudaSuccess) return e;
   const int units = a.n_layers_call * a.cv.B * a.cv.H;
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3(units * a.nsplit);
@@ -540,7 +623,7 @@ static cudaError_t launch_decode_t(const DecodeArgs& a, cudaStream_t st) {
   attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
-  cfg.numAttrs = a.nsplit == 1 ? 1 : 0;  // measured: early scheduling helps one-CTA-per-unit launches, hurts split ones
+  cfg.numAttrs = 1;
   e = cudaLaunchKernelEx(&cfg, decode_main_kernel<D, T>, a);
   count_launch();
   return e != cudaSuccess ? e : cudaGetLastError();

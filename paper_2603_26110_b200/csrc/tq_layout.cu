@@ -1,172 +1,142 @@
 // tq_layout.cu — conversion between the device tile layout and the canonical packed planes
 // (include/tq.h "Canonical packed format" / "Device cache format").  Byte shuffling only; not hot.
+// Both directions go through the position functions of tq_common.cuh (k_field_pos, sign_bit_pos, v_code_pos).
 #include "tq_common.cuh"
 
 namespace tq {
 
-// read/write a 6-bit field at position k of a little-endian word string
-__device__ __forceinline__ unsigned get_bits(const unsigned* words, int bitpos, int nbits) {
-  int w = bitpos >> 5, s = bitpos & 31;
-  unsigned long long v = words[w];
-  if (s + nbits > 32) v |= (unsigned long long)words[w + 1] << 32;
-  return (unsigned)((v >> s) & ((1u << nbits) - 1u));
+// bits [bit, bit + n) of lane l's word string in a section of W words per lane
+__device__ __forceinline__ unsigned sec_get(const unsigned char* sec, int W, int l, int bit, int n) {
+  const int w = bit >> 5, s = bit & 31;
+  unsigned long long v = *(const unsigned*)(sec + word_offset(W, w, l));
+  if (s + n > 32) v |= (unsigned long long)*(const unsigned*)(sec + word_offset(W, w + 1, l)) << 32;
+  return (unsigned)((v >> s) & ((1u << n) - 1u));
 }
-__device__ __forceinline__ void or_bits(unsigned* words, int bitpos, int nbits, unsigned val) {
-  int w = bitpos >> 5, s = bitpos & 31;
-  unsigned long long v = (unsigned long long)val << s;
+__device__ __forceinline__ void or_bits(unsigned* words, int bit, int n, unsigned val) {
+  const int w = bit >> 5, s = bit & 31;
+  const unsigned long long v = (unsigned long long)val << s;
   words[w] |= (unsigned)v;
-  if (s + nbits > 32) words[w + 1] |= (unsigned)(v >> 32);
+  if (s + n > 32) words[w + 1] |= (unsigned)(v >> 32);
+}
+// n bits at position `bit` of a canonical LSB-first byte stream
+__device__ __forceinline__ unsigned stream_get(const unsigned char* p, int bit, int n) {
+  unsigned v = 0;
+  for (int k = 0; k < n; ++k) v |= ((p[(bit + k) >> 3] >> ((bit + k) & 7)) & 1u) << k;
+  return v;
 }
 
-template <int D>
-__device__ void load_section(const unsigned char* sec, int W, int slot, unsigned* words) {
-  for (int w = 0; w < W; ++w) words[w] = *(const unsigned*)(sec + word_offset(W, w, slot));
-}
-template <int D>
-__device__ void store_section(unsigned char* sec, int W, int slot, const unsigned* words) {
-  for (int w = 0; w < W; ++w) *(unsigned*)(sec + word_offset(W, w, slot)) = words[w];
-}
-
+// one thread per (b, h, token): gathers its bits from the lanes that hold them
 template <int D>
 __global__ void export_kernel(CacheView cv, int layer, int n_tokens, tq_canonical out) {
   using Lo = Layout<D>;
-  long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
-  long total = (long)cv.B * cv.H * n_tokens;
+  const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  const long total = (long)cv.B * cv.H * n_tokens;
   if (idx >= total) return;
-  int t = (int)(idx % n_tokens);
-  long bh = idx / n_tokens;  // b*H + h
-  size_t unit = (size_t)layer * cv.B * cv.H + bh;
+  const int t = (int)(idx % n_tokens);
+  const long bh = idx / n_tokens;  // b*H + h
+  const size_t unit = (size_t)layer * cv.B * cv.H + bh;
   const unsigned char* tile = cv.tiles + unit * cv.stream_bytes + (size_t)(t / kTile) * Lo::kTileBytes;
-  int slot = t % kTile;
-  unsigned words[Lo::KCW + 1];
-  unsigned char codes[D];
-  // K codes: pair group g sits at field position (g - slot) mod P
-  load_section<D>(tile + Lo::kOffKC, Lo::KCW, slot, words);
-  words[Lo::KCW] = 0;
-  for (int g = 0; g < Lo::P; ++g) {
-    int k = (g - slot + 4 * Lo::P) % Lo::P;
-    unsigned f = get_bits(words, 6 * k, 6);
-    codes[2 * g] = f & 7;
-    codes[2 * g + 1] = f >> 3;
-  }
+  const int slot = t % kTile;
   unsigned char* kc = out.k_codes + (size_t)idx * (3 * D / 8);
-  for (int grp = 0; grp < D / 8; ++grp) {
-    unsigned p = 0;
-    for (int i = 0; i < 8; ++i) p |= (unsigned)codes[8 * grp + i] << (3 * i);
-    kc[3 * grp] = p & 0xff;
-    kc[3 * grp + 1] = (p >> 8) & 0xff;
-    kc[3 * grp + 2] = (p >> 16) & 0xff;
-  }
-  // K signs: nibble group n sits at nibble position (n - slot) mod NG
-  load_section<D>(tile + Lo::kOffKS, Lo::KSW, slot, words);
+  unsigned char* vc = out.v_codes + (size_t)idx * (3 * D / 8);
   unsigned char* ks = out.k_signs + (size_t)idx * (D / 8);
+  for (int grp = 0; grp < D / 8; ++grp) {  // 8 codes = 4 pair fields = 3 canonical bytes
+    unsigned pk = 0, pv = 0;
+    for (int q = 0; q < 4; ++q) {
+      const BitPos kp = k_field_pos<D>(slot, 4 * grp + q);
+      pk |= sec_get(tile + Lo::kOffKC, Lo::KCW, kp.lane, kp.bit, 6) << (6 * q);
+    }
+    for (int i = 0; i < 8; ++i) {
+      const BitPos vp = v_code_pos<D>(slot, 8 * grp + i);
+      pv |= sec_get(tile + Lo::kOffVC, Lo::KCW, vp.lane, vp.bit, 3) << (3 * i);
+    }
+    kc[3 * grp] = pk & 0xff, kc[3 * grp + 1] = (pk >> 8) & 0xff, kc[3 * grp + 2] = (pk >> 16) & 0xff;
+    vc[3 * grp] = pv & 0xff, vc[3 * grp + 1] = (pv >> 8) & 0xff, vc[3 * grp + 2] = (pv >> 16) & 0xff;
+  }
   for (int byte = 0; byte < D / 8; ++byte) {
     unsigned v = 0;
-    for (int half = 0; half < 2; ++half) {
-      int n = 2 * byte + half;
-      int k = (n - slot + 4 * Lo::NG) % Lo::NG;
-      v |= get_bits(words, 4 * k, 4) << (4 * half);
+    for (int k = 0; k < 8; ++k) {
+      const BitPos sp = sign_bit_pos<D>(slot, 8 * byte + k);
+      v |= sec_get(tile + Lo::kOffKS, Lo::KSW, sp.lane, sp.bit, 1) << k;
     }
     ks[byte] = (unsigned char)v;
   }
-  // V codes: lane g of the tile owns pair groups g (+32 for d = 128); token slot j sits at bits [6j, 6j+6)
-  for (int g = 0; g < Lo::P; ++g) {
-    const int lane = g % kTile, part = g / kTile;
-    const int bit = 192 * part + 6 * slot;
-    const unsigned char* sec = tile + Lo::kOffVC;
-    unsigned w0 = *(const unsigned*)(sec + word_offset(Lo::KCW, bit >> 5, lane));
-    unsigned w1 = ((bit & 31) > 26) ? *(const unsigned*)(sec + word_offset(Lo::KCW, (bit >> 5) + 1, lane)) : 0u;
-    unsigned long long v = w0 | ((unsigned long long)w1 << 32);
-    unsigned f = (unsigned)(v >> (bit & 31)) & 63u;
-    codes[2 * g] = f & 7;
-    codes[2 * g + 1] = f >> 3;
-  }
-  unsigned char* vc = out.v_codes + (size_t)idx * (3 * D / 8);
-  for (int grp = 0; grp < D / 8; ++grp) {
-    unsigned p = 0;
-    for (int i = 0; i < 8; ++i) p |= (unsigned)codes[8 * grp + i] << (3 * i);
-    vc[3 * grp] = p & 0xff;
-    vc[3 * grp + 1] = (p >> 8) & 0xff;
-    vc[3 * grp + 2] = (p >> 16) & 0xff;
-  }
-  out.k_norm[idx] = ((const unsigned short*)(tile + Lo::kOffKN))[slot];
-  out.k_rnorm[idx] = ((const unsigned short*)(tile + Lo::kOffKR))[slot];
-  out.v_norm[idx] = ((const unsigned short*)(tile + Lo::kOffVN))[slot];
+  const int nl = slot_lane(slot);
+  const unsigned nk = ((const unsigned*)(tile + Lo::kOffNK))[nl];
+  out.k_norm[idx] = (unsigned short)(nk & 0xffffu);
+  out.k_rnorm[idx] = (unsigned short)(nk >> 16);
+  out.v_norm[idx] = ((const unsigned short*)(tile + Lo::kOffVN))[nl];
 }
 
+// one thread per (b, h, tile, lane): assembles that lane's word strings from the canonical planes; the bits of
+// tokens at or beyond n_tokens keep whatever the tile held
 template <int D>
 __global__ void import_kernel(CacheView cv, int layer, int n_tokens, tq_canonical in) {
   using Lo = Layout<D>;
-  long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
-  long total = (long)cv.B * cv.H * n_tokens;
+  const int ntile = (n_tokens + kTile - 1) / kTile;
+  const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  const long total = (long)cv.B * cv.H * ntile * kTile;
   if (idx == 0)
     for (int b = 0; b < cv.B; ++b) cv.seq_len[layer * cv.B + b] = n_tokens;
   if (idx >= total) return;
-  int t = (int)(idx % n_tokens);
-  long bh = idx / n_tokens;
-  size_t unit = (size_t)layer * cv.B * cv.H + bh;
-  unsigned char* tile = cv.tiles + unit * cv.stream_bytes + (size_t)(t / kTile) * Lo::kTileBytes;
-  int slot = t % kTile;
-  unsigned words[Lo::KCW + 1];
-  unsigned char codes[D];
-  const unsigned char* kc = in.k_codes + (size_t)idx * (3 * D / 8);
-  for (int grp = 0; grp < D / 8; ++grp) {
-    unsigned p = kc[3 * grp] | ((unsigned)kc[3 * grp + 1] << 8) | ((unsigned)kc[3 * grp + 2] << 16);
-    for (int i = 0; i < 8; ++i) codes[8 * grp + i] = (p >> (3 * i)) & 7;
-  }
-  for (int w = 0; w <= Lo::KCW; ++w) words[w] = 0;
-  for (int g = 0; g < Lo::P; ++g) {
-    int k = (g - slot + 4 * Lo::P) % Lo::P;
-    or_bits(words, 6 * k, 6, codes[2 * g] | ((unsigned)codes[2 * g + 1] << 3));
-  }
-  store_section<D>(tile + Lo::kOffKC, Lo::KCW, slot, words);
-  const unsigned char* ks = in.k_signs + (size_t)idx * (D / 8);
-  for (int w = 0; w <= Lo::KSW; ++w) words[w] = 0;
-  for (int n = 0; n < Lo::NG; ++n) {
-    unsigned nib = (ks[n >> 1] >> (4 * (n & 1))) & 0xf;
-    int k = (n - slot + 4 * Lo::NG) % Lo::NG;
-    or_bits(words, 4 * k, 4, nib);
-  }
-  store_section<D>(tile + Lo::kOffKS, Lo::KSW, slot, words);
-  // V code words are shared by the 32 tokens of a tile: import_v_kernel (second pass) writes them.
-  ((unsigned short*)(tile + Lo::kOffKN))[slot] = in.k_norm[idx];
-  ((unsigned short*)(tile + Lo::kOffKR))[slot] = in.k_rnorm[idx];
-  ((unsigned short*)(tile + Lo::kOffVN))[slot] = in.v_norm[idx];
-}
-
-// V code words of one tile hold all 32 tokens: one thread per (b, h, tile, lane) assembles its words from the
-// canonical planes (tokens beyond n_tokens keep whatever the tile held).
-template <int D>
-__global__ void import_v_kernel(CacheView cv, int layer, int n_tokens, tq_canonical in) {
-  using Lo = Layout<D>;
-  const int ntile = (n_tokens + kTile - 1) / kTile;
-  long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
-  long total = (long)cv.B * cv.H * ntile * kTile;
-  if (idx >= total) return;
-  const int lane = (int)(idx % kTile);
+  const int lane = (int)(idx % kTile), g = lane >> 2, t = lane & 3;
   const int tl = (int)((idx / kTile) % ntile);
   const long bh = idx / ((long)kTile * ntile);
-  size_t unit = (size_t)layer * cv.B * cv.H + bh;
-  unsigned char* sec = cv.tiles + unit * cv.stream_bytes + (size_t)tl * Lo::kTileBytes + Lo::kOffVC;
-  unsigned words[Lo::KCW + 1];
-  unsigned keep[Lo::KCW + 1];
+  const size_t unit = (size_t)layer * cv.B * cv.H + bh;
+  unsigned char* tile = cv.tiles + unit * cv.stream_bytes + (size_t)tl * Lo::kTileBytes;
+  const size_t tok0 = (size_t)bh * n_tokens + (size_t)tl * kTile;  // canonical index of the tile's slot 0
+  auto in_call = [&](int s) { return tl * kTile + s < n_tokens; };
+  unsigned words[Lo::KCW + 1], keep[Lo::KCW + 1];
+  auto flush = [&](unsigned char* sec, int W) {
+    for (int w = 0; w < W; ++w) {
+      unsigned* p = (unsigned*)(sec + word_offset(W, w, lane));
+      *p = (*p & ~keep[w]) | words[w];
+    }
+  };
+  // K codes: slots g + 8 r, pairs t + 4 j
   for (int w = 0; w <= Lo::KCW; ++w) words[w] = 0, keep[w] = 0;
-  for (int part = 0; part < Lo::P / kTile; ++part) {
-    const int g = lane + kTile * part;
-    for (int j = 0; j < kTile; ++j) {
-      const int t = tl * kTile + j;
-      if (t >= n_tokens) continue;
-      const unsigned char* vc = in.v_codes + ((size_t)bh * n_tokens + t) * (3 * D / 8);
-      const int cbit = 6 * g;  // codes 2g, 2g+1 are 6 consecutive bits of the canonical stream
-      unsigned v = vc[cbit >> 3] | ((unsigned)vc[(cbit >> 3) + 1 < 3 * D / 8 ? (cbit >> 3) + 1 : (cbit >> 3)] << 8);
-      unsigned f = (v >> (cbit & 7)) & 63u;
-      or_bits(words, 192 * part + 6 * j, 6, f);
-      or_bits(keep, 192 * part + 6 * j, 6, 63u);
+  for (int r = 0; r < 4; ++r) {
+    const int s = g + 8 * r;
+    if (!in_call(s)) continue;
+    const unsigned char* kc = in.k_codes + (tok0 + s) * (3 * D / 8);
+    for (int j = 0; j < Lo::J; ++j) {
+      const int p = t + 4 * j;
+      or_bits(words, k_field_pos<D>(s, p).bit, 6, stream_get(kc, 6 * p, 6));
+      or_bits(keep, k_field_pos<D>(s, p).bit, 6, 63u);
     }
   }
-  for (int w = 0; w < Lo::KCW; ++w) {
-    unsigned* p = (unsigned*)(sec + word_offset(Lo::KCW, w, lane));
-    *p = (*p & ~keep[w]) | words[w];
+  flush(tile + Lo::kOffKC, Lo::KCW);
+  // K signs: slots g + 8 r, sketch rows [t d/4, (t + 1) d/4)
+  for (int w = 0; w <= Lo::KCW; ++w) words[w] = 0, keep[w] = 0;
+  for (int r = 0; r < 4; ++r) {
+    const int s = g + 8 * r;
+    if (!in_call(s)) continue;
+    const unsigned char* ks = in.k_signs + (tok0 + s) * (D / 8);
+    for (int i = 0; i < D / 4; ++i) {
+      const int rho = t * (D / 4) + i;
+      or_bits(words, sign_bit_pos<D>(s, rho).bit, 1, stream_get(ks, rho, 1));
+      or_bits(keep, sign_bit_pos<D>(s, rho).bit, 1, 1u);
+    }
+  }
+  flush(tile + Lo::kOffKS, Lo::KSW);
+  // V codes: token pairs t + 4 j, coordinates g + 8 c
+  for (int w = 0; w <= Lo::KCW; ++w) words[w] = 0, keep[w] = 0;
+  for (int j = 0; j < 4; ++j)
+    for (int e = 0; e < 2; ++e) {
+      const int s = 2 * (t + 4 * j) + e;
+      if (!in_call(s)) continue;
+      const unsigned char* vc = in.v_codes + (tok0 + s) * (3 * D / 8);
+      for (int c = 0; c < Lo::C; ++c) {
+        const int i = g + 8 * c;
+        or_bits(words, v_code_pos<D>(s, i).bit, 3, stream_get(vc, 3 * i, 3));
+        or_bits(keep, v_code_pos<D>(s, i).bit, 3, 7u);
+      }
+    }
+  flush(tile + Lo::kOffVC, Lo::KCW);
+  const int s = lane_slot(lane);
+  if (in_call(s)) {
+    ((unsigned*)(tile + Lo::kOffNK))[lane] = (unsigned)in.k_norm[tok0 + s] | ((unsigned)in.k_rnorm[tok0 + s] << 16);
+    ((unsigned short*)(tile + Lo::kOffVN))[lane] = in.v_norm[tok0 + s];
   }
 }
 
@@ -185,7 +155,7 @@ cudaError_t launch_export(const CacheGeom& g, const CacheView& cv, int layer, in
 
 cudaError_t launch_import(const CacheGeom& g, const CacheView& cv, int layer, int n_tokens, const tq_canonical& in,
                           cudaStream_t st) {
-  long total = (long)g.B * g.H * n_tokens;
+  long total = (long)g.B * g.H * ((n_tokens + kTile - 1) / kTile) * kTile;
   int blocks = (int)((total + 127) / 128);
   if (blocks == 0) blocks = 1;
   if (g.D == 64)
@@ -193,15 +163,6 @@ cudaError_t launch_import(const CacheGeom& g, const CacheView& cv, int layer, in
   else
     import_kernel<128><<<blocks, 128, 0, st>>>(cv, layer, n_tokens, in);
   count_launch();
-  if (total > 0) {
-    long vt = (long)g.B * g.H * ((n_tokens + kTile - 1) / kTile) * kTile;
-    int vb = (int)((vt + 127) / 128);
-    if (g.D == 64)
-      import_v_kernel<64><<<vb, 128, 0, st>>>(cv, layer, n_tokens, in);
-    else
-      import_v_kernel<128><<<vb, 128, 0, st>>>(cv, layer, n_tokens, in);
-    count_launch();
-  }
   return cudaGetLastError();
 }
 

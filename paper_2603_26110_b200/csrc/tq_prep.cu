@@ -31,7 +31,8 @@ struct PrepArgs {
   const void *q, *k, *v;                                    // [Lc][B][H][D] each (k, v: append; q: query)
   void* out;                                                // [Lc][B][H][D] (zeroed here for empty caches)
   const int32_t* q_pos;                                     // [Lc][B] or nullptr
-  float* qrot;                                              // workspace [units][2 D]
+  unsigned* frags;                                          // workspace [units][FragLayout<D>::kWords]
+  unsigned* tabs;                                           // workspace [layers_call * H][kTabWords]
   int layer_begin, rope_layout;
 };
 
@@ -82,6 +83,8 @@ __global__ void __launch_bounds__((kAppend ? 3 : 2) * PrepCfg<D>::GT) prep_kerne
   __shared__ unsigned char cK[BG][D], cV[BG][D], bitb[BG][D];
   __shared__ float redk[BG][WG], redv[BG][WG], redr[BG][WG];
   __shared__ float lutK[8], lutV[8];
+  __shared__ __align__(16) float zs[BG][D];  // z of the queries (unscaled)
+  __shared__ float fscal[BG][4];             // per entry: 2^eq kScaleK, 2^ez kScaleS (fragment scalings)
   __shared__ int s_len0[BG], s_full[BG];
 
   const int tid = threadIdx.x, lane = tid & 31;
@@ -118,8 +121,12 @@ __global__ void __launch_bounds__((kAppend ? 3 : 2) * PrepCfg<D>::GT) prep_kerne
     const float* M = grp == 0 ? a.pi_k + lh * D * D : grp == 1 ? a.S : a.pi_v + lh * D * D;
     rowreg.load(M + (size_t)row * D + part * 64);
   }
-  // ---- stage-4 work item of this thread (one word of one token), and an early read of the V word it will modify
-  constexpr int ITEMS = Lo::KCW + Lo::KSW + Lo::P + 1;
+  // ---- stage-4 work item of this thread (one 16-bit or 8-bit piece of one token in the device tile layout,
+  //      tq_common.cuh), and an early read of the V halfword it will modify (a V field is shared with the other token
+  //      of the pair, which was appended by an earlier call)
+  constexpr int HW = 3 * D / 64;  // halfwords per (lane, token) block of K fields, and per (lane, token pair) block of V fields
+  constexpr int IT_K = 4 * HW, IT_S = 4 * Lo::U * 2, IT_V = 8 * HW;
+  constexpr int ITEMS = IT_K + IT_S + IT_V + 1;
   static_assert(!kAppend || BG * ITEMS <= NT, "one output item per thread");
   const int it_e = tid / ITEMS, it = tid % ITEMS;
   int it_len = len_e[0];
@@ -129,17 +136,13 @@ __global__ void __launch_bounds__((kAppend ? 3 : 2) * PrepCfg<D>::GT) prep_kerne
   unsigned char* it_tp = a.cv.tiles + (((size_t)layer * B + b0 + min(it_e, nb - 1)) * H + h) * a.cv.stream_bytes +
                          (size_t)(min(it_len, a.cv.max_seq - 1) / kTile) * Lo::kTileBytes;
   const int it_slot = it_len % kTile;
-  unsigned vold0 = 0, vold1 = 0;
-  unsigned *vp0 = nullptr, *vp1 = nullptr;
-  if (it_on && it >= Lo::KCW + Lo::KSW && it < Lo::KCW + Lo::KSW + Lo::P) {
-    const int g = it - Lo::KCW - Lo::KSW, vl = g % kTile, vp = g / kTile;
-    const int bit = 192 * vp + 6 * it_slot;
-    vp0 = reinterpret_cast<unsigned*>(it_tp + Lo::kOffVC + word_offset(Lo::KCW, bit >> 5, vl));
-    vold0 = __ldcg(vp0);
-    if ((bit & 31) > 26) {
-      vp1 = reinterpret_cast<unsigned*>(it_tp + Lo::kOffVC + word_offset(Lo::KCW, (bit >> 5) + 1, vl));
-      vold1 = __ldcg(vp1);
-    }
+  unsigned short vold = 0;
+  unsigned short* vptr = nullptr;
+  if (it_on && it >= IT_K + IT_S && it < IT_K + IT_S + IT_V) {
+    const int vi = it - IT_K - IT_S, gi = vi / HW, hw = vi % HW, pp = it_slot >> 1;
+    const int hidx = (pp >> 2) * HW + hw;  // halfword of lane (gi, pp & 3)'s V string
+    vptr = reinterpret_cast<unsigned short*>(it_tp + Lo::kOffVC + word_offset(Lo::KCW, hidx >> 1, 4 * gi + (pp & 3))) + (hidx & 1);
+    vold = __ldcg(vptr);
   }
   if (tid < 8) lutK[tid] = a.lut_k[lh * 8 + tid];
   if (tid >= 32 && tid < 40) lutV[tid - 32] = a.lut_v[lh * 8 + tid - 32];
@@ -217,7 +220,6 @@ __global__ void __launch_bounds__((kAppend ? 3 : 2) * PrepCfg<D>::GT) prep_kerne
       }
       if (kQuery && part == 0) {
         yq[e][row] = aq[e];
-        if (e < nb) a.qrot[(((size_t)lc * B + b0 + e) * H + h) * 2 * D + row] = aq[e] * kScaleK;
       }
     }
   } else if (kAppend && grp == 2) {
@@ -285,52 +287,125 @@ __global__ void __launch_bounds__((kAppend ? 3 : 2) * PrepCfg<D>::GT) prep_kerne
       }
       if (part == 0) {
         if (kAppend) bitb[e][row] = sr[e] >= 0.f ? 1 : 0;
-        if (kQuery && e < nb) a.qrot[(((size_t)lc * B + b0 + e) * H + h) * 2 * D + D + row] = zq[e] * kScaleS;
+        if (kQuery) zs[e][row] = zq[e];
+      }
+    }
+  }
+  __syncthreads();
+  if (kQuery) {
+    // ---- the decode kernel's operands (tq_common.cuh FragLayout): power-of-two scalings that put max |q''_s|, max |z_s|
+    //      in [2^13, 2^14), fp16 hi + lo splits in B-fragment order; and the head's dequantisation tables
+    using FL = FragLayout<D>;
+    const int warp_id = tid >> 5;
+    if (warp_id < BG) {  // one warp per entry: maxima and the sum of z
+      const int e = warp_id;
+      float qm = 0.f, zm = 0.f, zsum = 0.f;
+#pragma unroll
+      for (int i = lane; i < D; i += 32) {
+        qm = fmaxf(qm, fabsf(yq[e][i] * kScaleK));
+        const float zv = zs[e][i] * kScaleS;
+        zm = fmaxf(zm, fabsf(zv));
+        zsum += zv;
+      }
+      qm = warp_max(qm), zm = warp_max(zm), zsum = warp_sum(zsum);
+      auto expo = [](float x) {
+        const int E = (int)((__float_as_uint(x) >> 23) & 0xffu);
+        return (E == 0 || E == 255) ? 0 : E - 127;
+      };
+      auto p2 = [](int ee) { return __uint_as_float((unsigned)(max(-100, min(100, ee)) + 127) << 23); };
+      const int eq = 13 - expo(qm), ez = 13 - expo(zm);
+      if (lane == 0) {
+        fscal[e][0] = p2(eq) * kScaleK;
+        fscal[e][1] = p2(ez) * kScaleS;
+        if (e < nb) {
+          float* sc = reinterpret_cast<float*>(a.frags + (((size_t)lc * B + b0 + e) * H + h) * FL::kWords + FL::kScalOff);
+          sc[0] = p2(-eq), sc[1] = p2(25 - ez), sc[2] = zsum, sc[3] = 0.f;
+        }
+      }
+    }
+    __syncthreads();
+    auto split2 = [](float x0, float x1, bool lo) {
+      const __half h0 = __float2half_rn(x0), h1 = __float2half_rn(x1);
+      const __half l0 = __float2half_rn(x0 - __half2float(h0)), l1 = __float2half_rn(x1 - __half2float(h1));
+      return lo ? ((unsigned)__half_as_ushort(l0) | ((unsigned)__half_as_ushort(l1) << 16))
+                : ((unsigned)__half_as_ushort(h0) | ((unsigned)__half_as_ushort(h1) << 16));
+    };
+    for (int idx = tid; idx < BG * FL::kScalOff; idx += NT) {
+      const int e = idx / FL::kScalOff, wi = idx % FL::kScalOff;
+      if (e >= nb) continue;
+      const int pat = wi / FL::kWordsPerPat, wd = wi % FL::kWordsPerPat, t = pat & 3;
+      const bool lo = pat >> 2;
+      unsigned word;
+      if (wd < 2 * FL::KS) {
+        const int c0 = 16 * (wd >> 1) + 2 * t + 8 * (wd & 1);
+        word = split2(yq[e][c0] * fscal[e][0], yq[e][c0 + 1] * fscal[e][0], lo);
+      } else {
+        const int ks = (wd - 2 * FL::KS) >> 1, reg = wd & 1, p0 = 2 * (ks & 3);
+        const int rho = t * (D / 4) + 16 * (ks >> 2) + p0 + reg;
+        const float sc = fscal[e][1] * __uint_as_float((unsigned)(127 - p0 - reg) << 23);
+        word = split2(zs[e][rho] * sc, zs[e][rho + 8] * sc, lo);
+      }
+      a.frags[(((size_t)lc * B + b0 + e) * H + h) * FL::kWords + wi] = word;
+    }
+    if (tid < 64) {  // every batch group of the head writes the same values
+      const int c0 = tid & 7, c1 = tid >> 3;
+      unsigned* tb = a.tabs + (size_t)lh_c * kTabWords;
+      tb[tid] = split2(lutK[c0], lutK[c1], false);
+      tb[64 + tid] = split2(lutK[c0], lutK[c1], true);
+      tb[128 + tid] = split2(lutV[c0], lutV[c1], false);
+      tb[192 + tid] = split2(lutV[c0], lutV[c1], true);
+      if (tid == 0) {
+        bool exact = true;
+#pragma unroll
+        for (int i = 0; i < 8; ++i)
+          exact = exact && __half2float(__float2half_rn(lutK[i])) == lutK[i] && __half2float(__float2half_rn(lutV[i])) == lutV[i];
+        tb[256] = exact ? 1u : 0u;
       }
     }
   }
   if (!kAppend) return;
-  __syncthreads();
 
-  // ---- stage 4 (append): every thread assembles one word of one token in the device layout (include/tq.h)
+  // ---- stage 4 (append): every thread assembles one piece of one token in the device tile layout
   if (it_on) {
-    const int e = it_e, slot = it_slot;
+    const int e = it_e, slot = it_slot, g = slot & 7, r = slot >> 3;
     unsigned char* tp = it_tp;
-    if (it < Lo::KCW) {
-      const int w = it;
-      unsigned long long word = 0;
-      const int k_lo = (32 * w) / 6, k_hi = (32 * w + 31) / 6;
-      for (int kf = k_lo; kf <= k_hi; ++kf) {
-        const int g = (kf + slot) % Lo::P;
-        unsigned long long f = cK[e][2 * g] | ((unsigned)cK[e][2 * g + 1] << 3);
-        const int sh = 6 * kf - 32 * w;  // negative for the field straddling in from the previous word
-        word |= sh >= 0 ? (f << sh) : (f >> (-sh));
+    // bits [16 hw, 16 hw + 16) of a string of NB-bit pieces at stride 6 bits: piece k = val(k) at bit 6 k + off
+    auto gather16 = [&](int hw, int nfields, int off, int nb_, auto val, unsigned& out, unsigned& mask) {
+      out = 0, mask = 0;
+      for (int k = 0; k < nfields; ++k) {
+        const int sh = 6 * k + off - 16 * hw;
+        if (sh <= -nb_ || sh >= 16) continue;
+        const unsigned v = val(k), mk = (1u << nb_) - 1u;
+        out |= sh >= 0 ? (v << sh) : (v >> (-sh));
+        mask |= sh >= 0 ? (mk << sh) : (mk >> (-sh));
       }
-      *reinterpret_cast<unsigned*>(tp + Lo::kOffKC + word_offset(Lo::KCW, w, slot)) = (unsigned)word;
-    } else if (it < Lo::KCW + Lo::KSW) {
-      const int w = it - Lo::KCW;
-      unsigned word = 0;
-      for (int kn = 0; kn < 8; ++kn) {
-        const int ng = (8 * w + kn + slot) % Lo::NG;
-        const unsigned char* bb = &bitb[e][4 * ng];
-        word |= (unsigned)(bb[0] | (bb[1] << 1) | (bb[2] << 2) | (bb[3] << 3)) << (4 * kn);
-      }
-      *reinterpret_cast<unsigned*>(tp + Lo::kOffKS + word_offset(Lo::KSW, w, slot)) = word;
-    } else if (it < Lo::KCW + Lo::KSW + Lo::P) {
-      // V: pair group g lives in lane (g mod 32)'s string at bits [192 part + 6 slot, +6): modify the word read at
-      // the top (nobody else writes this token slot's bits, and the other slots' bits are not written by this launch)
-      const int g = it - Lo::KCW - Lo::KSW;
-      const unsigned f = cV[e][2 * g] | ((unsigned)cV[e][2 * g + 1] << 3);
-      const int s = (192 * (g / kTile) + 6 * slot) & 31;
-      *vp0 = (vold0 & ~(63u << s)) | (f << s);
-      if (s > 26) *vp1 = (vold1 & ~(63u >> (32 - s))) | (f >> (32 - s));
+      out &= 0xffffu, mask &= 0xffffu;
+    };
+    if (it < IT_K) {  // K pair fields of lane (g, t): pairs t + 4 j, block r of the lane's string
+      const int t = it / HW, hw = it % HW;
+      unsigned v, mk;
+      gather16(hw, Lo::J, 0, 6, [&](int j) { const int p = t + 4 * j; return (unsigned)(cK[e][2 * p] | (cK[e][2 * p + 1] << 3)); }, v, mk);
+      const int hidx = r * HW + hw;
+      reinterpret_cast<unsigned short*>(tp + Lo::kOffKC + word_offset(Lo::KCW, hidx >> 1, 4 * g + t))[hidx & 1] = (unsigned short)v;
+    } else if (it < IT_K + IT_S) {  // sign bytes: lane (g, t), piece u, byte half hb
+      const int si = it - IT_K, t = si / (2 * Lo::U), u = (si / 2) % Lo::U, hb = si & 1;
+      unsigned v = 0;
+      for (int k = 0; k < 8; ++k) v |= (unsigned)bitb[e][t * (D / 4) + 16 * u + 8 * hb + k] << k;
+      const int word = (slot >> 4) * Lo::U + u, byte = 2 * hb + (r & 1);
+      *(tp + Lo::kOffKS + word_offset(Lo::KSW, word, 4 * g + t) + byte) = (unsigned char)v;
+    } else if (it < IT_K + IT_S + IT_V) {  // V codes: lane (gi, pp & 3), three-bit slices at 6 c + 3 (slot & 1)
+      const int vi = it - IT_K - IT_S, gi = vi / HW, hw = vi % HW;
+      unsigned v, mk;
+      gather16(hw, Lo::C, 3 * (slot & 1), 3, [&](int c) { return (unsigned)cV[e][gi + 8 * c]; }, v, mk);
+      *vptr = (unsigned short)((vold & ~mk) | v);
     } else {
       float nk = 0.f, nr = 0.f, nv = 0.f;
 #pragma unroll
       for (int w = 0; w < WG; ++w) nk += redk[e][w], nr += redr[e][w], nv += redv[e][w];
-      reinterpret_cast<unsigned short*>(tp + Lo::kOffKN)[slot] = f32_to_f16_bits_clamped(sqrtf(nk));
-      reinterpret_cast<unsigned short*>(tp + Lo::kOffKR)[slot] = f32_to_f16_bits_clamped(sqrtf(nr));
-      reinterpret_cast<unsigned short*>(tp + Lo::kOffVN)[slot] = f32_to_f16_bits_clamped(sqrtf(nv));
+      const int nl = slot_lane(slot);
+      reinterpret_cast<unsigned*>(tp + Lo::kOffNK)[nl] =
+          (unsigned)f32_to_f16_bits_clamped(sqrtf(nk)) | ((unsigned)f32_to_f16_bits_clamped(sqrtf(nr)) << 16);
+      reinterpret_cast<unsigned short*>(tp + Lo::kOffVN)[nl] = f32_to_f16_bits_clamped(sqrtf(nv));
     }
   }
   // ---- arrival: the last head of a batch entry publishes the new length
@@ -354,13 +429,11 @@ static cudaError_t launch_prep_t(const PrepArgs& a, int lh_count, int B, bool do
   const int nbg = (B + Cfg::BG - 1) / Cfg::BG;
   const int grid = lh_count * nbg;
   const size_t sm3 = D == 64 ? (size_t)3 * D * 68 * 4 : 0, sm2 = D == 64 ? (size_t)2 * D * 68 * 4 : 0;
-  static bool attr_set = false;
-  if (!attr_set && D == 64) {
+  if (D == 64) {  // per launch: the attribute is per device and a process may drive several
     cudaError_t e1 = cudaFuncSetAttribute(prep_kernel<D, T, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm3);
     cudaError_t e2 = cudaFuncSetAttribute(prep_kernel<D, T, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm3);
     if (e1 != cudaSuccess) return e1;
     if (e2 != cudaSuccess) return e2;
-    attr_set = true;
   }
   if (do_append && do_query) prep_kernel<D, T, true, true><<<grid, 3 * Cfg::GT, sm3, st>>>(a, nbg);
   else if (do_append) prep_kernel<D, T, true, false><<<grid, 3 * Cfg::GT, sm3, st>>>(a, nbg);
@@ -384,7 +457,8 @@ cudaError_t launch_prep(const DecodeArgs& d, const void* k, const void* v, int D
   a.v = v;
   a.out = d.out;
   a.q_pos = d.q_pos;
-  a.qrot = d.qrot;
+  a.frags = d.frags;
+  a.tabs = d.tabs;
   a.layer_begin = d.layer_begin;
   a.rope_layout = d.rope_layout;
   const int lh_count = d.n_layers_call * d.cv.H;

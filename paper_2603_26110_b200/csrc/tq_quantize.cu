@@ -10,11 +10,14 @@
 // followed by warp-shuffle norm reductions and a conflict-free word assembly.  All arithmetic is fp32
 // with IEEE division and square root so that codes agree with the fp64 oracle except inside the 1e-5
 // band around a threshold.
-#include <cstdlib>
+#include <atomic>
 
 #include "tq_common.cuh"
 
 namespace tq {
+
+static std::atomic<int> g_debug_quantize_fp32{0};
+void debug_set_quantize_fp32(int on) { g_debug_quantize_fp32.store(on, std::memory_order_relaxed); }
 
 
 __device__ __forceinline__ int swz(int k) { return ((k >> 1) * 4) & 31; }
@@ -201,64 +204,64 @@ __global__ void __launch_bounds__(2 * D) quantize_pack_kernel(QuantArgs a) {
     }
     __syncthreads();
     // ------------------------------------------------------------------ assemble and store the tile
+    // one thread per (section, word, lane) of the device tile layout (tq_common.cuh); tokens of the tile that are
+    // outside this call keep their bits (read-modify-write under a mask)
     unsigned char* tp = stream + (size_t)tile * Lo::kTileBytes;
-    // K code words: 32 slots x KCW words, field g of slot t at position (g - t) mod P
-    for (int idx = tid; idx < kTile * Lo::KCW; idx += NT) {
-      const int w = idx / kTile, slot = idx % kTile;  // lanes vary slot -> coalesced chunk-major stores
+    auto in_call = [&](int slot) {
       const int pos = tile * kTile + slot;
-      if (pos < a.start_pos || pos >= a.start_pos + a.n_tokens) continue;
-      const unsigned char* cb = cbK + slot * D;
-      unsigned long long word = 0;
-      const int k_lo = (32 * w) / 6, k_hi = (32 * w + 31) / 6;
-      for (int kf = k_lo; kf <= k_hi; ++kf) {
-        const int g = (kf + slot) % Lo::P;
-        unsigned long long f = cb[2 * g] | ((unsigned)cb[2 * g + 1] << 3);
-        const int sh = 6 * kf - 32 * w;  // may be negative for the field straddling in from the previous word
-        word |= sh >= 0 ? (f << sh) : (f >> (-sh));
-      }
-      *reinterpret_cast<unsigned*>(tp + Lo::kOffKC + word_offset(Lo::KCW, w, slot)) = (unsigned)word;
-    }
-    // V code words: lane g owns pair groups g (+32): token slot j at bits [6j, 6j+6) of its string; tokens of
-    // the tile that are outside this call keep their bits (read-modify-write under a mask)
-    for (int idx = tid; idx < kTile * Lo::KCW; idx += NT) {
-      const int w = idx / kTile, lane = idx % kTile;
-      const int part = (32 * w) / 192, sb = 32 * w - 192 * part;
-      const int g = lane + kTile * part;
+      return pos >= a.start_pos && pos < a.start_pos + a.n_tokens;
+    };
+    constexpr int WTOT = 2 * Lo::KCW + Lo::KSW;
+    for (int idx = tid; idx < kTile * WTOT; idx += NT) {
+      const int wq = idx / kTile, lane = idx % kTile, g = lane >> 2, t = lane & 3;
       unsigned long long word = 0, mask = 0;
-      const int j_lo = sb / 6, j_hi = (sb + 31) / 6;
-      for (int j = j_lo; j <= j_hi && j < kTile; ++j) {
-        const int pos = tile * kTile + j;
-        if (pos < a.start_pos || pos >= a.start_pos + a.n_tokens) continue;
-        unsigned long long f = cbV[j * D + 2 * g] | ((unsigned)cbV[j * D + 2 * g + 1] << 3);
-        const int sh = 6 * j - sb;
-        word |= sh >= 0 ? (f << sh) : (f >> (-sh));
-        mask |= sh >= 0 ? (63ull << sh) : (63ull >> (-sh));
+      auto put = [&](int bit, int nb, unsigned v) {  // bit relative to the word's first bit, may be negative
+        const unsigned long long mk = (1ull << nb) - 1ull;
+        if (bit <= -nb || bit >= 32) return;
+        word |= bit >= 0 ? ((unsigned long long)v << bit) : ((unsigned long long)v >> (-bit));
+        mask |= bit >= 0 ? (mk << bit) : (mk >> (-bit));
+      };
+      unsigned* p;
+      if (wq < Lo::KCW) {  // K pair fields: slots g + 8 r, pairs t + 4 j
+        const int w = wq;
+        for (int r = 0; r < 4; ++r) {
+          const int slot = g + 8 * r;
+          if (!in_call(slot)) continue;
+          for (int j = 0; j < Lo::J; ++j) {
+            const int pr = t + 4 * j;
+            put(6 * (Lo::J * r + j) - 32 * w, 6, cbK[slot * D + 2 * pr] | ((unsigned)cbK[slot * D + 2 * pr + 1] << 3));
+          }
+        }
+        p = reinterpret_cast<unsigned*>(tp + Lo::kOffKC + word_offset(Lo::KCW, w, lane));
+      } else if (wq < Lo::KCW + Lo::KSW) {  // sign bits: slots g + 8 r, sketch rows t d/4 + i
+        const int w = wq - Lo::KCW;
+        for (int r = 0; r < 4; ++r) {
+          const int slot = g + 8 * r;
+          if (!in_call(slot)) continue;
+          for (int i = 0; i < D / 4; ++i) {
+            const int rho = t * (D / 4) + i;
+            put(sign_bit_pos<D>(slot, rho).bit - 32 * w, 1, bbK[slot * D + rho]);
+          }
+        }
+        p = reinterpret_cast<unsigned*>(tp + Lo::kOffKS + word_offset(Lo::KSW, w, lane));
+      } else {  // V codes: token pairs t + 4 j, coordinates g + 8 c
+        const int w = wq - Lo::KCW - Lo::KSW;
+        for (int j = 0; j < 4; ++j)
+          for (int e = 0; e < 2; ++e) {
+            const int slot = 2 * (t + 4 * j) + e;
+            if (!in_call(slot)) continue;
+            for (int c = 0; c < Lo::C; ++c) put(v_code_pos<D>(slot, g + 8 * c).bit - 32 * w, 3, cbV[slot * D + g + 8 * c]);
+          }
+        p = reinterpret_cast<unsigned*>(tp + Lo::kOffVC + word_offset(Lo::KCW, w, lane));
       }
-      unsigned* p = reinterpret_cast<unsigned*>(tp + Lo::kOffVC + word_offset(Lo::KCW, w, lane));
       const unsigned m32 = (unsigned)mask;
       if (m32 == 0xffffffffu) *p = (unsigned)word;
       else if (m32) *p = (*p & ~m32) | ((unsigned)word & m32);
     }
-    for (int idx = tid; idx < kTile * Lo::KSW; idx += NT) {
-      const int w = idx / kTile, slot = idx % kTile;
-      const int pos = tile * kTile + slot;
-      if (pos < a.start_pos || pos >= a.start_pos + a.n_tokens) continue;
-      const unsigned char* bb = bbK + slot * D;
-      unsigned word = 0;
-      for (int kn = 0; kn < 8; ++kn) {
-        const int n = (8 * w + kn + slot) % Lo::NG;
-        unsigned nib = bb[4 * n] | (bb[4 * n + 1] << 1) | (bb[4 * n + 2] << 2) | (bb[4 * n + 3] << 3);
-        word |= nib << (4 * kn);
-      }
-      *reinterpret_cast<unsigned*>(tp + Lo::kOffKS + word_offset(Lo::KSW, w, slot)) = word;
-    }
-    if (tid < kTile) {
-      const int pos = tile * kTile + tid;
-      if (pos >= a.start_pos && pos < a.start_pos + a.n_tokens) {
-        reinterpret_cast<unsigned short*>(tp + Lo::kOffKN)[tid] = nK[tid];
-        reinterpret_cast<unsigned short*>(tp + Lo::kOffKR)[tid] = rK[tid];
-        reinterpret_cast<unsigned short*>(tp + Lo::kOffVN)[tid] = nV[tid];
-      }
+    if (tid < kTile && in_call(tid)) {
+      const int nl = slot_lane(tid);
+      reinterpret_cast<unsigned*>(tp + Lo::kOffNK)[nl] = (unsigned)nK[tid] | ((unsigned)rK[tid] << 16);
+      reinterpret_cast<unsigned short*>(tp + Lo::kOffVN)[nl] = nV[tid];
     }
     __syncthreads();
   }
@@ -299,11 +302,12 @@ cudaError_t launch_quantize_pack(const QuantArgs& a, int D, tq_dtype dt, int num
     count_launch();
     return cudaGetLastError();
   }
-  // the tensor-core kernel (tq_quantize_tc.cu) is the product path; TQ_QUANTIZE_IMPL=fp32 selects the CUDA-core kernel
-  // of this file (kept as a cross-check)
-  const char* impl = getenv("TQ_QUANTIZE_IMPL");  // read per call: a test switches it in-process
-  const bool force_fp32 = impl && impl[0] == 'f';
+  // the tensor-core kernel (tq_quantize_tc.cu) is the product path; tq_debug_set_quantize_impl(1) selects the CUDA-core
+  // kernel of this file (kept as a cross-check)
+  const bool force_fp32 = g_debug_quantize_fp32.load(std::memory_order_relaxed) != 0;
+#ifndef TQ_NO_TC_QUANTIZE
   if (!force_fp32) return launch_quantize_pack_tc(a, D, dt, num_sms, st);
+#endif
   if (D == 64) return dt == TQ_F16 ? launch_quant_t<64, __half>(a, num_sms, st) : launch_quant_t<64, float>(a, num_sms, st);
   return dt == TQ_F16 ? launch_quant_t<128, __half>(a, num_sms, st) : launch_quant_t<128, float>(a, num_sms, st);
 }

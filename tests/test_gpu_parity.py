@@ -283,13 +283,16 @@ def test_decode_d128(tq, oracle):
     _decode_case(tq, oracle, w, seq_len=[330, 77])
 
 
-def test_decode_is_independent_of_split_factor(tq, oracle, monkeypatch):
+def test_decode_is_independent_of_split_factor(tq, oracle):
     w = W.CONFIGS["cfg0_tiny"].scaled(batch=1, n_heads=2, seq=1024)
     outs = []
-    for ns in ("1", "3", "8", "64"):
-        monkeypatch.setenv("TQ_DECODE_NSPLIT", ns)
-        c, _ = _decode_case(tq, oracle, w)
-        outs.append(c.gpu_decode(0, 1, W.queries(w, 0)[None])[0])
+    try:
+        for ns in (1, 3, 8, 64):
+            tq.tq_debug_set_decode_nsplit(ns)
+            c, _ = _decode_case(tq, oracle, w)
+            outs.append(c.gpu_decode(0, 1, W.queries(w, 0)[None])[0])
+    finally:
+        tq.tq_debug_set_decode_nsplit(0)
     assert all(np.abs(outs[0] - o).max() < 1e-4 for o in outs[1:])
 
 
@@ -385,18 +388,21 @@ def test_full_size_cfg2_sampled_units(tq, oracle):
 @pytest.mark.gpu
 @pytest.mark.parametrize("name,kw", [("cfg2_650m_batch32", dict(batch=3, n_heads=4, seq=300)),
                                      ("cfg4_15b_heads", dict(batch=2, n_heads=3, seq=200))])
-def test_tensor_core_quantize_agrees_with_cuda_core_kernel(tq, oracle, monkeypatch, name, kw):
+def test_tensor_core_quantize_agrees_with_cuda_core_kernel(tq, oracle, name, kw):
     """The tcgen05 kernel (two-term fp16 split operands) and the fp32 CUDA-core kernel are two roundings of the same
     fp64 definition: they may only differ where the oracle marks a coordinate within 1e-5 of a threshold."""
     w = W.CONFIGS[name].scaled(**kw)
     k, v = W.layer_activations(w, 0)
     planes = {}
-    for impl in ("tc", "fp32"):
-        monkeypatch.setenv("TQ_QUANTIZE_IMPL", impl)
-        c = Case(tq, oracle, w)
-        tq.tq_quantize_pack(c.shape, c.params, c.cache, 0, c.dev(k), c.dev(v))
-        planes[impl] = c.gpu_export(0, w.seq)
-        can = c.oracle_quantize(0, k, v)
+    try:
+        for impl in ("tc", "fp32"):
+            tq.tq_debug_set_quantize_impl(impl == "fp32")
+            c = Case(tq, oracle, w)
+            tq.tq_quantize_pack(c.shape, c.params, c.cache, 0, c.dev(k), c.dev(v))
+            planes[impl] = c.gpu_export(0, w.seq)
+            can = c.oracle_quantize(0, k, v)
+    finally:
+        tq.tq_debug_set_quantize_impl(False)
     d = w.head_dim
     for key, near in (("k_codes", can.near_k), ("v_codes", can.near_v)):
         a = TL.unpack_codes_np(planes["tc"][key], d)
@@ -445,7 +451,7 @@ def test_model_step_host_equals_per_layer_host_steps(tq, oracle):
         kn = torch.from_numpy(np.stack([t[1] for t in toks])).pin_memory()
         vn = torch.from_numpy(np.stack([t[2] for t in toks])).pin_memory()
         out = torch.empty_like(q).pin_memory()
-        ws = tq.Workspace(c.shape, 1)
+        ws = tq.Workspace(c.shape, 1 if mode == "per_layer" else w.n_layers)
         dt = tq.TQ_F16 if w.dtype == "f16" else tq.TQ_F32
         if mode == "per_layer":
             st = torch.zeros(tq.tq_step_staging_bytes(c.shape, dt) + 256, dtype=torch.uint8, device="cuda")
@@ -460,6 +466,54 @@ def test_model_step_host_equals_per_layer_host_steps(tq, oracle):
         assert torch.all(c.cache.seq_len == w.seq + 1)
         outs.append(out.clone())
     assert torch.isfinite(outs[0].float()).all() and torch.equal(outs[0], outs[1])
+
+
+@pytest.mark.gpu
+def test_model_step_equals_per_layer_steps_and_replays_from_a_graph(tq, oracle):
+    """tq_decode_model_step (one prep launch for all layers, then a run-ahead chain of streaming launches) must give
+    bit-identical outputs and cache bytes to tq_append + tq_decode_attn called layer by layer; and a CUDA graph of it
+    replayed 100 times (seq_len rewound in between) must reproduce the same bits every time: the chain has no
+    ordering hole (programmatic dependent launch vs. the appended token)."""
+    import torch
+
+    w = W.CONFIGS["cfg2_650m_batch32"].scaled(n_layers=4, batch=5, n_heads=6, seq=300)
+    L = w.n_layers
+    cases = []
+    for mode in ("separate", "model"):
+        c = Case(tq, oracle, w, max_seq=w.seq + 40)
+        for layer in range(L):
+            k, v = W.layer_activations(w, layer)
+            tq.tq_quantize_pack(c.shape, c.params, c.cache, layer, c.dev(k), c.dev(v))
+        cases.append(c)
+    toks = [W.step_tokens(w, layer, 0) for layer in range(L)]
+    q, kn, vn = (cases[0].dev(np.stack([t[i] for t in toks])) for i in range(3))
+    out_a, out_b = torch.full_like(q, float("nan")), torch.full_like(q, float("nan"))
+    ca, cb = cases
+    ws1, wsL = tq.Workspace(ca.shape, 1), tq.Workspace(cb.shape, L)
+    for layer in range(L):
+        tq.tq_append(ca.shape, ca.params, ca.cache, layer, kn[layer], vn[layer])
+        tq.tq_decode_attn(ca.shape, ca.params, ca.cache, layer, 1, q[layer:layer + 1], out_a[layer:layer + 1], ws1, None, w.seq + 40)
+    tq.tq_decode_model_step(cb.shape, cb.params, cb.cache, 0, L, q, kn, vn, out_b, wsL, w.seq + 40)
+    torch.cuda.synchronize()
+    assert torch.isfinite(out_a.float()).all() and torch.equal(out_a, out_b)
+    assert torch.equal(ca.cache.data, cb.cache.data)
+    # graph replay: every replay starts from the same cache length and must give the same bits
+    stream = torch.cuda.Stream()
+    out_g = torch.full_like(q, float("nan"))
+    with torch.cuda.stream(stream):
+        cb.cache.seq_len.fill_(w.seq)
+        tq.tq_decode_model_step(cb.shape, cb.params, cb.cache, 0, L, q, kn, vn, out_g, wsL, w.seq + 40, stream)
+        stream.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=stream):
+            tq.tq_decode_model_step(cb.shape, cb.params, cb.cache, 0, L, q, kn, vn, out_g, wsL, w.seq + 40, stream)
+        for _ in range(100):
+            cb.cache.seq_len.fill_(w.seq)
+            out_g.fill_(float("nan"))
+            g.replay()
+            assert torch.equal(out_g, out_a)
+        stream.synchronize()
+    assert torch.equal(ca.cache.data, cb.cache.data)
 
 
 # ---------------------------------------------------------------------------------------------- ablation report
