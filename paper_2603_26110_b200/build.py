@@ -8,9 +8,9 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtq.so")
-SOURCES = ["tq_api.cu", "tq_layout.cu", "tq_quantize.cu", "tq_decode.cu", "tq_prep.cu", "tq_calibrate_host.cpp"]  # TEMP: tc quantize being ported
+SOURCES = ["tq_api.cu", "tq_layout.cu", "tq_quantize.cu", "tq_quantize_tc.cu", "tq_decode.cu", "tq_prep.cu", "tq_calibrate_host.cpp"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC",
-              "--expt-relaxed-constexpr", "-DTQ_NO_TC_QUANTIZE"]
+              "--expt-relaxed-constexpr"]
 
 
 def _stale() -> bool:

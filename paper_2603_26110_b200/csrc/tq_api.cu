@@ -75,7 +75,7 @@ static int check_params(const tq_params* p) {
 }
 
 struct WorkspaceGeom {
-  size_t off_counters, off_frags, off_tabs, off_partials, total;
+  size_t off_counters, off_frags, off_tabs, off_orot, off_partials, total;
   size_t frag_words;
 };
 static WorkspaceGeom workspace_geom(const CacheGeom& g, int n_layers_call) {
@@ -85,7 +85,8 @@ static WorkspaceGeom workspace_geom(const CacheGeom& g, int n_layers_call) {
   w.frag_words = g.D == 64 ? FragLayout<64>::kWords : FragLayout<128>::kWords;
   w.off_frags = (units * 4 + 255) / 256 * 256;
   w.off_tabs = w.off_frags + (units * w.frag_words * 4 + 255) / 256 * 256;
-  w.off_partials = w.off_tabs + ((size_t)n_layers_call * g.H * kTabWords * 4 + 255) / 256 * 256;
+  w.off_orot = w.off_tabs + ((size_t)n_layers_call * g.H * kTabWords * 4 + 255) / 256 * 256;
+  w.off_partials = w.off_orot + (units * g.D * 4 + 255) / 256 * 256;
   w.total = w.off_partials + units * kMaxSplits * (size_t)(g.D + 2) * 4;
   return w;
 }
@@ -212,6 +213,7 @@ static int run_decode(const tq_shape* shape, const tq_params* dev, const tq_cach
     a.counters = ws ? (int*)(ws + w.off_counters) + u0 : nullptr;
     a.frags = ws ? (unsigned*)(ws + w.off_frags) + u0 * w.frag_words : nullptr;
     a.tabs = ws ? (unsigned*)(ws + w.off_tabs) + (size_t)l0 * g.H * kTabWords : nullptr;
+    a.orot = nullptr;
     a.partials = ws ? (float*)(ws + w.off_partials) + u0 * kMaxSplits * (g.D + 2) : nullptr;
     a.layer_begin = layer_begin + l0;
     a.n_layers_call = nl;
@@ -225,7 +227,7 @@ static int run_decode(const tq_shape* shape, const tq_params* dev, const tq_cach
     if (!(g_profile_skip_prep && do_query && !do_append) &&
         launch_prep(a, kc, vc, g.D, do_append, do_query, (cudaStream_t)cuda_stream) != cudaSuccess)
       return TQ_ERR_CUDA;
-    if (do_query && launch_decode(a, g.D, (cudaStream_t)cuda_stream) != cudaSuccess) return TQ_ERR_CUDA;
+    if (do_query && launch_decode(a, g.D, true, (cudaStream_t)cuda_stream) != cudaSuccess) return TQ_ERR_CUDA;
   }
   return TQ_OK;
 }
@@ -312,12 +314,14 @@ int tq_decode_model_step(const tq_shape* shape, const tq_params* dev, tq_cache* 
   a.counters = (int*)(ws + w.off_counters);
   a.frags = (unsigned*)(ws + w.off_frags);
   a.tabs = (unsigned*)(ws + w.off_tabs);
+  a.orot = (float*)(ws + w.off_orot);
   a.partials = (float*)(ws + w.off_partials);
   a.layer_begin = layer_begin, a.n_layers_call = n_layers_call;
   a.nsplit = nsplit, a.per = (ntiles + nsplit - 1) / nsplit;
   a.chain_mode = 0, a.rope_layout = shape->rope_layout, a.dt = (int)dt;
   // one prep launch for every layer of the step (append + query operands), then one streaming launch per layer cache:
-  // the first waits for the prep kernel, the others run ahead of one another (DecodeArgs::chain_mode)
+  // the first waits for the prep kernel, the others run ahead of one another (DecodeArgs::chain_mode); they leave o'/l
+  // in the workspace and one last launch applies PI_V^T to every unit of the step
   if (!g_profile_skip_prep && launch_prep(a, k, v, g.D, true, true, st) != cudaSuccess) return TQ_ERR_CUDA;
   const size_t units = (size_t)g.B * g.H;
   for (int l = 0; l < n_layers_call; ++l) {
@@ -328,11 +332,13 @@ int tq_decode_model_step(const tq_shape* shape, const tq_params* dev, tq_cache* 
     b.counters = a.counters + u0;
     b.frags = a.frags + u0 * w.frag_words;
     b.tabs = a.tabs + (size_t)l * g.H * kTabWords;
+    b.orot = a.orot + u0 * g.D;
     b.partials = a.partials + u0 * kMaxSplits * (g.D + 2);
     b.layer_begin = layer_begin + l, b.n_layers_call = 1;
     b.chain_mode = l == 0 ? 0 : 1;
-    if (launch_decode(b, g.D, st) != cudaSuccess) return TQ_ERR_CUDA;
+    if (launch_decode(b, g.D, false, st) != cudaSuccess) return TQ_ERR_CUDA;
   }
+  if (launch_finish(a, g.D, st) != cudaSuccess) return TQ_ERR_CUDA;
   return TQ_OK;
 }
 

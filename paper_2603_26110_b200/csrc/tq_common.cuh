@@ -183,6 +183,7 @@ struct DecodeArgs {
   const int32_t* q_pos;  // [Lc][B] or nullptr
   unsigned* frags;       // workspace [units_call][FragLayout<D>::kWords] (tq_prep.cu)
   unsigned* tabs;        // workspace [layers_call * H][kTabWords]
+  float* orot;           // workspace [units_call][D]: o'/l in the rotated basis (tq_decode_model_step)
   float* partials;       // workspace [units_call][64][D + 2]
   int* counters;         // workspace [units_call]
   int layer_begin, n_layers_call, nsplit /* CTAs per unit, >= 1 */, per /* tiles per split planned from t_hint */, rope_layout, dt;
@@ -197,7 +198,8 @@ cudaError_t launch_quantize_pack(const QuantArgs& a, int D, tq_dtype dt, int num
 cudaError_t launch_quantize_pack_tc(const QuantArgs& a, int D, tq_dtype dt, int num_sms, cudaStream_t st);  // tcgen05
 cudaError_t launch_prep(const DecodeArgs& d, const void* k, const void* v, int D, bool do_append, bool do_query,
                         cudaStream_t st);
-cudaError_t launch_decode(const DecodeArgs& a, int D, cudaStream_t st);
+cudaError_t launch_decode(const DecodeArgs& a, int D, bool fused_out, cudaStream_t st);
+cudaError_t launch_finish(const DecodeArgs& a, int D, cudaStream_t st);
 int decode_ctas_per_sm(int D);
 cudaError_t launch_export(const CacheGeom& g, const CacheView& cv, int layer, int n_tokens, const tq_canonical& out,
                           cudaStream_t st);

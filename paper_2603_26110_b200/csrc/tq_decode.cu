@@ -384,7 +384,9 @@ __device__ __forceinline__ void stream_tiles(const unsigned char* stream, int ti
 // grid = units x nsplit.  CTA (unit uc, split sp) streams tiles [sp * per, (sp + 1) * per) of its unit, per = tiles per
 // split planned on the host from t_hint (the last split also takes whatever lies beyond); a shorter cache simply
 // leaves the trailing splits empty.  The four warps take tiles round-robin.
-template <int D, typename TIO>
+// kFusedOut: the finishing CTA applies PI_V^T and writes `out` (per-layer calls); otherwise it leaves o'/l in the
+// workspace and finish_kernel rotates every unit of the step at once (tq_decode_model_step).
+template <int D, typename TIO, bool kFusedOut>
 __global__ void __launch_bounds__(kDecodeThreads, DecodeCfg<D>::kCtasPerSm) decode_main_kernel(DecodeArgs a) {
   using Lo = Layout<D>;
   using Cfg = DecodeCfg<D>;
@@ -398,36 +400,28 @@ __global__ void __launch_bounds__(kDecodeThreads, DecodeCfg<D>::kCtasPerSm) deco
   int* flag = reinterpret_cast<int*>(abs0 + Cfg::kAbsFlag);
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  // grid = (nsplit, H, layers_in_call x B): no integer division on the way to the unit
   const int B = a.cv.B, H = a.cv.H;
-  const int nsplit = a.nsplit;
-  const int uc = (int)blockIdx.x / nsplit, sp = (int)blockIdx.x - uc * nsplit;
-  const int e = uc / H, h = uc - e * H;  // e = (layer-in-call, batch); seq_len is contiguous over e
-  const int lc = e / B, b = e - lc * B;
+  const int nsplit = (int)gridDim.x, sp = (int)blockIdx.x, h = (int)blockIdx.y, e = (int)blockIdx.z;
+  const int lc = a.n_layers_call == 1 ? 0 : e / B, b = e - lc * B;  // e = (layer-in-call, batch); seq_len is contiguous over e
+  const int uc = e * H + h;
   const int layer = a.layer_begin + lc;
   const size_t lh = (size_t)layer * H + h;
   const int per = a.per, tile0 = sp * per;
   const int cap1 = sp == nsplit - 1 ? a.cv.tiles_cap : min(a.cv.tiles_cap, tile0 + per);  // static bound of this split
   const unsigned char* stream = a.cv.tiles + (((size_t)layer * B + b) * H + h) * a.cv.stream_bytes;
 
-  // ---- before the PDL wait: only constants and hints.  The cache stream of this CTA starts towards L2 while the
-  //      kernel in front of this launch is still running (L2 stays coherent with whatever it still writes); the
-  //      dequantisation tables depend on the LUTs alone.
-#pragma unroll
-  for (int i = 0; i < kStages; ++i) {
-    const int tl = tile0 + warp + i * NW;
-    if (tl < cap1 && lane == 0)
-      asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(stream + (size_t)tl * Lo::kTileBytes), "r"(Lo::kTileBytes)
-                   : "memory");
-  }
   if (lane == 0) {
 #pragma unroll
     for (int i = 0; i < kStages; ++i) mbar_init(Cfg::kAbsBar + (warp * kStages + i) * 8, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   const float* Pv = a.pi_v + lh * D * D;
+  if constexpr (kFusedOut) {  // a hint: PI_V towards L2 for the epilogue
 #pragma unroll
-  for (int i = 0; i < D * D * 4 / 128 / kDecodeThreads; ++i)
-    asm volatile("prefetch.global.L2 [%0];" ::"l"(Pv + (size_t)(i * kDecodeThreads + tid) * 32));
+    for (int i = 0; i < D * D * 4 / 128 / kDecodeThreads; ++i)
+      asm volatile("prefetch.global.L2 [%0];" ::"l"(Pv + (size_t)(i * kDecodeThreads + tid) * 32));
+  }
 
   if (a.chain_mode == 0) pdl_wait();
   pdl_trigger();  // the launch behind this one may be scheduled: it either waits for this grid or belongs to the same chain
@@ -568,54 +562,101 @@ __global__ void __launch_bounds__(kDecodeThreads, DecodeCfg<D>::kCtasPerSm) deco
       }
     }
   }
-  // ---- out = PI_V^T (o' / l): the k range is split over the 128 / D thread groups; every load is issued before the
-  //      first multiply (one L2 round trip), four independent chains per thread
-  if (tid < D) omerged[tid] = Lsum > 0.f ? oi / Lsum : 0.f;
-  __syncthreads();
-  constexpr int PARTS = kDecodeThreads / D;  // 2 | 1
-  constexpr int KP = D / PARTS;              // 32 | 128
-  const int i = tid % D, part = (tid / D) % PARTS;
-  float r = 0.f;
-  {
-    const float* Pvp = Pv + (size_t)part * KP * D + i;
+  if constexpr (!kFusedOut) {
+    if (tid < D) a.orot[(size_t)uc * D + tid] = Lsum > 0.f ? oi / Lsum : 0.f;
+  } else {
+    // ---- out = PI_V^T (o' / l): the k range is split over the 128 / D thread groups; every load is issued before the
+    //      first multiply (one L2 round trip), four independent chains per thread
+    if (tid < D) omerged[tid] = Lsum > 0.f ? oi / Lsum : 0.f;
+    __syncthreads();
+    constexpr int PARTS = kDecodeThreads / D;  // 2 | 1
+    constexpr int KP = D / PARTS;              // 32 | 128
+    const int i = tid % D, part = (tid / D) % PARTS;
+    float r = 0.f;
+    {
+      const float* Pvp = Pv + (size_t)part * KP * D + i;
 #pragma unroll
-    for (int k0 = 0; k0 < KP; k0 += 32) {
-      float pv[32];
+      for (int k0 = 0; k0 < KP; k0 += 32) {
+        float pv[32];
 #pragma unroll
-      for (int k = 0; k < 32; ++k) pv[k] = __ldg(Pvp + (size_t)(k0 + k) * D);
-      float r0 = 0.f, r1 = 0.f, r2 = 0.f, r3 = 0.f;
+        for (int k = 0; k < 32; ++k) pv[k] = __ldg(Pvp + (size_t)(k0 + k) * D);
+        float r0 = 0.f, r1 = 0.f, r2 = 0.f, r3 = 0.f;
 #pragma unroll
-      for (int k = 0; k < 32; k += 4) {
-        r0 = fmaf(pv[k], omerged[part * KP + k0 + k], r0);
-        r1 = fmaf(pv[k + 1], omerged[part * KP + k0 + k + 1], r1);
-        r2 = fmaf(pv[k + 2], omerged[part * KP + k0 + k + 2], r2);
-        r3 = fmaf(pv[k + 3], omerged[part * KP + k0 + k + 3], r3);
+        for (int k = 0; k < 32; k += 4) {
+          r0 = fmaf(pv[k], omerged[part * KP + k0 + k], r0);
+          r1 = fmaf(pv[k + 1], omerged[part * KP + k0 + k + 1], r1);
+          r2 = fmaf(pv[k + 2], omerged[part * KP + k0 + k + 2], r2);
+          r3 = fmaf(pv[k + 3], omerged[part * KP + k0 + k + 3], r3);
+        }
+        r += (r0 + r1) + (r2 + r3);
       }
-      r += (r0 + r1) + (r2 + r3);
     }
-  }
-  if (PARTS > 1 && part > 0) omerged[part * D + i] = r;
-  __syncthreads();
-  if (tid < D) {
+    if (PARTS > 1 && part > 0) omerged[part * D + i] = r;
+    __syncthreads();
+    if (tid < D) {
 #pragma unroll
-    for (int pp = 1; pp < PARTS; ++pp) r += omerged[pp * D + i];
-    TIO* outp = reinterpret_cast<TIO*>(a.out) + (size_t)uc * D;
-    if constexpr (sizeof(TIO) == 2) outp[i] = __float2half_rn(r);
-    else outp[i] = r;
+      for (int pp = 1; pp < PARTS; ++pp) r += omerged[pp * D + i];
+      TIO* outp = reinterpret_cast<TIO*>(a.out) + (size_t)uc * D;
+      if constexpr (sizeof(TIO) == 2) outp[i] = __float2half_rn(r);
+      else outp[i] = r;
+    }
   }
   if (a.chain_mode != 0) pdl_wait();  // complete in launch order (see DecodeArgs::chain_mode)
 }
 
+// ---- out = PI_V^T orot for every unit of a model step (tq_decode_model_step): one CTA per (layer-in-call, head) and
+//      group of kFinB batch entries; thread i owns output coordinate i and column i of PI_V (coalesced over the CTA)
+constexpr int kFinB = 8;
+template <int D, typename TIO>
+__global__ void __launch_bounds__(D) finish_kernel(DecodeArgs a, int nbg) {
+  __shared__ float os[kFinB][D];
+  const int i = threadIdx.x, B = a.cv.B, H = a.cv.H;
+  const int bgi = (int)blockIdx.x % nbg, lh_c = (int)blockIdx.x / nbg, lc = lh_c / H, h = lh_c - lc * H;
+  const int b0 = bgi * kFinB, nb = min(kFinB, B - b0);
+  const float* Pv = a.pi_v + ((size_t)(a.layer_begin + lc) * H + h) * D * D;
+  pdl_wait();
+#pragma unroll
+  for (int e = 0; e < kFinB; ++e) os[e][i] = e < nb ? __ldcg(a.orot + (((size_t)lc * B + b0 + e) * H + h) * D + i) : 0.f;
+  __syncthreads();
+  // the same summation order as the fused epilogue of decode_main_kernel (32-element chunks, four interleaved chains),
+  // so that both forms give identical bits
+  float acc[kFinB];
+#pragma unroll
+  for (int e = 0; e < kFinB; ++e) acc[e] = 0.f;
+#pragma unroll 1
+  for (int k0 = 0; k0 < D; k0 += 32) {
+    float pv[32];
+#pragma unroll
+    for (int k = 0; k < 32; ++k) pv[k] = __ldg(Pv + (size_t)(k0 + k) * D + i);
+#pragma unroll
+    for (int e = 0; e < kFinB; ++e) {
+      float r0 = 0.f, r1 = 0.f, r2 = 0.f, r3 = 0.f;
+#pragma unroll
+      for (int k = 0; k < 32; k += 4) {
+        r0 = fmaf(pv[k], os[e][k0 + k], r0);
+        r1 = fmaf(pv[k + 1], os[e][k0 + k + 1], r1);
+        r2 = fmaf(pv[k + 2], os[e][k0 + k + 2], r2);
+        r3 = fmaf(pv[k + 3], os[e][k0 + k + 3], r3);
+      }
+      acc[e] += (r0 + r1) + (r2 + r3);
+    }
+  }
+  for (int e = 0; e < nb; ++e) {
+    TIO* outp = reinterpret_cast<TIO*>(a.out) + (((size_t)lc * B + b0 + e) * H + h) * D;
+    if constexpr (sizeof(TIO) == 2) outp[i] = __float2half_rn(acc[e]);
+    else outp[i] = acc[e];
+  }
+}
+
 // ------------------------------------------------------------------------------------------ launchers
-template <int D, typename T>
+template <int D, typename T, bool kFusedOut>
 static cudaError_t launch_decode_t(const DecodeArgs& a, cudaStream_t st) {
   constexpr int smem = DecodeCfg<D>::kSmemBytes;
   // per launch: the attribute is per device and a process may drive several
-  cudaError_t e = cudaFuncSetAttribute(decode_main_kernel<D, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+  cudaError_t e = cudaFuncSetAttribute(decode_main_kernel<D, T, kFusedOut>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
   if (e != cudaSuccess) return e;
-  const int units = a.n_layers_call * a.cv.B * a.cv.H;
   cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = dim3(units * a.nsplit);
+  cfg.gridDim = dim3(a.nsplit, a.cv.H, a.n_layers_call * a.cv.B);
   cfg.blockDim = dim3(kDecodeThreads);
   cfg.dynamicSmemBytes = smem;
   cfg.stream = st;
@@ -624,16 +665,33 @@ static cudaError_t launch_decode_t(const DecodeArgs& a, cudaStream_t st) {
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  e = cudaLaunchKernelEx(&cfg, decode_main_kernel<D, T>, a);
+  e = cudaLaunchKernelEx(&cfg, decode_main_kernel<D, T, kFusedOut>, a);
   count_launch();
   return e != cudaSuccess ? e : cudaGetLastError();
 }
 
+template <int D, typename T>
+static cudaError_t launch_finish_t(const DecodeArgs& a, cudaStream_t st) {
+  const int nbg = (a.cv.B + kFinB - 1) / kFinB;
+  finish_kernel<D, T><<<a.n_layers_call * a.cv.H * nbg, D, 0, st>>>(a, nbg);
+  count_launch();
+  return cudaGetLastError();
+}
+
+cudaError_t launch_finish(const DecodeArgs& a, int D, cudaStream_t st) {
+  if (D == 64) return a.dt == TQ_F16 ? launch_finish_t<64, __half>(a, st) : launch_finish_t<64, float>(a, st);
+  return a.dt == TQ_F16 ? launch_finish_t<128, __half>(a, st) : launch_finish_t<128, float>(a, st);
+}
+
 int decode_ctas_per_sm(int D) { return D == 64 ? DecodeCfg<64>::kCtasPerSm : DecodeCfg<128>::kCtasPerSm; }
 
-cudaError_t launch_decode(const DecodeArgs& a, int D, cudaStream_t st) {
-  if (D == 64) return a.dt == TQ_F16 ? launch_decode_t<64, __half>(a, st) : launch_decode_t<64, float>(a, st);
-  return a.dt == TQ_F16 ? launch_decode_t<128, __half>(a, st) : launch_decode_t<128, float>(a, st);
+cudaError_t launch_decode(const DecodeArgs& a, int D, bool fused_out, cudaStream_t st) {
+  if (fused_out) {
+    if (D == 64) return a.dt == TQ_F16 ? launch_decode_t<64, __half, true>(a, st) : launch_decode_t<64, float, true>(a, st);
+    return a.dt == TQ_F16 ? launch_decode_t<128, __half, true>(a, st) : launch_decode_t<128, float, true>(a, st);
+  }
+  if (D == 64) return launch_decode_t<64, __half, false>(a, st);  // the output type is finish_kernel's business
+  return launch_decode_t<128, __half, false>(a, st);
 }
 
 }  // namespace tq

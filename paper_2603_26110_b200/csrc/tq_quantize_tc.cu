@@ -12,9 +12,11 @@
 //     sqrt 2), r x8 (only sign(S r) is used); fp16 values V are exact operands and need two products only.  A numpy
 //     study (hard part 4) puts the code-flip rate of this scheme at 2e-7, that of an all-fp32 pipeline;
 //   * the epilogue is thread-per-token: tcgen05.ld hands every thread the rotated coordinates of ITS token, 32
-//     columns at a time (pass 1: the norm; pass 2: codes, residual, packing), so nothing crosses lanes, and lane =
-//     token is exactly the order of the device tile layout (coalesced 16-byte stores).  Only the V codes, which the
-//     cache stores per coordinate pair across tokens, go through a shared-memory transpose.
+//     columns at a time (pass 1: the norm; pass 2: codes, residual, packing), so nothing crosses lanes.  The device
+//     tile layout (tq_common.cuh) is the A-fragment order of the decode kernel's MMAs, so every thread drops its
+//     bytes into an image of the block's four tiles in shared memory (byte / halfword stores; V fields, which mix the
+//     two tokens of a pair, are assembled by the pair from a small per-token scratch) and the CTA then writes the
+//     image out with coalesced 16-byte stores.  Tiles only partly covered by the call are pre-loaded into the image.
 #include "tq_common.cuh"
 
 namespace tq {
@@ -33,11 +35,15 @@ struct TcCfg {
   static constexpr int kTmemCols = 2 * D;          // key CTAs: D_K [0,d), D_S [d,2d); value CTAs: D_V [0,d)
   // instruction descriptor: kind::f16, A = B = fp16 (K-major), D = fp32, N = d, M = 128
   static constexpr uint32_t kIdesc = (1u << 4) | ((uint32_t)(D >> 3) << 17) | ((128u >> 4) << 24);
-  static constexpr int kRotPitch = Lo::KCW + 1;    // 7 | 13 words per token: odd, so thread-per-row is conflict free
+  // image of one tile's sections owned by a CTA: keys [K codes | K signs | norms k,r], values [V codes | norm v]
+  static constexpr int kImgK = Lo::kCodeBytes + Lo::kSignBytes + 4 * kTile;
+  static constexpr int kImgV = Lo::kCodeBytes + 2 * kTile;
+  static constexpr int kImgBytes = kImgK;          // per tile (the larger of the two)
+  static constexpr int kScrPitch = Lo::C + 1;      // V scratch: C words (8 codes each) per token, odd pitch
   // shared memory: B operands 4 x kMatBytes (keys: PI_K hi/lo, S hi/lo; values: PI_V hi/lo) | A operands hi, lo |
-  // V pair fields [128][P] | rotation staging [128][kRotPitch] | LUT, barriers, TMEM slot
+  // tile images [4][kImgBytes] | V scratch [128][kScrPitch] | LUT, barriers, TMEM slot
   static constexpr int kOffA = 4 * kMatBytes, kOffMisc = kOffA + 2 * kOpBytes;
-  static constexpr int kSmemBytes = kOffMisc + kBlk * Lo::P + kBlk * kRotPitch * 4 + 8 * 4 + 3 * 8 + 16;
+  static constexpr int kSmemBytes = kOffMisc + 4 * kImgBytes + kBlk * kScrPitch * 4 + 8 * 4 + 3 * 8 + 16;
 };
 
 // byte offset of element (row, k) of a [rows][d] fp16 operand in the canonical K-major no-swizzle layout:
@@ -266,9 +272,9 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
   unsigned char *B0_hi = smem, *B0_lo = smem + Cfg::kMatBytes;                               // PI_K | PI_V
   unsigned char *B1_hi = smem + 2 * Cfg::kMatBytes, *B1_lo = smem + 3 * Cfg::kMatBytes;      // S (keys only)
   unsigned char *A_hi = smem + Cfg::kOffA, *A_lo = A_hi + Cfg::kOpBytes;
-  unsigned char* cbV = smem + Cfg::kOffMisc;                                  // [128 tokens][P pair fields]
-  unsigned* crot = reinterpret_cast<unsigned*>(cbV + kBlk * P);               // [128][kRotPitch] rotation staging
-  float* lut_s = reinterpret_cast<float*>(crot + kBlk * Cfg::kRotPitch);      // [8]
+  unsigned char* img = smem + Cfg::kOffMisc;                                  // [4 tiles][kImgBytes]
+  unsigned* vscr = reinterpret_cast<unsigned*>(img + 4 * Cfg::kImgBytes);     // [128][kScrPitch] V code groups
+  float* lut_s = reinterpret_cast<float*>(vscr + kBlk * Cfg::kScrPitch);      // [8]
   unsigned long long* mbar = reinterpret_cast<unsigned long long*>(lut_s + 8);  // [0]: first product, [1]: S product
   unsigned* tmem_slot = reinterpret_cast<unsigned*>(mbar + 3);
 
@@ -325,15 +331,38 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
 
   const T* src = reinterpret_cast<const T*>(kKey ? a.k : a.v) + (size_t)bh * a.n_tokens * D;
   unsigned char* stream = a.cv.tiles + ((size_t)a.layer * a.cv.B * a.cv.H + bh) * a.cv.stream_bytes;
-  const int slot = tid & 31;
-  unsigned* row = crot + tid * Cfg::kRotPitch;
+  const int slot = tid & 31, tl = tid >> 5, sg = slot & 7, sr = slot >> 3;
+  unsigned char* timg = img + tl * Cfg::kImgBytes;  // image of this token's tile
+  constexpr int kOffImgKS = Lo::kCodeBytes, kOffImgNK = Lo::kCodeBytes + Lo::kSignBytes;  // keys image
+  constexpr int kOffImgVN = Lo::kCodeBytes;                                                // values image
+  // byte `sb` of lane l's word string in a section of W words per lane
+  auto sec_byte = [](int W, int l, int sb) { return word_offset(W, sb >> 2, l) + (sb & 3); };
 
   for (int blk = blk0; blk <= blk1; ++blk) {
     const uint32_t parity = (uint32_t)(blk - blk0) & 1u;
     const int pos = blk * kBlk + tid;
     const int i = pos - a.start_pos;
     const bool valid = i >= 0 && i < a.n_tokens;
-    unsigned char* tp = stream + (size_t)(pos / kTile) * Lo::kTileBytes;
+    // tiles of this block: covered (some token of the call) / fully covered; partly covered ones are pre-loaded so that
+    // the bits of tokens outside the call survive the write-back
+    const int call_end = a.start_pos + a.n_tokens;
+    auto tile_cover = [&](int t4) {  // 0 none, 1 partial, 2 full
+      const int p0 = blk * kBlk + t4 * kTile, lo = max(p0, a.start_pos), hi = min(p0 + kTile, call_end);
+      return hi <= lo ? 0 : (hi - lo == kTile ? 2 : 1);
+    };
+    {
+      constexpr int kOwn = kKey ? Cfg::kImgK : Cfg::kImgV;
+      for (int idx = tid; idx < 4 * (kOwn / 16); idx += kBlk) {
+        const int t4 = idx / (kOwn / 16), q = idx % (kOwn / 16);
+        if (tile_cover(t4) != 1) continue;
+        const unsigned char* tg = stream + (size_t)(blk * 4 + t4) * Lo::kTileBytes;
+        // keys: [0, kOffVC) then the norms; values: the V codes then |v|
+        const int ib = 16 * q;
+        const int gb = kKey ? (ib < Lo::kOffVC ? ib : Lo::kOffNK + (ib - Lo::kOffVC))
+                            : (ib < Lo::kCodeBytes ? Lo::kOffVC + ib : Lo::kOffVN + (ib - Lo::kCodeBytes));
+        *reinterpret_cast<uint4*>(img + t4 * Cfg::kImgBytes + ib) = *reinterpret_cast<const uint4*>(tg + gb);
+      }
+    }
 
     // ---- stage the A operand rows of this thread's token and start the first product
     float inv_s;
@@ -368,14 +397,15 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
     const unsigned short n_h = f32_to_f16_bits_clamped(n * inv_s * 0.0625f);  // y = 16 s PI x
 
     if constexpr (kKey) {
-      // ---- pass 2: codes, residual (the A operand of the S product), canonical pair-field string into `row`
+      // ---- pass 2: codes, residual (the A operand of the S product); the pair fields go straight into the tile image:
+      //      pair p = 16 c + g belongs to lane (sg, t = g & 3) as field j = 4 c + (g >> 2) of this token's block
+      //      (bits [6 J sr + 6 j, + 6) of the lane's string): four fields = three bytes per lane and chunk
       float g2 = 0.f;
 #pragma unroll 1
       for (int c = 0; c < D / 32; ++c) {
         float y[32];
         tmem_ld32(t_lane + 32 * c, y);
-        unsigned long long lo64 = 0ull;  // 16 fields = 96 bits: bits [0,64) here, [64,96) in hi32
-        unsigned hi32 = 0u;
+        unsigned yt[4] = {0u, 0u, 0u, 0u};
 #pragma unroll
         for (int g = 0; g < 16; ++g) {
           const float u0 = y[2 * g] * inv, u1 = y[2 * g + 1] * inv;
@@ -383,12 +413,16 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
           const float r0 = u0 - lut_s[c0], r1 = u1 - lut_s[c1];
           g2 = fmaf(r0, r0, fmaf(r1, r1, g2));
           y[2 * g] = r0 * 8.f, y[2 * g + 1] = r1 * 8.f;  // scaled for the fp16 split (only sign(S r) is used)
-          const unsigned long long f = (unsigned long long)(c0 | (c1 << 3));
-          const int bit = 6 * g;
-          if (bit < 64) lo64 |= f << bit;
-          if (bit + 6 > 64) hi32 |= bit >= 64 ? (unsigned)f << (bit - 64) : (unsigned)(f >> (64 - bit));
+          yt[g & 3] |= (unsigned)(c0 | (c1 << 3)) << (6 * (g >> 2));
         }
-        row[3 * c] = (unsigned)lo64, row[3 * c + 1] = (unsigned)(lo64 >> 32), row[3 * c + 2] = hi32;
+        if (valid) {
+#pragma unroll
+          for (int t = 0; t < 4; ++t) {
+            const int sb = (6 * Lo::J * sr) / 8 + 3 * c;  // byte of the lane's K string
+#pragma unroll
+            for (int k = 0; k < 3; ++k) timg[sec_byte(KCW, 4 * sg + t, sb + k)] = (unsigned char)(yt[t] >> (8 * k));
+          }
+        }
 #pragma unroll
         for (int kj = 0; kj < 4; ++kj) {  // the first product is complete (barrier): the A buffers are free
           uint4 hi, lo;
@@ -405,32 +439,12 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
         gemm(D, a_hi, b1_hi, true), gemm(D, a_lo, b1_hi, false), gemm(D, a_hi, b1_lo, false);
         umma_commit(smem_u32(mbar + 1));
       }
-      // device layout: the token in slot t stores pair group g at field position (g - t) mod P, i.e. the canonical
-      // string rotated right by 6 t bits; the word part of the rotation is a runtime index into this thread's row
-      {
-        const int wa = (6 * slot) >> 5, wb = (6 * slot) & 31;
-        unsigned o[KCW];
-        unsigned prev = row[wa];
-#pragma unroll
-        for (int w = 0; w < KCW; ++w) {
-          int idx = wa + w + 1;
-          idx = idx >= KCW ? idx - KCW : idx;
-          const unsigned next = row[idx];
-          o[w] = __funnelshift_r(prev, next, wb);
-          prev = next;
-        }
-        if (valid) {
-#pragma unroll
-          for (int c4 = 0; c4 < KCW / 4; ++c4)
-            *reinterpret_cast<uint4*>(tp + Lo::kOffKC + c4 * 16 * kTile + slot * 16) =
-                make_uint4(o[4 * c4], o[4 * c4 + 1], o[4 * c4 + 2], o[4 * c4 + 3]);
-          if constexpr (KCW % 4 == 2)
-            *reinterpret_cast<uint2*>(tp + Lo::kOffKC + (KCW / 4) * 16 * kTile + slot * 8) = make_uint2(o[KCW - 2], o[KCW - 1]);
-          reinterpret_cast<unsigned short*>(tp + Lo::kOffKN)[slot] = n_h;
-          reinterpret_cast<unsigned short*>(tp + Lo::kOffKR)[slot] = f32_to_f16_bits_clamped(sqrtf(g2));
-        }
-      }
-      // ---- residual sketch: bit j = [(S r)_j >= 0]; nibble group n sits at nibble position (n - t) mod (d/4)
+      if (valid)
+        reinterpret_cast<unsigned*>(timg + kOffImgNK)[slot_lane(slot)] =
+            (unsigned)n_h | ((unsigned)f32_to_f16_bits_clamped(sqrtf(g2)) << 16);
+      // ---- residual sketch: bit j = [(S r)_j >= 0].  Sketch rows [t d/4, (t+1) d/4) belong to lane (sg, t) as 16-bit
+      //      pieces u; a piece is stored as two bytes of word (mt, u): byte (sr & 1) holds bits 0..7, byte 2 + (sr & 1)
+      //      bits 8..15 (the byte interleave with the slot 8 further on makes the decode kernel's fp16x2 masks work)
       mbar_wait(smem_u32(mbar + 1), parity);
       tc_fence_after();
 #pragma unroll 1
@@ -440,73 +454,100 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
         unsigned w = 0u;
 #pragma unroll
         for (int j = 0; j < 32; ++j) w |= (y[j] >= 0.f ? 1u : 0u) << j;
-        row[c] = w;
-      }
-      {
-        const int rs = (4 * slot) & (D - 1), wa = rs >> 5, wb = rs & 31;
-        unsigned o[KSW];
-        unsigned prev = row[wa];
-#pragma unroll
-        for (int w = 0; w < KSW; ++w) {
-          int idx = wa + w + 1;
-          idx = idx >= KSW ? idx - KSW : idx;
-          const unsigned next = row[idx];
-          o[w] = __funnelshift_r(prev, next, wb);
-          prev = next;
-        }
         if (valid) {
-          if constexpr (KSW == 2) *reinterpret_cast<uint2*>(tp + Lo::kOffKS + slot * 8) = make_uint2(o[0], o[1]);
-          else *reinterpret_cast<uint4*>(tp + Lo::kOffKS + slot * 16) = make_uint4(o[0], o[1], o[2], o[3]);
+#pragma unroll
+          for (int q = 0; q < 2; ++q) {
+            const int rho0 = 32 * c + 16 * q, t = rho0 / (D / 4), u = (rho0 % (D / 4)) >> 4;
+            const int word = (sr >> 1) * Lo::U + u;
+            unsigned char* wp = timg + kOffImgKS + word_offset(KSW, word, 4 * sg + t);
+            wp[sr & 1] = (unsigned char)(w >> (16 * q));
+            wp[2 + (sr & 1)] = (unsigned char)(w >> (16 * q + 8));
+          }
         }
       }
     } else {
-      // ---- values, pass 2: codes as pair fields; the cache stores them per coordinate pair across the tile's tokens
+      // ---- values, pass 2: codes, eight per scratch word; then the two tokens of a pair assemble the six-bit fields
+      //      code_i(even token) | code_i(odd token) << 3 of lane (i & 7, pp & 3), block j = pp >> 2: the even token
+      //      builds the lanes i & 7 < 4, the odd one the others
+      unsigned* myg = vscr + tid * Cfg::kScrPitch;
 #pragma unroll 1
       for (int c = 0; c < D / 32; ++c) {
         float y[32];
         tmem_ld32(t_lane + 32 * c, y);
 #pragma unroll
-        for (int g4 = 0; g4 < 4; ++g4) {  // four pair fields per 32-bit shared-memory store
+        for (int q = 0; q < 4; ++q) {
           unsigned w = 0;
 #pragma unroll
-          for (int j = 0; j < 4; ++j) {
-            const int g = 4 * g4 + j;
-            const int c0 = code_of(y[2 * g] * inv, thr), c1 = code_of(y[2 * g + 1] * inv, thr);
-            w |= (unsigned)(c0 | (c1 << 3)) << (8 * j);
-          }
-          reinterpret_cast<unsigned*>(cbV + tid * P + 16 * c)[g4] = w;
+          for (int i = 0; i < 8; ++i) w |= (unsigned)code_of(y[8 * q + i] * inv, thr) << (3 * i);
+          myg[4 * c + q] = w;
         }
       }
-      if (valid) reinterpret_cast<unsigned short*>(tp + Lo::kOffVN)[slot] = n_h;
-      __syncthreads();
-      {  // thread = (tile of the block, lane): KCW words of six-bit fields, lane g owns pair groups g (+32); tokens of
-         // the tile that are outside this call keep their bits (read-modify-write under a mask)
-        const int tl = tid >> 5, lane = tid & 31;
-        const int tile_pos = blk * kBlk + tl * kTile;
-        unsigned char* tpv = stream + (size_t)(tile_pos / kTile) * Lo::kTileBytes;
-        const int j_first = max(0, a.start_pos - tile_pos), j_end = min(kTile, a.start_pos + a.n_tokens - tile_pos);
-        if (j_first < j_end) {
+      if (valid) reinterpret_cast<unsigned short*>(timg + kOffImgVN)[slot_lane(slot)] = n_h;
+      __syncwarp();
+      {
+        const int e = slot & 1, pp = slot >> 1;
+        const unsigned* ge = vscr + (tid & ~1) * Cfg::kScrPitch;  // even token of the pair
+        const unsigned* go = ge + Cfg::kScrPitch;                 // odd token
+        const bool v_e = __shfl_sync(0xffffffffu, valid, (slot & ~1)), v_o = __shfl_sync(0xffffffffu, valid, (slot | 1));
+        if (v_e || v_o) {
+          constexpr int HW = 3 * D / 64;  // halfwords per (lane, token pair) block
 #pragma unroll
-          for (int w = 0; w < KCW; ++w) {
-            const int part = (32 * w) / 192, sb = 32 * w - 192 * part;
-            const int g = lane + kTile * part;
-            unsigned long long word = 0, mask = 0;
+          for (int gq = 0; gq < 4; ++gq) {
+            const int gi = 4 * e + gq;
+            unsigned short hw16[HW];
 #pragma unroll
-            for (int j = sb / 6; j <= (sb + 31) / 6 && j < kTile; ++j) {
-              if (j < j_first || j >= j_end) continue;
-              const unsigned long long f = cbV[(tl * kTile + j) * P + g];
-              const int sh = 6 * j - sb;
-              word |= sh >= 0 ? (f << sh) : (f >> (-sh));
-              mask |= sh >= 0 ? (63ull << sh) : (63ull >> (-sh));
+            for (int h = 0; h < HW; ++h) hw16[h] = 0;
+            unsigned long long acc = 0ull;  // fields stream through a 64-bit window, 16 bits out at a time
+            int nbits = 0, hout = 0;
+#pragma unroll
+            for (int c = 0; c < Lo::C; ++c) {
+              const unsigned f = ((ge[c] >> (3 * gi)) & 7u) | (((go[c] >> (3 * gi)) & 7u) << 3);
+              acc |= (unsigned long long)f << nbits;
+              nbits += 6;
+              if (nbits >= 16) {
+                hw16[hout++] = (unsigned short)acc;
+                acc >>= 16, nbits -= 16;
+              }
             }
-            unsigned* p = reinterpret_cast<unsigned*>(tpv + Lo::kOffVC + word_offset(KCW, w, lane));
-            const unsigned m32 = (unsigned)mask;
-            if (m32 == 0xffffffffu) *p = (unsigned)word;
-            else if (m32) *p = (*p & ~m32) | ((unsigned)word & m32);
+            const unsigned short keep_mask = (v_e && v_o) ? 0u : 0xffffu;  // partial pair: read-modify-write
+#pragma unroll
+            for (int h = 0; h < HW; ++h) {
+              const int hidx = (pp >> 2) * HW + h;
+              unsigned short* dst =
+                  reinterpret_cast<unsigned short*>(timg + word_offset(KCW, hidx >> 1, 4 * gi + (pp & 3))) + (hidx & 1);
+              if (keep_mask) {
+                // bits of the valid token inside this halfword: three of every six, phase by the bit offset 16 h
+                unsigned short m = 0;
+#pragma unroll
+                for (int bit = 0; bit < 16; ++bit) {
+                  const int fb = (16 * h + bit) % 6;
+                  if ((fb < 3) == v_e) m |= (unsigned short)(1u << bit);
+                }
+                *dst = (unsigned short)((*dst & ~m) | (hw16[h] & m));
+              } else {
+                *dst = hw16[h];
+              }
+            }
           }
         }
       }
     }
+    // ---- write the block's tile images out (every tile the call touches; the image of a partly covered tile carries
+    //      the old bits of the other tokens)
+    __syncthreads();
+    {
+      constexpr int kOwn = kKey ? Cfg::kImgK : Cfg::kImgV;
+      for (int idx = tid; idx < 4 * (kOwn / 16); idx += kBlk) {
+        const int t4 = idx / (kOwn / 16), q = idx % (kOwn / 16);
+        if (tile_cover(t4) == 0) continue;
+        unsigned char* tg = stream + (size_t)(blk * 4 + t4) * Lo::kTileBytes;
+        const int ib = 16 * q;
+        const int gb = kKey ? (ib < Lo::kOffVC ? ib : Lo::kOffNK + (ib - Lo::kOffVC))
+                            : (ib < Lo::kCodeBytes ? Lo::kOffVC + ib : Lo::kOffVN + (ib - Lo::kCodeBytes));
+        *reinterpret_cast<uint4*>(tg + gb) = *reinterpret_cast<const uint4*>(img + t4 * Cfg::kImgBytes + ib);
+      }
+    }
+    __syncthreads();  // the next block pre-loads into / writes the same images
     tc_fence_before();  // the next block's MMAs overwrite the accumulators every thread has just read
   }
   __syncthreads();
