@@ -1,24 +1,27 @@
 """bench.py — headline measurement of the TurboESM hot path on B200 (contract: DESIGN.md "Measurement").
 
-Workload: BASELINE.json:configs[2] — ESM-2-650M-shaped batched decode: 33 layers x batch 32 x 20 heads,
-head_dim 64, 1024 cached tokens, fp16 Student-t(4) activations with 2 outlier channels per head; every
-decode step appends one quantised token per head (tq_append) and runs the fused decode attention
-(tq_decode_attn) for every layer.  A "step" is one model decode step = 33 x (append + decode).
+Default workload: BASELINE.json:configs[2] — ESM-2-650M-shaped batched decode: 33 layers x batch 32 x 20 heads,
+head_dim 64, 1024 cached tokens, fp16 Student-t(4) activations with 2 outlier channels per head; every decode step
+appends one quantised token per head and runs the fused decode attention for every layer.  A "step" is one model
+decode step = 33 x (append + decode) through tq_decode_model_step.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--layers L]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--layers L] [--config cfg1|cfg2|cfg3|cfg4]
 
 value     : cached token-heads attended per second (L*B*H*T per step / step time), inputs resident in HBM,
-            the 33-layer step replayed as one CUDA graph.
+            the step replayed as one CUDA graph.
 e2e       : same metric through tq_decode_model_step_host with pinned HOST q/k/v/out buffers (copies inside).
 roofline  : fused decode kernel, algorithmic packed bytes (62 B per cached token-head) / its average launch
             duration measured live with CUDA events, against MEASURED_PEAKS.json hbm_gbs.
 cpu_baseline : the CPU oracle (oracle/, as it stands) timed on this box's host cores on a bounded sample.
+--config cfg1|cfg3|cfg4 : the other BASELINE.json configs (prefill quantize/pack GB/s and decode tokens/s), one line each.
 """
 from __future__ import annotations
 
 import argparse
+import glob
 import json
 import os
+import re
 import statistics
 import subprocess
 import sys
@@ -36,7 +39,7 @@ from paper_2603_26110_b200 import workloads as W
 METRIC = "fused 3-bit decode-attn cached tokens/s"
 UNIT = "cached token-heads/s"
 FALLBACK_HBM_GBS = 6650.0  # B200_PROFILING.md fallback
-NCU_DRAM_BYTES_PER_LAUNCH = 42.63e6  # decode_main_kernel, one ncu --set full capture (profiles/r01b_decode_main_full.md)
+CONFIG_NAMES = {"cfg1": "cfg1_650m_step", "cfg2": "cfg2_650m_batch32", "cfg3": "cfg3_long_splitk", "cfg4": "cfg4_15b_heads"}
 
 
 def measured_peaks():
@@ -48,6 +51,17 @@ def measured_peaks():
         except Exception:
             pass
     return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def ncu_traffic(kernel_tag: str):
+    """DRAM bytes per launch of the dominant kernel from the newest committed `ncu --set full` summary
+    (profiles/r*_<kernel_tag>_full.md, line `dram_bytes_per_launch: N`); None when no capture of this round exists."""
+    best = None
+    for f in sorted(glob.glob(os.path.join(ROOT, "profiles", f"r*_{kernel_tag}_full.md"))):
+        m = re.search(r"dram_bytes_per_launch:\s*([0-9.eE+]+)", open(f).read())
+        if m:
+            best = (float(m.group(1)), os.path.relpath(f, ROOT))
+    return best
 
 
 class ClockSampler:
@@ -118,83 +132,95 @@ def torch_activations(w: W.Workload, layer: int, shape, device, gen):
     return out
 
 
-# ------------------------------------------------------------------------------------------ reference arm
+def bytes_per_token_head(d: int) -> int:
+    return 62 if d == 64 else 118
+
+
+# ------------------------------------------------------------------------------------------ oracle legs
+def oracle_sample(w: W.Workload, sb: int):
+    from oracle import tq_oracle as O
+    import math
+
+    O.build()
+    ws = w.scaled(n_layers=1, batch=sb)
+    pi_k, pi_v = W.rotations(ws)
+    S = W.sketch(ws)
+    lut = O.lloyd_max_gauss(1.0 / math.sqrt(w.head_dim), 8)[0].astype(np.float32)
+    luts = np.tile(lut, (w.n_heads, 1))
+    k, v = W.layer_activations(ws, 0)
+    q = W.queries(ws, 0)
+    return O, ws, pi_k, pi_v, S, luts, k, v, q
+
+
 def run_reference(args, w: W.Workload):
     """--impl reference: the CPU oracle, as it stands, on this box's host cores.  Each step decodes a bounded
     sample of the workload (a few batch entries of one layer)."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    from oracle import tq_oracle as O
-    import math
-
-    O.build()
     sb = 2  # batch entries per sampled step
-    ws = w.scaled(n_layers=1, batch=sb)
-    pi_k, pi_v = W.rotations(ws)
-    S = W.sketch(ws)
-    lut = O.lloyd_max_gauss(1.0 / math.sqrt(w.head_dim), 8)[0].astype(np.float32)
-    luts = np.tile(lut, (w.n_heads, 1))
-    k, v = W.layer_activations(ws, 0)
+    tcap = min(w.seq, 4096)  # bounded sample of long contexts
+    O, ws, pi_k, pi_v, S, luts, k, v, q = oracle_sample(w.scaled(seq=tcap), sb)
     t0 = time.perf_counter()
     can = O.quantize_pack(k, v, pi_k[0], pi_v[0], luts, luts, S)
     tq_s = time.perf_counter() - t0
-    q = W.queries(ws, 0)
-    sl = np.full(sb, w.seq, np.int32)
+    sl = np.full(sb, tcap, np.int32)
     for _ in range(args.warmup):
         O.decode_attn(q, sl - 1, sl, pi_k[0], pi_v[0], luts, luts, S, can)
     t0 = time.perf_counter()
     for _ in range(args.steps):
         O.decode_attn(q, sl - 1, sl, pi_k[0], pi_v[0], luts, luts, S, can)
     dt = time.perf_counter() - t0
-    th = sb * w.n_heads * w.seq * args.steps
+    th = sb * w.n_heads * tcap * args.steps
     value = th / dt
-    sample = f"decode of {sb} batch entries x {w.n_heads} heads x {w.seq} tokens of one layer per step"
+    sample = f"decode of {sb} batch entries x {w.n_heads} heads x {tcap} tokens of one layer per step"
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": w.name, "sample": sample},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle", "sample": sample,
-                         "quantize_pack_vectors_per_s": 2 * sb * w.n_heads * w.seq / tq_s},
+                         "quantize_pack_vectors_per_s": 2 * sb * w.n_heads * tcap / tq_s},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
     print(json.dumps(line))
 
 
-# ------------------------------------------------------------------------------------------ CPU baseline leg
 def cpu_baseline(w: W.Workload):
-    """The oracle as it stands on this box's host cores, bounded sample (rank 0, N = 1 only)."""
-    from oracle import tq_oracle as O
-    import math
-
-    O.build()
+    """The oracle as it stands on this box's host cores, bounded sample (rank 0, N = 1 only): all cores (OpenMP over
+    units) and one thread."""
     sb = 4
-    ws = w.scaled(n_layers=1, batch=sb)
-    pi_k, pi_v = W.rotations(ws)
-    S = W.sketch(ws)
-    lut = O.lloyd_max_gauss(1.0 / math.sqrt(w.head_dim), 8)[0].astype(np.float32)
-    luts = np.tile(lut, (w.n_heads, 1))
-    k, v = W.layer_activations(ws, 0)
+    tcap = min(w.seq, 2048)
+    O, ws, pi_k, pi_v, S, luts, k, v, q = oracle_sample(w.scaled(seq=tcap), sb)
     t0 = time.perf_counter()
     can = O.quantize_pack(k, v, pi_k[0], pi_v[0], luts, luts, S)
     tq_s = time.perf_counter() - t0
-    q = W.queries(ws, 0)
-    sl = np.full(sb, w.seq, np.int32)
-    O.decode_attn(q, sl - 1, sl, pi_k[0], pi_v[0], luts, luts, S, can)
-    reps, t0 = 0, time.perf_counter()
-    while time.perf_counter() - t0 < 8.0 and reps < 200:
+    sl = np.full(sb, tcap, np.int32)
+    ncores = O.num_threads()
+
+    def timed(budget_s):
         O.decode_attn(q, sl - 1, sl, pi_k[0], pi_v[0], luts, luts, S, can)
-        reps += 1
-    dt = time.perf_counter() - t0
-    nvec = 2 * sb * w.n_heads * w.seq
+        reps, t0 = 0, time.perf_counter()
+        while time.perf_counter() - t0 < budget_s and reps < 200:
+            O.decode_attn(q, sl - 1, sl, pi_k[0], pi_v[0], luts, luts, S, can)
+            reps += 1
+        return sb * w.n_heads * tcap * reps / (time.perf_counter() - t0), reps
+
+    v_all, reps = timed(6.0)
+    O.set_num_threads(1)
+    try:
+        v_one, reps1 = timed(4.0)
+    finally:
+        O.set_num_threads(ncores)
+    nvec = 2 * sb * w.n_heads * tcap
     in_bytes = nvec * w.head_dim * 2
     return {
-        "value": sb * w.n_heads * w.seq * reps / dt, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle",
-        "sample": f"{reps} decode passes over {sb} batch entries x {w.n_heads} heads x {w.seq} tokens of one layer "
+        "value": v_all, "unit": UNIT, "cores": ncores, "kind": "oracle",
+        "sample": f"{reps} decode passes over {sb} batch entries x {w.n_heads} heads x {tcap} tokens of one layer "
                   f"(fp64, OpenMP over units); quantize/pack of the same {nvec} vectors once",
-        "quantize_pack_gbs": (in_bytes + nvec / 2 * 62) / tq_s / 1e9,
+        "single_thread_value": v_one, "single_thread_passes": reps1,
+        "quantize_pack_gbs": (in_bytes + nvec / 2 * bytes_per_token_head(w.head_dim)) / tq_s / 1e9,
         "quantize_pack_s": tq_s,
     }
 
@@ -217,12 +243,84 @@ def whole_job_value(tok_heads_per_rank: int, world: int, ms_max: float) -> float
     return world * tok_heads_per_rank / (ms_max * 1e-3)
 
 
-def run_ours(args, w: W.Workload):
+class Rig:
+    """Device-side state shared by the measurement legs of one workload."""
+
+    def __init__(self, w: W.Workload, L: int, max_seq: int, rank: int, local: int):
+        import torch
+        from paper_2603_26110_b200 import binding as tq
+
+        self.torch, self.tq, self.w, self.L = torch, tq, w, L
+        self.dev = torch.device("cuda", local)
+        self.B, self.H, self.d, self.T0 = w.batch, w.n_heads, w.head_dim, w.seq
+        self.max_seq = max_seq
+        self.shape = tq.make_shape(L, self.B, self.H, self.d, max_seq, w.rope_base, 0)
+        self.wl = w.scaled(n_layers=L)
+        cal = tq.tq_calibrate_host(self.shape, 1, seed=w.seed + rank)  # QR-of-Gaussian PI per (layer, head), Lloyd-Max LUT, S
+        self.params = tq.Params(cal, self.dev)
+        self.cache = tq.Cache(self.shape, self.dev)
+        self.gen = torch.Generator(device=self.dev)
+        self.gen.manual_seed(w.seed + 1000 * rank)
+        self.stream = torch.cuda.Stream(self.dev)
+        self.bpt = bytes_per_token_head(self.d)
+
+    def ev(self):
+        return self.torch.cuda.Event(enable_timing=True)
+
+    def prefill(self):
+        """tq_quantize_pack of T0 tokens into every layer cache, each launch timed; returns (ms list, bytes per layer)."""
+        q_ms = []
+        with self.torch.cuda.stream(self.stream):
+            for layer in range(self.L):
+                k, v = torch_activations(self.wl, layer, (self.B, self.H, self.T0, self.d), self.dev, self.gen)
+                e0, e1 = self.ev(), self.ev()
+                e0.record(self.stream)
+                self.tq.tq_quantize_pack(self.shape, self.params, self.cache, layer, k, v, 0, self.stream)
+                e1.record(self.stream)
+                e1.synchronize()
+                q_ms.append(e0.elapsed_time(e1))
+                del k, v
+        esz = 2 if self.w.dtype == "f16" else 4
+        q_bytes = 2 * self.B * self.H * self.T0 * self.d * esz + self.B * self.H * self.T0 * self.bpt
+        return q_ms, q_bytes
+
+    def step_inputs(self):
+        qs, kn, vn = [], [], []
+        for layer in range(self.L):
+            a, b_ = torch_activations(self.wl, layer, (self.B, self.H, self.d), self.dev, self.gen)
+            c_, _ = torch_activations(self.wl, layer, (self.B, self.H, self.d), self.dev, self.gen)
+            qs.append(a), kn.append(b_), vn.append(c_)
+        t = self.torch
+        return t.stack(qs), t.stack(kn), t.stack(vn)
+
+    def graph_us(self, body, per: int, reps: int = 6, before=None):
+        """Capture body() as a CUDA graph on self.stream and return the mean replay time / per, in microseconds."""
+        t = self.torch
+        with t.cuda.stream(self.stream):
+            if before:
+                before()
+            body()
+            self.stream.synchronize()
+            g = t.cuda.CUDAGraph()
+            with t.cuda.graph(g, stream=self.stream):
+                body()
+            ts = []
+            for it in range(reps):
+                if before:
+                    before()
+                e0, e1 = self.ev(), self.ev()
+                e0.record(self.stream)
+                g.replay()
+                e1.record(self.stream)
+                e1.synchronize()
+                if it > 0:
+                    ts.append(e0.elapsed_time(e1) / per * 1e3)
+        return statistics.mean(ts)
+
+
+def init_dist():
     import torch
     import torch.distributed as dist
-
-    from paper_2603_26110_b200 import binding as tq
-    from paper_2603_26110_b200 import build as tqbuild
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -232,58 +330,45 @@ def run_ours(args, w: W.Workload):
     torch.cuda.set_device(local)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    from paper_2603_26110_b200 import binding as tq
+    from paper_2603_26110_b200 import build as tqbuild
+
     if rank == 0:
         tqbuild.build()
     if world > 1:
         dist.barrier()
     tq.lib()
-    dev = torch.device("cuda", local)
+    return rank, world, local
 
-    L, B, H, d, T0 = args.layers, w.batch, w.n_heads, w.head_dim, w.seq
-    max_seq = T0 + 128
-    shape = tq.make_shape(L, B, H, d, max_seq, w.rope_base, 0)
-    wl = w.scaled(n_layers=L)
-    cal = tq.tq_calibrate_host(shape, 1, seed=w.seed + rank)  # QR-of-Gaussian PI per (layer, head), Lloyd-Max LUT, S
-    params = tq.Params(cal, dev)
-    cache = tq.Cache(shape, dev)
-    ws = tq.Workspace(shape, 1, dev)
-    gen = torch.Generator(device=dev)
-    gen.manual_seed(w.seed + 1000 * rank)
+
+def run_cfg2(args, w: W.Workload):
+    import torch
+    import torch.distributed as dist
+
+    rank, world, local = init_dist()
+    from paper_2603_26110_b200 import binding as tq
+
+    L = args.layers
+    rig = Rig(w, L, w.seq + 128, rank, local)
+    B, H, d, T0, dev, stream, shape, params, cache = rig.B, rig.H, rig.d, rig.T0, rig.dev, rig.stream, rig.shape, rig.params, rig.cache
+    max_seq = rig.max_seq
     dt_code = tq.TQ_F16
-    stream = torch.cuda.Stream(dev)
 
     # ---- prefill: quantize/pack every layer (timed separately: quantize/pack GB/s)
-    ev = lambda: torch.cuda.Event(enable_timing=True)
-    q_ms = []
-    with torch.cuda.stream(stream):
-        for layer in range(L):
-            k, v = torch_activations(wl, layer, (B, H, T0, d), dev, gen)
-            e0, e1 = ev(), ev()
-            e0.record(stream)
-            tq.tq_quantize_pack(shape, params, cache, layer, k, v, 0, stream)
-            e1.record(stream)
-            e1.synchronize()
-            q_ms.append(e0.elapsed_time(e1))
-            del k, v
-    q_bytes = 2 * B * H * T0 * d * 2 + B * H * T0 * 62
+    q_ms, q_bytes = rig.prefill()
     quant_gbs = q_bytes / (statistics.median(q_ms) * 1e-3) / 1e9
 
     # ---- per-step inputs, resident on the device: [L][B][H][d]
-    qs, kn, vn = [], [], []
-    for layer in range(L):
-        a, b_ = torch_activations(wl, layer, (B, H, d), dev, gen)
-        c_, _ = torch_activations(wl, layer, (B, H, d), dev, gen)
-        qs.append(a), kn.append(b_), vn.append(c_)
-    qs, kn, vn = torch.stack(qs), torch.stack(kn), torch.stack(vn)
+    qs, kn, vn = rig.step_inputs()
     outs = torch.empty_like(qs)
+    wsL = tq.Workspace(shape, L, dev)
+    ws1 = tq.Workspace(shape, 1, dev)
 
     def reset_len():
         cache.seq_len.fill_(T0)
 
-    def one_step():
-        for layer in range(L):  # tq_decode_step == tq_append followed by tq_decode_attn, two launches per layer
-            tq.tq_decode_step(shape, params, cache, layer, qs[layer], kn[layer], vn[layer], outs[layer], ws, max_seq,
-                              stream)
+    def one_step():  # one model decode step: append + fused decode attention for every layer
+        tq.tq_decode_model_step(shape, params, cache, 0, L, qs, kn, vn, outs, wsL, max_seq, stream)
 
     # ---- capture one model decode step as a CUDA graph (seq_len lives on the device, so it replays)
     with torch.cuda.stream(stream):
@@ -299,14 +384,14 @@ def run_ours(args, w: W.Workload):
 
     steps_per_fill = 100  # capacity: T0 .. T0+127
 
-    def run_steps(n, timed):
+    def run_steps(n):
         """n graph replays; seq_len is rewound every 100 steps so the cache never overflows."""
         done, total_ms, tok_heads = 0, 0.0, 0
         while done < n:
             chunk = min(steps_per_fill, n - done)
             with torch.cuda.stream(stream):
                 reset_len()
-                e0, e1 = ev(), ev()
+                e0, e1 = rig.ev(), rig.ev()
                 e0.record(stream)
                 for _ in range(chunk):
                     graph.replay()
@@ -318,78 +403,66 @@ def run_ours(args, w: W.Workload):
             done += chunk
         return total_ms, tok_heads
 
-    run_steps(max(args.warmup, 3), False)
+    run_steps(max(args.warmup, 3))
     if world > 1:
         dist.barrier()
     torch.cuda.synchronize()
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
-    ms, tok_heads = run_steps(args.steps, True)
+    ms, tok_heads = run_steps(args.steps)
     torch.cuda.synchronize()
     if world > 1:
         dist.barrier()
     clocks = sampler.stop() if rank == 0 else None
     assert int(cache.status.item()) == 0, "an append was refused during the timed region"
 
-    # ---- live duration of the decode call (query prep + streaming kernel) measured with CUDA events on
-    #      `stream`: one tq_decode_attn per layer over all L layer caches (L x 40.6 MB, larger than L2),
-    #      captured as a CUDA graph so that the host's launch cost does not bound the measurement
+    dec_bytes = B * H * T0 * rig.bpt  # algorithmic packed bytes of one streaming-kernel launch at T0 tokens
+
+    # ---- the same work as a real model must order it: tq_decode_step layer by layer (append + query prep kernel, then the
+    #      streaming kernel, each layer waiting for the one before)
+    def seq_step():
+        for layer in range(L):
+            tq.tq_decode_step(shape, params, cache, layer, qs[layer], kn[layer], vn[layer], outs[layer], ws1, max_seq, stream)
+
+    seq_us = rig.graph_us(seq_step, L, before=reset_len)
+
+    # ---- the decode call alone (query prep + streaming kernel), one tq_decode_attn per layer cache
+    def decode_all_layers():
+        for layer in range(L):
+            tq.tq_decode_attn(shape, params, cache, layer, 1, qs[layer:layer + 1], outs[layer:layer + 1], ws1, None, max_seq, stream)
+
+    reset_len()
+    call_us = rig.graph_us(decode_all_layers, L)
+
+    # ---- the dominant kernel (decode_main_kernel) with the library's measurement hook on (query operands of the preceding
+    #      ordinary call are re-used): (a) as the model step launches it — one launch per layer cache, a run-ahead chain,
+    #      plus the one finish kernel; (b) one launch per layer cache, each waiting for the one before (isolated launches)
     with torch.cuda.stream(stream):
         reset_len()
-
-        def decode_all_layers():
-            for layer in range(L):
-                tq.tq_decode_attn(shape, params, cache, layer, 1, qs[layer:layer + 1], outs[layer:layer + 1], ws, None,
-                                  max_seq, stream)
-
-        decode_all_layers()
+        one_step()
         stream.synchronize()
-        dgraph = torch.cuda.CUDAGraph()
-        with torch.cuda.graph(dgraph, stream=stream):
-            decode_all_layers()
-        dec_ms = []
-        for it in range(6):
-            e0, e1 = ev(), ev()
-            e0.record(stream)
-            dgraph.replay()
-            e1.record(stream)
-            e1.synchronize()
-            if it > 0:
-                dec_ms.append(e0.elapsed_time(e1) / L)
-    dec_bytes = B * H * T0 * 62
-    dec_s = statistics.mean(dec_ms) * 1e-3
+    reset_len()
+    tq.tq_profile_decode_main_only(True)
+    try:
+        chain_us = rig.graph_us(one_step, L)
+    finally:
+        tq.tq_profile_decode_main_only(False)
+    wss = [tq.Workspace(shape, 1, dev) for _ in range(L)]  # one workspace per layer keeps every layer's operands alive
 
-    # ---- the dominant kernel alone (decode_main_kernel): the same per-layer calls with the library's measurement hook
-    #      on (only the streaming kernel is launched, the rotated queries of the calls above are still in the
-    #      per-layer workspaces), one launch per layer cache, replayed from a graph between one CUDA event pair
+    def decode_all_layers_ws():
+        for layer in range(L):
+            tq.tq_decode_attn(shape, params, cache, layer, 1, qs[layer:layer + 1], outs[layer:layer + 1], wss[layer], None,
+                              max_seq, stream)
+
     with torch.cuda.stream(stream):
-        wss = [tq.Workspace(shape, 1, dev) for _ in range(L)]  # one workspace per layer keeps every layer's q'' alive
-
-        def decode_all_layers_ws():
-            for layer in range(L):
-                tq.tq_decode_attn(shape, params, cache, layer, 1, qs[layer:layer + 1], outs[layer:layer + 1], wss[layer],
-                                  None, max_seq, stream)
-
-        decode_all_layers_ws()  # ordinary calls: query preparation + streaming kernel
-        stream.synchronize()
-        tq.tq_profile_decode_main_only(True)
         decode_all_layers_ws()
         stream.synchronize()
-        mgraph = torch.cuda.CUDAGraph()
-        with torch.cuda.graph(mgraph, stream=stream):
-            decode_all_layers_ws()
+    tq.tq_profile_decode_main_only(True)
+    try:
+        iso_us = rig.graph_us(decode_all_layers_ws, L)
+    finally:
         tq.tq_profile_decode_main_only(False)
-        main_ms = []
-        for it in range(6):
-            e0, e1 = ev(), ev()
-            e0.record(stream)
-            mgraph.replay()
-            e1.record(stream)
-            e1.synchronize()
-            if it > 0:
-                main_ms.append(e0.elapsed_time(e1) / L)
-    main_s = statistics.mean(main_ms) * 1e-3
 
     # ---- end to end through the host-buffer call: pinned q/k/v in, out back, every layer of every step
     e2e_steps = max(3, min(args.steps, 20))
@@ -398,8 +471,8 @@ def run_ours(args, w: W.Workload):
     qh, kh, vh = qs.cpu().pin_memory(), kn.cpu().pin_memory(), vn.cpu().pin_memory()
     oh = torch.empty_like(qh).pin_memory()
 
-    def e2e_step():  # one model decode step: pinned q/k/v of all L layers in, L x (append + decode), outputs back, sync
-        tq.tq_decode_model_step_host(shape, params, cache, 0, L, qh, kh, vh, oh, staging, ws, max_seq, stream)
+    def e2e_step():  # one model decode step: pinned q/k/v of all L layers in, the step, outputs back, sync
+        tq.tq_decode_model_step_host(shape, params, cache, 0, L, qh, kh, vh, oh, staging, wsL, max_seq, stream)
 
     with torch.cuda.stream(stream):
         reset_len()
@@ -422,8 +495,10 @@ def run_ours(args, w: W.Workload):
             dist.destroy_process_group()
         return
     peak, peak_src = measured_peaks()
-    achieved = dec_bytes / main_s / 1e9
+    achieved = dec_bytes / (chain_us * 1e-6) / 1e9
     value = whole_job_value(tok_heads, world, ms_max)
+    traffic = ncu_traffic("decode_main")
+    us_layer = 1e3 * ms_max / args.steps / L
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
         "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -432,13 +507,18 @@ def run_ours(args, w: W.Workload):
             "workload": f"{w.name} (BASELINE.json configs[2]) x {L} layers: batch {B} x {H} heads x d {d}, "
                         f"{T0}+ cached tokens, fp16 Student-t(4) + 2 outlier channels x15, append + decode per layer per step",
             "layers": L, "batch_per_gpu": B, "heads": H, "head_dim": d, "cached_tokens": T0, "io_dtype": "f16",
-            "l2": f"inputs larger than L2: {L} layer caches x {B*H*T0*62/1e6:.1f} MB are cycled every step",
-            "cuda_graph": True, "bytes_per_token_head": 62,
-            "us_per_layer_step": 1e3 * ms_max / args.steps / L,
-            "packed_gbs_whole_step": value / world * 62 / 1e9,
-            "decode_call_us_live": dec_s * 1e6, "decode_call_packed_gbs": dec_bytes / dec_s / 1e9,
-            "decode_main_kernel_us_live": main_s * 1e6,
+            "l2": f"inputs larger than L2: {L} layer caches x {B*H*T0*rig.bpt/1e6:.1f} MB are cycled every step",
+            "cuda_graph": True, "bytes_per_token_head": rig.bpt,
+            "step_form": "tq_decode_model_step: one append+query-prep launch for all layers, one streaming launch per "
+                         "layer cache (run-ahead chain), one finish launch",
+            "us_per_layer_step": us_layer,
+            "packed_gbs_whole_step": value / world * rig.bpt / 1e9,
+            "us_per_layer_step_sequential": seq_us,
+            "value_sequential": L * B * H * (T0 + 1) / (seq_us * L * 1e-6),
+            "decode_call_us_live": call_us, "decode_call_packed_gbs": dec_bytes / call_us / 1e3,
+            "decode_main_kernel_us_live": chain_us, "decode_main_kernel_us_isolated_launch": iso_us,
             "quantize_pack_gbs": quant_gbs, "quantize_pack_ms_per_layer": statistics.median(q_ms),
+            "quantize_pack_frac_of_hbm": quant_gbs / peak,
             "parallelism": f"dp{world} (independent batches, no collective)",
         },
         "clocks": clocks,
@@ -446,12 +526,102 @@ def run_ours(args, w: W.Workload):
                 "d2h_bytes_per_step": L * vec_bytes, "steps": e2e_steps},
         "gpu_launches": int(launches_per_step * args.steps),
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": NCU_DRAM_BYTES_PER_LAUNCH, "kernel": "decode_main_kernel<64, __half>",
-                     "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum per launch, profiles/r01b_decode_main_full.md",
-                     "peak_source": peak_src, "bytes_per_launch": dec_bytes},
+                     "traffic": traffic[0] if traffic else None, "kernel": "decode_main_kernel<64, __half, false>",
+                     "traffic_source": (f"dram__bytes_read.sum + dram__bytes_write.sum per launch, {traffic[1]}" if traffic
+                                        else "no ncu capture of the current kernel is committed"),
+                     "peak_source": peak_src, "bytes_per_launch": dec_bytes,
+                     "how": f"{L} launches (one per layer cache) as the model step chains them, CUDA events around the graph, / {L}",
+                     "frac_isolated_launch": dec_bytes / iso_us / 1e3 / peak,
+                     "frac_call": dec_bytes / call_us / 1e3 / peak,
+                     "frac_step": value / world * rig.bpt / 1e9 / peak},
     }
     if world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(w)
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def run_aux(args, w: W.Workload, key: str):
+    """configs[1], [3], [4]: a full prefill tq_quantize_pack of every layer cache (GB/s on input + packed bytes), then the
+    fused decode over the cache(s); one JSON line."""
+    import torch
+    import torch.distributed as dist
+
+    rank, world, local = init_dist()
+    from paper_2603_26110_b200 import binding as tq
+
+    bpt = bytes_per_token_head(w.head_dim)
+    cache_mb = w.batch * w.n_heads * w.seq * bpt / 1e6
+    # enough layer caches to exceed the 126 MB L2 (configs[1] has its own 33 layers)
+    L = w.n_layers if key == "cfg1" else max(2, int(np.ceil(300.0 / cache_mb)))
+    if args.layers_aux:
+        L = args.layers_aux
+    rig = Rig(w, L, w.seq, rank, local)
+    B, H, d, T0, dev, stream, shape, params, cache = rig.B, rig.H, rig.d, rig.T0, rig.dev, rig.stream, rig.shape, rig.params, rig.cache
+    q_ms, q_bytes = rig.prefill()
+    quant_gbs = q_bytes / (statistics.median(q_ms) * 1e-3) / 1e9
+    qs = torch.stack([torch_activations(rig.wl, l, (B, H, d), dev, rig.gen)[0] for l in range(L)])
+    outs = torch.empty_like(qs)
+    wss = [tq.Workspace(shape, 1, dev) for _ in range(L)]
+    wsL = tq.Workspace(shape, L, dev)
+
+    def per_layer():
+        for layer in range(L):
+            tq.tq_decode_attn(shape, params, cache, layer, 1, qs[layer:layer + 1], outs[layer:layer + 1], wss[layer], None, T0, stream)
+
+    def batched():
+        tq.tq_decode_attn(shape, params, cache, 0, L, qs, outs, wsL, None, T0, stream)
+
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    reps = max(6, min(args.steps, 30))
+    call_us = rig.graph_us(per_layer, L, reps=reps)
+    batched_us = rig.graph_us(batched, L, reps=reps) if key == "cfg1" else None
+    with torch.cuda.stream(stream):
+        per_layer()
+        stream.synchronize()
+    tq.tq_profile_decode_main_only(True)
+    try:
+        main_us = rig.graph_us(per_layer, L, reps=reps)
+    finally:
+        tq.tq_profile_decode_main_only(False)
+    clocks = sampler.stop() if rank == 0 else None
+    step_us = (batched_us if batched_us is not None else call_us) * L
+    (ms_max,) = max_over_ranks([step_us * 1e-3], world, dev)
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    peak, peak_src = measured_peaks()
+    dec_bytes = B * H * T0 * bpt
+    value = world * L * B * H * T0 / (ms_max * 1e-3)
+    traffic = ncu_traffic(f"decode_main_{key}")
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": reps - 1, "warmup": 3,
+        "ms_per_step": ms_max, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {
+            "workload": f"{w.name} (BASELINE.json configs[{w.index}]): {L} layer cache(s) x batch {B} x {H} heads x d {d}, "
+                        f"{T0} cached tokens, {w.dtype} {w.dist}; full prefill tq_quantize_pack, then fused decode over every cache",
+            "layers": L, "batch_per_gpu": B, "heads": H, "head_dim": d, "cached_tokens": T0,
+            "l2": f"{L} layer caches x {cache_mb:.1f} MB are cycled", "cuda_graph": True, "bytes_per_token_head": bpt,
+            "step": "one tq_decode_attn per layer cache" if batched_us is None else "ONE tq_decode_attn call over all 33 layers",
+            "decode_call_us_per_layer": call_us, "decode_call_us_per_layer_batched": batched_us,
+            "decode_main_kernel_us_live": main_us,
+            "quantize_pack_gbs": quant_gbs, "quantize_pack_ms_per_layer": statistics.median(q_ms),
+            "quantize_pack_frac_of_hbm": quant_gbs / peak,
+            "quantize_pack_roofline": {"bound": "hbm (rotations on tcgen05)", "achieved": quant_gbs, "peak": peak, "unit": "GB/s",
+                                       "frac": quant_gbs / peak, "bytes_per_launch": q_bytes},
+        },
+        "clocks": clocks,
+        "e2e": None,
+        "gpu_launches": int(tq.tq_launch_count()),
+        "roofline": {"bound": "hbm", "achieved": dec_bytes / main_us / 1e3, "peak": peak, "unit": "GB/s",
+                     "frac": dec_bytes / main_us / 1e3 / peak, "traffic": traffic[0] if traffic else None,
+                     "kernel": f"decode_main_kernel<{d}, __half, true>", "peak_source": peak_src, "bytes_per_launch": dec_bytes,
+                     "frac_call": dec_bytes / call_us / 1e3 / peak},
+    }
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
@@ -463,14 +633,27 @@ def main():
     ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--layers", type=int, default=33, help="ESM-2-650M has 33 layers")
+    ap.add_argument("--config", default="cfg2", choices=sorted(CONFIG_NAMES))
+    ap.add_argument("--layers", type=int, default=33, help="ESM-2-650M has 33 layers (cfg2)")
+    ap.add_argument("--layers-aux", type=int, default=0, help="layer caches cycled by cfg3 / cfg4 (0 = enough to exceed L2)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
-    w = W.CONFIGS["cfg2_650m_batch32"]
+    w = W.CONFIGS[CONFIG_NAMES[args.config]]
     if args.impl == "reference":
         run_reference(args, w)
+        return
+    world_env = os.environ.get("WORLD_SIZE")
+    if world_env is None and args.gpus > 1:
+        # `python bench.py --gpus N`: one process per GPU under torchrun, as the driver launches it
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+               "--master-addr", "127.0.0.1", "--master-port", os.environ.get("MASTER_PORT", "29533"), os.path.abspath(__file__)] + sys.argv[1:]
+        raise SystemExit(subprocess.call(cmd))
+    if world_env is not None and int(world_env) != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} does not match WORLD_SIZE={world_env}")
+    if args.config == "cfg2":
+        run_cfg2(args, w)
     else:
-        run_ours(args, w)
+        run_aux(args, w, args.config)
 
 
 if __name__ == "__main__":

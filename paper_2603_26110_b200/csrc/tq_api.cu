@@ -225,7 +225,7 @@ static int run_decode(const tq_shape* shape, const tq_params* dev, const tq_cach
     const void* kc = k ? (const unsigned char*)k + u0 * g.D * esz : nullptr;
     const void* vc = v ? (const unsigned char*)v + u0 * g.D * esz : nullptr;
     if (!(g_profile_skip_prep && do_query && !do_append) &&
-        launch_prep(a, kc, vc, g.D, do_append, do_query, (cudaStream_t)cuda_stream) != cudaSuccess)
+        launch_prep(a, kc, vc, g.D, sms, do_append, do_query, (cudaStream_t)cuda_stream) != cudaSuccess)
       return TQ_ERR_CUDA;
     if (do_query && launch_decode(a, g.D, true, (cudaStream_t)cuda_stream) != cudaSuccess) return TQ_ERR_CUDA;
   }
@@ -322,7 +322,7 @@ int tq_decode_model_step(const tq_shape* shape, const tq_params* dev, tq_cache* 
   // one prep launch for every layer of the step (append + query operands), then one streaming launch per layer cache:
   // the first waits for the prep kernel, the others run ahead of one another (DecodeArgs::chain_mode); they leave o'/l
   // in the workspace and one last launch applies PI_V^T to every unit of the step
-  if (!g_profile_skip_prep && launch_prep(a, k, v, g.D, true, true, st) != cudaSuccess) return TQ_ERR_CUDA;
+  if (!g_profile_skip_prep && launch_prep(a, k, v, g.D, sms, true, true, st) != cudaSuccess) return TQ_ERR_CUDA;
   const size_t units = (size_t)g.B * g.H;
   for (int l = 0; l < n_layers_call; ++l) {
     DecodeArgs b = a;

@@ -196,8 +196,8 @@ struct DecodeArgs {
 
 cudaError_t launch_quantize_pack(const QuantArgs& a, int D, tq_dtype dt, int num_sms, cudaStream_t st);
 cudaError_t launch_quantize_pack_tc(const QuantArgs& a, int D, tq_dtype dt, int num_sms, cudaStream_t st);  // tcgen05
-cudaError_t launch_prep(const DecodeArgs& d, const void* k, const void* v, int D, bool do_append, bool do_query,
-                        cudaStream_t st);
+cudaError_t launch_prep(const DecodeArgs& d, const void* k, const void* v, int D, int num_sms, bool do_append,
+                        bool do_query, cudaStream_t st);
 cudaError_t launch_decode(const DecodeArgs& a, int D, bool fused_out, cudaStream_t st);
 cudaError_t launch_finish(const DecodeArgs& a, int D, cudaStream_t st);
 int decode_ctas_per_sm(int D);

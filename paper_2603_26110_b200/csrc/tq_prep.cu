@@ -69,7 +69,7 @@ struct RowRegs64 {
 };
 
 template <int D, typename T, bool kAppend, bool kQuery>
-__global__ void __launch_bounds__((kAppend ? 3 : 2) * PrepCfg<D>::GT) prep_kernel(PrepArgs a, int nbg) {
+__global__ void __launch_bounds__((kAppend ? 3 : 2) * PrepCfg<D>::GT) prep_kernel(PrepArgs a, int nbg, int groups_per_cta) {
   using Lo = Layout<D>;
   using Cfg = PrepCfg<D>;
   constexpr int TPR = Cfg::TPR, GT = Cfg::GT, BG = Cfg::BG;
@@ -90,17 +90,16 @@ __global__ void __launch_bounds__((kAppend ? 3 : 2) * PrepCfg<D>::GT) prep_kerne
   const int tid = threadIdx.x, lane = tid & 31;
   const int grp = tid / GT, gt = tid % GT, row = gt / TPR, part = gt % TPR, wg = gt >> 5;
   const int B = a.cv.B, H = a.cv.H;
-  const int bgi = (int)blockIdx.x % nbg, lh_c = (int)blockIdx.x / nbg;  // (layer-in-call, head), batch group
+  // one CTA per (layer-in-call, head) and run of groups_per_cta batch groups: the matrix rows are fetched once and
+  // stay in registers over the whole run (the multi-layer model step uses long runs, a single layer short ones)
+  const int ncta_lh = (nbg + groups_per_cta - 1) / groups_per_cta;
+  const int run = (int)blockIdx.x % ncta_lh, lh_c = (int)blockIdx.x / ncta_lh;
   const int lc = lh_c / H, h = lh_c % H;
   const int layer = a.layer_begin + lc;
-  const int b0 = bgi * BG, nb = min(BG, B - b0);
   const size_t lh = (size_t)layer * H + h;
+  const int bg_first = run * groups_per_cta, bg_end = min(nbg, bg_first + groups_per_cta);
 
   pdl_trigger();  // the streaming kernel behind this one may start its L2 prefetches
-  // ---- the cache lengths first: the RoPE positions and the target tile slot hang off them
-  int len_e[BG];
-#pragma unroll
-  for (int e = 0; e < BG; ++e) len_e[e] = e < nb ? __ldcg(a.cv.seq_len + layer * B + b0 + e) : 0;
   // ---- matrix rows into registers.  d = 64: the CTA copies its (up to) three 16 KB matrices with fully coalesced
   //      16-byte cp.async into shared memory (row pitch 68 floats: a thread-per-row read is then conflict free) and
   //      every thread picks up its row from there; d = 128: straight from global memory (three 64 KB matrices do not fit)
@@ -121,6 +120,14 @@ __global__ void __launch_bounds__((kAppend ? 3 : 2) * PrepCfg<D>::GT) prep_kerne
     const float* M = grp == 0 ? a.pi_k + lh * D * D : grp == 1 ? a.S : a.pi_v + lh * D * D;
     rowreg.load(M + (size_t)row * D + part * 64);
   }
+  if (tid < 8) lutK[tid] = a.lut_k[lh * 8 + tid];
+  if (tid >= 32 && tid < 40) lutV[tid - 32] = a.lut_v[lh * 8 + tid - 32];
+  for (int bgi = bg_first; bgi < bg_end; ++bgi) {
+  const int b0 = bgi * BG, nb = min(BG, B - b0);
+  // ---- the cache lengths first: the RoPE positions and the target tile slot hang off them
+  int len_e[BG];
+#pragma unroll
+  for (int e = 0; e < BG; ++e) len_e[e] = e < nb ? __ldcg(a.cv.seq_len + layer * B + b0 + e) : 0;
   // ---- stage-4 work item of this thread (one 16-bit or 8-bit piece of one token in the device tile layout,
   //      tq_common.cuh), and an early read of the V halfword it will modify (a V field is shared with the other token
   //      of the pair, which was appended by an earlier call)
@@ -144,8 +151,6 @@ __global__ void __launch_bounds__((kAppend ? 3 : 2) * PrepCfg<D>::GT) prep_kerne
     vptr = reinterpret_cast<unsigned short*>(it_tp + Lo::kOffVC + word_offset(Lo::KCW, hidx >> 1, 4 * gi + (pp & 3))) + (hidx & 1);
     vold = __ldcg(vptr);
   }
-  if (tid < 8) lutK[tid] = a.lut_k[lh * 8 + tid];
-  if (tid >= 32 && tid < 40) lutV[tid - 32] = a.lut_v[lh * 8 + tid - 32];
 
   // ---- inputs of the BG batch entries of this head, RoPE applied to k and q (positions read on the device)
   for (int idx = tid; idx < BG * HP; idx += NT) {
@@ -196,9 +201,9 @@ __global__ void __launch_bounds__((kAppend ? 3 : 2) * PrepCfg<D>::GT) prep_kerne
       xv[e][i] = e < nb ? load_as_float<T>(reinterpret_cast<const T*>(a.v) + (((size_t)lc * B + b0 + e) * H + h) * D + i) : 0.f;
     }
   }
-  if (kStageRows) asm volatile("cp.async.wait_group 0;" ::: "memory");
+  if (kStageRows && bgi == bg_first) asm volatile("cp.async.wait_group 0;" ::: "memory");
   __syncthreads();
-  if (kStageRows) rowreg.load_shared(msm + ((size_t)grp * D + row) * kPitch);
+  if (kStageRows && bgi == bg_first) rowreg.load_shared(msm + ((size_t)grp * D + row) * kPitch);
 
   // ---- stage 1: rotations (groups 0 and 2) and the norms of the rotated key / value
   float yk[BG], yv[BG];
@@ -347,7 +352,7 @@ __global__ void __launch_bounds__((kAppend ? 3 : 2) * PrepCfg<D>::GT) prep_kerne
       }
       a.frags[(((size_t)lc * B + b0 + e) * H + h) * FL::kWords + wi] = word;
     }
-    if (tid < 64) {  // every batch group of the head writes the same values
+    if (tid < 64 && bgi == bg_first) {  // every CTA of the head writes the same values
       const int c0 = tid & 7, c1 = tid >> 3;
       unsigned* tb = a.tabs + (size_t)lh_c * kTabWords;
       tb[tid] = split2(lutK[c0], lutK[c1], false);
@@ -363,7 +368,10 @@ __global__ void __launch_bounds__((kAppend ? 3 : 2) * PrepCfg<D>::GT) prep_kerne
       }
     }
   }
-  if (!kAppend) return;
+  if (!kAppend) {
+    __syncthreads();  // the next group of the run reuses the shared arrays
+    continue;
+  }
 
   // ---- stage 4 (append): every thread assembles one piece of one token in the device tile layout
   if (it_on) {
@@ -421,13 +429,20 @@ __global__ void __launch_bounds__((kAppend ? 3 : 2) * PrepCfg<D>::GT) prep_kerne
       __threadfence();
     }
   }
+  __syncthreads();  // the next group of the run reuses the shared arrays
+  }  // batch groups of this CTA's run
 }
 
 template <int D, typename T>
-static cudaError_t launch_prep_t(const PrepArgs& a, int lh_count, int B, bool do_append, bool do_query, cudaStream_t st) {
+static cudaError_t launch_prep_t(const PrepArgs& a, int lh_count, int B, int num_sms, bool do_append, bool do_query,
+                                 cudaStream_t st) {
   using Cfg = PrepCfg<D>;
   const int nbg = (B + Cfg::BG - 1) / Cfg::BG;
-  const int grid = lh_count * nbg;
+  // batch groups per CTA: a CTA re-uses its matrix rows over a run of groups.  Enough CTAs to fill the GPU twice
+  // (a single layer: one group per CTA, shortest latency); the rest of the batch goes into longer runs.
+  int gpc = (int)(((long)lh_count * nbg + 2L * num_sms - 1) / (2L * num_sms));
+  gpc = gpc < 1 ? 1 : (gpc > nbg ? nbg : gpc);
+  const int grid = lh_count * ((nbg + gpc - 1) / gpc);
   const size_t sm3 = D == 64 ? (size_t)3 * D * 68 * 4 : 0, sm2 = D == 64 ? (size_t)2 * D * 68 * 4 : 0;
   if (D == 64) {  // per launch: the attribute is per device and a process may drive several
     cudaError_t e1 = cudaFuncSetAttribute(prep_kernel<D, T, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm3);
@@ -435,15 +450,15 @@ static cudaError_t launch_prep_t(const PrepArgs& a, int lh_count, int B, bool do
     if (e1 != cudaSuccess) return e1;
     if (e2 != cudaSuccess) return e2;
   }
-  if (do_append && do_query) prep_kernel<D, T, true, true><<<grid, 3 * Cfg::GT, sm3, st>>>(a, nbg);
-  else if (do_append) prep_kernel<D, T, true, false><<<grid, 3 * Cfg::GT, sm3, st>>>(a, nbg);
-  else prep_kernel<D, T, false, true><<<grid, 2 * Cfg::GT, sm2, st>>>(a, nbg);
+  if (do_append && do_query) prep_kernel<D, T, true, true><<<grid, 3 * Cfg::GT, sm3, st>>>(a, nbg, gpc);
+  else if (do_append) prep_kernel<D, T, true, false><<<grid, 3 * Cfg::GT, sm3, st>>>(a, nbg, gpc);
+  else prep_kernel<D, T, false, true><<<grid, 2 * Cfg::GT, sm2, st>>>(a, nbg, gpc);
   count_launch();
   return cudaGetLastError();
 }
 
-cudaError_t launch_prep(const DecodeArgs& d, const void* k, const void* v, int D, bool do_append, bool do_query,
-                        cudaStream_t st) {
+cudaError_t launch_prep(const DecodeArgs& d, const void* k, const void* v, int D, int num_sms, bool do_append,
+                        bool do_query, cudaStream_t st) {
   PrepArgs a;
   a.cv = d.cv;
   a.pi_k = d.pi_k;
@@ -463,10 +478,10 @@ cudaError_t launch_prep(const DecodeArgs& d, const void* k, const void* v, int D
   a.rope_layout = d.rope_layout;
   const int lh_count = d.n_layers_call * d.cv.H;
   if (D == 64)
-    return d.dt == TQ_F16 ? launch_prep_t<64, __half>(a, lh_count, d.cv.B, do_append, do_query, st)
-                          : launch_prep_t<64, float>(a, lh_count, d.cv.B, do_append, do_query, st);
-  return d.dt == TQ_F16 ? launch_prep_t<128, __half>(a, lh_count, d.cv.B, do_append, do_query, st)
-                        : launch_prep_t<128, float>(a, lh_count, d.cv.B, do_append, do_query, st);
+    return d.dt == TQ_F16 ? launch_prep_t<64, __half>(a, lh_count, d.cv.B, num_sms, do_append, do_query, st)
+                          : launch_prep_t<64, float>(a, lh_count, d.cv.B, num_sms, do_append, do_query, st);
+  return d.dt == TQ_F16 ? launch_prep_t<128, __half>(a, lh_count, d.cv.B, num_sms, do_append, do_query, st)
+                        : launch_prep_t<128, float>(a, lh_count, d.cv.B, num_sms, do_append, do_query, st);
 }
 
 }  // namespace tq

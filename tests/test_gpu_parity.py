@@ -384,6 +384,72 @@ def test_full_size_cfg2_sampled_units(tq, oracle):
     assert np.all(np.isfinite(got.astype(np.float64)))
 
 
+def _full_size_sampled(tq, oracle, w, b_s, heads, what):
+    """Full prefill (tq_quantize_pack of every token) then decode at FULL size in the launch configuration bench.py
+    times; the oracle re-computes batch entry b_s x `heads`: quantize parity on its own vectors, decode parity on the
+    GPU's exported bytes."""
+    c = Case(tq, oracle, w, max_seq=w.seq)
+    k, v = W.layer_activations(w, 0)
+    tq.tq_quantize_pack(c.shape, c.params, c.cache, 0, c.dev(k), c.dev(v))
+    q = W.queries(w, 0)
+    T, d = w.seq, w.head_dim
+    got = c.gpu_decode(0, 1, q[None], t_hint=T)[0]
+    planes = c.gpu_export(0, T)
+    a = c.arr
+    hs = np.asarray(heads)
+    can = oracle.quantize_pack(k[b_s:b_s + 1][:, hs], v[b_s:b_s + 1][:, hs], a["pi_k"][0][hs], a["pi_v"][0][hs],
+                               a["lut_k"][0][hs], a["lut_v"][0][hs], a["S"], base=w.rope_base, near_eps=TL.NEAR_EPS)
+    sub = {n: p[b_s:b_s + 1][:, hs] for n, p in planes.items()}
+    rep = TL.compare_quantize(can, sub, d, what)
+    print(what, "quantize sample:", rep)
+    gcan = oracle.Canonical(*[sub[n] if "norm" not in n else sub[n].view(np.uint16)
+                              for n in ("k_codes", "k_signs", "k_norm", "k_rnorm", "v_codes", "v_norm")])
+    sl = np.full(1, T, np.int32)
+    want = oracle.decode_attn(q[b_s:b_s + 1][:, hs], sl - 1, sl, a["pi_k"][0][hs], a["pi_v"][0][hs], a["lut_k"][0][hs],
+                              a["lut_v"][0][hs], a["S"], gcan, base=w.rope_base)
+    g = got[b_s:b_s + 1][:, hs].astype(np.float64)
+    ulp = np.spacing(np.abs(want).astype(np.float16)).astype(np.float64) if w.dtype == "f16" else 0.0
+    assert np.all(np.abs(g - want) <= ulp + TL.OUT_MAX_ABS), (what, np.abs(g - want).max())
+    den = np.linalg.norm(g) * np.linalg.norm(want)
+    assert den > 0 and float(g.ravel() @ want.ravel() / den) >= TL.OUT_MIN_COS
+    assert np.all(np.isfinite(got.astype(np.float64)))
+
+
+def test_full_size_cfg3_long_context_sampled_units(tq, oracle):
+    """BASELINE.json:configs[3] at full size: 4 x 20 heads x 16384 tokens, full prefill then split-K decode."""
+    _full_size_sampled(tq, oracle, W.CONFIGS["cfg3_long_splitk"], 2, [0, 7, 19], "cfg3 full size")
+
+
+def test_full_size_cfg4_d128_sampled_units(tq, oracle):
+    """BASELINE.json:configs[4] at full size: 8 x 40 heads x 4096 tokens, head_dim 128."""
+    _full_size_sampled(tq, oracle, W.CONFIGS["cfg4_15b_heads"], 5, [3, 38], "cfg4 full size")
+
+
+def test_full_size_cfg2_fp32_outputs_at_the_bare_tolerance(tq, oracle):
+    """north_star's bare bar (max-abs 2e-3, cosine 0.9999, no binary16-ulp allowance) at configs[2] size: fp32 queries
+    and outputs, the decode kernel fed the ORACLE's cache bytes for the sampled batch entries (imported over the GPU's
+    own), launch configuration as in bench.py."""
+    w = W.CONFIGS["cfg2_650m_batch32"].scaled(dtype="f32")
+    c = Case(tq, oracle, w, max_seq=w.seq + 128)
+    k, v = W.layer_activations(w, 0)
+    tq.tq_quantize_pack(c.shape, c.params, c.cache, 0, c.dev(k), c.dev(v))
+    T = w.seq
+    planes = c.gpu_export(0, T)
+    sample = [4, 27]
+    can = c.oracle_quantize(0, k[sample], v[sample], near=False)
+    for n in ("k_codes", "k_signs", "k_norm", "k_rnorm", "v_codes", "v_norm"):
+        src = getattr(can, n)
+        planes[n][sample] = src if "norm" not in n else src.view(np.int16)
+    tq.tq_cache_import_canonical(c.shape, c.cache, 0, T, {n: c.dev(p) for n, p in planes.items()})
+    q = W.queries(w, 0)
+    got = c.gpu_decode(0, 1, q[None], t_hint=w.seq + 128)[0]
+    assert got.dtype == np.float32
+    sl = np.full(len(sample), T, np.int32)
+    want = c.oracle_decode(0, q[sample], sl - 1, sl, can)
+    rep = TL.compare_outputs(got[sample], want, "cfg2 fp32 full size")  # bare 2e-3 / 0.9999
+    print("cfg2 full size, fp32 outputs on the oracle's bytes:", rep)
+
+
 # ---------------------------------------------------------------------------------------------- cross-checks
 @pytest.mark.gpu
 @pytest.mark.parametrize("name,kw", [("cfg2_650m_batch32", dict(batch=3, n_heads=4, seq=300)),

@@ -354,3 +354,58 @@ def test_memory_accounting_against_paper_table4():
     # ours: 62 B per cached token-head at d = 64 (24 + 8 + 2 + 2 for K, 24 + 2 for V)
     ours = 33 * 20 * 1024 * 62 / MiB
     assert abs(ours - 40.0) < 0.1 and ours < vals["total"]
+
+
+# ---------------------------------------------------------------------------- whole-layer indexing
+def test_quantize_pack_start_pos_and_per_head_indexing(oracle):
+    """tqo_quantize_pack(start_pos = s) must equal tqo_quantize_vector(pos = s + t) plane by plane, with THAT head's PI and
+    LUT (pins the start_pos offset of the RoPE position and the pi + h d d / lut + 8 h indexing at B, H > 1;
+    SURVEY.md §8(c) steps 1-6).  The per-vector call is pinned on its own above."""
+    rng = np.random.default_rng(2603)
+    B, H, T, d, s = 2, 3, 5, 64, 7
+    pi_k = np.stack([haar(rng, d) for _ in range(H)])
+    pi_v = np.stack([haar(rng, d) for _ in range(H)])
+    lut0 = oracle.lloyd_max_gauss(1 / 8, 8)[0].astype(np.float32)
+    lut_k = np.sort(np.stack([lut0 * np.float32(1 + 0.07 * h) for h in range(H)]), axis=-1)
+    lut_v = np.sort(np.stack([lut0 * np.float32(1.3 - 0.05 * h) for h in range(H)]), axis=-1)
+    S = rng.standard_normal((d, d)).astype(np.float32)
+    k = rng.standard_normal((B, H, T, d)).astype(np.float32)
+    v = rng.standard_normal((B, H, T, d)).astype(np.float32)
+    k[..., 3] *= 20
+    can = oracle.quantize_pack(k, v, pi_k, pi_v, lut_k, lut_v, S, start_pos=s)
+    again0 = oracle.quantize_pack(k, v, pi_k, pi_v, lut_k, lut_v, S, start_pos=0)
+    assert not np.array_equal(can.k_codes, again0.k_codes)  # the position matters for keys ...
+    assert np.array_equal(can.v_codes, again0.v_codes)      # ... and not for values (no RoPE on V)
+    for b in range(B):
+        for h in range(H):
+            for t in range(T):
+                qk = oracle.quantize_vector(k[b, h, t], True, s + t, pi_k[h], lut_k[h], S)
+                qv = oracle.quantize_vector(v[b, h, t], False, 0, pi_v[h], lut_v[h], S)
+                assert np.array_equal(oracle.unpack_codes(can.k_codes[b, h, t], d), qk["codes"]), (b, h, t)
+                assert np.array_equal(oracle.unpack_bits(can.k_signs[b, h, t], d), qk["bits"]), (b, h, t)
+                assert can.k_norm[b, h, t] == qk["norm_h"] and can.k_rnorm[b, h, t] == qk["rnorm_h"]
+                assert np.array_equal(oracle.unpack_codes(can.v_codes[b, h, t], d), qv["codes"]), (b, h, t)
+                assert can.v_norm[b, h, t] == qv["norm_h"]
+    # a wrong head's matrices or table would not reproduce the planes
+    wrong = oracle.quantize_vector(k[1, 2, 4], True, s + 4, pi_k[1], lut_k[2], S)
+    assert not np.array_equal(oracle.unpack_codes(can.k_codes[1, 2, 4], d), wrong["codes"])
+
+
+def test_key_sketch_values_are_S_times_the_residual(oracle):
+    """tqo_key_sketch_values returns (S r)_j: rebuilt here with numpy from the per-vector call's unit vector and codes,
+    and its signs are the stored sign bits (>= 0 -> 1, D7).  The GPU parity tests use it to show that a sign
+    mismatch can only sit where |(S r)_j| is at rounding level."""
+    rng = np.random.default_rng(77)
+    d = 64
+    Pi = haar(rng, d)
+    S = rng.standard_normal((d, d)).astype(np.float32)
+    lut = oracle.lloyd_max_gauss(1 / 8, 8)[0].astype(np.float32)
+    for pos in (0, 5, 1023):
+        x = rng.standard_normal(d).astype(np.float32)
+        x[17] *= 20
+        qv = oracle.quantize_vector(x, True, pos, Pi, lut, S)
+        sr = oracle.key_sketch_values(x, pos, Pi, lut, S)
+        r = qv["u"] - lut[qv["codes"]].astype(np.float64)
+        assert np.allclose(sr, S.astype(np.float64) @ r, rtol=0, atol=1e-12)
+        assert np.array_equal((sr >= 0).astype(np.uint8), qv["bits"])
+        assert abs(np.linalg.norm(r) - oracle.f16_bits_to_f64(qv["rnorm_h"])) <= 2.0 ** -11 * np.linalg.norm(r) + 1e-12
