@@ -1,29 +1,26 @@
 // tq_prep.cu — the small kernel in front of the streaming decode kernel.
 //
-// One CTA per (layer-in-call, head, group of BG batch entries) does, depending on the template flags,
+// One CTA per (layer-in-call, head, run of up to 32 batch entries) does, depending on the template flags,
 //   kAppend : quantize-and-pack ONE new token per batch entry (PAPER.md:111-116 per vector;
 //             BASELINE.json:configs[2]): RoPE(k) -> PI_K -> norm, codes, residual -> S r -> bits;
-//             PI_V v -> norm, codes; the words are written into the tile slot seq_len[layer][b] and the last head of
-//             the batch entry to arrive bumps seq_len;
+//             PI_V v -> norm, codes; the pieces are written into the tile slot seq_len[layer][b] (device tile layout,
+//             tq_common.cuh) and the last head of the batch entry to arrive bumps seq_len;
 //   kQuery  : query preparation for the fused decode kernel (Eq. 4 moves PI to the query; north_star):
-//             q'' = PI_K RoPE(q), z = S q''  -> workspace, pre-scaled so that logits come out in log2 units.
-// tq_append = <true,false>, tq_decode_attn = <false,true>, tq_decode_step = <true,true>.
+//             q'' = PI_K RoPE(q), z = S q''  -> the decode kernel's MMA operands in the workspace (FragLayout), pre-scaled
+//             so that logits come out in log2 units; plus the head's fp16 dequantisation tables.
+// tq_append = <true,false>, tq_decode_attn = <false,true>, tq_decode_step / tq_decode_model_step = <true,true>.
 //
-// The work is tiny (five d x d mat-vecs per unit) and the kernel is bound by latency and by re-reading the three
-// d x d fp32 matrices of a head: so a CTA keeps them in REGISTERS — three thread groups (PI_K, S, PI_V), TPR = d/64
-// threads per matrix row, 64 row elements per thread — fetches them once and applies them to all BG batch entries
-// of its head at once (vectors are read from shared memory as broadcast float4).  Four barriers per CTA:
-//   inputs + RoPE | PI_K k, PI_K q, PI_V v and their norms | codes, residual, its norm | S r, S q'' | words out.
+// For the batch entries of one head the five d x d mat-vecs are two small GEMMs, [k; q; v rows] x PI^T and
+// [r; q'' rows] x S^T: they run on mma.sync.m16n8k16 with the same exactness scheme as the tcgen05 prefill kernel
+// (tq_quantize_tc.cu): fp16 two-term splits a = a_hi + a_lo of both operands, D = A_hi B_hi + A_lo B_hi + A_hi B_lo with
+// fp32 accumulation, power-of-two scalings that cancel exactly (PI x16, vectors by 2^-exponent(max |x|), r x8).  A warp
+// owns d/64 n-tiles (8 matrix rows each) and reads their B fragments straight from global memory (L2), so no matrix is
+// staged.  Everything per entry (RoPE, maxima, norms, codes, residual, operand splits) is done by one warp per entry with
+// shuffles: six CTA barriers in all, whatever the number of entries.  (A first version kept matrix rows in registers and
+// used CUDA-core FMAs, two of six warps at a time: 190 us for the 33-layer step; profiles/r02_prep.md.)
 #include "tq_common.cuh"
 
 namespace tq {
-
-__device__ __forceinline__ int code_of7(float u, const float* lut) {
-  int c = 0;
-#pragma unroll
-  for (int q = 0; q < 7; ++q) c += (u > 0.5f * (lut[q] + lut[q + 1])) ? 1 : 0;
-  return c;
-}
 
 struct PrepArgs {
   CacheView cv;
@@ -36,329 +33,415 @@ struct PrepArgs {
   int layer_begin, rope_layout;
 };
 
-template <int D>
+constexpr int kPrepThreads = 256;
+constexpr int kPrepWarps = kPrepThreads / 32;
+
+// EB = batch entries per CTA: 32 (two 16-row m-tiles per operand block; the multi-layer model step, where the instruction
+// count per SM matters) or 8 (k and q rows share one m-tile; a single layer, where the latency of one CTA matters)
+template <int D, int EB>
 struct PrepCfg {
-  static constexpr int TPR = D / 64;          // threads per matrix row (64 row elements each)
-  static constexpr int GT = D * TPR;          // threads per group: 64 | 256
-  static constexpr int BG = D == 64 ? 4 : 2;  // batch entries per CTA
+  static constexpr int HP = D + 8;   // row pitch of the fp16 operand rows, in halves: A-fragment reads are conflict free
+  static constexpr int FP = D + 8;   // row pitch of the fp32 result rows
+  static constexpr int ROWS = EB == 8 ? 32 : 3 * EB;  // operand rows: [0, EB) k then r | [EB, 2 EB) q then q'' | [2 EB, 3 EB) v
+  static constexpr size_t kSmemBytes = (size_t)2 * ROWS * HP * 2 /* hi, lo */ + (size_t)ROWS * FP * 4 /* results */ +
+                                       (size_t)2 * EB * D /* cK, cV */;
 };
 
-// 64 consecutive elements of one matrix row, in registers
-struct RowRegs64 {
-  float4 m[16];
-  __device__ __forceinline__ void load(const float* __restrict__ p) {
+__device__ __forceinline__ void mma16816p(float (&d)[4], unsigned a0, unsigned a1, unsigned a2, unsigned a3, unsigned b0, unsigned b1) {
+  asm("mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+      : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
+      : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
+}
+// (x0, x1) -> fp16 pairs hi and lo with x = hi + lo
+__device__ __forceinline__ void split_pair(float x0, float x1, unsigned& hi, unsigned& lo) {
+  const __half2 h = __floats2half2_rn(x0, x1);
+  const float2 hf = __half22float2(h);
+  const __half2 l = __floats2half2_rn(x0 - hf.x, x1 - hf.y);
+  hi = *reinterpret_cast<const unsigned*>(&h);
+  lo = *reinterpret_cast<const unsigned*>(&l);
+}
+// 2^-e and 2^e with 2^e <= amax < 2^(e+1) (1, 1 for zero / denormal amax)
+__device__ __forceinline__ void pow2_scale_p(float amax, float& s, float& inv_s) {
+  unsigned E = (__float_as_uint(amax) >> 23) & 0xffu;
+  E = E < 2u ? 127u : (E > 252u ? 252u : E);
+  s = __uint_as_float((254u - E) << 23);
+  inv_s = __uint_as_float(E << 23);
+}
+__device__ __forceinline__ int code_of7(float u, const float* lut) {
+  int c = 0;
 #pragma unroll
-    for (int c = 0; c < 16; ++c) m[c] = __ldg(reinterpret_cast<const float4*>(p) + c);
+  for (int q = 0; q < 7; ++q) c += (u > 0.5f * (lut[q] + lut[q + 1])) ? 1 : 0;
+  return c;
+}
+
+template <int HPITCH>
+struct PitchCfg {
+  static constexpr int HP = HPITCH, FP = HPITCH;
+};
+
+// C[rows m0 .. m0 + 16 MT) x [n-tile rows n0 .. n0 + 8) = A (fp16 hi / lo rows in shared memory) x M^T, M fp32 row-major in
+// global memory scaled by mscale; the accumulators are multiplied by rscale[row] and stored as fp32 rows.
+template <int D, int HPITCH, int MT, bool kLoTermA>
+__device__ __forceinline__ void gemm_rows(const __half* Ah, const __half* Al, int m0, const float* __restrict__ M, float mscale, int n0,
+                                          float* C, const float* rscale, int lane) {
+  using Cfg = PitchCfg<HPITCH>;
+  const int g = lane >> 2, t = lane & 3;
+  float acc[MT][4];
+#pragma unroll
+  for (int i = 0; i < MT; ++i) acc[i][0] = acc[i][1] = acc[i][2] = acc[i][3] = 0.f;
+  // B fragments of this n-tile for every k-step: M[n0 + g][16 ks + 2 t + {0, 1, 8, 9}]
+  float2 bf[D / 16][2];
+#pragma unroll
+  for (int ks = 0; ks < D / 16; ++ks) {
+    bf[ks][0] = __ldg(reinterpret_cast<const float2*>(M + (size_t)(n0 + g) * D + 16 * ks + 2 * t));
+    bf[ks][1] = __ldg(reinterpret_cast<const float2*>(M + (size_t)(n0 + g) * D + 16 * ks + 2 * t + 8));
   }
-  __device__ __forceinline__ void load_shared(const float* p) {  // 16-byte aligned, conflict-free for a 68-float row pitch
 #pragma unroll
-    for (int c = 0; c < 16; ++c) m[c] = *(reinterpret_cast<const float4*>(p) + c);
-  }
-  // acc[e] += <row part, x[e] part>, x in shared memory (every lane of a row group reads the same address)
-  template <int BG>
-  __device__ __forceinline__ void dot(const float* xs /* [BG][stride] */, int stride, float (&acc)[BG]) const {
+  for (int ks = 0; ks < D / 16; ++ks) {
+    unsigned bh0, bl0, bh1, bl1;
+    split_pair(bf[ks][0].x * mscale, bf[ks][0].y * mscale, bh0, bl0);
+    split_pair(bf[ks][1].x * mscale, bf[ks][1].y * mscale, bh1, bl1);
 #pragma unroll
-    for (int c = 0; c < 16; ++c) {
-#pragma unroll
-      for (int e = 0; e < BG; ++e) {
-        const float4 x = *reinterpret_cast<const float4*>(xs + e * stride + 4 * c);
-        acc[e] = fmaf(m[c].x, x.x, fmaf(m[c].y, x.y, fmaf(m[c].z, x.z, fmaf(m[c].w, x.w, acc[e]))));
+    for (int mt = 0; mt < MT; ++mt) {
+      const int r0 = m0 + 16 * mt + g;
+      const unsigned* ph = reinterpret_cast<const unsigned*>(Ah + (size_t)r0 * Cfg::HP + 16 * ks + 2 * t);
+      const unsigned* ph8 = reinterpret_cast<const unsigned*>(Ah + (size_t)(r0 + 8) * Cfg::HP + 16 * ks + 2 * t);
+      const unsigned a0 = ph[0], a1 = ph8[0], a2 = ph[4], a3 = ph8[4];
+      mma16816p(acc[mt], a0, a1, a2, a3, bh0, bh1);
+      mma16816p(acc[mt], a0, a1, a2, a3, bl0, bl1);
+      if (kLoTermA) {
+        const unsigned* pl = reinterpret_cast<const unsigned*>(Al + (size_t)r0 * Cfg::HP + 16 * ks + 2 * t);
+        const unsigned* pl8 = reinterpret_cast<const unsigned*>(Al + (size_t)(r0 + 8) * Cfg::HP + 16 * ks + 2 * t);
+        mma16816p(acc[mt], pl[0], pl8[0], pl[4], pl8[4], bh0, bh1);
       }
     }
   }
-};
+#pragma unroll
+  for (int mt = 0; mt < MT; ++mt) {
+    const int r0 = m0 + 16 * mt + g;
+    const float s0 = rscale[r0], s1 = rscale[r0 + 8];
+    *reinterpret_cast<float2*>(C + (size_t)r0 * Cfg::FP + n0 + 2 * t) = make_float2(acc[mt][0] * s0, acc[mt][1] * s0);
+    *reinterpret_cast<float2*>(C + (size_t)(r0 + 8) * Cfg::FP + n0 + 2 * t) = make_float2(acc[mt][2] * s1, acc[mt][3] * s1);
+  }
+}
 
-template <int D, typename T, bool kAppend, bool kQuery>
-__global__ void __launch_bounds__((kAppend ? 3 : 2) * PrepCfg<D>::GT) prep_kernel(PrepArgs a, int nbg, int groups_per_cta) {
+template <int D, typename T, bool kAppend, bool kQuery, int EB>
+__global__ void __launch_bounds__(kPrepThreads) prep_kernel(PrepArgs a) {
   using Lo = Layout<D>;
-  using Cfg = PrepCfg<D>;
-  constexpr int TPR = Cfg::TPR, GT = Cfg::GT, BG = Cfg::BG;
-  constexpr int NT = (kAppend ? 3 : 2) * GT;
-  constexpr int WG = GT / 32;  // warps per group
-  constexpr int HP = D / 2;
+  using Cfg = PrepCfg<D, EB>;
+  using FL = FragLayout<D>;
+  constexpr int NT = kPrepThreads, NW = kPrepWarps;
+  constexpr int HPAIR = D / 2;      // RoPE pairs per vector
+  constexpr int PL = D / 64;        // RoPE pairs per lane
   constexpr float kInvSqrtD = D == 64 ? 0.125f : 0.08838834764831845f;
   constexpr float kScaleK = 1.4426950408889634f * kInvSqrtD;             // log2(e) / sqrt(d)
   constexpr float kScaleS = kScaleK * 1.2533141373155003f / (float)D;  // ... * sqrt(pi/2) / m, m = D
-  __shared__ __align__(16) float xk[BG][D], xq[BG][D], xv[BG][D], yq[BG][D], rr[BG][D];
-  __shared__ unsigned char cK[BG][D], cV[BG][D], bitb[BG][D];
-  __shared__ float redk[BG][WG], redv[BG][WG], redr[BG][WG];
+  constexpr bool kValLo = sizeof(T) == 4;  // fp16 values are exact operands: no lo term
+  extern __shared__ __align__(16) unsigned char dsm[];
+  __half* Ah = reinterpret_cast<__half*>(dsm);                          // [ROWS][HP] hi parts
+  __half* Al = Ah + (size_t)Cfg::ROWS * Cfg::HP;                        // lo parts
+  float* Y = reinterpret_cast<float*>(Al + (size_t)Cfg::ROWS * Cfg::HP);  // [ROWS][FP]: y_k | q'' | y_v, then S r | z
+  unsigned char (*cK)[D] = reinterpret_cast<unsigned char (*)[D]>(Y + (size_t)Cfg::ROWS * Cfg::FP);
+  unsigned char (*cV)[D] = cK + EB;
+  __shared__ float rscale[Cfg::ROWS];  // accumulator -> result, per operand row
+  __shared__ float nrm[3][EB];         // |k|, |r|, |v| of the appended token
+  __shared__ float qsc[EB][2];         // 2^eq (scaling of the q'' operand rows), reserved
   __shared__ float lutK[8], lutV[8];
-  __shared__ __align__(16) float zs[BG][D];  // z of the queries (unscaled)
-  __shared__ float fscal[BG][4];             // per entry: 2^eq kScaleK, 2^ez kScaleS (fragment scalings)
-  __shared__ int s_len0[BG], s_full[BG];
+  __shared__ int s_len0[EB], s_full[EB];
 
-  const int tid = threadIdx.x, lane = tid & 31;
-  const int grp = tid / GT, gt = tid % GT, row = gt / TPR, part = gt % TPR, wg = gt >> 5;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int B = a.cv.B, H = a.cv.H;
-  // one CTA per (layer-in-call, head) and run of groups_per_cta batch groups: the matrix rows are fetched once and
-  // stay in registers over the whole run (the multi-layer model step uses long runs, a single layer short ones)
-  const int ncta_lh = (nbg + groups_per_cta - 1) / groups_per_cta;
-  const int run = (int)blockIdx.x % ncta_lh, lh_c = (int)blockIdx.x / ncta_lh;
+  const int nrun = (B + EB - 1) / EB;
+  const int run = (int)blockIdx.x % nrun, lh_c = (int)blockIdx.x / nrun;  // (layer-in-call, head), run of batch entries
   const int lc = lh_c / H, h = lh_c % H;
   const int layer = a.layer_begin + lc;
+  const int b0 = run * EB, nb = min(EB, B - b0);
+  const int mt_n = nb > 16 ? 2 : 1;  // m-tiles that hold entries (EB = 32)
   const size_t lh = (size_t)layer * H + h;
-  const int bg_first = run * groups_per_cta, bg_end = min(nbg, bg_first + groups_per_cta);
+  auto unit_of = [&](int e) { return ((size_t)lc * B + b0 + e) * H + h; };        // unit inside the call (q, k, v, out, operands)
+  auto stream_of = [&](int e) { return ((size_t)layer * B + b0 + e) * H + h; };  // unit inside the cache
 
-  pdl_trigger();  // the streaming kernel behind this one may start its L2 prefetches
-  // ---- matrix rows into registers.  d = 64: the CTA copies its (up to) three 16 KB matrices with fully coalesced
-  //      16-byte cp.async into shared memory (row pitch 68 floats: a thread-per-row read is then conflict free) and
-  //      every thread picks up its row from there; d = 128: straight from global memory (three 64 KB matrices do not fit)
-  constexpr bool kStageRows = D == 64;
-  constexpr int kPitch = 68;
-  extern __shared__ __align__(16) float msm[];  // [groups][D][kPitch] when kStageRows
-  RowRegs64 rowreg;
-  if (kStageRows) {
-    constexpr int NG_ = kAppend ? 3 : 2;
-    for (int idx = tid; idx < NG_ * D * (D / 4); idx += NT) {
-      const int gsel = idx / (D * (D / 4)), rem = idx % (D * (D / 4)), r = rem / (D / 4), c4 = rem % (D / 4);
-      const float* M = gsel == 0 ? a.pi_k + lh * D * D : gsel == 1 ? a.S : a.pi_v + lh * D * D;
-      const unsigned dst = (unsigned)__cvta_generic_to_shared(msm + ((size_t)gsel * D + r) * kPitch + 4 * c4);
-      asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(M + (size_t)r * D + 4 * c4) : "memory");
+  pdl_trigger();  // the streaming kernel behind this one may be scheduled
+  if constexpr (EB == 8) {  // rows [24, 32) pad the value block to a whole m-tile
+    for (int idx = tid; idx < 8 * Cfg::HP / 2; idx += NT) {
+      reinterpret_cast<unsigned*>(Ah + (size_t)24 * Cfg::HP)[idx] = 0u;
+      reinterpret_cast<unsigned*>(Al + (size_t)24 * Cfg::HP)[idx] = 0u;
     }
-    asm volatile("cp.async.commit_group;" ::: "memory");
-  } else {
-    const float* M = grp == 0 ? a.pi_k + lh * D * D : grp == 1 ? a.S : a.pi_v + lh * D * D;
-    rowreg.load(M + (size_t)row * D + part * 64);
+    if (tid < 8) rscale[24 + tid] = 0.f;
   }
   if (tid < 8) lutK[tid] = a.lut_k[lh * 8 + tid];
   if (tid >= 32 && tid < 40) lutV[tid - 32] = a.lut_v[lh * 8 + tid - 32];
-  for (int bgi = bg_first; bgi < bg_end; ++bgi) {
-  const int b0 = bgi * BG, nb = min(BG, B - b0);
-  // ---- the cache lengths first: the RoPE positions and the target tile slot hang off them
-  int len_e[BG];
-#pragma unroll
-  for (int e = 0; e < BG; ++e) len_e[e] = e < nb ? __ldcg(a.cv.seq_len + layer * B + b0 + e) : 0;
-  // ---- stage-4 work item of this thread (one 16-bit or 8-bit piece of one token in the device tile layout,
-  //      tq_common.cuh), and an early read of the V halfword it will modify (a V field is shared with the other token
-  //      of the pair, which was appended by an earlier call)
-  constexpr int HW = 3 * D / 64;  // halfwords per (lane, token) block of K fields, and per (lane, token pair) block of V fields
-  constexpr int IT_K = 4 * HW, IT_S = 4 * Lo::U * 2, IT_V = 8 * HW;
-  constexpr int ITEMS = IT_K + IT_S + IT_V + 1;
-  static_assert(!kAppend || BG * ITEMS <= NT, "one output item per thread");
-  const int it_e = tid / ITEMS, it = tid % ITEMS;
-  int it_len = len_e[0];
-#pragma unroll
-  for (int j = 1; j < BG; ++j) it_len = it_e == j ? len_e[j] : it_len;
-  const bool it_on = kAppend && it_e < nb && it_len < a.cv.max_seq;
-  unsigned char* it_tp = a.cv.tiles + (((size_t)layer * B + b0 + min(it_e, nb - 1)) * H + h) * a.cv.stream_bytes +
-                         (size_t)(min(it_len, a.cv.max_seq - 1) / kTile) * Lo::kTileBytes;
-  const int it_slot = it_len % kTile;
-  unsigned short vold = 0;
-  unsigned short* vptr = nullptr;
-  if (it_on && it >= IT_K + IT_S && it < IT_K + IT_S + IT_V) {
-    const int vi = it - IT_K - IT_S, gi = vi / HW, hw = vi % HW, pp = it_slot >> 1;
-    const int hidx = (pp >> 2) * HW + hw;  // halfword of lane (gi, pp & 3)'s V string
-    vptr = reinterpret_cast<unsigned short*>(it_tp + Lo::kOffVC + word_offset(Lo::KCW, hidx >> 1, 4 * gi + (pp & 3))) + (hidx & 1);
-    vold = __ldcg(vptr);
+  // ---- the cache lengths first: the RoPE positions and the target tile slots hang off them.  (The length of an entry
+  //      cannot change while its heads are still arriving.)
+  if (tid >= 64 && tid < 64 + EB) {
+    const int e = tid - 64;
+    const int len0 = e < nb ? __ldcg(a.cv.seq_len + layer * B + b0 + e) : 0;
+    s_len0[e] = len0;
+    s_full[e] = kAppend && len0 >= a.cv.max_seq;
   }
+  __syncthreads();
 
-  // ---- inputs of the BG batch entries of this head, RoPE applied to k and q (positions read on the device)
-  for (int idx = tid; idx < BG * HP; idx += NT) {
-    const int e = idx / HP, g = idx % HP;
-    const int ia = a.rope_layout == 0 ? 2 * g : g, ib = a.rope_layout == 0 ? 2 * g + 1 : g + HP;
-    float ka = 0.f, kb = 0.f, qa = 0.f, qb = 0.f;
-    if (e < nb) {
-      const int b = b0 + e;
-      int len0 = len_e[0];
+  // ---- the store stage at the end is warp-per-entry with fixed lane roles (device tile layout, tq_common.cuh):
+  //      lanes [0, 4)  : K pair fields of lane-target t = lane (one block of HW halfwords)
+  //      lanes [4, 4 + 8 U) : sign bytes (t, piece u, byte half hb)
+  //      lanes [20, 28): V fields of lane-target gi = lane - 20 (three-bit slices inside HW halfwords, read-modify-write:
+  //                      a V field is shared with the other token of the pair, appended by an earlier call)
+  //      lane 28       : the three norms
+  //      The V halfwords are requested here, long before they are needed.
+  constexpr int HW = 3 * D / 64;       // halfwords per (lane, token) block of K fields, and per (lane, token pair) block of V fields
+  constexpr int EPW = EB / NW;         // entries per warp in the store stage
+  unsigned short vold[EPW][HW];
+  if (kAppend) {
 #pragma unroll
-      for (int j = 1; j < BG; ++j) len0 = e == j ? len_e[j] : len0;
-      const bool full = kAppend && len0 >= a.cv.max_seq;
-      const int len1 = (kAppend && !full) ? len0 + 1 : len0;  // length the decode kernel will see
-      const size_t uc = ((size_t)lc * B + b) * H + h;
-      if (g == 0) {
-        s_len0[e] = len0;
-        s_full[e] = full;
-      }
-      if (kAppend) {  // the appended key sits at index len0
-        const int kpos = min(len0, a.cv.max_seq - 1);
-        const T* kp = reinterpret_cast<const T*>(a.k) + uc * D;
-        const float xa = load_as_float<T>(kp + ia), xb = load_as_float<T>(kp + ib);
-        const float2 cs = *reinterpret_cast<const float2*>(a.rope_cs + ((size_t)kpos * HP + g) * 2);
-        ka = xa * cs.x - xb * cs.y;
-        kb = xa * cs.y + xb * cs.x;
-      }
-      if (kQuery) {  // the query defaults to the newest cached token
-        int qpos = a.q_pos ? a.q_pos[lc * B + b] : len1 - 1;
-        qpos = max(0, min(qpos, a.cv.max_seq - 1));
-        const T* qp = reinterpret_cast<const T*>(a.q) + uc * D;
-        const float xa = load_as_float<T>(qp + ia), xb = load_as_float<T>(qp + ib);
-        const float2 cs = *reinterpret_cast<const float2*>(a.rope_cs + ((size_t)qpos * HP + g) * 2);
-        qa = xa * cs.x - xb * cs.y;
-        qb = xa * cs.y + xb * cs.x;
-        if (len1 <= 0) {  // empty cache: no tile for this unit in the streaming kernel, out = 0
-          T* outp = reinterpret_cast<T*>(a.out) + uc * D;
-          if constexpr (sizeof(T) == 2) outp[ia] = outp[ib] = __float2half_rn(0.f);
-          else outp[ia] = outp[ib] = 0.f;
+    for (int n = 0; n < EPW; ++n) {
+      const int e = warp + n * NW;
+#pragma unroll
+      for (int hw = 0; hw < HW; ++hw) vold[n][hw] = 0;
+      if (e < nb && lane >= 20 && lane < 28 && s_len0[e] < a.cv.max_seq) {
+        const int len = s_len0[e], slot = len % kTile, pp = slot >> 1, gi = lane - 20;
+        const unsigned char* tp = a.cv.tiles + stream_of(e) * a.cv.stream_bytes + (size_t)(len / kTile) * Lo::kTileBytes;
+#pragma unroll
+        for (int hw = 0; hw < HW; ++hw) {
+          const int hidx = (pp >> 2) * HW + hw;  // halfword of lane (gi, pp & 3)'s V string
+          vold[n][hw] = __ldcg(reinterpret_cast<const unsigned short*>(tp + Lo::kOffVC + word_offset(Lo::KCW, hidx >> 1, 4 * gi + (pp & 3))) +
+                               (hidx & 1));
         }
       }
     }
-    if (kAppend) xk[e][ia] = ka, xk[e][ib] = kb;
-    if (kQuery) xq[e][ia] = qa, xq[e][ib] = qb;
-  }
-  if (kAppend) {
-    for (int idx = tid; idx < BG * D; idx += NT) {
-      const int e = idx / D, i = idx % D;
-      xv[e][i] = e < nb ? load_as_float<T>(reinterpret_cast<const T*>(a.v) + (((size_t)lc * B + b0 + e) * H + h) * D + i) : 0.f;
-    }
-  }
-  if (kStageRows && bgi == bg_first) asm volatile("cp.async.wait_group 0;" ::: "memory");
-  __syncthreads();
-  if (kStageRows && bgi == bg_first) rowreg.load_shared(msm + ((size_t)grp * D + row) * kPitch);
-
-  // ---- stage 1: rotations (groups 0 and 2) and the norms of the rotated key / value
-  float yk[BG], yv[BG];
-  if (grp == 0) {
-    float aq[BG];
-#pragma unroll
-    for (int e = 0; e < BG; ++e) yk[e] = 0.f, aq[e] = 0.f;
-    if (kAppend) rowreg.dot<BG>(&xk[0][part * 64], D, yk);
-    if (kQuery) rowreg.dot<BG>(&xq[0][part * 64], D, aq);
-#pragma unroll
-    for (int e = 0; e < BG; ++e) {
-      if (TPR == 2) {
-        yk[e] += __shfl_xor_sync(0xffffffffu, yk[e], 1);
-        aq[e] += __shfl_xor_sync(0xffffffffu, aq[e], 1);
-      }
-      if (kAppend) {
-        const float ss = warp_sum(part == 0 ? yk[e] * yk[e] : 0.f);
-        if (lane == 0) redk[e][wg] = ss;
-      }
-      if (kQuery && part == 0) {
-        yq[e][row] = aq[e];
-      }
-    }
-  } else if (kAppend && grp == 2) {
-#pragma unroll
-    for (int e = 0; e < BG; ++e) yv[e] = 0.f;
-    rowreg.dot<BG>(&xv[0][part * 64], D, yv);
-#pragma unroll
-    for (int e = 0; e < BG; ++e) {
-      if (TPR == 2) yv[e] += __shfl_xor_sync(0xffffffffu, yv[e], 1);
-      const float ss = warp_sum(part == 0 ? yv[e] * yv[e] : 0.f);
-      if (lane == 0) redv[e][wg] = ss;
-    }
-  }
-  __syncthreads();
-
-  // ---- stage 2 (append): unit vectors, codes, residual and its norm
-  if (kAppend) {
-    if (grp == 0 && part == 0) {
-#pragma unroll
-      for (int e = 0; e < BG; ++e) {
-        float n2 = 0.f;
-#pragma unroll
-        for (int w = 0; w < WG; ++w) n2 += redk[e][w];
-        const float n = sqrtf(n2);
-        const float u = n > 0.f ? yk[e] / n : 0.f;
-        const int c = code_of7(u, lutK);
-        const float r = u - lutK[c];
-        cK[e][row] = (unsigned char)c;
-        rr[e][row] = r;
-        yk[e] = r * r;
-      }
-    }
-    if (grp == 0) {  // whole warps: the shuffles need every lane
-#pragma unroll
-      for (int e = 0; e < BG; ++e) {
-        const float ss = warp_sum(part == 0 ? yk[e] : 0.f);
-        if (lane == 0) redr[e][wg] = ss;
-      }
-    } else if (grp == 2 && part == 0) {
-#pragma unroll
-      for (int e = 0; e < BG; ++e) {
-        float n2 = 0.f;
-#pragma unroll
-        for (int w = 0; w < WG; ++w) n2 += redv[e][w];
-        const float n = sqrtf(n2);
-        const float u = n > 0.f ? yv[e] / n : 0.f;
-        cV[e][row] = (unsigned char)code_of7(u, lutV);
-      }
-    }
-    __syncthreads();
   }
 
-  // ---- stage 3: sketch of the residual (bits) and of the rotated query (z)
-  if (grp == 1) {
-    float sr[BG], zq[BG];
+  // ---- stage 1: one warp per (entry, vector): load, RoPE, 2^-exponent(max) scaling, fp16 hi / lo operand rows.
+  //      Lane l owns RoPE pairs l + 32 j.  The loads of kTB tasks are issued before the first one is used (a task is one
+  //      DRAM round trip; a warp has twelve of them).
+  constexpr int NVEC = (kAppend ? 2 : 0) + (kQuery ? 1 : 0);  // k, v | q
+  constexpr int NTASK = EB * NVEC / NW;                        // tasks per warp: 12 | 8 | 4 (EB = 32), 3 | 2 | 1 (EB = 8)
+  constexpr int kTB = NTASK <= 4 ? NTASK : ((D == 64 && NTASK == 12) ? 6 : 4);
+  static_assert(NTASK % kTB == 0, "whole batches");
+  for (int tb0 = 0; tb0 < NTASK; tb0 += kTB) {
+    float xa[kTB][PL], xb[kTB][PL];
+    float2 cs[kTB][PL];
 #pragma unroll
-    for (int e = 0; e < BG; ++e) sr[e] = 0.f, zq[e] = 0.f;
-    if (kAppend) rowreg.dot<BG>(&rr[0][part * 64], D, sr);
-    if (kQuery) rowreg.dot<BG>(&yq[0][part * 64], D, zq);
+    for (int q = 0; q < kTB; ++q) {
+      const int task = warp + (tb0 + q) * NW, e = task % EB;
+      const int vec = (!kAppend) ? 2 : (task / EB == 0 ? 0 : (task / EB == 1 ? 1 : 2));  // 0 = k, 1 = v, 2 = q
 #pragma unroll
-    for (int e = 0; e < BG; ++e) {
-      if (TPR == 2) {
-        sr[e] += __shfl_xor_sync(0xffffffffu, sr[e], 1);
-        zq[e] += __shfl_xor_sync(0xffffffffu, zq[e], 1);
+      for (int j = 0; j < PL; ++j) xa[q][j] = xb[q][j] = 0.f, cs[q][j] = make_float2(1.f, 0.f);
+      if (e < nb) {
+        const T* src = reinterpret_cast<const T*>(vec == 0 ? a.k : (vec == 1 ? a.v : a.q)) + unit_of(e) * D;
+        const int len0 = s_len0[e];
+        int pos = 0;
+        if (vec == 0) pos = min(len0, a.cv.max_seq - 1);  // the appended key sits at index len0
+        if (vec == 2) {                                    // the query defaults to the newest cached token
+          const int len1 = (kAppend && !s_full[e]) ? len0 + 1 : len0;
+          pos = a.q_pos ? a.q_pos[lc * B + b0 + e] : len1 - 1;
+          pos = max(0, min(pos, a.cv.max_seq - 1));
+          if (len1 <= 0) {  // empty cache: no tile for this unit in the streaming kernel, out = 0
+            T* outp = reinterpret_cast<T*>(a.out) + unit_of(e) * D;
+            for (int i = lane; i < D; i += 32) {
+              if constexpr (sizeof(T) == 2) outp[i] = __float2half_rn(0.f);
+              else outp[i] = 0.f;
+            }
+          }
+        }
+#pragma unroll
+        for (int j = 0; j < PL; ++j) {
+          const int gp = lane + 32 * j;
+          const bool adj = vec == 1 || a.rope_layout == 0;
+          const int ia = adj ? 2 * gp : gp, ib = adj ? 2 * gp + 1 : gp + HPAIR;
+          xa[q][j] = load_as_float<T>(src + ia), xb[q][j] = load_as_float<T>(src + ib);
+          if (vec != 1) cs[q][j] = __ldg(reinterpret_cast<const float2*>(a.rope_cs + ((size_t)pos * HPAIR + gp) * 2));
+        }
       }
-      if (part == 0) {
-        if (kAppend) bitb[e][row] = sr[e] >= 0.f ? 1 : 0;
-        if (kQuery) zs[e][row] = zq[e];
+    }
+#pragma unroll
+    for (int q = 0; q < kTB; ++q) {
+      const int task = warp + (tb0 + q) * NW, e = task % EB;
+      const int vec = (!kAppend) ? 2 : (task / EB == 0 ? 0 : (task / EB == 1 ? 1 : 2));
+      const int orow = vec == 0 ? e : (vec == 2 ? EB + e : 2 * EB + e);
+      float amax = 0.f;
+#pragma unroll
+      for (int j = 0; j < PL; ++j) {
+        amax = fmaxf(amax, fmaxf(fabsf(xa[q][j]), fabsf(xb[q][j])));
+        const float ya = xa[q][j] * cs[q][j].x - xb[q][j] * cs[q][j].y, yb = xa[q][j] * cs[q][j].y + xb[q][j] * cs[q][j].x;
+        xa[q][j] = ya, xb[q][j] = yb;
+      }
+      amax = warp_max(amax);
+      float sc, inv_s;
+      pow2_scale_p(amax, sc, inv_s);  // |RoPE(x) s| < 2 sqrt 2
+      if (lane == 0) rscale[orow] = inv_s * 0.0625f;  // y = 16 s PI x
+#pragma unroll
+      for (int j = 0; j < PL; ++j) {
+        const int gp = lane + 32 * j;
+        const bool adj = vec == 1 || a.rope_layout == 0;
+        const int ia = adj ? 2 * gp : gp, ib = adj ? 2 * gp + 1 : gp + HPAIR;
+        if (adj) {
+          unsigned hi, lo;
+          split_pair(xa[q][j] * sc, xb[q][j] * sc, hi, lo);
+          *reinterpret_cast<unsigned*>(Ah + (size_t)orow * Cfg::HP + ia) = hi;
+          *reinterpret_cast<unsigned*>(Al + (size_t)orow * Cfg::HP + ia) = lo;
+        } else {
+          const __half ha = __float2half_rn(xa[q][j] * sc), hb = __float2half_rn(xb[q][j] * sc);
+          Ah[(size_t)orow * Cfg::HP + ia] = ha, Ah[(size_t)orow * Cfg::HP + ib] = hb;
+          Al[(size_t)orow * Cfg::HP + ia] = __float2half_rn(xa[q][j] * sc - __half2float(ha));
+          Al[(size_t)orow * Cfg::HP + ib] = __float2half_rn(xb[q][j] * sc - __half2float(hb));
+        }
       }
     }
   }
   __syncthreads();
+
+  // ---- stage 2: [k rows; q rows] x PI_K^T and [v rows] x PI_V^T: a warp owns n-tiles warp, warp + 8, ...
+  //      product over the k / q row blocks with matrix M (EB = 8: both blocks are one m-tile)
+  auto kq_product = [&](const float* M, float mscale, int n0) {
+    constexpr int HPI = Cfg::HP;
+    if constexpr (EB == 8) {
+      gemm_rows<D, HPI, 1, true>(Ah, Al, 0, M, mscale, n0, Y, rscale, lane);
+    } else if (kAppend && kQuery) {
+      if (mt_n == 2) gemm_rows<D, HPI, 4, true>(Ah, Al, 0, M, mscale, n0, Y, rscale, lane);
+      else {
+        gemm_rows<D, HPI, 1, true>(Ah, Al, 0, M, mscale, n0, Y, rscale, lane);
+        gemm_rows<D, HPI, 1, true>(Ah, Al, EB, M, mscale, n0, Y, rscale, lane);
+      }
+    } else {
+      const int m0 = kAppend ? 0 : EB;
+      if (mt_n == 2) gemm_rows<D, HPI, 2, true>(Ah, Al, m0, M, mscale, n0, Y, rscale, lane);
+      else gemm_rows<D, HPI, 1, true>(Ah, Al, m0, M, mscale, n0, Y, rscale, lane);
+    }
+  };
+  for (int nt = warp; nt < D / 8; nt += NW) {
+    kq_product(a.pi_k + lh * D * D, 16.f, 8 * nt);
+    if (kAppend) {
+      const float* Pv = a.pi_v + lh * D * D;
+      if (EB == 8 || mt_n == 1) gemm_rows<D, Cfg::HP, 1, kValLo>(Ah, Al, 2 * EB, Pv, 16.f, 8 * nt, Y, rscale, lane);
+      else gemm_rows<D, Cfg::HP, 2, kValLo>(Ah, Al, 2 * EB, Pv, 16.f, 8 * nt, Y, rscale, lane);
+    }
+  }
+  __syncthreads();
+
+  // ---- stage 3: one warp per (entry, vector): norms, codes, residual; operand rows of the sketch product
+  //      (rows [0, 32): r x 8; rows [32, 64): q'' 2^eq, which are also the decode kernel's q operand)
+  for (int task = warp; task < EB * NVEC; task += NW) {
+    const int e = task % EB;
+    const int vec = (!kAppend) ? 2 : (task / EB == 0 ? 0 : (task / EB == 1 ? 1 : 2));
+    const int yrow = vec == 0 ? e : (vec == 2 ? EB + e : 2 * EB + e);
+    if (e >= nb) continue;  // padding rows stay zero
+    const float* y = Y + (size_t)yrow * Cfg::FP;
+    float2 v2[PL];
+#pragma unroll
+    for (int j = 0; j < PL; ++j) v2[j] = *reinterpret_cast<const float2*>(y + 2 * (lane + 32 * j));
+    if (vec == 2) {  // q'': power-of-two scaling that puts max |q''| 2^eq in [2^13, 2^14), hi / lo rows
+      float qm = 0.f;
+#pragma unroll
+      for (int j = 0; j < PL; ++j) qm = fmaxf(qm, fmaxf(fabsf(v2[j].x), fabsf(v2[j].y)));
+      qm = warp_max(qm);
+      const int E = (int)((__float_as_uint(qm) >> 23) & 0xffu);
+      const int eq = 13 - ((E == 0 || E == 255) ? 0 : E - 127);
+      const float sq = __uint_as_float((unsigned)(max(-100, min(100, eq)) + 127) << 23);
+#pragma unroll
+      for (int j = 0; j < PL; ++j) {
+        unsigned hi, lo;
+        split_pair(v2[j].x * sq, v2[j].y * sq, hi, lo);
+        *reinterpret_cast<unsigned*>(Ah + (size_t)yrow * Cfg::HP + 2 * (lane + 32 * j)) = hi;
+        *reinterpret_cast<unsigned*>(Al + (size_t)yrow * Cfg::HP + 2 * (lane + 32 * j)) = lo;
+      }
+      if (lane == 0) {
+        rscale[yrow] = 1.f / sq;  // z = S q'': undo 2^eq (exact)
+        qsc[e][0] = 1.f / sq;
+      }
+      continue;
+    }
+    float n2 = 0.f;
+#pragma unroll
+    for (int j = 0; j < PL; ++j) n2 = fmaf(v2[j].x, v2[j].x, fmaf(v2[j].y, v2[j].y, n2));
+    n2 = warp_sum(n2);
+    const float n = sqrtf(n2);
+    const float inv = n > 0.f ? 1.0f / n : 0.f;
+    const float* lut = vec == 0 ? lutK : lutV;
+    float g2 = 0.f;
+#pragma unroll
+    for (int j = 0; j < PL; ++j) {
+      const int i0 = 2 * (lane + 32 * j);
+      const float u0 = v2[j].x * inv, u1 = v2[j].y * inv;
+      const int c0 = code_of7(u0, lut), c1 = code_of7(u1, lut);
+      if (vec == 0) {
+        const float r0 = u0 - lut[c0], r1 = u1 - lut[c1];
+        g2 = fmaf(r0, r0, fmaf(r1, r1, g2));
+        cK[e][i0] = (unsigned char)c0, cK[e][i0 + 1] = (unsigned char)c1;
+        unsigned hi, lo;
+        split_pair(r0 * 8.f, r1 * 8.f, hi, lo);  // only sign(S r) is used
+        *reinterpret_cast<unsigned*>(Ah + (size_t)yrow * Cfg::HP + i0) = hi;
+        *reinterpret_cast<unsigned*>(Al + (size_t)yrow * Cfg::HP + i0) = lo;
+      } else {
+        cV[e][i0] = (unsigned char)c0, cV[e][i0 + 1] = (unsigned char)c1;
+      }
+    }
+    if (vec == 0) {
+      g2 = warp_sum(g2);
+      if (lane == 0) nrm[0][e] = n, nrm[1][e] = sqrtf(g2), rscale[yrow] = 1.f;
+    } else if (lane == 0) {
+      nrm[2][e] = n;
+    }
+  }
+  __syncthreads();
+
+  // ---- stage 4: [r rows; q'' rows] x S^T -> sign bits | z
+  for (int nt = warp; nt < D / 8; nt += NW) kq_product(a.S, 1.f, 8 * nt);
+  __syncthreads();
+
   if (kQuery) {
-    // ---- the decode kernel's operands (tq_common.cuh FragLayout): power-of-two scalings that put max |q''_s|, max |z_s|
-    //      in [2^13, 2^14), fp16 hi + lo splits in B-fragment order; and the head's dequantisation tables
-    using FL = FragLayout<D>;
-    const int warp_id = tid >> 5;
-    if (warp_id < BG) {  // one warp per entry: maxima and the sum of z
-      const int e = warp_id;
-      float qm = 0.f, zm = 0.f, zsum = 0.f;
+    // ---- the decode kernel's operands (tq_common.cuh FragLayout), one warp per entry.  The q words are the q'' 2^eq
+    //      operand rows as they stand (kscale = 2^-eq log2(e)/sqrt(d)); z = S q'' is scaled to max |z_s| 2^ez in
+    //      [2^13, 2^14) and split per sketch row with the fragment's 2^-p weights.
+    for (int e = warp; e < nb; e += NW) {
+      const float* z = Y + (size_t)(EB + e) * Cfg::FP;
+      float zm = 0.f, zsum = 0.f;
 #pragma unroll
       for (int i = lane; i < D; i += 32) {
-        qm = fmaxf(qm, fabsf(yq[e][i] * kScaleK));
-        const float zv = zs[e][i] * kScaleS;
+        const float zv = z[i] * kScaleS;
         zm = fmaxf(zm, fabsf(zv));
         zsum += zv;
       }
-      qm = warp_max(qm), zm = warp_max(zm), zsum = warp_sum(zsum);
-      auto expo = [](float x) {
-        const int E = (int)((__float_as_uint(x) >> 23) & 0xffu);
-        return (E == 0 || E == 255) ? 0 : E - 127;
-      };
+      zm = warp_max(zm), zsum = warp_sum(zsum);
+      const int E = (int)((__float_as_uint(zm) >> 23) & 0xffu);
+      const int ez = 13 - ((E == 0 || E == 255) ? 0 : E - 127);
       auto p2 = [](int ee) { return __uint_as_float((unsigned)(max(-100, min(100, ee)) + 127) << 23); };
-      const int eq = 13 - expo(qm), ez = 13 - expo(zm);
-      if (lane == 0) {
-        fscal[e][0] = p2(eq) * kScaleK;
-        fscal[e][1] = p2(ez) * kScaleS;
-        if (e < nb) {
-          float* sc = reinterpret_cast<float*>(a.frags + (((size_t)lc * B + b0 + e) * H + h) * FL::kWords + FL::kScalOff);
-          sc[0] = p2(-eq), sc[1] = p2(25 - ez), sc[2] = zsum, sc[3] = 0.f;
+      unsigned* fb = a.frags + unit_of(e) * FL::kWords;
+      const __half* qh = Ah + (size_t)(EB + e) * Cfg::HP;
+      const __half* ql = Al + (size_t)(EB + e) * Cfg::HP;
+      for (int wi = lane; wi < FL::kScalOff; wi += 32) {
+        const int pat = wi / FL::kWordsPerPat, wd = wi % FL::kWordsPerPat, t = pat & 3;
+        const bool lo = pat >> 2;
+        unsigned word;
+        if (wd < 2 * FL::KS) {
+          const int c0 = 16 * (wd >> 1) + 2 * t + 8 * (wd & 1);
+          word = *reinterpret_cast<const unsigned*>((lo ? ql : qh) + c0);
+        } else {
+          const int ks = (wd - 2 * FL::KS) >> 1, reg = wd & 1, p0 = 2 * (ks & 3);
+          const int rho = t * (D / 4) + 16 * (ks >> 2) + p0 + reg;
+          const float sc = kScaleS * p2(ez - p0 - reg);
+          unsigned hi, lw;
+          split_pair(z[rho] * sc, z[rho + 8] * sc, hi, lw);
+          word = lo ? lw : hi;
         }
+        fb[wi] = word;
+      }
+      if (lane == 0) {
+        float* sc = reinterpret_cast<float*>(fb + FL::kScalOff);
+        sc[0] = qsc[e][0] * kScaleK, sc[1] = p2(25 - ez), sc[2] = zsum, sc[3] = 0.f;
       }
     }
-    __syncthreads();
-    auto split2 = [](float x0, float x1, bool lo) {
-      const __half h0 = __float2half_rn(x0), h1 = __float2half_rn(x1);
-      const __half l0 = __float2half_rn(x0 - __half2float(h0)), l1 = __float2half_rn(x1 - __half2float(h1));
-      return lo ? ((unsigned)__half_as_ushort(l0) | ((unsigned)__half_as_ushort(l1) << 16))
-                : ((unsigned)__half_as_ushort(h0) | ((unsigned)__half_as_ushort(h1) << 16));
-    };
-    for (int idx = tid; idx < BG * FL::kScalOff; idx += NT) {
-      const int e = idx / FL::kScalOff, wi = idx % FL::kScalOff;
-      if (e >= nb) continue;
-      const int pat = wi / FL::kWordsPerPat, wd = wi % FL::kWordsPerPat, t = pat & 3;
-      const bool lo = pat >> 2;
-      unsigned word;
-      if (wd < 2 * FL::KS) {
-        const int c0 = 16 * (wd >> 1) + 2 * t + 8 * (wd & 1);
-        word = split2(yq[e][c0] * fscal[e][0], yq[e][c0 + 1] * fscal[e][0], lo);
-      } else {
-        const int ks = (wd - 2 * FL::KS) >> 1, reg = wd & 1, p0 = 2 * (ks & 3);
-        const int rho = t * (D / 4) + 16 * (ks >> 2) + p0 + reg;
-        const float sc = fscal[e][1] * __uint_as_float((unsigned)(127 - p0 - reg) << 23);
-        word = split2(zs[e][rho] * sc, zs[e][rho + 8] * sc, lo);
-      }
-      a.frags[(((size_t)lc * B + b0 + e) * H + h) * FL::kWords + wi] = word;
-    }
-    if (tid < 64 && bgi == bg_first) {  // every CTA of the head writes the same values
+    if (tid < 64 && run == 0) {  // the head's dequantisation tables
+      auto pair16 = [](float x0, float x1, bool lo) {
+        unsigned hi, lw;
+        split_pair(x0, x1, hi, lw);
+        return lo ? lw : hi;
+      };
       const int c0 = tid & 7, c1 = tid >> 3;
       unsigned* tb = a.tabs + (size_t)lh_c * kTabWords;
-      tb[tid] = split2(lutK[c0], lutK[c1], false);
-      tb[64 + tid] = split2(lutK[c0], lutK[c1], true);
-      tb[128 + tid] = split2(lutV[c0], lutV[c1], false);
-      tb[192 + tid] = split2(lutV[c0], lutV[c1], true);
+      tb[tid] = pair16(lutK[c0], lutK[c1], false);
+      tb[64 + tid] = pair16(lutK[c0], lutK[c1], true);
+      tb[128 + tid] = pair16(lutV[c0], lutV[c1], false);
+      tb[192 + tid] = pair16(lutV[c0], lutV[c1], true);
       if (tid == 0) {
         bool exact = true;
 #pragma unroll
@@ -368,52 +451,68 @@ __global__ void __launch_bounds__((kAppend ? 3 : 2) * PrepCfg<D>::GT) prep_kerne
       }
     }
   }
-  if (!kAppend) {
-    __syncthreads();  // the next group of the run reuses the shared arrays
-    continue;
-  }
+  if (!kAppend) return;
 
-  // ---- stage 4 (append): every thread assembles one piece of one token in the device tile layout
-  if (it_on) {
-    const int e = it_e, slot = it_slot, g = slot & 7, r = slot >> 3;
-    unsigned char* tp = it_tp;
-    // bits [16 hw, 16 hw + 16) of a string of NB-bit pieces at stride 6 bits: piece k = val(k) at bit 6 k + off
-    auto gather16 = [&](int hw, int nfields, int off, int nb_, auto val, unsigned& out, unsigned& mask) {
-      out = 0, mask = 0;
-      for (int k = 0; k < nfields; ++k) {
-        const int sh = 6 * k + off - 16 * hw;
-        if (sh <= -nb_ || sh >= 16) continue;
-        const unsigned v = val(k), mk = (1u << nb_) - 1u;
-        out |= sh >= 0 ? (v << sh) : (v >> (-sh));
-        mask |= sh >= 0 ? (mk << sh) : (mk >> (-sh));
+  // ---- stage 5 (append): one warp per entry assembles the token's pieces (lane roles above)
+#pragma unroll
+  for (int n = 0; n < EPW; ++n) {
+    const int e = warp + n * NW;
+    if (e >= nb || s_full[e]) continue;
+    const int len = s_len0[e], slot = len % kTile, g = slot & 7, r = slot >> 3;
+    unsigned char* tp = a.cv.tiles + stream_of(e) * a.cv.stream_bytes + (size_t)(len / kTile) * Lo::kTileBytes;
+    if (lane < 4) {  // K: pairs t + 4 j, field j at bit 6 j of the block
+      const int t = lane;
+      unsigned long long lo = 0ull, hi = 0ull;
+#pragma unroll
+      for (int j = 0; j < Lo::J; ++j) {
+        const int p = t + 4 * j;
+        const unsigned long long f = (unsigned)(cK[e][2 * p] | (cK[e][2 * p + 1] << 3));
+        const int bit = 6 * j;
+        if (bit < 64) lo |= f << bit;
+        if (bit + 6 > 64) hi |= bit >= 64 ? f << (bit - 64) : f >> (64 - bit);
       }
-      out &= 0xffffu, mask &= 0xffffu;
-    };
-    if (it < IT_K) {  // K pair fields of lane (g, t): pairs t + 4 j, block r of the lane's string
-      const int t = it / HW, hw = it % HW;
-      unsigned v, mk;
-      gather16(hw, Lo::J, 0, 6, [&](int j) { const int p = t + 4 * j; return (unsigned)(cK[e][2 * p] | (cK[e][2 * p + 1] << 3)); }, v, mk);
-      const int hidx = r * HW + hw;
-      reinterpret_cast<unsigned short*>(tp + Lo::kOffKC + word_offset(Lo::KCW, hidx >> 1, 4 * g + t))[hidx & 1] = (unsigned short)v;
-    } else if (it < IT_K + IT_S) {  // sign bytes: lane (g, t), piece u, byte half hb
-      const int si = it - IT_K, t = si / (2 * Lo::U), u = (si / 2) % Lo::U, hb = si & 1;
+#pragma unroll
+      for (int hw = 0; hw < HW; ++hw) {
+        const int hidx = r * HW + hw;
+        const unsigned short v = (unsigned short)(hw < 4 ? lo >> (16 * hw) : hi >> (16 * (hw - 4)));
+        reinterpret_cast<unsigned short*>(tp + Lo::kOffKC + word_offset(Lo::KCW, hidx >> 1, 4 * g + t))[hidx & 1] = v;
+      }
+    } else if (lane < 4 + 8 * Lo::U) {  // sign bytes: bit k = [(S r)_rho >= 0], rho = t d/4 + 16 u + 8 hb + k
+      const int si = lane - 4, t = si / (2 * Lo::U), u = (si / 2) % Lo::U, hb = si & 1;
+      const float* sr = Y + (size_t)e * Cfg::FP + t * (D / 4) + 16 * u + 8 * hb;
       unsigned v = 0;
-      for (int k = 0; k < 8; ++k) v |= (unsigned)bitb[e][t * (D / 4) + 16 * u + 8 * hb + k] << k;
+#pragma unroll
+      for (int k = 0; k < 8; ++k) v |= (sr[k] >= 0.f ? 1u : 0u) << k;
       const int word = (slot >> 4) * Lo::U + u, byte = 2 * hb + (r & 1);
       *(tp + Lo::kOffKS + word_offset(Lo::KSW, word, 4 * g + t) + byte) = (unsigned char)v;
-    } else if (it < IT_K + IT_S + IT_V) {  // V codes: lane (gi, pp & 3), three-bit slices at 6 c + 3 (slot & 1)
-      const int vi = it - IT_K - IT_S, gi = vi / HW, hw = vi % HW;
-      unsigned v, mk;
-      gather16(hw, Lo::C, 3 * (slot & 1), 3, [&](int c) { return (unsigned)cV[e][gi + 8 * c]; }, v, mk);
-      *vptr = (unsigned short)((vold & ~mk) | v);
-    } else {
-      float nk = 0.f, nr = 0.f, nv = 0.f;
+    } else if (lane >= 20 && lane < 28) {  // V: coordinates gi + 8 c, three-bit slices at 6 c + 3 (slot & 1)
+      const int gi = lane - 20, pp = slot >> 1, sh0 = 3 * (slot & 1);
+      unsigned long long lo = 0ull, hi = 0ull, mlo = 0ull, mhi = 0ull;
 #pragma unroll
-      for (int w = 0; w < WG; ++w) nk += redk[e][w], nr += redr[e][w], nv += redv[e][w];
+      for (int c = 0; c < Lo::C; ++c) {
+        const unsigned long long f = cV[e][gi + 8 * c], m7 = 7ull;
+        const int bit = 6 * c;  // + sh0 (< 6), so a slice never straddles bit 64 when 6 c + 6 <= 64 or 6 c >= 64
+        if (bit + 6 <= 64) lo |= f << (bit + sh0), mlo |= m7 << (bit + sh0);
+        else if (bit >= 64) hi |= f << (bit - 64 + sh0), mhi |= m7 << (bit - 64 + sh0);
+        else {  // field 10 of d = 128 covers bits [60, 66)
+          const unsigned long long f6 = f << sh0, m6 = m7 << sh0;
+          lo |= f6 << bit, mlo |= m6 << bit;
+          hi |= f6 >> (64 - bit), mhi |= m6 >> (64 - bit);
+        }
+      }
+#pragma unroll
+      for (int hw = 0; hw < HW; ++hw) {
+        const int hidx = (pp >> 2) * HW + hw;
+        const unsigned short v = (unsigned short)(hw < 4 ? lo >> (16 * hw) : hi >> (16 * (hw - 4)));
+        const unsigned short mk = (unsigned short)(hw < 4 ? mlo >> (16 * hw) : mhi >> (16 * (hw - 4)));
+        unsigned short* vptr = reinterpret_cast<unsigned short*>(tp + Lo::kOffVC + word_offset(Lo::KCW, hidx >> 1, 4 * gi + (pp & 3))) + (hidx & 1);
+        *vptr = (unsigned short)((vold[n][hw] & ~mk) | v);
+      }
+    } else if (lane == 28) {
       const int nl = slot_lane(slot);
       reinterpret_cast<unsigned*>(tp + Lo::kOffNK)[nl] =
-          (unsigned)f32_to_f16_bits_clamped(sqrtf(nk)) | ((unsigned)f32_to_f16_bits_clamped(sqrtf(nr)) << 16);
-      reinterpret_cast<unsigned short*>(tp + Lo::kOffVN)[nl] = f32_to_f16_bits_clamped(sqrtf(nv));
+          (unsigned)f32_to_f16_bits_clamped(nrm[0][e]) | ((unsigned)f32_to_f16_bits_clamped(nrm[1][e]) << 16);
+      reinterpret_cast<unsigned short*>(tp + Lo::kOffVN)[nl] = f32_to_f16_bits_clamped(nrm[2][e]);
     }
   }
   // ---- arrival: the last head of a batch entry publishes the new length
@@ -429,32 +528,34 @@ __global__ void __launch_bounds__((kAppend ? 3 : 2) * PrepCfg<D>::GT) prep_kerne
       __threadfence();
     }
   }
-  __syncthreads();  // the next group of the run reuses the shared arrays
-  }  // batch groups of this CTA's run
+}
+
+template <int D, typename T, int EB>
+static cudaError_t launch_prep_e(const PrepArgs& a, int lh_count, int B, bool do_append, bool do_query, cudaStream_t st) {
+  using Cfg = PrepCfg<D, EB>;
+  const int grid = lh_count * ((B + EB - 1) / EB);
+  const int smem = (int)Cfg::kSmemBytes;
+  cudaError_t e;
+  // the attribute is set per launch: it is per device and a process may drive several
+  if (do_append && do_query) {
+    if ((e = cudaFuncSetAttribute(prep_kernel<D, T, true, true, EB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)) != cudaSuccess) return e;
+    prep_kernel<D, T, true, true, EB><<<grid, kPrepThreads, smem, st>>>(a);
+  } else if (do_append) {
+    if ((e = cudaFuncSetAttribute(prep_kernel<D, T, true, false, EB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)) != cudaSuccess) return e;
+    prep_kernel<D, T, true, false, EB><<<grid, kPrepThreads, smem, st>>>(a);
+  } else {
+    if ((e = cudaFuncSetAttribute(prep_kernel<D, T, false, true, EB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)) != cudaSuccess) return e;
+    prep_kernel<D, T, false, true, EB><<<grid, kPrepThreads, smem, st>>>(a);
+  }
+  count_launch();
+  return cudaGetLastError();
 }
 
 template <int D, typename T>
-static cudaError_t launch_prep_t(const PrepArgs& a, int lh_count, int B, int num_sms, bool do_append, bool do_query,
-                                 cudaStream_t st) {
-  using Cfg = PrepCfg<D>;
-  const int nbg = (B + Cfg::BG - 1) / Cfg::BG;
-  // batch groups per CTA: a CTA re-uses its matrix rows over a run of groups.  Enough CTAs to fill the GPU twice
-  // (a single layer: one group per CTA, shortest latency); the rest of the batch goes into longer runs.
-  int gpc = (int)(((long)lh_count * nbg + 2L * num_sms - 1) / (2L * num_sms));
-  gpc = gpc < 1 ? 1 : (gpc > nbg ? nbg : gpc);
-  const int grid = lh_count * ((nbg + gpc - 1) / gpc);
-  const size_t sm3 = D == 64 ? (size_t)3 * D * 68 * 4 : 0, sm2 = D == 64 ? (size_t)2 * D * 68 * 4 : 0;
-  if (D == 64) {  // per launch: the attribute is per device and a process may drive several
-    cudaError_t e1 = cudaFuncSetAttribute(prep_kernel<D, T, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm3);
-    cudaError_t e2 = cudaFuncSetAttribute(prep_kernel<D, T, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm3);
-    if (e1 != cudaSuccess) return e1;
-    if (e2 != cudaSuccess) return e2;
-  }
-  if (do_append && do_query) prep_kernel<D, T, true, true><<<grid, 3 * Cfg::GT, sm3, st>>>(a, nbg, gpc);
-  else if (do_append) prep_kernel<D, T, true, false><<<grid, 3 * Cfg::GT, sm3, st>>>(a, nbg, gpc);
-  else prep_kernel<D, T, false, true><<<grid, 2 * Cfg::GT, sm2, st>>>(a, nbg, gpc);
-  count_launch();
-  return cudaGetLastError();
+static cudaError_t launch_prep_t(const PrepArgs& a, int lh_count, int B, int num_sms, bool do_append, bool do_query, cudaStream_t st) {
+  // 32 entries per CTA when that still gives every SM a few CTAs (fewest instructions per unit), else 8 (shortest CTA)
+  if ((long)lh_count * ((B + 31) / 32) >= 2L * num_sms) return launch_prep_e<D, T, 32>(a, lh_count, B, do_append, do_query, st);
+  return launch_prep_e<D, T, 8>(a, lh_count, B, do_append, do_query, st);
 }
 
 cudaError_t launch_prep(const DecodeArgs& d, const void* k, const void* v, int D, int num_sms, bool do_append,
