@@ -38,7 +38,7 @@ constexpr int kMaxSegments = 64;      // split-K partial slots per unit (tq_api.
 #define TQ_DECODE_CTAS64 5
 #endif
 #ifndef TQ_DECODE_STAGES
-#define TQ_DECODE_STAGES 3
+#define TQ_DECODE_STAGES 2  // measured at configs[2] x 33 layers: 2 slots 11.4 us per layer, 3 slots 11.5, 4 slots 13.2
 #endif
 constexpr int kDecodeThreads = 128;   // warps of one CTA share the dequantisation tables of one head
 constexpr int kDecodeWarps = kDecodeThreads / 32;

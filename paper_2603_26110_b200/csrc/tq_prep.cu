@@ -181,31 +181,25 @@ __global__ void __launch_bounds__(kPrepThreads) prep_kernel(PrepArgs a) {
   }
   __syncthreads();
 
-  // ---- the store stage at the end is warp-per-entry with fixed lane roles (device tile layout, tq_common.cuh):
-  //      lanes [0, 4)  : K pair fields of lane-target t = lane (one block of HW halfwords)
-  //      lanes [4, 4 + 8 U) : sign bytes (t, piece u, byte half hb)
-  //      lanes [20, 28): V fields of lane-target gi = lane - 20 (three-bit slices inside HW halfwords, read-modify-write:
-  //                      a V field is shared with the other token of the pair, appended by an earlier call)
-  //      lane 28       : the three norms
-  //      The V halfwords are requested here, long before they are needed.
+  // ---- the store stage at the end: a warp owns entries warp, warp + 8, ... (EPW of them) and makes four passes over
+  //      them with lane = (entry n, piece): K blocks (4 per entry), sign bytes (8 U), V blocks (8, read-modify-write: a V
+  //      field is shared with the other token of the pair, appended by an earlier call), norms (1).  The V halfwords are
+  //      requested here, long before they are needed.
   constexpr int HW = 3 * D / 64;       // halfwords per (lane, token) block of K fields, and per (lane, token pair) block of V fields
   constexpr int EPW = EB / NW;         // entries per warp in the store stage
-  unsigned short vold[EPW][HW];
-  if (kAppend) {
+  unsigned short vold[HW];
 #pragma unroll
-    for (int n = 0; n < EPW; ++n) {
-      const int e = warp + n * NW;
+  for (int hw = 0; hw < HW; ++hw) vold[hw] = 0;
+  if (kAppend && lane < 8 * EPW) {
+    const int e = warp + (lane >> 3) * NW, gi = lane & 7;
+    if (e < nb && s_len0[e] < a.cv.max_seq) {
+      const int len = s_len0[e], slot = len % kTile, pp = slot >> 1;
+      const unsigned char* tp = a.cv.tiles + stream_of(e) * a.cv.stream_bytes + (size_t)(len / kTile) * Lo::kTileBytes;
 #pragma unroll
-      for (int hw = 0; hw < HW; ++hw) vold[n][hw] = 0;
-      if (e < nb && lane >= 20 && lane < 28 && s_len0[e] < a.cv.max_seq) {
-        const int len = s_len0[e], slot = len % kTile, pp = slot >> 1, gi = lane - 20;
-        const unsigned char* tp = a.cv.tiles + stream_of(e) * a.cv.stream_bytes + (size_t)(len / kTile) * Lo::kTileBytes;
-#pragma unroll
-        for (int hw = 0; hw < HW; ++hw) {
-          const int hidx = (pp >> 2) * HW + hw;  // halfword of lane (gi, pp & 3)'s V string
-          vold[n][hw] = __ldcg(reinterpret_cast<const unsigned short*>(tp + Lo::kOffVC + word_offset(Lo::KCW, hidx >> 1, 4 * gi + (pp & 3))) +
-                               (hidx & 1));
-        }
+      for (int hw = 0; hw < HW; ++hw) {
+        const int hidx = (pp >> 2) * HW + hw;  // halfword of lane (gi, pp & 3)'s V string
+        vold[hw] = __ldcg(reinterpret_cast<const unsigned short*>(tp + Lo::kOffVC + word_offset(Lo::KCW, hidx >> 1, 4 * gi + (pp & 3))) +
+                          (hidx & 1));
       }
     }
   }
@@ -453,15 +447,18 @@ __global__ void __launch_bounds__(kPrepThreads) prep_kernel(PrepArgs a) {
   }
   if (!kAppend) return;
 
-  // ---- stage 5 (append): one warp per entry assembles the token's pieces (lane roles above)
-#pragma unroll
-  for (int n = 0; n < EPW; ++n) {
-    const int e = warp + n * NW;
-    if (e >= nb || s_full[e]) continue;
-    const int len = s_len0[e], slot = len % kTile, g = slot & 7, r = slot >> 3;
-    unsigned char* tp = a.cv.tiles + stream_of(e) * a.cv.stream_bytes + (size_t)(len / kTile) * Lo::kTileBytes;
-    if (lane < 4) {  // K: pairs t + 4 j, field j at bit 6 j of the block
-      const int t = lane;
+  // ---- stage 5 (append): the four store passes (see above)
+  auto tile_of = [&](int e, int& slot) {
+    const int len = s_len0[e];
+    slot = len % kTile;
+    return a.cv.tiles + stream_of(e) * a.cv.stream_bytes + (size_t)(len / kTile) * Lo::kTileBytes;
+  };
+  if (lane < 4 * EPW) {  // K: pairs t + 4 j, field j at bit 6 j of the block
+    const int e = warp + (lane >> 2) * NW, t = lane & 3;
+    if (e < nb && !s_full[e]) {
+      int slot;
+      unsigned char* tp = tile_of(e, slot);
+      const int g = slot & 7, r = slot >> 3;
       unsigned long long lo = 0ull, hi = 0ull;
 #pragma unroll
       for (int j = 0; j < Lo::J; ++j) {
@@ -477,21 +474,34 @@ __global__ void __launch_bounds__(kPrepThreads) prep_kernel(PrepArgs a) {
         const unsigned short v = (unsigned short)(hw < 4 ? lo >> (16 * hw) : hi >> (16 * (hw - 4)));
         reinterpret_cast<unsigned short*>(tp + Lo::kOffKC + word_offset(Lo::KCW, hidx >> 1, 4 * g + t))[hidx & 1] = v;
       }
-    } else if (lane < 4 + 8 * Lo::U) {  // sign bytes: bit k = [(S r)_rho >= 0], rho = t d/4 + 16 u + 8 hb + k
-      const int si = lane - 4, t = si / (2 * Lo::U), u = (si / 2) % Lo::U, hb = si & 1;
+    }
+  }
+  for (int item = lane; item < 8 * Lo::U * EPW; item += 32) {  // sign bytes: bit k = [(S r)_rho >= 0], rho = t d/4 + 16 u + 8 hb + k
+    const int e = warp + (item / (8 * Lo::U)) * NW, si = item % (8 * Lo::U);
+    if (e < nb && !s_full[e]) {
+      int slot;
+      unsigned char* tp = tile_of(e, slot);
+      const int g = slot & 7, r = slot >> 3;
+      const int t = si / (2 * Lo::U), u = (si / 2) % Lo::U, hb = si & 1;
       const float* sr = Y + (size_t)e * Cfg::FP + t * (D / 4) + 16 * u + 8 * hb;
       unsigned v = 0;
 #pragma unroll
       for (int k = 0; k < 8; ++k) v |= (sr[k] >= 0.f ? 1u : 0u) << k;
       const int word = (slot >> 4) * Lo::U + u, byte = 2 * hb + (r & 1);
       *(tp + Lo::kOffKS + word_offset(Lo::KSW, word, 4 * g + t) + byte) = (unsigned char)v;
-    } else if (lane >= 20 && lane < 28) {  // V: coordinates gi + 8 c, three-bit slices at 6 c + 3 (slot & 1)
-      const int gi = lane - 20, pp = slot >> 1, sh0 = 3 * (slot & 1);
+    }
+  }
+  if (lane < 8 * EPW) {  // V: coordinates gi + 8 c, three-bit slices at 6 c + 3 (slot & 1)
+    const int e = warp + (lane >> 3) * NW, gi = lane & 7;
+    if (e < nb && !s_full[e]) {
+      int slot;
+      unsigned char* tp = tile_of(e, slot);
+      const int pp = slot >> 1, sh0 = 3 * (slot & 1);
       unsigned long long lo = 0ull, hi = 0ull, mlo = 0ull, mhi = 0ull;
 #pragma unroll
       for (int c = 0; c < Lo::C; ++c) {
         const unsigned long long f = cV[e][gi + 8 * c], m7 = 7ull;
-        const int bit = 6 * c;  // + sh0 (< 6), so a slice never straddles bit 64 when 6 c + 6 <= 64 or 6 c >= 64
+        const int bit = 6 * c;
         if (bit + 6 <= 64) lo |= f << (bit + sh0), mlo |= m7 << (bit + sh0);
         else if (bit >= 64) hi |= f << (bit - 64 + sh0), mhi |= m7 << (bit - 64 + sh0);
         else {  // field 10 of d = 128 covers bits [60, 66)
@@ -506,9 +516,15 @@ __global__ void __launch_bounds__(kPrepThreads) prep_kernel(PrepArgs a) {
         const unsigned short v = (unsigned short)(hw < 4 ? lo >> (16 * hw) : hi >> (16 * (hw - 4)));
         const unsigned short mk = (unsigned short)(hw < 4 ? mlo >> (16 * hw) : mhi >> (16 * (hw - 4)));
         unsigned short* vptr = reinterpret_cast<unsigned short*>(tp + Lo::kOffVC + word_offset(Lo::KCW, hidx >> 1, 4 * gi + (pp & 3))) + (hidx & 1);
-        *vptr = (unsigned short)((vold[n][hw] & ~mk) | v);
+        *vptr = (unsigned short)((vold[hw] & ~mk) | v);
       }
-    } else if (lane == 28) {
+    }
+  }
+  if (lane < EPW) {
+    const int e = warp + lane * NW;
+    if (e < nb && !s_full[e]) {
+      int slot;
+      unsigned char* tp = tile_of(e, slot);
       const int nl = slot_lane(slot);
       reinterpret_cast<unsigned*>(tp + Lo::kOffNK)[nl] =
           (unsigned)f32_to_f16_bits_clamped(nrm[0][e]) | ((unsigned)f32_to_f16_bits_clamped(nrm[1][e]) << 16);
