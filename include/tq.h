@@ -31,19 +31,23 @@
  *
  * Device cache format (opaque to callers; tq_cache_export_canonical / tq_cache_import_canonical convert):
  *   tokens are grouped in tiles of TQ_TILE_TOKENS = 32 and every (layer, batch, head) owns one contiguous
- *   stream of ceil(max_seq/32) tiles.  Inside a tile every per-token word string is stored "chunk-major"
- *   ([16-byte chunk][token]) so that a warp with lane = token reads it with coalesced 128-bit loads:
- *     K codes : P = d/2 six-bit fields (code_{2g} | code_{2g+1} << 3); the token in tile slot t stores pair
- *               group g at field position (g - t) mod P  (the rotation makes the decode kernel's
- *               shared-memory table reads bank-conflict free);
- *     K signs : m/4 nibbles; nibble group n (coordinates 4n..4n+3, bit b = coordinate 4n+b) is stored at
- *               nibble position (n - t) mod (m/4);
- *     V codes : stored per coordinate pair, not per token: "lane" g (< 32) of the tile owns the string of
- *               pair group g (and g + 32 for d = 128, appended after it); inside it token slot j of the tile
- *               sits at bits [6j, 6j + 6).  The decode kernel accumulates V with lane = coordinate pair, so
- *               it needs two fp32 accumulators per lane instead of d;
- *     norms   : three 64-byte arrays of binary16: |k|, |r_k|, |v|.
+ *   stream of ceil(max_seq/32) tiles.  The fused decode kernel runs its contractions as warp-level tensor-core MMAs
+ *   (mma.sync.m16n8k16), so a tile stores every word in the order of the MMA A-fragment: "lane" = 4 g + t, g = lane / 4
+ *   the fragment row, t = lane % 4 the fragment column group; per-lane word strings are stored chunk-major
+ *   ([16-byte chunk][lane]) so that lane-wise 128-bit reads are contiguous:
+ *     K codes : lane (g, t) holds, for the token slots g, g + 8, g + 16, g + 24, the six-bit fields
+ *               (code_{2p} | code_{2p+1} << 3) of the coordinate pairs p = t, t + 4, t + 8, ...;
+ *     K signs : lane (g, t) holds sketch rows [t m/4, (t+1) m/4) of the same four slots in 16-bit pieces; the pieces of
+ *               slots s and s + 8 are byte-interleaved in one 32-bit word so that (word >> 8 ab) & (0x00010001 << p) is an
+ *               fp16 pair whose halves are 0 or the subnormal 2^(p-24): the sign bits feed the MMA without unpacking;
+ *     V codes : lane (g, t) holds coordinates g, g + 8, g + 16, ... of the token pairs t, t + 4, t + 8, t + 12 as six-bit
+ *               fields code(token 2pp) | code(token 2pp + 1) << 3;
+ *     norms   : one u32 per lane (binary16 |k| | binary16 |r_k| << 16) and one u16 (binary16 |v|); lane (g, t) owns
+ *               slot g + 8 t.
  *   Bytes per cached token-head: 62 (d = 64), 118 (d = 128) — the same as the canonical format.
+ *   A cache has ONE writer at a time: tq_quantize_pack / tq_append / tq_decode_step / tq_decode_model_step /
+ *   tq_cache_import_canonical calls that touch the same layer must be ordered by the caller (same stream, or events);
+ *   concurrent readers (tq_decode_attn, export) of a layer that is not being written are fine.
  */
 #ifndef TQ_H_
 #define TQ_H_
@@ -104,8 +108,10 @@ size_t tq_cache_bytes_per_token_head(const tq_shape *shape); /* 62 or 118       
  * int32 sticky status word (0, or TQ_ERR_CAPACITY once an append was refused on the device).          */
 size_t tq_cache_seq_len_offset(const tq_shape *shape);
 size_t tq_cache_status_offset(const tq_shape *shape);
-/* Workspace for tq_decode_attn over n_layers_call layers: rotated queries, split-K partials, arrival
- * counters.  Must be zero-filled once by the caller; every call leaves it reusable.                    */
+/* Workspace for tq_decode_attn / tq_decode_step (n_layers_call = the call's) and tq_decode_model_step (its
+ * n_layers_call): the decode kernel's query operands and dequantisation tables, split-K partials, arrival
+ * counters.  Must be zero-filled once by the caller; every call leaves it reusable.  Calls that share a
+ * workspace must be ordered on one stream.                                                               */
 size_t tq_decode_workspace_bytes(const tq_shape *shape, int32_t n_layers_call);
 /* Canonical plane sizes in bytes for n_tokens tokens of every (layer?, batch, head) of ONE layer:
  * plane 0 k_codes, 1 k_signs, 2 k_norm, 3 k_rnorm, 4 v_codes, 5 v_norm.                                */
@@ -153,7 +159,7 @@ int tq_decode_attn(const tq_shape *shape, const tq_params *dev, const tq_cache *
 
 /* ---- one decode step of one layer, fused: tq_append(k, v) followed by tq_decode_attn(q) with the query at
  * the newly appended position, in two kernel launches instead of three (the append and the query
- * preparation share one kernel and the rows of PI_K and S).  q, k, v, out: DEVICE [B][H][d], dtype dt.
+ * preparation share one kernel and its two small tensor-core products).  q, k, v, out: DEVICE [B][H][d], dtype dt.
  * Result and cache state are identical to calling the two entry points one after the other
  * (BASELINE.json:configs[2] "each step appending one quantized token per head via tq_append").            */
 int tq_decode_step(const tq_shape *shape, const tq_params *dev, tq_cache *cache, int32_t layer, const void *q,
@@ -211,10 +217,11 @@ int tq_decode_model_step(const tq_shape *shape, const tq_params *dev, tq_cache *
 const char *tq_status_string(int status);
 /* Number of kernels the library launched since load (bench.py's gpu_launches).                          */
 int64_t tq_launch_count(void);
-/* Measurement hook (bench.py's roofline leg): while on, tq_decode_attn launches ONLY the streaming
- * fused-attention kernel and re-uses the rotated queries its previous ordinary call left in the workspace
- * (same queries, same layers), so that a run of such calls times that kernel alone.  Process-wide state;
- * results are only meaningful directly after an ordinary call with the same arguments.                   */
+/* Measurement hook, NOT part of the product path (bench.py's roofline leg and one test use it): while on,
+ * tq_decode_attn / tq_decode_model_step skip the append + query-prep kernel and re-use the query operands their
+ * previous ordinary call left in the workspace (same queries, same layers), so that a run of such calls times
+ * the streaming kernel alone.  Process-wide, not thread-safe; results are only meaningful directly after an
+ * ordinary call with the same arguments; always switch it off again.                                      */
 void tq_profile_decode_main_only(int on);
 /* Test / sweep knobs (process-wide, not part of the product path; both default to 0 = the library's own choice):
  * CTAs per unit of the streaming decode kernel; 1 = route tq_quantize_pack to the fp32 CUDA-core cross-check kernel. */
