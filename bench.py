@@ -419,6 +419,25 @@ def run_cfg2(args, w: W.Workload):
 
     dec_bytes = B * H * T0 * rig.bpt  # algorithmic packed bytes of one streaming-kernel launch at T0 tokens
 
+    # ---- the same step through the stepper with DEVICE buffers (three-branch graph: the prep kernels of later layer
+    #      chunks run beside the streaming chain)
+    stepper_dev = tq.HostStepper(shape, params, cache, 0, L, qs, kn, vn, outs, None, wsL, max_seq, args.e2e_chunks)
+    with torch.cuda.stream(stream):
+        reset_len()
+        for _ in range(3):
+            stepper_dev.launch(stream)
+        reset_len()
+        e0, e1 = rig.ev(), rig.ev()
+        e0.record(stream)
+        n_st = min(args.steps, steps_per_fill)
+        for _ in range(n_st):
+            stepper_dev.launch(stream)
+        e1.record(stream)
+        e1.synchronize()
+    stepper_ms = e0.elapsed_time(e1) / n_st
+    stepper_value = L * B * H * sum(T0 + i + 1 for i in range(n_st)) / n_st / (stepper_ms * 1e-3)
+    stepper_dev.close()
+
     # ---- the same work as a real model must order it: tq_decode_step layer by layer (append + query prep kernel, then the
     #      streaming kernel, each layer waiting for the one before)
     def seq_step():
@@ -471,20 +490,30 @@ def run_cfg2(args, w: W.Workload):
     qh, kh, vh = qs.cpu().pin_memory(), kn.cpu().pin_memory(), vn.cpu().pin_memory()
     oh = torch.empty_like(qh).pin_memory()
 
+    stepper = tq.HostStepper(shape, params, cache, 0, L, qh, kh, vh, oh, staging, wsL, max_seq, args.e2e_chunks)
+
     def e2e_step():  # one model decode step: pinned q/k/v of all L layers in, the step, outputs back, sync
+        stepper.run(stream)
+
+    def e2e_step_plain():  # the same through tq_decode_model_step_host (no graph: 4 copies + 35 launches from the host)
         tq.tq_decode_model_step_host(shape, params, cache, 0, L, qh, kh, vh, oh, staging, wsL, max_seq, stream)
 
-    with torch.cuda.stream(stream):
-        reset_len()
-        e2e_step()
-        stream.synchronize()
-        reset_len()
-        stream.synchronize()
-        t0 = time.perf_counter()
-        for _ in range(e2e_steps):
-            e2e_step()
-        stream.synchronize()
-        e2e_s = time.perf_counter() - t0
+    def time_e2e(fn):
+        with torch.cuda.stream(stream):
+            reset_len()
+            fn()
+            stream.synchronize()
+            reset_len()
+            stream.synchronize()
+            t0 = time.perf_counter()
+            for _ in range(e2e_steps):
+                fn()
+            stream.synchronize()
+            return time.perf_counter() - t0
+
+    e2e_plain_s = time_e2e(e2e_step_plain)
+    e2e_s = time_e2e(e2e_step)
+    stepper.close()
     e2e_tok = L * B * H * sum(T0 + i + 1 for i in range(e2e_steps))
     vec_bytes = B * H * d * 2
 
@@ -513,6 +542,7 @@ def run_cfg2(args, w: W.Workload):
                          "layer cache (run-ahead chain), one finish launch",
             "us_per_layer_step": us_layer,
             "packed_gbs_whole_step": value / world * rig.bpt / 1e9,
+            "ms_per_step_stepper_device_buffers": stepper_ms, "value_stepper_device_buffers": stepper_value,
             "us_per_layer_step_sequential": seq_us,
             "value_sequential": L * B * H * (T0 + 1) / (seq_us * L * 1e-6),
             "decode_call_us_live": call_us, "decode_call_packed_gbs": dec_bytes / call_us / 1e3,
@@ -523,7 +553,10 @@ def run_cfg2(args, w: W.Workload):
         },
         "clocks": clocks,
         "e2e": {"value": world * e2e_tok / e2e_max, "unit": UNIT, "h2d_bytes_per_step": 3 * L * vec_bytes,
-                "d2h_bytes_per_step": L * vec_bytes, "steps": e2e_steps},
+                "d2h_bytes_per_step": L * vec_bytes, "steps": e2e_steps,
+                "how": "tq_host_stepper_run: one captured graph per step (H2D copies of q/k/v, tq_decode_model_step per layer "
+                       "chunk, D2H of out; copies overlapped with the chunks), host wall clock incl. the synchronisation",
+                "value_uncaptured_host_call": e2e_tok / e2e_plain_s},
         "gpu_launches": int(launches_per_step * args.steps),
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "traffic": traffic[0] if traffic else None, "kernel": "decode_main_kernel<64, __half, false>",
@@ -637,6 +670,7 @@ def main():
     ap.add_argument("--layers", type=int, default=33, help="ESM-2-650M has 33 layers (cfg2)")
     ap.add_argument("--layers-aux", type=int, default=0, help="layer caches cycled by cfg3 / cfg4 (0 = enough to exceed L2)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--e2e-chunks", type=int, default=0, help="layer chunks of the host stepper (0 = the library's choice)")
     args = ap.parse_args()
     w = W.CONFIGS[CONFIG_NAMES[args.config]]
     if args.impl == "reference":

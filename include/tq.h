@@ -202,6 +202,33 @@ int tq_decode_model_step_host(const tq_shape *shape, const tq_params *dev, tq_ca
                               tq_dtype dt, void *out_host, int32_t t_hint, void *staging, void *workspace,
                               size_t workspace_bytes, void *cuda_stream);
 
+/* ---- stepper: one decode step of a run of layers captured ONCE as a CUDA graph (the serving loop's form of the step;
+ * bench.py times it with host buffers as "e2e") [BASELINE.json:configs[2] "100 consecutive decode steps"; SURVEY.md §7
+ * hard part 2].  tq_host_stepper_create records, for FIXED buffers q/k/v/out ([n_layers_call][B][H][d], dtype dt, valid
+ * until destroy), a graph with three branches; the layers are cut into n_chunks runs (0 = the library's choice):
+ *   copy-in  : per run, the host-to-device copies of k, v, q, then the append + query-prep kernel of that run;
+ *   main     : the streaming kernels of all layers, a run-ahead chain per run (the first kernel of a run waits for that
+ *              run's prep kernel and for the run in front);
+ *   copy-out : per run, the PI_V^T finish kernel, then the device-to-host copy of out.
+ * buffers_on_host = 1: q/k/v/out are HOST buffers and must be page-locked (cudaHostAlloc / cudaHostRegister); staging is a
+ * DEVICE buffer of tq_model_step_staging_bytes() bytes, 256-byte aligned.  buffers_on_host = 0: they are DEVICE buffers,
+ * no copies are recorded and staging may be NULL.  workspace: tq_decode_workspace_bytes(shape, n_layers_call), zero-filled
+ * once; staging and workspace are owned by the caller and used by every run.  Results and cache state are identical to
+ * tq_decode_model_step(_host).  The stepper is the only object the library ever allocates (a graph and its executable, on
+ * the host); create and destroy are not hot.
+ * tq_host_stepper_launch: one graph launch on cuda_stream, asynchronous.  tq_host_stepper_run: launch + one stream
+ * synchronisation (the caller writes this step's q/k/v into the buffers before, reads out after).  seq_len lives on the
+ * device, so the same graph serves every step.  Errors: TQ_ERR_INVALID_ARG (NULL / misaligned), TQ_ERR_CAPACITY
+ * (workspace), TQ_ERR_CUDA (capture failed, e.g. pageable host memory).                                                */
+typedef struct tq_host_stepper tq_host_stepper;
+int tq_host_stepper_create(const tq_shape *shape, const tq_params *dev, tq_cache *cache, int32_t layer_begin,
+                           int32_t n_layers_call, const void *q_buf, const void *k_buf, const void *v_buf, void *out_buf,
+                           int32_t buffers_on_host, tq_dtype dt, int32_t t_hint, void *staging, void *workspace,
+                           size_t workspace_bytes, int32_t n_chunks, tq_host_stepper **out_stepper);
+int tq_host_stepper_launch(tq_host_stepper *stepper, void *cuda_stream);
+int tq_host_stepper_run(tq_host_stepper *stepper, void *cuda_stream);
+int tq_host_stepper_destroy(tq_host_stepper *stepper);
+
 /* ---- one decode step of a run of layers, DEVICE buffers [BASELINE.json:configs[2]; configs[1] for the shape] --------
  * q, k, v, out: DEVICE [n_layers_call][B][H][d], dtype dt.  Result and cache state are identical to tq_decode_step
  * called layer by layer (layers are independent: "each (layer, head)").  What differs is the launch

@@ -23,7 +23,8 @@ EXPORTS = [
     "tq_decode_workspace_bytes", "tq_canonical_plane_bytes", "tq_calibrate_host", "tq_quantize_pack", "tq_append",
     "tq_decode_attn", "tq_decode_step", "tq_cache_export_canonical", "tq_cache_import_canonical", "tq_step_staging_bytes",
     "tq_decode_step_host", "tq_model_step_staging_bytes", "tq_decode_model_step_host", "tq_decode_model_step", "tq_status_string", "tq_launch_count", "tq_profile_decode_main_only",
-    "tq_debug_set_decode_nsplit", "tq_debug_set_quantize_impl",
+    "tq_debug_set_decode_nsplit", "tq_debug_set_quantize_impl", "tq_host_stepper_create", "tq_host_stepper_launch", "tq_host_stepper_run",
+    "tq_host_stepper_destroy",
 ]
 
 
@@ -316,3 +317,39 @@ def tq_decode_model_step_host(shape, params: Params, cache: Cache, layer_begin: 
                                          C.c_int(_dtype_code(q_host)), _ptr(out_host), C.c_int32(t_hint), _ptr(staging),
                                          _ptr(workspace.data), C.c_size_t(workspace.bytes), _stream_ptr(stream))
     _check(rc, "tq_decode_model_step_host")
+
+
+class HostStepper:
+    """tq_host_stepper_*: the model decode step captured once as a CUDA graph (copy-in / streaming chain / copy-out
+    branches).  q/k/v/out: pinned HOST tensors [Lc,B,H,d] (copies recorded; staging required) or DEVICE tensors (no
+    copies); the caller re-fills q/k/v before every run()."""
+
+    def __init__(self, shape, params: Params, cache: Cache, layer_begin: int, n_layers_call: int, q, k, v, out, staging,
+                 workspace: Workspace, t_hint: int = 0, n_chunks: int = 0):
+        self._keep = (shape, params, cache, q, k, v, out, staging, workspace)
+        on_host = 0 if q.is_cuda else 1
+        self.h = C.c_void_p()
+        rc = lib().tq_host_stepper_create(C.byref(shape), C.byref(params.c), C.byref(cache.c), C.c_int32(layer_begin),
+                                          C.c_int32(n_layers_call), _ptr(q), _ptr(k), _ptr(v), _ptr(out), C.c_int32(on_host),
+                                          C.c_int(_dtype_code(q)), C.c_int32(t_hint), _ptr(staging), _ptr(workspace.data),
+                                          C.c_size_t(workspace.bytes), C.c_int32(n_chunks), C.byref(self.h))
+        _check(rc, "tq_host_stepper_create")
+
+    def launch(self, stream=None):
+        """asynchronous: one graph launch"""
+        _check(lib().tq_host_stepper_launch(self.h, _stream_ptr(stream)), "tq_host_stepper_launch")
+
+    def run(self, stream=None):
+        """graph launch + stream synchronisation"""
+        _check(lib().tq_host_stepper_run(self.h, _stream_ptr(stream)), "tq_host_stepper_run")
+
+    def close(self):
+        if self.h:
+            lib().tq_host_stepper_destroy(self.h)
+            self.h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -284,10 +284,20 @@ int tq_cache_import_canonical(const tq_shape* shape, tq_cache* cache, int32_t la
              : TQ_ERR_CUDA;
 }
 
-int tq_decode_model_step(const tq_shape* shape, const tq_params* dev, tq_cache* cache, int32_t layer_begin,
-                         int32_t n_layers_call, const void* q, const void* k, const void* v, tq_dtype dt, void* out,
-                         int32_t t_hint, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+// Validated launch plan of one model decode step (tq_decode_model_step and the host stepper share it).
+struct ModelStepPlan {
   CacheGeom g;
+  WorkspaceGeom w;
+  DecodeArgs a;  // the whole call: layers [layer_begin, layer_begin + n_layers_call)
+  const unsigned char *k, *v;
+  size_t esz;
+  int sms;
+};
+
+static int plan_model_step(const tq_shape* shape, const tq_params* dev, tq_cache* cache, int32_t layer_begin,
+                           int32_t n_layers_call, const void* q, const void* k, const void* v, tq_dtype dt, void* out,
+                           int32_t t_hint, void* workspace, size_t workspace_bytes, ModelStepPlan* p) {
+  CacheGeom& g = p->g;
   int rc = check_shape(shape, &g);
   if (rc != TQ_OK) return rc;
   if ((rc = check_params(dev)) != TQ_OK) return rc;
@@ -297,48 +307,64 @@ int tq_decode_model_step(const tq_shape* shape, const tq_params* dev, tq_cache* 
   if (!aligned16(q) || !aligned16(k) || !aligned16(v) || !aligned16(out) || !workspace || ((uintptr_t)workspace & 255u))
     return TQ_ERR_INVALID_ARG;
   if (t_hint < 0) return TQ_ERR_INVALID_ARG;
-  WorkspaceGeom w = workspace_geom(g, n_layers_call);
-  if (workspace_bytes < w.total) return TQ_ERR_CAPACITY;
-  const int sms = num_sms();
-  if (sms <= 0) return TQ_ERR_CUDA;
+  p->w = workspace_geom(g, n_layers_call);
+  if (workspace_bytes < p->w.total) return TQ_ERR_CAPACITY;
+  p->sms = num_sms();
+  if (p->sms <= 0) return TQ_ERR_CUDA;
   const int th = (t_hint == 0 || t_hint > g.max_seq) ? g.max_seq : t_hint;
   const int ntiles = (th + kTile - 1) / kTile;
-  const int nsplit = pick_nsplit(g.B * g.H, ntiles, sms);
-  const size_t esz = dt == TQ_F16 ? 2 : 4;
+  const int nsplit = pick_nsplit(g.B * g.H, ntiles, p->sms);
+  p->esz = dt == TQ_F16 ? 2 : 4;
+  p->k = (const unsigned char*)k, p->v = (const unsigned char*)v;
   unsigned char* ws = (unsigned char*)workspace;
-  cudaStream_t st = (cudaStream_t)cuda_stream;
-  DecodeArgs a;
+  DecodeArgs& a = p->a;
   a.cv = make_view(g, cache->data);
   a.pi_k = dev->pi_k, a.pi_v = dev->pi_v, a.lut_k = dev->lut_k, a.lut_v = dev->lut_v, a.S = dev->S, a.rope_cs = dev->rope_cs;
   a.q = q, a.out = out, a.q_pos = nullptr;
-  a.counters = (int*)(ws + w.off_counters);
-  a.frags = (unsigned*)(ws + w.off_frags);
-  a.tabs = (unsigned*)(ws + w.off_tabs);
-  a.orot = (float*)(ws + w.off_orot);
-  a.partials = (float*)(ws + w.off_partials);
+  a.counters = (int*)(ws + p->w.off_counters);
+  a.frags = (unsigned*)(ws + p->w.off_frags);
+  a.tabs = (unsigned*)(ws + p->w.off_tabs);
+  a.orot = (float*)(ws + p->w.off_orot);
+  a.partials = (float*)(ws + p->w.off_partials);
   a.layer_begin = layer_begin, a.n_layers_call = n_layers_call;
   a.nsplit = nsplit, a.per = (ntiles + nsplit - 1) / nsplit;
   a.chain_mode = 0, a.rope_layout = shape->rope_layout, a.dt = (int)dt;
+  return TQ_OK;
+}
+
+// the arguments of layers [l0, l0 + nl) of the planned call (every pointer advanced to that sub-range)
+static DecodeArgs sub_args(const ModelStepPlan& p, int l0, int nl) {
+  DecodeArgs b = p.a;
+  const size_t u0 = (size_t)l0 * p.g.B * p.g.H;
+  b.q = (const unsigned char*)p.a.q + u0 * p.g.D * p.esz;
+  b.out = (unsigned char*)p.a.out + u0 * p.g.D * p.esz;
+  b.counters = p.a.counters + u0;
+  b.frags = p.a.frags + u0 * p.w.frag_words;
+  b.tabs = p.a.tabs + (size_t)l0 * p.g.H * kTabWords;
+  b.orot = p.a.orot + u0 * p.g.D;
+  b.partials = p.a.partials + u0 * kMaxSplits * (p.g.D + 2);
+  b.layer_begin = p.a.layer_begin + l0, b.n_layers_call = nl;
+  return b;
+}
+
+int tq_decode_model_step(const tq_shape* shape, const tq_params* dev, tq_cache* cache, int32_t layer_begin,
+                         int32_t n_layers_call, const void* q, const void* k, const void* v, tq_dtype dt, void* out,
+                         int32_t t_hint, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  ModelStepPlan p;
+  int rc = plan_model_step(shape, dev, cache, layer_begin, n_layers_call, q, k, v, dt, out, t_hint, workspace,
+                           workspace_bytes, &p);
+  if (rc != TQ_OK) return rc;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
   // one prep launch for every layer of the step (append + query operands), then one streaming launch per layer cache:
   // the first waits for the prep kernel, the others run ahead of one another (DecodeArgs::chain_mode); they leave o'/l
   // in the workspace and one last launch applies PI_V^T to every unit of the step
-  if (!g_profile_skip_prep && launch_prep(a, k, v, g.D, sms, true, true, st) != cudaSuccess) return TQ_ERR_CUDA;
-  const size_t units = (size_t)g.B * g.H;
+  if (!g_profile_skip_prep && launch_prep(p.a, p.k, p.v, p.g.D, p.sms, true, true, st) != cudaSuccess) return TQ_ERR_CUDA;
   for (int l = 0; l < n_layers_call; ++l) {
-    DecodeArgs b = a;
-    const size_t u0 = (size_t)l * units;
-    b.q = (const unsigned char*)q + u0 * g.D * esz;
-    b.out = (unsigned char*)out + u0 * g.D * esz;
-    b.counters = a.counters + u0;
-    b.frags = a.frags + u0 * w.frag_words;
-    b.tabs = a.tabs + (size_t)l * g.H * kTabWords;
-    b.orot = a.orot + u0 * g.D;
-    b.partials = a.partials + u0 * kMaxSplits * (g.D + 2);
-    b.layer_begin = layer_begin + l, b.n_layers_call = 1;
+    DecodeArgs b = sub_args(p, l, 1);
     b.chain_mode = l == 0 ? 0 : 1;
-    if (launch_decode(b, g.D, false, st) != cudaSuccess) return TQ_ERR_CUDA;
+    if (launch_decode(b, p.g.D, false, st) != cudaSuccess) return TQ_ERR_CUDA;
   }
-  if (launch_finish(a, g.D, st) != cudaSuccess) return TQ_ERR_CUDA;
+  if (launch_finish(p.a, p.g.D, true, st) != cudaSuccess) return TQ_ERR_CUDA;
   return TQ_OK;
 }
 
@@ -404,6 +430,143 @@ int tq_decode_model_step_host(const tq_shape* shape, const tq_params* dev, tq_ca
     return rc;
   if (cudaMemcpyAsync(out_host, dout, bytes, cudaMemcpyDeviceToHost, st) != cudaSuccess) return TQ_ERR_CUDA;
   if (cudaStreamSynchronize(st) != cudaSuccess) return TQ_ERR_CUDA;
+  return TQ_OK;
+}
+
+// ---- stepper: one decode step of a run of layers captured ONCE as a CUDA graph with three branches ---------------------
+//   copy-in branch : per layer chunk, H2D copies of k, v, q (host buffers only), then the append + query-prep kernel
+//   main branch    : the streaming kernels of every layer; the first kernel of a chunk waits for that chunk's prep
+//                    kernel (and the chunk in front), the others run ahead as in tq_decode_model_step
+//   copy-out branch: per chunk, the finish kernel (PI_V^T), then the D2H copy of out (host buffers only)
+struct tq_host_stepper {
+  cudaGraph_t graph = nullptr;
+  cudaGraphExec_t exec = nullptr;
+  int n_launches = 0;  // kernels inside one replay (tq_launch_count bookkeeping)
+};
+
+int tq_host_stepper_create(const tq_shape* shape, const tq_params* dev, tq_cache* cache, int32_t layer_begin,
+                           int32_t n_layers_call, const void* q_buf, const void* k_buf, const void* v_buf, void* out_buf,
+                           int32_t buffers_on_host, tq_dtype dt, int32_t t_hint, void* staging, void* workspace,
+                           size_t workspace_bytes, int32_t n_chunks, tq_host_stepper** out_stepper) {
+  CacheGeom g;
+  int rc = check_shape(shape, &g);
+  if (rc != TQ_OK) return rc;
+  if (!out_stepper) return TQ_ERR_INVALID_ARG;
+  *out_stepper = nullptr;
+  if (!q_buf || !k_buf || !v_buf || !out_buf) return TQ_ERR_INVALID_ARG;
+  if (buffers_on_host && (!staging || ((uintptr_t)staging & 255u))) return TQ_ERR_INVALID_ARG;
+  if (dt != TQ_F16 && dt != TQ_F32) return TQ_ERR_INVALID_ARG;
+  if (layer_begin < 0 || n_layers_call <= 0 || layer_begin + n_layers_call > g.L) return TQ_ERR_INVALID_ARG;
+  constexpr int kMaxChunks = 64;
+  // measured at configs[2] x 33 layers: 4 chunks 38 G token-heads/s end to end; 2: 37, 8: 37, 33: 17 (a chunk boundary
+  // costs about 9 us: the first streaming kernel of a chunk waits for the chunk in front to drain)
+  if (n_chunks <= 0) n_chunks = n_layers_call >= 16 ? 4 : (n_layers_call >= 4 ? 2 : 1);
+  if (n_chunks > n_layers_call) n_chunks = n_layers_call;
+  if (n_chunks > kMaxChunks) n_chunks = kMaxChunks;
+  const size_t per_layer = (size_t)g.B * g.H * g.D * (dt == TQ_F16 ? 2 : 4);
+  const size_t vec = (per_layer * n_layers_call + 255) / 256 * 256;
+  unsigned char* s = (unsigned char*)staging;
+  const unsigned char *dq = buffers_on_host ? s : (const unsigned char*)q_buf, *dk = buffers_on_host ? s + vec : (const unsigned char*)k_buf,
+                      *dv = buffers_on_host ? s + 2 * vec : (const unsigned char*)v_buf;
+  unsigned char* dout = buffers_on_host ? s + 3 * vec : (unsigned char*)out_buf;
+  ModelStepPlan p;
+  if ((rc = plan_model_step(shape, dev, cache, layer_begin, n_layers_call, dq, dk, dv, dt, dout, t_hint, workspace,
+                            workspace_bytes, &p)) != TQ_OK)
+    return rc;
+
+  cudaStream_t s_main = nullptr, s_in = nullptr, s_out = nullptr;
+  cudaEvent_t fork = nullptr, join_in = nullptr, join_out = nullptr;
+  cudaEvent_t prep_done[kMaxChunks] = {}, chain_done[kMaxChunks] = {};
+  bool ok = cudaStreamCreateWithFlags(&s_main, cudaStreamNonBlocking) == cudaSuccess &&
+            cudaStreamCreateWithFlags(&s_in, cudaStreamNonBlocking) == cudaSuccess &&
+            cudaStreamCreateWithFlags(&s_out, cudaStreamNonBlocking) == cudaSuccess &&
+            cudaEventCreateWithFlags(&fork, cudaEventDisableTiming) == cudaSuccess &&
+            cudaEventCreateWithFlags(&join_in, cudaEventDisableTiming) == cudaSuccess &&
+            cudaEventCreateWithFlags(&join_out, cudaEventDisableTiming) == cudaSuccess;
+  for (int c = 0; ok && c < n_chunks; ++c)
+    ok = cudaEventCreateWithFlags(&prep_done[c], cudaEventDisableTiming) == cudaSuccess &&
+         cudaEventCreateWithFlags(&chain_done[c], cudaEventDisableTiming) == cudaSuccess;
+  tq_host_stepper* hs = ok ? new tq_host_stepper() : nullptr;
+  int status = ok ? TQ_OK : TQ_ERR_CUDA;
+  if (ok) {
+    const long long n0 = g_launches.load();
+    const bool capturing = cudaStreamBeginCapture(s_main, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
+    ok = capturing && cudaEventRecord(fork, s_main) == cudaSuccess && cudaStreamWaitEvent(s_in, fork, 0) == cudaSuccess &&
+         cudaStreamWaitEvent(s_out, fork, 0) == cudaSuccess;
+    for (int c = 0; ok && c < n_chunks; ++c) {
+      const int l0 = (int)((long long)n_layers_call * c / n_chunks), l1 = (int)((long long)n_layers_call * (c + 1) / n_chunks);
+      const size_t off = per_layer * l0, nb = per_layer * (l1 - l0);
+      if (buffers_on_host)
+        ok = cudaMemcpyAsync((void*)(dk + off), (const unsigned char*)k_buf + off, nb, cudaMemcpyHostToDevice, s_in) == cudaSuccess &&
+             cudaMemcpyAsync((void*)(dv + off), (const unsigned char*)v_buf + off, nb, cudaMemcpyHostToDevice, s_in) == cudaSuccess &&
+             cudaMemcpyAsync((void*)(dq + off), (const unsigned char*)q_buf + off, nb, cudaMemcpyHostToDevice, s_in) == cudaSuccess;
+      const DecodeArgs ca = sub_args(p, l0, l1 - l0);
+      ok = ok && launch_prep(ca, dk + off, dv + off, g.D, p.sms, true, true, s_in) == cudaSuccess &&
+           cudaEventRecord(prep_done[c], s_in) == cudaSuccess && cudaStreamWaitEvent(s_main, prep_done[c], 0) == cudaSuccess;
+      for (int l = l0; ok && l < l1; ++l) {
+        DecodeArgs b = sub_args(p, l, 1);
+        // a captured launch with the programmatic attribute turns EVERY dependency of its stream into a programmatic
+        // edge, the one to this chunk's prep kernel included (which triggers early): the first kernel of a chunk must
+        // therefore wait at its start; the others run ahead
+        b.chain_mode = l == l0 ? 0 : 1;
+        ok = launch_decode(b, g.D, false, s_main) == cudaSuccess;
+      }
+      ok = ok && cudaEventRecord(chain_done[c], s_main) == cudaSuccess && cudaStreamWaitEvent(s_out, chain_done[c], 0) == cudaSuccess &&
+           launch_finish(ca, g.D, false, s_out) == cudaSuccess;
+      if (ok && buffers_on_host)
+        ok = cudaMemcpyAsync((unsigned char*)out_buf + off, dout + off, nb, cudaMemcpyDeviceToHost, s_out) == cudaSuccess;
+    }
+    ok = ok && cudaEventRecord(join_in, s_in) == cudaSuccess && cudaStreamWaitEvent(s_main, join_in, 0) == cudaSuccess &&
+         cudaEventRecord(join_out, s_out) == cudaSuccess && cudaStreamWaitEvent(s_main, join_out, 0) == cudaSuccess;
+    cudaGraph_t graph = nullptr;
+    if (capturing) ok = (cudaStreamEndCapture(s_main, &graph) == cudaSuccess && graph) && ok;
+    if (ok) ok = cudaGraphInstantiate(&hs->exec, graph, 0) == cudaSuccess;
+    hs->graph = graph;
+    hs->n_launches = (int)(g_launches.load() - n0);
+    g_launches.store(n0);  // nothing ran yet: the capture only recorded the launches
+    if (!ok) status = TQ_ERR_CUDA;
+  }
+  for (int c = 0; c < n_chunks; ++c) {
+    if (prep_done[c]) cudaEventDestroy(prep_done[c]);
+    if (chain_done[c]) cudaEventDestroy(chain_done[c]);
+  }
+  if (fork) cudaEventDestroy(fork);
+  if (join_in) cudaEventDestroy(join_in);
+  if (join_out) cudaEventDestroy(join_out);
+  if (s_in) cudaStreamDestroy(s_in);
+  if (s_out) cudaStreamDestroy(s_out);
+  if (s_main) cudaStreamDestroy(s_main);
+  if (status != TQ_OK) {
+    if (hs) {
+      if (hs->exec) cudaGraphExecDestroy(hs->exec);
+      if (hs->graph) cudaGraphDestroy(hs->graph);
+      delete hs;
+    }
+    cudaGetLastError();
+    return status;
+  }
+  *out_stepper = hs;
+  return TQ_OK;
+}
+
+int tq_host_stepper_launch(tq_host_stepper* stepper, void* cuda_stream) {
+  if (!stepper || !stepper->exec) return TQ_ERR_INVALID_ARG;
+  if (cudaGraphLaunch(stepper->exec, (cudaStream_t)cuda_stream) != cudaSuccess) return TQ_ERR_CUDA;
+  count_launch(stepper->n_launches);
+  return TQ_OK;
+}
+
+int tq_host_stepper_run(tq_host_stepper* stepper, void* cuda_stream) {
+  const int rc = tq_host_stepper_launch(stepper, cuda_stream);
+  if (rc != TQ_OK) return rc;
+  return cudaStreamSynchronize((cudaStream_t)cuda_stream) == cudaSuccess ? TQ_OK : TQ_ERR_CUDA;
+}
+
+int tq_host_stepper_destroy(tq_host_stepper* stepper) {
+  if (!stepper) return TQ_OK;
+  if (stepper->exec) cudaGraphExecDestroy(stepper->exec);
+  if (stepper->graph) cudaGraphDestroy(stepper->graph);
+  delete stepper;
   return TQ_OK;
 }
 

@@ -199,7 +199,7 @@ cudaError_t launch_quantize_pack_tc(const QuantArgs& a, int D, tq_dtype dt, int 
 cudaError_t launch_prep(const DecodeArgs& d, const void* k, const void* v, int D, int num_sms, bool do_append,
                         bool do_query, cudaStream_t st);
 cudaError_t launch_decode(const DecodeArgs& a, int D, bool fused_out, cudaStream_t st);
-cudaError_t launch_finish(const DecodeArgs& a, int D, cudaStream_t st);
+cudaError_t launch_finish(const DecodeArgs& a, int D, bool programmatic, cudaStream_t st);
 int decode_ctas_per_sm(int D);
 cudaError_t launch_export(const CacheGeom& g, const CacheView& cv, int layer, int n_tokens, const tq_canonical& out,
                           cudaStream_t st);

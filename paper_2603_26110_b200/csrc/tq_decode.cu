@@ -614,6 +614,11 @@ __global__ void __launch_bounds__(D) finish_kernel(DecodeArgs a, int nbg) {
   const int bgi = (int)blockIdx.x % nbg, lh_c = (int)blockIdx.x / nbg, lc = lh_c / H, h = lh_c - lc * H;
   const int b0 = bgi * kFinB, nb = min(kFinB, B - b0);
   const float* Pv = a.pi_v + ((size_t)(a.layer_begin + lc) * H + h) * D * D;
+  // launched with programmatic stream serialization: PI_V is a constant of the call, so its first 32 rows are fetched
+  // while the last streaming kernels of the chain are still running; only orot has to wait for them
+  float pv[32];
+#pragma unroll
+  for (int k = 0; k < 32; ++k) pv[k] = __ldg(Pv + (size_t)k * D + i);
   pdl_wait();
 #pragma unroll
   for (int e = 0; e < kFinB; ++e) os[e][i] = e < nb ? __ldcg(a.orot + (((size_t)lc * B + b0 + e) * H + h) * D + i) : 0.f;
@@ -625,9 +630,10 @@ __global__ void __launch_bounds__(D) finish_kernel(DecodeArgs a, int nbg) {
   for (int e = 0; e < kFinB; ++e) acc[e] = 0.f;
 #pragma unroll 1
   for (int k0 = 0; k0 < D; k0 += 32) {
-    float pv[32];
+    if (k0 > 0) {
 #pragma unroll
-    for (int k = 0; k < 32; ++k) pv[k] = __ldg(Pv + (size_t)(k0 + k) * D + i);
+      for (int k = 0; k < 32; ++k) pv[k] = __ldg(Pv + (size_t)(k0 + k) * D + i);
+    }
 #pragma unroll
     for (int e = 0; e < kFinB; ++e) {
       float r0 = 0.f, r1 = 0.f, r2 = 0.f, r3 = 0.f;
@@ -671,16 +677,25 @@ static cudaError_t launch_decode_t(const DecodeArgs& a, cudaStream_t st) {
 }
 
 template <int D, typename T>
-static cudaError_t launch_finish_t(const DecodeArgs& a, cudaStream_t st) {
+static cudaError_t launch_finish_t(const DecodeArgs& a, bool programmatic, cudaStream_t st) {
   const int nbg = (a.cv.B + kFinB - 1) / kFinB;
-  finish_kernel<D, T><<<a.n_layers_call * a.cv.H * nbg, D, 0, st>>>(a, nbg);
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(a.n_layers_call * a.cv.H * nbg);
+  cfg.blockDim = dim3(D);
+  cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = programmatic ? 1 : 0;  // after a kernel of the same stream only (the stepper puts it behind a copy)
+  cudaError_t e = cudaLaunchKernelEx(&cfg, finish_kernel<D, T>, a, nbg);
   count_launch();
-  return cudaGetLastError();
+  return e != cudaSuccess ? e : cudaGetLastError();
 }
 
-cudaError_t launch_finish(const DecodeArgs& a, int D, cudaStream_t st) {
-  if (D == 64) return a.dt == TQ_F16 ? launch_finish_t<64, __half>(a, st) : launch_finish_t<64, float>(a, st);
-  return a.dt == TQ_F16 ? launch_finish_t<128, __half>(a, st) : launch_finish_t<128, float>(a, st);
+cudaError_t launch_finish(const DecodeArgs& a, int D, bool programmatic, cudaStream_t st) {
+  if (D == 64) return a.dt == TQ_F16 ? launch_finish_t<64, __half>(a, programmatic, st) : launch_finish_t<64, float>(a, programmatic, st);
+  return a.dt == TQ_F16 ? launch_finish_t<128, __half>(a, programmatic, st) : launch_finish_t<128, float>(a, programmatic, st);
 }
 
 int decode_ctas_per_sm(int D) { return D == 64 ? DecodeCfg<64>::kCtasPerSm : DecodeCfg<128>::kCtasPerSm; }

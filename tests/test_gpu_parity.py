@@ -535,6 +535,59 @@ def test_model_step_host_equals_per_layer_host_steps(tq, oracle):
 
 
 @pytest.mark.gpu
+@pytest.mark.parametrize("n_chunks", [0, 1, 3, 5])
+def test_host_stepper_equals_model_step_host_over_several_steps(tq, oracle, n_chunks):
+    """tq_host_stepper_* (the host-buffer step captured once as a CUDA graph, copies overlapped with the layer chunks)
+    == tq_decode_model_step_host, step after step (seq_len advances on the device; the same graph serves every step),
+    outputs and cache bytes bit for bit, for every chunking."""
+    import torch
+
+    w = W.CONFIGS["cfg1_650m_step"].scaled(n_layers=5, batch=2, n_heads=4, seq=61)
+    L, n_steps = w.n_layers, 4
+    results = []
+    for mode in ("host_call", "stepper", "stepper_device"):
+        c = Case(tq, oracle, w, max_seq=w.seq + 8)
+        for layer in range(L):
+            k, v = W.layer_activations(w, layer)
+            tq.tq_quantize_pack(c.shape, c.params, c.cache, layer, c.dev(k), c.dev(v))
+        dt = tq.TQ_F16 if w.dtype == "f16" else tq.TQ_F32
+        st = torch.zeros(tq.tq_model_step_staging_bytes(c.shape, dt, L) + 256, dtype=torch.uint8, device="cuda")
+        st = st[(-st.data_ptr()) % 256:]
+        ws = tq.Workspace(c.shape, L)
+        toks0 = [W.step_tokens(w, layer, 0) for layer in range(L)]
+        q = torch.from_numpy(np.stack([t[0] for t in toks0])).pin_memory()
+        kn, vn, out = torch.empty_like(q).pin_memory(), torch.empty_like(q).pin_memory(), torch.empty_like(q).pin_memory()
+        stepper = tq.HostStepper(c.shape, c.params, c.cache, 0, L, q, kn, vn, out, st, ws, w.seq + 8, n_chunks) if mode == "stepper" else None
+        if mode == "stepper_device":  # DEVICE buffers: no copies in the graph
+            qd, kd, vd, od = (torch.empty_like(q, device="cuda") for _ in range(4))
+            stepper_d = tq.HostStepper(c.shape, c.params, c.cache, 0, L, qd, kd, vd, od, None, ws, w.seq + 8, n_chunks)
+        outs = []
+        for step in range(n_steps):
+            toks = [W.step_tokens(w, layer, step) for layer in range(L)]
+            for i, t in enumerate((q, kn, vn)):
+                t.copy_(torch.from_numpy(np.stack([x[i] for x in toks])))
+            out.fill_(float("nan"))
+            if mode == "host_call":
+                tq.tq_decode_model_step_host(c.shape, c.params, c.cache, 0, L, q, kn, vn, out, st, ws, w.seq + 8)
+            elif mode == "stepper":
+                stepper.run()
+            else:
+                qd.copy_(q), kd.copy_(kn), vd.copy_(vn)
+                od.fill_(float("nan"))
+                stepper_d.launch()
+                out.copy_(od)
+            outs.append(out.clone())
+        if stepper is not None:
+            stepper.close()
+        assert torch.all(c.cache.seq_len == w.seq + n_steps)
+        results.append((outs, c.cache.data.clone()))
+    for other in results[1:]:
+        for a, b in zip(results[0][0], other[0]):
+            assert torch.isfinite(a.float()).all() and torch.equal(a, b)
+        assert torch.equal(results[0][1], other[1])
+
+
+@pytest.mark.gpu
 def test_model_step_equals_per_layer_steps_and_replays_from_a_graph(tq, oracle):
     """tq_decode_model_step (one prep launch for all layers, then a run-ahead chain of streaming launches) must give
     bit-identical outputs and cache bytes to tq_append + tq_decode_attn called layer by layer; and a CUDA graph of it
