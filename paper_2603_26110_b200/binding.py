@@ -260,7 +260,7 @@ def tq_debug_set_decode_nsplit(nsplit: int):
 
 def tq_debug_set_quantize_impl(fp32_cuda_cores: bool):
     """Test knob: route tq_quantize_pack to the fp32 CUDA-core kernel (cross-check of the tensor-core kernel)."""
-    lib().tq_debug_set_quantize_impl(C.c_int(1 if fp32_cuda_cores else 0))
+    lib().tq_debug_set_quantize_impl(C.c_int(int(fp32_cuda_cores)))
 
 
 def _canon_struct(planes: dict) -> TqCanonical:

@@ -3,26 +3,31 @@
 // Same arithmetic as tq_quantize.cu (PAPER.md:111-116 prefill steps 1,3,4; §3.3 Eq. 5; §3.4 Eq. 6 in the sign(S r)
 // form of BASELINE.json:north_star), but the three rotations y = PI_K x', S r, PI_V v — a dense
 // (tokens x d) x (d x d) contraction — run as tcgen05.mma with the accumulators in tensor memory:
-//   * a CTA of 128 threads owns 128-token blocks of one (batch, head): UMMA M = 128 tokens, N = d outputs, K = 16;
-//     keys (RoPE, PI_K, then S on the residual) and values (PI_V) run as separate CTAs (blockIdx.z);
+//   * a CTA of 256 threads owns 128-token blocks of one (batch, head): UMMA M = 128 tokens, N = d outputs, K = 16;
+//     keys (RoPE, PI_K, then S on the residual) and values (PI_V) run as separate CTAs (alternating along blockIdx.x);
 //   * operands are fp16 in shared memory in the canonical K-major no-swizzle layout (8 x 8 core matrices);
 //     fp32 accuracy comes from two-term splits a = a_hi + a_lo (each product exact in the fp32 accumulator):
 //     D = A_hi B_hi + A_lo B_hi + A_hi B_lo.  Power-of-two scalings keep every split away from the fp16 range
 //     limits and cancel exactly: PI x16, the token vector by 2^-exponent(max |x|) (RoPE grows a pair by at most
 //     sqrt 2), r x8 (only sign(S r) is used); fp16 values V are exact operands and need two products only.  A numpy
 //     study (hard part 4) puts the code-flip rate of this scheme at 2e-7, that of an all-fp32 pipeline;
-//   * the epilogue is thread-per-token: tcgen05.ld hands every thread the rotated coordinates of ITS token, 32
-//     columns at a time (pass 1: the norm; pass 2: codes, residual, packing), so nothing crosses lanes.  The device
-//     tile layout (tq_common.cuh) is the A-fragment order of the decode kernel's MMAs, so every thread drops its
-//     bytes into an image of the block's four tiles in shared memory (byte / halfword stores; V fields, which mix the
-//     two tokens of a pair, are assembled by the pair from a small per-token scratch) and the CTA then writes the
-//     image out with coalesced 16-byte stores.  Tiles only partly covered by the call are pre-loaded into the image.
+//   * the prologue is warp-cooperative: a warp stages 8 token rows at a time, lane = (16-byte chunk, row), so that the
+//     global reads are sector-exact and the 128-bit shared-memory stores of the operand rows are conflict free;
+//   * the epilogue runs two threads per token: thread (token, half) reads the d/2 accumulator columns of ITS half of
+//     ITS token with ONE tcgen05.ld and keeps them in registers for the norm, the code search, the residual and the
+//     packing (the two halves exchange their partial sums of squares through shared memory).  The code search and the
+//     sign bits are computed on the FMA pipe (see code_f).  The device tile layout (tq_common.cuh) is the A-fragment
+//     order of the decode kernel's MMAs, so every thread drops its bytes into an image of the block's four tiles in
+//     shared memory (V fields, which mix the two tokens of a pair, are assembled after one shuffle with the neighbour
+//     token) and the CTA then writes the image out with coalesced 16-byte stores.  Tiles only partly covered by the
+//     call are pre-loaded into the image.
 #include "tq_common.cuh"
 
 namespace tq {
 namespace {
 
-constexpr int kBlk = 128;  // tokens per block = UMMA M = threads per CTA
+constexpr int kBlk = 128;      // tokens per block = UMMA M
+constexpr int kThreads = 256;  // two threads per token: thread (token = tid & 127, half = tid >> 7)
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -39,11 +44,11 @@ struct TcCfg {
   static constexpr int kImgK = Lo::kCodeBytes + Lo::kSignBytes + 4 * kTile;
   static constexpr int kImgV = Lo::kCodeBytes + 2 * kTile;
   static constexpr int kImgBytes = kImgK;          // per tile (the larger of the two)
-  static constexpr int kScrPitch = Lo::C + 1;      // V scratch: C words (8 codes each) per token, odd pitch
   // shared memory: B operands 4 x kMatBytes (keys: PI_K hi/lo, S hi/lo; values: PI_V hi/lo) | A operands hi, lo |
-  // tile images [4][kImgBytes] | V scratch [128][kScrPitch] | LUT, barriers, TMEM slot
+  // tile images [4][kImgBytes] | partial sums [2 kinds][2 halves][128] | row scales [128] | LUT pair table [64] float2,
+  // barriers, TMEM slot
   static constexpr int kOffA = 4 * kMatBytes, kOffMisc = kOffA + 2 * kOpBytes;
-  static constexpr int kSmemBytes = kOffMisc + 4 * kImgBytes + kBlk * kScrPitch * 4 + 8 * 4 + 3 * 8 + 16;
+  static constexpr int kSmemBytes = kOffMisc + 4 * kImgBytes + 4 * kBlk * 4 + kBlk * 4 + 64 * 8 + 3 * 8 + 16;
 };
 
 // byte offset of element (row, k) of a [rows][d] fp16 operand in the canonical K-major no-swizzle layout:
@@ -87,9 +92,9 @@ __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.a
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
 
-// 32 consecutive fp32 accumulator columns of this thread's TMEM lane (= its token)
-__device__ __forceinline__ void tmem_ld32(uint32_t taddr, float (&v)[32]) {
-  uint32_t r[32];
+// NC (32 or 64) consecutive fp32 accumulator columns of this thread's TMEM lane (= its token): every 32-column load is
+// issued before the one wait
+__device__ __forceinline__ void tmem_ld32_nowait(uint32_t taddr, uint32_t* r) {
   asm volatile(
       "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
       "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
@@ -99,9 +104,15 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, float (&v)[32]) {
         "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]),
         "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
       : "r"(taddr));
+}
+template <int NC>
+__device__ __forceinline__ void tmem_ld(uint32_t taddr, float (&v)[NC]) {
+  uint32_t r[NC];
+#pragma unroll
+  for (int c = 0; c < NC / 32; ++c) tmem_ld32_nowait(taddr + 32 * c, r + 32 * c);
   asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 #pragma unroll
-  for (int i = 0; i < 32; ++i) v[i] = __uint_as_float(r[i]);
+  for (int i = 0; i < NC; ++i) v[i] = __uint_as_float(r[i]);
 }
 // two-term fp16 split of 8 consecutive values, packed as two 16-byte rows of the operand layout
 __device__ __forceinline__ void split8(const float* x, uint4& hi, uint4& lo) {
@@ -122,8 +133,10 @@ __device__ __forceinline__ void split8(const float* x, uint4& hi, uint4& lo) {
 template <int D>
 __device__ __forceinline__ void stage_matrix(unsigned char* bhi, unsigned char* blo, const float* __restrict__ M, float scale,
                                              int tid) {
-  for (int idx = tid; idx < D * D / 8; idx += kBlk) {
-    const int n = idx / (D / 8), kj = idx % (D / 8);
+  // consecutive threads take consecutive rows n of one 16-byte column chunk: eight of them fill one core matrix row
+  // group (128 contiguous bytes), so the 128-bit stores are conflict free; the reads are whole 32-byte sectors
+  for (int idx = tid; idx < D * D / 8; idx += kThreads) {
+    const int n = idx % D, kj = idx / D;
     const float4 a = __ldg(reinterpret_cast<const float4*>(M + n * D + 8 * kj));
     const float4 b = __ldg(reinterpret_cast<const float4*>(M + n * D + 8 * kj) + 1);
     const float x[8] = {a.x * scale, a.y * scale, a.z * scale, a.w * scale, b.x * scale, b.y * scale, b.z * scale, b.w * scale};
@@ -142,16 +155,47 @@ __device__ __forceinline__ void pow2_scale(float amax, float& s, float& inv_s) {
   inv_s = __uint_as_float(E << 23);
 }
 
-// code = #{k : u > thr[k]} for ascending thresholds, as a three-step binary search (3 compares + 4 selects instead of
-// 7 compares + 7 adds); identical result, ties included (u > t is evaluated on the same thresholds)
-__device__ __forceinline__ int code_of(float u, const float (&thr)[7]) {
-  const bool b2 = u > thr[3];
-  const float tm = b2 ? thr[5] : thr[1];
-  const bool b1 = u > tm;
-  const float tl = b2 ? (b1 ? thr[6] : thr[4]) : (b1 ? thr[2] : thr[0]);
-  const bool b0 = u > tl;
-  return (b2 ? 4 : 0) + (b1 ? 2 : 0) + (b0 ? 1 : 0);
+// ---- code search on the FMA pipe ---------------------------------------------------------------------------------------
+// code = #{k : u > t_k} for the seven ascending thresholds t_k, u = y / n.  The compare-and-select form (FSETP / FSEL /
+// SEL) runs on the half-rate integer ALU pipe, which ncu showed to be the busiest pipe of this kernel (47 %) while the FMA
+// pipe idled at 15 %; here the three-step binary search is arithmetic only:
+//   [y > T] = sat((y - T) 2^100)  is exactly 0 or 1 (one FFMA.SAT: the fused product-sum has the exact sign, a nonzero
+//   difference of two floats of ordinary magnitude times 2^100 exceeds 1, a tie gives 0 = the lower code);
+//   the next threshold is picked by multiplying with those 0 / 1 values: T1 + b2 (T5 - T1), and
+//   T0 + b1 (T2 - T0) + b2 (T4 - T0) + b1 b2 (T6 - T4 - T2 + T0).
+// Everything is compared on the accumulator y against T = t n (n = |y|; 1 for a zero vector, whose codes are those of
+// u = 0), so u is never formed.  The picked thresholds are sums of rounded differences and t n is rounded: they differ
+// from the fp32 midpoints by a few ulp (relative 2e-7), far inside the 1e-5 band in which a code may differ from the
+// fp64 oracle (and of the same size as the rounding of y itself).  Thresholds closer to zero than 2^-70 other than an
+// exact 0 would break the 0 / 1 property; Lloyd-Max midpoints are not.
+constexpr float kBig = 1.2676506002282294e30f;  // 2^100
+struct Search {
+  float k3, k1, k51, k0, kA, kB, kC;  // -T 2^100: T3, T1, T5 - T1, T0, T2 - T0, T4 - T0, (T6 - T4) - (T2 - T0)
+};
+__device__ __forceinline__ Search make_search(const float (&t)[7]) {
+  Search s;
+  s.k3 = -t[3] * kBig, s.k1 = -t[1] * kBig, s.k51 = -(t[5] - t[1]) * kBig, s.k0 = -t[0] * kBig;
+  s.kA = -(t[2] - t[0]) * kBig, s.kB = -(t[4] - t[0]) * kBig;
+  s.kC = -((t[6] - t[4]) - (t[2] - t[0])) * kBig;
+  return s;
 }
+__device__ __forceinline__ Search scaled(const Search& c, float nn) {
+  return Search{c.k3 * nn, c.k1 * nn, c.k51 * nn, c.k0 * nn, c.kA * nn, c.kB * nn, c.kC * nn};
+}
+__device__ __forceinline__ float fma_sat(float a, float b, float c) {
+  float d;
+  asm("fma.rn.sat.f32 %0, %1, %2, %3;" : "=f"(d) : "f"(a), "f"(b), "f"(c));
+  return d;
+}
+// the code of y as a float (0.0 .. 7.0)
+__device__ __forceinline__ float code_f(float y, const Search& s) {
+  const float b2 = fma_sat(y, kBig, s.k3);
+  const float b1 = fma_sat(y, kBig, fmaf(b2, s.k51, s.k1));
+  const float b0 = fma_sat(y, kBig, fmaf(b1 * b2, s.kC, fmaf(b2, s.kB, fmaf(b1, s.kA, s.k0))));
+  return fmaf(b2, 4.f, fmaf(b1, 2.f, b0));
+}
+// an exact small integer held in a float, as an unsigned (F2I runs on the otherwise idle conversion pipe)
+__device__ __forceinline__ unsigned f2u(float x) { return __float2uint_rn(x); }
 
 
 // 8 consecutive input values of one token as floats (zeros for a token outside the call)
@@ -176,20 +220,6 @@ __device__ __forceinline__ void load8(const T* p, bool valid, float (&x)[8]) {
   }
 }
 
-// max |x| over one token's d input values (first pass over the row; the second pass hits L1/L2)
-template <int D, typename T>
-__device__ __forceinline__ float row_amax(const T* p, bool valid) {
-  float amax = 0.f;
-#pragma unroll 4
-  for (int kj = 0; kj < D / 8; ++kj) {
-    float x[8];
-    load8<T>(p + 8 * kj, valid, x);
-#pragma unroll
-    for (int j = 0; j < 8; ++j) amax = fmaxf(amax, fabsf(x[j]));
-  }
-  return amax;
-}
-
 template <int D>
 __device__ __forceinline__ void store_split8(const float (&x)[8], float s, unsigned char* ahi, unsigned char* alo, int row, int k0) {
   float xs[8];
@@ -201,90 +231,112 @@ __device__ __forceinline__ void store_split8(const float (&x)[8], float s, unsig
   *reinterpret_cast<uint4*>(alo + core_off<D>(row, k0)) = lo;
 }
 
-// keys: RoPE (fp64-evaluated table), scale, split, store both operand rows; returns the exact inverse scale
-template <int D, typename T>
-__device__ __forceinline__ float stage_key_row(const T* p, bool valid, const float* __restrict__ cs_row /* [d/2][2] */,
-                                               int rope_layout, unsigned char* ahi, unsigned char* alo, int row) {
-  float s, inv_s;
-  pow2_scale(row_amax<D, T>(p, valid), s, inv_s);  // |RoPE(x) s| < 2 sqrt 2
-  if (rope_layout == 0) {  // pairs (2g, 2g+1): four pairs per 8-value chunk
-#pragma unroll 4
-    for (int kj = 0; kj < D / 8; ++kj) {
-      float x[8];
-      load8<T>(p + 8 * kj, valid, x);
-      const float4 c0 = __ldg(reinterpret_cast<const float4*>(cs_row + 8 * kj)), c1 = __ldg(reinterpret_cast<const float4*>(cs_row + 8 * kj) + 1);
-      const float cs[8] = {c0.x, c0.y, c0.z, c0.w, c1.x, c1.y, c1.z, c1.w};
-      float y[8];
+// ---- prologue: the A operand rows of one 128-token block -------------------------------------------------------------
+// Warp w stages rows [16 w, 16 w + 16) in two groups of 8; lane = 8 kk + r owns row r of the group and the 8-value
+// chunks kj = kk + 4 i (i < d/32).  A quarter-warp (fixed kk) reads 8 rows x 16 bytes (whole sectors once the other
+// chunks of the row are counted) and writes 8 consecutive 16-byte rows of one core matrix: no bank conflict.
+// Keys: RoPE from the fp64-evaluated table, power-of-two row scale, two-term split.  Values: fp16 rows are exact
+// operands (copied), fp32 rows are scaled and split.  scale_s[row] = the exact inverse row scale.
+template <int D, typename T, bool kKey>
+__device__ __forceinline__ void stage_rows(const T* __restrict__ src, int i_first /* call index of block row 0 */, int n_tokens,
+                                           const float* __restrict__ cs_blk /* rope_cs row of block row 0 */, int rows_cs /* rows of the table left */,
+                                           int rope_layout, unsigned char* ahi, unsigned char* alo, float* scale_s, int warp, int lane) {
+  constexpr int NI = D / 32;  // chunks per lane and row
+  const int r = lane & 7, kk = lane >> 3;
 #pragma unroll
-      for (int j = 0; j < 4; ++j) {
-        y[2 * j] = x[2 * j] * cs[2 * j] - x[2 * j + 1] * cs[2 * j + 1];
-        y[2 * j + 1] = x[2 * j] * cs[2 * j + 1] + x[2 * j + 1] * cs[2 * j];
-      }
-      store_split8<D>(y, s, ahi, alo, row, 8 * kj);
-    }
-  } else {  // pairs (g, g + d/2): chunk kj with chunk kj + d/16
-#pragma unroll 2
-    for (int kj = 0; kj < D / 16; ++kj) {
-      float xa[8], xb[8], ya[8], yb[8];
-      load8<T>(p + 8 * kj, valid, xa);
-      load8<T>(p + D / 2 + 8 * kj, valid, xb);
+  for (int gi = 0; gi < 2; ++gi) {
+    const int row = 16 * warp + 8 * gi + r;
+    const int i = i_first + row;
+    const bool valid = i >= 0 && i < n_tokens;
+    const T* p = src + (size_t)i * D;
+    if constexpr (!kKey && sizeof(T) == 2) {
 #pragma unroll
-      for (int q = 0; q < 4; ++q) {
-        const float4 c = __ldg(reinterpret_cast<const float4*>(cs_row + 16 * kj) + q);  // pairs g = 8 kj + 2q, + 1
-        ya[2 * q] = xa[2 * q] * c.x - xb[2 * q] * c.y, yb[2 * q] = xa[2 * q] * c.y + xb[2 * q] * c.x;
-        ya[2 * q + 1] = xa[2 * q + 1] * c.z - xb[2 * q + 1] * c.w, yb[2 * q + 1] = xa[2 * q + 1] * c.w + xb[2 * q + 1] * c.z;
+      for (int ii = 0; ii < NI; ++ii) {
+        const int kj = kk + 4 * ii;
+        *reinterpret_cast<uint4*>(ahi + core_off<D>(row, 8 * kj)) =
+            valid ? __ldg(reinterpret_cast<const uint4*>(p) + kj) : make_uint4(0, 0, 0, 0);
       }
-      store_split8<D>(ya, s, ahi, alo, row, 8 * kj);
-      store_split8<D>(yb, s, ahi, alo, row, D / 2 + 8 * kj);
+      if (kk == 0) scale_s[row] = 1.f;
+    } else {
+      float x[NI][8];
+#pragma unroll
+      for (int ii = 0; ii < NI; ++ii) load8<T>(p + 8 * (kk + 4 * ii), valid, x[ii]);
+      float amax = 0.f;
+#pragma unroll
+      for (int ii = 0; ii < NI; ++ii)
+#pragma unroll
+        for (int j = 0; j < 8; ++j) amax = fmaxf(amax, fabsf(x[ii][j]));
+      amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, 8));
+      amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, 16));
+      float s, inv_s;
+      pow2_scale(amax, s, inv_s);  // |RoPE(x) s| < 2 sqrt 2
+      if (kk == 0) scale_s[row] = inv_s;
+      if constexpr (kKey) {
+        const float* cs_row = cs_blk + (size_t)min(row, rows_cs - 1) * D;
+        if (rope_layout == 0) {  // pairs (2g, 2g+1): four pairs per chunk
+#pragma unroll
+          for (int ii = 0; ii < NI; ++ii) {
+            const int kj = kk + 4 * ii;
+            const float4 c0 = __ldg(reinterpret_cast<const float4*>(cs_row + 8 * kj)), c1 = __ldg(reinterpret_cast<const float4*>(cs_row + 8 * kj) + 1);
+            const float cs[8] = {c0.x, c0.y, c0.z, c0.w, c1.x, c1.y, c1.z, c1.w};
+            float y[8];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+              y[2 * j] = x[ii][2 * j] * cs[2 * j] - x[ii][2 * j + 1] * cs[2 * j + 1];
+              y[2 * j + 1] = x[ii][2 * j] * cs[2 * j + 1] + x[ii][2 * j + 1] * cs[2 * j];
+            }
+            store_split8<D>(y, s, ahi, alo, row, 8 * kj);
+          }
+        } else {  // pairs (g, g + d/2): chunk kj with chunk kj + d/16, both owned by this lane
+#pragma unroll
+          for (int ii = 0; ii < NI / 2; ++ii) {
+            const int kj = kk + 4 * ii;
+            float ya[8], yb[8];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+              const float4 c = __ldg(reinterpret_cast<const float4*>(cs_row + 16 * kj) + q);  // pairs g = 8 kj + 2q, + 1
+              ya[2 * q] = x[ii][2 * q] * c.x - x[ii + NI / 2][2 * q] * c.y, yb[2 * q] = x[ii][2 * q] * c.y + x[ii + NI / 2][2 * q] * c.x;
+              ya[2 * q + 1] = x[ii][2 * q + 1] * c.z - x[ii + NI / 2][2 * q + 1] * c.w;
+              yb[2 * q + 1] = x[ii][2 * q + 1] * c.w + x[ii + NI / 2][2 * q + 1] * c.z;
+            }
+            store_split8<D>(ya, s, ahi, alo, row, 8 * kj);
+            store_split8<D>(yb, s, ahi, alo, row, D / 2 + 8 * kj);
+          }
+        }
+      } else {
+#pragma unroll
+        for (int ii = 0; ii < NI; ++ii) store_split8<D>(x[ii], s, ahi, alo, row, 8 * (kk + 4 * ii));
+      }
     }
-  }
-  return inv_s;
-}
-
-// values: fp16 inputs are exact operands (copied as they are, no scale); fp32 inputs are scaled and split
-template <int D, typename T>
-__device__ __forceinline__ float stage_value_row(const T* p, bool valid, unsigned char* ahi, unsigned char* alo, int row) {
-  if constexpr (sizeof(T) == 2) {
-#pragma unroll 4
-    for (int kj = 0; kj < D / 8; ++kj)
-      *reinterpret_cast<uint4*>(ahi + core_off<D>(row, 8 * kj)) =
-          valid ? __ldg(reinterpret_cast<const uint4*>(p) + kj) : make_uint4(0, 0, 0, 0);
-    return 1.f;
-  } else {
-    float s, inv_s;
-    pow2_scale(row_amax<D, T>(p, valid), s, inv_s);
-#pragma unroll 4
-    for (int kj = 0; kj < D / 8; ++kj) {
-      float x[8];
-      load8<T>(p + 8 * kj, valid, x);
-      store_split8<D>(x, s, ahi, alo, row, 8 * kj);
-    }
-    return inv_s;
   }
 }
 
 template <int D, typename T, bool kKey>
-__device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int blocks_per_cta, unsigned char* smem) {
+__device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int blocks_per_cta, int cta_x, unsigned char* smem) {
   using Cfg = TcCfg<D>;
   using Lo = Layout<D>;
   constexpr bool kF16 = sizeof(T) == 2;
-  constexpr int KCW = Lo::KCW, KSW = Lo::KSW, P = Lo::P;
+  constexpr int KCW = Lo::KCW, KSW = Lo::KSW;
+  constexpr int NC = D / 2;  // accumulator columns per thread
   unsigned char *B0_hi = smem, *B0_lo = smem + Cfg::kMatBytes;                               // PI_K | PI_V
   unsigned char *B1_hi = smem + 2 * Cfg::kMatBytes, *B1_lo = smem + 3 * Cfg::kMatBytes;      // S (keys only)
   unsigned char *A_hi = smem + Cfg::kOffA, *A_lo = A_hi + Cfg::kOpBytes;
   unsigned char* img = smem + Cfg::kOffMisc;                                  // [4 tiles][kImgBytes]
-  unsigned* vscr = reinterpret_cast<unsigned*>(img + 4 * Cfg::kImgBytes);     // [128][kScrPitch] V code groups
-  float* lut_s = reinterpret_cast<float*>(vscr + kBlk * Cfg::kScrPitch);      // [8]
-  unsigned long long* mbar = reinterpret_cast<unsigned long long*>(lut_s + 8);  // [0]: first product, [1]: S product
+  float* red_n = reinterpret_cast<float*>(img + 4 * Cfg::kImgBytes);          // [2 halves][128] partial |y|^2
+  float* red_g = red_n + 2 * kBlk;                                            // [2 halves][128] partial |8 r|^2
+  float* scale_s = red_g + 2 * kBlk;                                          // [128] inverse row scales
+  float2* lutp = reinterpret_cast<float2*>(scale_s + kBlk);                   // [64] keys: (-8 lut[c0], -8 lut[c1]) at c0 + 8 c1
+  unsigned long long* mbar = reinterpret_cast<unsigned long long*>(lutp + 64);  // [0]: first product, [1]: S product
   unsigned* tmem_slot = reinterpret_cast<unsigned*>(mbar + 3);
 
-  const int tid = threadIdx.x, warp = tid >> 5;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int tok = tid & (kBlk - 1), half = tid >> 7;  // epilogue role: token row and column half
   const int bh = blockIdx.y, b = bh / a.cv.H, h = bh % a.cv.H;
   const int first_blk = a.start_pos / kBlk, last_blk = (a.start_pos + a.n_tokens - 1) / kBlk;
-  const int blk0 = first_blk + (int)blockIdx.x * blocks_per_cta;
+  const int blk0 = first_blk + cta_x * blocks_per_cta;
   if (blk0 > last_blk) return;
   const int blk1 = min(last_blk, blk0 + blocks_per_cta - 1);
-  if (kKey && blockIdx.x == 0 && h == 0 && tid == 0) a.cv.seq_len[a.layer * a.cv.B + b] = a.start_pos + a.n_tokens;
+  if (kKey && cta_x == 0 && h == 0 && tid == 0) a.cv.seq_len[a.layer * a.cv.B + b] = a.start_pos + a.n_tokens;
 
   // ---- one-time setup: tensor memory, barriers, the B operands of this head, LUT
   if (warp == 0) {
@@ -304,22 +356,27 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
   } else {
     stage_matrix<D>(B0_hi, B0_lo, a.pi_v + (size_t)h * D * D, 16.f, tid);
   }
-  float thr[7];
+  // thresholds t_k = (lut_k + lut_{k+1}) / 2 in fp32, as search constants; keys also keep a table of LUT pairs for the
+  // residual: the S product takes 8 r (only sign(S r) is used, and 8 r splits cleanly in fp16), |r| = |8 r| / 8
+  Search search0;
   {
     const float* lut_g = (kKey ? a.lut_k : a.lut_v) + h * 8;
-    float l8[8];
+    float l8[8], thr[7];
 #pragma unroll
     for (int q = 0; q < 8; ++q) l8[q] = __ldg(lut_g + q);
 #pragma unroll
     for (int q = 0; q < 7; ++q) thr[q] = 0.5f * (l8[q] + l8[q + 1]);
-    if (tid < 8) lut_s[tid] = __ldg(lut_g + tid);
+    search0 = make_search(thr);
+    if (kKey && tid < 64) lutp[tid] = make_float2(-8.f * __ldg(lut_g + (tid & 7)), -8.f * __ldg(lut_g + (tid >> 3)));
   }
+  const float lutp_base = (float)smem_u32(lutp);  // shared-window address, exact in fp32
   fence_async_smem();
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = *tmem_slot;
-  const uint32_t t_lane = tmem + ((uint32_t)(warp * 32) << 16);  // this warp's quadrant of TMEM lanes
+  // this thread's TMEM lane (its token) and first column: warps w and w + 4 share the lane quadrant w % 4
+  const uint32_t t_lane = tmem + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)(half * NC);
   const uint32_t a_hi = smem_u32(A_hi), a_lo = smem_u32(A_lo), b0_hi = smem_u32(B0_hi), b0_lo = smem_u32(B0_lo),
                  b1_hi = smem_u32(B1_hi), b1_lo = smem_u32(B1_lo);
   auto gemm = [&](uint32_t dcol, uint32_t a_op, uint32_t b_op, bool first) {  // D[:, dcol..dcol+d) (+)= A B^T, K = d
@@ -331,7 +388,7 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
 
   const T* src = reinterpret_cast<const T*>(kKey ? a.k : a.v) + (size_t)bh * a.n_tokens * D;
   unsigned char* stream = a.cv.tiles + ((size_t)a.layer * a.cv.B * a.cv.H + bh) * a.cv.stream_bytes;
-  const int slot = tid & 31, tl = tid >> 5, sg = slot & 7, sr = slot >> 3;
+  const int slot = tok & 31, tl = tok >> 5, sg = slot & 7, sr = slot >> 3;
   unsigned char* timg = img + tl * Cfg::kImgBytes;  // image of this token's tile
   constexpr int kOffImgKS = Lo::kCodeBytes, kOffImgNK = Lo::kCodeBytes + Lo::kSignBytes;  // keys image
   constexpr int kOffImgVN = Lo::kCodeBytes;                                                // values image
@@ -340,7 +397,7 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
 
   for (int blk = blk0; blk <= blk1; ++blk) {
     const uint32_t parity = (uint32_t)(blk - blk0) & 1u;
-    const int pos = blk * kBlk + tid;
+    const int pos = blk * kBlk + tok;
     const int i = pos - a.start_pos;
     const bool valid = i >= 0 && i < a.n_tokens;
     // tiles of this block: covered (some token of the call) / fully covered; partly covered ones are pre-loaded so that
@@ -352,7 +409,7 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
     };
     {
       constexpr int kOwn = kKey ? Cfg::kImgK : Cfg::kImgV;
-      for (int idx = tid; idx < 4 * (kOwn / 16); idx += kBlk) {
+      for (int idx = tid; idx < 4 * (kOwn / 16); idx += kThreads) {
         const int t4 = idx / (kOwn / 16), q = idx % (kOwn / 16);
         if (tile_cover(t4) != 1) continue;
         const unsigned char* tg = stream + (size_t)(blk * 4 + t4) * Lo::kTileBytes;
@@ -364,13 +421,12 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
       }
     }
 
-    // ---- stage the A operand rows of this thread's token and start the first product
-    float inv_s;
-    if constexpr (kKey)
-      inv_s = stage_key_row<D, T>(src + (size_t)i * D, valid, a.rope_cs + (size_t)min(pos, a.cv.max_seq - 1) * D, a.rope_layout,
-                                  A_hi, A_lo, tid);
-    else
-      inv_s = stage_value_row<D, T>(src + (size_t)i * D, valid, A_hi, A_lo, tid);
+    // ---- stage the A operand rows of the block and start the first product
+    {
+      const int p0 = blk * kBlk;  // cache position (= RoPE position) of block row 0
+      stage_rows<D, T, kKey>(src, p0 - a.start_pos, a.n_tokens, a.rope_cs + (size_t)min(p0, a.cv.max_seq - 1) * D,
+                             a.cv.max_seq - min(p0, a.cv.max_seq - 1), a.rope_layout, A_hi, A_lo, scale_s, warp, lane);
+    }
     fence_async_smem();
     tc_fence_before();
     __syncthreads();
@@ -380,56 +436,70 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
       if (kKey || !kF16) gemm(0, a_lo, b0_hi, false);
       umma_commit(smem_u32(mbar + 0));
     }
+    if (tid == 32 && blk < blk1) {  // the next block's input rows on their way to L2 while this block is worked on
+      const int lo = max((blk + 1) * kBlk - a.start_pos, 0), hi = min((blk + 2) * kBlk - a.start_pos, a.n_tokens);
+      if (hi > lo)
+        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src + (size_t)lo * D), "r"((unsigned)((hi - lo) * D * sizeof(T))) : "memory");
+    }
     mbar_wait(smem_u32(mbar + 0), parity);
     tc_fence_after();
 
-    // ---- thread = token, pass 1: |y|^2 over the d accumulator columns
-    float n2 = 0.f;
-#pragma unroll 1
-    for (int c = 0; c < D / 32; ++c) {
-      float y[32];
-      tmem_ld32(t_lane + 32 * c, y);
+    // ---- thread = (token, column half): its d/2 accumulator columns, once; |y|^2 through shared memory
+    float y[NC];
+    tmem_ld<NC>(t_lane, y);
+    {
+      float p0 = 0.f, p1 = 0.f, p2 = 0.f, p3 = 0.f;
 #pragma unroll
-      for (int j = 0; j < 32; ++j) n2 = fmaf(y[j], y[j], n2);
+      for (int j = 0; j < NC; j += 4) {
+        p0 = fmaf(y[j], y[j], p0), p1 = fmaf(y[j + 1], y[j + 1], p1);
+        p2 = fmaf(y[j + 2], y[j + 2], p2), p3 = fmaf(y[j + 3], y[j + 3], p3);
+      }
+      red_n[half * kBlk + tok] = (p0 + p1) + (p2 + p3);
     }
-    const float n = sqrtf(n2);
-    const float inv = n > 0.f ? 1.0f / n : 0.f;
-    const unsigned short n_h = f32_to_f16_bits_clamped(n * inv_s * 0.0625f);  // y = 16 s PI x
+    __syncthreads();
+    const float n = sqrtf(red_n[tok] + red_n[kBlk + tok]);
+    const unsigned short n_h = f32_to_f16_bits_clamped(n * scale_s[tok] * 0.0625f);  // y = 16 s PI x
+    const Search sr_n = scaled(search0, n > 0.f ? n : 1.f);  // thresholds on the accumulator scale
 
     if constexpr (kKey) {
-      // ---- pass 2: codes, residual (the A operand of the S product); the pair fields go straight into the tile image:
-      //      pair p = 16 c + g belongs to lane (sg, t = g & 3) as field j = 4 c + (g >> 2) of this token's block
-      //      (bits [6 J sr + 6 j, + 6) of the lane's string): four fields = three bytes per lane and chunk
-      float g2 = 0.f;
-#pragma unroll 1
-      for (int c = 0; c < D / 32; ++c) {
-        float y[32];
-        tmem_ld32(t_lane + 32 * c, y);
-        unsigned yt[4] = {0u, 0u, 0u, 0u};
+      // ---- codes, residual (the A operand of the S product, written over this token's operand row: the first product is
+      //      complete).  Pair p = half d/4 + g belongs to lane (sg, t = g & 3) as field j = half d/32 + (g >> 2) of this
+      //      token's block, bits [6 (J sr + j), + 6) of the lane's string: four fields = three bytes
+      const float inv8 = n > 0.f ? 8.0f / n : 0.f;
+      float g2a = 0.f, g2b = 0.f;
+      float yt[4][NC / 32];  // four six-bit fields = one 24-bit word, accumulated exactly in fp32
 #pragma unroll
-        for (int g = 0; g < 16; ++g) {
-          const float u0 = y[2 * g] * inv, u1 = y[2 * g + 1] * inv;
-          const int c0 = code_of(u0, thr), c1 = code_of(u1, thr);
-          const float r0 = u0 - lut_s[c0], r1 = u1 - lut_s[c1];
-          g2 = fmaf(r0, r0, fmaf(r1, r1, g2));
-          y[2 * g] = r0 * 8.f, y[2 * g + 1] = r1 * 8.f;  // scaled for the fp16 split (only sign(S r) is used)
-          yt[g & 3] |= (unsigned)(c0 | (c1 << 3)) << (6 * (g >> 2));
-        }
-        if (valid) {
+      for (int t = 0; t < 4; ++t)
 #pragma unroll
-          for (int t = 0; t < 4; ++t) {
-            const int sb = (6 * Lo::J * sr) / 8 + 3 * c;  // byte of the lane's K string
+        for (int wi = 0; wi < NC / 32; ++wi) yt[t][wi] = 0.f;
 #pragma unroll
-            for (int k = 0; k < 3; ++k) timg[sec_byte(KCW, 4 * sg + t, sb + k)] = (unsigned char)(yt[t] >> (8 * k));
+      for (int g = 0; g < NC / 2; ++g) {
+        const float field = fmaf(code_f(y[2 * g + 1], sr_n), 8.f, code_f(y[2 * g], sr_n));  // c0 | c1 << 3
+        float2 nl;  // (-8 lut[c0], -8 lut[c1])
+        asm("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(nl.x), "=f"(nl.y) : "r"(f2u(fmaf(field, 8.f, lutp_base))));
+        const float r0 = fmaf(y[2 * g], inv8, nl.x), r1 = fmaf(y[2 * g + 1], inv8, nl.y);  // 8 (u - lut[c])
+        g2a = fmaf(r0, r0, g2a), g2b = fmaf(r1, r1, g2b);
+        y[2 * g] = r0, y[2 * g + 1] = r1;
+        yt[g & 3][g >> 4] = fmaf(field, (float)(1u << (6 * ((g >> 2) & 3))), yt[g & 3][g >> 4]);
+      }
+      red_g[half * kBlk + tok] = g2a + g2b;
+      if (valid) {
+#pragma unroll
+        for (int t = 0; t < 4; ++t)
+#pragma unroll
+          for (int wi = 0; wi < NC / 32; ++wi) {
+            const int sb = (6 * Lo::J * sr) / 8 + 3 * (half * (NC / 32) + wi);  // byte of the lane's K string
+            const unsigned w24 = f2u(yt[t][wi]);
+#pragma unroll
+            for (int k = 0; k < 3; ++k) timg[sec_byte(KCW, 4 * sg + t, sb + k)] = (unsigned char)(w24 >> (8 * k));
           }
-        }
+      }
 #pragma unroll
-        for (int kj = 0; kj < 4; ++kj) {  // the first product is complete (barrier): the A buffers are free
-          uint4 hi, lo;
-          split8(&y[8 * kj], hi, lo);
-          *reinterpret_cast<uint4*>(A_hi + core_off<D>(tid, 32 * c + 8 * kj)) = hi;
-          *reinterpret_cast<uint4*>(A_lo + core_off<D>(tid, 32 * c + 8 * kj)) = lo;
-        }
+      for (int kj = 0; kj < NC / 8; ++kj) {
+        uint4 hi, lo;
+        split8(&y[8 * kj], hi, lo);
+        *reinterpret_cast<uint4*>(A_hi + core_off<D>(tok, half * NC + 8 * kj)) = hi;
+        *reinterpret_cast<uint4*>(A_lo + core_off<D>(tok, half * NC + 8 * kj)) = lo;
       }
       fence_async_smem();
       tc_fence_before();
@@ -439,25 +509,30 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
         gemm(D, a_hi, b1_hi, true), gemm(D, a_lo, b1_hi, false), gemm(D, a_hi, b1_lo, false);
         umma_commit(smem_u32(mbar + 1));
       }
-      if (valid)
+      if (valid && half == 0)
         reinterpret_cast<unsigned*>(timg + kOffImgNK)[slot_lane(slot)] =
-            (unsigned)n_h | ((unsigned)f32_to_f16_bits_clamped(sqrtf(g2)) << 16);
-      // ---- residual sketch: bit j = [(S r)_j >= 0].  Sketch rows [t d/4, (t+1) d/4) belong to lane (sg, t) as 16-bit
-      //      pieces u; a piece is stored as two bytes of word (mt, u): byte (sr & 1) holds bits 0..7, byte 2 + (sr & 1)
-      //      bits 8..15 (the byte interleave with the slot 8 further on makes the decode kernel's fp16x2 masks work)
+            (unsigned)n_h | ((unsigned)f32_to_f16_bits_clamped(sqrtf(red_g[tok] + red_g[kBlk + tok]) * 0.125f) << 16);
+      // ---- residual sketch: bit j = [(S r)_j >= 0] for this thread's sketch rows [half d/2, + d/2).  Sketch rows
+      //      [t d/4, (t+1) d/4) belong to lane (sg, t) as 16-bit pieces u; a piece is stored as two bytes of word (mt, u):
+      //      byte (sr & 1) holds bits 0..7, byte 2 + (sr & 1) bits 8..15 (the byte interleave with the slot 8 further on
+      //      makes the decode kernel's fp16x2 masks work)
       mbar_wait(smem_u32(mbar + 1), parity);
       tc_fence_after();
-#pragma unroll 1
-      for (int c = 0; c < D / 32; ++c) {
-        float y[32];
-        tmem_ld32(t_lane + D + 32 * c, y);
-        unsigned w = 0u;
+      tmem_ld<NC>(t_lane + D, y);
 #pragma unroll
-        for (int j = 0; j < 32; ++j) w |= (y[j] >= 0.f ? 1u : 0u) << j;
+      for (int c = 0; c < NC / 32; ++c) {
+        // [y >= 0] = sat(y 2^100 + 1), sixteen bits summed exactly in one float
+        float w0 = 0.f, w1 = 0.f;
+#pragma unroll
+        for (int j = 0; j < 16; ++j) {
+          w0 = fmaf(fma_sat(y[32 * c + j], kBig, 1.f), (float)(1u << j), w0);
+          w1 = fmaf(fma_sat(y[32 * c + 16 + j], kBig, 1.f), (float)(1u << j), w1);
+        }
+        const unsigned w = f2u(w0) | (f2u(w1) << 16);
         if (valid) {
 #pragma unroll
           for (int q = 0; q < 2; ++q) {
-            const int rho0 = 32 * c + 16 * q, t = rho0 / (D / 4), u = (rho0 % (D / 4)) >> 4;
+            const int rho0 = half * NC + 32 * c + 16 * q, t = rho0 / (D / 4), u = (rho0 % (D / 4)) >> 4;
             const int word = (sr >> 1) * Lo::U + u;
             unsigned char* wp = timg + kOffImgKS + word_offset(KSW, word, 4 * sg + t);
             wp[sr & 1] = (unsigned char)(w >> (16 * q));
@@ -466,66 +541,49 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
         }
       }
     } else {
-      // ---- values, pass 2: codes, eight per scratch word; then the two tokens of a pair assemble the six-bit fields
-      //      code_i(even token) | code_i(odd token) << 3 of lane (i & 7, pp & 3), block j = pp >> 2: the even token
-      //      builds the lanes i & 7 < 4, the odd one the others
-      unsigned* myg = vscr + tid * Cfg::kScrPitch;
-#pragma unroll 1
-      for (int c = 0; c < D / 32; ++c) {
-        float y[32];
-        tmem_ld32(t_lane + 32 * c, y);
+      // ---- values: codes of this thread's coordinates, eight per word; one shuffle hands them to the neighbour token
+      //      of the pair, then the pair assembles the six-bit fields code_i(even token) | code_i(odd token) << 3 of lane
+      //      (i & 7, pp & 3), block j = pp >> 2: the even token builds the lanes i & 7 < 4, the odd one the others.
+      //      This thread's coordinates 8 c + (i & 7), c in [half d/16, + d/16), are d/16 fields = 3 d/64 bytes per lane
+      constexpr int CW = NC / 8;  // code words of this thread
+      unsigned mine[CW], other[CW];
 #pragma unroll
-        for (int q = 0; q < 4; ++q) {
-          unsigned w = 0;
+      for (int c = 0; c < CW; ++c) {
+        float w = 0.f;  // eight codes = 24 bits, exact in fp32
 #pragma unroll
-          for (int i = 0; i < 8; ++i) w |= (unsigned)code_of(y[8 * q + i] * inv, thr) << (3 * i);
-          myg[4 * c + q] = w;
-        }
+        for (int q = 0; q < 8; ++q) w = fmaf(code_f(y[8 * c + q], sr_n), (float)(1u << (3 * q)), w);
+        mine[c] = f2u(w);
       }
-      if (valid) reinterpret_cast<unsigned short*>(timg + kOffImgVN)[slot_lane(slot)] = n_h;
-      __syncwarp();
+#pragma unroll
+      for (int c = 0; c < CW; ++c) other[c] = __shfl_xor_sync(0xffffffffu, mine[c], 1);
+      if (valid && half == 0) reinterpret_cast<unsigned short*>(timg + kOffImgVN)[slot_lane(slot)] = n_h;
       {
         const int e = slot & 1, pp = slot >> 1;
-        const unsigned* ge = vscr + (tid & ~1) * Cfg::kScrPitch;  // even token of the pair
-        const unsigned* go = ge + Cfg::kScrPitch;                 // odd token
-        const bool v_e = __shfl_sync(0xffffffffu, valid, (slot & ~1)), v_o = __shfl_sync(0xffffffffu, valid, (slot | 1));
+        const bool v_partner = __shfl_xor_sync(0xffffffffu, (int)valid, 1) != 0;
+        const bool v_e = e ? v_partner : valid, v_o = e ? valid : v_partner;
         if (v_e || v_o) {
-          constexpr int HW = 3 * D / 64;  // halfwords per (lane, token pair) block
+          constexpr int NB = 6 * CW / 8;  // bytes per (lane, token pair, column half): 3 | 6
+          // bits of the even token inside three consecutive bytes of a field string (period 24 bits)
+          constexpr unsigned kEvenMask[3] = {0xC7u, 0x71u, 0x1Cu};
 #pragma unroll
           for (int gq = 0; gq < 4; ++gq) {
             const int gi = 4 * e + gq;
-            unsigned short hw16[HW];
+            unsigned long long acc = 0ull;
 #pragma unroll
-            for (int h = 0; h < HW; ++h) hw16[h] = 0;
-            unsigned long long acc = 0ull;  // fields stream through a 64-bit window, 16 bits out at a time
-            int nbits = 0, hout = 0;
-#pragma unroll
-            for (int c = 0; c < Lo::C; ++c) {
-              const unsigned f = ((ge[c] >> (3 * gi)) & 7u) | (((go[c] >> (3 * gi)) & 7u) << 3);
-              acc |= (unsigned long long)f << nbits;
-              nbits += 6;
-              if (nbits >= 16) {
-                hw16[hout++] = (unsigned short)acc;
-                acc >>= 16, nbits -= 16;
-              }
+            for (int c = 0; c < CW; ++c) {
+              const unsigned ce = ((e ? other[c] : mine[c]) >> (3 * gi)) & 7u, co = ((e ? mine[c] : other[c]) >> (3 * gi)) & 7u;
+              acc |= (unsigned long long)(ce | (co << 3)) << (6 * c);
             }
-            const unsigned short keep_mask = (v_e && v_o) ? 0u : 0xffffu;  // partial pair: read-modify-write
+            const int sb0 = (pp >> 2) * (6 * Lo::C / 8) + half * NB;  // byte of the lane's V string
 #pragma unroll
-            for (int h = 0; h < HW; ++h) {
-              const int hidx = (pp >> 2) * HW + h;
-              unsigned short* dst =
-                  reinterpret_cast<unsigned short*>(timg + word_offset(KCW, hidx >> 1, 4 * gi + (pp & 3))) + (hidx & 1);
-              if (keep_mask) {
-                // bits of the valid token inside this halfword: three of every six, phase by the bit offset 16 h
-                unsigned short m = 0;
-#pragma unroll
-                for (int bit = 0; bit < 16; ++bit) {
-                  const int fb = (16 * h + bit) % 6;
-                  if ((fb < 3) == v_e) m |= (unsigned short)(1u << bit);
-                }
-                *dst = (unsigned short)((*dst & ~m) | (hw16[h] & m));
-              } else {
-                *dst = hw16[h];
+            for (int k = 0; k < NB; ++k) {
+              unsigned char* dst = timg + sec_byte(KCW, 4 * gi + (pp & 3), sb0 + k);
+              const unsigned char nb = (unsigned char)(acc >> (8 * k));
+              if (v_e && v_o) {
+                *dst = nb;
+              } else {  // partial pair: keep the other token's bits
+                const unsigned char m = (unsigned char)(v_e ? kEvenMask[k % 3] : ~kEvenMask[k % 3]);
+                *dst = (unsigned char)((*dst & ~m) | (nb & m));
               }
             }
           }
@@ -537,7 +595,7 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
     __syncthreads();
     {
       constexpr int kOwn = kKey ? Cfg::kImgK : Cfg::kImgV;
-      for (int idx = tid; idx < 4 * (kOwn / 16); idx += kBlk) {
+      for (int idx = tid; idx < 4 * (kOwn / 16); idx += kThreads) {
         const int t4 = idx / (kOwn / 16), q = idx % (kOwn / 16);
         if (tile_cover(t4) == 0) continue;
         unsigned char* tg = stream + (size_t)(blk * 4 + t4) * Lo::kTileBytes;
@@ -557,11 +615,13 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
   }
 }
 
+// grid = (2 x block groups, batch x heads): key and value CTAs alternate along x, so that every SM holds a mix of the
+// two (the value CTAs are short and fill the issue slots the key CTAs leave idle)
 template <int D, typename T>
-__global__ void __launch_bounds__(kBlk) quantize_pack_tc_kernel(QuantArgs a, int blocks_per_cta) {
+__global__ void __launch_bounds__(kThreads, D == 64 ? 3 : 1) quantize_pack_tc_kernel(QuantArgs a, int blocks_per_cta) {
   extern __shared__ __align__(1024) unsigned char smem_dyn[];
-  if (blockIdx.z == 0) quantize_pack_tc_body<D, T, true>(a, blocks_per_cta, smem_dyn);
-  else quantize_pack_tc_body<D, T, false>(a, blocks_per_cta, smem_dyn);
+  if ((blockIdx.x & 1) == 0) quantize_pack_tc_body<D, T, true>(a, blocks_per_cta, (int)blockIdx.x >> 1, smem_dyn);
+  else quantize_pack_tc_body<D, T, false>(a, blocks_per_cta, (int)blockIdx.x >> 1, smem_dyn);
 }
 
 template <int D, typename T>
@@ -573,10 +633,11 @@ cudaError_t launch_quant_tc_t(const QuantArgs& a, int num_sms, cudaStream_t st) 
   const long want = 4L * num_sms;  // CTAs per operand: enough to balance the SMs, few enough to amortise the matrices
   int bpc = (int)(((long)nblk * BH + want - 1) / want);
   bpc = bpc < 1 ? 1 : (bpc > 16 ? 16 : bpc);
-  dim3 grid((nblk + bpc - 1) / bpc, BH, 2);  // z: keys | values
+  if (debug_quantize_knob() >= 16) bpc = debug_quantize_knob() - 16;  // SWEEP ONLY
+  dim3 grid(2 * ((nblk + bpc - 1) / bpc), BH);  // x: (block group, keys | values)
   cudaError_t e = cudaFuncSetAttribute(quantize_pack_tc_kernel<D, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
-  quantize_pack_tc_kernel<D, T><<<grid, kBlk, smem, st>>>(a, bpc);
+  quantize_pack_tc_kernel<D, T><<<grid, kThreads, smem, st>>>(a, bpc);
   count_launch();
   return cudaGetLastError();
 }
