@@ -207,7 +207,6 @@ cudaError_t launch_import(const CacheGeom& g, const CacheView& cv, int layer, in
                           cudaStream_t st);
 
 void debug_set_quantize_fp32(int on);
-int debug_quantize_knob();
 
 // ---- launch bookkeeping ---------------------------------------------------------------------------------
 void count_launch(int n = 1);

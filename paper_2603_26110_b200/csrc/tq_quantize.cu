@@ -18,7 +18,6 @@ namespace tq {
 
 static std::atomic<int> g_debug_quantize_fp32{0};
 void debug_set_quantize_fp32(int on) { g_debug_quantize_fp32.store(on, std::memory_order_relaxed); }
-int debug_quantize_knob() { return g_debug_quantize_fp32.load(std::memory_order_relaxed); }
 
 
 __device__ __forceinline__ int swz(int k) { return ((k >> 1) * 4) & 31; }
@@ -305,7 +304,7 @@ cudaError_t launch_quantize_pack(const QuantArgs& a, int D, tq_dtype dt, int num
   }
   // the tensor-core kernel (tq_quantize_tc.cu) is the product path; tq_debug_set_quantize_impl(1) selects the CUDA-core
   // kernel of this file (kept as a cross-check)
-  const bool force_fp32 = g_debug_quantize_fp32.load(std::memory_order_relaxed) == 1;
+  const bool force_fp32 = g_debug_quantize_fp32.load(std::memory_order_relaxed) != 0;
 #ifndef TQ_NO_TC_QUANTIZE
   if (!force_fp32) return launch_quantize_pack_tc(a, D, dt, num_sms, st);
 #endif

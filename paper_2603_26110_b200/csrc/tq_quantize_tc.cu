@@ -4,7 +4,7 @@
 // form of BASELINE.json:north_star), but the three rotations y = PI_K x', S r, PI_V v — a dense
 // (tokens x d) x (d x d) contraction — run as tcgen05.mma with the accumulators in tensor memory:
 //   * a CTA of 256 threads owns 128-token blocks of one (batch, head): UMMA M = 128 tokens, N = d outputs, K = 16;
-//     keys (RoPE, PI_K, then S on the residual) and values (PI_V) run as separate CTAs (alternating along blockIdx.x);
+//     keys (RoPE, PI_K, then S on the residual) and values (PI_V) run as separate CTAs (blockIdx.z);
 //   * operands are fp16 in shared memory in the canonical K-major no-swizzle layout (8 x 8 core matrices);
 //     fp32 accuracy comes from two-term splits a = a_hi + a_lo (each product exact in the fp32 accumulator):
 //     D = A_hi B_hi + A_lo B_hi + A_hi B_lo.  Power-of-two scalings keep every split away from the fp16 range
@@ -615,13 +615,13 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
   }
 }
 
-// grid = (2 x block groups, batch x heads): key and value CTAs alternate along x, so that every SM holds a mix of the
-// two (the value CTAs are short and fill the issue slots the key CTAs leave idle)
+// grid = (block groups, batch x heads, keys | values): the key CTAs (the long ones) are dispatched first and the value
+// CTAs fill in behind them (measured: alternating key and value CTAs along x is 8 % slower at configs[2])
 template <int D, typename T>
 __global__ void __launch_bounds__(kThreads, D == 64 ? 3 : 1) quantize_pack_tc_kernel(QuantArgs a, int blocks_per_cta) {
   extern __shared__ __align__(1024) unsigned char smem_dyn[];
-  if ((blockIdx.x & 1) == 0) quantize_pack_tc_body<D, T, true>(a, blocks_per_cta, (int)blockIdx.x >> 1, smem_dyn);
-  else quantize_pack_tc_body<D, T, false>(a, blocks_per_cta, (int)blockIdx.x >> 1, smem_dyn);
+  if (blockIdx.z == 0) quantize_pack_tc_body<D, T, true>(a, blocks_per_cta, (int)blockIdx.x, smem_dyn);
+  else quantize_pack_tc_body<D, T, false>(a, blocks_per_cta, (int)blockIdx.x, smem_dyn);
 }
 
 template <int D, typename T>
@@ -633,8 +633,7 @@ cudaError_t launch_quant_tc_t(const QuantArgs& a, int num_sms, cudaStream_t st) 
   const long want = 4L * num_sms;  // CTAs per operand: enough to balance the SMs, few enough to amortise the matrices
   int bpc = (int)(((long)nblk * BH + want - 1) / want);
   bpc = bpc < 1 ? 1 : (bpc > 16 ? 16 : bpc);
-  if (debug_quantize_knob() >= 16) bpc = debug_quantize_knob() - 16;  // SWEEP ONLY
-  dim3 grid(2 * ((nblk + bpc - 1) / bpc), BH);  // x: (block group, keys | values)
+  dim3 grid((nblk + bpc - 1) / bpc, BH, 2);  // z: keys | values
   cudaError_t e = cudaFuncSetAttribute(quantize_pack_tc_kernel<D, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
   quantize_pack_tc_kernel<D, T><<<grid, kThreads, smem, st>>>(a, bpc);
