@@ -130,6 +130,15 @@ def layer_activations(w: Workload, layer: int, n_tokens: int | None = None, stre
     return out[0], out[1]
 
 
+def layer_values_cold(w: Workload, layer: int, n_tokens: int | None = None):
+    """Values of one layer as the paper describes them ("substantially colder ... kurtosis near 3.0"):
+    plain N(0,1) per channel, no outlier channels, [B,H,T,d] in the workload dtype.  Used by the dual-LUT / shared-LUT
+    ablation rows, where K and V must follow different distributions."""
+    T = w.seq if n_tokens is None else n_tokens
+    rng = _rng(w, 500_000 + layer)
+    return rng.standard_normal((w.batch, w.n_heads, T, w.head_dim)).astype(_np_dtype(w))
+
+
 def step_tokens(w: Workload, layer: int, step: int):
     """(q, k_new, v_new) of decode step `step` for one layer: each [B,H,d] in the workload dtype."""
     B, H, d = w.batch, w.n_heads, w.head_dim
