@@ -15,6 +15,7 @@
  *                              as BASELINE.json:north_star requires (reading D2)
  *   packing                    PAPER.md:199-213 (8 codes at shifts 0,3,..,21), 3 bytes per 8 codes (D5)
  *   decode                     PAPER.md:118-124 and Algorithm 1, two-pass exact softmax
+ *   paper-literal Eq. 6-7 mode PAPER.md:166-179 as printed (tqo_quantize_vector_literal / _pack_literal)
  *
  * Pins (tests/test_oracle_*.py): every function below is checked against something other than itself —
  * closed forms, textbook tables, numpy library routines, brute force, Monte-Carlo.  Parity unpinned: none
@@ -279,6 +280,84 @@ void tqo_quantize_pack(int B, int H, int T, int d, int m, double base, int layou
         }
         near_v[(size_t)idx * d + i] = nr;
       }
+  }
+}
+
+/* ---- paper-literal residual correction, Eq. 6-7 as printed ---------
+ * The paper stores s = sign(x - x^) per coordinate (Eq. 6) and reconstructs x~ = x^ + s e-bar with ONE pre-calibrated
+ * scalar e-bar per head (Eq. 7); its LUT is calibrated on the rotated activations themselves (no norm is stored,
+ * PAPER.md:159-164) and V is not rotated (PAPER.md:157, 162 — PI_V = I is passed as data).  In the canonical planes
+ * this is: codes on y = PI x' (no normalisation), norm plane = 1.0, bits_j = [(S e)_j >= 0] with e = y - lut[code]
+ * (S = I as data gives Eq. 6's sign(e_j)), and the rnorm plane = binary16(e-bar m sqrt(2/pi)), so that the decode
+ * correction  sqrt(pi/2)/m * rnorm * <S q'', sigma>  of tqo_decode_attn equals  e-bar <q'', s>  — Eq. 7 contracted
+ * with the query (Algorithm 1 line 6).  y_out (optional): the coded coordinates.                     */
+void tqo_quantize_vector_literal(const double *x, int d, int m, int is_key, double pos, double base, int layout,
+                                 const float *Pi, const float *lut8, const float *S, double ebar, uint8_t *codes,
+                                 uint8_t *bits, uint16_t *norm_h, uint16_t *rnorm_h, double *y_out) {
+  double xr[256], y[256], e[256], se[256];
+  if (is_key)
+    tqo_rope(x, d, pos, base, layout, xr);
+  else
+    memcpy(xr, x, sizeof(double) * (size_t)d);
+  matvec_f32(Pi, d, d, xr, y);
+  *norm_h = tqo_f64_to_f16(1.0);
+  for (int i = 0; i < d; ++i) codes[i] = (uint8_t)tqo_code(y[i], lut8); /* Eq. 5 on the activation itself */
+  if (y_out) memcpy(y_out, y, sizeof(double) * (size_t)d);
+  if (is_key) {
+    for (int i = 0; i < d; ++i) e[i] = y[i] - (double)lut8[codes[i]];  /* e = x - x^                 (Eq. 6) */
+    matvec_f32(S, m, d, e, se);
+    for (int j = 0; j < m; ++j) bits[j] = (uint8_t)(se[j] >= 0.0 ? 1 : 0);
+    *rnorm_h = tqo_f64_to_f16(ebar * (double)m * sqrt(2.0 / TQO_PI)); /* e-bar, in the units of the rnorm plane */
+  }
+}
+
+/* Layer form of the above; same conventions as tqo_quantize_pack.  ebar_k: [H].  near_k / near_v: 1 where the coded
+ * coordinate lies within near_eps * max(1, |y|_2) of a decision threshold (the band scales with the vector here,
+ * because the coordinates are not normalised).                                                                  */
+void tqo_quantize_pack_literal(int B, int H, int T, int d, int m, double base, int layout, int start_pos,
+                               const float *k, const float *v, const float *pi_k, const float *pi_v,
+                               const float *lut_k, const float *lut_v, const float *S, const float *ebar_k,
+                               uint8_t *k_codes, uint8_t *k_signs, uint16_t *k_norm, uint16_t *k_rnorm,
+                               uint8_t *v_codes, uint16_t *v_norm, double near_eps, uint8_t *near_k, uint8_t *near_v) {
+  const int cb = 3 * d / 8, sb = m / 8;
+  long total = (long)B * H * T;
+#pragma omp parallel for schedule(static)
+  for (long idx = 0; idx < total; ++idx) {
+    int t = (int)(idx % T);
+    int h = (int)((idx / T) % H);
+    double x[256], y[256];
+    uint8_t codes[256], bits[256];
+    uint16_t nh = 0, rh = 0;
+    for (int side = 0; side < 2; ++side) {
+      const float *xp = (side == 0 ? k : v) + (size_t)idx * d;
+      const float *lu = (side == 0 ? lut_k : lut_v) + (size_t)h * 8;
+      for (int i = 0; i < d; ++i) x[i] = (double)xp[i];
+      tqo_quantize_vector_literal(x, d, m, side == 0, (double)(start_pos + t), base, layout,
+                                  (side == 0 ? pi_k : pi_v) + (size_t)h * d * d, lu, S, side == 0 ? (double)ebar_k[h] : 0.0,
+                                  codes, bits, &nh, &rh, y);
+      tqo_pack_codes(codes, d, (side == 0 ? k_codes : v_codes) + (size_t)idx * cb);
+      if (side == 0) {
+        tqo_pack_bits(bits, m, k_signs + (size_t)idx * sb);
+        k_norm[idx] = nh;
+        k_rnorm[idx] = rh;
+      } else {
+        v_norm[idx] = nh;
+      }
+      uint8_t *near = side == 0 ? near_k : near_v;
+      if (near) {
+        double n2 = 0.0;
+        for (int i = 0; i < d; ++i) n2 += y[i] * y[i];
+        double band = near_eps * fmax(1.0, sqrt(n2));
+        for (int i = 0; i < d; ++i) {
+          uint8_t nr = 0;
+          for (int q = 0; q < 7; ++q) {
+            float th = 0.5f * (lu[q] + lu[q + 1]);
+            if (fabs(y[i] - (double)th) < band) nr = 1;
+          }
+          near[(size_t)idx * d + i] = nr;
+        }
+      }
+    }
   }
 }
 

@@ -240,6 +240,46 @@ def quantize_pack(k, v, pi_k, pi_v, lut_k, lut_v, S, start_pos: int = 0, base: f
     return out
 
 
+def quantize_vector_literal(x, is_key: bool, pos: float, Pi, lut8, S, ebar: float, base: float = 10000.0, layout: int = 0):
+    """Paper-literal Eq. 6-7 mode, one vector -> dict(codes[d], bits[m], norm_h, rnorm_h, y[d])."""
+    x = _f64(x)
+    d = x.shape[0]
+    S = _f32(S)
+    m = S.shape[0]
+    codes, bits = np.zeros(d, np.uint8), np.zeros(m, np.uint8)
+    nh, rh = C.c_uint16(0), C.c_uint16(0)
+    y = np.zeros(d, np.float64)
+    lib().tqo_quantize_vector_literal(_p(x), C.c_int(d), C.c_int(m), C.c_int(1 if is_key else 0), C.c_double(pos),
+                                      C.c_double(base), C.c_int(layout), _p(_f32(Pi)), _p(_f32(lut8)), _p(S),
+                                      C.c_double(ebar), _p(codes), _p(bits), C.byref(nh), C.byref(rh), _p(y))
+    return dict(codes=codes, bits=bits, norm_h=nh.value, rnorm_h=rh.value, y=y)
+
+
+def quantize_pack_literal(k, v, pi_k, pi_v, lut_k, lut_v, S, ebar_k, start_pos: int = 0, base: float = 10000.0,
+                          layout: int = 0, near_eps: float | None = None) -> Canonical:
+    """Layer form of the paper-literal mode; ebar_k: [H].  Same planes as quantize_pack."""
+    k = _f32(k)
+    v = _f32(v)
+    B, H, T, d = k.shape
+    S = _f32(S)
+    m = S.shape[0]
+    pi_k, pi_v, lut_k, lut_v, ebar_k = _f32(pi_k), _f32(pi_v), _f32(lut_k), _f32(lut_v), _f32(ebar_k)
+    assert pi_k.shape == (H, d, d) and lut_k.shape == (H, 8) and ebar_k.shape == (H,)
+    cb, sb = 3 * d // 8, m // 8
+    out = Canonical(np.zeros((B, H, T, cb), np.uint8), np.zeros((B, H, T, sb), np.uint8),
+                    np.zeros((B, H, T), np.uint16), np.zeros((B, H, T), np.uint16),
+                    np.zeros((B, H, T, cb), np.uint8), np.zeros((B, H, T), np.uint16))
+    if near_eps is not None:
+        out.near_k = np.zeros((B, H, T, d), np.uint8)
+        out.near_v = np.zeros((B, H, T, d), np.uint8)
+    lib().tqo_quantize_pack_literal(C.c_int(B), C.c_int(H), C.c_int(T), C.c_int(d), C.c_int(m), C.c_double(base),
+                                    C.c_int(layout), C.c_int(start_pos), _p(k), _p(v), _p(pi_k), _p(pi_v), _p(lut_k),
+                                    _p(lut_v), _p(S), _p(ebar_k), _p(out.k_codes), _p(out.k_signs), _p(out.k_norm),
+                                    _p(out.k_rnorm), _p(out.v_codes), _p(out.v_norm), C.c_double(near_eps or 0.0),
+                                    _p(out.near_k), _p(out.near_v))
+    return out
+
+
 def decode_attn(q, q_pos, seq_len, pi_k, pi_v, lut_k, lut_v, S, cache: Canonical, base: float = 10000.0,
                 layout: int = 0, use_qjl: bool = True):
     """q: [B,H,d]; q_pos, seq_len: [B] int32 -> out [B,H,d] fp64."""

@@ -199,3 +199,90 @@ def test_workloads_are_seeded_and_shaped():
     assert np.abs(pk[1, 3].astype(np.float64).T @ pk[1, 3] - np.eye(64)).max() < 1e-6
     assert W.CONFIGS["cfg0_tiny"].fixed_outliers == (3, 17)
     assert W.CONFIGS["cfg4_15b_heads"].head_dim == 128 and W.CONFIGS["cfg3_long_splitk"].seq == 16384
+
+
+# ------------------------------------------------------------------------------------------------ paper-literal Eq. 6-7 mode
+def _literal_case(oracle, B=2, H=3, T=37, d=64, seed=11):
+    """Raw-scale activations (|y| is NOT 1), LUT on the activation scale, S = I and PI_V = I as the paper has them."""
+    rng = np.random.default_rng(seed)
+    pi_k = np.stack([W.orthogonal_from_gaussian(rng, d) for _ in range(H)])
+    pi_v = np.broadcast_to(np.eye(d, dtype=np.float32), (H, d, d)).copy()
+    S = np.eye(d, dtype=np.float32)
+    sig = np.array([0.7, 1.3, 2.1], np.float32)[:H]
+    lut_k = np.stack([oracle.lloyd_max_gauss(float(s), 8)[0] for s in sig]).astype(np.float32)
+    lut_v = np.stack([oracle.lloyd_max_gauss(float(1.5 * s), 8)[0] for s in sig]).astype(np.float32)
+    k = (rng.standard_normal((B, H, T, d)) * sig[None, :, None, None]).astype(np.float32)
+    v = (rng.standard_normal((B, H, T, d)) * 1.5 * sig[None, :, None, None]).astype(np.float32)
+    q = rng.standard_normal((B, H, d)).astype(np.float32)
+    ebar = np.array([0.21, 0.4, 0.66], np.float32)[:H]
+    return dict(pi_k=pi_k, pi_v=pi_v, S=S, lut_k=lut_k, lut_v=lut_v, k=k, v=v, q=q, ebar=ebar, sig=sig)
+
+
+def test_literal_mode_is_eq6_eq7_as_printed(oracle):
+    """PAPER.md:170-179.  Per vector: codes = nearest LUT entry of the rotated activation itself (no normalisation),
+    bits = sign(x - x^) (Eq. 6, S = I), norm plane = 1.0, rnorm plane decodes to e-bar m sqrt(2/pi).  And Eq. 7's claim
+    "reducing the expected squared error by approximately e-bar^2 per element" is an identity when e-bar = mean |e|:
+    mean (x - x~)^2 = mean e^2 - e-bar^2, checked on the reconstruction built from the oracle's own codes and bits."""
+    c = _literal_case(oracle)
+    d = 64
+    rng = np.random.default_rng(5)
+    x = rng.standard_normal(d) * 1.3
+    h, pos = 1, 9
+    out = oracle.quantize_vector_literal(x, True, pos, c["pi_k"][h], c["lut_k"][h], c["S"], float(c["ebar"][h]))
+    y = c["pi_k"][h].astype(np.float64) @ np_rope(x, pos)
+    assert np.allclose(out["y"], y, atol=1e-12)
+    lut = c["lut_k"][h].astype(np.float64)
+    want_codes = np.abs(y[:, None] - lut[None, :]).argmin(1)
+    assert np.array_equal(out["codes"], want_codes)
+    assert np.array_equal(out["bits"], (y - lut[want_codes] >= 0).astype(np.uint8))            # Eq. 6
+    assert oracle.f16_bits_to_f64(out["norm_h"]) == 1.0
+    g = oracle.f16_bits_to_f64(out["rnorm_h"])
+    assert abs(g / (float(c["ebar"][h]) * d * math.sqrt(2 / math.pi)) - 1) <= 2.0 ** -11        # binary16 rounding only
+    # values: no RoPE, no sketch, not normalised
+    outv = oracle.quantize_vector_literal(x, False, pos, c["pi_v"][h], c["lut_v"][h], c["S"], 0.0)
+    lv = c["lut_v"][h].astype(np.float64)
+    assert np.array_equal(outv["codes"], np.abs(x[:, None] - lv[None, :]).argmin(1))
+    # Eq. 7 error identity over many vectors, e-bar := the sample mean of |e|
+    X = rng.standard_normal((400, d)) * float(c["sig"][h])
+    E, S_, XH = [], [], []
+    for xv in X:
+        o = oracle.quantize_vector_literal(xv, True, 0.0, c["pi_k"][h], c["lut_k"][h], c["S"], 0.0)
+        E.append(o["y"] - lut[o["codes"]]), S_.append(2.0 * o["bits"] - 1.0), XH.append(lut[o["codes"]])
+    E, S_ = np.array(E), np.array(S_)
+    ebar = np.abs(E).mean()
+    assert abs(np.mean((E - S_ * ebar) ** 2) - (np.mean(E ** 2) - ebar ** 2)) < 1e-12
+    assert np.mean((E - S_ * ebar) ** 2) < np.mean(E ** 2)
+
+
+def test_literal_pack_indexing_and_decode_equals_attention_over_eq7_keys(oracle):
+    """(a) tqo_quantize_pack_literal == the per-vector call with THAT head's PI / LUT / e-bar at position start_pos + t.
+    (b) tqo_decode_attn over the literal planes == brute-force softmax attention over the Eq. 7 reconstruction
+    k~ = lut_K[codes] + s e-bar (rotated back by PI_K^T) and v^ = lut_V[codes] (Algorithm 1 lines 6-11 with S = I)."""
+    c = _literal_case(oracle)
+    B, H, T, d = c["k"].shape
+    sp = 5
+    can = oracle.quantize_pack_literal(c["k"], c["v"], c["pi_k"], c["pi_v"], c["lut_k"], c["lut_v"], c["S"], c["ebar"], start_pos=sp)
+    for (b, h, t) in [(0, 0, 0), (1, 2, 36), (0, 1, 17)]:
+        o = oracle.quantize_vector_literal(c["k"][b, h, t], True, sp + t, c["pi_k"][h], c["lut_k"][h], c["S"], float(c["ebar"][h]))
+        assert np.array_equal(oracle.unpack_codes(can.k_codes[b, h, t], d), o["codes"])
+        assert np.array_equal(oracle.unpack_bits(can.k_signs[b, h, t], d), o["bits"])
+        assert can.k_norm[b, h, t] == o["norm_h"] and can.k_rnorm[b, h, t] == o["rnorm_h"]
+        ov = oracle.quantize_vector_literal(c["v"][b, h, t], False, 0.0, c["pi_v"][h], c["lut_v"][h], c["S"], 0.0)
+        assert np.array_equal(oracle.unpack_codes(can.v_codes[b, h, t], d), ov["codes"]) and can.v_norm[b, h, t] == ov["norm_h"]
+    # (b) decode: the cache holds positions 0..T-1 when start_pos = 0
+    can = oracle.quantize_pack_literal(c["k"], c["v"], c["pi_k"], c["pi_v"], c["lut_k"], c["lut_v"], c["S"], c["ebar"])
+    sl = np.full(B, T, np.int32)
+    got = oracle.decode_attn(c["q"], sl - 1, sl, c["pi_k"], c["pi_v"], c["lut_k"], c["lut_v"], c["S"], can)
+    for b in range(B):
+        for h in range(H):
+            lk, lv = c["lut_k"][h].astype(np.float64), c["lut_v"][h].astype(np.float64)
+            eb = oracle.f16_bits_to_f64(int(can.k_rnorm[b, h, 0])) * math.sqrt(math.pi / 2) / d  # e-bar as stored
+            kt = np.stack([lk[oracle.unpack_codes(can.k_codes[b, h, t], d)] + (2.0 * oracle.unpack_bits(can.k_signs[b, h, t], d) - 1.0) * eb
+                           for t in range(T)])                                   # Eq. 7, rotated basis
+            vh = np.stack([lv[oracle.unpack_codes(can.v_codes[b, h, t], d)] for t in range(T)])
+            q2 = c["pi_k"][h].astype(np.float64) @ np_rope(c["q"][b, h].astype(np.float64), T - 1)
+            s = kt @ q2 / math.sqrt(d)
+            p = np.exp(s - s.max())
+            p /= p.sum()
+            want = c["pi_v"][h].astype(np.float64).T @ (p @ vh)
+            assert np.allclose(got[b, h], want, atol=1e-9)
