@@ -82,6 +82,8 @@ typedef struct {
   float rope_base;     /* theta_g = rope_base^(-2g/d); 10000 in BASELINE.json:configs[0]                */
   int32_t rope_layout; /* 0 = interleaved pairs (2g, 2g+1) [PAPER.md:102, Eq. 2]; 1 = half-split (g, g+d/2) */
   int32_t v_qjl;       /* 0 = K-only residual sketch (reading D3); 1 is TQ_ERR_UNSUPPORTED     */
+  int32_t residual_mode; /* 0 = north_star form: unit vector coded, |y| and |r| stored per token, bits = sign(S r);
+                            1 = the paper's literal Eq. 6-7 [PAPER.md:170-179]: see "Paper-literal mode" below   */
 } tq_shape;
 
 /* Calibration arrays.  HOST pointers for tq_calibrate_host, DEVICE pointers for every other call.     */
@@ -92,7 +94,21 @@ typedef struct {
   float *lut_v;   /* [L][H][8]     same for values                                                      */
   float *S;       /* [m][d]        QJL sketch matrix, shared by all layers and heads                    */
   float *rope_cs; /* [max_seq][d/2][2]  (cos, sin)(p * theta_g), evaluated in fp64 and rounded to fp32  */
+  float *ebar_k;  /* [L][H]  residual_mode 1 only (else may be NULL): the pre-calibrated mean absolute residual of the
+                     keys of that head, the scalar of Eq. 7 [PAPER.md:176-179]                                     */
 } tq_params;
+
+/* Paper-literal mode (tq_shape.residual_mode = 1).  The paper's own residual correction
+ * [PAPER.md:170-179, Eq. 6-7] stores s = sign(x - x^) per coordinate and reconstructs x~ = x^ + s e-bar with one
+ * pre-calibrated scalar e-bar per head; its LUTs are calibrated on the raw rotated activations (no norm is stored) and
+ * values are not rotated [PAPER.md:157-162].  In this mode tq_quantize_pack / tq_append
+ *   - do NOT normalise: codes are taken on y = PI x' itself (LUT entries live on the scale of the activations), and the
+ *     stored binary16 norm is exactly 1.0 for keys and values;
+ *   - take the residual e = y - lut[code] and store bits_j = [(S e)_j >= 0];
+ *   - store, in place of |r|, the binary16 rounding (from fp64) of  e-bar[layer][head] * m * sqrt(2/pi),
+ * so that the decode kernel's correction term  sqrt(pi/2)/m * (stored) * <S q'', sigma>  equals  e-bar <S q'', sigma>.
+ * With S = I and PI_V = I passed as data (what tq_calibrate_host emits in this mode) this is Eq. 6-7 word for word:
+ * bits = sign(e), logit = <q'', lut[codes] + s e-bar> / sqrt(d).  tq_decode_attn itself is the same in both modes.   */
 
 /* Packed cache: one caller-allocated DEVICE buffer of tq_cache_bytes() bytes, zero-filled by the caller
  * before first use.  It holds a header (seq_len[L][B], append arrival counters, a sticky status word)
@@ -126,6 +142,9 @@ size_t tq_canonical_plane_bytes(const tq_shape *shape, int32_t plane, int32_t n_
  *          diag(R) > 0) [BASELINE.json:configs[0]]; LUTs = Lloyd-Max fixed point for N(0, 1/d) [configs[0]].
  *          k_samples / v_samples may be NULL.
  * S: seeded i.i.d. N(0,1).  rope_cs: fp64 evaluation rounded to fp32.
+ * residual_mode 1 (paper-literal): S = I, PI_V = I; the LUTs are fitted to the raw rotated coordinates (mode 0) or stay
+ * the N(0, 1/d) tables (mode 1); ebar_k (required) = the mean absolute residual of the keys under lut_k (mode 0: over
+ * the samples; mode 1: the Gaussian integral).
  * k_samples: [L][H][n_samples][d] post-RoPE keys; v_samples: same shape, values.                        */
 int tq_calibrate_host(const tq_shape *shape, int32_t mode, const float *k_samples, const float *v_samples,
                       int64_t n_samples, uint64_t seed, tq_params *out_host);

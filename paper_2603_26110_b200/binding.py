@@ -37,11 +37,11 @@ class TqError(RuntimeError):
 class TqShape(C.Structure):
     _fields_ = [("n_layers", C.c_int32), ("batch", C.c_int32), ("n_heads", C.c_int32), ("head_dim", C.c_int32),
                 ("qjl_dim", C.c_int32), ("max_seq", C.c_int32), ("rope_base", C.c_float), ("rope_layout", C.c_int32),
-                ("v_qjl", C.c_int32)]
+                ("v_qjl", C.c_int32), ("residual_mode", C.c_int32)]
 
 
 class TqParams(C.Structure):
-    _fields_ = [(n, C.c_void_p) for n in ("pi_k", "pi_v", "lut_k", "lut_v", "S", "rope_cs")]
+    _fields_ = [(n, C.c_void_p) for n in ("pi_k", "pi_v", "lut_k", "lut_v", "S", "rope_cs", "ebar_k")]
 
 
 class TqCache(C.Structure):
@@ -84,9 +84,9 @@ def _check(rc: int, where: str):
 
 
 def make_shape(n_layers, batch, n_heads, head_dim, max_seq, rope_base=10000.0, rope_layout=0, qjl_dim=None,
-               v_qjl=0) -> TqShape:
+               v_qjl=0, residual_mode=0) -> TqShape:
     return TqShape(n_layers, batch, n_heads, head_dim, head_dim if qjl_dim is None else qjl_dim, max_seq, rope_base,
-                   rope_layout, v_qjl)
+                   rope_layout, v_qjl, residual_mode)
 
 
 def _ptr(t):
@@ -154,7 +154,10 @@ def tq_calibrate_host(shape: TqShape, mode: int, k_samples=None, v_samples=None,
     out = dict(pi_k=np.zeros((L, H, d, d), np.float32), pi_v=np.zeros((L, H, d, d), np.float32),
                lut_k=np.zeros((L, H, 8), np.float32), lut_v=np.zeros((L, H, 8), np.float32),
                S=np.zeros((m, d), np.float32), rope_cs=np.zeros((shape.max_seq, d // 2, 2), np.float32))
-    p = TqParams(*[C.c_void_p(out[n].ctypes.data) for n in ("pi_k", "pi_v", "lut_k", "lut_v", "S", "rope_cs")])
+    if shape.residual_mode == 1:
+        out["ebar_k"] = np.zeros((L, H), np.float32)
+    p = TqParams(*[C.c_void_p(out[n].ctypes.data) if n in out else None
+                   for n in ("pi_k", "pi_v", "lut_k", "lut_v", "S", "rope_cs", "ebar_k")])
     n_samples = 0
     if k_samples is not None:
         k_samples = np.ascontiguousarray(k_samples, np.float32)
@@ -173,9 +176,10 @@ class Params:
     def __init__(self, arrays: dict, device="cuda"):
         import torch
 
+        names = ("pi_k", "pi_v", "lut_k", "lut_v", "S", "rope_cs", "ebar_k")  # ebar_k: paper-literal mode only
         self.t = {n: torch.as_tensor(np.ascontiguousarray(arrays[n], np.float32)).to(device).contiguous()
-                  for n in ("pi_k", "pi_v", "lut_k", "lut_v", "S", "rope_cs")}
-        self.c = TqParams(*[C.c_void_p(self.t[n].data_ptr()) for n in ("pi_k", "pi_v", "lut_k", "lut_v", "S", "rope_cs")])
+                  for n in names if arrays.get(n) is not None}
+        self.c = TqParams(*[C.c_void_p(self.t[n].data_ptr()) if n in self.t else None for n in names])
 
 
 class Cache:

@@ -59,6 +59,7 @@ static int check_shape(const tq_shape* s, CacheGeom* g) {
   if (s->n_layers <= 0 || s->batch <= 0 || s->n_heads <= 0 || s->max_seq <= 0 || !(s->rope_base > 0.f))
     return TQ_ERR_INVALID_ARG;
   if (s->rope_layout != 0 && s->rope_layout != 1) return TQ_ERR_INVALID_ARG;
+  if (s->residual_mode != 0 && s->residual_mode != 1) return TQ_ERR_INVALID_ARG;
   if ((s->head_dim != 64 && s->head_dim != 128) || s->qjl_dim != s->head_dim || s->v_qjl != 0) return TQ_ERR_UNSUPPORTED;
   if (!make_geom(s, g)) return TQ_ERR_INVALID_ARG;
   return TQ_OK;
@@ -66,8 +67,9 @@ static int check_shape(const tq_shape* s, CacheGeom* g) {
 
 static bool aligned16(const void* p) { return p && ((uintptr_t)p & 15u) == 0; }
 
-static int check_params(const tq_params* p) {
+static int check_params(const tq_params* p, const tq_shape* s) {
   if (!p) return TQ_ERR_INVALID_ARG;
+  if (s->residual_mode == 1 && (!p->ebar_k || ((uintptr_t)p->ebar_k & 3u))) return TQ_ERR_INVALID_ARG;
   if (!aligned16(p->pi_k) || !aligned16(p->pi_v) || !aligned16(p->lut_k) || !aligned16(p->lut_v) || !aligned16(p->S) ||
       !aligned16(p->rope_cs))
     return TQ_ERR_INVALID_ARG;
@@ -142,7 +144,7 @@ int tq_quantize_pack(const tq_shape* shape, const tq_params* dev, tq_cache* cach
   CacheGeom g;
   int rc = check_shape(shape, &g);
   if (rc != TQ_OK) return rc;
-  if ((rc = check_params(dev)) != TQ_OK) return rc;
+  if ((rc = check_params(dev, shape)) != TQ_OK) return rc;
   if (!cache || !cache->data || ((uintptr_t)cache->data & 255u)) return TQ_ERR_INVALID_ARG;
   if (layer < 0 || layer >= g.L || n_tokens < 0 || start_pos < 0) return TQ_ERR_INVALID_ARG;
   if (dt != TQ_F16 && dt != TQ_F32) return TQ_ERR_INVALID_ARG;
@@ -165,6 +167,8 @@ int tq_quantize_pack(const tq_shape* shape, const tq_params* dev, tq_cache* cach
   a.start_pos = start_pos;
   a.rope_layout = shape->rope_layout;
   a.tiles_per_cta = 1;
+  a.literal = shape->residual_mode == 1;
+  a.ebar_k = a.literal ? dev->ebar_k + (size_t)layer * g.H : nullptr;
   return launch_quantize_pack(a, g.D, dt, sms, (cudaStream_t)cuda_stream) == cudaSuccess ? TQ_OK : TQ_ERR_CUDA;
 }
 
@@ -177,7 +181,7 @@ static int run_decode(const tq_shape* shape, const tq_params* dev, const tq_cach
   CacheGeom g;
   int rc = check_shape(shape, &g);
   if (rc != TQ_OK) return rc;
-  if ((rc = check_params(dev)) != TQ_OK) return rc;
+  if ((rc = check_params(dev, shape)) != TQ_OK) return rc;
   if (!cache || !cache->data || ((uintptr_t)cache->data & 255u)) return TQ_ERR_INVALID_ARG;
   if (layer_begin < 0 || n_layers_call <= 0 || layer_begin + n_layers_call > g.L) return TQ_ERR_INVALID_ARG;
   if (dt != TQ_F16 && dt != TQ_F32) return TQ_ERR_INVALID_ARG;
@@ -222,6 +226,8 @@ static int run_decode(const tq_shape* shape, const tq_params* dev, const tq_cach
     a.chain_mode = 0;
     a.rope_layout = shape->rope_layout;
     a.dt = (int)dt;
+    a.literal = shape->residual_mode == 1;
+    a.ebar_k = a.literal ? dev->ebar_k : nullptr;
     const void* kc = k ? (const unsigned char*)k + u0 * g.D * esz : nullptr;
     const void* vc = v ? (const unsigned char*)v + u0 * g.D * esz : nullptr;
     if (!(g_profile_skip_prep && do_query && !do_append) &&
@@ -300,7 +306,7 @@ static int plan_model_step(const tq_shape* shape, const tq_params* dev, tq_cache
   CacheGeom& g = p->g;
   int rc = check_shape(shape, &g);
   if (rc != TQ_OK) return rc;
-  if ((rc = check_params(dev)) != TQ_OK) return rc;
+  if ((rc = check_params(dev, shape)) != TQ_OK) return rc;
   if (!cache || !cache->data || ((uintptr_t)cache->data & 255u)) return TQ_ERR_INVALID_ARG;
   if (layer_begin < 0 || n_layers_call <= 0 || layer_begin + n_layers_call > g.L) return TQ_ERR_INVALID_ARG;
   if (dt != TQ_F16 && dt != TQ_F32) return TQ_ERR_INVALID_ARG;
@@ -329,6 +335,8 @@ static int plan_model_step(const tq_shape* shape, const tq_params* dev, tq_cache
   a.layer_begin = layer_begin, a.n_layers_call = n_layers_call;
   a.nsplit = nsplit, a.per = (ntiles + nsplit - 1) / nsplit;
   a.chain_mode = 0, a.rope_layout = shape->rope_layout, a.dt = (int)dt;
+  a.literal = shape->residual_mode == 1;
+  a.ebar_k = a.literal ? dev->ebar_k : nullptr;
   return TQ_OK;
 }
 

@@ -216,6 +216,57 @@ void pooled_unit_coords(const float* X, int64_t n, int d, const float* pi, std::
   }
 }
 
+// raw rotated coordinates y = PI x of every sample (paper-literal mode: the LUT lives on the activation scale)
+void pooled_raw_coords(const float* X, int64_t n, int d, const float* pi, std::vector<double>& pool) {
+  pool.clear();
+  pool.reserve((size_t)n * d);
+  for (int64_t r = 0; r < n; ++r) {
+    const float* x = X + r * d;
+    for (int i = 0; i < d; ++i) {
+      double acc = 0.0;
+      for (int k = 0; k < d; ++k) acc += (double)pi[(size_t)i * d + k] * (double)x[k];
+      pool.push_back(acc);
+    }
+  }
+}
+
+int code_of(double u, const float* lut8) {
+  int c = 0;
+  for (int k = 0; k < 7; ++k) c += u > (double)(0.5f * (lut8[k] + lut8[k + 1])) ? 1 : 0;
+  return c;
+}
+
+// e-bar of Eq. 7 [PAPER.md:176-179]: mean |y - lut[code(y)]| over the samples
+double mean_abs_residual(const std::vector<double>& pool, const float* lut8) {
+  double acc = 0.0;
+  for (double y : pool) acc += std::fabs(y - (double)lut8[code_of(y, lut8)]);
+  return pool.empty() ? 0.0 : acc / (double)pool.size();
+}
+
+// the same for y ~ N(0, sigma^2): sum over the cells [a, b] around centroid c of  int |y - c| dN, with
+// int_p^q (y - c) dN = sigma (phi(p/sigma) - phi(q/sigma)) - c (Phi(q/sigma) - Phi(p/sigma))
+double mean_abs_residual_gauss(double sigma, const float* lut8) {
+  auto part = [&](double p, double q, double c) {  // p, q in units of sigma (may be +-inf)
+    const double pp = std::isinf(p) ? 0.0 : phi(p), pq = std::isinf(q) ? 0.0 : phi(q);
+    const double Pp = std::isinf(p) ? (p < 0 ? 0.0 : 1.0) : Phi(p), Pq = std::isinf(q) ? (q < 0 ? 0.0 : 1.0) : Phi(q);
+    return sigma * (pp - pq) - c * (Pq - Pp);
+  };
+  double acc = 0.0;
+  for (int k = 0; k < 8; ++k) {
+    const double c = lut8[k];
+    const double a = k == 0 ? -INFINITY : (double)(0.5f * (lut8[k - 1] + lut8[k])) / sigma;
+    const double b = k == 7 ? INFINITY : (double)(0.5f * (lut8[k] + lut8[k + 1])) / sigma;
+    const double cs = std::min(std::max(c / sigma, a), b);
+    acc += -part(a, cs, c) + part(cs, b, c);
+  }
+  return acc;
+}
+
+void set_identity(float* M, int d) {
+  for (int i = 0; i < d; ++i)
+    for (int k = 0; k < d; ++k) M[(size_t)i * d + k] = i == k ? 1.f : 0.f;
+}
+
 }  // namespace
 
 extern "C" int tq_calibrate_host(const tq_shape* shape, int32_t mode, const float* k_samples, const float* v_samples,
@@ -227,9 +278,13 @@ extern "C" int tq_calibrate_host(const tq_shape* shape, int32_t mode, const floa
   if (!out->pi_k || !out->pi_v || !out->lut_k || !out->lut_v || !out->S || !out->rope_cs) return TQ_ERR_INVALID_ARG;
   if (mode != 0 && mode != 1) return TQ_ERR_INVALID_ARG;
   if (mode == 0 && (!k_samples || !v_samples || n_samples < d)) return TQ_ERR_INVALID_ARG;
+  const bool literal = shape->residual_mode == 1;  // the paper's Eq. 6-7 as printed (include/tq.h "Paper-literal mode")
+  if (shape->residual_mode != 0 && shape->residual_mode != 1) return TQ_ERR_INVALID_ARG;
+  if (literal && !out->ebar_k) return TQ_ERR_INVALID_ARG;
 
   Rng rs(seed ^ 0x5151515151515151ull);
   for (size_t i = 0; i < (size_t)m * d; ++i) out->S[i] = (float)rs.normal();
+  if (literal) set_identity(out->S, d);  // Eq. 6: the sign of every residual coordinate
 
   for (int p = 0; p < shape->max_seq; ++p)
     for (int g = 0; g < d / 2; ++g) {
@@ -251,6 +306,10 @@ extern "C" int tq_calibrate_host(const tq_shape* shape, int32_t mode, const floa
       qr_q(g, d, q);
       for (size_t i = 0; i < (size_t)d * d; ++i) out->pi_v[(size_t)lh * d * d + i] = (float)q[i];
       for (int k = 0; k < 8; ++k) out->lut_k[(size_t)lh * 8 + k] = out->lut_v[(size_t)lh * 8 + k] = lut[k];
+      if (literal) {
+        set_identity(out->pi_v + (size_t)lh * d * d, d);  // values are not rotated
+        out->ebar_k[lh] = (float)mean_abs_residual_gauss(1.0 / std::sqrt((double)d), lut);
+      }
     }
     return TQ_OK;
   }
@@ -261,6 +320,15 @@ extern "C" int tq_calibrate_host(const tq_shape* shape, int32_t mode, const floa
     float* pk = out->pi_k + (size_t)lh * d * d;
     float* pv = out->pi_v + (size_t)lh * d * d;
     svd_rotation(xk, n_samples, d, pk);
+    if (literal) {  // LUTs on the raw (rotated) activations, values unrotated, e-bar over the key samples
+      set_identity(pv, d);
+      pooled_raw_coords(xk, n_samples, d, pk, pool);
+      lloyd_max_samples8(pool, out->lut_k + (size_t)lh * 8);
+      out->ebar_k[lh] = (float)mean_abs_residual(pool, out->lut_k + (size_t)lh * 8);
+      pooled_raw_coords(xv, n_samples, d, pv, pool);
+      lloyd_max_samples8(pool, out->lut_v + (size_t)lh * 8);
+      continue;
+    }
     svd_rotation(xv, n_samples, d, pv);
     pooled_unit_coords(xk, n_samples, d, pk, pool);
     if (pool.size() < 8) return TQ_ERR_INVALID_ARG;

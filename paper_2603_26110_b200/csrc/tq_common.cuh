@@ -168,6 +168,9 @@ struct QuantArgs {
   const float* S;        // [D][D]
   const float* rope_cs;  // [max_seq][D/2][2]
   int layer, n_tokens, start_pos, rope_layout, tiles_per_cta;
+  // paper-literal Eq. 6-7 mode (include/tq.h): no normalisation, norm plane 1.0, rnorm plane = e-bar m sqrt(2/pi)
+  int literal;
+  const float* ebar_k;  // [H] of this layer (literal mode)
 };
 
 struct DecodeArgs {
@@ -192,6 +195,8 @@ struct DecodeArgs {
   //    multi-layer prep kernel) was already awaited by the first of the chain: nothing is awaited at the start, and the
   //    CTAs wait for the kernel in front only before they exit, so that the chain still completes in order.
   int chain_mode;
+  int literal;          // paper-literal mode of the append (see QuantArgs)
+  const float* ebar_k;  // [L][H]
 };
 
 cudaError_t launch_quantize_pack(const QuantArgs& a, int D, tq_dtype dt, int num_sms, cudaStream_t st);
@@ -236,6 +241,12 @@ __device__ __forceinline__ unsigned short f32_to_f16_bits_clamped(float x) {
   return __half_as_ushort(__float2half_rn(x));
 }
 __device__ __forceinline__ float f16_bits_to_f32(unsigned short h) { return __half2float(__ushort_as_half(h)); }
+// paper-literal mode: the rnorm plane holds e-bar m sqrt(2/pi), rounded to binary16 straight from fp64
+__device__ __forceinline__ unsigned short literal_rnorm_bits(float ebar, int m) {
+  const double g = fmin((double)ebar * (double)m * 0.79788456080286535588, 65504.0);
+  return __half_as_ushort(__double2half(g));
+}
+constexpr unsigned short kF16One = 0x3C00;
 
 template <typename T>
 __device__ __forceinline__ float load_as_float(const T* p);

@@ -31,6 +31,8 @@ struct PrepArgs {
   unsigned* frags;                                          // workspace [units][FragLayout<D>::kWords]
   unsigned* tabs;                                           // workspace [layers_call * H][kTabWords]
   int layer_begin, rope_layout;
+  int literal;          // paper-literal Eq. 6-7 mode of the append (include/tq.h)
+  const float* ebar_k;  // [L][H]
 };
 
 constexpr int kPrepThreads = 256;
@@ -348,9 +350,21 @@ __global__ void __launch_bounds__(kPrepThreads) prep_kernel(PrepArgs a) {
 #pragma unroll
     for (int j = 0; j < PL; ++j) n2 = fmaf(v2[j].x, v2[j].x, fmaf(v2[j].y, v2[j].y, n2));
     n2 = warp_sum(n2);
-    const float n = sqrtf(n2);
-    const float inv = n > 0.f ? 1.0f / n : 0.f;
+    const float n = a.literal ? 1.f : sqrtf(n2);                  // literal mode: the activation itself is coded
+    const float inv = a.literal ? 1.f : (n > 0.f ? 1.0f / n : 0.f);
     const float* lut = vec == 0 ? lutK : lutV;
+    // residual operand scale: 8 for a unit vector; in literal mode a power of two that keeps r inside the fp16 range
+    float rsc = 8.f;
+    if (a.literal && vec == 0) {
+      float rm = 0.f;
+#pragma unroll
+      for (int j = 0; j < PL; ++j) {
+        rm = fmaxf(rm, fmaxf(fabsf(v2[j].x - lut[code_of7(v2[j].x, lut)]), fabsf(v2[j].y - lut[code_of7(v2[j].y, lut)])));
+      }
+      rm = warp_max(rm);
+      float inv_r;
+      pow2_scale_p(rm, rsc, inv_r);
+    }
     float g2 = 0.f;
 #pragma unroll
     for (int j = 0; j < PL; ++j) {
@@ -362,7 +376,7 @@ __global__ void __launch_bounds__(kPrepThreads) prep_kernel(PrepArgs a) {
         g2 = fmaf(r0, r0, fmaf(r1, r1, g2));
         cK[e][i0] = (unsigned char)c0, cK[e][i0 + 1] = (unsigned char)c1;
         unsigned hi, lo;
-        split_pair(r0 * 8.f, r1 * 8.f, hi, lo);  // only sign(S r) is used
+        split_pair(r0 * rsc, r1 * rsc, hi, lo);  // only sign(S r) is used
         *reinterpret_cast<unsigned*>(Ah + (size_t)yrow * Cfg::HP + i0) = hi;
         *reinterpret_cast<unsigned*>(Al + (size_t)yrow * Cfg::HP + i0) = lo;
       } else {
@@ -526,8 +540,8 @@ __global__ void __launch_bounds__(kPrepThreads) prep_kernel(PrepArgs a) {
       int slot;
       unsigned char* tp = tile_of(e, slot);
       const int nl = slot_lane(slot);
-      reinterpret_cast<unsigned*>(tp + Lo::kOffNK)[nl] =
-          (unsigned)f32_to_f16_bits_clamped(nrm[0][e]) | ((unsigned)f32_to_f16_bits_clamped(nrm[1][e]) << 16);
+      const unsigned short rn = a.literal ? literal_rnorm_bits(__ldg(a.ebar_k + lh), D) : f32_to_f16_bits_clamped(nrm[1][e]);
+      reinterpret_cast<unsigned*>(tp + Lo::kOffNK)[nl] = (unsigned)f32_to_f16_bits_clamped(nrm[0][e]) | ((unsigned)rn << 16);
       reinterpret_cast<unsigned short*>(tp + Lo::kOffVN)[nl] = f32_to_f16_bits_clamped(nrm[2][e]);
     }
   }
@@ -593,6 +607,8 @@ cudaError_t launch_prep(const DecodeArgs& d, const void* k, const void* v, int D
   a.tabs = d.tabs;
   a.layer_begin = d.layer_begin;
   a.rope_layout = d.rope_layout;
+  a.literal = d.literal;
+  a.ebar_k = d.ebar_k;
   const int lh_count = d.n_layers_call * d.cv.H;
   if (D == 64)
     return d.dt == TQ_F16 ? launch_prep_t<64, __half>(a, lh_count, d.cv.B, num_sms, do_append, do_query, st)

@@ -311,7 +311,9 @@ __device__ __forceinline__ void stage_rows(const T* __restrict__ src, int i_firs
   }
 }
 
-template <int D, typename T, bool kKey>
+// kLit: the paper-literal Eq. 6-7 mode (include/tq.h): the accumulator is compared as it stands (no normalisation), the
+// norm plane is 1.0 and the rnorm plane the per-head constant e-bar m sqrt(2/pi)
+template <int D, typename T, bool kKey, bool kLit>
 __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int blocks_per_cta, int cta_x, unsigned char* smem) {
   using Cfg = TcCfg<D>;
   using Lo = Layout<D>;
@@ -359,6 +361,7 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
   // thresholds t_k = (lut_k + lut_{k+1}) / 2 in fp32, as search constants; keys also keep a table of LUT pairs for the
   // residual: the S product takes 8 r (only sign(S r) is used, and 8 r splits cleanly in fp16), |r| = |8 r| / 8
   Search search0;
+  float lut_cap = 1.f;
   {
     const float* lut_g = (kKey ? a.lut_k : a.lut_v) + h * 8;
     float l8[8], thr[7];
@@ -368,7 +371,13 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
     for (int q = 0; q < 7; ++q) thr[q] = 0.5f * (l8[q] + l8[q + 1]);
     search0 = make_search(thr);
     if (kKey && tid < 64) lutp[tid] = make_float2(-8.f * __ldg(lut_g + (tid & 7)), -8.f * __ldg(lut_g + (tid >> 3)));
+    if constexpr (kLit) {  // power of two that puts the largest LUT entry in [2^8, 2^9): bound of the residual operand scale
+      float s_l, inv_l;
+      pow2_scale(fmaxf(fabsf(l8[0]), fabsf(l8[7])), s_l, inv_l);
+      lut_cap = s_l * 256.f;
+    }
   }
+  const unsigned short lit_rnorm = (kLit && kKey) ? literal_rnorm_bits(__ldg(a.ebar_k + h), D) : (unsigned short)0;
   const float lutp_base = (float)smem_u32(lutp);  // shared-window address, exact in fp32
   fence_async_smem();
   tc_fence_before();
@@ -458,14 +467,19 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
     }
     __syncthreads();
     const float n = sqrtf(red_n[tok] + red_n[kBlk + tok]);
-    const unsigned short n_h = f32_to_f16_bits_clamped(n * scale_s[tok] * 0.0625f);  // y = 16 s PI x
-    const Search sr_n = scaled(search0, n > 0.f ? n : 1.f);  // thresholds on the accumulator scale
+    const float row_scale = 16.f / scale_s[tok];  // y = 16 s PI x, s a power of two
+    const unsigned short n_h = kLit ? kF16One : f32_to_f16_bits_clamped(n * scale_s[tok] * 0.0625f);
+    // thresholds on the accumulator scale: t |y| for the unit vector, t 16 s for the activation itself (literal mode)
+    const Search sr_n = scaled(search0, kLit ? row_scale : (n > 0.f ? n : 1.f));
 
     if constexpr (kKey) {
       // ---- codes, residual (the A operand of the S product, written over this token's operand row: the first product is
       //      complete).  Pair p = half d/4 + g belongs to lane (sg, t = g & 3) as field j = half d/32 + (g >> 2) of this
       //      token's block, bits [6 (J sr + j), + 6) of the lane's string: four fields = three bytes
       const float inv8 = n > 0.f ? 8.0f / n : 0.f;
+      // literal mode: residual operand = rs (y_true - lut[c]) with the power of two rs = min(16 s, lut_cap), so that
+      // neither term leaves the fp16 range whatever the scale of the row
+      const float rs = fminf(row_scale, lut_cap), rA = rs / row_scale, rB = rs * 0.125f;
       float g2a = 0.f, g2b = 0.f;
       float yt[4][NC / 32];  // four six-bit fields = one 24-bit word, accumulated exactly in fp32
 #pragma unroll
@@ -477,7 +491,9 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
         const float field = fmaf(code_f(y[2 * g + 1], sr_n), 8.f, code_f(y[2 * g], sr_n));  // c0 | c1 << 3
         float2 nl;  // (-8 lut[c0], -8 lut[c1])
         asm("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(nl.x), "=f"(nl.y) : "r"(f2u(fmaf(field, 8.f, lutp_base))));
-        const float r0 = fmaf(y[2 * g], inv8, nl.x), r1 = fmaf(y[2 * g + 1], inv8, nl.y);  // 8 (u - lut[c])
+        float r0, r1;
+        if constexpr (kLit) r0 = fmaf(y[2 * g], rA, nl.x * rB), r1 = fmaf(y[2 * g + 1], rA, nl.y * rB);
+        else r0 = fmaf(y[2 * g], inv8, nl.x), r1 = fmaf(y[2 * g + 1], inv8, nl.y);  // 8 (u - lut[c])
         g2a = fmaf(r0, r0, g2a), g2b = fmaf(r1, r1, g2b);
         y[2 * g] = r0, y[2 * g + 1] = r1;
         yt[g & 3][g >> 4] = fmaf(field, (float)(1u << (6 * ((g >> 2) & 3))), yt[g & 3][g >> 4]);
@@ -511,7 +527,8 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
       }
       if (valid && half == 0)
         reinterpret_cast<unsigned*>(timg + kOffImgNK)[slot_lane(slot)] =
-            (unsigned)n_h | ((unsigned)f32_to_f16_bits_clamped(sqrtf(red_g[tok] + red_g[kBlk + tok]) * 0.125f) << 16);
+            (unsigned)n_h |
+            ((unsigned)(kLit ? lit_rnorm : f32_to_f16_bits_clamped(sqrtf(red_g[tok] + red_g[kBlk + tok]) * 0.125f)) << 16);
       // ---- residual sketch: bit j = [(S r)_j >= 0] for this thread's sketch rows [half d/2, + d/2).  Sketch rows
       //      [t d/4, (t+1) d/4) belong to lane (sg, t) as 16-bit pieces u; a piece is stored as two bytes of word (mt, u):
       //      byte (sr & 1) holds bits 0..7, byte 2 + (sr & 1) bits 8..15 (the byte interleave with the slot 8 further on
@@ -617,14 +634,14 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
 
 // grid = (block groups, batch x heads, keys | values): the key CTAs (the long ones) are dispatched first and the value
 // CTAs fill in behind them (measured: alternating key and value CTAs along x is 8 % slower at configs[2])
-template <int D, typename T>
+template <int D, typename T, bool kLit>
 __global__ void __launch_bounds__(kThreads, D == 64 ? 3 : 1) quantize_pack_tc_kernel(QuantArgs a, int blocks_per_cta) {
   extern __shared__ __align__(1024) unsigned char smem_dyn[];
-  if (blockIdx.z == 0) quantize_pack_tc_body<D, T, true>(a, blocks_per_cta, (int)blockIdx.x, smem_dyn);
-  else quantize_pack_tc_body<D, T, false>(a, blocks_per_cta, (int)blockIdx.x, smem_dyn);
+  if (blockIdx.z == 0) quantize_pack_tc_body<D, T, true, kLit>(a, blocks_per_cta, (int)blockIdx.x, smem_dyn);
+  else quantize_pack_tc_body<D, T, false, kLit>(a, blocks_per_cta, (int)blockIdx.x, smem_dyn);
 }
 
-template <int D, typename T>
+template <int D, typename T, bool kLit>
 cudaError_t launch_quant_tc_t(const QuantArgs& a, int num_sms, cudaStream_t st) {
   const size_t smem = TcCfg<D>::kSmemBytes;
   const int first_blk = a.start_pos / kBlk, last_blk = (a.start_pos + a.n_tokens - 1) / kBlk;
@@ -634,9 +651,9 @@ cudaError_t launch_quant_tc_t(const QuantArgs& a, int num_sms, cudaStream_t st) 
   int bpc = (int)(((long)nblk * BH + want - 1) / want);
   bpc = bpc < 1 ? 1 : (bpc > 16 ? 16 : bpc);
   dim3 grid((nblk + bpc - 1) / bpc, BH, 2);  // z: keys | values
-  cudaError_t e = cudaFuncSetAttribute(quantize_pack_tc_kernel<D, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  cudaError_t e = cudaFuncSetAttribute(quantize_pack_tc_kernel<D, T, kLit>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
-  quantize_pack_tc_kernel<D, T><<<grid, kThreads, smem, st>>>(a, bpc);
+  quantize_pack_tc_kernel<D, T, kLit><<<grid, kThreads, smem, st>>>(a, bpc);
   count_launch();
   return cudaGetLastError();
 }
@@ -644,8 +661,12 @@ cudaError_t launch_quant_tc_t(const QuantArgs& a, int num_sms, cudaStream_t st) 
 }  // namespace
 
 cudaError_t launch_quantize_pack_tc(const QuantArgs& a, int D, tq_dtype dt, int num_sms, cudaStream_t st) {
-  if (D == 64) return dt == TQ_F16 ? launch_quant_tc_t<64, __half>(a, num_sms, st) : launch_quant_tc_t<64, float>(a, num_sms, st);
-  return dt == TQ_F16 ? launch_quant_tc_t<128, __half>(a, num_sms, st) : launch_quant_tc_t<128, float>(a, num_sms, st);
+  if (a.literal) {
+    if (D == 64) return dt == TQ_F16 ? launch_quant_tc_t<64, __half, true>(a, num_sms, st) : launch_quant_tc_t<64, float, true>(a, num_sms, st);
+    return dt == TQ_F16 ? launch_quant_tc_t<128, __half, true>(a, num_sms, st) : launch_quant_tc_t<128, float, true>(a, num_sms, st);
+  }
+  if (D == 64) return dt == TQ_F16 ? launch_quant_tc_t<64, __half, false>(a, num_sms, st) : launch_quant_tc_t<64, float, false>(a, num_sms, st);
+  return dt == TQ_F16 ? launch_quant_tc_t<128, __half, false>(a, num_sms, st) : launch_quant_tc_t<128, float, false>(a, num_sms, st);
 }
 
 }  // namespace tq

@@ -744,3 +744,83 @@ def test_synthetic_ablation_shared_lut_row(tq, oracle):
     print(f"  SNR lost by sharing: K {rows['dual'][1] - rows['shared'][1]:.2f} dB, V {rows['dual'][2] - rows['shared'][2]:.2f} dB"
           "   [paper: ~1.2 dB]")
     assert rows["dual"][1] >= rows["shared"][1] - 0.02 and rows["dual"][2] >= rows["shared"][2] - 0.02
+
+
+# ---------------------------------------------------------------------------------------------- paper-literal Eq. 6-7 mode
+def _np_rope_keys(k, start_pos, base):
+    B, H, T, d = k.shape
+    th = base ** (-2.0 * np.arange(d // 2) / d)
+    ang = (start_pos + np.arange(T))[:, None] * th[None, :]
+    kf = k.astype(np.float64).reshape(B, H, T, d // 2, 2)
+    kr = np.stack((kf[..., 0] * np.cos(ang) - kf[..., 1] * np.sin(ang), kf[..., 0] * np.sin(ang) + kf[..., 1] * np.cos(ang)), -1)
+    return kr.reshape(B, H, T, d)
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("name,kw,gauss_S", [("cfg2_650m_batch32", dict(batch=3, n_heads=4, seq=300), False),
+                                             ("cfg4_15b_heads", dict(batch=2, n_heads=3, seq=170), False),
+                                             ("cfg2_650m_batch32", dict(batch=2, n_heads=3, seq=140), True)])
+def test_paper_literal_mode_matches_oracle(tq, oracle, name, kw, gauss_S):
+    """residual_mode = 1.  Calibration from the product
+    (tq_calibrate_host mode 0 in literal mode: SVD PI_K, PI_V = I, S = I, LUTs on the raw rotated activations, e-bar =
+    mean |e| of the key samples); prefill in unaligned chunks + appended tokens vs tqo_quantize_pack_literal (codes and
+    sign bits bit-exact outside the band, norm plane exactly 1.0, rnorm plane exactly the oracle's constant); decode on
+    the oracle's bytes vs tqo_decode_attn at 2e-3 / 0.9999; and the GPU cache decodes like the oracle's."""
+    import torch
+
+    w = W.CONFIGS[name].scaled(**kw)
+    d, H, B, T = w.head_dim, w.n_heads, w.batch, w.seq
+    k, v = W.layer_activations(w, 0)
+    n_app = 3
+    toks = [W.step_tokens(w, 0, s) for s in range(n_app)]
+    shape = tq.make_shape(1, B, H, d, T + 8, w.rope_base, 0, residual_mode=1)
+    ks = np.ascontiguousarray(_np_rope_keys(k, 0, w.rope_base).transpose(1, 0, 2, 3).reshape(1, H, -1, d), np.float32)
+    vs = np.ascontiguousarray(v.astype(np.float32).transpose(1, 0, 2, 3).reshape(1, H, -1, d))
+    cal = tq.tq_calibrate_host(shape, 0, ks, vs, seed=3)
+    assert np.array_equal(cal["S"], np.eye(d, dtype=np.float32)) and np.array_equal(cal["pi_v"][0, 1], np.eye(d, dtype=np.float32))
+    # e-bar is the sample mean of |y - lut[code]| over the rotated key samples
+    for h in range(H):
+        y = ks[0, h].astype(np.float64) @ cal["pi_k"][0, h].astype(np.float64).T
+        lut = cal["lut_k"][0, h].astype(np.float64)
+        assert abs(np.abs(y - lut[np.abs(y[..., None] - lut).argmin(-1)]).mean() / cal["ebar_k"][0, h] - 1) < 1e-5
+    if gauss_S:  # the kernels take any S; only S = I is the paper's Eq. 6
+        cal["S"] = W.sketch(w)
+    params = tq.Params(cal)
+    cache = tq.Cache(shape)
+    dev = lambda x: torch.from_numpy(np.ascontiguousarray(x)).cuda()
+    cut = 77  # unaligned chunk boundary
+    tq.tq_quantize_pack(shape, params, cache, 0, dev(k[:, :, :cut]), dev(v[:, :, :cut]), 0)
+    tq.tq_quantize_pack(shape, params, cache, 0, dev(k[:, :, cut:]), dev(v[:, :, cut:]), cut)
+    for (_, kn, vn) in toks:
+        tq.tq_append(shape, params, cache, 0, dev(kn), dev(vn))
+    Tn = T + n_app
+    assert torch.all(cache.seq_len == Tn)
+    planes = {n: p.cpu().numpy() for n, p in tq.tq_cache_export_canonical(shape, cache, 0, Tn).items()}
+    kk = np.concatenate([k] + [t[1][:, :, None] for t in toks], axis=2)
+    vv = np.concatenate([v] + [t[2][:, :, None] for t in toks], axis=2)
+    can = oracle.quantize_pack_literal(kk, vv, cal["pi_k"][0], cal["pi_v"][0], cal["lut_k"][0], cal["lut_v"][0], cal["S"],
+                                       cal["ebar_k"][0], base=w.rope_base, near_eps=TL.NEAR_EPS)
+    rep = TL.compare_quantize(can, planes, d, "paper-literal mode")
+    assert np.all(planes["k_norm"].view(np.uint16) == 0x3C00) and np.all(planes["v_norm"].view(np.uint16) == 0x3C00)
+    assert np.array_equal(planes["k_rnorm"].view(np.uint16), can.k_rnorm)
+    print("paper-literal quantize:", {k_: v_ for k_, v_ in rep.items() if not k_.endswith("equal")})
+    # decode on the oracle's bytes
+    cache2 = tq.Cache(shape)
+    tq.tq_cache_import_canonical(shape, cache2, 0, Tn, TL.to_torch_canonical(can))
+    q = W.queries(w, 0)
+    qd = dev(q[None])
+    out, out_own = torch.full_like(qd, float("nan")), torch.full_like(qd, float("nan"))
+    ws = tq.Workspace(shape, 1)
+    tq.tq_decode_attn(shape, params, cache2, 0, 1, qd, out, ws)
+    tq.tq_decode_attn(shape, params, cache, 0, 1, qd, out_own, ws)
+    torch.cuda.synchronize()
+    sl = np.full(B, Tn, np.int32)
+    want = oracle.decode_attn(q, sl - 1, sl, cal["pi_k"][0], cal["pi_v"][0], cal["lut_k"][0], cal["lut_v"][0], cal["S"], can,
+                              base=w.rope_base)
+    got = out[0].float().cpu().numpy()
+    ulp = np.spacing(np.abs(want).astype(np.float16)).astype(np.float64)  # fp16 outputs: one binary16 ulp on top
+    assert np.all(np.abs(got.astype(np.float64) - want) <= ulp + TL.OUT_MAX_ABS)
+    print("paper-literal decode:", TL.compare_outputs(got, want, "paper-literal decode", max_abs=float(ulp.max()) + TL.OUT_MAX_ABS))
+    # the GPU's own cache differs from the oracle's only inside the band: its decode stays close
+    a, b_ = out_own[0].float().cpu().numpy().reshape(-1, d).astype(np.float64), want.reshape(-1, d)
+    assert np.mean(np.sum(a * b_, -1) / (np.linalg.norm(a, axis=-1) * np.linalg.norm(b_, axis=-1))) > 0.999

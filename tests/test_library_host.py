@@ -164,3 +164,36 @@ def test_calibrate_mode0_svd_and_kmeans(tq, oracle):
         co, _ = oracle.lloyd_max_samples(U, 8, iters=300)
         assert np.allclose(co, lut, atol=5e-3)
     assert not np.allclose(out["lut_k"][0, 0], out["lut_v"][0, 0], atol=1e-3)  # dual LUTs differ
+
+
+def test_calibrate_paper_literal_mode(tq, oracle):
+    """residual_mode = 1: S = I, PI_V = I, e-bar = mean |y - lut[code]|; mode 1 gives the
+    Gaussian integral for N(0, 1/d) (checked by quadrature), mode 0 the sample mean on the raw rotated key samples with
+    LUTs fitted on that raw scale."""
+    d = 64
+    s = tq.make_shape(2, 1, 2, d, 16, residual_mode=1)
+    out = tq.tq_calibrate_host(s, 1, seed=5)
+    assert np.array_equal(out["S"], np.eye(d, dtype=np.float32))
+    assert all(np.array_equal(out["pi_v"][l, h], np.eye(d, dtype=np.float32)) for l in range(2) for h in range(2))
+    lut = out["lut_k"][0, 0].astype(np.float64)
+    sig = 1 / 8
+    x = np.linspace(-8 * sig, 8 * sig, 2_000_001)
+    pdf = np.exp(-0.5 * (x / sig) ** 2) / (sig * math.sqrt(2 * math.pi))
+    thr = (0.5 * (out["lut_k"][0, 0][:-1] + out["lut_k"][0, 0][1:])).astype(np.float64)
+    e = np.abs(x - lut[np.searchsorted(thr, x, side="left")])
+    want = float(np.sum(e * pdf) * (x[1] - x[0]))
+    assert np.allclose(out["ebar_k"], want, rtol=1e-5)
+    # mode 0: raw-scale LUT and sample e-bar
+    rng = np.random.default_rng(1)
+    n = 2000
+    ks = (rng.standard_normal((2, 2, n, d)) * 2.5).astype(np.float32)
+    vs = (rng.standard_normal((2, 2, n, d)) * 0.7).astype(np.float32)
+    o0 = tq.tq_calibrate_host(s, 0, ks, vs, seed=5)
+    y = ks[1, 0].astype(np.float64) @ o0["pi_k"][1, 0].astype(np.float64).T
+    l0 = o0["lut_k"][1, 0].astype(np.float64)
+    assert 2.0 < np.abs(l0).max() < 8.0                      # on the scale of the activations, not of a unit vector
+    assert abs(np.abs(y - l0[np.abs(y[..., None] - l0).argmin(-1)]).mean() / o0["ebar_k"][1, 0] - 1) < 1e-5
+    assert 0.5 < np.abs(o0["lut_v"][0, 1]).max() < 2.5 and np.array_equal(o0["pi_v"][0, 1], np.eye(d, dtype=np.float32))
+    # the mode must be declared and e-bar supplied
+    bad = tq.make_shape(1, 1, 1, d, 16, residual_mode=2)
+    assert tq.tq_cache_bytes(bad) == 0
