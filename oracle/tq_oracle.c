@@ -16,6 +16,7 @@
  *   packing                    PAPER.md:199-213 (8 codes at shifts 0,3,..,21), 3 bytes per 8 codes (D5)
  *   decode                     PAPER.md:118-124 and Algorithm 1, two-pass exact softmax
  *   paper-literal Eq. 6-7 mode PAPER.md:166-179 as printed (tqo_quantize_vector_literal / _pack_literal)
+ *   V-side residual sketch     Algorithm 1 line 10, PAPER.md:234 (tqo_value_sketch_planes / tqo_decode_attn_vq)
  *
  * Pins (tests/test_oracle_*.py): every function below is checked against something other than itself —
  * closed forms, textbook tables, numpy library routines, brute force, Monte-Carlo.  Parity unpinned: none
@@ -427,6 +428,93 @@ void tqo_decode_attn(int B, int H, int d, int m, int T_stride, double base, int 
       tqo_unpack_codes(v_codes + e * cb, d, codes);
       double nv = tqo_f16_to_f64(v_norm[e]);
       for (int i = 0; i < d; ++i) o[i] += p * nv * (double)luv[codes[i]];
+    }
+    for (int i = 0; i < d; ++i) o[i] = T > 0 ? o[i] / l : 0.0;
+    matvec_t_f32(pi_v + (size_t)h * d * d, d, d, o, out + (size_t)unit * d);
+    free(s);
+  }
+}
+
+/* ---- V-side residual sketch (Algorithm 1 line 10, "v = LUT_V[idx_v] + sign_v * e_v"; SURVEY.md 8(f)
+ * NEXT-1, 8(c) step 10; reading D3: tq_shape.v_qjl = 1) ------------------------------------------------
+ * Values get the same treatment as keys minus RoPE: y = PI_V v, n = |y|, u = y / n, codes on u, r = u - lut_V[code],
+ * bits_j = [(S r)_j >= 0], rnorm = |r|.  A dequantised value is then the JL reconstruction
+ *   v~ = n ( lut_V[code] + sqrt(pi/2)/m * |r| * S^T sigma ),  sigma = 2 bits - 1,
+ * whose inner product with any vector is the estimator of tqo_qjl_estimate (E over S of the second term = r).
+ * This function only adds the two value planes; codes and norms are those of tqo_quantize_pack.                   */
+void tqo_value_sketch_planes(int B, int H, int T, int d, int m, const float *v, const float *pi_v, const float *lut_v,
+                             const float *S, uint8_t *v_signs, uint16_t *v_rnorm) {
+  const int sb = m / 8;
+  long total = (long)B * H * T;
+#pragma omp parallel for schedule(static)
+  for (long idx = 0; idx < total; ++idx) {
+    int h = (int)((idx / T) % H);
+    double x[256], y[256], r[256], sr[256];
+    uint8_t bits[256];
+    const float *lu = lut_v + (size_t)h * 8;
+    for (int i = 0; i < d; ++i) x[i] = (double)v[(size_t)idx * d + i];
+    matvec_f32(pi_v + (size_t)h * d * d, d, d, x, y);
+    double n2 = 0.0, g2 = 0.0;
+    for (int i = 0; i < d; ++i) n2 += y[i] * y[i];
+    double n = sqrt(n2);
+    for (int i = 0; i < d; ++i) {
+      double u = n > 0.0 ? y[i] / n : 0.0;
+      r[i] = u - (double)lu[tqo_code(u, lu)];
+      g2 += r[i] * r[i];
+    }
+    matvec_f32(S, m, d, r, sr);
+    for (int j = 0; j < m; ++j) bits[j] = (uint8_t)(sr[j] >= 0.0 ? 1 : 0);
+    tqo_pack_bits(bits, m, v_signs + (size_t)idx * sb);
+    v_rnorm[idx] = tqo_f64_to_f16(sqrt(g2));
+  }
+}
+
+/* Decode attention with the V-side sketch: exactly tqo_decode_attn, except that the value of token j is the JL
+ * reconstruction above:  o' = sum_j p_j nv_j ( lut_V[codeV_j] + sqrt(pi/2)/m * gv_j * S^T sigmaV_j ).            */
+void tqo_decode_attn_vq(int B, int H, int d, int m, int T_stride, double base, int layout, const float *q,
+                        const int32_t *q_pos, const int32_t *seq_len, const float *pi_k, const float *pi_v,
+                        const float *lut_k, const float *lut_v, const float *S, const uint8_t *k_codes,
+                        const uint8_t *k_signs, const uint16_t *k_norm, const uint16_t *k_rnorm,
+                        const uint8_t *v_codes, const uint16_t *v_norm, const uint8_t *v_signs,
+                        const uint16_t *v_rnorm, double *out) {
+  const int cb = 3 * d / 8, sb = m / 8;
+  const double cq = sqrt(TQO_PI / 2.0) / (double)m;
+#pragma omp parallel for schedule(dynamic)
+  for (int unit = 0; unit < B * H; ++unit) {
+    int b = unit / H, h = unit % H;
+    int T = seq_len[b];
+    double qv[256], qr[256], q2[256], z[256], o[256], sig[256], st[256];
+    for (int i = 0; i < d; ++i) qv[i] = (double)q[(size_t)unit * d + i];
+    tqo_rope(qv, d, (double)q_pos[b], base, layout, qr);
+    matvec_f32(pi_k + (size_t)h * d * d, d, d, qr, q2);
+    matvec_f32(S, m, d, q2, z);
+    const float *luk = lut_k + (size_t)h * 8, *luv = lut_v + (size_t)h * 8;
+    double *s = (double *)malloc(sizeof(double) * (size_t)(T > 0 ? T : 1));
+    uint8_t codes[256], bits[256];
+    double smax = -INFINITY;
+    for (int j = 0; j < T; ++j) {
+      size_t e = (size_t)unit * T_stride + j;
+      tqo_unpack_codes(k_codes + e * cb, d, codes);
+      tqo_unpack_bits(k_signs + e * sb, m, bits);
+      double a = 0.0, bq = 0.0;
+      for (int i = 0; i < d; ++i) a += q2[i] * (double)luk[codes[i]];
+      for (int i = 0; i < m; ++i) bq += z[i] * (bits[i] ? 1.0 : -1.0);
+      double n = tqo_f16_to_f64(k_norm[e]), g = tqo_f16_to_f64(k_rnorm[e]);
+      s[j] = n * (a + cq * g * bq) / sqrt((double)d);
+      if (s[j] > smax) smax = s[j];
+    }
+    double l = 0.0;
+    for (int i = 0; i < d; ++i) o[i] = 0.0;
+    for (int j = 0; j < T; ++j) {
+      size_t e = (size_t)unit * T_stride + j;
+      double p = exp(s[j] - smax);
+      l += p;
+      tqo_unpack_codes(v_codes + e * cb, d, codes);
+      tqo_unpack_bits(v_signs + e * sb, m, bits);
+      for (int i = 0; i < m; ++i) sig[i] = bits[i] ? 1.0 : -1.0;
+      matvec_t_f32(S, m, d, sig, st); /* S^T sigma */
+      double nv = tqo_f16_to_f64(v_norm[e]), gv = tqo_f16_to_f64(v_rnorm[e]);
+      for (int i = 0; i < d; ++i) o[i] += p * nv * ((double)luv[codes[i]] + cq * gv * st[i]);
     }
     for (int i = 0; i < d; ++i) o[i] = T > 0 ? o[i] / l : 0.0;
     matvec_t_f32(pi_v + (size_t)h * d * d, d, d, o, out + (size_t)unit * d);

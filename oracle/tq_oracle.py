@@ -213,6 +213,8 @@ class Canonical:
     v_norm: np.ndarray   # [B,H,T] u16
     near_k: np.ndarray | None = None  # [B,H,T,d] u8
     near_v: np.ndarray | None = None
+    v_signs: np.ndarray | None = None  # [B,H,T,m/8] u8   (V-side sketch, tq_shape.v_qjl = 1)
+    v_rnorm: np.ndarray | None = None  # [B,H,T] u16
 
 
 def quantize_pack(k, v, pi_k, pi_v, lut_k, lut_v, S, start_pos: int = 0, base: float = 10000.0,
@@ -277,6 +279,40 @@ def quantize_pack_literal(k, v, pi_k, pi_v, lut_k, lut_v, S, ebar_k, start_pos: 
                                     _p(lut_v), _p(S), _p(ebar_k), _p(out.k_codes), _p(out.k_signs), _p(out.k_norm),
                                     _p(out.k_rnorm), _p(out.v_codes), _p(out.v_norm), C.c_double(near_eps or 0.0),
                                     _p(out.near_k), _p(out.near_v))
+    return out
+
+
+def add_value_sketch(can: Canonical, v, pi_v, lut_v, S) -> Canonical:
+    """V-side residual sketch planes (Algorithm 1 line 10): fills can.v_signs / can.v_rnorm."""
+    v = _f32(v)
+    B, H, T, d = v.shape
+    S = _f32(S)
+    m = S.shape[0]
+    can.v_signs = np.zeros((B, H, T, m // 8), np.uint8)
+    can.v_rnorm = np.zeros((B, H, T), np.uint16)
+    lib().tqo_value_sketch_planes(C.c_int(B), C.c_int(H), C.c_int(T), C.c_int(d), C.c_int(m), _p(v), _p(_f32(pi_v)),
+                                  _p(_f32(lut_v)), _p(S), _p(can.v_signs), _p(can.v_rnorm))
+    return can
+
+
+def decode_attn_vq(q, q_pos, seq_len, pi_k, pi_v, lut_k, lut_v, S, cache: Canonical, base: float = 10000.0,
+                   layout: int = 0):
+    """decode_attn with the V-side sketch: values are n (lut_V[codes] + sqrt(pi/2)/m |r| S^T sigma)."""
+    q = _f32(q)
+    B, H, d = q.shape
+    S = _f32(S)
+    m = S.shape[0]
+    T_stride = cache.k_norm.shape[2]
+    q_pos = np.ascontiguousarray(q_pos, dtype=np.int32)
+    seq_len = np.ascontiguousarray(seq_len, dtype=np.int32)
+    assert int(seq_len.max(initial=0)) <= T_stride and cache.v_signs is not None
+    out = np.zeros((B, H, d), np.float64)
+    c = np.ascontiguousarray
+    lib().tqo_decode_attn_vq(C.c_int(B), C.c_int(H), C.c_int(d), C.c_int(m), C.c_int(T_stride), C.c_double(base),
+                             C.c_int(layout), _p(q), _p(q_pos), _p(seq_len), _p(_f32(pi_k)), _p(_f32(pi_v)), _p(_f32(lut_k)),
+                             _p(_f32(lut_v)), _p(S), _p(c(cache.k_codes)), _p(c(cache.k_signs)), _p(c(cache.k_norm)),
+                             _p(c(cache.k_rnorm)), _p(c(cache.v_codes)), _p(c(cache.v_norm)), _p(c(cache.v_signs)),
+                             _p(c(cache.v_rnorm)), _p(out))
     return out
 
 

@@ -286,3 +286,86 @@ def test_literal_pack_indexing_and_decode_equals_attention_over_eq7_keys(oracle)
             p /= p.sum()
             want = c["pi_v"][h].astype(np.float64).T @ (p @ vh)
             assert np.allclose(got[b, h], want, atol=1e-9)
+
+
+# ------------------------------------------------------------------------------------------------ V-side residual sketch
+def test_value_sketch_planes_and_decode_vq(oracle):
+    """Algorithm 1 line 10, SURVEY.md 8(f) NEXT-1.  (a) The value planes are the key-side recipe without
+    RoPE: bits = [S (u - lut[code]) >= 0], rnorm = |u - lut[code]|, rebuilt here with numpy.  (b) T = 1: out is the JL
+    reconstruction PI_V^T n (lut_V[codes] + sqrt(pi/2)/m |r| S^T sigma).  (c) decode_attn_vq == brute-force softmax
+    attention over those reconstructed values with the logits of the pinned decode_attn."""
+    c = make_case(oracle, B=2, H=3, T=23, d=64, seed=4)
+    B, H, T, d = c["k"].shape
+    can = oracle.quantize_pack(c["k"], c["v"], c["pi_k"], c["pi_v"], c["lut_k"], c["lut_v"], c["S"])
+    oracle.add_value_sketch(can, c["v"], c["pi_v"], c["lut_v"], c["S"])
+    cq = math.sqrt(math.pi / 2) / d
+
+    def recon(b, h, t):  # rotated-basis JL reconstruction of value (b, h, t) from the stored planes
+        lv = c["lut_v"][h].astype(np.float64)
+        codes = oracle.unpack_codes(can.v_codes[b, h, t], d)
+        sig = 2.0 * oracle.unpack_bits(can.v_signs[b, h, t], d) - 1.0
+        n, g = oracle.f16_bits_to_f64(int(can.v_norm[b, h, t])), oracle.f16_bits_to_f64(int(can.v_rnorm[b, h, t]))
+        return n * (lv[codes] + cq * g * (c["S"].astype(np.float64).T @ sig))
+
+    for (b, h, t) in [(0, 0, 0), (1, 2, 22), (0, 1, 11)]:
+        y = c["pi_v"][h].astype(np.float64) @ c["v"][b, h, t].astype(np.float64)
+        u = y / np.linalg.norm(y)
+        lv = c["lut_v"][h].astype(np.float64)
+        r = u - lv[np.abs(u[:, None] - lv[None, :]).argmin(1)]
+        assert np.array_equal(oracle.unpack_bits(can.v_signs[b, h, t], d), (c["S"].astype(np.float64) @ r >= 0).astype(np.uint8))
+        assert abs(oracle.f16_bits_to_f64(int(can.v_rnorm[b, h, t])) / np.linalg.norm(r) - 1) <= 2.0 ** -11
+    # (b) T = 1
+    one = np.ones(B, np.int32)
+    got1 = oracle.decode_attn_vq(c["q"], one - 1, one, c["pi_k"], c["pi_v"], c["lut_k"], c["lut_v"], c["S"], can)
+    for b in range(B):
+        for h in range(H):
+            assert np.allclose(got1[b, h], c["pi_v"][h].astype(np.float64).T @ recon(b, h, 0), atol=1e-12)
+    # (c) full attention: weights from the pinned K side (decode_attn with V = one-hot trick is not needed: recompute the
+    #     logits through decode_attn's own definition by probing with unit values) -> here simply by brute force
+    sl = np.array([T, 9], np.int32)
+    got = oracle.decode_attn_vq(c["q"], sl - 1, sl, c["pi_k"], c["pi_v"], c["lut_k"], c["lut_v"], c["S"], can)
+    base = oracle.decode_attn(c["q"], sl - 1, sl, c["pi_k"], c["pi_v"], c["lut_k"], c["lut_v"], c["S"], can)
+    for b in range(B):
+        for h in range(H):
+            Tb = int(sl[b])
+            q2 = c["pi_k"][h].astype(np.float64) @ np_rope(c["q"][b, h].astype(np.float64), Tb - 1)
+            z = c["S"].astype(np.float64) @ q2
+            lk = c["lut_k"][h].astype(np.float64)
+            s = np.empty(Tb)
+            for t in range(Tb):
+                kc = oracle.unpack_codes(can.k_codes[b, h, t], d)
+                sg = 2.0 * oracle.unpack_bits(can.k_signs[b, h, t], d) - 1.0
+                n, g = oracle.f16_bits_to_f64(int(can.k_norm[b, h, t])), oracle.f16_bits_to_f64(int(can.k_rnorm[b, h, t]))
+                s[t] = n * (q2 @ lk[kc] + cq * g * (z @ sg)) / math.sqrt(d)
+            p = np.exp(s - s.max())
+            p /= p.sum()
+            vt = np.stack([recon(b, h, t) for t in range(Tb)])
+            want = c["pi_v"][h].astype(np.float64).T @ (p @ vt)
+            assert np.allclose(got[b, h], want, atol=1e-10)
+            # and it differs from the K-only decode by exactly the sketch term
+            lv = c["lut_v"][h].astype(np.float64)
+            plain = np.stack([oracle.f16_bits_to_f64(int(can.v_norm[b, h, t])) * lv[oracle.unpack_codes(can.v_codes[b, h, t], d)] for t in range(Tb)])
+            assert np.allclose(base[b, h], c["pi_v"][h].astype(np.float64).T @ (p @ plain), atol=1e-10)
+
+
+def test_value_sketch_reconstruction_is_unbiased_over_S(oracle):
+    """E_S[ sqrt(pi/2)/m |r| S^T sign(S r) ] = r (the vector form of the pinned inner-product estimator): Monte-Carlo over
+    seeded Gaussian S, every coordinate within 4.5 standard errors, and the mean reconstruction error shrinks."""
+    rng = np.random.default_rng(8)
+    d = m = 64
+    lut = gauss_lut(oracle, d)
+    x = rng.standard_normal(d)
+    u = x / np.linalg.norm(x)
+    r = u - lut.astype(np.float64)[np.abs(u[:, None] - lut.astype(np.float64)[None, :]).argmin(1)]
+    g = np.linalg.norm(r)
+    n_draw = 4000
+    acc, acc2 = np.zeros(d), np.zeros(d)
+    for _ in range(n_draw):
+        S = rng.standard_normal((m, d))
+        est = math.sqrt(math.pi / 2) / m * g * (S.T @ np.where(S @ r >= 0, 1.0, -1.0))
+        acc += est
+        acc2 += est * est
+    mean = acc / n_draw
+    se = np.sqrt(np.maximum(acc2 / n_draw - mean ** 2, 1e-30) / n_draw)
+    assert np.all(np.abs(mean - r) < 4.5 * se)
+    assert np.linalg.norm(mean - r) < 0.1 * g
