@@ -45,6 +45,8 @@
  *     norms   : one u32 per lane (binary16 |k| | binary16 |r_k| << 16) and one u16 (binary16 |v|); lane (g, t) owns
  *               slot g + 8 t.
  *   Bytes per cached token-head: 62 (d = 64), 118 (d = 128) — the same as the canonical format.
+ *   With v_qjl = 1 every (layer, batch, head) owns a second stream of 32-token tiles for the value sketch (sign bits in
+ *   the A-fragment order of the sketch accumulation, binary16 |r_v|): + 10 / 18 bytes per token-head.
  *   A cache has ONE writer at a time: tq_quantize_pack / tq_append / tq_decode_step / tq_decode_model_step /
  *   tq_cache_import_canonical calls that touch the same layer must be ordered by the caller (same stream, or events);
  *   concurrent readers (tq_decode_attn, export) of a layer that is not being written are fine.
@@ -81,7 +83,10 @@ typedef struct {
   int32_t max_seq;     /* cache capacity in tokens per (layer, batch, head)                             */
   float rope_base;     /* theta_g = rope_base^(-2g/d); 10000 in BASELINE.json:configs[0]                */
   int32_t rope_layout; /* 0 = interleaved pairs (2g, 2g+1) [PAPER.md:102, Eq. 2]; 1 = half-split (g, g+d/2) */
-  int32_t v_qjl;       /* 0 = K-only residual sketch (reading D3); 1 is TQ_ERR_UNSUPPORTED     */
+  int32_t v_qjl;       /* 0 = K-only residual sketch (reading D3); 1 = values carry one too [Algorithm 1
+                          line 10, PAPER.md:234]: bits sign(S r_v) and binary16 |r_v| per token, +m/8 + 2 bytes; a
+                          dequantised value is then n_v (lut_V[codes] + sqrt(pi/2)/m |r_v| S^T sigma_v).  Not combined
+                          with residual_mode 1 (TQ_ERR_UNSUPPORTED)                                              */
   int32_t residual_mode; /* 0 = north_star form: unit vector coded, |y| and |r| stored per token, bits = sign(S r);
                             1 = the paper's literal Eq. 6-7 [PAPER.md:170-179]: see "Paper-literal mode" below   */
 } tq_shape;
@@ -119,7 +124,7 @@ typedef struct {
 
 /* ---- sizes (pure host arithmetic; return 0 on an invalid shape) ---------------------------------- */
 size_t tq_cache_bytes(const tq_shape *shape);
-size_t tq_cache_bytes_per_token_head(const tq_shape *shape); /* 62 or 118                               */
+size_t tq_cache_bytes_per_token_head(const tq_shape *shape); /* 62 or 118; 72 or 136 with v_qjl = 1        */
 /* Byte offset inside tq_cache.data of int32 seq_len[L][B] (tokens currently cached) and of the
  * int32 sticky status word (0, or TQ_ERR_CAPACITY once an append was refused on the device).          */
 size_t tq_cache_seq_len_offset(const tq_shape *shape);
@@ -130,7 +135,7 @@ size_t tq_cache_status_offset(const tq_shape *shape);
  * workspace must be ordered on one stream.                                                               */
 size_t tq_decode_workspace_bytes(const tq_shape *shape, int32_t n_layers_call);
 /* Canonical plane sizes in bytes for n_tokens tokens of every (layer?, batch, head) of ONE layer:
- * plane 0 k_codes, 1 k_signs, 2 k_norm, 3 k_rnorm, 4 v_codes, 5 v_norm.                                */
+ * plane 0 k_codes, 1 k_signs, 2 k_norm, 3 k_rnorm, 4 v_codes, 5 v_norm, 6 v_signs, 7 v_rnorm (6, 7: v_qjl = 1). */
 size_t tq_canonical_plane_bytes(const tq_shape *shape, int32_t plane, int32_t n_tokens);
 
 /* ---- host-side calibration (not hot) [PAPER.md:128-143 §3.2; 145-164 §3.3; north_star] ------------
@@ -194,6 +199,8 @@ typedef struct {
   uint16_t *k_norm, *k_rnorm;
   uint8_t *v_codes;
   uint16_t *v_norm;
+  uint8_t *v_signs;  /* v_qjl = 1 only (else ignored, may be NULL): m/8 bytes per entry, like k_signs */
+  uint16_t *v_rnorm; /* v_qjl = 1 only: binary16 |r_v|                                                */
 } tq_canonical;
 
 int tq_cache_export_canonical(const tq_shape *shape, const tq_cache *cache, int32_t layer, int32_t n_tokens,

@@ -49,7 +49,7 @@ class TqCache(C.Structure):
 
 
 class TqCanonical(C.Structure):
-    _fields_ = [(n, C.c_void_p) for n in ("k_codes", "k_signs", "k_norm", "k_rnorm", "v_codes", "v_norm")]
+    _fields_ = [(n, C.c_void_p) for n in ("k_codes", "k_signs", "k_norm", "k_rnorm", "v_codes", "v_norm", "v_signs", "v_rnorm")]
 
 
 _lib = None
@@ -268,14 +268,19 @@ def tq_debug_set_quantize_impl(fp32_cuda_cores: bool):
 
 
 def _canon_struct(planes: dict) -> TqCanonical:
-    return TqCanonical(*[_ptr(planes[n]) for n in ("k_codes", "k_signs", "k_norm", "k_rnorm", "v_codes", "v_norm")])
+    return TqCanonical(*[_ptr(planes.get(n)) for n in ("k_codes", "k_signs", "k_norm", "k_rnorm", "v_codes", "v_norm",
+                                                       "v_signs", "v_rnorm")])
 
 
 def alloc_canonical(shape, n_tokens: int, device="cuda") -> dict:
     import torch
 
     B, H, d, m = shape.batch, shape.n_heads, shape.head_dim, shape.qjl_dim
-    return dict(k_codes=torch.zeros((B, H, n_tokens, 3 * d // 8), dtype=torch.uint8, device=device),
+    extra = {}
+    if shape.v_qjl == 1:  # V-side sketch planes
+        extra = dict(v_signs=torch.zeros((B, H, n_tokens, m // 8), dtype=torch.uint8, device=device),
+                     v_rnorm=torch.zeros((B, H, n_tokens), dtype=torch.int16, device=device))
+    return dict(**extra, k_codes=torch.zeros((B, H, n_tokens, 3 * d // 8), dtype=torch.uint8, device=device),
                 k_signs=torch.zeros((B, H, n_tokens, m // 8), dtype=torch.uint8, device=device),
                 k_norm=torch.zeros((B, H, n_tokens), dtype=torch.int16, device=device),
                 k_rnorm=torch.zeros((B, H, n_tokens), dtype=torch.int16, device=device),

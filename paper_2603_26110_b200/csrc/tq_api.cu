@@ -60,7 +60,9 @@ static int check_shape(const tq_shape* s, CacheGeom* g) {
     return TQ_ERR_INVALID_ARG;
   if (s->rope_layout != 0 && s->rope_layout != 1) return TQ_ERR_INVALID_ARG;
   if (s->residual_mode != 0 && s->residual_mode != 1) return TQ_ERR_INVALID_ARG;
-  if ((s->head_dim != 64 && s->head_dim != 128) || s->qjl_dim != s->head_dim || s->v_qjl != 0) return TQ_ERR_UNSUPPORTED;
+  if (s->v_qjl != 0 && s->v_qjl != 1) return TQ_ERR_INVALID_ARG;
+  if ((s->head_dim != 64 && s->head_dim != 128) || s->qjl_dim != s->head_dim || (s->v_qjl == 1 && s->residual_mode == 1))
+    return TQ_ERR_UNSUPPORTED;
   if (!make_geom(s, g)) return TQ_ERR_INVALID_ARG;
   return TQ_OK;
 }
@@ -79,6 +81,7 @@ static int check_params(const tq_params* p, const tq_shape* s) {
 struct WorkspaceGeom {
   size_t off_counters, off_frags, off_tabs, off_orot, off_partials, total;
   size_t frag_words;
+  size_t rec;  // floats per split-K partial record
 };
 static WorkspaceGeom workspace_geom(const CacheGeom& g, int n_layers_call) {
   WorkspaceGeom w;
@@ -89,7 +92,8 @@ static WorkspaceGeom workspace_geom(const CacheGeom& g, int n_layers_call) {
   w.off_tabs = w.off_frags + (units * w.frag_words * 4 + 255) / 256 * 256;
   w.off_orot = w.off_tabs + ((size_t)n_layers_call * g.H * kTabWords * 4 + 255) / 256 * 256;
   w.off_partials = w.off_orot + (units * g.D * 4 + 255) / 256 * 256;
-  w.total = w.off_partials + units * kMaxSplits * (size_t)(g.D + 2) * 4;
+  w.rec = (size_t)decode_record_floats(g.D, g.vq != 0);
+  w.total = w.off_partials + units * kMaxSplits * w.rec * 4;
   return w;
 }
 
@@ -105,7 +109,7 @@ size_t tq_cache_bytes(const tq_shape* shape) {
 }
 size_t tq_cache_bytes_per_token_head(const tq_shape* shape) {
   CacheGeom g;
-  return check_shape(shape, &g) == TQ_OK ? g.tile_bytes / kTile : 0;
+  return check_shape(shape, &g) == TQ_OK ? (g.tile_bytes + g.vsk_tile_bytes) / kTile : 0;
 }
 size_t tq_cache_seq_len_offset(const tq_shape* shape) {
   CacheGeom g;
@@ -130,10 +134,14 @@ size_t tq_canonical_plane_bytes(const tq_shape* shape, int32_t plane, int32_t n_
       return e * (3 * g.D / 8);
     case 1:
       return e * (g.D / 8);
+    case 6:
+      return g.vq ? e * (g.D / 8) : 0;
     case 2:
     case 3:
     case 5:
       return e * 2;
+    case 7:
+      return g.vq ? e * 2 : 0;
     default:
       return 0;
   }
@@ -218,7 +226,7 @@ static int run_decode(const tq_shape* shape, const tq_params* dev, const tq_cach
     a.frags = ws ? (unsigned*)(ws + w.off_frags) + u0 * w.frag_words : nullptr;
     a.tabs = ws ? (unsigned*)(ws + w.off_tabs) + (size_t)l0 * g.H * kTabWords : nullptr;
     a.orot = nullptr;
-    a.partials = ws ? (float*)(ws + w.off_partials) + u0 * kMaxSplits * (g.D + 2) : nullptr;
+    a.partials = ws ? (float*)(ws + w.off_partials) + u0 * kMaxSplits * w.rec : nullptr;
     a.layer_begin = layer_begin + l0;
     a.n_layers_call = nl;
     a.nsplit = nsplit;
@@ -266,7 +274,7 @@ int tq_cache_export_canonical(const tq_shape* shape, const tq_cache* cache, int3
   if (!cache || !cache->data || !out_dev || layer < 0 || layer >= g.L || n_tokens < 0) return TQ_ERR_INVALID_ARG;
   if (n_tokens > g.max_seq) return TQ_ERR_CAPACITY;
   if (n_tokens > 0 && (!out_dev->k_codes || !out_dev->k_signs || !out_dev->k_norm || !out_dev->k_rnorm ||
-                       !out_dev->v_codes || !out_dev->v_norm))
+                       !out_dev->v_codes || !out_dev->v_norm || (g.vq && (!out_dev->v_signs || !out_dev->v_rnorm))))
     return TQ_ERR_INVALID_ARG;
   if (num_sms() <= 0) return TQ_ERR_CUDA;
   return launch_export(g, make_view(g, cache->data), layer, n_tokens, *out_dev, (cudaStream_t)cuda_stream) == cudaSuccess
@@ -282,7 +290,7 @@ int tq_cache_import_canonical(const tq_shape* shape, tq_cache* cache, int32_t la
   if (!cache || !cache->data || !in_dev || layer < 0 || layer >= g.L || n_tokens < 0) return TQ_ERR_INVALID_ARG;
   if (n_tokens > g.max_seq) return TQ_ERR_CAPACITY;
   if (n_tokens > 0 && (!in_dev->k_codes || !in_dev->k_signs || !in_dev->k_norm || !in_dev->k_rnorm || !in_dev->v_codes ||
-                       !in_dev->v_norm))
+                       !in_dev->v_norm || (g.vq && (!in_dev->v_signs || !in_dev->v_rnorm))))
     return TQ_ERR_INVALID_ARG;
   if (num_sms() <= 0) return TQ_ERR_CUDA;
   return launch_import(g, make_view(g, cache->data), layer, n_tokens, *in_dev, (cudaStream_t)cuda_stream) == cudaSuccess
@@ -350,7 +358,7 @@ static DecodeArgs sub_args(const ModelStepPlan& p, int l0, int nl) {
   b.frags = p.a.frags + u0 * p.w.frag_words;
   b.tabs = p.a.tabs + (size_t)l0 * p.g.H * kTabWords;
   b.orot = p.a.orot + u0 * p.g.D;
-  b.partials = p.a.partials + u0 * kMaxSplits * (p.g.D + 2);
+  b.partials = p.a.partials + u0 * kMaxSplits * p.w.rec;
   b.layer_begin = p.a.layer_begin + l0, b.n_layers_call = nl;
   return b;
 }

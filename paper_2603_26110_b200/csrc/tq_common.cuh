@@ -80,6 +80,29 @@ __host__ __device__ constexpr BitPos v_code_pos(int s, int i) {
   return BitPos{4 * (i & 7) + (pp & 3), 6 * (Layout<D>::C * (pp >> 2) + (i >> 3)) + 3 * (s & 1)};
 }
 
+// ---- V-side sketch tiles (tq_shape.v_qjl = 1; Algorithm 1 line 10) ------------------------------------------
+// A second stream of tiles per unit, one per 32 tokens, next to the main stream (which stays exactly as above):
+//   V signs : KSW words per lane in the A-fragment order of  b[rho] += bits^T (16 sketch rows x 16 tokens) x w' :
+//             sketch row rho = 16 mt + 8 rh + g, token slot s = 16 ks + 8 th + 2 t + e  ->  lane (g, t),
+//             word ks (D/64) + (mt >> 2), bit 16 e + 4 (mt & 3) + 2 rh + th, so that word & (0x00010001 << p) is an
+//             fp16 pair (token 2t [+8 th], token 2t + 1 [+8 th]) of one sketch row with halves 0 or 2^(p - 24);
+//   v_rnorm : one u16 per lane (binary16 |r_v|), lane (g, t) owns slot g + 8 t as for the other norms.
+// 10 (d = 64) / 18 (d = 128) bytes per token.
+template <int D>
+struct VskLayout {
+  static constexpr int KSW = D / 32;
+  static constexpr int kSignBytes = KSW * 4 * kTile;
+  static constexpr int kOffVS = 0;
+  static constexpr int kOffVR = kSignBytes;
+  static constexpr int kTileBytes = kSignBytes + 2 * kTile;  // 320 | 576
+};
+template <int D>
+__host__ __device__ constexpr BitPos vsign_bit_pos(int s, int rho) {
+  const int ks = s >> 4, th = (s >> 3) & 1, t = (s & 7) >> 1, e = s & 1;
+  const int mt = rho >> 4, rh = (rho >> 3) & 1, g = rho & 7;
+  return BitPos{4 * g + t, 32 * (ks * (D / 64) + (mt >> 2)) + 16 * e + 4 * (mt & 3) + 2 * rh + th};
+}
+
 // ---- per-unit operands of the fused decode kernel (written by the prep kernel into the workspace) -------------------
 // The decode kernel feeds q'' and z to mma.sync.m16n8k16 as B fragments in fp16, split hi + lo (column n of B holds
 // the hi part for even n and the lo part for odd n).  A lane (g, t) needs the pattern x = g & 1, t:
@@ -107,6 +130,10 @@ struct CacheGeom {
   size_t stream_bytes;   // tiles_cap * tile_bytes
   size_t total_bytes;
   size_t off_seq_len, off_arrive, off_status;
+  int vq;                   // tq_shape.v_qjl
+  size_t vsk_tile_bytes;    // VskLayout<D>::kTileBytes, 0 when off
+  size_t vsk_stream_bytes;  // tiles_cap * vsk_tile_bytes
+  size_t off_vsk;           // byte offset of the first V-sketch tile
 };
 
 inline __host__ bool make_geom(const tq_shape* s, CacheGeom* g) {
@@ -126,7 +153,11 @@ inline __host__ bool make_geom(const tq_shape* s, CacheGeom* g) {
   g->hdr_bytes = ((2 * lb * 4 + 4) + 255) / 256 * 256;
   g->tile_bytes = g->D == 64 ? Layout<64>::kTileBytes : Layout<128>::kTileBytes;
   g->stream_bytes = (size_t)g->tiles_cap * g->tile_bytes;
-  g->total_bytes = g->hdr_bytes + (size_t)g->L * g->B * g->H * g->stream_bytes;
+  g->vq = s->v_qjl == 1;
+  g->vsk_tile_bytes = !g->vq ? 0 : (g->D == 64 ? VskLayout<64>::kTileBytes : VskLayout<128>::kTileBytes);
+  g->vsk_stream_bytes = (size_t)g->tiles_cap * g->vsk_tile_bytes;
+  g->off_vsk = g->hdr_bytes + (size_t)g->L * g->B * g->H * g->stream_bytes;
+  g->total_bytes = g->off_vsk + (size_t)g->L * g->B * g->H * g->vsk_stream_bytes;
   return true;
 }
 
@@ -138,6 +169,8 @@ struct CacheView {
   int32_t* status;
   int B, H, max_seq, tiles_cap;
   size_t stream_bytes;
+  unsigned char* vsk;       // first V-sketch tile of unit 0, or nullptr (v_qjl = 0)
+  size_t vsk_stream_bytes;
 };
 
 inline __host__ CacheView make_view(const CacheGeom& g, void* data) {
@@ -152,6 +185,8 @@ inline __host__ CacheView make_view(const CacheGeom& g, void* data) {
   v.max_seq = g.max_seq;
   v.tiles_cap = g.tiles_cap;
   v.stream_bytes = g.stream_bytes;
+  v.vsk = g.vq ? p + g.off_vsk : nullptr;
+  v.vsk_stream_bytes = g.vsk_stream_bytes;
   return v;
 }
 
@@ -206,6 +241,7 @@ cudaError_t launch_prep(const DecodeArgs& d, const void* k, const void* v, int D
 cudaError_t launch_decode(const DecodeArgs& a, int D, bool fused_out, cudaStream_t st);
 cudaError_t launch_finish(const DecodeArgs& a, int D, bool programmatic, cudaStream_t st);
 int decode_ctas_per_sm(int D);
+int decode_record_floats(int D, bool vq);  // floats of one split-K partial record
 cudaError_t launch_export(const CacheGeom& g, const CacheView& cv, int layer, int n_tokens, const tq_canonical& out,
                           cudaStream_t st);
 cudaError_t launch_import(const CacheGeom& g, const CacheView& cv, int layer, int n_tokens, const tq_canonical& in,

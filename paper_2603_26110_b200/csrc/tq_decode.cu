@@ -47,23 +47,28 @@ constexpr int kStages = TQ_DECODE_STAGES;  // tile slots per warp
 // Shared-memory map in ABSOLUTE shared-window addresses: the table and ring bases are immediates of the ld.shared
 // instructions, so a lookup address is one LOP3 ((field & mask) | lane * 4).  Dynamic shared memory starts right after
 // the 1 KB the driver reserves; the kernel traps if the window starts later than kAbsMisc.
-template <int D>
+// kVq: the values carry a residual sketch (tq_shape.v_qjl = 1): every ring slot also holds the tile of the V-sketch stream
+// and the per-warp / per-split records carry the sketch accumulator b[m] and the weight sum W'
+template <int D, bool kVq = false>
 struct DecodeCfg {
   using Lo = Layout<D>;
+  using Vs = VskLayout<D>;
+  static constexpr int kSlotBytes = Lo::kTileBytes + (kVq ? Vs::kTileBytes : 0);
+  static constexpr int kRec = kVq ? 2 * D + 3 : D + 2;  // floats of one (m, l, o'[D] [, b[D], W']) record
   static constexpr unsigned kAbsMisc = 1024;   // mbarriers [warps][kStages], weights [warps][2][32] halves, flag
   static constexpr unsigned kAbsBar = kAbsMisc;
-  static constexpr unsigned kAbsWbuf = kAbsMisc + 128;
-  static constexpr unsigned kAbsFlag = kAbsWbuf + kDecodeWarps * 128;
-  static constexpr unsigned kAbsRed = 2048;    // per-warp (m, l, o'[D]) then the merged o [2 D]
-  static constexpr int kRedBytes = kDecodeWarps * (D + 2) * 4 + 2 * D * 4;
+  static constexpr unsigned kAbsWbuf = kAbsMisc + 128;  // per warp [hi | lo][32] halves of w, then the same of w'
+  static constexpr unsigned kAbsFlag = kAbsWbuf + kDecodeWarps * 256;
+  static constexpr unsigned kAbsRed = 2304;    // per-warp records then the merged o [2 D] and t [D]
+  static constexpr int kRedBytes = kDecodeWarps * kRec * 4 + 3 * D * 4;
   static constexpr unsigned kAbsRing = (kAbsRed + kRedBytes + 127) / 128 * 128;
-  static constexpr int kRingBytes = kDecodeWarps * kStages * Lo::kTileBytes;
+  static constexpr int kRingBytes = kDecodeWarps * kStages * kSlotBytes;
   static constexpr unsigned kAbsTab = (kAbsRing + kRingBytes + 255) / 256 * 256;  // K table then V table
   // bytes per table: [64 entries][32 lanes] fp16 pairs, or [64][16] (hi pair, lo pair) for LUTs that are not
   // binary16-representable (64-bit reads are served one half-warp at a time, so 16 columns are conflict free)
   static constexpr int kTabBytes = 64 * 32 * 4;
   static constexpr int kSmemBytes = kAbsTab + 2 * kTabBytes;  // requested dynamic bytes (window start <= 1 KB)
-  static constexpr int kCtasPerSm = D == 64 ? TQ_DECODE_CTAS64 : 2;
+  static constexpr int kCtasPerSm = D == 64 ? (kVq ? 4 : TQ_DECODE_CTAS64) : 2;
 };
 
 // ---- small PTX helpers --------------------------------------------------------------------------------------------
@@ -114,6 +119,18 @@ __device__ __forceinline__ void tma_load_tile(unsigned dst, const void* src, uns
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
                "l"(src), "r"(bytes), "r"(bar)
+               : "memory");
+}
+
+// the same for a main tile and its V-sketch tile: two copies into one slot, one transaction count
+__device__ __forceinline__ void tma_load_tile2(unsigned dst, const void* src, unsigned bytes, const void* src2, unsigned bytes2,
+                                               unsigned bar) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes + bytes2) : "memory");
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+               "l"(src), "r"(bytes), "r"(bar)
+               : "memory");
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst + bytes),
+               "l"(src2), "r"(bytes2), "r"(bar)
                : "memory");
 }
 
@@ -195,10 +212,10 @@ __device__ __forceinline__ void load_frags(UnitFrags<D>& f, const unsigned* fb, 
 // ---- one 32-token tile ------------------------------------------------------------------------------------------------
 // kFast: the LUT entries are binary16-representable, the tables hold fp16 pairs (one 32-bit read per field);
 // otherwise they hold (hi pair, lo pair) and every field costs one 64-bit read and two MMAs.
-template <int D, bool kFast>
+template <int D, bool kFast, bool kVq>
 struct TileMath {
   using Lo = Layout<D>;
-  using Cfg = DecodeCfg<D>;
+  using Cfg = DecodeCfg<D, kVq>;
   static constexpr int KS = D / 16;       // k-steps of the K / sign contractions
   static constexpr int MV = D / 16;       // m-tiles (16 coordinates each) of the V contraction
   static constexpr int LS = 7;            // log2 of the table row pitch (32 lanes x 4 bytes | 16 x 8 bytes)
@@ -281,26 +298,29 @@ __device__ __forceinline__ void lds_words(unsigned (&dst)[W], unsigned sec, int 
 }
 
 // ---- the streaming loop of one warp -----------------------------------------------------------------------------------
-template <int D, bool kFast>
-__device__ __forceinline__ void stream_tiles(const unsigned char* stream, int tile_first, int tile1, int T, int warp, int lane,
-                                             const UnitFrags<D>& f, float& m_out, float& l_out, float (&o)[D / 16][4]) {
+template <int D, bool kFast, bool kVq>
+__device__ __forceinline__ void stream_tiles(const unsigned char* stream, const unsigned char* vstream, int tile_first, int tile1, int T,
+                                             int warp, int lane, const UnitFrags<D>& f, float& m_out, float& l_out,
+                                             float (&o)[D / 16][4], float (&ob)[D / 16][4], float& wsum_out) {
   using Lo = Layout<D>;
-  using Cfg = DecodeCfg<D>;
-  using TM = TileMath<D, kFast>;
+  using Vs = VskLayout<D>;
+  using Cfg = DecodeCfg<D, kVq>;
+  using TM = TileMath<D, kFast, kVq>;
   constexpr int NW = kDecodeWarps;
   const int t = lane & 3;
   const unsigned lane_off = kFast ? (unsigned)lane << 2 : (unsigned)(lane & 15) << 3;  // table column of this lane
-  const unsigned ring = Cfg::kAbsRing + warp * kStages * Lo::kTileBytes;
+  const unsigned ring = Cfg::kAbsRing + warp * kStages * Cfg::kSlotBytes;
   const unsigned bar0 = Cfg::kAbsBar + warp * kStages * 8;
-  const unsigned wbuf = Cfg::kAbsWbuf + warp * 128;  // [hi | lo][32 slots] binary16
+  const unsigned wbuf = Cfg::kAbsWbuf + warp * 256;  // [hi | lo][32 slots] binary16 of w, then of w'
   const int my_slot = lane_slot(lane);
-  float m = -INFINITY, l = 0.f;
+  float m = -INFINITY, l = 0.f, wsum = 0.f;
 
   // ring state: slot image and barrier of the tile at hand, phase parity of this round over the ring, and the global
   // address of the tile kStages rounds ahead
   unsigned img = ring, bar = bar0, parity = 0;
   int st = 0;
   const unsigned char* src_next = stream + (size_t)(tile_first + kStages * NW) * Lo::kTileBytes;
+  [[maybe_unused]] const unsigned char* vsrc_next = kVq ? vstream + (size_t)(tile_first + kStages * NW) * Vs::kTileBytes : nullptr;
   for (int tile = tile_first; tile < tile1; tile += NW) {
     mbar_wait(bar, parity);
 
@@ -339,9 +359,22 @@ __device__ __forceinline__ void stream_tiles(const unsigned char* stream, int ti
       for (int i = 0; i < D / 16; ++i)
 #pragma unroll
         for (int j = 0; j < 4; ++j) o[i][j] *= fsc;
+      if constexpr (kVq) {
+#pragma unroll
+        for (int i = 0; i < D / 16; ++i)
+#pragma unroll
+          for (int j = 0; j < 4; ++j) ob[i][j] *= fsc;
+      }
     }
     m = mnew;
     const float wv = valid ? p * f16_bits_to_f32(nv) : 0.f;
+    [[maybe_unused]] float wq = 0.f;  // w' = w |r_v|: the weight of this token's value sign bits
+    if constexpr (kVq) {
+      unsigned short gv;
+      asm volatile("ld.shared.u16 %0, [%1];" : "=h"(gv) : "r"(img + Lo::kTileBytes + Vs::kOffVR + lane * 2) : "memory");
+      wq = wv * f16_bits_to_f32(gv);
+      wsum = fmaf(wsum, fsc, wq);
+    }
     const unsigned nz = __ballot_sync(0xffffffffu, wv != 0.f);
     if (nz) {
       // hand the weights from lane = slot to the B-fragment order (tokens 2t, 2t+1, 2t+8, 2t+9 of each k-step) through
@@ -351,6 +384,12 @@ __device__ __forceinline__ void stream_tiles(const unsigned char* stream, int ti
       __syncwarp();
       asm volatile("st.shared.u16 [%0], %1;" ::"r"(wbuf + my_slot * 2), "h"(__half_as_ushort(wh)) : "memory");
       asm volatile("st.shared.u16 [%0], %1;" ::"r"(wbuf + 64 + my_slot * 2), "h"(__half_as_ushort(wl)) : "memory");
+      if constexpr (kVq) {  // tokens of the upper half of a k-step sit one bit higher in the sign words: halve their weight
+        __half qh, ql;
+        split_h((my_slot & 8) ? 0.5f * wq : wq, qh, ql);
+        asm volatile("st.shared.u16 [%0], %1;" ::"r"(wbuf + 128 + my_slot * 2), "h"(__half_as_ushort(qh)) : "memory");
+        asm volatile("st.shared.u16 [%0], %1;" ::"r"(wbuf + 192 + my_slot * 2), "h"(__half_as_ushort(ql)) : "memory");
+      }
       __syncwarp();
       unsigned vw[Lo::KCW];
       lds_words<Lo::KCW>(vw, img + Lo::kOffVC, lane);
@@ -368,16 +407,42 @@ __device__ __forceinline__ void stream_tiles(const unsigned char* stream, int ti
         asm volatile("ld.shared.u32 %0, [%1+48];" : "=r"(b1) : "r"(wsrc) : "memory");
         TM::template values<1>(vw, lane_off, b0, b1, o, std::make_integer_sequence<int, D / 16>{});
       }
+      if constexpr (kVq) {
+        // ---- value sign bits: ob[mt] += bits (16 sketch rows x 16 tokens of k-step ks) x w'; word ks (D/64) + (mt >> 2),
+        //      bit 4 (mt & 3) + {0: row g, 2: row g + 8} + {0: tokens 2t, 2t+1; 1: tokens 2t+8, 2t+9} (+16 for the odd token)
+        unsigned vsw[Vs::KSW];
+        lds_words<Vs::KSW>(vsw, img + Lo::kTileBytes + Vs::kOffVS, lane);
+#pragma unroll
+        for (int ks = 0; ks < 2; ++ks) {
+          if (!(nz & (ks == 0 ? 0x33333333u : 0xccccccccu))) continue;
+          unsigned b0, b1;
+          asm volatile("ld.shared.u32 %0, [%1];" : "=r"(b0) : "r"(wsrc + 128 + 32 * ks) : "memory");
+          asm volatile("ld.shared.u32 %0, [%1];" : "=r"(b1) : "r"(wsrc + 128 + 32 * ks + 16) : "memory");
+#pragma unroll
+          for (int mt = 0; mt < D / 16; ++mt) {
+            // the upper byte of each half is brought down first: only bits 0..9 of an fp16 are plain 2^(p - 24) subnormals
+            const unsigned wd = (mt & 2) ? vsw[ks * (D / 64) + (mt >> 2)] >> 8 : vsw[ks * (D / 64) + (mt >> 2)];
+            const int p0 = 4 * (mt & 1);
+            mma16816(ob[mt], wd & (0x00010001u << p0), wd & (0x00010001u << (p0 + 2)), wd & (0x00010001u << (p0 + 1)),
+                     wd & (0x00010001u << (p0 + 3)), b0, b1);
+          }
+        }
+      }
     }
     // ---- the slot is consumed (every word of the image has been used): refill it with the tile kStages rounds ahead
     __syncwarp();
-    if (lane == 0 && tile + kStages * NW < tile1) tma_load_tile(img, src_next, Lo::kTileBytes, bar);
+    if (lane == 0 && tile + kStages * NW < tile1) {
+      if constexpr (kVq) tma_load_tile2(img, src_next, Lo::kTileBytes, vsrc_next, Vs::kTileBytes, bar);
+      else tma_load_tile(img, src_next, Lo::kTileBytes, bar);
+    }
     src_next += NW * Lo::kTileBytes;
-    img += Lo::kTileBytes, bar += 8;
+    if constexpr (kVq) vsrc_next += NW * Vs::kTileBytes;
+    img += Cfg::kSlotBytes, bar += 8;
     if (++st == kStages) st = 0, img = ring, bar = bar0, parity ^= 1u;
   }
   m_out = m;
   l_out = l;
+  wsum_out = wsum;
 }
 
 // ---- the streaming kernel ------------------------------------------------------------------------------------
@@ -386,17 +451,19 @@ __device__ __forceinline__ void stream_tiles(const unsigned char* stream, int ti
 // leaves the trailing splits empty.  The four warps take tiles round-robin.
 // kFusedOut: the finishing CTA applies PI_V^T and writes `out` (per-layer calls); otherwise it leaves o'/l in the
 // workspace and finish_kernel rotates every unit of the step at once (tq_decode_model_step).
-template <int D, typename TIO, bool kFusedOut>
-__global__ void __launch_bounds__(kDecodeThreads, DecodeCfg<D>::kCtasPerSm) decode_main_kernel(DecodeArgs a) {
+template <int D, typename TIO, bool kFusedOut, bool kVq>
+__global__ void __launch_bounds__(kDecodeThreads, DecodeCfg<D, kVq>::kCtasPerSm) decode_main_kernel(DecodeArgs a) {
   using Lo = Layout<D>;
-  using Cfg = DecodeCfg<D>;
-  constexpr int NW = kDecodeWarps;
+  using Vs = VskLayout<D>;
+  using Cfg = DecodeCfg<D, kVq>;
+  constexpr int NW = kDecodeWarps, REC = Cfg::kRec;
   extern __shared__ unsigned char smem_raw[];
   const unsigned raw = (unsigned)__cvta_generic_to_shared(smem_raw);
   if (raw > Cfg::kAbsMisc) __trap();  // the fixed shared-memory map does not fit: fail loudly
   unsigned char* abs0 = smem_raw - raw;  // generic pointer to absolute shared address 0 of this CTA's window
-  float* red = reinterpret_cast<float*>(abs0 + Cfg::kAbsRed);  // NW x (D + 2)
-  float* omerged = red + NW * (D + 2);                          // [D] + [D] partial matvec
+  float* red = reinterpret_cast<float*>(abs0 + Cfg::kAbsRed);  // NW records
+  float* omerged = red + NW * REC;                              // [D] + [D] partial matvec
+  [[maybe_unused]] float* tmerged = omerged + 2 * D;            // [D] sketch vector t = 2 b - W'
   int* flag = reinterpret_cast<int*>(abs0 + Cfg::kAbsFlag);
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -410,6 +477,7 @@ __global__ void __launch_bounds__(kDecodeThreads, DecodeCfg<D>::kCtasPerSm) deco
   const int per = a.per, tile0 = sp * per;
   const int cap1 = sp == nsplit - 1 ? a.cv.tiles_cap : min(a.cv.tiles_cap, tile0 + per);  // static bound of this split
   const unsigned char* stream = a.cv.tiles + (((size_t)layer * B + b) * H + h) * a.cv.stream_bytes;
+  [[maybe_unused]] const unsigned char* vstream = kVq ? a.cv.vsk + (((size_t)layer * B + b) * H + h) * a.cv.vsk_stream_bytes : nullptr;
 
   if (lane == 0) {
 #pragma unroll
@@ -434,9 +502,14 @@ __global__ void __launch_bounds__(kDecodeThreads, DecodeCfg<D>::kCtasPerSm) deco
 #pragma unroll
     for (int i = 0; i < kStages; ++i) {
       const int tl = tile0 + warp + i * NW;
-      if (tl < cap1)
-        tma_load_tile(Cfg::kAbsRing + (warp * kStages + i) * Lo::kTileBytes, stream + (size_t)tl * Lo::kTileBytes, Lo::kTileBytes,
-                      Cfg::kAbsBar + (warp * kStages + i) * 8);
+      if (tl < cap1) {
+        if constexpr (kVq)
+          tma_load_tile2(Cfg::kAbsRing + (warp * kStages + i) * Cfg::kSlotBytes, stream + (size_t)tl * Lo::kTileBytes, Lo::kTileBytes,
+                         vstream + (size_t)tl * Vs::kTileBytes, Vs::kTileBytes, Cfg::kAbsBar + (warp * kStages + i) * 8);
+        else
+          tma_load_tile(Cfg::kAbsRing + (warp * kStages + i) * Lo::kTileBytes, stream + (size_t)tl * Lo::kTileBytes, Lo::kTileBytes,
+                        Cfg::kAbsBar + (warp * kStages + i) * 8);
+      }
     }
   }
   int T;
@@ -494,17 +567,24 @@ __global__ void __launch_bounds__(kDecodeThreads, DecodeCfg<D>::kCtasPerSm) deco
   for (int i = 0; i < D / 16; ++i)
 #pragma unroll
     for (int j = 0; j < 4; ++j) o[i][j] = 0.f;
-  float m, l;
-  if (fast) stream_tiles<D, true>(stream, tile0 + warp, tile1, T, warp, lane, fr, m, l, o);
-  else stream_tiles<D, false>(stream, tile0 + warp, tile1, T, warp, lane, fr, m, l, o);
+  float ob[D / 16][4];  // sketch accumulator (kVq)
+#pragma unroll
+  for (int i = 0; i < D / 16; ++i)
+#pragma unroll
+    for (int j = 0; j < 4; ++j) ob[i][j] = 0.f;
+  float m, l, wsum;
+  if (fast) stream_tiles<D, true, kVq>(stream, vstream, tile0 + warp, tile1, T, warp, lane, fr, m, l, o, ob, wsum);
+  else stream_tiles<D, false, kVq>(stream, vstream, tile0 + warp, tile1, T, warp, lane, fr, m, l, o, ob, wsum);
 
   // ---- reduce over the CTA's warps.  o[mt] = {coordinate 16 mt + g: hi, lo; coordinate 16 mt + g + 8: hi, lo}, the same
   //      in all four lanes of a quad
   l = warp_sum(l);
-  float* wr = red + warp * (D + 2);
+  if constexpr (kVq) wsum = warp_sum(wsum);
+  float* wr = red + warp * REC;
   if (lane == 0) {
     wr[0] = m;
     wr[1] = l;
+    if constexpr (kVq) wr[2 + 2 * D] = wsum;
   }
   if ((lane & 3) == 0) {
     const int g = lane >> 2;
@@ -512,28 +592,40 @@ __global__ void __launch_bounds__(kDecodeThreads, DecodeCfg<D>::kCtasPerSm) deco
     for (int mt = 0; mt < D / 16; ++mt) {
       wr[2 + 16 * mt + g] = o[mt][0] + o[mt][1];
       wr[2 + 16 * mt + g + 8] = o[mt][2] + o[mt][3];
+      if constexpr (kVq) {  // undo the 2^(p - 24) of the sign bits: row g sat at bit 4 (mt & 1), row g + 8 two bits higher
+        wr[2 + D + 16 * mt + g] = (ob[mt][0] + ob[mt][1]) * pow2i(24 - 4 * (mt & 1));
+        wr[2 + D + 16 * mt + g + 8] = (ob[mt][2] + ob[mt][3]) * pow2i(22 - 4 * (mt & 1));
+      }
     }
   }
   __syncthreads();
   float M = -INFINITY;
 #pragma unroll
-  for (int w = 0; w < NW; ++w) M = fmaxf(M, red[w * (D + 2)]);
-  float Lsum = 0.f, oi = 0.f;
+  for (int w = 0; w < NW; ++w) M = fmaxf(M, red[w * REC]);
+  float Lsum = 0.f, oi = 0.f, bi = 0.f, Wq = 0.f;  // bi: sketch accumulator row tid; Wq: sum of the sketch weights
   if (tid < D) {
 #pragma unroll
     for (int w = 0; w < NW; ++w) {
-      const float mw = red[w * (D + 2)];
+      const float mw = red[w * REC];
       const float fw = mw == -INFINITY ? 0.f : ex2_ftz(mw - M);
-      Lsum = fmaf(red[w * (D + 2) + 1], fw, Lsum);
-      oi = fmaf(red[w * (D + 2) + 2 + tid], fw, oi);
+      Lsum = fmaf(red[w * REC + 1], fw, Lsum);
+      oi = fmaf(red[w * REC + 2 + tid], fw, oi);
+      if constexpr (kVq) {
+        bi = fmaf(red[w * REC + 2 + D + tid], fw, bi);
+        Wq = fmaf(red[w * REC + 2 + 2 * D], fw, Wq);
+      }
     }
   }
   if (nseg > 1) {
-    float* part = a.partials + ((size_t)uc * kMaxSegments + sp) * (D + 2);
-    if (tid < D) part[2 + tid] = oi;
+    float* part = a.partials + ((size_t)uc * kMaxSegments + sp) * REC;
+    if (tid < D) {
+      part[2 + tid] = oi;
+      if constexpr (kVq) part[2 + D + tid] = bi;
+    }
     if (tid == 0) {
       part[0] = M;
       part[1] = Lsum;
+      if constexpr (kVq) part[2 + 2 * D] = Wq;
     }
     __syncthreads();
     if (tid == 0) {  // release: the barrier orders the CTA's partial stores before this fence (cumulativity)
@@ -548,18 +640,37 @@ __global__ void __launch_bounds__(kDecodeThreads, DecodeCfg<D>::kCtasPerSm) deco
       if (a.chain_mode != 0) pdl_wait();
       return;
     }
-    const float* pp = a.partials + (size_t)uc * kMaxSegments * (D + 2);
+    const float* pp = a.partials + (size_t)uc * kMaxSegments * REC;
     M = -INFINITY;
-    for (int s = 0; s < nseg; ++s) M = fmaxf(M, __ldcg(pp + s * (D + 2)));
+    for (int s = 0; s < nseg; ++s) M = fmaxf(M, __ldcg(pp + s * REC));
     Lsum = 0.f;
-    oi = 0.f;
+    oi = 0.f, bi = 0.f, Wq = 0.f;
     if (tid < D) {
       for (int s = 0; s < nseg; ++s) {
-        const float ms = __ldcg(pp + s * (D + 2));
+        const float ms = __ldcg(pp + s * REC);
         const float fs = ms == -INFINITY ? 0.f : ex2_ftz(ms - M);
-        Lsum = fmaf(__ldcg(pp + s * (D + 2) + 1), fs, Lsum);
-        oi = fmaf(__ldcg(pp + s * (D + 2) + 2 + tid), fs, oi);
+        Lsum = fmaf(__ldcg(pp + s * REC + 1), fs, Lsum);
+        oi = fmaf(__ldcg(pp + s * REC + 2 + tid), fs, oi);
+        if constexpr (kVq) {
+          bi = fmaf(__ldcg(pp + s * REC + 2 + D + tid), fs, bi);
+          Wq = fmaf(__ldcg(pp + s * REC + 2 + 2 * D), fs, Wq);
+        }
       }
+    }
+  }
+  if constexpr (kVq) {
+    // ---- o' += sqrt(pi/2)/m S^T t, t = sum_j w'_j sigma_j = 2 b - W' (sigma = 2 bits - 1): thread i owns coordinate i and
+    //      column i of S (coalesced over the CTA)
+    if (tid < D) tmerged[tid] = 2.f * bi - Wq;
+    __syncthreads();
+    if (tid < D) {
+      float acc0 = 0.f, acc1 = 0.f;
+#pragma unroll 8
+      for (int rho = 0; rho < D; rho += 2) {
+        acc0 = fmaf(__ldg(a.S + (size_t)rho * D + tid), tmerged[rho], acc0);
+        acc1 = fmaf(__ldg(a.S + (size_t)(rho + 1) * D + tid), tmerged[rho + 1], acc1);
+      }
+      oi = fmaf(acc0 + acc1, (D == 64 ? 0.01958303339555469f : 0.009791516697777345f), oi);  // sqrt(pi/2) / m
     }
   }
   if constexpr (!kFusedOut) {
@@ -655,11 +766,11 @@ __global__ void __launch_bounds__(D) finish_kernel(DecodeArgs a, int nbg) {
 }
 
 // ------------------------------------------------------------------------------------------ launchers
-template <int D, typename T, bool kFusedOut>
+template <int D, typename T, bool kFusedOut, bool kVq>
 static cudaError_t launch_decode_t(const DecodeArgs& a, cudaStream_t st) {
-  constexpr int smem = DecodeCfg<D>::kSmemBytes;
+  constexpr int smem = DecodeCfg<D, kVq>::kSmemBytes;
   // per launch: the attribute is per device and a process may drive several
-  cudaError_t e = cudaFuncSetAttribute(decode_main_kernel<D, T, kFusedOut>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+  cudaError_t e = cudaFuncSetAttribute(decode_main_kernel<D, T, kFusedOut, kVq>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
   if (e != cudaSuccess) return e;
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3(a.nsplit, a.cv.H, a.n_layers_call * a.cv.B);
@@ -671,7 +782,7 @@ static cudaError_t launch_decode_t(const DecodeArgs& a, cudaStream_t st) {
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  e = cudaLaunchKernelEx(&cfg, decode_main_kernel<D, T, kFusedOut>, a);
+  e = cudaLaunchKernelEx(&cfg, decode_main_kernel<D, T, kFusedOut, kVq>, a);
   count_launch();
   return e != cudaSuccess ? e : cudaGetLastError();
 }
@@ -700,13 +811,20 @@ cudaError_t launch_finish(const DecodeArgs& a, int D, bool programmatic, cudaStr
 
 int decode_ctas_per_sm(int D) { return D == 64 ? DecodeCfg<64>::kCtasPerSm : DecodeCfg<128>::kCtasPerSm; }
 
-cudaError_t launch_decode(const DecodeArgs& a, int D, bool fused_out, cudaStream_t st) {
+template <bool kVq>
+static cudaError_t launch_decode_v(const DecodeArgs& a, int D, bool fused_out, cudaStream_t st) {
   if (fused_out) {
-    if (D == 64) return a.dt == TQ_F16 ? launch_decode_t<64, __half, true>(a, st) : launch_decode_t<64, float, true>(a, st);
-    return a.dt == TQ_F16 ? launch_decode_t<128, __half, true>(a, st) : launch_decode_t<128, float, true>(a, st);
+    if (D == 64) return a.dt == TQ_F16 ? launch_decode_t<64, __half, true, kVq>(a, st) : launch_decode_t<64, float, true, kVq>(a, st);
+    return a.dt == TQ_F16 ? launch_decode_t<128, __half, true, kVq>(a, st) : launch_decode_t<128, float, true, kVq>(a, st);
   }
-  if (D == 64) return launch_decode_t<64, __half, false>(a, st);  // the output type is finish_kernel's business
-  return launch_decode_t<128, __half, false>(a, st);
+  if (D == 64) return launch_decode_t<64, __half, false, kVq>(a, st);  // the output type is finish_kernel's business
+  return launch_decode_t<128, __half, false, kVq>(a, st);
 }
+
+cudaError_t launch_decode(const DecodeArgs& a, int D, bool fused_out, cudaStream_t st) {
+  return a.cv.vsk ? launch_decode_v<true>(a, D, fused_out, st) : launch_decode_v<false>(a, D, fused_out, st);
+}
+
+int decode_record_floats(int D, bool vq) { return vq ? 2 * D + 3 : D + 2; }
 
 }  // namespace tq

@@ -66,6 +66,20 @@ __global__ void export_kernel(CacheView cv, int layer, int n_tokens, tq_canonica
   out.k_norm[idx] = (unsigned short)(nk & 0xffffu);
   out.k_rnorm[idx] = (unsigned short)(nk >> 16);
   out.v_norm[idx] = ((const unsigned short*)(tile + Lo::kOffVN))[nl];
+  if (cv.vsk) {  // V-side sketch tiles
+    using Vs = VskLayout<D>;
+    const unsigned char* vt = cv.vsk + unit * cv.vsk_stream_bytes + (size_t)(t / kTile) * Vs::kTileBytes;
+    unsigned char* vs = out.v_signs + (size_t)idx * (D / 8);
+    for (int byte = 0; byte < D / 8; ++byte) {
+      unsigned v = 0;
+      for (int k = 0; k < 8; ++k) {
+        const BitPos sp = vsign_bit_pos<D>(slot, 8 * byte + k);
+        v |= sec_get(vt + Vs::kOffVS, Vs::KSW, sp.lane, sp.bit, 1) << k;
+      }
+      vs[byte] = (unsigned char)v;
+    }
+    out.v_rnorm[idx] = ((const unsigned short*)(vt + Vs::kOffVR))[nl];
+  }
 }
 
 // one thread per (b, h, tile, lane): assembles that lane's word strings from the canonical planes; the bits of
@@ -137,6 +151,23 @@ __global__ void import_kernel(CacheView cv, int layer, int n_tokens, tq_canonica
   if (in_call(s)) {
     ((unsigned*)(tile + Lo::kOffNK))[lane] = (unsigned)in.k_norm[tok0 + s] | ((unsigned)in.k_rnorm[tok0 + s] << 16);
     ((unsigned short*)(tile + Lo::kOffVN))[lane] = in.v_norm[tok0 + s];
+  }
+  if (cv.vsk) {  // V-side sketch tiles: this lane's sketch rows g + 8 q of the tokens 2t + e + 8 th + 16 ks
+    using Vs = VskLayout<D>;
+    unsigned char* vt = cv.vsk + unit * cv.vsk_stream_bytes + (size_t)tl * Vs::kTileBytes;
+    for (int w = 0; w <= Lo::KCW; ++w) words[w] = 0, keep[w] = 0;
+    for (int sq = 0; sq < 8; ++sq) {
+      const int sv = 16 * (sq >> 2) + 8 * ((sq >> 1) & 1) + 2 * t + (sq & 1);
+      if (!in_call(sv)) continue;
+      const unsigned char* vsg = in.v_signs + (tok0 + sv) * (D / 8);
+      for (int q = 0; q < D / 8; ++q) {
+        const int rho = g + 8 * q;
+        or_bits(words, vsign_bit_pos<D>(sv, rho).bit, 1, stream_get(vsg, rho, 1));
+        or_bits(keep, vsign_bit_pos<D>(sv, rho).bit, 1, 1u);
+      }
+    }
+    flush(vt + Vs::kOffVS, Vs::KSW);
+    if (in_call(s)) ((unsigned short*)(vt + Vs::kOffVR))[lane] = in.v_rnorm[tok0 + s];
   }
 }
 

@@ -146,7 +146,7 @@ __global__ void __launch_bounds__(kPrepThreads) prep_kernel(PrepArgs a) {
   unsigned char (*cK)[D] = reinterpret_cast<unsigned char (*)[D]>(Y + (size_t)Cfg::ROWS * Cfg::FP);
   unsigned char (*cV)[D] = cK + EB;
   __shared__ float rscale[Cfg::ROWS];  // accumulator -> result, per operand row
-  __shared__ float nrm[3][EB];         // |k|, |r|, |v| of the appended token
+  __shared__ float nrm[4][EB];         // |k|, |r_k|, |v|, |r_v| of the appended token
   __shared__ float qsc[EB][2];         // 2^eq (scaling of the q'' operand rows), reserved
   __shared__ float lutK[8], lutV[8];
   __shared__ int s_len0[EB], s_full[EB];
@@ -163,6 +163,7 @@ __global__ void __launch_bounds__(kPrepThreads) prep_kernel(PrepArgs a) {
   auto unit_of = [&](int e) { return ((size_t)lc * B + b0 + e) * H + h; };        // unit inside the call (q, k, v, out, operands)
   auto stream_of = [&](int e) { return ((size_t)layer * B + b0 + e) * H + h; };  // unit inside the cache
 
+  const bool vsk = kAppend && a.cv.vsk != nullptr;  // V-side sketch (tq_shape.v_qjl = 1)
   pdl_trigger();  // the streaming kernel behind this one may be scheduled
   if constexpr (EB == 8) {  // rows [24, 32) pad the value block to a whole m-tile
     for (int idx = tid; idx < 8 * Cfg::HP / 2; idx += NT) {
@@ -381,19 +382,37 @@ __global__ void __launch_bounds__(kPrepThreads) prep_kernel(PrepArgs a) {
         *reinterpret_cast<unsigned*>(Al + (size_t)yrow * Cfg::HP + i0) = lo;
       } else {
         cV[e][i0] = (unsigned char)c0, cV[e][i0 + 1] = (unsigned char)c1;
+        if (vsk) {  // V-side sketch: the residual of the value becomes an operand row of the S product too
+          const float r0 = u0 - lut[c0], r1 = u1 - lut[c1];
+          g2 = fmaf(r0, r0, fmaf(r1, r1, g2));
+          unsigned hi, lo;
+          split_pair(r0 * 8.f, r1 * 8.f, hi, lo);
+          *reinterpret_cast<unsigned*>(Ah + (size_t)yrow * Cfg::HP + i0) = hi;
+          *reinterpret_cast<unsigned*>(Al + (size_t)yrow * Cfg::HP + i0) = lo;
+        }
       }
     }
     if (vec == 0) {
       g2 = warp_sum(g2);
       if (lane == 0) nrm[0][e] = n, nrm[1][e] = sqrtf(g2), rscale[yrow] = 1.f;
-    } else if (lane == 0) {
-      nrm[2][e] = n;
+    } else {
+      if (vsk) g2 = warp_sum(g2);
+      if (lane == 0) {
+        nrm[2][e] = n;
+        if (vsk) nrm[3][e] = sqrtf(g2), rscale[yrow] = 1.f;
+      }
     }
   }
   __syncthreads();
 
-  // ---- stage 4: [r rows; q'' rows] x S^T -> sign bits | z
-  for (int nt = warp; nt < D / 8; nt += NW) kq_product(a.S, 1.f, 8 * nt);
+  // ---- stage 4: [r rows; q'' rows] x S^T -> sign bits | z   (and the value residual rows with the V-side sketch)
+  for (int nt = warp; nt < D / 8; nt += NW) {
+    kq_product(a.S, 1.f, 8 * nt);
+    if (kAppend && vsk) {
+      if (EB == 8 || mt_n == 1) gemm_rows<D, Cfg::HP, 1, true>(Ah, Al, 2 * EB, a.S, 1.f, 8 * nt, Y, rscale, lane);
+      else gemm_rows<D, Cfg::HP, 2, true>(Ah, Al, 2 * EB, a.S, 1.f, 8 * nt, Y, rscale, lane);
+    }
+  }
   __syncthreads();
 
   if (kQuery) {
@@ -532,6 +551,34 @@ __global__ void __launch_bounds__(kPrepThreads) prep_kernel(PrepArgs a) {
         unsigned short* vptr = reinterpret_cast<unsigned short*>(tp + Lo::kOffVC + word_offset(Lo::KCW, hidx >> 1, 4 * gi + (pp & 3))) + (hidx & 1);
         *vptr = (unsigned short)((vold[hw] & ~mk) | v);
       }
+    }
+  }
+  if (vsk) {
+    // V-side sketch tile: the token's bit of sketch row rho sits in lane (rho & 7, t of the slot), word ks (D/64) + (mt >> 2),
+    // bit 16 e + 4 (mt & 3) + 2 rh + th: one lane per (g, word) clears the token's eight bits of that word and sets the new ones
+    using Vs = VskLayout<D>;
+    constexpr int WPT = 8 * (D / 64);  // words a token touches
+    for (int k = 0; k < EPW; ++k) {
+      const int e = warp + k * NW;
+      if (e >= nb || s_full[e] || lane >= WPT) continue;
+      const int len = s_len0[e], slot = len % kTile;
+      unsigned char* vt = a.cv.vsk + stream_of(e) * a.cv.vsk_stream_bytes + (size_t)(len / kTile) * Vs::kTileBytes;
+      const int ks = slot >> 4, th = (slot >> 3) & 1, ts = (slot & 7) >> 1, eo = slot & 1;
+      const int g = lane & 7, wsel = lane >> 3;  // wsel = mt >> 2
+      const float* sr = Y + (size_t)(2 * EB + e) * Cfg::FP;  // S r_v of this entry
+      unsigned own = 0u, bits = 0u;
+#pragma unroll
+      for (int mq = 0; mq < 4; ++mq)
+#pragma unroll
+        for (int rh = 0; rh < 2; ++rh) {
+          const int mt = 4 * wsel + mq;
+          const unsigned pos = 16u * eo + 4u * mq + 2u * rh + th;
+          own |= 1u << pos;
+          bits |= (sr[16 * mt + 8 * rh + g] >= 0.f ? 1u : 0u) << pos;
+        }
+      unsigned* wp = reinterpret_cast<unsigned*>(vt + Vs::kOffVS + word_offset(Vs::KSW, ks * (D / 64) + wsel, 4 * g + ts));
+      *wp = (__ldcg(wp) & ~own) | bits;
+      if (lane == 0) reinterpret_cast<unsigned short*>(vt + Vs::kOffVR)[slot_lane(slot)] = f32_to_f16_bits_clamped(nrm[3][e]);
     }
   }
   if (lane < EPW) {

@@ -305,7 +305,7 @@ cudaError_t launch_quantize_pack(const QuantArgs& a, int D, tq_dtype dt, int num
   // the tensor-core kernel (tq_quantize_tc.cu) is the product path; tq_debug_set_quantize_impl(1) selects the CUDA-core
   // kernel of this file (kept as a cross-check)
   // (the cross-check kernel only knows the default residual mode)
-  const bool force_fp32 = g_debug_quantize_fp32.load(std::memory_order_relaxed) != 0 && !a.literal;
+  const bool force_fp32 = g_debug_quantize_fp32.load(std::memory_order_relaxed) != 0 && !a.literal && !a.cv.vsk;
 #ifndef TQ_NO_TC_QUANTIZE
   if (!force_fp32) return launch_quantize_pack_tc(a, D, dt, num_sms, st);
 #endif

@@ -313,7 +313,10 @@ __device__ __forceinline__ void stage_rows(const T* __restrict__ src, int i_firs
 
 // kLit: the paper-literal Eq. 6-7 mode (include/tq.h): the accumulator is compared as it stands (no normalisation), the
 // norm plane is 1.0 and the rnorm plane the per-head constant e-bar m sqrt(2/pi)
-template <int D, typename T, bool kKey, bool kLit>
+// kVq: the values carry a residual sketch too (tq_shape.v_qjl = 1): the value CTAs then run the S product on 8 r_v and
+// drop its sign bits into the V-sketch tile (tq_common.cuh VskLayout), whose image lives in the unused tail of the
+// value CTA's tile image
+template <int D, typename T, bool kKey, bool kLit, bool kVq>
 __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int blocks_per_cta, int cta_x, unsigned char* smem) {
   using Cfg = TcCfg<D>;
   using Lo = Layout<D>;
@@ -357,6 +360,7 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
     stage_matrix<D>(B1_hi, B1_lo, a.S, 1.f, tid);
   } else {
     stage_matrix<D>(B0_hi, B0_lo, a.pi_v + (size_t)h * D * D, 16.f, tid);
+    if constexpr (kVq) stage_matrix<D>(B1_hi, B1_lo, a.S, 1.f, tid);
   }
   // thresholds t_k = (lut_k + lut_{k+1}) / 2 in fp32, as search constants; keys also keep a table of LUT pairs for the
   // residual: the S product takes 8 r (only sign(S r) is used, and 8 r splits cleanly in fp16), |r| = |8 r| / 8
@@ -370,7 +374,7 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
 #pragma unroll
     for (int q = 0; q < 7; ++q) thr[q] = 0.5f * (l8[q] + l8[q + 1]);
     search0 = make_search(thr);
-    if (kKey && tid < 64) lutp[tid] = make_float2(-8.f * __ldg(lut_g + (tid & 7)), -8.f * __ldg(lut_g + (tid >> 3)));
+    if ((kKey || kVq) && tid < 64) lutp[tid] = make_float2(-8.f * __ldg(lut_g + (tid & 7)), -8.f * __ldg(lut_g + (tid >> 3)));
     if constexpr (kLit) {  // power of two that puts the largest LUT entry in [2^8, 2^9): bound of the residual operand scale
       float s_l, inv_l;
       pow2_scale(fmaxf(fabsf(l8[0]), fabsf(l8[7])), s_l, inv_l);
@@ -397,6 +401,9 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
 
   const T* src = reinterpret_cast<const T*>(kKey ? a.k : a.v) + (size_t)bh * a.n_tokens * D;
   unsigned char* stream = a.cv.tiles + ((size_t)a.layer * a.cv.B * a.cv.H + bh) * a.cv.stream_bytes;
+  using Vs = VskLayout<D>;
+  unsigned char* vstream = kVq ? a.cv.vsk + ((size_t)a.layer * a.cv.B * a.cv.H + bh) * a.cv.vsk_stream_bytes : nullptr;
+  static_assert(Cfg::kImgBytes - Cfg::kImgV >= Vs::kTileBytes, "the V-sketch image fits behind the value image");
   const int slot = tok & 31, tl = tok >> 5, sg = slot & 7, sr = slot >> 3;
   unsigned char* timg = img + tl * Cfg::kImgBytes;  // image of this token's tile
   constexpr int kOffImgKS = Lo::kCodeBytes, kOffImgNK = Lo::kCodeBytes + Lo::kSignBytes;  // keys image
@@ -430,6 +437,14 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
       }
     }
 
+    if constexpr (!kKey && kVq) {  // V-sketch image: partly covered tiles keep their other tokens' bits, the rest start at zero
+      for (int idx = tid; idx < 4 * (Vs::kTileBytes / 16); idx += kThreads) {
+        const int t4 = idx / (Vs::kTileBytes / 16), q = idx % (Vs::kTileBytes / 16);
+        uint4 v = make_uint4(0, 0, 0, 0);
+        if (tile_cover(t4) == 1) v = *reinterpret_cast<const uint4*>(vstream + (size_t)(blk * 4 + t4) * Vs::kTileBytes + 16 * q);
+        *reinterpret_cast<uint4*>(img + t4 * Cfg::kImgBytes + Cfg::kImgV + 16 * q) = v;
+      }
+    }
     // ---- stage the A operand rows of the block and start the first product
     {
       const int p0 = blk * kBlk;  // cache position (= RoPE position) of block row 0
@@ -564,12 +579,45 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
       //      This thread's coordinates 8 c + (i & 7), c in [half d/16, + d/16), are d/16 fields = 3 d/64 bytes per lane
       constexpr int CW = NC / 8;  // code words of this thread
       unsigned mine[CW], other[CW];
+      [[maybe_unused]] const float inv8 = n > 0.f ? 8.0f / n : 0.f;
+      [[maybe_unused]] float g2a = 0.f, g2b = 0.f;
 #pragma unroll
       for (int c = 0; c < CW; ++c) {
         float w = 0.f;  // eight codes = 24 bits, exact in fp32
+        if constexpr (kVq) {  // pairs of coordinates share one look-up of (-8 lut[c0], -8 lut[c1]); y becomes 8 r_v
 #pragma unroll
-        for (int q = 0; q < 8; ++q) w = fmaf(code_f(y[8 * c + q], sr_n), (float)(1u << (3 * q)), w);
+          for (int q = 0; q < 8; q += 2) {
+            const float c0 = code_f(y[8 * c + q], sr_n), c1 = code_f(y[8 * c + q + 1], sr_n);
+            w = fmaf(c1, (float)(1u << (3 * q + 3)), fmaf(c0, (float)(1u << (3 * q)), w));
+            float2 nl;
+            asm("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(nl.x), "=f"(nl.y) : "r"(f2u(fmaf(fmaf(c1, 8.f, c0), 8.f, lutp_base))));
+            const float r0 = fmaf(y[8 * c + q], inv8, nl.x), r1 = fmaf(y[8 * c + q + 1], inv8, nl.y);
+            g2a = fmaf(r0, r0, g2a), g2b = fmaf(r1, r1, g2b);
+            y[8 * c + q] = r0, y[8 * c + q + 1] = r1;
+          }
+        } else {
+#pragma unroll
+          for (int q = 0; q < 8; ++q) w = fmaf(code_f(y[8 * c + q], sr_n), (float)(1u << (3 * q)), w);
+        }
         mine[c] = f2u(w);
+      }
+      if constexpr (kVq) {  // the residual operand of the S product over this token's operand row
+        red_g[half * kBlk + tok] = g2a + g2b;
+#pragma unroll
+        for (int kj = 0; kj < NC / 8; ++kj) {
+          uint4 hi, lo;
+          split8(&y[8 * kj], hi, lo);
+          *reinterpret_cast<uint4*>(A_hi + core_off<D>(tok, half * NC + 8 * kj)) = hi;
+          *reinterpret_cast<uint4*>(A_lo + core_off<D>(tok, half * NC + 8 * kj)) = lo;
+        }
+        fence_async_smem();
+        tc_fence_before();
+        __syncthreads();
+        if (tid == 0) {
+          tc_fence_after();
+          gemm(D, a_hi, b1_hi, true), gemm(D, a_lo, b1_hi, false), gemm(D, a_hi, b1_lo, false);
+          umma_commit(smem_u32(mbar + 1));
+        }
       }
 #pragma unroll
       for (int c = 0; c < CW; ++c) other[c] = __shfl_xor_sync(0xffffffffu, mine[c], 1);
@@ -607,9 +655,48 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
         }
       }
     }
+    if constexpr (!kKey && kVq) {
+      // ---- V-side sketch: bit [(S r_v)_rho >= 0] of this thread's sketch rows [half d/2, + d/2) goes to lane
+      //      (rho & 7, t of the slot), one word per (thread, lane): the token's old bits are cleared, the new ones set
+      unsigned char* vimg = timg + Cfg::kImgV;
+      if (valid && half == 0)
+        reinterpret_cast<unsigned short*>(vimg + Vs::kOffVR)[slot_lane(slot)] =
+            f32_to_f16_bits_clamped(sqrtf(red_g[tok] + red_g[kBlk + tok]) * 0.125f);
+      mbar_wait(smem_u32(mbar + 1), parity);
+      tc_fence_after();
+      tmem_ld<NC>(t_lane + D, y);
+      if (valid) {
+        const int ks = slot >> 4, th = (slot >> 3) & 1, ts = (slot & 7) >> 1, e = slot & 1;
+        const int word = ks * (D / 64) + (D == 64 ? 0 : half);  // the m-tiles of this thread's rows share one word
+#pragma unroll
+        for (int g = 0; g < 8; ++g) {
+          unsigned bits = 0u, own = 0u;
+#pragma unroll
+          for (int mq = 0; mq < NC / 16; ++mq)  // m-tile half NC/16 + mq, row halves rh
+#pragma unroll
+            for (int rh = 0; rh < 2; ++rh) {
+              const int mt = half * (NC / 16) + mq;
+              const unsigned pos = 16u * e + 4u * (mt & 3) + 2u * rh + th;
+              own |= 1u << pos;
+              bits |= (y[16 * mq + 8 * rh + g] >= 0.f ? 1u : 0u) << pos;
+            }
+          unsigned* wp = reinterpret_cast<unsigned*>(vimg + Vs::kOffVS + word_offset(Vs::KSW, word, 4 * g + ts));
+          atomicAnd(wp, ~own);
+          atomicOr(wp, bits);
+        }
+      }
+    }
     // ---- write the block's tile images out (every tile the call touches; the image of a partly covered tile carries
     //      the old bits of the other tokens)
     __syncthreads();
+    if constexpr (!kKey && kVq) {
+      for (int idx = tid; idx < 4 * (Vs::kTileBytes / 16); idx += kThreads) {
+        const int t4 = idx / (Vs::kTileBytes / 16), q = idx % (Vs::kTileBytes / 16);
+        if (tile_cover(t4) == 0) continue;
+        *reinterpret_cast<uint4*>(vstream + (size_t)(blk * 4 + t4) * Vs::kTileBytes + 16 * q) =
+            *reinterpret_cast<const uint4*>(img + t4 * Cfg::kImgBytes + Cfg::kImgV + 16 * q);
+      }
+    }
     {
       constexpr int kOwn = kKey ? Cfg::kImgK : Cfg::kImgV;
       for (int idx = tid; idx < 4 * (kOwn / 16); idx += kThreads) {
@@ -634,14 +721,14 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
 
 // grid = (block groups, batch x heads, keys | values): the key CTAs (the long ones) are dispatched first and the value
 // CTAs fill in behind them (measured: alternating key and value CTAs along x is 8 % slower at configs[2])
-template <int D, typename T, bool kLit>
+template <int D, typename T, bool kLit, bool kVq>
 __global__ void __launch_bounds__(kThreads, D == 64 ? 3 : 1) quantize_pack_tc_kernel(QuantArgs a, int blocks_per_cta) {
   extern __shared__ __align__(1024) unsigned char smem_dyn[];
-  if (blockIdx.z == 0) quantize_pack_tc_body<D, T, true, kLit>(a, blocks_per_cta, (int)blockIdx.x, smem_dyn);
-  else quantize_pack_tc_body<D, T, false, kLit>(a, blocks_per_cta, (int)blockIdx.x, smem_dyn);
+  if (blockIdx.z == 0) quantize_pack_tc_body<D, T, true, kLit, kVq>(a, blocks_per_cta, (int)blockIdx.x, smem_dyn);
+  else quantize_pack_tc_body<D, T, false, kLit, kVq>(a, blocks_per_cta, (int)blockIdx.x, smem_dyn);
 }
 
-template <int D, typename T, bool kLit>
+template <int D, typename T, bool kLit, bool kVq>
 cudaError_t launch_quant_tc_t(const QuantArgs& a, int num_sms, cudaStream_t st) {
   const size_t smem = TcCfg<D>::kSmemBytes;
   const int first_blk = a.start_pos / kBlk, last_blk = (a.start_pos + a.n_tokens - 1) / kBlk;
@@ -651,22 +738,26 @@ cudaError_t launch_quant_tc_t(const QuantArgs& a, int num_sms, cudaStream_t st) 
   int bpc = (int)(((long)nblk * BH + want - 1) / want);
   bpc = bpc < 1 ? 1 : (bpc > 16 ? 16 : bpc);
   dim3 grid((nblk + bpc - 1) / bpc, BH, 2);  // z: keys | values
-  cudaError_t e = cudaFuncSetAttribute(quantize_pack_tc_kernel<D, T, kLit>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  cudaError_t e = cudaFuncSetAttribute(quantize_pack_tc_kernel<D, T, kLit, kVq>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
-  quantize_pack_tc_kernel<D, T, kLit><<<grid, kThreads, smem, st>>>(a, bpc);
+  quantize_pack_tc_kernel<D, T, kLit, kVq><<<grid, kThreads, smem, st>>>(a, bpc);
   count_launch();
   return cudaGetLastError();
 }
 
 }  // namespace
 
+template <bool kLit, bool kVq>
+static cudaError_t launch_quant_tc_mode(const QuantArgs& a, int D, tq_dtype dt, int num_sms, cudaStream_t st) {
+  if (D == 64)
+    return dt == TQ_F16 ? launch_quant_tc_t<64, __half, kLit, kVq>(a, num_sms, st) : launch_quant_tc_t<64, float, kLit, kVq>(a, num_sms, st);
+  return dt == TQ_F16 ? launch_quant_tc_t<128, __half, kLit, kVq>(a, num_sms, st) : launch_quant_tc_t<128, float, kLit, kVq>(a, num_sms, st);
+}
+
 cudaError_t launch_quantize_pack_tc(const QuantArgs& a, int D, tq_dtype dt, int num_sms, cudaStream_t st) {
-  if (a.literal) {
-    if (D == 64) return dt == TQ_F16 ? launch_quant_tc_t<64, __half, true>(a, num_sms, st) : launch_quant_tc_t<64, float, true>(a, num_sms, st);
-    return dt == TQ_F16 ? launch_quant_tc_t<128, __half, true>(a, num_sms, st) : launch_quant_tc_t<128, float, true>(a, num_sms, st);
-  }
-  if (D == 64) return dt == TQ_F16 ? launch_quant_tc_t<64, __half, false>(a, num_sms, st) : launch_quant_tc_t<64, float, false>(a, num_sms, st);
-  return dt == TQ_F16 ? launch_quant_tc_t<128, __half, false>(a, num_sms, st) : launch_quant_tc_t<128, float, false>(a, num_sms, st);
+  if (a.literal) return launch_quant_tc_mode<true, false>(a, D, dt, num_sms, st);
+  if (a.cv.vsk) return launch_quant_tc_mode<false, true>(a, D, dt, num_sms, st);
+  return launch_quant_tc_mode<false, false>(a, D, dt, num_sms, st);
 }
 
 }  // namespace tq

@@ -824,3 +824,125 @@ def test_paper_literal_mode_matches_oracle(tq, oracle, name, kw, gauss_S):
     # the GPU's own cache differs from the oracle's only inside the band: its decode stays close
     a, b_ = out_own[0].float().cpu().numpy().reshape(-1, d).astype(np.float64), want.reshape(-1, d)
     assert np.mean(np.sum(a * b_, -1) / (np.linalg.norm(a, axis=-1) * np.linalg.norm(b_, axis=-1))) > 0.999
+
+
+# ---------------------------------------------------------------------------------------------- V-side residual sketch
+def _vq_compare(can, planes, d, what):
+    """compare_quantize for the six usual planes + the two value-sketch planes (bits only where the value codes agree)."""
+    rep = TL.compare_quantize(can, planes, d, what)
+    ok = ~(TL.unpack_codes_np(can.v_codes, d) != TL.unpack_codes_np(planes["v_codes"], d)).any(axis=-1)
+    so = np.unpackbits(can.v_signs, axis=-1, bitorder="little")
+    sg = np.unpackbits(planes["v_signs"], axis=-1, bitorder="little")
+    sdiff = (so != sg) & ok[..., None]
+    rep["v_sign_mismatch_frac"] = float(sdiff.sum() / max(1, ok.sum() * so.shape[-1]))
+    assert rep["v_sign_mismatch_frac"] <= TL.MAX_MISMATCH_FRAC, (what, rep["v_sign_mismatch_frac"])
+    dd = np.abs(can.v_rnorm.astype(np.int32) - planes["v_rnorm"].view(np.uint16).astype(np.int32))[ok]
+    assert dd.max(initial=0) <= 1 and (dd > 0).mean() <= 5e-3 + 1.0 / max(1, dd.size), (what, dd.max(initial=0), (dd > 0).mean())
+    return rep
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("name,kw", [("cfg2_650m_batch32", dict(batch=3, n_heads=4, seq=300)),
+                                     ("cfg4_15b_heads", dict(batch=2, n_heads=3, seq=170)),
+                                     ("cfg0_tiny", dict())])
+def test_value_sketch_quantize_append_decode_match_oracle(tq, oracle, name, kw):
+    """SURVEY.md 8(f) NEXT-1 (Algorithm 1 line 10): tq_shape.v_qjl = 1.  Prefill in unaligned chunks and
+    appended tokens vs the oracle's planes (value sign bits / |r_v| included); canonical round trip; decode on the
+    oracle's bytes vs tqo_decode_attn_vq at 2e-3 / 0.9999, unsplit and split-K."""
+    import torch
+
+    w = W.CONFIGS[name].scaled(**kw) if kw else W.CONFIGS[name]
+    d, H, B, T = w.head_dim, w.n_heads, w.batch, w.seq
+    n_app = 3
+    shape = tq.make_shape(1, B, H, d, T + 8, w.rope_base, 0, v_qjl=1)
+    assert tq.tq_cache_bytes_per_token_head(shape) == (72 if d == 64 else 136)
+    rope_cs = tq.tq_calibrate_host(shape, 1, seed=1)["rope_cs"]
+    arr = TL.make_arrays(oracle, w, rope_cs, lut_scale_v=1.1)
+    params = tq.Params(arr)
+    cache = tq.Cache(shape)
+    dev = lambda x: torch.from_numpy(np.ascontiguousarray(x)).cuda()
+    k, v = W.layer_activations(w, 0)
+    toks = [W.step_tokens(w, 0, s) for s in range(n_app)]
+    cut = min(77, T // 2)
+    tq.tq_quantize_pack(shape, params, cache, 0, dev(k[:, :, :cut]), dev(v[:, :, :cut]), 0)
+    tq.tq_quantize_pack(shape, params, cache, 0, dev(k[:, :, cut:]), dev(v[:, :, cut:]), cut)
+    for (_, kn, vn) in toks:
+        tq.tq_append(shape, params, cache, 0, dev(kn), dev(vn))
+    Tn = T + n_app
+    assert torch.all(cache.seq_len == Tn)
+    planes = {n: p.cpu().numpy() for n, p in tq.tq_cache_export_canonical(shape, cache, 0, Tn).items()}
+    kk = np.concatenate([k] + [t[1][:, :, None] for t in toks], axis=2)
+    vv = np.concatenate([v] + [t[2][:, :, None] for t in toks], axis=2)
+    can = oracle.quantize_pack(kk, vv, arr["pi_k"][0], arr["pi_v"][0], arr["lut_k"][0], arr["lut_v"][0], arr["S"],
+                               base=w.rope_base, near_eps=TL.NEAR_EPS)
+    oracle.add_value_sketch(can, vv, arr["pi_v"][0], arr["lut_v"][0], arr["S"])
+    rep = _vq_compare(can, planes, d, "v_qjl quantize + append")
+    print("v_qjl quantize:", {k_: v_ for k_, v_ in rep.items() if not k_.endswith("equal")})
+    # canonical round trip of the oracle's planes, then decode on those bytes
+    cache2 = tq.Cache(shape)
+    tc = TL.to_torch_canonical(can)
+    tc["v_signs"] = torch.from_numpy(can.v_signs).cuda()
+    tc["v_rnorm"] = torch.from_numpy(can.v_rnorm.view(np.int16)).cuda()
+    tq.tq_cache_import_canonical(shape, cache2, 0, Tn, tc)
+    back = {n: p.cpu().numpy() for n, p in tq.tq_cache_export_canonical(shape, cache2, 0, Tn).items()}
+    assert np.array_equal(back["v_signs"], can.v_signs) and np.array_equal(back["v_rnorm"].view(np.uint16), can.v_rnorm)
+    assert np.array_equal(back["k_codes"], can.k_codes) and np.array_equal(back["v_codes"], can.v_codes)
+    q = W.queries(w, 0)
+    sl = np.full(B, Tn, np.int32)
+    want = oracle.decode_attn_vq(q, sl - 1, sl, arr["pi_k"][0], arr["pi_v"][0], arr["lut_k"][0], arr["lut_v"][0], arr["S"], can,
+                                 base=w.rope_base)
+    plain = oracle.decode_attn(q, sl - 1, sl, arr["pi_k"][0], arr["pi_v"][0], arr["lut_k"][0], arr["lut_v"][0], arr["S"], can,
+                               base=w.rope_base)
+    assert np.abs(want - plain).max() > 1e-3  # the sketch term is really there
+    qd = dev(q[None])
+    ws = tq.Workspace(shape, 1)
+    try:
+        for nsplit in (0, 1, 3):
+            tq.tq_debug_set_decode_nsplit(nsplit)
+            out = torch.full_like(qd, float("nan"))
+            tq.tq_decode_attn(shape, params, cache2, 0, 1, qd, out, ws)
+            torch.cuda.synchronize()
+            got = out[0].float().cpu().numpy()
+            ulp = np.spacing(np.abs(want).astype(np.float16)).astype(np.float64) if w.dtype == "f16" else 0.0
+            assert np.all(np.abs(got.astype(np.float64) - want) <= ulp + TL.OUT_MAX_ABS), (nsplit, np.abs(got - want).max())
+            r = TL.compare_outputs(got, want, f"v_qjl decode nsplit={nsplit}", max_abs=float(np.max(ulp)) + TL.OUT_MAX_ABS)
+        print("v_qjl decode:", r)
+    finally:
+        tq.tq_debug_set_decode_nsplit(0)
+
+
+@pytest.mark.gpu
+def test_value_sketch_model_step_equals_per_layer_calls(tq, oracle):
+    """v_qjl = 1 through tq_decode_model_step (run-ahead chain + finish kernel) and through the stepper graph == tq_append +
+    tq_decode_attn layer by layer, outputs and cache bytes bit for bit."""
+    import torch
+
+    w = W.CONFIGS["cfg2_650m_batch32"].scaled(n_layers=3, batch=4, n_heads=5, seq=200)
+    L = w.n_layers
+    shape = tq.make_shape(L, w.batch, w.n_heads, w.head_dim, w.seq + 16, w.rope_base, 0, v_qjl=1)
+    cal = tq.tq_calibrate_host(shape, 1, seed=2)
+    params = tq.Params(cal)
+    dev = lambda x: torch.from_numpy(np.ascontiguousarray(x)).cuda()
+    caches = []
+    for _ in range(3):
+        c = tq.Cache(shape)
+        for layer in range(L):
+            k, v = W.layer_activations(w, layer)
+            tq.tq_quantize_pack(shape, params, c, layer, dev(k), dev(v))
+        caches.append(c)
+    toks = [W.step_tokens(w, layer, 0) for layer in range(L)]
+    q, kn, vn = (dev(np.stack([t[i] for t in toks])) for i in range(3))
+    outs = [torch.full_like(q, float("nan")) for _ in range(3)]
+    ws1, wsL = tq.Workspace(shape, 1), tq.Workspace(shape, L)
+    for layer in range(L):
+        tq.tq_append(shape, params, caches[0], layer, kn[layer], vn[layer])
+        tq.tq_decode_attn(shape, params, caches[0], layer, 1, q[layer:layer + 1], outs[0][layer:layer + 1], ws1, None, w.seq + 16)
+    tq.tq_decode_model_step(shape, params, caches[1], 0, L, q, kn, vn, outs[1], wsL, w.seq + 16)
+    st = tq.HostStepper(shape, params, caches[2], 0, L, q, kn, vn, outs[2], None, wsL, w.seq + 16, 2)
+    torch.cuda.synchronize()
+    st.launch()
+    torch.cuda.synchronize()
+    st.close()
+    for i in (1, 2):
+        assert torch.isfinite(outs[0].float()).all() and torch.equal(outs[0], outs[i])
+        assert torch.equal(caches[0].data, caches[i].data)

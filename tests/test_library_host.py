@@ -61,7 +61,13 @@ def test_size_arithmetic(tq):
     assert tq.tq_cache_bytes(tq.make_shape(1, 1, 1, 96, 64)) == 0
     assert tq.tq_cache_bytes(tq.make_shape(0, 1, 1, 64, 64)) == 0
     assert tq.tq_cache_bytes(tq.make_shape(1, 1, 1, 64, 64, qjl_dim=32)) == 0
-    assert tq.tq_cache_bytes(tq.make_shape(1, 1, 1, 64, 64, v_qjl=1)) == 0
+    # V-side sketch: a second stream of 320-byte tiles (d = 64), 72 bytes per token-head; not with the literal mode
+    sv = tq.make_shape(1, 1, 1, 64, 64, v_qjl=1)
+    assert tq.tq_cache_bytes(sv) == 256 + 2 * (1984 + 320) and tq.tq_cache_bytes_per_token_head(sv) == 72
+    assert tq.tq_canonical_plane_bytes(sv, 6, 10) == 10 * 8 and tq.tq_canonical_plane_bytes(sv, 7, 10) == 10 * 2
+    assert tq.tq_canonical_plane_bytes(s, 6, 10) == 0
+    assert tq.tq_cache_bytes(tq.make_shape(1, 1, 1, 64, 64, v_qjl=2)) == 0
+    assert tq.tq_cache_bytes(tq.make_shape(1, 1, 1, 64, 64, v_qjl=1, residual_mode=1)) == 0
 
 
 def test_validation_is_synchronous_and_there_is_no_fallback(tq):
