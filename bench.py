@@ -39,6 +39,7 @@ from paper_2603_26110_b200 import workloads as W
 METRIC = "fused 3-bit decode-attn cached tokens/s"
 UNIT = "cached token-heads/s"
 FALLBACK_HBM_GBS = 6650.0  # B200_PROFILING.md fallback
+V_QJL = 0  # --v-qjl: the V-side residual sketch, +10 / +18 bytes per token-head
 CONFIG_NAMES = {"cfg1": "cfg1_650m_step", "cfg2": "cfg2_650m_batch32", "cfg3": "cfg3_long_splitk", "cfg4": "cfg4_15b_heads"}
 
 
@@ -318,7 +319,7 @@ class Rig:
         self.dev = torch.device("cuda", local)
         self.B, self.H, self.d, self.T0 = w.batch, w.n_heads, w.head_dim, w.seq
         self.max_seq = max_seq
-        self.shape = tq.make_shape(L, self.B, self.H, self.d, max_seq, w.rope_base, 0)
+        self.shape = tq.make_shape(L, self.B, self.H, self.d, max_seq, w.rope_base, 0, v_qjl=V_QJL)
         self.wl = w.scaled(n_layers=L)
         cal = tq.tq_calibrate_host(self.shape, 1, seed=w.seed + rank)  # QR-of-Gaussian PI per (layer, head), Lloyd-Max LUT, S
         self.params = tq.Params(cal, self.dev)
@@ -326,7 +327,7 @@ class Rig:
         self.gen = torch.Generator(device=self.dev)
         self.gen.manual_seed(w.seed + 1000 * rank)
         self.stream = torch.cuda.Stream(self.dev)
-        self.bpt = bytes_per_token_head(self.d)
+        self.bpt = tq.tq_cache_bytes_per_token_head(self.shape)  # 62 | 118; 72 | 136 with the V-side sketch
 
     def ev(self):
         return self.torch.cuda.Event(enable_timing=True)
@@ -549,7 +550,7 @@ def run_cfg2(args, w: W.Workload):
 
     # ---- the paper's comparison system on this box: PyTorch two-step path (dequantise to fp16, then attend) on layer 0
     two_step = None
-    if not args.no_two_step:
+    if not args.no_two_step and not V_QJL:
         with torch.cuda.stream(stream):
             reset_len()
             tq.tq_decode_attn(shape, params, cache, 0, 1, qs[0:1], outs[0:1], ws1, None, max_seq, stream)
@@ -599,7 +600,7 @@ def run_cfg2(args, w: W.Workload):
     peak, peak_src = measured_peaks()
     achieved = dec_bytes / (chain_us * 1e-6) / 1e9
     value = whole_job_value(tok_heads, world, ms_max)
-    traffic = ncu_traffic("decode_main")
+    traffic = None if V_QJL else ncu_traffic("decode_main")
     us_layer = 1e3 * ms_max / args.steps / L
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
@@ -610,7 +611,7 @@ def run_cfg2(args, w: W.Workload):
                         f"{T0}+ cached tokens, fp16 Student-t(4) + 2 outlier channels x15, append + decode per layer per step",
             "layers": L, "batch_per_gpu": B, "heads": H, "head_dim": d, "cached_tokens": T0, "io_dtype": "f16",
             "l2": f"inputs larger than L2: {L} layer caches x {B*H*T0*rig.bpt/1e6:.1f} MB are cycled every step",
-            "cuda_graph": True, "bytes_per_token_head": rig.bpt,
+            "cuda_graph": True, "bytes_per_token_head": rig.bpt, "v_qjl": V_QJL,
             "step_form": "tq_decode_model_step: one append+query-prep launch for all layers, one streaming launch per "
                          "layer cache (run-ahead chain), one finish launch",
             "us_per_layer_step": us_layer,
@@ -637,7 +638,7 @@ def run_cfg2(args, w: W.Workload):
                 "value_uncaptured_host_call": e2e_tok / e2e_plain_s},
         "gpu_launches": int(launches_per_step * args.steps),
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": traffic[0] if traffic else None, "kernel": "decode_main_kernel<64, __half, false>",
+                     "traffic": traffic[0] if traffic else None, "kernel": "decode_main_kernel<64, __half, false, %s>" % ("true" if V_QJL else "false"),
                      "traffic_source": (f"dram__bytes_read.sum + dram__bytes_write.sum per launch, {traffic[1]}" if traffic
                                         else "no ncu capture of the current kernel is committed"),
                      "peak_source": peak_src, "bytes_per_launch": dec_bytes,
@@ -662,7 +663,7 @@ def run_aux(args, w: W.Workload, key: str):
     rank, world, local = init_dist()
     from paper_2603_26110_b200 import binding as tq
 
-    bpt = bytes_per_token_head(w.head_dim)
+    bpt = bytes_per_token_head(w.head_dim) + (0 if not V_QJL else (10 if w.head_dim == 64 else 18))
     cache_mb = w.batch * w.n_heads * w.seq * bpt / 1e6
     # enough layer caches to exceed the 126 MB L2 (configs[1] has its own 33 layers)
     L = w.n_layers if key == "cfg1" else max(2, int(np.ceil(300.0 / cache_mb)))
@@ -749,9 +750,12 @@ def main():
     ap.add_argument("--layers-aux", type=int, default=0, help="layer caches cycled by cfg3 / cfg4 (0 = enough to exceed L2)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-two-step", action="store_true", help="skip the PyTorch two-step GPU baseline (NEXT-4)")
+    ap.add_argument("--v-qjl", action="store_true", help="measure with the V-side residual sketch on (tq_shape.v_qjl = 1)")
     ap.add_argument("--e2e-chunks", type=int, default=0, help="layer chunks of the host stepper (0 = the library's choice)")
     args = ap.parse_args()
     w = W.CONFIGS[CONFIG_NAMES[args.config]]
+    global V_QJL
+    V_QJL = 1 if args.v_qjl else 0
     if args.impl == "reference":
         run_reference(args, w)
         return

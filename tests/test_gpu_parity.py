@@ -682,6 +682,16 @@ def test_synthetic_ablation_report(tq, oracle):
     can.k_rnorm[...] = 0
     o_noqjl = cosine(c.oracle_decode(0, q, sl - 1, sl, can))
     print(f"  oracle: full {o_full:.4f}, no QJL {o_noqjl:.4f}")
+    # NEXT-1: the same inputs with the V-side sketch on (72 instead of 62 bytes per token-head)
+    import torch
+    shape_v = tq.make_shape(1, w.batch, w.n_heads, w.head_dim, w.seq, w.rope_base, 0, v_qjl=1)
+    cache_v = tq.Cache(shape_v)
+    tq.tq_quantize_pack(shape_v, c.params, cache_v, 0, c.dev(k), c.dev(v))
+    qd = c.dev(q[None])
+    out_v = torch.full_like(qd, float("nan"))
+    tq.tq_decode_attn(shape_v, c.params, cache_v, 0, 1, qd, out_v, tq.Workspace(shape_v, 1))
+    torch.cuda.synchronize()
+    print(f"  full + V sketch      {cosine(out_v[0].float().cpu().numpy()):.4f}   [Algorithm 1 line 10; +10 B per token-head]")
     assert abs(o_full - rows[(True, True)]) < 2e-3 and abs(o_noqjl - rows[(True, False)]) < 2e-3
 
 
