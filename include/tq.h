@@ -231,11 +231,13 @@ int tq_decode_model_step_host(const tq_shape *shape, const tq_params *dev, tq_ca
 /* ---- stepper: one decode step of a run of layers captured ONCE as a CUDA graph (the serving loop's form of the step;
  * bench.py times it with host buffers as "e2e") [BASELINE.json:configs[2] "100 consecutive decode steps"; SURVEY.md §7
  * hard part 2].  tq_host_stepper_create records, for FIXED buffers q/k/v/out ([n_layers_call][B][H][d], dtype dt, valid
- * until destroy), a graph with three branches; the layers are cut into n_chunks runs (0 = the library's choice):
- *   copy-in  : per run, the host-to-device copies of k, v, q, then the append + query-prep kernel of that run;
- *   main     : the streaming kernels of all layers, a run-ahead chain per run (the first kernel of a run waits for that
- *              run's prep kernel and for the run in front);
- *   copy-out : per run, the PI_V^T finish kernel, then the device-to-host copy of out.
+ * until destroy), a graph with several branches; the layers are cut into n_chunks runs of growing length (0 = the
+ * library's choice):
+ *   copy     : per run, the host-to-device copies of k, v, q, back to back;
+ *   prep     : per run, the append + query-prep kernel behind that run's copies;
+ *   main x 2 : the streaming kernels of all layers; the chains of consecutive runs alternate between two branches, so the
+ *              first kernel of a run waits only for that run's prep kernel;
+ *   copy-out : per group of six layers, the PI_V^T finish kernel, then the device-to-host copy of out.
  * buffers_on_host = 1: q/k/v/out are HOST buffers and must be page-locked (cudaHostAlloc / cudaHostRegister); staging is a
  * DEVICE buffer of tq_model_step_staging_bytes() bytes, 256-byte aligned.  buffers_on_host = 0: they are DEVICE buffers,
  * no copies are recorded and staging may be NULL.  workspace: tq_decode_workspace_bytes(shape, n_layers_call), zero-filled

@@ -449,11 +449,13 @@ int tq_decode_model_step_host(const tq_shape* shape, const tq_params* dev, tq_ca
   return TQ_OK;
 }
 
-// ---- stepper: one decode step of a run of layers captured ONCE as a CUDA graph with three branches ---------------------
-//   copy-in branch : per layer chunk, H2D copies of k, v, q (host buffers only), then the append + query-prep kernel
-//   main branch    : the streaming kernels of every layer; the first kernel of a chunk waits for that chunk's prep
-//                    kernel (and the chunk in front), the others run ahead as in tq_decode_model_step
-//   copy-out branch: per chunk, the finish kernel (PI_V^T), then the D2H copy of out (host buffers only)
+// ---- stepper: one decode step of a run of layers captured ONCE as a CUDA graph with five branches -----------------------
+//   copy      : (host buffers only) per layer chunk, the H2D copies of k, v, q, back to back
+//   prep      : per chunk, the append + query-prep kernel, behind that chunk's copies
+//   main, main2: the streaming kernels; the chains of consecutive chunks alternate between the two branches, so the first
+//                kernel of a chunk waits for that chunk's prep kernel only (and for the chunk two in front), the others run
+//                ahead as in tq_decode_model_step
+//   copy-out  : per group of six layers, the finish kernel (PI_V^T), then the D2H copy of out (host buffers only)
 struct tq_host_stepper {
   cudaGraph_t graph = nullptr;
   cudaGraphExec_t exec = nullptr;
@@ -474,8 +476,8 @@ int tq_host_stepper_create(const tq_shape* shape, const tq_params* dev, tq_cache
   if (dt != TQ_F16 && dt != TQ_F32) return TQ_ERR_INVALID_ARG;
   if (layer_begin < 0 || n_layers_call <= 0 || layer_begin + n_layers_call > g.L) return TQ_ERR_INVALID_ARG;
   constexpr int kMaxChunks = 64;
-  // measured at configs[2] x 33 layers: 4 chunks 38 G token-heads/s end to end; 2: 37, 8: 37, 33: 17 (a chunk boundary
-  // costs about 9 us: the first streaming kernel of a chunk waits for the chunk in front to drain)
+  // measured at configs[2] x 33 layers (value 48.8 G token-heads/s): 2 chunks 37.6 G end to end, 3: 41.7, 4: 42.5, 6: 39.4,
+  // 8: 37.4 (more chunks = more and smaller prep launches)
   if (n_chunks <= 0) n_chunks = n_layers_call >= 16 ? 4 : (n_layers_call >= 4 ? 2 : 1);
   if (n_chunks > n_layers_call) n_chunks = n_layers_call;
   if (n_chunks > kMaxChunks) n_chunks = kMaxChunks;
@@ -490,49 +492,88 @@ int tq_host_stepper_create(const tq_shape* shape, const tq_params* dev, tq_cache
                             workspace_bytes, &p)) != TQ_OK)
     return rc;
 
-  cudaStream_t s_main = nullptr, s_in = nullptr, s_out = nullptr;
-  cudaEvent_t fork = nullptr, join_in = nullptr, join_out = nullptr;
-  cudaEvent_t prep_done[kMaxChunks] = {}, chain_done[kMaxChunks] = {};
+  cudaStream_t s_main = nullptr, s_main2 = nullptr, s_in = nullptr, s_out = nullptr, s_copy = nullptr;
+  cudaEvent_t fork = nullptr, join_in = nullptr, join_out = nullptr, join_copy = nullptr, join_main2 = nullptr;
+  cudaEvent_t prep_done[kMaxChunks] = {}, chain_done[kMaxChunks] = {}, copy_done[kMaxChunks] = {};
   bool ok = cudaStreamCreateWithFlags(&s_main, cudaStreamNonBlocking) == cudaSuccess &&
             cudaStreamCreateWithFlags(&s_in, cudaStreamNonBlocking) == cudaSuccess &&
             cudaStreamCreateWithFlags(&s_out, cudaStreamNonBlocking) == cudaSuccess &&
+            cudaStreamCreateWithFlags(&s_copy, cudaStreamNonBlocking) == cudaSuccess &&
+            cudaStreamCreateWithFlags(&s_main2, cudaStreamNonBlocking) == cudaSuccess &&
+            cudaEventCreateWithFlags(&join_main2, cudaEventDisableTiming) == cudaSuccess &&
+            cudaEventCreateWithFlags(&join_copy, cudaEventDisableTiming) == cudaSuccess &&
             cudaEventCreateWithFlags(&fork, cudaEventDisableTiming) == cudaSuccess &&
             cudaEventCreateWithFlags(&join_in, cudaEventDisableTiming) == cudaSuccess &&
             cudaEventCreateWithFlags(&join_out, cudaEventDisableTiming) == cudaSuccess;
+  const int n_out_max = kMaxChunks;
   for (int c = 0; ok && c < n_chunks; ++c)
     ok = cudaEventCreateWithFlags(&prep_done[c], cudaEventDisableTiming) == cudaSuccess &&
-         cudaEventCreateWithFlags(&chain_done[c], cudaEventDisableTiming) == cudaSuccess;
+         cudaEventCreateWithFlags(&copy_done[c], cudaEventDisableTiming) == cudaSuccess;
+  for (int c = 0; ok && c < n_out_max; ++c) ok = cudaEventCreateWithFlags(&chain_done[c], cudaEventDisableTiming) == cudaSuccess;
   tq_host_stepper* hs = ok ? new tq_host_stepper() : nullptr;
   int status = ok ? TQ_OK : TQ_ERR_CUDA;
   if (ok) {
     const long long n0 = g_launches.load();
     const bool capturing = cudaStreamBeginCapture(s_main, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
     ok = capturing && cudaEventRecord(fork, s_main) == cudaSuccess && cudaStreamWaitEvent(s_in, fork, 0) == cudaSuccess &&
-         cudaStreamWaitEvent(s_out, fork, 0) == cudaSuccess;
+         cudaStreamWaitEvent(s_out, fork, 0) == cudaSuccess && cudaStreamWaitEvent(s_copy, fork, 0) == cudaSuccess &&
+         cudaStreamWaitEvent(s_main2, fork, 0) == cudaSuccess;
+    // copy-in chunks grow geometrically (x 1.6): the first is short, so that the streaming chain starts after a small copy
+    // and a small prep kernel, and every later chunk's copy + prep fits under the chain of the chunks in front of it.
+    // The copies run on a branch of their own (a prep kernel never holds up the next copy).  Copy-out groups of
+    // kOutLayers layers are independent of the chunks: a group's finish kernel and copy leave as soon as its last
+    // streaming kernel is done
+    int bound[kMaxChunks + 1];
+    {
+      double wsum = 0.0, w = 1.0, acc = 0.0;
+      for (int c = 0; c < n_chunks; ++c, w *= 1.6) wsum += w;
+      bound[0] = 0;
+      w = 1.0;
+      for (int c = 1; c <= n_chunks; ++c, w *= 1.6) {
+        acc += w;
+        int b = (int)(n_layers_call * acc / wsum + 0.5);
+        b = b < bound[c - 1] + 1 ? bound[c - 1] + 1 : b;                                  // at least one layer per chunk
+        b = b > n_layers_call - (n_chunks - c) ? n_layers_call - (n_chunks - c) : b;      // and one left for each to come
+        bound[c] = c == n_chunks ? n_layers_call : b;
+      }
+    }
+    const int out_layers = n_layers_call > 6 * kMaxChunks ? (n_layers_call + kMaxChunks - 1) / kMaxChunks : 6;
+    int out_begin = 0, n_out = 0;
     for (int c = 0; ok && c < n_chunks; ++c) {
-      const int l0 = (int)((long long)n_layers_call * c / n_chunks), l1 = (int)((long long)n_layers_call * (c + 1) / n_chunks);
+      const int l0 = bound[c], l1 = bound[c + 1];
       const size_t off = per_layer * l0, nb = per_layer * (l1 - l0);
       if (buffers_on_host)
-        ok = cudaMemcpyAsync((void*)(dk + off), (const unsigned char*)k_buf + off, nb, cudaMemcpyHostToDevice, s_in) == cudaSuccess &&
-             cudaMemcpyAsync((void*)(dv + off), (const unsigned char*)v_buf + off, nb, cudaMemcpyHostToDevice, s_in) == cudaSuccess &&
-             cudaMemcpyAsync((void*)(dq + off), (const unsigned char*)q_buf + off, nb, cudaMemcpyHostToDevice, s_in) == cudaSuccess;
+        ok = cudaMemcpyAsync((void*)(dk + off), (const unsigned char*)k_buf + off, nb, cudaMemcpyHostToDevice, s_copy) == cudaSuccess &&
+             cudaMemcpyAsync((void*)(dv + off), (const unsigned char*)v_buf + off, nb, cudaMemcpyHostToDevice, s_copy) == cudaSuccess &&
+             cudaMemcpyAsync((void*)(dq + off), (const unsigned char*)q_buf + off, nb, cudaMemcpyHostToDevice, s_copy) == cudaSuccess &&
+             cudaEventRecord(copy_done[c], s_copy) == cudaSuccess && cudaStreamWaitEvent(s_in, copy_done[c], 0) == cudaSuccess;
       const DecodeArgs ca = sub_args(p, l0, l1 - l0);
+      // the chains of consecutive chunks alternate between two branches: the first kernel of a chunk then waits for its prep
+      // kernel only, not for the chunk in front to drain (layers are independent)
+      cudaStream_t s_chain = (c & 1) ? s_main2 : s_main;
       ok = ok && launch_prep(ca, dk + off, dv + off, g.D, p.sms, true, true, s_in) == cudaSuccess &&
-           cudaEventRecord(prep_done[c], s_in) == cudaSuccess && cudaStreamWaitEvent(s_main, prep_done[c], 0) == cudaSuccess;
+           cudaEventRecord(prep_done[c], s_in) == cudaSuccess && cudaStreamWaitEvent(s_chain, prep_done[c], 0) == cudaSuccess;
       for (int l = l0; ok && l < l1; ++l) {
         DecodeArgs b = sub_args(p, l, 1);
         // a captured launch with the programmatic attribute turns EVERY dependency of its stream into a programmatic
         // edge, the one to this chunk's prep kernel included (which triggers early): the first kernel of a chunk must
         // therefore wait at its start; the others run ahead
         b.chain_mode = l == l0 ? 0 : 1;
-        ok = launch_decode(b, g.D, false, s_main) == cudaSuccess;
+        ok = launch_decode(b, g.D, false, s_chain) == cudaSuccess;
+        if (ok && (l + 1 - out_begin == out_layers || l + 1 == l1)) {  // a copy-out group is complete (groups end with the chunk)
+          const DecodeArgs oa = sub_args(p, out_begin, l + 1 - out_begin);
+          const size_t ooff = per_layer * out_begin, onb = per_layer * (l + 1 - out_begin);
+          ok = n_out < kMaxChunks && cudaEventRecord(chain_done[n_out], s_chain) == cudaSuccess &&
+               cudaStreamWaitEvent(s_out, chain_done[n_out], 0) == cudaSuccess && launch_finish(oa, g.D, false, s_out) == cudaSuccess;
+          if (ok && buffers_on_host)
+            ok = cudaMemcpyAsync((unsigned char*)out_buf + ooff, dout + ooff, onb, cudaMemcpyDeviceToHost, s_out) == cudaSuccess;
+          out_begin = l + 1, ++n_out;
+        }
       }
-      ok = ok && cudaEventRecord(chain_done[c], s_main) == cudaSuccess && cudaStreamWaitEvent(s_out, chain_done[c], 0) == cudaSuccess &&
-           launch_finish(ca, g.D, false, s_out) == cudaSuccess;
-      if (ok && buffers_on_host)
-        ok = cudaMemcpyAsync((unsigned char*)out_buf + off, dout + off, nb, cudaMemcpyDeviceToHost, s_out) == cudaSuccess;
     }
-    ok = ok && cudaEventRecord(join_in, s_in) == cudaSuccess && cudaStreamWaitEvent(s_main, join_in, 0) == cudaSuccess &&
+    ok = ok && cudaEventRecord(join_main2, s_main2) == cudaSuccess && cudaStreamWaitEvent(s_main, join_main2, 0) == cudaSuccess &&
+         cudaEventRecord(join_copy, s_copy) == cudaSuccess && cudaStreamWaitEvent(s_main, join_copy, 0) == cudaSuccess &&
+         cudaEventRecord(join_in, s_in) == cudaSuccess && cudaStreamWaitEvent(s_main, join_in, 0) == cudaSuccess &&
          cudaEventRecord(join_out, s_out) == cudaSuccess && cudaStreamWaitEvent(s_main, join_out, 0) == cudaSuccess;
     cudaGraph_t graph = nullptr;
     if (capturing) ok = (cudaStreamEndCapture(s_main, &graph) == cudaSuccess && graph) && ok;
@@ -542,10 +583,15 @@ int tq_host_stepper_create(const tq_shape* shape, const tq_params* dev, tq_cache
     g_launches.store(n0);  // nothing ran yet: the capture only recorded the launches
     if (!ok) status = TQ_ERR_CUDA;
   }
-  for (int c = 0; c < n_chunks; ++c) {
+  for (int c = 0; c < kMaxChunks; ++c) {
     if (prep_done[c]) cudaEventDestroy(prep_done[c]);
     if (chain_done[c]) cudaEventDestroy(chain_done[c]);
+    if (copy_done[c]) cudaEventDestroy(copy_done[c]);
   }
+  if (join_copy) cudaEventDestroy(join_copy);
+  if (join_main2) cudaEventDestroy(join_main2);
+  if (s_copy) cudaStreamDestroy(s_copy);
+  if (s_main2) cudaStreamDestroy(s_main2);
   if (fork) cudaEventDestroy(fork);
   if (join_in) cudaEventDestroy(join_in);
   if (join_out) cudaEventDestroy(join_out);
