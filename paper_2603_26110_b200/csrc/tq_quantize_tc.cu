@@ -3,7 +3,8 @@
 // Same arithmetic as tq_quantize.cu (PAPER.md:111-116 prefill steps 1,3,4; §3.3 Eq. 5; §3.4 Eq. 6 in the sign(S r)
 // form of BASELINE.json:north_star), but the three rotations y = PI_K x', S r, PI_V v — a dense
 // (tokens x d) x (d x d) contraction — run as tcgen05.mma with the accumulators in tensor memory:
-//   * a CTA of 256 threads owns 128-token blocks of one (batch, head): UMMA M = 128 tokens, N = d outputs, K = 16;
+//   * a CTA of 256 (d = 64) / 512 (d = 128) threads owns 128-token blocks of one (batch, head): UMMA M = 128 tokens,
+//     N = d outputs, K = 16;
 //     keys (RoPE, PI_K, then S on the residual) and values (PI_V) run as separate CTAs (blockIdx.z);
 //   * operands are fp16 in shared memory in the canonical K-major no-swizzle layout (8 x 8 core matrices);
 //     fp32 accuracy comes from two-term splits a = a_hi + a_lo (each product exact in the fp32 accumulator):
@@ -13,9 +14,9 @@
 //     study (hard part 4) puts the code-flip rate of this scheme at 2e-7, that of an all-fp32 pipeline;
 //   * the prologue is warp-cooperative: a warp stages 8 token rows at a time, lane = (16-byte chunk, row), so that the
 //     global reads are sector-exact and the 128-bit shared-memory stores of the operand rows are conflict free;
-//   * the epilogue runs two threads per token: thread (token, half) reads the d/2 accumulator columns of ITS half of
+//   * the epilogue runs d/32 threads per token: thread (token, part) reads the 32 accumulator columns of ITS part of
 //     ITS token with ONE tcgen05.ld and keeps them in registers for the norm, the code search, the residual and the
-//     packing (the two halves exchange their partial sums of squares through shared memory).  The code search and the
+//     packing (the parts exchange their partial sums of squares through shared memory).  The code search and the
 //     sign bits are computed on the FMA pipe (see code_f).  The device tile layout (tq_common.cuh) is the A-fragment
 //     order of the decode kernel's MMAs, so every thread drops its bytes into an image of the block's four tiles in
 //     shared memory (V fields, which mix the two tokens of a pair, are assembled after one shuffle with the neighbour
@@ -27,13 +28,19 @@ namespace tq {
 namespace {
 
 constexpr int kBlk = 128;      // tokens per block = UMMA M
-constexpr int kThreads = 256;  // two threads per token: thread (token = tid & 127, half = tid >> 7)
+// d/32 threads per token: thread (token = tid & 127, part = tid >> 7) owns the 32 accumulator columns [32 part, 32 part + 32)
+// of its token; 256 threads per CTA at d = 64, 512 at d = 128 (where shared memory allows one CTA per SM: the wider CTA
+// doubles the resident warps)
+template <int D>
+constexpr int kThreadsOf = 128 * (D / 32);
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
 template <int D>
 struct TcCfg {
   using Lo = Layout<D>;
+  static constexpr int kParts = D / 32;            // threads per token
+  static constexpr int kThreads = kThreadsOf<D>;
   static constexpr int kSBO = 16 * D;              // bytes between 8-row groups of an operand: 1024 | 2048
   static constexpr int kOpBytes = kBlk * D * 2;    // one fp16 A operand: 16 | 32 KB
   static constexpr int kMatBytes = D * D * 2;      // one fp16 B operand: 8 | 32 KB
@@ -45,10 +52,10 @@ struct TcCfg {
   static constexpr int kImgV = Lo::kCodeBytes + 2 * kTile;
   static constexpr int kImgBytes = kImgK;          // per tile (the larger of the two)
   // shared memory: B operands 4 x kMatBytes (keys: PI_K hi/lo, S hi/lo; values: PI_V hi/lo) | A operands hi, lo |
-  // tile images [4][kImgBytes] | partial sums [2 kinds][2 halves][128] | row scales [128] | LUT pair table [64] float2,
+  // tile images [4][kImgBytes] | partial sums [2 kinds][d/32 parts][128] | row scales [128] | LUT pair table [64] float2,
   // barriers, TMEM slot
   static constexpr int kOffA = 4 * kMatBytes, kOffMisc = kOffA + 2 * kOpBytes;
-  static constexpr int kSmemBytes = kOffMisc + 4 * kImgBytes + 4 * kBlk * 4 + kBlk * 4 + 64 * 8 + 3 * 8 + 16;
+  static constexpr int kSmemBytes = kOffMisc + 4 * kImgBytes + 2 * kParts * kBlk * 4 + kBlk * 4 + 64 * 8 + 3 * 8 + 16;
 };
 
 // byte offset of element (row, k) of a [rows][d] fp16 operand in the canonical K-major no-swizzle layout:
@@ -135,7 +142,7 @@ __device__ __forceinline__ void stage_matrix(unsigned char* bhi, unsigned char* 
                                              int tid) {
   // consecutive threads take consecutive rows n of one 16-byte column chunk: eight of them fill one core matrix row
   // group (128 contiguous bytes), so the 128-bit stores are conflict free; the reads are whole 32-byte sectors
-  for (int idx = tid; idx < D * D / 8; idx += kThreads) {
+  for (int idx = tid; idx < D * D / 8; idx += kThreadsOf<D>) {
     const int n = idx % D, kj = idx / D;
     const float4 a = __ldg(reinterpret_cast<const float4*>(M + n * D + 8 * kj));
     const float4 b = __ldg(reinterpret_cast<const float4*>(M + n * D + 8 * kj) + 1);
@@ -232,7 +239,7 @@ __device__ __forceinline__ void store_split8(const float (&x)[8], float s, unsig
 }
 
 // ---- prologue: the A operand rows of one 128-token block -------------------------------------------------------------
-// Warp w stages rows [16 w, 16 w + 16) in two groups of 8; lane = 8 kk + r owns row r of the group and the 8-value
+// Warp w stages rows [16 w, 16 w + 16) in two groups of 8 (d = 64; [8 w, 8 w + 8) with the 16 warps of d = 128); lane = 8 kk + r owns row r of the group and the 8-value
 // chunks kj = kk + 4 i (i < d/32).  A quarter-warp (fixed kk) reads 8 rows x 16 bytes (whole sectors once the other
 // chunks of the row are counted) and writes 8 consecutive 16-byte rows of one core matrix: no bank conflict.
 // Keys: RoPE from the fp64-evaluated table, power-of-two row scale, two-term split.  Values: fp16 rows are exact
@@ -242,10 +249,11 @@ __device__ __forceinline__ void stage_rows(const T* __restrict__ src, int i_firs
                                            const float* __restrict__ cs_blk /* rope_cs row of block row 0 */, int rows_cs /* rows of the table left */,
                                            int rope_layout, unsigned char* ahi, unsigned char* alo, float* scale_s, int warp, int lane) {
   constexpr int NI = D / 32;  // chunks per lane and row
+  constexpr int GPW = 16 / (kThreadsOf<D> / 32);  // groups of 8 rows per warp: 2 (8 warps) | 1 (16 warps)
   const int r = lane & 7, kk = lane >> 3;
 #pragma unroll
-  for (int gi = 0; gi < 2; ++gi) {
-    const int row = 16 * warp + 8 * gi + r;
+  for (int gi = 0; gi < GPW; ++gi) {
+    const int row = 8 * GPW * warp + 8 * gi + r;
     const int i = i_first + row;
     const bool valid = i >= 0 && i < n_tokens;
     const T* p = src + (size_t)i * D;
@@ -322,20 +330,27 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
   using Lo = Layout<D>;
   constexpr bool kF16 = sizeof(T) == 2;
   constexpr int KCW = Lo::KCW, KSW = Lo::KSW;
-  constexpr int NC = D / 2;  // accumulator columns per thread
+  constexpr int NC = 32;                       // accumulator columns per thread
+  constexpr int kParts = Cfg::kParts, kThreads = Cfg::kThreads;
   unsigned char *B0_hi = smem, *B0_lo = smem + Cfg::kMatBytes;                               // PI_K | PI_V
   unsigned char *B1_hi = smem + 2 * Cfg::kMatBytes, *B1_lo = smem + 3 * Cfg::kMatBytes;      // S (keys only)
   unsigned char *A_hi = smem + Cfg::kOffA, *A_lo = A_hi + Cfg::kOpBytes;
   unsigned char* img = smem + Cfg::kOffMisc;                                  // [4 tiles][kImgBytes]
-  float* red_n = reinterpret_cast<float*>(img + 4 * Cfg::kImgBytes);          // [2 halves][128] partial |y|^2
-  float* red_g = red_n + 2 * kBlk;                                            // [2 halves][128] partial |8 r|^2
-  float* scale_s = red_g + 2 * kBlk;                                          // [128] inverse row scales
+  float* red_n = reinterpret_cast<float*>(img + 4 * Cfg::kImgBytes);          // [parts][128] partial |y|^2
+  float* red_g = red_n + kParts * kBlk;                                       // [parts][128] partial |8 r|^2
+  float* scale_s = red_g + kParts * kBlk;                                     // [128] inverse row scales
   float2* lutp = reinterpret_cast<float2*>(scale_s + kBlk);                   // [64] keys: (-8 lut[c0], -8 lut[c1]) at c0 + 8 c1
   unsigned long long* mbar = reinterpret_cast<unsigned long long*>(lutp + 64);  // [0]: first product, [1]: S product
   unsigned* tmem_slot = reinterpret_cast<unsigned*>(mbar + 3);
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int tok = tid & (kBlk - 1), half = tid >> 7;  // epilogue role: token row and column half
+  const int tok = tid & (kBlk - 1), half = tid >> 7;  // epilogue role: token row and column part ("half" at d = 64)
+  auto part_sum = [&](const float* red) {               // the token's sum over the parts, in a fixed order
+    float acc = red[tok];
+#pragma unroll
+    for (int q = 1; q < kParts; ++q) acc += red[q * kBlk + tok];
+    return acc;
+  };
   const int bh = blockIdx.y, b = bh / a.cv.H, h = bh % a.cv.H;
   const int first_blk = a.start_pos / kBlk, last_blk = (a.start_pos + a.n_tokens - 1) / kBlk;
   const int blk0 = first_blk + cta_x * blocks_per_cta;
@@ -481,7 +496,7 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
       red_n[half * kBlk + tok] = (p0 + p1) + (p2 + p3);
     }
     __syncthreads();
-    const float n = sqrtf(red_n[tok] + red_n[kBlk + tok]);
+    const float n = sqrtf(part_sum(red_n));
     const float row_scale = 16.f / scale_s[tok];  // y = 16 s PI x, s a power of two
     const unsigned short n_h = kLit ? kF16One : f32_to_f16_bits_clamped(n * scale_s[tok] * 0.0625f);
     // thresholds on the accumulator scale: t |y| for the unit vector, t 16 s for the activation itself (literal mode)
@@ -543,7 +558,7 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
       if (valid && half == 0)
         reinterpret_cast<unsigned*>(timg + kOffImgNK)[slot_lane(slot)] =
             (unsigned)n_h |
-            ((unsigned)(kLit ? lit_rnorm : f32_to_f16_bits_clamped(sqrtf(red_g[tok] + red_g[kBlk + tok]) * 0.125f)) << 16);
+            ((unsigned)(kLit ? lit_rnorm : f32_to_f16_bits_clamped(sqrtf(part_sum(red_g)) * 0.125f)) << 16);
       // ---- residual sketch: bit j = [(S r)_j >= 0] for this thread's sketch rows [half d/2, + d/2).  Sketch rows
       //      [t d/4, (t+1) d/4) belong to lane (sg, t) as 16-bit pieces u; a piece is stored as two bytes of word (mt, u):
       //      byte (sr & 1) holds bits 0..7, byte 2 + (sr & 1) bits 8..15 (the byte interleave with the slot 8 further on
@@ -661,13 +676,13 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
       unsigned char* vimg = timg + Cfg::kImgV;
       if (valid && half == 0)
         reinterpret_cast<unsigned short*>(vimg + Vs::kOffVR)[slot_lane(slot)] =
-            f32_to_f16_bits_clamped(sqrtf(red_g[tok] + red_g[kBlk + tok]) * 0.125f);
+            f32_to_f16_bits_clamped(sqrtf(part_sum(red_g)) * 0.125f);
       mbar_wait(smem_u32(mbar + 1), parity);
       tc_fence_after();
       tmem_ld<NC>(t_lane + D, y);
       if (valid) {
         const int ks = slot >> 4, th = (slot >> 3) & 1, ts = (slot & 7) >> 1, e = slot & 1;
-        const int word = ks * (D / 64) + (D == 64 ? 0 : half);  // the m-tiles of this thread's rows share one word
+        const int word = ks * (D / 64) + (half >> 1);  // the two m-tiles of this thread's rows (2 part, 2 part + 1) share one word
 #pragma unroll
         for (int g = 0; g < 8; ++g) {
           unsigned bits = 0u, own = 0u;
@@ -722,7 +737,7 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
 // grid = (block groups, batch x heads, keys | values): the key CTAs (the long ones) are dispatched first and the value
 // CTAs fill in behind them (measured: alternating key and value CTAs along x is 8 % slower at configs[2])
 template <int D, typename T, bool kLit, bool kVq>
-__global__ void __launch_bounds__(kThreads, D == 64 ? 3 : 1) quantize_pack_tc_kernel(QuantArgs a, int blocks_per_cta) {
+__global__ void __launch_bounds__(kThreadsOf<D>, D == 64 ? 3 : 1) quantize_pack_tc_kernel(QuantArgs a, int blocks_per_cta) {
   extern __shared__ __align__(1024) unsigned char smem_dyn[];
   if (blockIdx.z == 0) quantize_pack_tc_body<D, T, true, kLit, kVq>(a, blocks_per_cta, (int)blockIdx.x, smem_dyn);
   else quantize_pack_tc_body<D, T, false, kLit, kVq>(a, blocks_per_cta, (int)blockIdx.x, smem_dyn);
@@ -740,7 +755,7 @@ cudaError_t launch_quant_tc_t(const QuantArgs& a, int num_sms, cudaStream_t st) 
   dim3 grid((nblk + bpc - 1) / bpc, BH, 2);  // z: keys | values
   cudaError_t e = cudaFuncSetAttribute(quantize_pack_tc_kernel<D, T, kLit, kVq>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
-  quantize_pack_tc_kernel<D, T, kLit, kVq><<<grid, kThreads, smem, st>>>(a, bpc);
+  quantize_pack_tc_kernel<D, T, kLit, kVq><<<grid, kThreadsOf<D>, smem, st>>>(a, bpc);
   count_launch();
   return cudaGetLastError();
 }
