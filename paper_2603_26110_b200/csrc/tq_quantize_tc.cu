@@ -424,7 +424,24 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
   constexpr int kOffImgKS = Lo::kCodeBytes, kOffImgNK = Lo::kCodeBytes + Lo::kSignBytes;  // keys image
   constexpr int kOffImgVN = Lo::kCodeBytes;                                                // values image
   // byte `sb` of lane l's word string in a section of W words per lane
-  auto sec_byte = [](int W, int l, int sb) { return word_offset(W, sb >> 2, l) + (sb & 3); };
+  // The code section of the IMAGE is not in the order of the tile: inside every [16-byte chunk][lane] array the lane index
+  // is permuted so that the byte stores of one warp instruction (32 consecutive tokens, one fixed byte of their fields) land
+  // in eight different 16-byte bank groups instead of two (ncu: 4-6 wavefronts per byte store before).  Keys: the eight
+  // lanes 4 g + t (g = 0..7) of a fixed t -> g + 8 t; values: lanes 4 gi + tt with (tt, gi >> 2) varying -> tt + 4 (gi >> 2)
+  // + 8 (gi & 3).  The copies between image and tile (pre-load, write-out) apply the permutation per 16-byte unit.
+  auto perm_lane = [](int l) { return kKey ? (l >> 2) + 8 * (l & 3) : (l & 3) + 4 * (l >> 4) + 8 * ((l >> 2) & 3); };
+  // byte `sb` of lane l's word string in the code section (W words per lane) of the image
+  auto sec_byte = [&](int W, int l, int sb) {
+    const int w = sb >> 2;
+    return (w < (W / 4) * 4 ? word_offset(W, w, perm_lane(l)) : word_offset(W, w, l)) + (sb & 3);
+  };
+  // image offset of the 16-byte unit at byte `ib` of the CTA's share of a tile (code section first, then the rest)
+  auto img_unit = [&](int ib) {
+    constexpr int kChunked = (KCW / 4) * 16 * kTile;  // bytes of the [chunk][lane] arrays of the code section
+    if (ib >= kChunked) return ib;
+    const int q = ib >> 4;
+    return ((q & ~31) + perm_lane(q & 31)) << 4;
+  };
 
   for (int blk = blk0; blk <= blk1; ++blk) {
     const uint32_t parity = (uint32_t)(blk - blk0) & 1u;
@@ -448,7 +465,7 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
         const int ib = 16 * q;
         const int gb = kKey ? (ib < Lo::kOffVC ? ib : Lo::kOffNK + (ib - Lo::kOffVC))
                             : (ib < Lo::kCodeBytes ? Lo::kOffVC + ib : Lo::kOffVN + (ib - Lo::kCodeBytes));
-        *reinterpret_cast<uint4*>(img + t4 * Cfg::kImgBytes + ib) = *reinterpret_cast<const uint4*>(tg + gb);
+        *reinterpret_cast<uint4*>(img + t4 * Cfg::kImgBytes + img_unit(ib)) = *reinterpret_cast<const uint4*>(tg + gb);
       }
     }
 
@@ -721,7 +738,7 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
         const int ib = 16 * q;
         const int gb = kKey ? (ib < Lo::kOffVC ? ib : Lo::kOffNK + (ib - Lo::kOffVC))
                             : (ib < Lo::kCodeBytes ? Lo::kOffVC + ib : Lo::kOffVN + (ib - Lo::kCodeBytes));
-        *reinterpret_cast<uint4*>(tg + gb) = *reinterpret_cast<const uint4*>(img + t4 * Cfg::kImgBytes + ib);
+        *reinterpret_cast<uint4*>(tg + gb) = *reinterpret_cast<const uint4*>(img + t4 * Cfg::kImgBytes + img_unit(ib));
       }
     }
     __syncthreads();  // the next block pre-loads into / writes the same images
