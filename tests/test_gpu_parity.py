@@ -956,3 +956,48 @@ def test_value_sketch_model_step_equals_per_layer_calls(tq, oracle):
     for i in (1, 2):
         assert torch.isfinite(outs[0].float()).all() and torch.equal(outs[0], outs[i])
         assert torch.equal(caches[0].data, caches[i].data)
+
+
+@pytest.mark.gpu
+def test_full_size_cfg2_with_value_sketch_sampled_units(tq, oracle):
+    """configs[2] at full size with v_qjl = 1, in the launch configuration `bench.py --v-qjl` times (batch 32 x 20 heads x
+    1024 tokens + one appended token, fp16, 4 CTAs per SM): the GPU quantises and decodes everything, the oracle
+    re-computes two batch entries (all eight planes; decode on the GPU's exported bytes vs tqo_decode_attn_vq)."""
+    import torch
+
+    w = W.CONFIGS["cfg2_650m_batch32"]
+    d, H, B, T0 = w.head_dim, w.n_heads, w.batch, w.seq
+    shape = tq.make_shape(1, B, H, d, T0 + 128, w.rope_base, 0, v_qjl=1)
+    cal = tq.tq_calibrate_host(shape, 1, seed=w.seed)  # the bench's calibration: binary16-representable LUTs (fast path)
+    params = tq.Params(cal)
+    cache = tq.Cache(shape)
+    dev = lambda x: torch.from_numpy(np.ascontiguousarray(x)).cuda()
+    k, v = W.layer_activations(w, 0)
+    tq.tq_quantize_pack(shape, params, cache, 0, dev(k), dev(v))
+    q, kn, vn = W.step_tokens(w, 0, 0)
+    qd = dev(q[None])
+    out = torch.full_like(qd, float("nan"))
+    ws = tq.Workspace(shape, 1)
+    tq.tq_decode_step(shape, params, cache, 0, qd[0], dev(kn), dev(vn), out[0], ws, T0 + 128)
+    torch.cuda.synchronize()
+    T = T0 + 1
+    assert torch.all(cache.seq_len == T)
+    planes = {n: p.cpu().numpy() for n, p in tq.tq_cache_export_canonical(shape, cache, 0, T).items()}
+    sample = [5, 30]
+    kk = np.concatenate([k[sample], kn[sample][:, :, None]], axis=2)
+    vv = np.concatenate([v[sample], vn[sample][:, :, None]], axis=2)
+    can = oracle.quantize_pack(kk, vv, cal["pi_k"][0], cal["pi_v"][0], cal["lut_k"][0], cal["lut_v"][0], cal["S"],
+                               base=w.rope_base, near_eps=TL.NEAR_EPS)
+    oracle.add_value_sketch(can, vv, cal["pi_v"][0], cal["lut_v"][0], cal["S"])
+    rep = _vq_compare(can, {n: p[sample] for n, p in planes.items()}, d, "cfg2 full size, v_qjl")
+    print("cfg2 full size with the V sketch, quantize (2 of 32 batch entries):", {a: b for a, b in rep.items() if not a.endswith("equal")})
+    gcan = oracle.Canonical(*[planes[n][sample] if "norm" not in n else planes[n][sample].view(np.uint16)
+                              for n in ("k_codes", "k_signs", "k_norm", "k_rnorm", "v_codes", "v_norm")])
+    gcan.v_signs, gcan.v_rnorm = planes["v_signs"][sample], planes["v_rnorm"][sample].view(np.uint16)
+    sl = np.full(len(sample), T, np.int32)
+    want = oracle.decode_attn_vq(q[sample], sl - 1, sl, cal["pi_k"][0], cal["pi_v"][0], cal["lut_k"][0], cal["lut_v"][0],
+                                 cal["S"], gcan, base=w.rope_base)
+    got = out[0].float().cpu().numpy()
+    ulp = np.spacing(np.abs(want).astype(np.float16)).astype(np.float64)
+    assert np.all(np.abs(got[sample].astype(np.float64) - want) <= ulp + TL.OUT_MAX_ABS)
+    assert np.all(np.isfinite(got))
