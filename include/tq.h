@@ -276,7 +276,8 @@ int64_t tq_launch_count(void);
  * tq_decode_attn / tq_decode_model_step skip the append + query-prep kernel and re-use the query operands their
  * previous ordinary call left in the workspace (same queries, same layers), so that a run of such calls times
  * the streaming kernel alone.  Process-wide, not thread-safe; results are only meaningful directly after an
- * ordinary call with the same arguments; always switch it off again.                                      */
+ * ordinary call with the same arguments; always switch it off again.  on = 2: tq_decode_model_step also leaves out its
+ * finish kernel (the streaming launches alone; the outputs are then not written).                          */
 void tq_profile_decode_main_only(int on);
 /* Test / sweep knobs (process-wide, not part of the product path; both default to 0 = the library's own choice):
  * CTAs per unit of the streaming decode kernel; 1 = route tq_quantize_pack to the fp32 CUDA-core cross-check kernel. */

@@ -144,7 +144,7 @@ def tq_launch_count() -> int:
 
 def tq_profile_decode_main_only(on: bool):
     """Measurement hook: tq_decode_attn launches only the streaming kernel (queries from the previous ordinary call)."""
-    lib().tq_profile_decode_main_only(C.c_int(1 if on else 0))
+    lib().tq_profile_decode_main_only(C.c_int(int(on)))  # 0 off, 1 skip the prep kernel, 2 also skip the finish kernel
 
 
 # ---- calibration (host) -------------------------------------------------------------------------------

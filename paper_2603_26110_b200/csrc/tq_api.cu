@@ -380,7 +380,8 @@ int tq_decode_model_step(const tq_shape* shape, const tq_params* dev, tq_cache* 
     b.chain_mode = l == 0 ? 0 : 1;
     if (launch_decode(b, p.g.D, false, st) != cudaSuccess) return TQ_ERR_CUDA;
   }
-  if (launch_finish(p.a, p.g.D, true, st) != cudaSuccess) return TQ_ERR_CUDA;
+  // (measurement hook level 2: the streaming launches alone, without the finish kernel)
+  if (g_profile_skip_prep != 2 && launch_finish(p.a, p.g.D, true, st) != cudaSuccess) return TQ_ERR_CUDA;
   return TQ_OK;
 }
 
@@ -651,7 +652,7 @@ const char* tq_status_string(int status) {
 
 int64_t tq_launch_count(void) { return (int64_t)tq::g_launches.load(); }
 
-void tq_profile_decode_main_only(int on) { tq::g_profile_skip_prep = on != 0; }
+void tq_profile_decode_main_only(int on) { tq::g_profile_skip_prep = on < 0 ? 0 : (on > 2 ? 2 : on); }
 
 void tq_debug_set_quantize_impl(int fp32_cuda_cores) { tq::debug_set_quantize_fp32(fp32_cuda_cores); }
 
