@@ -535,6 +535,24 @@ def run_cfg2(args, w: W.Workload):
         chain_us = rig.graph_us(one_step, L)          # the streaming launches alone: the dominant kernel
     finally:
         tq.tq_profile_decode_main_only(0)
+    # ---- the same chain with a FLAT softmax (queries = 0: every logit equal, every cached value contributes).  On the
+    #      configs[2] inputs the softmax is extremely peaked and the kernel skips the value MMAs of 16-token halves whose
+    #      weights underflow to exactly 0; the flat case is the other end: all of the work, every tile
+    qz = torch.zeros_like(qs)
+
+    def flat_step():
+        tq.tq_decode_model_step(shape, params, cache, 0, L, qz, kn, vn, outs, wsL, max_seq, stream)
+
+    with torch.cuda.stream(stream):
+        reset_len()
+        flat_step()
+        stream.synchronize()
+    reset_len()
+    tq.tq_profile_decode_main_only(2)
+    try:
+        chain_flat_us = rig.graph_us(flat_step, L)
+    finally:
+        tq.tq_profile_decode_main_only(0)
     wss = [tq.Workspace(shape, 1, dev) for _ in range(L)]  # one workspace per layer keeps every layer's operands alive
 
     def decode_all_layers_ws():
@@ -649,6 +667,9 @@ def run_cfg2(args, w: W.Workload):
                      "how": f"{L} launches (one per layer cache) as the model step chains them (prep and finish kernels left out "
                             f"through the library's measurement hook), CUDA events around the graph, / {L}",
                      "frac_with_finish_kernel": dec_bytes / chain_finish_us / 1e3 / peak,
+                     "frac_flat_softmax": dec_bytes / chain_flat_us / 1e3 / peak,
+                     "flat_softmax": "same chain with zero queries (uniform weights: no value work is skipped); the headline "
+                                     "inputs have a peaked softmax and the kernel skips value MMAs of halves whose weights are 0",
                      "frac_isolated_launch": dec_bytes / iso_us / 1e3 / peak,
                      "frac_call": dec_bytes / call_us / 1e3 / peak,
                      "frac_step": value / world * rig.bpt / 1e9 / peak},
