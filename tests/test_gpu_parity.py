@@ -769,7 +769,8 @@ def _np_rope_keys(k, start_pos, base):
 @pytest.mark.gpu
 @pytest.mark.parametrize("name,kw,gauss_S", [("cfg2_650m_batch32", dict(batch=3, n_heads=4, seq=300), False),
                                              ("cfg4_15b_heads", dict(batch=2, n_heads=3, seq=170), False),
-                                             ("cfg2_650m_batch32", dict(batch=2, n_heads=3, seq=140), True)])
+                                             ("cfg2_650m_batch32", dict(batch=2, n_heads=3, seq=140), True),
+                                             ("cfg0_tiny", dict(batch=2, n_heads=2, seq=100), False)])
 def test_paper_literal_mode_matches_oracle(tq, oracle, name, kw, gauss_S):
     """residual_mode = 1.  Calibration from the product
     (tq_calibrate_host mode 0 in literal mode: SVD PI_K, PI_V = I, S = I, LUTs on the raw rotated activations, e-bar =
@@ -1001,3 +1002,47 @@ def test_full_size_cfg2_with_value_sketch_sampled_units(tq, oracle):
     ulp = np.spacing(np.abs(want).astype(np.float16)).astype(np.float64)
     assert np.all(np.abs(got[sample].astype(np.float64) - want) <= ulp + TL.OUT_MAX_ABS)
     assert np.all(np.isfinite(got))
+
+
+@pytest.mark.gpu
+def test_value_sketch_ragged_and_empty_caches(tq, oracle):
+    """v_qjl = 1 with a different cache length per batch entry (one of them empty, one ending inside a tile, one on a tile
+    boundary), explicit query positions, split and unsplit: decode on the oracle's bytes vs tqo_decode_attn_vq."""
+    import torch
+
+    w = W.CONFIGS["cfg2_650m_batch32"].scaled(batch=4, n_heads=3, seq=200)
+    d, H, B, T = w.head_dim, w.n_heads, w.batch, w.seq
+    shape = tq.make_shape(1, B, H, d, T, w.rope_base, 0, v_qjl=1)
+    rope_cs = tq.tq_calibrate_host(shape, 1, seed=1)["rope_cs"]
+    arr = TL.make_arrays(oracle, w, rope_cs, lut_scale_v=0.9, per_head_lut=True)
+    params = tq.Params(arr)
+    k, v = W.layer_activations(w, 0)
+    can = oracle.quantize_pack(k, v, arr["pi_k"][0], arr["pi_v"][0], arr["lut_k"][0], arr["lut_v"][0], arr["S"], base=w.rope_base)
+    oracle.add_value_sketch(can, v, arr["pi_v"][0], arr["lut_v"][0], arr["S"])
+    cache = tq.Cache(shape)
+    tc = TL.to_torch_canonical(can)
+    tc["v_signs"] = torch.from_numpy(can.v_signs).cuda()
+    tc["v_rnorm"] = torch.from_numpy(can.v_rnorm.view(np.int16)).cuda()
+    tq.tq_cache_import_canonical(shape, cache, 0, T, tc)
+    sl = np.array([0, 77, 128, 200], np.int32)
+    qp = np.array([0, 90, 127, 3], np.int32)
+    cache.seq_len[0] = torch.from_numpy(sl).cuda()
+    q = W.queries(w, 0)
+    want = oracle.decode_attn_vq(q, qp, sl, arr["pi_k"][0], arr["pi_v"][0], arr["lut_k"][0], arr["lut_v"][0], arr["S"], can,
+                                 base=w.rope_base)
+    assert np.all(want[0] == 0)
+    qd = torch.from_numpy(q[None]).cuda()
+    qpd = torch.from_numpy(qp[None]).cuda()
+    ws = tq.Workspace(shape, 1)
+    try:
+        for nsplit in (0, 2, 5):
+            tq.tq_debug_set_decode_nsplit(nsplit)
+            out = torch.full_like(qd, float("nan"))
+            tq.tq_decode_attn(shape, params, cache, 0, 1, qd, out, ws, qpd)
+            torch.cuda.synchronize()
+            got = out[0].float().cpu().numpy()
+            assert np.all(got[0] == 0), "an empty cache gives out = 0"
+            ulp = np.spacing(np.abs(want).astype(np.float16)).astype(np.float64)
+            assert np.all(np.abs(got.astype(np.float64) - want) <= ulp + TL.OUT_MAX_ABS), (nsplit, np.abs(got - want).max())
+    finally:
+        tq.tq_debug_set_decode_nsplit(0)
