@@ -44,7 +44,9 @@ struct TcCfg {
   static constexpr int kSBO = 16 * D;              // bytes between 8-row groups of an operand: 1024 | 2048
   static constexpr int kOpBytes = kBlk * D * 2;    // one fp16 A operand: 16 | 32 KB
   static constexpr int kMatBytes = D * D * 2;      // one fp16 B operand: 8 | 32 KB
-  static constexpr int kTmemCols = 2 * D;          // key CTAs: D_K [0,d), D_S [d,2d); value CTAs: D_V [0,d)
+  // tensor memory columns: [0, d) the accumulator (D_K / D_V, then — once every thread holds those in registers — D_S of the
+  // residual product); [d, 3d/2) and [3d/2, 2d) the residual operand 8 r as fp16 hi and lo parts (two k per column)
+  static constexpr int kTmemCols = 2 * D;
   // instruction descriptor: kind::f16, A = B = fp16 (K-major), D = fp32, N = d, M = 128
   static constexpr uint32_t kIdesc = (1u << 4) | ((uint32_t)(D >> 3) << 17) | ((128u >> 4) << 24);
   // image of one tile's sections owned by a CTA: keys [K codes | K signs | norms k,r], values [V codes | norm v]
@@ -76,6 +78,23 @@ __device__ __forceinline__ void umma_f16(uint32_t tmem_d, uint64_t adesc, uint64
       "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
       "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
       ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
+// the same with the A operand in tensor memory (lane = row, one 32-bit column per two consecutive k): no shared-memory read
+// for A at all
+__device__ __forceinline__ void umma_f16_ts(uint32_t tmem_d, uint32_t tmem_a, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}"
+      ::"r"(tmem_d), "r"(tmem_a), "l"(bdesc), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
+// 16 consecutive 32-bit columns of this thread's TMEM lane, from registers
+__device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&r)[16]) {
+  asm volatile(
+      "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};"
+      ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]),
+        "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15])
       : "memory");
 }
 __device__ __forceinline__ void umma_commit(uint32_t bar) {
@@ -414,6 +433,27 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
                (first && ks == 0) ? 0u : 1u);
   };
 
+  // the residual product D[:, 0..d) (+)= R S^T with the operand R in tensor memory (column of k-step ks: + 8 ks)
+  auto gemm_ts = [&](uint32_t a_col, uint32_t b_op, bool first) {
+#pragma unroll
+    for (int ks = 0; ks < D / 16; ++ks)
+      umma_f16_ts(tmem, tmem + a_col + 8 * ks, umma_desc<D>(b_op + ks * 256), Cfg::kIdesc, (first && ks == 0) ? 0u : 1u);
+  };
+  // this thread's 32 residual values (k = 32 part .. 32 part + 31 of its token) as hi / lo halves into tensor memory
+  auto store_residual = [&](const float (&r)[32]) {
+    uint32_t hi[16], lo[16];
+#pragma unroll
+    for (int kj = 0; kj < 4; ++kj) {
+      uint4 h4, l4;
+      split8(&r[8 * kj], h4, l4);
+      hi[4 * kj] = h4.x, hi[4 * kj + 1] = h4.y, hi[4 * kj + 2] = h4.z, hi[4 * kj + 3] = h4.w;
+      lo[4 * kj] = l4.x, lo[4 * kj + 1] = l4.y, lo[4 * kj + 2] = l4.z, lo[4 * kj + 3] = l4.w;
+    }
+    const uint32_t lane_base = tmem + ((uint32_t)((warp & 3) * 32) << 16);
+    tmem_st16(lane_base + D + 16 * half, hi);
+    tmem_st16(lane_base + D + D / 2 + 16 * half, lo);
+    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+  };
   const T* src = reinterpret_cast<const T*>(kKey ? a.k : a.v) + (size_t)bh * a.n_tokens * D;
   unsigned char* stream = a.cv.tiles + ((size_t)a.layer * a.cv.B * a.cv.H + bh) * a.cv.stream_bytes;
   using Vs = VskLayout<D>;
@@ -557,19 +597,12 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
             for (int k = 0; k < 3; ++k) timg[sec_byte(KCW, 4 * sg + t, sb + k)] = (unsigned char)(w24 >> (8 * k));
           }
       }
-#pragma unroll
-      for (int kj = 0; kj < NC / 8; ++kj) {
-        uint4 hi, lo;
-        split8(&y[8 * kj], hi, lo);
-        *reinterpret_cast<uint4*>(A_hi + core_off<D>(tok, half * NC + 8 * kj)) = hi;
-        *reinterpret_cast<uint4*>(A_lo + core_off<D>(tok, half * NC + 8 * kj)) = lo;
-      }
-      fence_async_smem();
+      store_residual(y);
       tc_fence_before();
       __syncthreads();
       if (tid == 0) {
         tc_fence_after();
-        gemm(D, a_hi, b1_hi, true), gemm(D, a_lo, b1_hi, false), gemm(D, a_hi, b1_lo, false);
+        gemm_ts(D, b1_hi, true), gemm_ts(D + D / 2, b1_hi, false), gemm_ts(D, b1_lo, false);
         umma_commit(smem_u32(mbar + 1));
       }
       if (valid && half == 0)
@@ -582,7 +615,7 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
       //      makes the decode kernel's fp16x2 masks work)
       mbar_wait(smem_u32(mbar + 1), parity);
       tc_fence_after();
-      tmem_ld<NC>(t_lane + D, y);
+      tmem_ld<NC>(t_lane, y);  // D_S took the accumulator columns
 #pragma unroll
       for (int c = 0; c < NC / 32; ++c) {
         // [y >= 0] = sat(y 2^100 + 1), sixteen bits summed exactly in one float
@@ -635,19 +668,12 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
       }
       if constexpr (kVq) {  // the residual operand of the S product over this token's operand row
         red_g[half * kBlk + tok] = g2a + g2b;
-#pragma unroll
-        for (int kj = 0; kj < NC / 8; ++kj) {
-          uint4 hi, lo;
-          split8(&y[8 * kj], hi, lo);
-          *reinterpret_cast<uint4*>(A_hi + core_off<D>(tok, half * NC + 8 * kj)) = hi;
-          *reinterpret_cast<uint4*>(A_lo + core_off<D>(tok, half * NC + 8 * kj)) = lo;
-        }
-        fence_async_smem();
+        store_residual(y);
         tc_fence_before();
         __syncthreads();
         if (tid == 0) {
           tc_fence_after();
-          gemm(D, a_hi, b1_hi, true), gemm(D, a_lo, b1_hi, false), gemm(D, a_hi, b1_lo, false);
+          gemm_ts(D, b1_hi, true), gemm_ts(D + D / 2, b1_hi, false), gemm_ts(D, b1_lo, false);
           umma_commit(smem_u32(mbar + 1));
         }
       }
@@ -696,7 +722,7 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
             f32_to_f16_bits_clamped(sqrtf(part_sum(red_g)) * 0.125f);
       mbar_wait(smem_u32(mbar + 1), parity);
       tc_fence_after();
-      tmem_ld<NC>(t_lane + D, y);
+      tmem_ld<NC>(t_lane, y);  // D_S took the accumulator columns
       if (valid) {
         const int ks = slot >> 4, th = (slot >> 3) & 1, ts = (slot & 7) >> 1, e = slot & 1;
         const int word = ks * (D / 64) + (half >> 1);  // the two m-tiles of this thread's rows (2 part, 2 part + 1) share one word
