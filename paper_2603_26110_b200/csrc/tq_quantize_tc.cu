@@ -42,7 +42,11 @@ struct TcCfg {
   static constexpr int kParts = D / 32;            // threads per token
   static constexpr int kThreads = kThreadsOf<D>;
   static constexpr int kSBO = 16 * D;              // bytes between 8-row groups of an operand: 1024 | 2048
-  static constexpr int kOpBytes = kBlk * D * 2;    // one fp16 A operand: 16 | 32 KB
+  // d = 64: the A operand of the FIRST product goes through tensor memory as well (stage_rows_tmem), no operand rows in
+  // shared memory at all; d = 128 keeps them in shared memory (two warps share a row there: the row maximum would need
+  // another exchange)
+  static constexpr bool kTmemA = D == 64;
+  static constexpr int kOpBytes = kTmemA ? 0 : kBlk * D * 2;    // one fp16 A operand in shared memory: 0 | 32 KB
   static constexpr int kMatBytes = D * D * 2;      // one fp16 B operand: 8 | 32 KB
   // tensor memory columns: [0, d) the accumulator (D_K / D_V, then — once every thread holds those in registers — D_S of the
   // residual product); [d, 3d/2) and [3d/2, 2d) the residual operand 8 r as fp16 hi and lo parts (two k per column)
@@ -93,6 +97,15 @@ __device__ __forceinline__ void umma_f16_ts(uint32_t tmem_d, uint32_t tmem_a, ui
 __device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&r)[16]) {
   asm volatile(
       "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};"
+      ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]),
+        "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15])
+      : "memory");
+}
+// 16 lanes x 32 columns from the warp's registers in the 16x256b shape: thread t holds, for each of the 4 repeats i, rows
+// t / 4 and t / 4 + 8 of the 16 and the columns 8 i + 2 (t % 4), + 1: {row a col 0, row a col 1, row b col 0, row b col 1}
+__device__ __forceinline__ void tmem_st_16x256b_x4(uint32_t taddr, const uint32_t (&r)[16]) {
+  asm volatile(
+      "tcgen05.st.sync.aligned.16x256b.x4.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};"
       ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]),
         "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15])
       : "memory");
@@ -338,6 +351,102 @@ __device__ __forceinline__ void stage_rows(const T* __restrict__ src, int i_firs
   }
 }
 
+// ---- prologue through tensor memory (d = 64) -------------------------------------------------------------------------------
+// Warp w stages the 16 rows [32 (w & 3) + 16 (w >> 2), + 16) of the block — the TMEM lanes it may write — in the 16x256b
+// shape: thread t owns rows t / 4 and t / 4 + 8 of them and, for i = 0..3, the four values k = 16 i + 4 (t % 4) .. + 3 (two
+// 32-bit columns of packed fp16 pairs).  A quad reads 32 contiguous bytes of a row per load (whole sectors); RoPE pairs
+// (2g, 2g + 1) sit inside a piece, pairs (g, g + 32) in pieces i and i + 2 of the same thread; the row maximum is two
+// shuffles.  The hi parts go to columns [a_col, a_col + 32), the lo parts to [a_col + 32, a_col + 64).
+template <typename T, bool kKey>
+__device__ __forceinline__ void stage_rows_tmem(const T* __restrict__ src, int i_first, int n_tokens, const float* __restrict__ cs_blk,
+                                                int rows_cs, int rope_layout, uint32_t tmem, uint32_t a_col, float* scale_s, int warp,
+                                                int lane) {
+  constexpr int D = 64;
+  const int row0 = 32 * (warp & 3) + 16 * (warp >> 2), tq4 = lane & 3;
+  uint32_t hi[16], lo[16];
+#pragma unroll
+  for (int rb = 0; rb < 2; ++rb) {  // rows t / 4 and t / 4 + 8
+    const int row = row0 + (lane >> 2) + 8 * rb;
+    const int i = i_first + row;
+    const bool valid = i >= 0 && i < n_tokens;
+    const T* p = src + (size_t)i * D + 4 * tq4;
+    if constexpr (!kKey && sizeof(T) == 2) {  // fp16 values are exact operands: the raw halves
+#pragma unroll
+      for (int ii = 0; ii < 4; ++ii) {
+        const uint2 v = valid ? __ldg(reinterpret_cast<const uint2*>(p + 16 * ii)) : make_uint2(0u, 0u);
+        hi[4 * ii + 2 * rb] = v.x, hi[4 * ii + 2 * rb + 1] = v.y;
+      }
+      if (tq4 == 0) scale_s[row] = 1.f;
+    } else {
+      float x[4][4];
+#pragma unroll
+      for (int ii = 0; ii < 4; ++ii) {
+        if (!valid) {
+          x[ii][0] = x[ii][1] = x[ii][2] = x[ii][3] = 0.f;
+        } else if constexpr (sizeof(T) == 2) {
+          const uint2 v = __ldg(reinterpret_cast<const uint2*>(p + 16 * ii));
+          const float2 f0 = __half22float2(*reinterpret_cast<const __half2*>(&v.x)), f1 = __half22float2(*reinterpret_cast<const __half2*>(&v.y));
+          x[ii][0] = f0.x, x[ii][1] = f0.y, x[ii][2] = f1.x, x[ii][3] = f1.y;
+        } else {
+          const float4 v = __ldg(reinterpret_cast<const float4*>(p + 16 * ii));
+          x[ii][0] = v.x, x[ii][1] = v.y, x[ii][2] = v.z, x[ii][3] = v.w;
+        }
+      }
+      float amax = 0.f;
+#pragma unroll
+      for (int ii = 0; ii < 4; ++ii)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) amax = fmaxf(amax, fabsf(x[ii][j]));
+      amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, 1));
+      amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, 2));
+      float sc, inv_s;
+      pow2_scale(amax, sc, inv_s);  // |RoPE(x) s| < 2 sqrt 2
+      if (tq4 == 0) scale_s[row] = inv_s;
+      if constexpr (kKey) {
+        const float* cs_row = cs_blk + (size_t)min(row, rows_cs - 1) * D;
+        if (rope_layout == 0) {  // pairs (2g, 2g + 1): values k, k + 1 use the (cos, sin) at floats [k, k + 2)
+#pragma unroll
+          for (int ii = 0; ii < 4; ++ii) {
+            const float4 c = __ldg(reinterpret_cast<const float4*>(cs_row + 16 * ii + 4 * tq4));
+            const float y0 = x[ii][0] * c.x - x[ii][1] * c.y, y1 = x[ii][0] * c.y + x[ii][1] * c.x;
+            const float y2 = x[ii][2] * c.z - x[ii][3] * c.w, y3 = x[ii][2] * c.w + x[ii][3] * c.z;
+            x[ii][0] = y0, x[ii][1] = y1, x[ii][2] = y2, x[ii][3] = y3;
+          }
+        } else {  // pairs (g, g + 32): pieces ii and ii + 2; pair g = 16 ii + 4 tq4 + j uses floats [2 g, 2 g + 2)
+#pragma unroll
+          for (int ii = 0; ii < 2; ++ii) {
+            const float4 c0 = __ldg(reinterpret_cast<const float4*>(cs_row + 2 * (16 * ii + 4 * tq4)));
+            const float4 c1 = __ldg(reinterpret_cast<const float4*>(cs_row + 2 * (16 * ii + 4 * tq4)) + 1);
+            const float cs[8] = {c0.x, c0.y, c0.z, c0.w, c1.x, c1.y, c1.z, c1.w};
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+              const float xa = x[ii][j], xb = x[ii + 2][j];
+              x[ii][j] = xa * cs[2 * j] - xb * cs[2 * j + 1];
+              x[ii + 2][j] = xa * cs[2 * j + 1] + xb * cs[2 * j];
+            }
+          }
+        }
+      }
+#pragma unroll
+      for (int ii = 0; ii < 4; ++ii) {
+#pragma unroll
+        for (int h2 = 0; h2 < 2; ++h2) {
+          const float a0 = x[ii][2 * h2] * sc, a1 = x[ii][2 * h2 + 1] * sc;
+          const __half2 hh = __floats2half2_rn(a0, a1);
+          const float2 hf = __half22float2(hh);
+          const __half2 ll = __floats2half2_rn(a0 - hf.x, a1 - hf.y);
+          hi[4 * ii + 2 * rb + h2] = *reinterpret_cast<const unsigned*>(&hh);
+          lo[4 * ii + 2 * rb + h2] = *reinterpret_cast<const unsigned*>(&ll);
+        }
+      }
+    }
+  }
+  const uint32_t taddr = tmem + ((uint32_t)row0 << 16) + a_col;
+  tmem_st_16x256b_x4(taddr, hi);
+  if constexpr (kKey || sizeof(T) == 4) tmem_st_16x256b_x4(taddr + D / 2, lo);
+  asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+}
+
 // kLit: the paper-literal Eq. 6-7 mode (include/tq.h): the accumulator is compared as it stands (no normalisation), the
 // norm plane is 1.0 and the rnorm plane the per-head constant e-bar m sqrt(2/pi)
 // kVq: the values carry a residual sketch too (tq_shape.v_qjl = 1): the value CTAs then run the S product on 8 r_v and
@@ -520,16 +629,25 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
     // ---- stage the A operand rows of the block and start the first product
     {
       const int p0 = blk * kBlk;  // cache position (= RoPE position) of block row 0
-      stage_rows<D, T, kKey>(src, p0 - a.start_pos, a.n_tokens, a.rope_cs + (size_t)min(p0, a.cv.max_seq - 1) * D,
-                             a.cv.max_seq - min(p0, a.cv.max_seq - 1), a.rope_layout, A_hi, A_lo, scale_s, warp, lane);
+      if constexpr (Cfg::kTmemA)
+        stage_rows_tmem<T, kKey>(src, p0 - a.start_pos, a.n_tokens, a.rope_cs + (size_t)min(p0, a.cv.max_seq - 1) * D,
+                                 a.cv.max_seq - min(p0, a.cv.max_seq - 1), a.rope_layout, tmem, D, scale_s, warp, lane);
+      else
+        stage_rows<D, T, kKey>(src, p0 - a.start_pos, a.n_tokens, a.rope_cs + (size_t)min(p0, a.cv.max_seq - 1) * D,
+                               a.cv.max_seq - min(p0, a.cv.max_seq - 1), a.rope_layout, A_hi, A_lo, scale_s, warp, lane);
     }
-    fence_async_smem();
+    if constexpr (!Cfg::kTmemA) fence_async_smem();
     tc_fence_before();
     __syncthreads();
     if (tid == 0) {
       tc_fence_after();
-      gemm(0, a_hi, b0_hi, true), gemm(0, a_hi, b0_lo, false);
-      if (kKey || !kF16) gemm(0, a_lo, b0_hi, false);
+      if constexpr (Cfg::kTmemA) {
+        gemm_ts(D, b0_hi, true), gemm_ts(D, b0_lo, false);
+        if (kKey || !kF16) gemm_ts(D + D / 2, b0_hi, false);
+      } else {
+        gemm(0, a_hi, b0_hi, true), gemm(0, a_hi, b0_lo, false);
+        if (kKey || !kF16) gemm(0, a_lo, b0_hi, false);
+      }
       umma_commit(smem_u32(mbar + 0));
     }
     if (tid == 32 && blk < blk1) {  // the next block's input rows on their way to L2 while this block is worked on
