@@ -897,8 +897,11 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
 
 // grid = (block groups, batch x heads, keys | values): the key CTAs (the long ones) are dispatched first and the value
 // CTAs fill in behind them (measured: alternating key and value CTAs along x is 8 % slower at configs[2])
+#ifndef TQ_QUANT_CTAS64
+#define TQ_QUANT_CTAS64 4  // 64 registers: four CTAs per SM also fill tensor memory (4 x 128 columns); measured 147 us vs 158 us with three
+#endif
 template <int D, typename T, bool kLit, bool kVq>
-__global__ void __launch_bounds__(kThreadsOf<D>, D == 64 ? 3 : 1) quantize_pack_tc_kernel(QuantArgs a, int blocks_per_cta) {
+__global__ void __launch_bounds__(kThreadsOf<D>, D == 64 ? TQ_QUANT_CTAS64 : 1) quantize_pack_tc_kernel(QuantArgs a, int blocks_per_cta) {
   extern __shared__ __align__(1024) unsigned char smem_dyn[];
   if (blockIdx.z == 0) quantize_pack_tc_body<D, T, true, kLit, kVq>(a, blocks_per_cta, (int)blockIdx.x, smem_dyn);
   else quantize_pack_tc_body<D, T, false, kLit, kVq>(a, blocks_per_cta, (int)blockIdx.x, smem_dyn);
