@@ -760,18 +760,20 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
       //      of the pair, then the pair assembles the six-bit fields code_i(even token) | code_i(odd token) << 3 of lane
       //      (i & 7, pp & 3), block j = pp >> 2: the even token builds the lanes i & 7 < 4, the odd one the others.
       //      This thread's coordinates 8 c + (i & 7), c in [half d/16, + d/16), are d/16 fields = 3 d/64 bytes per lane
-      constexpr int CW = NC / 8;  // code words of this thread
-      unsigned mine[CW], other[CW];
+      constexpr int CW = NC / 8;  // coordinates 8 c + q, c < CW, of this thread
+      // F[q] = sum_c code(8 c + q) 64^c: the token's three-bit halves of the CW six-bit fields of lane q, exact in fp32
+      float F[8];
+#pragma unroll
+      for (int q = 0; q < 8; ++q) F[q] = 0.f;
       [[maybe_unused]] const float inv8 = n > 0.f ? 8.0f / n : 0.f;
       [[maybe_unused]] float g2a = 0.f, g2b = 0.f;
 #pragma unroll
       for (int c = 0; c < CW; ++c) {
-        float w = 0.f;  // eight codes = 24 bits, exact in fp32
         if constexpr (kVq) {  // pairs of coordinates share one look-up of (-8 lut[c0], -8 lut[c1]); y becomes 8 r_v
 #pragma unroll
           for (int q = 0; q < 8; q += 2) {
             const float c0 = code_f(y[8 * c + q], sr_n), c1 = code_f(y[8 * c + q + 1], sr_n);
-            w = fmaf(c1, (float)(1u << (3 * q + 3)), fmaf(c0, (float)(1u << (3 * q)), w));
+            F[q] = fmaf(c0, (float)(1u << (6 * c)), F[q]), F[q + 1] = fmaf(c1, (float)(1u << (6 * c)), F[q + 1]);
             float2 nl;
             asm("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(nl.x), "=f"(nl.y) : "r"(f2u(fmaf(fmaf(c1, 8.f, c0), 8.f, lutp_base))));
             const float r0 = fmaf(y[8 * c + q], inv8, nl.x), r1 = fmaf(y[8 * c + q + 1], inv8, nl.y);
@@ -780,9 +782,8 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
           }
         } else {
 #pragma unroll
-          for (int q = 0; q < 8; ++q) w = fmaf(code_f(y[8 * c + q], sr_n), (float)(1u << (3 * q)), w);
+          for (int q = 0; q < 8; ++q) F[q] = fmaf(code_f(y[8 * c + q], sr_n), (float)(1u << (6 * c)), F[q]);
         }
-        mine[c] = f2u(w);
       }
       if constexpr (kVq) {  // the residual operand of the S product over this token's operand row
         red_g[half * kBlk + tok] = g2a + g2b;
@@ -795,26 +796,25 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
           umma_commit(smem_u32(mbar + 1));
         }
       }
-#pragma unroll
-      for (int c = 0; c < CW; ++c) other[c] = __shfl_xor_sync(0xffffffffu, mine[c], 1);
       if (valid && half == 0) reinterpret_cast<unsigned short*>(timg + kOffImgVN)[slot_lane(slot)] = n_h;
       {
+        // the even token of a pair builds the lanes gi = 0..3, the odd one 4..7: each hands the other the four F it needs,
+        // field word = F(even token) + 8 F(odd token), 24 bits = three bytes of lane (gi, pp & 3)'s string
         const int e = slot & 1, pp = slot >> 1;
         const bool v_partner = __shfl_xor_sync(0xffffffffu, (int)valid, 1) != 0;
         const bool v_e = e ? v_partner : valid, v_o = e ? valid : v_partner;
+        float recv[4];
+#pragma unroll
+        for (int gq = 0; gq < 4; ++gq) recv[gq] = __shfl_xor_sync(0xffffffffu, e ? F[gq] : F[4 + gq], 1);
         if (v_e || v_o) {
-          constexpr int NB = 6 * CW / 8;  // bytes per (lane, token pair, column half): 3 | 6
+          constexpr int NB = 6 * CW / 8;  // bytes per (lane, token pair, column part): 3
           // bits of the even token inside three consecutive bytes of a field string (period 24 bits)
           constexpr unsigned kEvenMask[3] = {0xC7u, 0x71u, 0x1Cu};
 #pragma unroll
           for (int gq = 0; gq < 4; ++gq) {
             const int gi = 4 * e + gq;
-            unsigned long long acc = 0ull;
-#pragma unroll
-            for (int c = 0; c < CW; ++c) {
-              const unsigned ce = ((e ? other[c] : mine[c]) >> (3 * gi)) & 7u, co = ((e ? mine[c] : other[c]) >> (3 * gi)) & 7u;
-              acc |= (unsigned long long)(ce | (co << 3)) << (6 * c);
-            }
+            const float own = e ? F[4 + gq] : F[gq];
+            const unsigned acc = f2u(e ? fmaf(own, 8.f, recv[gq]) : fmaf(recv[gq], 8.f, own));
             const int sb0 = (pp >> 2) * (6 * Lo::C / 8) + half * NB;  // byte of the lane's V string
 #pragma unroll
             for (int k = 0; k < NB; ++k) {
