@@ -9,7 +9,7 @@ import sys
 
 from .build import LIB, build
 
-WANT = ["UTCHMMA", "LDTM", "HMMA", "UBLKCP", "UBLKPF", "SYNCS", "UTMALDG", "LDGSTS", "LDS", "STS", "LDG", "STG", "LOP3", "SHF",
+WANT = ["UTCHMMA", "LDTM", "STTM", "HMMA", "UBLKCP", "UBLKPF", "SYNCS", "UTMALDG", "LDGSTS", "LDS", "STS", "LDG", "STG", "LOP3", "SHF",
         "IMAD", "FFMA", "FFMA2", "MUFU", "CREDUX", "BAR", "LDL", "STL"]
 KERNELS = ("decode_main", "prep_kernel", "quantize_pack", "finish_kernel")
 
