@@ -42,10 +42,12 @@ struct TcCfg {
   static constexpr int kParts = D / 32;            // threads per token
   static constexpr int kThreads = kThreadsOf<D>;
   static constexpr int kSBO = 16 * D;              // bytes between 8-row groups of an operand: 1024 | 2048
-  // d = 64: the A operand of the FIRST product goes through tensor memory as well (stage_rows_tmem), no operand rows in
-  // shared memory at all; d = 128 keeps them in shared memory (two warps share a row there: the row maximum would need
-  // another exchange)
-  static constexpr bool kTmemA = D == 64;
+  // the A operand of the FIRST product goes through tensor memory as well (stage_rows_tmem): no operand rows in shared
+  // memory at all (TQ_QUANT_SMEM_A = 1 keeps the shared-memory path of stage_rows for comparison)
+#ifndef TQ_QUANT_SMEM_A
+#define TQ_QUANT_SMEM_A 0
+#endif
+  static constexpr bool kTmemA = !TQ_QUANT_SMEM_A;
   static constexpr int kOpBytes = kTmemA ? 0 : kBlk * D * 2;    // one fp16 A operand in shared memory: 0 | 32 KB
   static constexpr int kMatBytes = D * D * 2;      // one fp16 B operand: 8 | 32 KB
   // tensor memory columns: [0, d) the accumulator (D_K / D_V, then — once every thread holds those in registers — D_S of the
@@ -378,78 +380,112 @@ __device__ __forceinline__ void stage_rows(const T* __restrict__ src, int i_firs
   }
 }
 
-// ---- prologue through tensor memory (d = 64) -------------------------------------------------------------------------------
-// Warp w stages the 16 rows [32 (w & 3) + 16 (w >> 2), + 16) of the block — the TMEM lanes it may write — in the 16x256b
-// shape: thread t owns rows t / 4 and t / 4 + 8 of them and, for i = 0..3, the four values k = 16 i + 4 (t % 4) .. + 3 (two
-// 32-bit columns of packed fp16 pairs).  A quad reads 32 contiguous bytes of a row per load (whole sectors); RoPE pairs
-// (2g, 2g + 1) sit inside a piece, pairs (g, g + 32) in pieces i and i + 2 of the same thread; the row maximum is two
-// shuffles.  The hi parts go to columns [a_col, a_col + 32), the lo parts to [a_col + 32, a_col + 64).
-template <typename T, bool kKey>
+// ---- prologue through tensor memory ------------------------------------------------------------------------------------
+// Warp w stages 16 rows x 64 values of the block in the 16x256b shape: rows [32 (w & 3) + 16 (j & 1), + 16) — TMEM lanes it
+// may write — and the values k in [64 cj, 64 cj + 64), j = w >> 2, cj = j >> 1 (d = 64: 8 warps, cj = 0; d = 128: 16 warps,
+// two warps share a row).  Thread t owns rows t / 4 and t / 4 + 8 of the 16 and, for i = 0..3, the four values
+// k = 64 cj + 16 i + 4 (t % 4) .. + 3 (two 32-bit columns of packed fp16 pairs).  A quad reads 32 contiguous bytes of a
+// row per load (whole sectors); RoPE pairs (2g, 2g + 1) sit inside a piece; pairs (g, g + d/2) sit in pieces i and i + 2 of
+// the same thread at d = 64 and in the other warp of the row at d = 128 (which therefore loads the partner values as
+// well); the row maximum is two shuffles, plus one exchange through shared memory at d = 128.  The hi parts go to columns
+// [a_col, a_col + d/2), the lo parts to [a_col + d/2, a_col + d).
+template <int D, typename T, bool kKey>
 __device__ __forceinline__ void stage_rows_tmem(const T* __restrict__ src, int i_first, int n_tokens, const float* __restrict__ cs_blk,
-                                                int rows_cs, int rope_layout, uint32_t tmem, uint32_t a_col, float* scale_s, int warp,
-                                                int lane) {
-  constexpr int D = 64;
-  const int row0 = 32 * (warp & 3) + 16 * (warp >> 2), tq4 = lane & 3;
+                                                int rows_cs, int rope_layout, uint32_t tmem, uint32_t a_col, float* scale_s,
+                                                float* pmax /* [2][128] scratch, d = 128 */, int warp, int lane) {
+  const int j = warp >> 2, cj = j >> 1;
+  const int row0 = 32 * (warp & 3) + 16 * (j & 1), tq4 = lane & 3, k0 = 64 * cj + 4 * tq4;
+  constexpr bool kRaw = !kKey && sizeof(T) == 2;  // fp16 values are exact operands: the raw halves
   uint32_t hi[16], lo[16];
-#pragma unroll
-  for (int rb = 0; rb < 2; ++rb) {  // rows t / 4 and t / 4 + 8
+  float x[2][4][4];
+  [[maybe_unused]] float xp[2][4][4];  // d = 128, half-split RoPE: the partner values k +- 64
+  float amax[2] = {0.f, 0.f};
+  const bool split128 = kKey && D == 128 && rope_layout == 1;
+  auto load_row = [&](int rb) {  // rows t / 4 (rb = 0) and t / 4 + 8 (rb = 1)
     const int row = row0 + (lane >> 2) + 8 * rb;
     const int i = i_first + row;
     const bool valid = i >= 0 && i < n_tokens;
-    const T* p = src + (size_t)i * D + 4 * tq4;
-    if constexpr (!kKey && sizeof(T) == 2) {  // fp16 values are exact operands: the raw halves
+    const T* p = src + (size_t)i * D + k0;
+    if constexpr (kRaw) {
 #pragma unroll
       for (int ii = 0; ii < 4; ++ii) {
         const uint2 v = valid ? __ldg(reinterpret_cast<const uint2*>(p + 16 * ii)) : make_uint2(0u, 0u);
         hi[4 * ii + 2 * rb] = v.x, hi[4 * ii + 2 * rb + 1] = v.y;
       }
-      if (tq4 == 0) scale_s[row] = 1.f;
+      if (tq4 == 0 && cj == 0) scale_s[row] = 1.f;
     } else {
-      float x[4][4];
-#pragma unroll
-      for (int ii = 0; ii < 4; ++ii) {
+      auto load4 = [&](const T* q, float (&o)[4]) {
         if (!valid) {
-          x[ii][0] = x[ii][1] = x[ii][2] = x[ii][3] = 0.f;
+          o[0] = o[1] = o[2] = o[3] = 0.f;
         } else if constexpr (sizeof(T) == 2) {
-          const uint2 v = __ldg(reinterpret_cast<const uint2*>(p + 16 * ii));
+          const uint2 v = __ldg(reinterpret_cast<const uint2*>(q));
           const float2 f0 = __half22float2(*reinterpret_cast<const __half2*>(&v.x)), f1 = __half22float2(*reinterpret_cast<const __half2*>(&v.y));
-          x[ii][0] = f0.x, x[ii][1] = f0.y, x[ii][2] = f1.x, x[ii][3] = f1.y;
+          o[0] = f0.x, o[1] = f0.y, o[2] = f1.x, o[3] = f1.y;
         } else {
-          const float4 v = __ldg(reinterpret_cast<const float4*>(p + 16 * ii));
-          x[ii][0] = v.x, x[ii][1] = v.y, x[ii][2] = v.z, x[ii][3] = v.w;
+          const float4 v = __ldg(reinterpret_cast<const float4*>(q));
+          o[0] = v.x, o[1] = v.y, o[2] = v.z, o[3] = v.w;
+        }
+      };
+#pragma unroll
+      for (int ii = 0; ii < 4; ++ii) load4(p + 16 * ii, x[rb][ii]);
+      if constexpr (D == 128 && kKey) {
+        if (split128) {
+#pragma unroll
+          for (int ii = 0; ii < 4; ++ii) load4(p + 16 * ii + (cj ? -64 : 64), xp[rb][ii]);
         }
       }
-      float amax = 0.f;
 #pragma unroll
       for (int ii = 0; ii < 4; ++ii)
 #pragma unroll
-        for (int j = 0; j < 4; ++j) amax = fmaxf(amax, fabsf(x[ii][j]));
-      amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, 1));
-      amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, 2));
+        for (int e = 0; e < 4; ++e) amax[rb] = fmaxf(amax[rb], fabsf(x[rb][ii][e]));
+      amax[rb] = fmaxf(amax[rb], __shfl_xor_sync(0xffffffffu, amax[rb], 1));
+      amax[rb] = fmaxf(amax[rb], __shfl_xor_sync(0xffffffffu, amax[rb], 2));
+      if constexpr (D == 128) {
+        if (tq4 == 0) pmax[cj * kBlk + row] = amax[rb];
+      }
+    }
+  };
+  auto finish_row = [&](int rb) {
+    {
+      const int row = row0 + (lane >> 2) + 8 * rb;
+      if constexpr (D == 128) amax[rb] = fmaxf(pmax[row], pmax[kBlk + row]);
       float sc, inv_s;
-      pow2_scale(amax, sc, inv_s);  // |RoPE(x) s| < 2 sqrt 2
-      if (tq4 == 0) scale_s[row] = inv_s;
+      pow2_scale(amax[rb], sc, inv_s);  // |RoPE(x) s| < 2 sqrt 2
+      if (tq4 == 0 && cj == 0) scale_s[row] = inv_s;
       if constexpr (kKey) {
         const float* cs_row = cs_blk + (size_t)min(row, rows_cs - 1) * D;
         if (rope_layout == 0) {  // pairs (2g, 2g + 1): values k, k + 1 use the (cos, sin) at floats [k, k + 2)
 #pragma unroll
           for (int ii = 0; ii < 4; ++ii) {
-            const float4 c = __ldg(reinterpret_cast<const float4*>(cs_row + 16 * ii + 4 * tq4));
-            const float y0 = x[ii][0] * c.x - x[ii][1] * c.y, y1 = x[ii][0] * c.y + x[ii][1] * c.x;
-            const float y2 = x[ii][2] * c.z - x[ii][3] * c.w, y3 = x[ii][2] * c.w + x[ii][3] * c.z;
-            x[ii][0] = y0, x[ii][1] = y1, x[ii][2] = y2, x[ii][3] = y3;
+            const float4 c = __ldg(reinterpret_cast<const float4*>(cs_row + k0 + 16 * ii));
+            float(&v)[4] = x[rb][ii];
+            const float y0 = v[0] * c.x - v[1] * c.y, y1 = v[0] * c.y + v[1] * c.x;
+            const float y2 = v[2] * c.z - v[3] * c.w, y3 = v[2] * c.w + v[3] * c.z;
+            v[0] = y0, v[1] = y1, v[2] = y2, v[3] = y3;
           }
-        } else {  // pairs (g, g + 32): pieces ii and ii + 2; pair g = 16 ii + 4 tq4 + j uses floats [2 g, 2 g + 2)
+        } else if constexpr (D == 64) {  // pairs (g, g + 32): pieces ii and ii + 2; pair g uses floats [2 g, 2 g + 2)
 #pragma unroll
           for (int ii = 0; ii < 2; ++ii) {
             const float4 c0 = __ldg(reinterpret_cast<const float4*>(cs_row + 2 * (16 * ii + 4 * tq4)));
             const float4 c1 = __ldg(reinterpret_cast<const float4*>(cs_row + 2 * (16 * ii + 4 * tq4)) + 1);
             const float cs[8] = {c0.x, c0.y, c0.z, c0.w, c1.x, c1.y, c1.z, c1.w};
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
-              const float xa = x[ii][j], xb = x[ii + 2][j];
-              x[ii][j] = xa * cs[2 * j] - xb * cs[2 * j + 1];
-              x[ii + 2][j] = xa * cs[2 * j + 1] + xb * cs[2 * j];
+            for (int e = 0; e < 4; ++e) {
+              const float xa = x[rb][ii][e], xb = x[rb][ii + 2][e];
+              x[rb][ii][e] = xa * cs[2 * e] - xb * cs[2 * e + 1];
+              x[rb][ii + 2][e] = xa * cs[2 * e + 1] + xb * cs[2 * e];
+            }
+          }
+        } else {  // d = 128, pairs (g, g + 64): this warp holds one member, xp the other; pair g = 16 ii + 4 tq4 + e
+#pragma unroll
+          for (int ii = 0; ii < 4; ++ii) {
+            const float4 c0 = __ldg(reinterpret_cast<const float4*>(cs_row + 2 * (16 * ii + 4 * tq4)));
+            const float4 c1 = __ldg(reinterpret_cast<const float4*>(cs_row + 2 * (16 * ii + 4 * tq4)) + 1);
+            const float cs[8] = {c0.x, c0.y, c0.z, c0.w, c1.x, c1.y, c1.z, c1.w};
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+              const float xa = cj ? xp[rb][ii][e] : x[rb][ii][e], xb = cj ? x[rb][ii][e] : xp[rb][ii][e];
+              x[rb][ii][e] = cj ? xa * cs[2 * e + 1] + xb * cs[2 * e] : xa * cs[2 * e] - xb * cs[2 * e + 1];
             }
           }
         }
@@ -458,7 +494,7 @@ __device__ __forceinline__ void stage_rows_tmem(const T* __restrict__ src, int i
       for (int ii = 0; ii < 4; ++ii) {
 #pragma unroll
         for (int h2 = 0; h2 < 2; ++h2) {
-          const float a0 = x[ii][2 * h2] * sc, a1 = x[ii][2 * h2 + 1] * sc;
+          const float a0 = x[rb][ii][2 * h2] * sc, a1 = x[rb][ii][2 * h2 + 1] * sc;
           const __half2 hh = __floats2half2_rn(a0, a1);
           const float2 hf = __half22float2(hh);
           const __half2 ll = __floats2half2_rn(a0 - hf.x, a1 - hf.y);
@@ -467,10 +503,25 @@ __device__ __forceinline__ void stage_rows_tmem(const T* __restrict__ src, int i
         }
       }
     }
+  };
+  // d = 64: one row after the other (fewest live registers); d = 128: both rows loaded, the row maxima exchanged between
+  // the two warps of a row through shared memory, then both rows finished
+  if constexpr (D == 64) {
+#pragma unroll
+    for (int rb = 0; rb < 2; ++rb) {
+      load_row(rb);
+      if constexpr (!kRaw) finish_row(rb);
+    }
+  } else {
+    load_row(0), load_row(1);
+    if constexpr (!kRaw) {
+      __syncthreads();
+      finish_row(0), finish_row(1);
+    }
   }
-  const uint32_t taddr = tmem + ((uint32_t)row0 << 16) + a_col;
+  const uint32_t taddr = tmem + ((uint32_t)row0 << 16) + a_col + 32 * cj;
   tmem_st_16x256b_x4(taddr, hi);
-  if constexpr (kKey || sizeof(T) == 4) tmem_st_16x256b_x4(taddr + D / 2, lo);
+  if constexpr (!kRaw) tmem_st_16x256b_x4(taddr + D / 2, lo);
   asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
 }
 
@@ -657,8 +708,8 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
     {
       const int p0 = blk * kBlk;  // cache position (= RoPE position) of block row 0
       if constexpr (Cfg::kTmemA)
-        stage_rows_tmem<T, kKey>(src, p0 - a.start_pos, a.n_tokens, a.rope_cs + (size_t)min(p0, a.cv.max_seq - 1) * D,
-                                 a.cv.max_seq - min(p0, a.cv.max_seq - 1), a.rope_layout, tmem, D, scale_s, warp, lane);
+        stage_rows_tmem<D, T, kKey>(src, p0 - a.start_pos, a.n_tokens, a.rope_cs + (size_t)min(p0, a.cv.max_seq - 1) * D,
+                                    a.cv.max_seq - min(p0, a.cv.max_seq - 1), a.rope_layout, tmem, D, scale_s, red_g, warp, lane);
       else
         stage_rows<D, T, kKey>(src, p0 - a.start_pos, a.n_tokens, a.rope_cs + (size_t)min(p0, a.cv.max_seq - 1) * D,
                                a.cv.max_seq - min(p0, a.cv.max_seq - 1), a.rope_layout, A_hi, A_lo, scale_s, warp, lane);

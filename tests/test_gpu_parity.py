@@ -1046,3 +1046,23 @@ def test_value_sketch_ragged_and_empty_caches(tq, oracle):
             assert np.all(np.abs(got.astype(np.float64) - want) <= ulp + TL.OUT_MAX_ABS), (nsplit, np.abs(got - want).max())
     finally:
         tq.tq_debug_set_decode_nsplit(0)
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("layout,dtype", [(0, "f16"), (1, "f16"), (1, "f32")])
+def test_quantize_pack_d128_rope_layouts_and_dtypes(tq, oracle, layout, dtype):
+    """head_dim 128, both RoPE pair conventions (the half-split one pairs coordinates that two different warps of the
+    tensor-memory prologue hold), fp16 and fp32 inputs, unaligned chunks + appended tokens vs one oracle pass."""
+    import dataclasses
+
+    # (enough vectors for the norm statistic of compare_quantize: its 2e-3 allowance for binary16 rounding ties is a rate)
+    w = dataclasses.replace(W.CONFIGS["cfg4_15b_heads"].scaled(batch=3, n_heads=4, seq=420), dtype=dtype)
+    c = Case(tq, oracle, w, max_seq=448, layout=layout, per_head_lut=True)
+    k, v = W.layer_activations(w, 0)
+    tq.tq_quantize_pack(c.shape, c.params, c.cache, 0, c.dev(k[:, :, :37]), c.dev(v[:, :, :37]), 0)
+    tq.tq_quantize_pack(c.shape, c.params, c.cache, 0, c.dev(k[:, :, 37:]), c.dev(v[:, :, 37:]), 37)
+    _, kn, vn = W.step_tokens(w, 0, 0)
+    tq.tq_append(c.shape, c.params, c.cache, 0, c.dev(kn), c.dev(vn))
+    kk, vv = np.concatenate([k, kn[:, :, None]], axis=2), np.concatenate([v, vn[:, :, None]], axis=2)
+    rep = TL.compare_quantize(c.oracle_quantize(0, kk, vv), c.gpu_export(0, w.seq + 1), w.head_dim, f"d128 layout{layout} {dtype}")
+    print(rep)
