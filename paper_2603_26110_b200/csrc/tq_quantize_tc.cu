@@ -764,7 +764,8 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
       // literal mode: residual operand = rs (y_true - lut[c]) with the power of two rs = min(16 s, lut_cap), so that
       // neither term leaves the fp16 range whatever the scale of the row
       const float rs = fminf(row_scale, lut_cap), rA = rs / row_scale, rB = rs * 0.125f;
-      float g2a = 0.f, g2b = 0.f;
+      float2 g2 = make_float2(0.f, 0.f);
+      const float2 inv8_2 = make_float2(inv8, inv8);
       float yt[4][NC / 32];  // four six-bit fields = one 24-bit word, accumulated exactly in fp32
 #pragma unroll
       for (int t = 0; t < 4; ++t)
@@ -776,14 +777,14 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
         const float field = fmaf(cc.y, 8.f, cc.x);  // c0 | c1 << 3
         float2 nl;  // (-8 lut[c0], -8 lut[c1])
         asm("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(nl.x), "=f"(nl.y) : "r"(f2u(fmaf(field, 8.f, lutp_base))));
-        float r0, r1;
-        if constexpr (kLit) r0 = fmaf(y[2 * g], rA, nl.x * rB), r1 = fmaf(y[2 * g + 1], rA, nl.y * rB);
-        else r0 = fmaf(y[2 * g], inv8, nl.x), r1 = fmaf(y[2 * g + 1], inv8, nl.y);  // 8 (u - lut[c])
-        g2a = fmaf(r0, r0, g2a), g2b = fmaf(r1, r1, g2b);
-        y[2 * g] = r0, y[2 * g + 1] = r1;
+        float2 rr;
+        if constexpr (kLit) rr = ffma2(make_float2(y[2 * g], y[2 * g + 1]), make_float2(rA, rA), fmul2(nl, make_float2(rB, rB)));
+        else rr = ffma2(make_float2(y[2 * g], y[2 * g + 1]), inv8_2, nl);  // 8 (u - lut[c])
+        g2 = ffma2(rr, rr, g2);
+        y[2 * g] = rr.x, y[2 * g + 1] = rr.y;
         yt[g & 3][g >> 4] = fmaf(field, (float)(1u << (6 * ((g >> 2) & 3))), yt[g & 3][g >> 4]);
       }
-      red_g[half * kBlk + tok] = g2a + g2b;
+      red_g[half * kBlk + tok] = g2.x + g2.y;
       if (valid) {
 #pragma unroll
         for (int t = 0; t < 4; ++t)
@@ -817,13 +818,13 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
 #pragma unroll
       for (int c = 0; c < NC / 32; ++c) {
         // [y >= 0] = sat(y 2^100 + 1), sixteen bits summed exactly in one float
-        float w0 = 0.f, w1 = 0.f;
+        float2 w01 = make_float2(0.f, 0.f);
 #pragma unroll
         for (int j = 0; j < 16; ++j) {
-          w0 = fmaf(fma_sat(y[32 * c + j], kBig, 1.f), (float)(1u << j), w0);
-          w1 = fmaf(fma_sat(y[32 * c + 16 + j], kBig, 1.f), (float)(1u << j), w1);
+          const float pw = (float)(1u << j);
+          w01 = ffma2(make_float2(fma_sat(y[32 * c + j], kBig, 1.f), fma_sat(y[32 * c + 16 + j], kBig, 1.f)), make_float2(pw, pw), w01);
         }
-        const unsigned w = f2u(w0) | (f2u(w1) << 16);
+        const unsigned w = f2u(w01.x) | (f2u(w01.y) << 16);
         if (valid) {
 #pragma unroll
           for (int q = 0; q < 2; ++q) {
