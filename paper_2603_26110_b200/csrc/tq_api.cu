@@ -481,7 +481,7 @@ int tq_host_stepper_create(const tq_shape* shape, const tq_params* dev, tq_cache
   // 8: 37.4 (more chunks = more and smaller prep launches)
   if (n_chunks <= 0) n_chunks = n_layers_call >= 16 ? 4 : (n_layers_call >= 4 ? 2 : 1);
   if (n_chunks > n_layers_call) n_chunks = n_layers_call;
-  if (n_chunks > kMaxChunks) n_chunks = kMaxChunks;
+  if (n_chunks > kMaxChunks / 2) n_chunks = kMaxChunks / 2;
   const size_t per_layer = (size_t)g.B * g.H * g.D * (dt == TQ_F16 ? 2 : 4);
   const size_t vec = (per_layer * n_layers_call + 255) / 256 * 256;
   unsigned char* s = (unsigned char*)staging;
@@ -538,7 +538,9 @@ int tq_host_stepper_create(const tq_shape* shape, const tq_params* dev, tq_cache
         bound[c] = c == n_chunks ? n_layers_call : b;
       }
     }
-    const int out_layers = n_layers_call > 6 * kMaxChunks ? (n_layers_call + kMaxChunks - 1) / kMaxChunks : 6;
+    // (a group also ends with its chunk: at most n_layers_call / out_layers + n_chunks groups, kept below kMaxChunks events)
+    const int out_room = kMaxChunks - n_chunks > 1 ? kMaxChunks - n_chunks : 1;
+    const int out_layers = n_layers_call > 6 * out_room ? (n_layers_call + out_room - 1) / out_room : 6;
     int out_begin = 0, n_out = 0;
     for (int c = 0; ok && c < n_chunks; ++c) {
       const int l0 = bound[c], l1 = bound[c + 1];
