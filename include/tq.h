@@ -181,6 +181,42 @@ int tq_decode_attn(const tq_shape *shape, const tq_params *dev, const tq_cache *
                    int32_t n_layers_call, const void *q, const int32_t *q_pos, tq_dtype dt, void *out,
                    int32_t t_hint, void *workspace, size_t workspace_bytes, void *cuda_stream);
 
+/* ---- (b) fused decode attention for callers that cannot allocate device memory -------------------------------------
+ * Who this is for.  tq_decode_attn needs a workspace, and somebody has to cudaMalloc it.  Some callers cannot: a
+ * plug-in living inside a host application whose memory pool owns the whole device and hands out input and output
+ * tensors only; code that runs where an allocation is forbidden because cudaMalloc synchronises the device (a serving
+ * loop with a latency budget, a callback of somebody else's runtime); a process started with every byte of HBM already
+ * handed to other tenants.  For them the library carries its own workspace: a zero-initialised array of
+ * TQ_NOALLOC_SCRATCH_BYTES (24 MiB) in device global memory, part of the library image.  Every GPU on which the
+ * process uses the library holds those 24 MiB from the moment the library's device code is loaded there until the
+ * process exits, whether this entry point is ever called or not.
+ *
+ * What it computes: exactly tq_decode_attn (same arguments minus workspace / workspace_bytes, same kernels, same
+ * validation and status codes, same results); the split-K partials, query operands, dequantisation tables and arrival
+ * counters live in the built-in array.  The caller still owns and passes q, q_pos, out, the cache and the calibration
+ * arrays.  The call performs no cudaMalloc / cudaFree and calls no routine that allocates; it enqueues one small
+ * cudaMemsetAsync (the arrival counters, which must start at zero) and the two kernels on cuda_stream.
+ *
+ * Limit: tq_decode_workspace_bytes(shape, n_layers_call) must not exceed TQ_NOALLOC_SCRATCH_BYTES, otherwise the
+ * call returns TQ_ERR_CAPACITY and launches nothing (tq_noalloc_scratch_bytes() returns the limit at run time).
+ * 24 MiB covers every configuration of BASELINE.json, v_qjl = 1 and all 33 layers of configs[1] in one call
+ * included (22.3 MiB); ask for fewer layers per call when a shape does not fit.
+ *
+ * First call on each device: the library looks up the device address of the array (cudaGetSymbolAddress, once per
+ * device, with that device current) and remembers it.  Make that first call outside any stream capture — e.g. one
+ * warm-up call at start-up on every device the thread will use.
+ *
+ * Sharing: there is ONE array per device and every call on that device uses it, with whatever the previous call left
+ * in it (the entry point clears the only part that has to start at zero).  Two such calls that can overlap on the
+ * GPU — different streams without an event between them, or two host threads — race on it and give wrong results:
+ * keep the calls of one device on one stream, or order them with events.  tq_decode_attn with a caller-owned
+ * workspace has no such restriction across workspaces and stays the entry point for everybody who can allocate.    */
+#define TQ_NOALLOC_SCRATCH_BYTES (24u << 20)
+size_t tq_noalloc_scratch_bytes(void);
+int tq_decode_attn_noalloc(const tq_shape *shape, const tq_params *dev, const tq_cache *cache, int32_t layer_begin,
+                           int32_t n_layers_call, const void *q, const int32_t *q_pos, tq_dtype dt, void *out,
+                           int32_t t_hint, void *cuda_stream);
+
 /* ---- one decode step of one layer, fused: tq_append(k, v) followed by tq_decode_attn(q) with the query at
  * the newly appended position, in two kernel launches instead of three (the append and the query
  * preparation share one kernel and its two small tensor-core products).  q, k, v, out: DEVICE [B][H][d], dtype dt.

@@ -21,7 +21,7 @@ TILE_TOKENS = 32
 EXPORTS = [
     "tq_cache_bytes", "tq_cache_bytes_per_token_head", "tq_cache_seq_len_offset", "tq_cache_status_offset",
     "tq_decode_workspace_bytes", "tq_canonical_plane_bytes", "tq_calibrate_host", "tq_quantize_pack", "tq_append",
-    "tq_decode_attn", "tq_decode_step", "tq_cache_export_canonical", "tq_cache_import_canonical", "tq_step_staging_bytes",
+    "tq_decode_attn", "tq_decode_attn_noalloc", "tq_noalloc_scratch_bytes", "tq_decode_step", "tq_cache_export_canonical", "tq_cache_import_canonical", "tq_step_staging_bytes",
     "tq_decode_step_host", "tq_model_step_staging_bytes", "tq_decode_model_step_host", "tq_decode_model_step", "tq_status_string", "tq_launch_count", "tq_profile_decode_main_only",
     "tq_debug_set_decode_nsplit", "tq_debug_set_quantize_impl", "tq_host_stepper_create", "tq_host_stepper_launch", "tq_host_stepper_run",
     "tq_host_stepper_destroy",
@@ -66,7 +66,7 @@ def lib():
         l = C.CDLL(LIB_PATH)
         for n in ("tq_cache_bytes", "tq_cache_bytes_per_token_head", "tq_cache_seq_len_offset",
                   "tq_cache_status_offset", "tq_decode_workspace_bytes", "tq_canonical_plane_bytes",
-                  "tq_step_staging_bytes", "tq_model_step_staging_bytes"):
+                  "tq_step_staging_bytes", "tq_model_step_staging_bytes", "tq_noalloc_scratch_bytes"):
             getattr(l, n).restype = C.c_size_t
         l.tq_status_string.restype = C.c_char_p
         l.tq_launch_count.restype = C.c_int64
@@ -237,6 +237,31 @@ def tq_decode_attn(shape, params: Params, cache: Cache, layer_begin: int, n_laye
                               C.c_int32(n_layers_call), _ptr(q), _ptr(q_pos), C.c_int(_dtype_code(q)), _ptr(out),
                               C.c_int32(t_hint), _ptr(workspace.data), C.c_size_t(workspace.bytes), _stream_ptr(stream))
     _check(rc, "tq_decode_attn")
+
+
+def tq_noalloc_scratch_bytes() -> int:
+    """Size of the workspace array built into the library (the limit of tq_decode_attn_noalloc)."""
+    return int(lib().tq_noalloc_scratch_bytes())
+
+
+def tq_decode_attn_noalloc(shape, params: Params, cache: Cache, layer_begin: int, n_layers_call: int, q, out, q_pos=None,
+                           t_hint: int = 0, stream=None):
+    """tq_decode_attn for a caller that has no way of allocating the workspace (a plug-in inside an application whose
+    memory pool owns the device, code on a path where cudaMalloc's device-wide synchronisation is not allowed, a process
+    whose HBM is already given away): the workspace is a 24 MiB array built into libtq.so, so there is no `workspace`
+    argument and the call allocates nothing.  q, out, q_pos as in tq_decode_attn.  A shape whose workspace exceeds
+    tq_noalloc_scratch_bytes() is refused (TqError, TQ_ERR_CAPACITY) before anything is launched.  All such calls on one
+    device share the array: keep them on one stream (overlapping calls race).  The first call on a device looks up the
+    array's address; make it before any stream capture."""
+    need = tq_decode_workspace_bytes(shape, n_layers_call)
+    rc = lib().tq_decode_attn_noalloc(C.byref(shape), C.byref(params.c), C.byref(cache.c), C.c_int32(layer_begin),
+                                      C.c_int32(n_layers_call), _ptr(q), _ptr(q_pos), C.c_int(_dtype_code(q)), _ptr(out),
+                                      C.c_int32(t_hint), _stream_ptr(stream))
+    if rc == TQ_ERR_CAPACITY:
+        raise TqError(rc, f"tq_decode_attn_noalloc: this shape needs {need} bytes of workspace, the array built into "
+                          f"the library holds {tq_noalloc_scratch_bytes()} (use fewer layers per call, or tq_decode_attn "
+                          "with a workspace of your own)")
+    _check(rc, "tq_decode_attn_noalloc")
 
 
 def tq_decode_step(shape, params: Params, cache: Cache, layer: int, q, k, v, out, workspace: Workspace, t_hint: int = 0,

@@ -259,6 +259,61 @@ int tq_decode_attn(const tq_shape* shape, const tq_params* dev, const tq_cache* 
                     workspace_bytes, false, true, cuda_stream);
 }
 
+}  // extern "C"
+
+// ---- tq_decode_attn_noalloc: the decode workspace inside the library image (include/tq.h says for whom) -------------
+// The array below is the workspace of tq_decode_attn for callers that cannot cudaMalloc one.  In HOST code its name is
+// only a handle for the runtime, never a pointer a kernel may be given: the device address comes from
+// cudaGetSymbolAddress, asked once per device with that device current, and is remembered per device ordinal (every
+// device has its own copy of the array at its own address).
+namespace tq {
+static __device__ __align__(256) unsigned char g_noalloc_scratch[TQ_NOALLOC_SCRATCH_BYTES];
+
+static int noalloc_scratch_address(unsigned char** out) {
+  constexpr int kMaxDev = 64;
+  static std::atomic<unsigned char*> cached[kMaxDev];  // zero-initialised: nullptr = not asked yet on that device
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess) return TQ_ERR_CUDA;
+  const bool slot = dev >= 0 && dev < kMaxDev;
+  unsigned char* p = slot ? cached[dev].load(std::memory_order_acquire) : nullptr;
+  if (!p) {  // set-up of this device (two threads may both ask: they get the same answer)
+    if (cudaGetSymbolAddress((void**)&p, g_noalloc_scratch) != cudaSuccess || !p) {
+      cudaGetLastError();
+      return TQ_ERR_CUDA;
+    }
+    if (slot) cached[dev].store(p, std::memory_order_release);
+  }
+  *out = p;
+  return TQ_OK;
+}
+}  // namespace tq
+
+extern "C" {
+
+size_t tq_noalloc_scratch_bytes(void) { return (size_t)TQ_NOALLOC_SCRATCH_BYTES; }
+
+int tq_decode_attn_noalloc(const tq_shape* shape, const tq_params* dev, const tq_cache* cache, int32_t layer_begin,
+                           int32_t n_layers_call, const void* q, const int32_t* q_pos, tq_dtype dt, void* out,
+                           int32_t t_hint, void* cuda_stream) {
+  // shape and layer count first (the size check needs them), with tq_decode_attn's own status codes; every other
+  // argument is checked by the shared validation of run_decode below, which launches nothing on an error
+  CacheGeom g;
+  int rc = check_shape(shape, &g);
+  if (rc != TQ_OK) return rc;
+  if (n_layers_call <= 0 || n_layers_call > g.L) return TQ_ERR_INVALID_ARG;
+  const WorkspaceGeom w = workspace_geom(g, n_layers_call);
+  if (w.total > (size_t)TQ_NOALLOC_SCRATCH_BYTES) return TQ_ERR_CAPACITY;  // the built-in array is too small: fewer layers per call
+  unsigned char* scratch = nullptr;
+  if ((rc = noalloc_scratch_address(&scratch)) != TQ_OK) return rc;
+  // The array keeps what the last call left there, possibly a call of another shape whose query operands or partials
+  // lie where this call's split-K arrival counters are: those must start at zero (nothing else is read before this
+  // call's own kernels have written it)
+  if (cudaMemsetAsync(scratch + w.off_counters, 0, w.off_frags - w.off_counters, (cudaStream_t)cuda_stream) != cudaSuccess)
+    return TQ_ERR_CUDA;
+  return run_decode(shape, dev, cache, layer_begin, n_layers_call, q, nullptr, nullptr, q_pos, dt, out, t_hint, scratch,
+                    (size_t)TQ_NOALLOC_SCRATCH_BYTES, false, true, cuda_stream);
+}
+
 int tq_decode_step(const tq_shape* shape, const tq_params* dev, tq_cache* cache, int32_t layer, const void* q,
                    const void* k, const void* v, tq_dtype dt, void* out, int32_t t_hint, void* workspace,
                    size_t workspace_bytes, void* cuda_stream) {
