@@ -372,7 +372,7 @@ __device__ __forceinline__ void stream_tiles(const unsigned char* stream, const 
     if constexpr (kVq) {
       unsigned short gv;
       asm volatile("ld.shared.u16 %0, [%1];" : "=h"(gv) : "r"(img + Lo::kTileBytes + Vs::kOffVR + lane * 2) : "memory");
-      wq = wv * f16_bits_to_f32(gv);
+      wq = valid ? wv * f16_bits_to_f32(gv) : 0.f;  // slots past seq_len may hold any bits (0 x NaN would poison the unit)
       wsum = fmaf(wsum, fsc, wq);
     }
     const unsigned nz = __ballot_sync(0xffffffffu, wv != 0.f);

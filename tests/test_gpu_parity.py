@@ -1049,6 +1049,61 @@ def test_value_sketch_ragged_and_empty_caches(tq, oracle):
 
 
 @pytest.mark.gpu
+@pytest.mark.parametrize("v_qjl", [0, 1])
+def test_decode_ignores_whatever_lies_beyond_seq_len(tq, oracle, v_qjl):
+    """Slots at or past seq_len belong to nobody: a cache that was imported, or never zero-filled, may hold any bits
+    there, NaN and Inf norm patterns included.  Every norm plane of the tail is set to 0x7E00 (NaN) / 0x7C00 (Inf) and
+    the code and sign planes to 0xFF; the outputs must still equal the oracle's over the first seq_len tokens (a
+    0 x NaN in the value-sketch weight used to poison the whole unit)."""
+    import torch
+
+    w = W.CONFIGS["cfg2_650m_batch32"].scaled(batch=4, n_heads=3, seq=200)
+    d, H, B, T = w.head_dim, w.n_heads, w.batch, w.seq
+    shape = tq.make_shape(1, B, H, d, T, w.rope_base, 0, v_qjl=v_qjl)
+    rope_cs = tq.tq_calibrate_host(shape, 1, seed=1)["rope_cs"]
+    arr = TL.make_arrays(oracle, w, rope_cs, lut_scale_v=0.9)
+    params = tq.Params(arr)
+    k, v = W.layer_activations(w, 0)
+    can = oracle.quantize_pack(k, v, arr["pi_k"][0], arr["pi_v"][0], arr["lut_k"][0], arr["lut_v"][0], arr["S"], base=w.rope_base)
+    sl = np.array([1, 77, 128, 183], np.int32)
+    q = W.queries(w, 0)
+    if v_qjl:
+        oracle.add_value_sketch(can, v, arr["pi_v"][0], arr["lut_v"][0], arr["S"])
+        want = oracle.decode_attn_vq(q, sl - 1, sl, arr["pi_k"][0], arr["pi_v"][0], arr["lut_k"][0], arr["lut_v"][0], arr["S"],
+                                     can, base=w.rope_base)
+    else:
+        want = oracle.decode_attn(q, sl - 1, sl, arr["pi_k"][0], arr["pi_v"][0], arr["lut_k"][0], arr["lut_v"][0], arr["S"], can,
+                                  base=w.rope_base)
+    tc = TL.to_torch_canonical(can)
+    if v_qjl:
+        tc["v_signs"] = torch.from_numpy(can.v_signs).cuda()
+        tc["v_rnorm"] = torch.from_numpy(can.v_rnorm.view(np.int16)).cuda()
+    for b in range(B):  # the oracle's planes stay as they are: only the copies handed to the GPU are spoiled
+        for n, t in tc.items():
+            if "norm" in n:
+                t[b, :, sl[b]:] = 0x7E00 if (b & 1) else 0x7C00
+            else:
+                t[b, :, sl[b]:] = 0xFF
+    cache = tq.Cache(shape)
+    tq.tq_cache_import_canonical(shape, cache, 0, T, tc)
+    cache.seq_len[0] = torch.from_numpy(sl).cuda()
+    qd = torch.from_numpy(q[None]).cuda()
+    ws = tq.Workspace(shape, 1)
+    try:
+        for nsplit in (0, 3):
+            tq.tq_debug_set_decode_nsplit(nsplit)
+            out = torch.full_like(qd, float("nan"))
+            tq.tq_decode_attn(shape, params, cache, 0, 1, qd, out, ws)
+            torch.cuda.synchronize()
+            got = out[0].float().cpu().numpy()
+            assert np.all(np.isfinite(got)), (v_qjl, nsplit)
+            ulp = np.spacing(np.abs(want).astype(np.float16)).astype(np.float64)
+            assert np.all(np.abs(got.astype(np.float64) - want) <= ulp + TL.OUT_MAX_ABS), (nsplit, np.abs(got - want).max())
+    finally:
+        tq.tq_debug_set_decode_nsplit(0)
+
+
+@pytest.mark.gpu
 @pytest.mark.parametrize("layout,dtype", [(0, "f16"), (1, "f16"), (1, "f32")])
 def test_quantize_pack_d128_rope_layouts_and_dtypes(tq, oracle, layout, dtype):
     """head_dim 128, both RoPE pair conventions (the half-split one pairs coordinates that two different warps of the
