@@ -66,7 +66,7 @@ extern "C" {
 typedef enum {
   TQ_OK = 0,
   TQ_ERR_INVALID_ARG = 1, /* NULL / misaligned pointer, negative size, layer out of range, ...          */
-  TQ_ERR_UNSUPPORTED = 2, /* head_dim not in {64,128}, qjl_dim != head_dim, v_qjl != 0                    */
+  TQ_ERR_UNSUPPORTED = 2, /* head_dim not in {64,128}, qjl_dim != head_dim, v_qjl = 1 with residual_mode = 1 */
   TQ_ERR_CAPACITY = 3,    /* host-visible: start_pos + n_tokens > max_seq; workspace / buffer too small   */
   TQ_ERR_CUDA = 4         /* a CUDA runtime call or launch failed (or no device)                         */
 } tq_status;
@@ -316,7 +316,9 @@ int64_t tq_launch_count(void);
  * finish kernel (the streaming launches alone; the outputs are then not written).                          */
 void tq_profile_decode_main_only(int on);
 /* Test / sweep knobs (process-wide, not part of the product path; both default to 0 = the library's own choice):
- * CTAs per unit of the streaming decode kernel; 1 = route tq_quantize_pack to the fp32 CUDA-core cross-check kernel. */
+ * CTAs per unit of the streaming decode kernel; 1 = route tq_quantize_pack to the fp32 CUDA-core cross-check kernel.
+ * That kernel implements the default mode only: with residual_mode = 1 or v_qjl = 1 the setting is ignored and the
+ * tensor-core kernel runs.                                                                                            */
 void tq_debug_set_decode_nsplit(int nsplit);
 void tq_debug_set_quantize_impl(int fp32_cuda_cores);
 

@@ -9,8 +9,17 @@
 namespace tq {
 
 static std::atomic<long long> g_launches{0};
-static int g_profile_skip_prep = 0;  // tq_profile_decode_main_only
-void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
+static std::atomic<int> g_profile_skip_prep{0};  // tq_profile_decode_main_only (a setter may run on another thread)
+// Launches recorded into a stream capture are not launches yet: while the stepper captures (thread-local capture mode,
+// so every recorded launch comes from this thread) they are counted apart and added at every replay.
+static thread_local bool t_capturing = false;
+static thread_local int t_captured = 0;
+void count_launch(int n) {
+  if (t_capturing)
+    t_captured += n;
+  else
+    g_launches.fetch_add(n, std::memory_order_relaxed);
+}
 
 
 constexpr int kMaxSplits = 64;  // = kMaxSegments in tq_decode.cu
@@ -238,7 +247,7 @@ static int run_decode(const tq_shape* shape, const tq_params* dev, const tq_cach
     a.ebar_k = a.literal ? dev->ebar_k : nullptr;
     const void* kc = k ? (const unsigned char*)k + u0 * g.D * esz : nullptr;
     const void* vc = v ? (const unsigned char*)v + u0 * g.D * esz : nullptr;
-    if (!(g_profile_skip_prep && do_query && !do_append) &&
+    if (!(g_profile_skip_prep.load(std::memory_order_relaxed) && do_query && !do_append) &&
         launch_prep(a, kc, vc, g.D, sms, do_append, do_query, (cudaStream_t)cuda_stream) != cudaSuccess)
       return TQ_ERR_CUDA;
     if (do_query && launch_decode(a, g.D, true, (cudaStream_t)cuda_stream) != cudaSuccess) return TQ_ERR_CUDA;
@@ -429,14 +438,15 @@ int tq_decode_model_step(const tq_shape* shape, const tq_params* dev, tq_cache* 
   // one prep launch for every layer of the step (append + query operands), then one streaming launch per layer cache:
   // the first waits for the prep kernel, the others run ahead of one another (DecodeArgs::chain_mode); they leave o'/l
   // in the workspace and one last launch applies PI_V^T to every unit of the step
-  if (!g_profile_skip_prep && launch_prep(p.a, p.k, p.v, p.g.D, p.sms, true, true, st) != cudaSuccess) return TQ_ERR_CUDA;
+  const int hook = g_profile_skip_prep.load(std::memory_order_relaxed);  // measurement hook, 0 on the product path
+  if (!hook && launch_prep(p.a, p.k, p.v, p.g.D, p.sms, true, true, st) != cudaSuccess) return TQ_ERR_CUDA;
   for (int l = 0; l < n_layers_call; ++l) {
     DecodeArgs b = sub_args(p, l, 1);
     b.chain_mode = l == 0 ? 0 : 1;
     if (launch_decode(b, p.g.D, false, st) != cudaSuccess) return TQ_ERR_CUDA;
   }
   // (measurement hook level 2: the streaming launches alone, without the finish kernel)
-  if (g_profile_skip_prep != 2 && launch_finish(p.a, p.g.D, true, st) != cudaSuccess) return TQ_ERR_CUDA;
+  if (hook != 2 && launch_finish(p.a, p.g.D, true, st) != cudaSuccess) return TQ_ERR_CUDA;
   return TQ_OK;
 }
 
@@ -505,7 +515,7 @@ int tq_decode_model_step_host(const tq_shape* shape, const tq_params* dev, tq_ca
   return TQ_OK;
 }
 
-// ---- stepper: one decode step of a run of layers captured ONCE as a CUDA graph with five branches -----------------------
+// ---- stepper: one decode step of a run of layers captured ONCE as a CUDA graph; its branches -----------------------
 //   copy      : (host buffers only) per layer chunk, the H2D copies of k, v, q, back to back
 //   prep      : per chunk, the append + query-prep kernel, behind that chunk's copies
 //   main, main2: the streaming kernels; the chains of consecutive chunks alternate between the two branches, so the first
@@ -569,7 +579,7 @@ int tq_host_stepper_create(const tq_shape* shape, const tq_params* dev, tq_cache
   tq_host_stepper* hs = ok ? new tq_host_stepper() : nullptr;
   int status = ok ? TQ_OK : TQ_ERR_CUDA;
   if (ok) {
-    const long long n0 = g_launches.load();
+    t_capturing = true, t_captured = 0;
     const bool capturing = cudaStreamBeginCapture(s_main, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
     ok = capturing && cudaEventRecord(fork, s_main) == cudaSuccess && cudaStreamWaitEvent(s_in, fork, 0) == cudaSuccess &&
          cudaStreamWaitEvent(s_out, fork, 0) == cudaSuccess && cudaStreamWaitEvent(s_copy, fork, 0) == cudaSuccess &&
@@ -637,8 +647,8 @@ int tq_host_stepper_create(const tq_shape* shape, const tq_params* dev, tq_cache
     if (capturing) ok = (cudaStreamEndCapture(s_main, &graph) == cudaSuccess && graph) && ok;
     if (ok) ok = cudaGraphInstantiate(&hs->exec, graph, 0) == cudaSuccess;
     hs->graph = graph;
-    hs->n_launches = (int)(g_launches.load() - n0);
-    g_launches.store(n0);  // nothing ran yet: the capture only recorded the launches
+    hs->n_launches = t_captured;  // nothing ran yet: the capture only recorded the launches
+    t_capturing = false;
     if (!ok) status = TQ_ERR_CUDA;
   }
   for (int c = 0; c < kMaxChunks; ++c) {
@@ -709,7 +719,7 @@ const char* tq_status_string(int status) {
 
 int64_t tq_launch_count(void) { return (int64_t)tq::g_launches.load(); }
 
-void tq_profile_decode_main_only(int on) { tq::g_profile_skip_prep = on < 0 ? 0 : (on > 2 ? 2 : on); }
+void tq_profile_decode_main_only(int on) { tq::g_profile_skip_prep.store(on < 0 ? 0 : (on > 2 ? 2 : on), std::memory_order_relaxed); }
 
 void tq_debug_set_quantize_impl(int fp32_cuda_cores) { tq::debug_set_quantize_fp32(fp32_cuda_cores); }
 

@@ -222,7 +222,7 @@ struct DecodeArgs {
   unsigned* frags;       // workspace [units_call][FragLayout<D>::kWords] (tq_prep.cu)
   unsigned* tabs;        // workspace [layers_call * H][kTabWords]
   float* orot;           // workspace [units_call][D]: o'/l in the rotated basis (tq_decode_model_step)
-  float* partials;       // workspace [units_call][64][D + 2]
+  float* partials;       // workspace [units_call][64][decode_record_floats(D, v_qjl)]: D + 2 floats, 2 D + 3 with the V sketch
   int* counters;         // workspace [units_call]
   int layer_begin, n_layers_call, nsplit /* CTAs per unit, >= 1 */, per /* tiles per split planned from t_hint */, rope_layout, dt;
   // 0: wait for the kernel in front of this launch before touching memory (any stream order is safe);

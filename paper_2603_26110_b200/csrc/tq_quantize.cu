@@ -1,4 +1,10 @@
-// tq_quantize.cu — KV quantize-and-pack kernels (prefill tiles and single-token append), sm_100a.
+// tq_quantize.cu — the fp32 CUDA-core quantize-and-pack kernel (prefill tiles), sm_100a.
+//
+// NOT the product kernel: tq_quantize_pack runs the tcgen05 kernel of tq_quantize_tc.cu, and the single-token append
+// lives in tq_prep.cu.  This file is the independent second implementation the tests cross-check the tensor-core
+// kernel against (test_tensor_core_quantize_agrees_with_cuda_core_kernel); it is reached only through the test knob
+// tq_debug_set_quantize_impl(1), implements the default mode only (no paper-literal mode, no V-side sketch) and is
+// never timed by bench.py.
 //
 // Per vector (PAPER.md:111-116 prefill steps 1,3,4; §3.3 Eq. 5; §3.4 Eq. 6 in the sign(S r) form of
 // BASELINE.json:north_star): RoPE (keys) -> y = PI x' -> n = |y|, u = y / n -> code_i = #{k: u_i > t_k}

@@ -588,6 +588,53 @@ def test_host_stepper_equals_model_step_host_over_several_steps(tq, oracle, n_ch
 
 
 @pytest.mark.gpu
+def test_host_stepper_very_deep_layer_run(tq, oracle):
+    """400 layers in one stepper with the maximum number of copy-in chunks (32): the copy-out groups no longer fit the
+    event budget at six layers each and grow to ceil(400 / 32) = 13 layers (tq_host_stepper_create).  Creation must
+    succeed, every replay must equal tq_decode_model_step bit for bit (outputs and cache bytes), and the launch counter
+    must advance by the graph's kernels per replay and by nothing at creation."""
+    import torch
+
+    L, B, H, d, T = 400, 1, 2, 64, 40
+    shape = tq.make_shape(L, B, H, d, T + 8)
+    params = tq.Params(tq.tq_calibrate_host(shape, 1, seed=11))
+    rng = np.random.default_rng(400)
+    kv = torch.from_numpy(rng.standard_normal((2, L, B, H, T, d)).astype(np.float16)).cuda()
+    steps = [torch.from_numpy(rng.standard_normal((3, L, B, H, d)).astype(np.float16)) for _ in range(3)]
+    caches = [tq.Cache(shape), tq.Cache(shape)]
+    for c in caches:
+        for layer in range(L):
+            tq.tq_quantize_pack(shape, params, c, layer, kv[0, layer], kv[1, layer])
+    ws = [tq.Workspace(shape, L), tq.Workspace(shape, L)]
+    q, kn, vn = (steps[0][i].clone().pin_memory() for i in range(3))
+    out = torch.empty_like(q).pin_memory()
+    st = torch.zeros(tq.tq_model_step_staging_bytes(shape, tq.TQ_F16, L) + 256, dtype=torch.uint8, device="cuda")
+    st = st[(-st.data_ptr()) % 256:]
+    torch.cuda.synchronize()
+    n0 = tq.tq_launch_count()
+    stepper = tq.HostStepper(shape, params, caches[1], 0, L, q, kn, vn, out, st, ws[1], T + 8, 32)
+    assert tq.tq_launch_count() == n0, "a capture records launches, it does not perform them"
+    per_replay = None
+    for qkv in steps:
+        qd, kd, vd = (qkv[i].cuda() for i in range(3))
+        want = torch.full_like(qd, float("nan"))
+        tq.tq_decode_model_step(shape, params, caches[0], 0, L, qd, kd, vd, want, ws[0], T + 8)
+        for dst, src in zip((q, kn, vn), qkv):
+            dst.copy_(src)
+        out.fill_(float("nan"))
+        n1 = tq.tq_launch_count()
+        stepper.run()
+        n2 = tq.tq_launch_count()
+        per_replay = n2 - n1 if per_replay is None else per_replay
+        assert n2 - n1 == per_replay and per_replay >= L + 32 + 400 // 13
+        torch.cuda.synchronize()
+        assert torch.isfinite(want.float()).all() and torch.equal(out.cuda(), want)
+    stepper.close()
+    assert torch.all(caches[1].seq_len == T + 3)
+    assert torch.equal(caches[0].data, caches[1].data)
+
+
+@pytest.mark.gpu
 def test_model_step_equals_per_layer_steps_and_replays_from_a_graph(tq, oracle):
     """tq_decode_model_step (one prep launch for all layers, then a run-ahead chain of streaming launches) must give
     bit-identical outputs and cache bytes to tq_append + tq_decode_attn called layer by layer; and a CUDA graph of it
