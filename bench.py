@@ -10,8 +10,11 @@ decode step = 33 x (append + decode) through tq_decode_model_step.
 value     : cached token-heads attended per second (L*B*H*T per step / step time), inputs resident in HBM,
             the step replayed as one CUDA graph.
 e2e       : same metric through tq_decode_model_step_host with pinned HOST q/k/v/out buffers (copies inside).
+value_sequential : the same step in the order a model must run it (tq_decode_step layer after layer); `value` is the
+            run-ahead form, an upper bound a transformer cannot call.
 roofline  : fused decode kernel, algorithmic packed bytes (62 B per cached token-head) / its average launch
-            duration measured live with CUDA events, against MEASURED_PEAKS.json hbm_gbs.
+            duration measured live with CUDA events, against MEASURED_PEAKS.json hbm_gbs; `frac` is taken on zero
+            queries (flat softmax: no value work skipped), `frac_peaked_inputs` on the configs[2] queries.
 cpu_baseline : the CPU oracle (oracle/, as it stands) timed on this box's host cores on a bounded sample.
 --config cfg1|cfg3|cfg4 : the other BASELINE.json configs (prefill quantize/pack GB/s and decode tokens/s), one line each.
 """
@@ -54,14 +57,27 @@ def measured_peaks():
     return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
+def kernel_source_sha(name: str = "tq_decode.cu") -> str:
+    """sha256 (first 12 hex digits) of a kernel source file as it is now (the GPU box has no .git to ask)."""
+    import hashlib
+
+    path = os.path.join(ROOT, "paper_2603_26110_b200", "csrc", name)
+    return hashlib.sha256(open(path, "rb").read()).hexdigest()[:12]
+
+
 def ncu_traffic(kernel_tag: str):
     """DRAM bytes per launch of the dominant kernel from the newest committed `ncu --set full` summary
-    (profiles/r*_<kernel_tag>_full.md, line `dram_bytes_per_launch: N`); None when no capture of this round exists."""
+    (profiles/r*_<kernel_tag>_full.md, line `dram_bytes_per_launch: N`); None when no capture exists.  This is a number
+    READ FROM A COMMITTED FILE, not measured by this run: the summary names the source it was captured from
+    (`kernel_source_sha256: <12 hex digits of tq_decode.cu>`), and the third element says whether that is still the
+    source this run was built from (True / False, None when the summary does not say)."""
     best = None
     for f in sorted(glob.glob(os.path.join(ROOT, "profiles", f"r*_{kernel_tag}_full.md"))):
-        m = re.search(r"dram_bytes_per_launch:\s*([0-9.eE+]+)", open(f).read())
+        text = open(f).read()
+        m = re.search(r"dram_bytes_per_launch:\s*([0-9.eE+]+)", text)
         if m:
-            best = (float(m.group(1)), os.path.relpath(f, ROOT))
+            sha = re.search(r"kernel_source_sha256:\s*([0-9a-f]{12})", text)
+            best = (float(m.group(1)), os.path.relpath(f, ROOT), (sha.group(1) == kernel_source_sha()) if sha else None)
     return best
 
 
@@ -620,18 +636,32 @@ def run_cfg2(args, w: W.Workload):
             dist.destroy_process_group()
         return
     peak, peak_src = measured_peaks()
-    achieved = dec_bytes / (chain_us * 1e-6) / 1e9
+    # roofline.frac is the DATA-INDEPENDENT figure: the chain on zero queries, where no value work can be skipped.  The
+    # figure on the configs[2] inputs (peaked softmax, value MMAs of zero-weight halves skipped) is frac_peaked_inputs.
+    achieved = dec_bytes / (chain_flat_us * 1e-6) / 1e9
+    achieved_peaked = dec_bytes / (chain_us * 1e-6) / 1e9
     value = whole_job_value(tok_heads, world, ms_max)
     traffic = None if V_QJL else ncu_traffic("decode_main")
     us_layer = 1e3 * ms_max / args.steps / L
+    # the order a model must run the layers in (layer l + 1's q/k/v come from layer l's output): tq_decode_step per layer
+    value_sequential = world * L * B * H * (T0 + 1) / (seq_us * L * 1e-6)
+    # what a competent two-pass path must move per layer: read the packed cache, write fp16 K and V, read them back
+    two_pass_bytes = dec_bytes + 2 * (2 * B * H * T0 * d * 2)
+    two_pass_bound_us = two_pass_bytes / peak / 1e3
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
         "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f32", "data": "synthetic",
+        "dtype": "f16", "data": "synthetic",
+        # `value` is the run-ahead form (tq_decode_model_step: every layer's q/k/v known before the step) — an upper bound
+        # that a transformer cannot call, because layer l + 1's inputs depend on layer l's output.  The form a model can
+        # call (tq_decode_step layer after layer, one graph) is value_sequential.
+        "value_sequential": value_sequential,
+        "value_is": "run-ahead upper bound (all layers' q/k/v before the step); value_sequential is the model-order step",
         "config": {
             "workload": f"{w.name} (BASELINE.json configs[2]) x {L} layers: batch {B} x {H} heads x d {d}, "
                         f"{T0}+ cached tokens, fp16 Student-t(4) + 2 outlier channels x15, append + decode per layer per step",
             "layers": L, "batch_per_gpu": B, "heads": H, "head_dim": d, "cached_tokens": T0, "io_dtype": "f16",
+            "arithmetic": "fp16 inputs / outputs and MMA operands (two-term split), fp32 accumulation and softmax",
             "l2": f"inputs larger than L2: {L} layer caches x {B*H*T0*rig.bpt/1e6:.1f} MB are cycled every step",
             "cuda_graph": True, "bytes_per_token_head": rig.bpt, "v_qjl": V_QJL,
             "step_form": "tq_decode_model_step: one append+query-prep launch for all layers, one streaming launch per "
@@ -640,12 +670,17 @@ def run_cfg2(args, w: W.Workload):
             "packed_gbs_whole_step": value / world * rig.bpt / 1e9,
             "ms_per_step_stepper_device_buffers": stepper_ms, "value_stepper_device_buffers": stepper_value,
             "us_per_layer_step_sequential": seq_us,
-            "value_sequential": L * B * H * (T0 + 1) / (seq_us * L * 1e-6),
+            "value_sequential": value_sequential,
             "decode_call_us_live": call_us, "decode_call_packed_gbs": dec_bytes / call_us / 1e3,
             "two_step_torch_baseline": None if two_step is None else {
                 "what": "PAPER.md:221 / Table 6 comparison restated: PyTorch GPU ops dequantise one layer cache to fp16 K, V "
                         "in HBM, then torch SDPA (not the product; context, like the paper's 1.96x on its own hardware)",
-                "us_per_layer_call": two_step[0], "fused_call_us": call_us, "fused_speedup": two_step[0] / call_us,
+                "us_per_layer_call": two_step[0], "fused_call_us": call_us,
+                "eager_torch_over_fused": two_step[0] / call_us,
+                "note": "eager PyTorch with fp32 gathers: an untuned path, not a yardstick; the ratio that means something is "
+                        "against the traffic a two-pass path cannot avoid",
+                "two_pass_traffic_bound_us": two_pass_bound_us, "two_pass_bytes_per_layer": two_pass_bytes,
+                "two_pass_bound_over_fused_call": two_pass_bound_us / call_us,
                 "cosine_vs_fused_output": two_step[1]},
             "decode_main_kernel_us_live": chain_us, "decode_main_kernel_plus_finish_us_live": chain_finish_us,
             "decode_main_kernel_us_isolated_launch": iso_us,
@@ -662,19 +697,28 @@ def run_cfg2(args, w: W.Workload):
         "gpu_launches": int(launches_per_step * args.steps),
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "traffic": traffic[0] if traffic else None, "kernel": "decode_main_kernel<64, __half, false, %s>" % ("true" if V_QJL else "false"),
-                     "traffic_source": (f"dram__bytes_read.sum + dram__bytes_write.sum per launch, {traffic[1]}" if traffic
+                     "traffic_source": (f"READ FROM A COMMITTED FILE, not measured by this run: dram__bytes_read.sum + "
+                                        f"dram__bytes_write.sum per launch, {traffic[1]}" if traffic
                                         else "no ncu capture of the current kernel is committed"),
+                     "traffic_capture_matches_this_source": traffic[2] if traffic else None,
                      "peak_source": peak_src, "bytes_per_launch": dec_bytes,
                      "how": f"{L} launches (one per layer cache) as the model step chains them (prep and finish kernels left out "
-                            f"through the library's measurement hook), CUDA events around the graph, / {L}",
-                     "frac_with_finish_kernel": dec_bytes / chain_finish_us / 1e3 / peak,
-                     "frac_flat_softmax": dec_bytes / chain_flat_us / 1e3 / peak,
-                     "flat_softmax": "same chain with zero queries (uniform weights: no value work is skipped); the headline "
-                                     "inputs have a peaked softmax and the kernel skips value MMAs of halves whose weights are 0",
+                            f"through the library's measurement hook), zero queries = flat softmax so that no value work is "
+                            f"skipped, CUDA events around the graph, / {L}",
+                     "frac_flat_softmax": achieved / peak,
+                     "frac_peaked_inputs": achieved_peaked / peak,
+                     "peaked_inputs": "the same chain on the configs[2] queries: the softmax is peaked and the kernel skips the "
+                                      "value MMAs of 16-token halves whose weights underflow to 0 (data-dependent, so not the headline)",
+                     "frac_with_finish_kernel_peaked_inputs": dec_bytes / chain_finish_us / 1e3 / peak,
                      "frac_isolated_launch": dec_bytes / iso_us / 1e3 / peak,
                      "frac_call": dec_bytes / call_us / 1e3 / peak,
-                     "frac_step": value / world * rig.bpt / 1e9 / peak},
+                     "frac_step": value / world * rig.bpt / 1e9 / peak,
+                     "frac_sequential_step": value_sequential / world * rig.bpt / 1e9 / peak,
+                     "sequential_step": "tq_decode_step layer after layer in one graph (append + query prep launch, then the "
+                                        "streaming launch, each layer behind the one before): the order a model runs"},
     }
+    if world == 1 and not args.no_aux:
+        line["config"]["aux"] = aux_legs(args)
     if world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(w)
     print(json.dumps(line))
@@ -682,13 +726,18 @@ def run_cfg2(args, w: W.Workload):
         dist.destroy_process_group()
 
 
-def run_aux(args, w: W.Workload, key: str):
-    """configs[1], [3], [4]: a full prefill tq_quantize_pack of every layer cache (GB/s on input + packed bytes), then the
-    fused decode over the cache(s); one JSON line."""
+def run_aux(args, w: W.Workload, key: str, nested: bool = False):
+    """configs[1], [3], [4] (and configs[2] with the V-side sketch): a full prefill tq_quantize_pack of every layer cache
+    (GB/s on input + packed bytes), then the fused decode over the cache(s); one JSON line.  nested = True: called from
+    the default run on one GPU, which folds the returned line into its own `config.aux` (no print, no clock sampler of
+    its own, no process-group work)."""
     import torch
     import torch.distributed as dist
 
-    rank, world, local = init_dist()
+    if nested:
+        rank, world, local = 0, 1, int(os.environ.get("LOCAL_RANK", "0"))
+    else:
+        rank, world, local = init_dist()
     from paper_2603_26110_b200 import binding as tq
 
     bpt = bytes_per_token_head(w.head_dim) + (0 if not V_QJL else (10 if w.head_dim == 64 else 18))
@@ -715,7 +764,7 @@ def run_aux(args, w: W.Workload, key: str):
         tq.tq_decode_attn(shape, params, cache, 0, L, qs, outs, wsL, None, T0, stream)
 
     sampler = ClockSampler(local)
-    if rank == 0:
+    if rank == 0 and not nested:
         sampler.start()
     reps = max(6, min(args.steps, 30))
     call_us = rig.graph_us(per_layer, L, reps=reps)
@@ -738,7 +787,7 @@ def run_aux(args, w: W.Workload, key: str):
             main_batched_us = rig.graph_us(batched, 1, reps=reps)
         finally:
             tq.tq_profile_decode_main_only(False)
-    clocks = sampler.stop() if rank == 0 else None
+    clocks = sampler.stop() if rank == 0 and not nested else None
     step_us = (batched_us if batched_us is not None else call_us) * L
     (ms_max,) = max_over_ranks([step_us * 1e-3], world, dev)
     if rank != 0:
@@ -751,7 +800,7 @@ def run_aux(args, w: W.Workload, key: str):
     traffic = ncu_traffic(f"decode_main_{key}")
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": reps - 1, "warmup": 3,
-        "ms_per_step": ms_max, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "ms_per_step": ms_max, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f16", "data": "synthetic",
         "config": {
             "workload": f"{w.name} (BASELINE.json configs[{w.index}]): {L} layer cache(s) x batch {B} x {H} heads x d {d}, "
                         f"{T0} cached tokens, {w.dtype} {w.dist}; full prefill tq_quantize_pack, then fused decode over every cache",
@@ -779,9 +828,42 @@ def run_aux(args, w: W.Workload, key: str):
                       "us_per_launch": main_batched_us, "frac_call": L * dec_bytes / (batched_us * L) / 1e3 / peak,
                       "frac_one_layer_per_launch": dec_bytes / main_us / 1e3 / peak}),
     }
+    if nested:
+        return line
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
+
+
+def aux_legs(args):
+    """The other BASELINE.json configs in the line the driver runs (config.aux): configs[1], [3], [4] and configs[2] with
+    the V-side sketch, each the few-second leg `--config cfgN` (`--v-qjl`) runs on its own, boiled down to its numbers."""
+    import gc
+
+    import torch
+
+    global V_QJL
+    out = {}
+    for name, key, vq in (("cfg1", "cfg1", 0), ("cfg3", "cfg3", 0), ("cfg4", "cfg4", 0), ("cfg2_v_qjl", "cfg2", 1)):
+        keep, V_QJL = V_QJL, vq
+        try:
+            line = run_aux(args, W.CONFIGS[CONFIG_NAMES[key]], key, nested=True)
+        finally:
+            V_QJL = keep
+        c, r = line["config"], line["roofline"]
+        out[name] = {
+            "workload": c["workload"], "layers": c["layers"], "bytes_per_token_head": c["bytes_per_token_head"],
+            "value": line["value"], "unit": UNIT, "step": c["step"], "us_per_step": line["ms_per_step"] * 1e3,
+            "decode_call_us_per_layer": c["decode_call_us_per_layer"], "decode_main_kernel_us_live": c["decode_main_kernel_us_live"],
+            "roofline": {k: r.get(k) for k in ("bound", "achieved", "peak", "unit", "frac", "frac_call", "bytes_per_launch",
+                                               "us_per_launch", "frac_one_layer_per_launch", "how") if k in r},
+            "inputs": "the workload's own queries (softmax as the inputs make it; no flat-softmax leg here)",
+            "quantize_pack_gbs": c["quantize_pack_gbs"], "quantize_pack_ms_per_layer": c["quantize_pack_ms_per_layer"],
+            "quantize_pack_frac_of_hbm": c["quantize_pack_frac_of_hbm"],
+        }
+        gc.collect()
+        torch.cuda.empty_cache()
+    return out
 
 
 def main():
@@ -794,6 +876,7 @@ def main():
     ap.add_argument("--layers", type=int, default=33, help="ESM-2-650M has 33 layers (cfg2)")
     ap.add_argument("--layers-aux", type=int, default=0, help="layer caches cycled by cfg3 / cfg4 (0 = enough to exceed L2)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-aux", action="store_true", help="skip the configs[1] / [3] / [4] / v_qjl legs of the default line (config.aux)")
     ap.add_argument("--no-two-step", action="store_true", help="skip the PyTorch two-step GPU baseline (NEXT-4)")
     ap.add_argument("--v-qjl", action="store_true", help="measure with the V-side residual sketch on (tq_shape.v_qjl = 1)")
     ap.add_argument("--e2e-chunks", type=int, default=0, help="layer chunks of the host stepper (0 = the library's choice)")
