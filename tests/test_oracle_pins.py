@@ -409,3 +409,98 @@ def test_key_sketch_values_are_S_times_the_residual(oracle):
         assert np.allclose(sr, S.astype(np.float64) @ r, rtol=0, atol=1e-12)
         assert np.array_equal((sr >= 0).astype(np.uint8), qv["bits"])
         assert abs(np.linalg.norm(r) - oracle.f16_bits_to_f64(qv["rnorm_h"])) <= 2.0 ** -11 * np.linalg.norm(r) + 1e-12
+
+
+# ---------------------------------------------------------------------------- the tolerance band (near_k / near_v)
+def _planted_unit_vector(rng, th, plan, d):
+    """fp64 unit vector whose coordinate i equals th[q] + delta for (i, q, delta) in plan; the other coordinates are random
+    and scaled so that the norm is exactly 1."""
+    u = np.zeros(d)
+    for i, q, delta in plan:
+        u[i] = float(th[q]) + delta
+    free = np.array([i for i in range(d) if i not in {p[0] for p in plan}])
+    r = rng.standard_normal(free.size)
+    u[free] = r * math.sqrt((1.0 - (u ** 2).sum()) / (r ** 2).sum())
+    assert abs(np.linalg.norm(u) - 1.0) < 1e-14
+    return u
+
+
+def test_tolerance_band_marks_exactly_the_coordinates_within_eps_of_a_threshold(oracle):
+    """north_star: codes are bit-exact "except coordinates within 1e-5 of a decision boundary".  near_k / near_v of
+    tqo_quantize_pack decide which mismatches the GPU tests forgive, so the band itself is pinned here: unit coordinates
+    are PLANTED at threshold +- 0.5e-5 (must be marked) and threshold +- 2e-5 (must not be), per head with that head's own
+    LUT, behind a permutation PI for the values (the mask is indexed by the ROTATED coordinate).  A band ten times too
+    wide, a band taken on the un-normalised vector, the other head's LUT or an un-permuted index each fail."""
+    d, H = 64, 2
+    eps = 1e-5
+    lut0 = oracle.lloyd_max_gauss(1.0 / math.sqrt(d), 8)[0].astype(np.float32)
+    luts = np.stack([lut0, (lut0 * np.float32(0.8)).astype(np.float32)])
+    th = np.stack([(np.float32(0.5) * (l[:-1] + l[1:])).astype(np.float32) for l in luts])  # [H, 7] fp32, as the method rounds them
+    plan = [(0, 1, +0.5e-5), (1, 4, -0.5e-5), (2, 5, +2e-5), (3, 2, -2e-5), (4, 3, +0.9e-5), (5, 0, -1.1e-5)]
+    marked, unmarked = [0, 1, 4], [2, 3, 5]
+    rng = np.random.default_rng(2603)
+    perm = rng.permutation(d)
+    inv = np.argsort(perm)
+    P = np.zeros((d, d), np.float32)
+    P[np.arange(d), perm] = 1.0  # y[i] = x[perm[i]]
+    eye = np.eye(d, dtype=np.float32)
+    k = np.zeros((1, H, 1, d), np.float32)
+    v = np.zeros((1, H, 1, d), np.float32)
+    for h in range(H):
+        uk = _planted_unit_vector(rng, th[h], plan, d)
+        uv = _planted_unit_vector(rng, th[h], plan, d)
+        k[0, h, 0] = (uk * 3.7).astype(np.float32)        # position 0: RoPE is the identity, PI_K = I
+        v[0, h, 0] = (uv * 0.41).astype(np.float32)[inv]  # PI_V = P brings coordinate i of uv back to slot i
+    S = rng.standard_normal((d, d)).astype(np.float32)
+    can = oracle.quantize_pack(k, v, np.stack([eye, eye]), np.stack([P, P]), luts, luts, S, near_eps=eps)
+    for h in range(H):
+        for name, near, x in (("k", can.near_k, k[0, h, 0].astype(np.float64)), ("v", can.near_v, v[0, h, 0].astype(np.float64)[perm])):
+            got = near[0, h, 0].astype(bool)
+            assert all(got[i] for i in marked), (name, h, got[:6])
+            assert not any(got[i] for i in unmarked), (name, h, got[:6])
+            # ... and nothing else: the definition written out in numpy on the same fp32 inputs
+            u = x / np.linalg.norm(x)
+            want = (np.abs(u[:, None] - th[h].astype(np.float64)[None, :]) < eps).any(axis=1)
+            assert np.array_equal(got, want), (name, h)
+            assert got.sum() == len(marked)
+    # the other head's thresholds would not do: head 1's coordinates planted on non-zero thresholds are far from head 0's
+    u1 = k[0, 1, 0].astype(np.float64) / np.linalg.norm(k[0, 1, 0].astype(np.float64))
+    assert not (np.abs(u1[[0, 1], None] - th[0].astype(np.float64)[None, :]) < 10 * eps).any()
+
+
+def test_tolerance_band_of_the_paper_literal_mode_scales_with_the_vector_norm(oracle):
+    """DESIGN.md section 2, reading D17: in the paper-literal mode the coded coordinates are not normalised, so the band is
+    near_eps x max(1, |y|).  Planted on y itself: |y| = 5 -> band 5e-5 (a coordinate 2.5e-5 from a threshold is marked,
+    one 1e-4 away is not); |y| = 0.5 -> band stays 1e-5 (0.7e-5 marked, 2e-5 not)."""
+    d, H = 64, 1
+    eps = 1e-5
+    lut = (oracle.lloyd_max_gauss(1.0 / math.sqrt(d), 8)[0] * 4.0).astype(np.float32)[None]
+    th = (np.float32(0.5) * (lut[0, :-1] + lut[0, 1:])).astype(np.float32)
+    rng = np.random.default_rng(7)
+    eye = np.eye(d, dtype=np.float32)[None]
+
+    def planted(norm, plan):
+        y = np.zeros(d)
+        for i, q, delta in plan:
+            y[i] = float(th[q]) + delta
+        free = np.arange(len(plan), d)
+        r = rng.standard_normal(free.size)
+        y[free] = r * math.sqrt((norm ** 2 - (y ** 2).sum()) / (r ** 2).sum())
+        return y.astype(np.float32)
+
+    big = planted(5.0, [(0, 1, +2.5e-5), (1, 5, -2.5e-5), (2, 3, +1e-4), (3, 2, -1e-4)])
+    small = planted(0.5, [(0, 3, +0.7e-5), (1, 4, -0.7e-5), (2, 2, +2e-5), (3, 3, -2e-5)])
+    k = np.stack([big, small])[None, None]  # [1, 1, 2, d]: two tokens ... position 1 would rotate the second: use v
+    can = oracle.quantize_pack_literal(np.zeros_like(k), k, eye, eye, lut, lut, np.eye(d, dtype=np.float32),
+                                       np.array([0.01], np.float32), near_eps=eps)
+    for t, x in enumerate((big, small)):
+        got = can.near_v[0, 0, t].astype(bool)
+        assert got[0] and got[1] and not got[2] and not got[3], (t, got[:4])
+        y = x.astype(np.float64)
+        band = eps * max(1.0, float(np.linalg.norm(y)))
+        want = (np.abs(y[:, None] - th.astype(np.float64)[None, :]) < band).any(axis=1)
+        assert np.array_equal(got, want) and got.sum() == 2
+    # keys at position 0 (RoPE = identity) take the same band
+    can_k = oracle.quantize_pack_literal(big[None, None, None], np.zeros((1, 1, 1, d), np.float32), eye, eye, lut, lut,
+                                         np.eye(d, dtype=np.float32), np.array([0.01], np.float32), near_eps=eps)
+    assert np.array_equal(can_k.near_k[0, 0, 0], can.near_v[0, 0, 0])
