@@ -14,6 +14,23 @@ NEAR_EPS = 1e-5
 MAX_MISMATCH_FRAC = 1e-4
 OUT_MAX_ABS = 2e-3
 OUT_MIN_COS = 0.9999
+# Stored binary16 norms ("norm rule"): north_star states no norm tolerance.  A kernel that computes
+# the norm in fp32 (relative error e <= about 5e-7: two-term fp16 products, fp32 accumulation of d terms, fp32 sqrt) rounds
+# to a different binary16 than the fp64 oracle only when the exact value lies within e n of a rounding tie; ties are
+# 2^-11 .. 2^-10 apart relative to n, so that happens to at most about 2 e 2^11 = 2e-3 of the entries and never by more
+# than one ulp.  One entry is always allowed (small cases hold a few hundred norms).  Two fp32 kernels compared with
+# each other (the tensor-core and the CUDA-core quantize kernels) each carry their own e: twice the rate.
+NORM_MAX_ULP = 1
+NORM_ULP_RATE = 2e-3
+
+
+def assert_norm_ulps(a, b, what="", fp32_sides: int = 1):
+    """a, b: binary16 bit patterns (any integer dtype / view) of the same norms from two implementations."""
+    dd = np.abs(np.asarray(a).astype(np.int32) - np.asarray(b).astype(np.int32))
+    rate = float((dd > 0).mean()) if dd.size else 0.0
+    assert dd.max(initial=0) <= NORM_MAX_ULP, (what, int(dd.max(initial=0)))
+    assert rate <= fp32_sides * NORM_ULP_RATE + 1.0 / max(1, dd.size), (what, rate)
+    return rate
 
 
 def make_arrays(oracle, w: W.Workload, rope_cs, lut_scale_v: float = 1.0, per_head_lut: bool = False):
@@ -68,14 +85,9 @@ def compare_quantize(can_oracle, gpu: dict, d: int, what: str = ""):
     for name, mask in (("k_norm", None), ("k_rnorm", ok), ("v_norm", None)):
         a = getattr(can_oracle, name).astype(np.int32)
         b = gpu[name].view(np.uint16).astype(np.int32)
-        dd = np.abs(a - b)
-        if mask is not None:
-            dd = dd[mask]
-        assert dd.max(initial=0) <= 1, (what, name, dd.max())
-        rep[f"{name}_ulp_mismatch_frac"] = float((dd > 0).mean()) if dd.size else 0.0
-        # ... which happens to a fraction ~ (relative error of the fp32 norm) / (binary16 spacing 2^-11) of the entries;
-        # a single such entry is always allowed (small cases have only a few hundred norms)
-        assert rep[f"{name}_ulp_mismatch_frac"] <= max(2e-3, 1.0 / max(1, dd.size)), (what, name, rep[f"{name}_ulp_mismatch_frac"])
+        if mask is not None:  # |r| is only comparable where the codes agree
+            a, b = a[mask], b[mask]
+        rep[f"{name}_ulp_mismatch_frac"] = assert_norm_ulps(a, b, f"{what} {name}")
     del rep["k_vec_equal"], rep["v_vec_equal"]
     return rep
 
