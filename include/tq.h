@@ -308,10 +308,16 @@ int tq_decode_model_step(const tq_shape *shape, const tq_params *dev, tq_cache *
 const char *tq_status_string(int status);
 /* Number of kernels the library launched since load (bench.py's gpu_launches).                          */
 int64_t tq_launch_count(void);
+/* ---- measurement and test hooks: compiled ONLY with -DTQ_TEST_HOOKS ------------------------------------------------
+ * The three functions below, and the fp32 CUDA-core cross-check kernel behind the last of them, exist only in a library
+ * built with -DTQ_TEST_HOOKS.  That is the build the tests, bench.py and __graft_entry__ use
+ * (`python -m paper_2603_26110_b200.build`, the default).  `python -m paper_2603_26110_b200.build --product` leaves them
+ * out: that library exports none of the three symbols and its product path reads no process-wide switch.            */
+#ifdef TQ_TEST_HOOKS
 /* Measurement hook, NOT part of the product path (bench.py's roofline leg and one test use it): while on,
  * tq_decode_attn / tq_decode_model_step skip the append + query-prep kernel and re-use the query operands their
  * previous ordinary call left in the workspace (same queries, same layers), so that a run of such calls times
- * the streaming kernel alone.  Process-wide, not thread-safe; results are only meaningful directly after an
+ * the streaming kernel alone.  Process-wide (an atomic flag); results are only meaningful directly after an
  * ordinary call with the same arguments; always switch it off again.  on = 2: tq_decode_model_step also leaves out its
  * finish kernel (the streaming launches alone; the outputs are then not written).                          */
 void tq_profile_decode_main_only(int on);
@@ -321,6 +327,7 @@ void tq_profile_decode_main_only(int on);
  * tensor-core kernel runs.                                                                                            */
 void tq_debug_set_decode_nsplit(int nsplit);
 void tq_debug_set_quantize_impl(int fp32_cuda_cores);
+#endif /* TQ_TEST_HOOKS */
 
 #ifdef __cplusplus
 }

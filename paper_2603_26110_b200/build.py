@@ -21,16 +21,21 @@ def _stale() -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and not _stale():
-        return LIB
+def build(force: bool = False, verbose: bool = False, test_hooks: bool = True) -> str:
+    """test_hooks = True (what the tests, bench.py and __graft_entry__ build): libtq.so with -DTQ_TEST_HOOKS, i.e. with
+    tq_profile_decode_main_only, tq_debug_set_decode_nsplit, tq_debug_set_quantize_impl and the fp32 cross-check kernel.
+    test_hooks = False (`python -m paper_2603_26110_b200.build --product`): build/libtq_product.so without them — no
+    measurement or test switch, no process-wide mutable state on the product path."""
+    lib = LIB if test_hooks else os.path.join(HERE, "build", "libtq_product.so")
+    if test_hooks and not force and not _stale():
+        return lib
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    extra = os.environ.get("TQ_NVCC_EXTRA", "").split()  # experiments only, e.g. -DTQ_DECODE_THREADS=192
+    extra = ["-DTQ_TEST_HOOKS"] if test_hooks else []
     objs = []
     procs = []
     os.makedirs(os.path.join(HERE, "build"), exist_ok=True)
     for src in SOURCES:
-        obj = os.path.join(HERE, "build", src + ".o")
+        obj = os.path.join(HERE, "build", src + (".o" if test_hooks else ".product.o"))
         cmd = [nvcc, *NVCC_FLAGS, *extra, "-c", os.path.join(CSRC, src), "-o", obj]
         if verbose:
             cmd.insert(1, "-Xptxas=-v")
@@ -42,9 +47,9 @@ def build(force: bool = False, verbose: bool = False) -> str:
             sys.stderr.write(out)
         if p.returncode != 0:
             raise RuntimeError(f"nvcc failed on {src}")
-    subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", LIB, *objs, "-lcudart"], check=True)
-    return LIB
+    subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", lib, *objs, "-lcudart"], check=True)
+    return lib
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv, test_hooks="--product" not in sys.argv))

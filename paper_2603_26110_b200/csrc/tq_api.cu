@@ -9,7 +9,17 @@
 namespace tq {
 
 static std::atomic<long long> g_launches{0};
+// Measurement / test hooks exist only in builds with -DTQ_TEST_HOOKS (what the tests and bench.py build; include/tq.h).
+// Without it the three values below are compile-time zeros and the product path carries no mutable process-wide state.
+#ifdef TQ_TEST_HOOKS
 static std::atomic<int> g_profile_skip_prep{0};  // tq_profile_decode_main_only (a setter may run on another thread)
+static std::atomic<int> g_debug_nsplit{0};       // tq_debug_set_decode_nsplit
+static int profile_skip_prep() { return g_profile_skip_prep.load(std::memory_order_relaxed); }
+static int debug_nsplit() { return g_debug_nsplit.load(std::memory_order_relaxed); }
+#else
+static constexpr int profile_skip_prep() { return 0; }
+static constexpr int debug_nsplit() { return 0; }
+#endif
 // Launches recorded into a stream capture are not launches yet: while the stepper captures (thread-local capture mode,
 // so every recorded launch comes from this thread) they are counted apart and added at every replay.
 static thread_local bool t_capturing = false;
@@ -45,9 +55,8 @@ static int choose_nsplit(int units, int ntiles, int sms) {
 }
 
 // split factor of a launch: the plan above, or the value set with tq_debug_set_decode_nsplit (tests, sweeps)
-static std::atomic<int> g_debug_nsplit{0};
 static int pick_nsplit(int units, int ntiles, int sms) {
-  const int forced = g_debug_nsplit.load(std::memory_order_relaxed);
+  const int forced = debug_nsplit();
   return forced >= 1 && forced <= kMaxSplits ? forced : choose_nsplit(units, ntiles, sms);
 }
 
@@ -189,7 +198,7 @@ int tq_quantize_pack(const tq_shape* shape, const tq_params* dev, tq_cache* cach
   return launch_quantize_pack(a, g.D, dt, sms, (cudaStream_t)cuda_stream) == cudaSuccess ? TQ_OK : TQ_ERR_CUDA;
 }
 
-// Shared body of tq_append / tq_decode_attn / tq_decode_step: validation, then per launch chunk
+// Shared body of tq_append / tq_decode_attn / tq_decode_step: validation, then
 // [prep kernel (append and/or query prep)] + [streaming decode kernel].
 static int run_decode(const tq_shape* shape, const tq_params* dev, const tq_cache* cache, int32_t layer_begin,
                       int32_t n_layers_call, const void* q, const void* k, const void* v, const int32_t* q_pos,
@@ -214,44 +223,37 @@ static int run_decode(const tq_shape* shape, const tq_params* dev, const tq_cach
   const int th = (t_hint == 0 || t_hint > g.max_seq) ? g.max_seq : t_hint;
   const int ntiles = (th + kTile - 1) / kTile;
   const int nsplit = pick_nsplit(n_layers_call * g.B * g.H, ntiles, sms);
-  const size_t esz = dt == TQ_F16 ? 2 : 4;
   unsigned char* ws = (unsigned char*)workspace;
-  const int layers_per_launch = n_layers_call;
-  for (int l0 = 0; l0 < n_layers_call; l0 += layers_per_launch) {
-    const int nl = n_layers_call - l0 < layers_per_launch ? n_layers_call - l0 : layers_per_launch;
-    const size_t u0 = (size_t)l0 * g.B * g.H;  // first unit of this launch inside the call
-    DecodeArgs a;
-    a.cv = make_view(g, cache->data);
-    a.pi_k = dev->pi_k;
-    a.pi_v = dev->pi_v;
-    a.lut_k = dev->lut_k;
-    a.lut_v = dev->lut_v;
-    a.S = dev->S;
-    a.rope_cs = dev->rope_cs;
-    a.q = q ? (const unsigned char*)q + u0 * g.D * esz : nullptr;
-    a.out = out ? (unsigned char*)out + u0 * g.D * esz : nullptr;
-    a.q_pos = q_pos ? q_pos + (size_t)l0 * g.B : nullptr;
-    a.counters = ws ? (int*)(ws + w.off_counters) + u0 : nullptr;
-    a.frags = ws ? (unsigned*)(ws + w.off_frags) + u0 * w.frag_words : nullptr;
-    a.tabs = ws ? (unsigned*)(ws + w.off_tabs) + (size_t)l0 * g.H * kTabWords : nullptr;
-    a.orot = nullptr;
-    a.partials = ws ? (float*)(ws + w.off_partials) + u0 * kMaxSplits * w.rec : nullptr;
-    a.layer_begin = layer_begin + l0;
-    a.n_layers_call = nl;
-    a.nsplit = nsplit;
-    a.per = (ntiles + nsplit - 1) / nsplit;
-    a.chain_mode = 0;
-    a.rope_layout = shape->rope_layout;
-    a.dt = (int)dt;
-    a.literal = shape->residual_mode == 1;
-    a.ebar_k = a.literal ? dev->ebar_k : nullptr;
-    const void* kc = k ? (const unsigned char*)k + u0 * g.D * esz : nullptr;
-    const void* vc = v ? (const unsigned char*)v + u0 * g.D * esz : nullptr;
-    if (!(g_profile_skip_prep.load(std::memory_order_relaxed) && do_query && !do_append) &&
-        launch_prep(a, kc, vc, g.D, sms, do_append, do_query, (cudaStream_t)cuda_stream) != cudaSuccess)
-      return TQ_ERR_CUDA;
-    if (do_query && launch_decode(a, g.D, true, (cudaStream_t)cuda_stream) != cudaSuccess) return TQ_ERR_CUDA;
-  }
+  DecodeArgs a;
+  a.cv = make_view(g, cache->data);
+  a.pi_k = dev->pi_k;
+  a.pi_v = dev->pi_v;
+  a.lut_k = dev->lut_k;
+  a.lut_v = dev->lut_v;
+  a.S = dev->S;
+  a.rope_cs = dev->rope_cs;
+  a.q = q;
+  a.out = out;
+  a.q_pos = q_pos;
+  a.counters = ws ? (int*)(ws + w.off_counters) : nullptr;
+  a.frags = ws ? (unsigned*)(ws + w.off_frags) : nullptr;
+  a.tabs = ws ? (unsigned*)(ws + w.off_tabs) : nullptr;
+  a.orot = nullptr;
+  a.partials = ws ? (float*)(ws + w.off_partials) : nullptr;
+  a.layer_begin = layer_begin;
+  a.n_layers_call = n_layers_call;
+  a.nsplit = nsplit;
+  a.per = (ntiles + nsplit - 1) / nsplit;
+  a.chain_mode = 0;
+  a.rope_layout = shape->rope_layout;
+  a.dt = (int)dt;
+  a.literal = shape->residual_mode == 1;
+  a.ebar_k = a.literal ? dev->ebar_k : nullptr;
+  // one prep launch (append and / or query operands of every layer of the call), then one streaming launch over all units
+  if (!(profile_skip_prep() && do_query && !do_append) &&
+      launch_prep(a, k, v, g.D, sms, do_append, do_query, (cudaStream_t)cuda_stream) != cudaSuccess)
+    return TQ_ERR_CUDA;
+  if (do_query && launch_decode(a, g.D, true, (cudaStream_t)cuda_stream) != cudaSuccess) return TQ_ERR_CUDA;
   return TQ_OK;
 }
 
@@ -438,7 +440,7 @@ int tq_decode_model_step(const tq_shape* shape, const tq_params* dev, tq_cache* 
   // one prep launch for every layer of the step (append + query operands), then one streaming launch per layer cache:
   // the first waits for the prep kernel, the others run ahead of one another (DecodeArgs::chain_mode); they leave o'/l
   // in the workspace and one last launch applies PI_V^T to every unit of the step
-  const int hook = g_profile_skip_prep.load(std::memory_order_relaxed);  // measurement hook, 0 on the product path
+  const int hook = profile_skip_prep();  // measurement hook, always 0 without TQ_TEST_HOOKS
   if (!hook && launch_prep(p.a, p.k, p.v, p.g.D, p.sms, true, true, st) != cudaSuccess) return TQ_ERR_CUDA;
   for (int l = 0; l < n_layers_call; ++l) {
     DecodeArgs b = sub_args(p, l, 1);
@@ -719,10 +721,12 @@ const char* tq_status_string(int status) {
 
 int64_t tq_launch_count(void) { return (int64_t)tq::g_launches.load(); }
 
+#ifdef TQ_TEST_HOOKS
 void tq_profile_decode_main_only(int on) { tq::g_profile_skip_prep.store(on < 0 ? 0 : (on > 2 ? 2 : on), std::memory_order_relaxed); }
 
 void tq_debug_set_quantize_impl(int fp32_cuda_cores) { tq::debug_set_quantize_fp32(fp32_cuda_cores); }
 
 void tq_debug_set_decode_nsplit(int nsplit) { tq::g_debug_nsplit.store(nsplit, std::memory_order_relaxed); }
+#endif
 
 }  // extern "C"

@@ -34,15 +34,10 @@
 namespace tq {
 
 constexpr int kMaxSegments = 64;      // split-K partial slots per unit (tq_api.cu sizes the workspace)
-#ifndef TQ_DECODE_CTAS64
-#define TQ_DECODE_CTAS64 5
-#endif
-#ifndef TQ_DECODE_STAGES
-#define TQ_DECODE_STAGES 2  // measured at configs[2] x 33 layers: 2 slots 11.4 us per layer, 3 slots 11.5, 4 slots 13.2
-#endif
+constexpr int kDecodeCtasPerSm64 = 5;  // d = 64 without the V sketch: 96 registers, 36 KB shared memory
 constexpr int kDecodeThreads = 128;   // warps of one CTA share the dequantisation tables of one head
 constexpr int kDecodeWarps = kDecodeThreads / 32;
-constexpr int kStages = TQ_DECODE_STAGES;  // tile slots per warp
+constexpr int kStages = 2;  // tile slots per warp (measured at configs[2] x 33 layers: 2 slots 11.4 us per layer, 3 slots 11.5, 4 slots 13.2)
 
 // Shared-memory map in ABSOLUTE shared-window addresses: the table and ring bases are immediates of the ld.shared
 // instructions, so a lookup address is one LOP3 ((field & mask) | lane * 4).  Dynamic shared memory starts right after
@@ -68,7 +63,7 @@ struct DecodeCfg {
   // binary16-representable (64-bit reads are served one half-warp at a time, so 16 columns are conflict free)
   static constexpr int kTabBytes = 64 * 32 * 4;
   static constexpr int kSmemBytes = kAbsTab + 2 * kTabBytes;  // requested dynamic bytes (window start <= 1 KB)
-  static constexpr int kCtasPerSm = D == 64 ? (kVq ? 4 : TQ_DECODE_CTAS64) : 2;
+  static constexpr int kCtasPerSm = D == 64 ? (kVq ? 4 : kDecodeCtasPerSm64) : 2;
 };
 
 // ---- small PTX helpers --------------------------------------------------------------------------------------------

@@ -22,6 +22,7 @@
 
 namespace tq {
 
+#ifdef TQ_TEST_HOOKS  // the cross-check kernel and its switch exist only in builds for the tests (include/tq.h)
 static std::atomic<int> g_debug_quantize_fp32{0};
 void debug_set_quantize_fp32(int on) { g_debug_quantize_fp32.store(on, std::memory_order_relaxed); }
 
@@ -273,12 +274,15 @@ __global__ void __launch_bounds__(2 * D) quantize_pack_kernel(QuantArgs a) {
   }
 }
 
+#endif  // TQ_TEST_HOOKS
+
 __global__ void set_seq_len_kernel(CacheView cv, int layer, int value) {
   int b = blockIdx.x * blockDim.x + threadIdx.x;
   if (b < cv.B) cv.seq_len[layer * cv.B + b] = value;
 }
 
 // ---- launchers --------------------------------------------------------------------------------------------
+#ifdef TQ_TEST_HOOKS
 template <int D>
 static size_t quant_smem_bytes() {
   return (size_t)(3 * D * D + D * kTile) * 4 + 3 * kTile * D + 16 * 4 + 3 * kTile * 2;
@@ -302,21 +306,23 @@ static cudaError_t launch_quant_t(const QuantArgs& a, int num_sms, cudaStream_t 
   return cudaGetLastError();
 }
 
+#endif  // TQ_TEST_HOOKS
+
 cudaError_t launch_quantize_pack(const QuantArgs& a, int D, tq_dtype dt, int num_sms, cudaStream_t st) {
   if (a.n_tokens == 0) {
     set_seq_len_kernel<<<(a.cv.B + 127) / 128, 128, 0, st>>>(a.cv, a.layer, a.start_pos);
     count_launch();
     return cudaGetLastError();
   }
-  // the tensor-core kernel (tq_quantize_tc.cu) is the product path; tq_debug_set_quantize_impl(1) selects the CUDA-core
-  // kernel of this file (kept as a cross-check)
-  // (the cross-check kernel only knows the default residual mode)
-  const bool force_fp32 = g_debug_quantize_fp32.load(std::memory_order_relaxed) != 0 && !a.literal && !a.cv.vsk;
-#ifndef TQ_NO_TC_QUANTIZE
-  if (!force_fp32) return launch_quantize_pack_tc(a, D, dt, num_sms, st);
+  // the tensor-core kernel (tq_quantize_tc.cu) is the product path
+#ifdef TQ_TEST_HOOKS
+  // tq_debug_set_quantize_impl(1) selects the CUDA-core kernel of this file (it only knows the default residual mode)
+  if (g_debug_quantize_fp32.load(std::memory_order_relaxed) != 0 && !a.literal && !a.cv.vsk) {
+    if (D == 64) return dt == TQ_F16 ? launch_quant_t<64, __half>(a, num_sms, st) : launch_quant_t<64, float>(a, num_sms, st);
+    return dt == TQ_F16 ? launch_quant_t<128, __half>(a, num_sms, st) : launch_quant_t<128, float>(a, num_sms, st);
+  }
 #endif
-  if (D == 64) return dt == TQ_F16 ? launch_quant_t<64, __half>(a, num_sms, st) : launch_quant_t<64, float>(a, num_sms, st);
-  return dt == TQ_F16 ? launch_quant_t<128, __half>(a, num_sms, st) : launch_quant_t<128, float>(a, num_sms, st);
+  return launch_quantize_pack_tc(a, D, dt, num_sms, st);
 }
 
 }  // namespace tq

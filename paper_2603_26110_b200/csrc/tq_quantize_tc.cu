@@ -43,11 +43,8 @@ struct TcCfg {
   static constexpr int kThreads = kThreadsOf<D>;
   static constexpr int kSBO = 16 * D;              // bytes between 8-row groups of an operand: 1024 | 2048
   // the A operand of the FIRST product goes through tensor memory as well (stage_rows_tmem): no operand rows in shared
-  // memory at all (TQ_QUANT_SMEM_A = 1 keeps the shared-memory path of stage_rows for comparison)
-#ifndef TQ_QUANT_SMEM_A
-#define TQ_QUANT_SMEM_A 0
-#endif
-  static constexpr bool kTmemA = !TQ_QUANT_SMEM_A;
+  // memory at all (kTmemA = false keeps the shared-memory path of stage_rows for comparison)
+  static constexpr bool kTmemA = true;
   static constexpr int kOpBytes = kTmemA ? 0 : kBlk * D * 2;    // one fp16 A operand in shared memory: 0 | 32 KB
   static constexpr int kMatBytes = D * D * 2;      // one fp16 B operand: 8 | 32 KB
   // tensor memory columns: [0, d) the accumulator (D_K / D_V, then — once every thread holds those in registers — D_S of the
@@ -982,11 +979,9 @@ __device__ __forceinline__ void quantize_pack_tc_body(const QuantArgs& a, int bl
 
 // grid = (block groups, batch x heads, keys | values): the key CTAs (the long ones) are dispatched first and the value
 // CTAs fill in behind them (measured: alternating key and value CTAs along x is 8 % slower at configs[2])
-#ifndef TQ_QUANT_CTAS64
-#define TQ_QUANT_CTAS64 4  // 64 registers: four CTAs per SM also fill tensor memory (4 x 128 columns); measured 147 us vs 158 us with three
-#endif
+constexpr int kQuantCtasPerSm64 = 4;  // 64 registers: four CTAs per SM also fill tensor memory (4 x 128 columns); measured 147 us vs 158 us with three
 template <int D, typename T, bool kLit, bool kVq>
-__global__ void __launch_bounds__(kThreadsOf<D>, D == 64 ? TQ_QUANT_CTAS64 : 1) quantize_pack_tc_kernel(QuantArgs a, int blocks_per_cta) {
+__global__ void __launch_bounds__(kThreadsOf<D>, D == 64 ? kQuantCtasPerSm64 : 1) quantize_pack_tc_kernel(QuantArgs a, int blocks_per_cta) {
   extern __shared__ __align__(1024) unsigned char smem_dyn[];
   if (blockIdx.z == 0) quantize_pack_tc_body<D, T, true, kLit, kVq>(a, blocks_per_cta, (int)blockIdx.x, smem_dyn);
   else quantize_pack_tc_body<D, T, false, kLit, kVq>(a, blocks_per_cta, (int)blockIdx.x, smem_dyn);

@@ -34,6 +34,27 @@ def test_exports_every_declared_symbol(tq):
     assert sorted(declared) == sorted(tq.EXPORTS)
 
 
+def test_product_build_exports_no_test_hooks(tq):
+    """include/tq.h: the measurement / test hooks exist only with -DTQ_TEST_HOOKS (the build the tests and bench.py use).
+    `build --product` must export every other declared symbol and none of the three hooks, and must not contain the fp32
+    cross-check kernel."""
+    import subprocess
+
+    from paper_2603_26110_b200 import build
+
+    lib = build.build(test_hooks=False)
+    out = subprocess.run(["nm", "-D", "--defined-only", lib], capture_output=True, text=True).stdout
+    names = {l.split()[-1] for l in out.splitlines() if " T " in l}
+    hooks = {"tq_profile_decode_main_only", "tq_debug_set_decode_nsplit", "tq_debug_set_quantize_impl"}
+    hdr = open(os.path.join(ROOT, "include", "tq.h")).read()
+    block = hdr[hdr.index("#ifdef TQ_TEST_HOOKS"):hdr.index("#endif /* TQ_TEST_HOOKS */")]
+    assert hooks == set(re.findall(r"\b(tq_[a-z0-9_]+)\s*\(", re.sub(r"/\*.*?\*/", "", block, flags=re.S)))
+    assert not (hooks & names)
+    assert set(tq.EXPORTS) - hooks <= names
+    allsyms = subprocess.run(["nm", "-C", lib], capture_output=True, text=True).stdout
+    assert "quantize_pack_tc_kernel" in allsyms and "quantize_pack_kernel<" not in allsyms
+
+
 def test_no_torch_or_python_symbols_in_abi(tq):
     import subprocess
 
